@@ -1,0 +1,197 @@
+"""ctypes wrapper of oracle/sup_oracle.c -- the fp64 CPU ORACLE (TEST INFRASTRUCTURE, not the product).
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import this.
+It never imports the CUDA package.  Inputs are the fp32-rounded arrays of a gen.Problem, widened exactly
+to fp64.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "sup_oracle.c")
+_LIB = os.path.join(_HERE, "_sup_oracle.so")
+_lib = None
+
+OBJ_KIND = {None: 0, "none": 0, "tv2d": 1, "tv1d": 2, "dose": 3}
+PER_TRIAL, PER_SWEEP = 0, 1
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2 (no -ffast-math, no OpenMP: the oracle is single-threaded scalar code)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(["gcc", "-O2", "-shared", "-fPIC", "-o", _LIB, _SRC, "-lm"])
+    return _LIB
+
+
+def _L():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = ctypes.CDLL(_LIB)
+        _lib.orc_proximity.restype = ctypes.c_double
+        _lib.orc_tv2d.restype = ctypes.c_double
+        _lib.orc_tv1d.restype = ctypes.c_double
+        _lib.orc_dose.restype = ctypes.c_double
+        _lib.orc_perturb_phase.restype = ctypes.c_int64
+        _lib.orc_setup.restype = ctypes.c_int
+        _lib.orc_superiorize.restype = ctypes.c_int
+    return _lib
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+
+
+_i64, _dbl, _int = ctypes.c_int64, ctypes.c_double, ctypes.c_int
+
+
+class Oracle:
+    """fp64 oracle bound to one problem (CSR + bounds + box [+ weights, blocks, dose matrix])."""
+
+    def __init__(self, m, n, rowptr, col, val, lb, ub, lo, hi, weights=None, block_rowptr=None, dose=None,
+                 objective=None, shape=None):
+        f8 = lambda a: None if a is None else np.ascontiguousarray(a, np.float64)
+        self.m, self.n = int(m), int(n)
+        self.rowptr = np.ascontiguousarray(rowptr, np.int64)
+        self.col = np.ascontiguousarray(col, np.int32)
+        self.val = f8(val)
+        self.lb, self.ub, self.lo, self.hi = f8(lb), f8(ub), f8(lo), f8(hi)
+        self.w = np.empty(self.m)
+        self.rho = np.empty(self.m)
+        self.d = np.empty(self.m)
+        rc = _L().orc_setup(_i64(self.m), _p(self.rowptr), _p(self.col), _p(self.val), _p(f8(weights)), _p(self.w),
+                            _p(self.rho), _p(self.d))
+        if rc:
+            raise ValueError("weights must be > 0")
+        self.block_rowptr = None if block_rowptr is None else np.ascontiguousarray(block_rowptr, np.int64)
+        self.objective = objective
+        self.shape = shape
+        if dose is not None:
+            self.d_rowptr = np.ascontiguousarray(dose[0], np.int64)
+            self.d_col = np.ascontiguousarray(dose[1], np.int32)
+            self.d_val = f8(dose[2])
+            self.md = int(dose[3])
+        else:
+            self.d_rowptr = self.d_col = self.d_val = None
+            self.md = 0
+
+    @classmethod
+    def from_problem(cls, P, blocks=True):
+        return cls(P.m, P.n, P.rowptr, P.col, P.val, P.lb, P.ub, P.lo, P.hi, P.weights,
+                   P.block_rowptr if blocks else None, P.dose, P.objective, P.shape)
+
+    # ---- feasibility-seeking --------------------------------------------------------------
+    def sweep(self, x, lam=1.0, n_sweeps=1):
+        x = np.array(x, np.float64)
+        u = np.empty(self.n)
+        for _ in range(n_sweeps):
+            _L().orc_sweep(_i64(self.m), _i64(self.n), _p(self.rowptr), _p(self.col), _p(self.val), _p(self.lb),
+                           _p(self.ub), _p(self.d), _p(self.lo), _p(self.hi), _dbl(lam), _p(x), _p(u))
+        return x
+
+    def block_sweep(self, x, lam=1.0, n_sweeps=1, block_rowptr=None):
+        br = self.block_rowptr if block_rowptr is None else np.ascontiguousarray(block_rowptr, np.int64)
+        x = np.array(x, np.float64)
+        u = np.empty(self.n)
+        for _ in range(n_sweeps):
+            _L().orc_block_sweep(_i64(self.m), _i64(self.n), _p(self.rowptr), _p(self.col), _p(self.val), _p(self.lb),
+                                 _p(self.ub), _p(self.w), _p(self.d), _p(self.lo), _p(self.hi), _dbl(lam),
+                                 _int(br.size - 1), _p(br), _p(x), _p(u))
+        return x
+
+    def proximity(self, x, mode=0, p=2.0):
+        x = np.ascontiguousarray(x, np.float64)
+        return _L().orc_proximity(_i64(self.m), _p(self.rowptr), _p(self.col), _p(self.val), _p(self.lb), _p(self.ub),
+                                  _p(self.w), _p(self.rho), _p(x), _int(mode), _dbl(p))
+
+    # ---- objectives -----------------------------------------------------------------------
+    def _obj_args(self, kind=None, shape=None):
+        kind = self.objective if kind is None else kind
+        shape = self.shape if shape is None else shape
+        k = OBJ_KIND[kind]
+        ny, nx = (shape if k == 1 else (0, 0))
+        return (_int(k), _i64(ny), _i64(nx), _i64(self.md), _p(self.d_rowptr), _p(self.d_col), _p(self.d_val))
+
+    def objective_value(self, x, kind=None, shape=None):
+        kind = self.objective if kind is None else kind
+        shape = self.shape if shape is None else shape
+        x = np.ascontiguousarray(x, np.float64)
+        L = _L()
+        if kind == "tv2d":
+            return L.orc_tv2d(_p(x), _i64(shape[0]), _i64(shape[1]))
+        if kind == "tv1d":
+            return L.orc_tv1d(_p(x), _i64(x.size))
+        if kind == "dose":
+            return L.orc_dose(_i64(self.md), _p(self.d_rowptr), _p(self.d_col), _p(self.d_val), _p(x))
+        return 0.0
+
+    def objective_grad(self, x, kind=None, shape=None):
+        kind = self.objective if kind is None else kind
+        shape = self.shape if shape is None else shape
+        x = np.ascontiguousarray(x, np.float64)
+        g = np.zeros_like(x)
+        L = _L()
+        if kind == "tv2d":
+            L.orc_tv2d_grad(_p(x), _i64(shape[0]), _i64(shape[1]), _p(g))
+        elif kind == "tv1d":
+            L.orc_tv1d_grad(_p(x), _i64(x.size), _p(g))
+        elif kind == "dose":
+            L.orc_dose_grad(_i64(self.md), _i64(self.n), _p(self.d_rowptr), _p(self.d_col), _p(self.d_val), _p(x), _p(g))
+        return g
+
+    # ---- perturbation phase / superiorization ---------------------------------------------
+    def perturb(self, x, ell, N, beta0, a, k=0, policy=PER_TRIAL, kind=None, shape=None, forced=None, cap=1 << 20):
+        """One perturbation phase (Alg. 1 lines 4-17).  Returns dict(x, ell, trials, decisions, margins, fx, warn)."""
+        x = np.array(x, np.float64)
+        ell_c = _i64(int(ell))
+        dec = np.zeros(cap, np.int8)
+        mar = np.zeros(cap)
+        ndec = _i64(0)
+        warn = _int(0)
+        fx = _dbl(0.0)
+        forced_a = None if forced is None else np.ascontiguousarray(forced, np.int8)
+        t = _L().orc_perturb_phase(_i64(self.n), *self._obj_args(kind, shape), _p(x), ctypes.byref(ell_c), _i64(k),
+                                   _int(N), _dbl(beta0), _dbl(a), _int(policy), _p(dec), _p(mar), _i64(cap),
+                                   ctypes.byref(ndec), _p(forced_a), ctypes.byref(warn), ctypes.byref(fx))
+        nd = min(ndec.value, cap)
+        return dict(x=x, ell=ell_c.value, trials=int(t), decisions=dec[:nd].copy(), margins=mar[:nd].copy(), fx=fx.value,
+                    warn=warn.value)
+
+    def superiorize(self, x0, n_iter, N, beta0, a, lam=1.0, policy=PER_TRIAL, block=False, snapshots=(), ell0=0,
+                    forced=None, kind=None, shape=None, cap=1 << 22):
+        """Algorithm 1 for n_iter sweeps.  snapshots: sweep counts (1-based: 'after s sweeps') at which x is copied.
+        Returns dict(x, ell, trace[n_iter,4] = (prox0, f, trials, ell), snaps{count: x}, decisions, margins, warn)."""
+        x = np.array(x0, np.float64)
+        ell = _i64(int(ell0))
+        trace = np.zeros((n_iter, 4))
+        dec = np.zeros(cap, np.int8)
+        mar = np.zeros(cap)
+        ndec = _i64(0)
+        forced_a = None if forced is None else np.ascontiguousarray(forced, np.int8)
+        nb = 0 if not block else self.block_rowptr.size - 1
+        snaps = {}
+        stops = sorted(set(int(s) for s in snapshots if 0 < int(s) < n_iter)) + [n_iter]
+        k = 0
+        warn = 0
+        for stop in stops:
+            cnt = stop - k
+            if cnt <= 0:
+                continue
+            tr = np.zeros((cnt, 4))
+            warn |= _L().orc_superiorize(
+                _i64(self.m), _i64(self.n), _p(self.rowptr), _p(self.col), _p(self.val), _p(self.lb), _p(self.ub),
+                _p(self.w), _p(self.rho), _p(self.d), _p(self.lo), _p(self.hi), _dbl(lam), _int(nb),
+                _p(self.block_rowptr) if nb else None, *self._obj_args(kind, shape), _p(x), ctypes.byref(ell), _i64(k),
+                _int(cnt), _int(N), _dbl(beta0), _dbl(a), _int(policy), _p(tr), _p(dec), _p(mar), _i64(cap),
+                ctypes.byref(ndec), _p(forced_a))
+            trace[k:stop] = tr
+            k = stop
+            snaps[stop] = x.copy()
+        nd = min(ndec.value, cap)
+        return dict(x=x, ell=ell.value, trace=trace, snaps=snaps, decisions=dec[:nd].copy(), margins=mar[:nd].copy(),
+                    warn=warn)

@@ -1,0 +1,315 @@
+/*
+ * oracle/sup_oracle.c -- plain, slow, fp64 CPU ORACLE of the superiorized simultaneous-projection path.
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference legs may call it.  It shares no code with the CUDA path
+ * (paper_2606_27086_b200/csrc) and is written from the paper alone:
+ *   /root/reference/PAPER.md = arXiv 2606.27086 (SupPy), cited as PAPER.md:L<line>.
+ * Scalar loops, CSR traversed in storage order, back-projection as a scatter (no transposed matrix),
+ * plain left-to-right fp64 sums.  Readings of the paper where it is silent/garbled are listed in
+ * DESIGN.md ("Readings", A-1 .. A-22) and named at the line that uses them.
+ *
+ * Parity pins (tests/test_oracle_*.py): every function below is pinned by closed forms, invariants,
+ * library special cases or brute force; nothing here is "parity unpinned".
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+typedef struct {
+    int64_t m, n;
+    const int64_t* rowptr;
+    const int32_t* col;
+    const double* val;
+} csr_t;
+
+/* ---- O-SETUP: weights and row scaling.  PAPER.md:L63 (w_i > 0, sum w_i = 1), L608 (D = diag(w_i/||a^i||^2)).
+ * A-3: no weights => 1/m; given weights are divided by their sum.  A-4: empty rows get d_i = 0.
+ * Returns 0, or 1 if a weight is not > 0. */
+int orc_setup(int64_t m, const int64_t* rowptr, const int32_t* col, const double* val, const double* w_in,
+              double* w, double* rho, double* d) {
+    (void)col;
+    double sw = 0.0;
+    for (int64_t i = 0; i < m; ++i) {
+        double wi = w_in ? w_in[i] : 1.0;
+        if (!(wi > 0.0)) return 1;
+        sw += wi;
+    }
+    for (int64_t i = 0; i < m; ++i) {
+        w[i] = (w_in ? w_in[i] : 1.0) / sw;
+        double r = 0.0;
+        for (int64_t k = rowptr[i]; k < rowptr[i + 1]; ++k) r += val[k] * val[k]; /* ||a^i||^2 */
+        rho[i] = r;
+        d[i] = r > 0.0 ? w[i] / r : 0.0;
+    }
+    return 0;
+}
+
+/* hyperslab violation of row value r against [lb, ub]: Eq. 2 applied to each face of
+ * lb <= <a,x> <= ub (Eq. 20); at most one face is violated. */
+static double violation(double r, double lb, double ub) {
+    if (r > ub) return r - ub;
+    if (r < lb) return r - lb;
+    return 0.0;
+}
+
+/* ---- O-SWEEP on rows [r0, r1): x <- P_box(x - lambda * A^T D c(x)).
+ * A-1: T(x) = x + lambda * sum_i w_i (P_{C_i}(x) - x)  (Eq. 2, 3 and the weights of Eq. 5 / Table A.5's D).
+ * A-2: the box is applied after the relaxed step, un-relaxed.
+ * dscale multiplies d_i (1 for the simultaneous sweep; 1/W_t for block t, A-14).  u is scratch [n]. */
+static void sweep_rows(const csr_t* A, int64_t r0, int64_t r1, const double* lb, const double* ub, const double* d,
+                       double dscale, const double* lo, const double* hi, double lambda, double* x, double* u) {
+    for (int64_t j = 0; j < A->n; ++j) u[j] = 0.0;
+    for (int64_t i = r0; i < r1; ++i) {
+        double r = 0.0;
+        for (int64_t k = A->rowptr[i]; k < A->rowptr[i + 1]; ++k) r += A->val[k] * x[A->col[k]]; /* <a^i, x>, L41 */
+        double c = violation(r, lb[i], ub[i]);
+        if (c != 0.0) {
+            double y = (d[i] * dscale) * c;
+            for (int64_t k = A->rowptr[i]; k < A->rowptr[i + 1]; ++k) u[A->col[k]] += A->val[k] * y;
+        }
+    }
+    for (int64_t j = 0; j < A->n; ++j) {
+        double t = x[j] - lambda * u[j]; /* Eq. 3 (L46) */
+        if (t < lo[j]) t = lo[j];        /* BoxProjection, L427 */
+        if (t > hi[j]) t = hi[j];
+        x[j] = t;
+    }
+}
+
+void orc_sweep(int64_t m, int64_t n, const int64_t* rowptr, const int32_t* col, const double* val, const double* lb,
+               const double* ub, const double* d, const double* lo, const double* hi, double lambda, double* x,
+               double* u) {
+    csr_t A = {m, n, rowptr, col, val};
+    sweep_rows(&A, 0, m, lb, ub, d, 1.0, lo, hi, lambda, x, u);
+}
+
+/* ---- O-BLOCK-SWEEP (block-iterative family; A-14): blocks of contiguous rows visited in
+ * index order; within block t a simultaneous step with weights w_i / W_t, W_t = sum_{i in B_t} w_i;
+ * box after every block. */
+void orc_block_sweep(int64_t m, int64_t n, const int64_t* rowptr, const int32_t* col, const double* val,
+                     const double* lb, const double* ub, const double* w, const double* d, const double* lo,
+                     const double* hi, double lambda, int n_blocks, const int64_t* block_rowptr, double* x,
+                     double* u) {
+    csr_t A = {m, n, rowptr, col, val};
+    for (int t = 0; t < n_blocks; ++t) {
+        double W = 0.0;
+        for (int64_t i = block_rowptr[t]; i < block_rowptr[t + 1]; ++i) W += w[i];
+        if (!(W > 0.0)) continue;
+        sweep_rows(&A, block_rowptr[t], block_rowptr[t + 1], lb, ub, d, 1.0 / W, lo, hi, lambda, x, u);
+    }
+}
+
+/* ---- O-PROX.  delta_i = |c_i| / ||a^i|| = Euclidean distance to C_i (0 for empty rows, A-4/A-5).
+ * mode 0: 1/2 sum w_i delta_i^2 (Eq. 5); mode 1: sum w_i delta_i^p (Eq. 12);
+ * mode 2: max_i delta_i (Eq. 13). */
+double orc_proximity(int64_t m, const int64_t* rowptr, const int32_t* col, const double* val, const double* lb,
+                     const double* ub, const double* w, const double* rho, const double* x, int mode, double p) {
+    double acc = 0.0;
+    for (int64_t i = 0; i < m; ++i) {
+        double r = 0.0;
+        for (int64_t k = rowptr[i]; k < rowptr[i + 1]; ++k) r += val[k] * x[col[k]];
+        double c = violation(r, lb[i], ub[i]);
+        double delta = rho[i] > 0.0 ? fabs(c) / sqrt(rho[i]) : 0.0;
+        if (mode == 0) acc += w[i] * delta * delta;
+        else if (mode == 1) acc += w[i] * pow(delta, p);
+        else if (delta > acc) acc = delta;
+    }
+    return mode == 0 ? 0.5 * acc : acc;
+}
+
+/* ---- objectives ---------------------------------------------------------------------------------- */
+/* TV2D, Eq. 15 on an ny x nx row-major image X[i*nx+j]: terms only for i < ny-1, j < nx-1. */
+double orc_tv2d(const double* X, int64_t ny, int64_t nx) {
+    double s = 0.0;
+    for (int64_t i = 0; i + 1 < ny; ++i)
+        for (int64_t j = 0; j + 1 < nx; ++j) {
+            double dx = X[(i + 1) * nx + j] - X[i * nx + j];
+            double dy = X[i * nx + j + 1] - X[i * nx + j];
+            s += sqrt(dx * dx + dy * dy);
+        }
+    return s;
+}
+
+/* Gradient of Eq. 15 as printed, term by term (A-8); a term with t = 0 contributes 0 (A-9). */
+void orc_tv2d_grad(const double* X, int64_t ny, int64_t nx, double* g) {
+    for (int64_t q = 0; q < ny * nx; ++q) g[q] = 0.0;
+    for (int64_t i = 0; i + 1 < ny; ++i)
+        for (int64_t j = 0; j + 1 < nx; ++j) {
+            double dx = X[(i + 1) * nx + j] - X[i * nx + j];
+            double dy = X[i * nx + j + 1] - X[i * nx + j];
+            double t = sqrt(dx * dx + dy * dy);
+            if (t > 0.0) {
+                g[i * nx + j] -= (dx + dy) / t;
+                g[(i + 1) * nx + j] += dx / t;
+                g[i * nx + j + 1] += dy / t;
+            }
+        }
+}
+
+/* TV1D (A-16): f = sum_{i<n-1} |x_{i+1} - x_i|, subgradient with sgn(0) = 0. */
+double orc_tv1d(const double* x, int64_t n) {
+    double s = 0.0;
+    for (int64_t i = 0; i + 1 < n; ++i) s += fabs(x[i + 1] - x[i]);
+    return s;
+}
+void orc_tv1d_grad(const double* x, int64_t n, double* g) {
+    for (int64_t i = 0; i < n; ++i) g[i] = 0.0;
+    for (int64_t i = 0; i + 1 < n; ++i) {
+        double dlt = x[i + 1] - x[i];
+        double s = (dlt > 0.0) - (dlt < 0.0);
+        g[i] -= s;
+        g[i + 1] += s;
+    }
+}
+
+/* DOSE (A-15): f = ||D x||^2, g = 2 D^T (D x); D is md x n CSR. */
+double orc_dose(int64_t md, const int64_t* rowptr, const int32_t* col, const double* val, const double* x) {
+    double s = 0.0;
+    for (int64_t i = 0; i < md; ++i) {
+        double r = 0.0;
+        for (int64_t k = rowptr[i]; k < rowptr[i + 1]; ++k) r += val[k] * x[col[k]];
+        s += r * r;
+    }
+    return s;
+}
+void orc_dose_grad(int64_t md, int64_t n, const int64_t* rowptr, const int32_t* col, const double* val,
+                   const double* x, double* g) {
+    for (int64_t j = 0; j < n; ++j) g[j] = 0.0;
+    for (int64_t i = 0; i < md; ++i) {
+        double r = 0.0;
+        for (int64_t k = rowptr[i]; k < rowptr[i + 1]; ++k) r += val[k] * x[col[k]];
+        for (int64_t k = rowptr[i]; k < rowptr[i + 1]; ++k) g[col[k]] += 2.0 * val[k] * r;
+    }
+}
+
+/* objective descriptor: kind 0 = none (f = 0, g = 0), 1 = TV2D (ny, nx), 2 = TV1D, 3 = DOSE */
+typedef struct {
+    int kind;
+    int64_t ny, nx;
+    int64_t md;
+    const int64_t* d_rowptr;
+    const int32_t* d_col;
+    const double* d_val;
+} obj_t;
+
+static double obj_value(const obj_t* O, int64_t n, const double* x) {
+    switch (O->kind) {
+        case 1: return orc_tv2d(x, O->ny, O->nx);
+        case 2: return orc_tv1d(x, n);
+        case 3: return orc_dose(O->md, O->d_rowptr, O->d_col, O->d_val, x);
+        default: return 0.0;
+    }
+}
+static void obj_grad(const obj_t* O, int64_t n, const double* x, double* g) {
+    switch (O->kind) {
+        case 1: orc_tv2d_grad(x, O->ny, O->nx, g); break;
+        case 2: orc_tv1d_grad(x, n, g); break;
+        case 3: orc_dose_grad(O->md, n, O->d_rowptr, O->d_col, O->d_val, x, g); break;
+        default: for (int64_t j = 0; j < n; ++j) g[j] = 0.0;
+    }
+}
+
+/* ---- O-PERTURB: the perturbation phase, Algorithm 1 lines 4-17.
+ *  fx <- f(x); for n = 0..N-1: g <- grad f(x^{k,n}) (A-7: recomputed at every reduction step);
+ *  v <- -g/||g|| (A-6: minus sign per L84/L93; v = 0 if ||g|| = 0);
+ *  trial loop: beta <- beta0 * a^l (A-10, A-20: pow in fp64), z <- x + beta v, l <- l+1,
+ *  accept iff f(z) <= f(x^{k,n}) (L149, A-11).  J_max trials per step (A-12).
+ *  policy 0 = PER_TRIAL: one persistent counter *ell, incremented on every trial, never reset.
+ *  policy 1 = PER_SWEEP: beta_{k,j} = beta0 * a^{k+j}, j reset to 0 at every reduction step (literal Alg. 1).
+ *  decisions/n_dec: optional log of every trial (1 accept / 0 reject), capacity cap_dec.
+ *  forced: optional replay of a decision sequence (A-13 trace-replay); NULL = decide by the test.
+ *  margins: optional per-trial |fz-fx|/max(1,|fx|).  Returns number of trials; *warn |= 1 if J_max hit. */
+#define J_MAX 10000
+int64_t orc_perturb(int64_t n, const obj_t* O, double* x, int64_t* ell, int64_t k, int N, double beta0, double a,
+                    int policy, double* g, double* z, int8_t* decisions, double* margins, int64_t cap_dec,
+                    int64_t* n_dec, const int8_t* forced, int* warn, double* fx_out) {
+    double fx = obj_value(O, n, x);
+    int64_t trials = 0;
+    for (int nred = 0; nred < N; ++nred) {
+        obj_grad(O, n, x, g);
+        double s = 0.0;
+        for (int64_t j = 0; j < n; ++j) s += g[j] * g[j];
+        s = sqrt(s);
+        int64_t jloc = 0;
+        int accepted = 0;
+        for (int trial = 0; trial < J_MAX && !accepted; ++trial) {
+            double expo = policy == 0 ? (double)(*ell) : (double)(k + jloc);
+            double beta = beta0 * pow(a, expo);
+            for (int64_t j = 0; j < n; ++j) z[j] = s > 0.0 ? x[j] + beta * (-g[j] / s) : x[j];
+            (*ell)++;
+            jloc++;
+            trials++;
+            double fz = obj_value(O, n, z);
+            int acc = forced ? (int)forced[*n_dec] : (fz <= fx);
+            if (decisions && *n_dec < cap_dec) {
+                decisions[*n_dec] = (int8_t)acc;
+                if (margins) margins[*n_dec] = fabs(fz - fx) / fmax(1.0, fabs(fx));
+            }
+            (*n_dec)++;
+            if (acc) {
+                memcpy(x, z, sizeof(double) * (size_t)n);
+                fx = fz;
+                accepted = 1;
+            }
+        }
+        if (!accepted && warn) *warn |= 1; /* A-12: step skipped */
+    }
+    if (fx_out) *fx_out = fx;
+    return trials;
+}
+
+/* ---- O-SUPERIORIZE: Algorithm 1, Eq. 10 (L91): for each sweep k the perturbation
+ * phase comes first, then T (simultaneous, or block-iterative when n_blocks > 0).  Runs sweeps
+ * k0 .. k0+n_iter-1 so that a caller can take snapshots between calls (state = x, ell, k).
+ * trace[k-k0][0..3] = {proximity mode 0 after the sweep, f(x) after the sweep, #trials, ell}. */
+int orc_superiorize(int64_t m, int64_t n, const int64_t* rowptr, const int32_t* col, const double* val,
+                    const double* lb, const double* ub, const double* w, const double* rho, const double* d,
+                    const double* lo, const double* hi, double lambda, int n_blocks, const int64_t* block_rowptr,
+                    int obj_kind, int64_t ny, int64_t nx, int64_t md, const int64_t* d_rowptr, const int32_t* d_col,
+                    const double* d_val, double* x, int64_t* ell, int64_t k0, int n_iter, int N, double beta0,
+                    double a, int policy, double* trace, int8_t* decisions, double* margins, int64_t cap_dec,
+                    int64_t* n_dec, const int8_t* forced) {
+    obj_t O = {obj_kind, ny, nx, md, d_rowptr, d_col, d_val};
+    double* g = (double*)malloc(sizeof(double) * (size_t)n);
+    double* z = (double*)malloc(sizeof(double) * (size_t)n);
+    double* u = (double*)malloc(sizeof(double) * (size_t)n);
+    int warn = 0;
+    for (int it = 0; it < n_iter; ++it) {
+        int64_t k = k0 + it;
+        int64_t trials = 0;
+        if (N > 0 && obj_kind != 0)
+            trials = orc_perturb(n, &O, x, ell, k, N, beta0, a, policy, g, z, decisions, margins, cap_dec, n_dec,
+                                 forced, &warn, NULL);
+        if (n_blocks > 0)
+            orc_block_sweep(m, n, rowptr, col, val, lb, ub, w, d, lo, hi, lambda, n_blocks, block_rowptr, x, u);
+        else
+            orc_sweep(m, n, rowptr, col, val, lb, ub, d, lo, hi, lambda, x, u);
+        if (trace) {
+            trace[4 * it + 0] = orc_proximity(m, rowptr, col, val, lb, ub, w, rho, x, 0, 2.0);
+            trace[4 * it + 1] = obj_value(&O, n, x);
+            trace[4 * it + 2] = (double)trials;
+            trace[4 * it + 3] = (double)(*ell);
+        }
+    }
+    free(g);
+    free(z);
+    free(u);
+    return warn;
+}
+
+/* stand-alone perturbation phase (what sup_perturb_tv / sup_perturb_dose are checked against) */
+int64_t orc_perturb_phase(int64_t n, int obj_kind, int64_t ny, int64_t nx, int64_t md, const int64_t* d_rowptr,
+                          const int32_t* d_col, const double* d_val, double* x, int64_t* ell, int64_t k, int N,
+                          double beta0, double a, int policy, int8_t* decisions, double* margins, int64_t cap_dec,
+                          int64_t* n_dec, const int8_t* forced, int* warn, double* fx_out) {
+    obj_t O = {obj_kind, ny, nx, md, d_rowptr, d_col, d_val};
+    double* g = (double*)malloc(sizeof(double) * (size_t)n);
+    double* z = (double*)malloc(sizeof(double) * (size_t)n);
+    int64_t t = orc_perturb(n, &O, x, ell, k, N, beta0, a, policy, g, z, decisions, margins, cap_dec, n_dec, forced,
+                            warn, fx_out);
+    free(g);
+    free(z);
+    return t;
+}
