@@ -1,0 +1,319 @@
+#!/usr/bin/env python
+"""bench.py -- superiorized projection sweeps/s on BASELINE.json's headline workload (512x512 low-dose CT, configs[2]).
+
+    python bench.py --gpus N --steps K --warmup W [--impl ours|reference] [--workload cfg3|cfg1|cfg2|cfg5:<log2m>:<k>]
+
+One "step" = one whole pass of the hot path over the workload: sup_superiorize for the config's sweep count
+(cfg3: 100 sweeps, each = perturbation phase of N=5 TV reduction steps + one simultaneous sweep), restarted
+from x0.  Prints ONE JSON line (contract in DESIGN.md "Measurement").  N > 1 runs N independent replicas
+(the path is single-GPU: "replicas only"), value = all ranks' sweeps / max-over-ranks time.
+
+--impl reference times the fp64 CPU oracle (oracle/) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "superiorized projection sweeps/s"
+UNIT = "sweeps/s"
+
+
+def load_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def make_problem(name):
+    import gen
+
+    if name == "cfg3":
+        return gen.config3_lowdose_ct()
+    if name == "cfg1":
+        return gen.config1_tiny_ct()
+    if name == "cfg2":
+        return gen.config2_crosswell()
+    if name == "cfg4":
+        return gen.config4_imrt()
+    if name.startswith("cfg5"):
+        _, lg, k = name.split(":")
+        return gen.config5_sweep_point(int(lg), int(k))
+    raise SystemExit(f"unknown workload {name}")
+
+
+WORKLOAD_TEXT = {
+    "cfg3": "BASELINE.json configs[2]: low-dose parallel-beam CT 512x512, 720 angles x 729 bins, fp32 CSR + explicit A^T, "
+            "TV superiorization N=5 a=0.99, 100 simultaneous sweeps per step",
+}
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index = index
+        self.samples = []
+        self.stop_flag = False
+
+    def run(self):
+        while not self.stop_flag:
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits"],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.samples.append([t.strip() for t in out.split(",")])
+            except Exception:
+                pass
+            time.sleep(0.1)
+
+    def summary(self):
+        sm, mx, reasons = [], 0, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for s in self.samples:
+            try:
+                sm.append(float(s[0]))
+                mx = max(mx, float(s[1]))
+                for nm, v in zip(names, s[2:6]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+            except Exception:
+                continue
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx or None, "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def time_oracle(P, budget_s=20.0):
+    """cpu_baseline: the oracle as it stands, single thread, on a bounded sample (a few superiorized sweeps)."""
+    from oracle.oracle import Oracle
+
+    O = Oracle.from_problem(P)
+    t0 = time.perf_counter()
+    done = 0
+    x, ell = P.x0, 0
+    while True:
+        R = O.superiorize(x, 1, P.N, P.beta0, P.a, lam=P.lam, ell0=ell)
+        x, ell = R["x"], R["ell"]
+        done += 1
+        el = time.perf_counter() - t0
+        if el >= budget_s or done >= P.n_sweeps or el + el / done > 1.5 * budget_s:
+            break
+    return done / el, done, el
+
+
+def run_reference(args, rank, world):
+    if rank != 0:
+        return
+    P = make_problem(args.workload)
+    from oracle.oracle import Oracle
+
+    O = Oracle.from_problem(P)
+    sweeps_per_step = 1  # bounded sample: one superiorized sweep of the workload per step
+    x, ell = P.x0, 0
+    for _ in range(args.warmup):
+        R = O.superiorize(x, sweeps_per_step, P.N, P.beta0, P.a, lam=P.lam, ell0=ell)
+        x, ell = R["x"], R["ell"]
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        R = O.superiorize(x, sweeps_per_step, P.N, P.beta0, P.a, lam=P.lam, ell0=ell)
+        x, ell = R["x"], R["ell"]
+    el = time.perf_counter() - t0
+    v = args.steps * sweeps_per_step / el
+    sample = f"{sweeps_per_step} superiorized sweep(s) of the workload per step, continuing one run (sweeps 0..{args.steps + args.warmup - 1})"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * el / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": {"workload": WORKLOAD_TEXT.get(args.workload, args.workload), "m": P.m, "n": P.n, "nnz": P.nnz},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args, rank, world, local_rank):
+    import numpy as np
+    import torch
+
+    import paper_2606_27086_b200 as sup
+    from paper_2606_27086_b200.binding import create_from_problem
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (libsup has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dev = f"cuda:{local_rank}"
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+
+    P = make_problem(args.workload)
+    t0 = time.perf_counter()
+    H = create_from_problem(P, dtype=sup.F32, device=dev)
+    torch.cuda.synchronize()
+    setup_s = time.perf_counter() - t0
+    S = P.n_sweeps
+    x0 = torch.tensor(P.x0, dtype=torch.float32, device=dev)
+    x = x0.clone()
+    kw = dict(objective=P.objective, shape=P.shape, lam=P.lam)
+
+    def step():
+        x.copy_(x0)
+        sup.sup_superiorize(H, x, S, P.N, P.beta0, P.a, **kw)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    launches0 = H.launches
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = H.launches - launches0
+    st = sup.sup_get_state(H)
+    sampler.stop_flag = True
+    if dist is not None:
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * args.steps * S / (ms * 1e-3)
+
+    # ---- e2e: the C-ABI call with HOST buffers (pinned), H2D + D2H inside the timed region -------------------
+    xh0 = torch.tensor(P.x0, dtype=torch.float32).pin_memory()
+    xh = xh0.clone().pin_memory()
+    for _ in range(2):
+        xh.copy_(xh0)
+        sup.sup_superiorize_host(H, xh, S, P.N, P.beta0, P.a, **kw)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        xh.copy_(xh0)
+        sup.sup_superiorize_host(H, xh, S, P.N, P.beta0, P.a, **kw)  # synchronises
+    e2e_s = time.perf_counter() - t0
+    if dist is not None:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e = world * args.steps * S / e2e_s
+    checksum = float(xh.double().sum())
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the two product kernels, each timed alone with CUDA events on the library's stream ------
+    peak, peak_src = load_peak()
+    reps = 20
+    xs = x0.clone()
+    sup.sup_project_simultaneous(H, xs, 1.0, 3)  # a realistic iterate / y
+    torch.cuda.synchronize()
+    kern = {}
+    bytes_fwd = 8 * P.nnz + 24 * P.m + 4 * P.n   # val+col, rowptr 8 + lb 4 + ub 4 + d 4 + y written 4, x read 4
+    bytes_bwd = 8 * P.nnz + 24 * P.n + 4 * P.m   # val+idx, colptr 8 + x read 4 + lo 4 + hi 4 + x written 4, y read 4
+    for name, fn, nbytes in (("k_fwd (S1+S2)", lambda: sup.sup_forward_violation(H, xs, sync_streams=False), bytes_fwd),
+                             ("k_bwd (S3)", lambda: sup.sup_backproject_update(H, xs, 1.0, sync_streams=False), bytes_bwd)):
+        for _ in range(3):
+            fn()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        H.stream.synchronize()
+        a.record(H.stream)
+        for _ in range(reps):
+            fn()
+        b.record(H.stream)
+        H.stream.synchronize()
+        t_ms = a.elapsed_time(b) / reps
+        kern[name] = {"ms": t_ms, "algorithmic_bytes": nbytes, "gbs": nbytes / (t_ms * 1e-3) / 1e9}
+    # unperturbed sweep (both kernels) for the share check
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    H.stream.synchronize()
+    a.record(H.stream)
+    H._check(sup.lib().sup_project_simultaneous(H.h, xs.data_ptr(), 1.0, reps))
+    b.record(H.stream)
+    H.stream.synchronize()
+    sweep_ms = a.elapsed_time(b) / reps
+    dom = max(kern, key=lambda k: kern[k]["ms"])
+    roof = {"bound": "hbm", "kernel": dom, "achieved": kern[dom]["gbs"], "peak": peak, "unit": "GB/s", "frac": kern[dom]["gbs"] / peak,
+            "traffic": None, "peak_source": peak_src, "frac_of_nominal_8000": kern[dom]["gbs"] / 8000.0,
+            "kernels": kern, "basic_sweep_ms": sweep_ms,
+            "basic_sweep_gbs": (bytes_fwd + bytes_bwd) / (sweep_ms * 1e-3) / 1e9,
+            "superiorized_sweep_ms": ms / (args.steps * S)}
+    tr = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tr):
+        try:
+            roof["traffic"] = json.load(open(tr)).get(args.workload, {}).get(dom)
+        except Exception:
+            pass
+
+    cpu_v, cpu_done, cpu_el = time_oracle(P, args.cpu_budget)
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic",
+        "config": {"workload": WORKLOAD_TEXT.get(args.workload, args.workload), "name": P.name, "m": P.m, "n": P.n, "nnz": P.nnz,
+                   "sweeps_per_step": S, "N": P.N, "beta0": P.beta0, "a": P.a, "lambda": P.lam, "objective": P.objective,
+                   "l2_note": "A and A^T (3.85 GB) are far larger than the 126 MB L2, so every sweep streams them from HBM; no flush needed",
+                   "parallelism": "replicas only" if world > 1 else "single GPU", "setup_s": setup_s,
+                   "final_ell": st["ell"], "trials_per_step": st["n_trials"], "checksum_x": checksum},
+        "roofline": roof,
+        "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": 1, "kind": "oracle",
+                         "sample": f"first {cpu_done} superiorized sweeps of the same workload ({cpu_el:.1f} s, single thread, host has {os.cpu_count()} cores)"},
+        "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": int(P.n * 4), "d2h_bytes_per_step": int(P.n * 4)},
+        "gpu_launches": int(launches),
+        "clocks": sampler.summary(),
+    }
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg3")
+    ap.add_argument("--cpu-budget", type=float, default=15.0)
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,190 @@
+/*
+ * sup.h -- C ABI of libsup: the superiorized simultaneous-projection iteration over hyperslabs + box,
+ * hand-written CUDA for NVIDIA B200 (sm_100a).
+ *
+ * Method: arXiv 2606.27086 ("GPU-accelerated superiorization ... with SupPy"), cited as PAPER.md:L<line>.
+ * Readings of the paper where it is silent or garbled are numbered A-1 .. A-22 in DESIGN.md.
+ *
+ *   constraint sets   C_i = { x : lb_i <= <a_i, x> <= ub_i },  i = 0..m-1        (Eq. 1-2, L384 Eq. 20)
+ *   box               lo_j <= x_j <= hi_j                                          (PAPER.md:L427 BoxProjection)
+ *   weights           w_i > 0, sum_i w_i = 1;  d_i = w_i / ||a_i||^2
+ *   sweep             x <- P_box( x - lambda * A^T D c(x) ),   c_i = hyperslab violation of <a_i,x>   (A-1, A-2)
+ *   perturbation      x <- x + beta * v,  v = -grad f / ||grad f||,  beta = beta0 * a^l,
+ *                     accepted iff f(z) <= f(x)                                   (Alg. 1)
+ *
+ * CONVENTIONS
+ *  - Every array argument is a DEVICE pointer owned by the caller unless its comment says "host".
+ *    The library BORROWS A, lb, ub, box_lo, box_hi (and D_body) for the handle's lifetime and never frees them.
+ *  - The library never allocates device memory.  Everything it derives (transposed CSR, row scaling, scratch
+ *    vectors, reduction partials, device-side state) lives in caller-provided WORKSPACE memory whose size comes
+ *    from sup_workspace_bytes().  "persistent" workspace must stay alive until sup_destroy(); "scratch"
+ *    workspace is only used during the call that takes it and may be freed once that call's stream work is done
+ *    (the calls that take scratch synchronise the stream before returning).
+ *  - Working precision: SUP_F32 = fp32 storage and fp32 row dot products, fp64 for every global reduction,
+ *    objective value, norm and step size; SUP_F64 = everything fp64.  `val`, lb, ub, box, weights, x are arrays
+ *    of the handle's dtype.  Column indices are int32, row pointers int64.  CSR must be canonical: columns
+ *    strictly increasing within a row, 0 <= col < n.  +-INFINITY encodes a one-sided bound.
+ *  - All work is enqueued on the cudaStream_t given at sup_create (passed as void*; NULL = default stream).
+ *    Calls that return a host scalar synchronise that stream; sup_project_simultaneous / sup_block_iterative /
+ *    sup_superiorize are asynchronous with respect to the host.
+ *  - Errors: every call returns a sup_status; nothing throws or aborts.  Argument errors are detected before
+ *    any launch.  sup_last_error() gives a text for the last failure on that handle (or of sup_create when
+ *    called with NULL).  There is NO CPU fallback: without a CUDA device every call fails with SUP_ERR_CUDA.
+ */
+#ifndef SUP_H
+#define SUP_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sup_ctx* sup_handle;
+
+typedef enum {
+    SUP_OK = 0,
+    SUP_ERR_INVALID_ARG = 1, /* null pointer, bad size, lambda outside [0,2], a outside (0,1) (L99), ... */
+    SUP_ERR_FORMAT = 2,      /* CSR not canonical, lb > ub, lo > hi, weight <= 0 */
+    SUP_ERR_WORKSPACE = 3,   /* workspace too small or misaligned (256 B) */
+    SUP_ERR_CUDA = 4,        /* a CUDA runtime call or kernel failed */
+    SUP_ERR_STATE = 5,       /* call needs something not set (blocks, dose matrix) */
+    SUP_ERR_NONFINITE = 6    /* NaN/Inf met in a reduction */
+} sup_status;
+
+typedef enum { SUP_F32 = 0, SUP_F64 = 1 } sup_dtype;
+
+/* objective kinds of the perturbation phase */
+typedef enum {
+    SUP_OBJ_NONE = 0, /* no perturbation: the basic algorithm (Eq. 10 with beta v = 0) */
+    SUP_OBJ_TV2D = 1, /* isotropic total variation, Eq. 15, on x viewed as ny x nx row-major */
+    SUP_OBJ_TV1D = 2, /* sum |x_{i+1} - x_i|  (A-16) */
+    SUP_OBJ_DOSE = 3  /* || D_body x ||^2     (A-15; north_star) */
+} sup_objective_kind;
+
+/* step-size exponent policy (A-10) */
+typedef enum {
+    SUP_STEP_PER_TRIAL = 0, /* one persistent counter l, beta = beta0*a^l used then l += 1 on EVERY trial */
+    SUP_STEP_PER_SWEEP = 1  /* literal Alg. 1: beta_{k,j} = beta0 * a^(k+j), j reset at every reduction step */
+} sup_step_policy;
+
+/* what a workspace query is for */
+typedef enum { SUP_WS_CREATE = 0, SUP_WS_BLOCKS = 1, SUP_WS_DOSE = 2 } sup_ws_kind;
+
+/* m x n CSR matrix in device memory */
+typedef struct {
+    int64_t m, n, nnz;
+    const int64_t* rowptr; /* [m+1], rowptr[0] = 0, rowptr[m] = nnz */
+    const int32_t* col;    /* [nnz] */
+    const void* val;       /* [nnz] of the handle's dtype */
+} sup_csr;
+
+/* options of sup_superiorize; zero-initialise, then set what is needed */
+typedef struct {
+    int objective;         /* sup_objective_kind */
+    int64_t shape[3];      /* TV2D: {ny, nx, 0} with ny*nx == n; others ignored */
+    double lambda;         /* relaxation in [0,2] (Eq. 3) */
+    int block_iterative;   /* 0: simultaneous sweep; 1: block-iterative sweep (needs sup_set_blocks) */
+    int step_policy;       /* sup_step_policy */
+    int64_t ell0;          /* step-size exponent to start from (resume state) */
+    int64_t k0;            /* index of the first sweep (resume state; only PER_SWEEP uses it) */
+    int trace_mode;        /* 1: after every sweep also evaluate proximity (Eq. 5) and f(x) into `trace` (slow: one extra pass) */
+    double* trace;         /* device, [n_iter][4] = {proximity mode 0, f(x), #trials, l} after each sweep; NULL = off */
+    int8_t* decisions;     /* device, [decisions_cap]: 1 = accepted / 0 = rejected, one per trial; NULL = off */
+    double* decision_f;    /* device, [decisions_cap][2] = {f(z), f(x^{k,n})} per trial; NULL = off */
+    int64_t decisions_cap;
+    int use_graph;         /* 1: capture one sweep into a CUDA graph and replay it (default path of bench.py) */
+} sup_options;
+
+/* final state of a run, read back by sup_get_state (host struct) */
+typedef struct {
+    int64_t ell;         /* step-size exponent after the run */
+    int64_t k;           /* number of sweeps done since k0 (absolute index of the next sweep) */
+    int64_t n_trials;    /* trials since the last sup_superiorize / sup_perturb_* call started */
+    int64_t n_decisions; /* entries written to `decisions` (may exceed the capacity: then only the first cap are stored) */
+    int32_t warn;        /* bit 0: a reduction step hit J_max = 10000 trials and was skipped (A-12) */
+    int32_t fault;       /* bit 0: device-side barrier timed out; bit 1: non-finite objective */
+    double f;            /* objective value carried by the last perturbation phase */
+} sup_state;
+
+/* Bytes of workspace for `kind` on a matrix of the given shape (for SUP_WS_BLOCKS pass A's shape; for SUP_WS_DOSE
+ * pass D_body's shape).  n_blocks is read for SUP_WS_BLOCKS only.  Both sizes are multiples of 256. */
+sup_status sup_workspace_bytes(int kind, int64_t m, int64_t n, int64_t nnz, int dtype, int n_blocks,
+                               size_t* persistent_bytes, size_t* scratch_bytes);
+
+/* O-SETUP (A-3, A-4): normalises the weights (NULL => 1/m), computes ||a_i||^2 and
+ * d_i = w_i/||a_i||^2 (0 for empty rows), validates the inputs, builds the explicit transposed CSR of A
+ * (stable: every row of A^T is sorted by original row index).  Synchronises the stream. */
+sup_status sup_create(sup_handle* out, const sup_csr* A, const void* lb, const void* ub, /* [m] */
+                      const void* box_lo, const void* box_hi,                            /* [n] */
+                      const void* weights,                                               /* [m] or NULL */
+                      int dtype, void* workspace, size_t workspace_bytes, void* scratch, size_t scratch_bytes,
+                      void* cuda_stream);
+
+/* Block-iterative structure (PAPER.md:L54 BIP family; A-14): rows of A are block-contiguous, block t = rows
+ * [block_rowptr[t], block_rowptr[t+1]).  Builds per-block transposed CSRs and the block-renormalised row scaling
+ * (w_i / W_t) / ||a_i||^2.  block_rowptr is a HOST array [n_blocks+1].  Synchronises the stream. */
+sup_status sup_set_blocks(sup_handle h, int n_blocks, const int64_t* block_rowptr, void* workspace,
+                          size_t workspace_bytes, void* scratch, size_t scratch_bytes);
+
+/* Dose objective matrix D_body (md x n CSR, same dtype; A-15): borrowed; builds its transposed CSR. */
+sup_status sup_set_dose_matrix(sup_handle h, const sup_csr* D_body, void* workspace, size_t workspace_bytes,
+                               void* scratch, size_t scratch_bytes);
+
+/* n_sweeps simultaneous sweeps x <- P_box(x - lambda A^T D c(x)), in place (O-SWEEP; Eq. 2, 3; L427). */
+sup_status sup_project_simultaneous(sup_handle h, void* x, double lambda, int n_sweeps);
+
+/* The two halves of one simultaneous sweep as separate calls (what bench.py times one kernel at a time):
+ * sup_forward_violation: S1+S2, y_i = d_i c_i(x) into the handle's internal y;  sup_backproject_update: S3,
+ * x <- P_box(x - lambda A^T y) with that y.  Calling them in this order equals one sup_project_simultaneous sweep. */
+sup_status sup_forward_violation(sup_handle h, const void* x);
+sup_status sup_backproject_update(sup_handle h, void* x, double lambda);
+
+/* n_sweeps block-iterative sweeps (O-BLOCK-SWEEP), in place. */
+sup_status sup_block_iterative(sup_handle h, void* x, double lambda, int n_sweeps);
+
+/* One perturbation phase (Alg. 1 lines 4-17) with the TV objective, step policy PER_TRIAL:
+ * N accepted reduction steps from x, in place.  dims = 1 (shape[0] = n) or 2 (shape = {ny, nx}); shape is a HOST
+ * array.  *ell (HOST) is read as the starting exponent and overwritten with the final one.  Synchronises. */
+sup_status sup_perturb_tv(sup_handle h, void* x, int dims, const int64_t* shape, int N, double beta0, double a,
+                          int64_t* ell);
+
+/* Same with the dose objective ||D_body x||^2 (needs sup_set_dose_matrix). */
+sup_status sup_perturb_dose(sup_handle h, void* x, int N, double beta0, double a, int64_t* ell);
+
+/* Algorithm 1, Eq. 10 (L91): for k = k0 .. k0+n_iter-1: perturbation phase of N reduction steps
+ * (beta = beta0 * a^l), then one sweep.  x in place.  N = 0 or objective NONE gives the basic algorithm.
+ * Asynchronous; read the final state with sup_get_state. */
+sup_status sup_superiorize(sup_handle h, void* x, int n_iter, int N, double beta0, double a, const sup_options* opt);
+
+/* Same run with x in HOST memory (pinned for best speed): copies x to the device, runs, copies it back and
+ * synchronises.  This is the end-to-end entry bench.py times as "e2e". */
+sup_status sup_superiorize_host(sup_handle h, void* x_host, int n_iter, int N, double beta0, double a,
+                                const sup_options* opt);
+
+/* Synchronises and copies the device-side run state to *out (HOST). */
+sup_status sup_get_state(sup_handle h, sup_state* out);
+
+/* Proximity of x (O-PROX): mode 0 = 1/2 sum w_i dist_i^2 (Eq. 5), mode 1 = sum w_i dist_i^p (L211 Eq. 12),
+ * mode 2 = max_i dist_i (L215 Eq. 13); dist_i = |c_i| / ||a_i|| (0 for empty rows).  *out is HOST.  Synchronises. */
+sup_status sup_proximity(sup_handle h, const void* x, int mode, double p, double* out);
+
+/* Objective value f(x) for `kind` (sup_objective_kind); shape is a HOST array (TV2D: {ny, nx}).  *out is HOST. */
+sup_status sup_objective(sup_handle h, const void* x, int kind, const int64_t* shape, double* out);
+
+/* Copies derived arrays for inspection/tests: which = 0: d [m] (dtype); 1: A^T rowptr [n+1] int64;
+ * 2: A^T col [nnz] int32 (original row indices); 3: A^T val [nnz] (dtype).  dst is a DEVICE pointer. */
+sup_status sup_get_derived(sup_handle h, int which, void* dst, size_t dst_bytes);
+
+/* Number of kernel launches this handle has enqueued so far (graph replays count their kernel nodes). */
+int64_t sup_launch_count(sup_handle h);
+
+const char* sup_last_error(sup_handle h);
+sup_status sup_destroy(sup_handle h);
+const char* sup_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SUP_H */

@@ -1,0 +1,540 @@
+// sup_api.cu -- the C ABI of libsup (include/sup.h): argument checks, workspace layout, the sweep loops
+// (O-SWEEP, O-BLOCK-SWEEP, O-SUPERIORIZE of DESIGN.md) and CUDA-graph capture of one superiorized sweep (S8).
+#include <math.h>
+#include <stddef.h>
+#include <string.h>
+
+#include <new>
+
+#include "sup_internal.cuh"
+
+static size_t al(size_t b) { return (b + 255) & ~size_t(255); }
+
+extern "C" const char* sup_version(void) { return "libsup 0.1 (sm_100a)"; }
+
+extern "C" const char* sup_last_error(sup_handle h) { return h ? h->err : g_create_error; }
+
+extern "C" int64_t sup_launch_count(sup_handle h) { return h ? h->launches : 0; }
+
+extern "C" sup_status sup_workspace_bytes(int kind, int64_t m, int64_t n, int64_t nnz, int dtype, int n_blocks,
+                                          size_t* persistent_bytes, size_t* scratch_bytes) {
+    if (m <= 0 || n <= 0 || nnz < 0 || (dtype != SUP_F32 && dtype != SUP_F64) || !persistent_bytes || !scratch_bytes)
+        return sup_fail(nullptr, SUP_ERR_INVALID_ARG, "sup_workspace_bytes: bad argument");
+    const size_t esz = dtype == SUP_F32 ? 4 : 8;
+    size_t p = 0, s = 0;
+    switch (kind) {
+        case SUP_WS_CREATE:
+            p = al(size_t(n + 1) * 8) + al(size_t(nnz) * 4) + al(size_t(nnz) * esz)  // A^T
+                + al(size_t(m) * esz)                                                // d
+                + 2 * al(size_t(m) * 8)                                              // w, 1/||a||
+                + al(size_t(m) * esz) + 2 * al(size_t(n) * esz)                      // y, g, xdev
+                + al(2 * SUP_MAX_PARTIALS * 8) + al(sizeof(DevState)) + 1024;
+            s = sup_transpose_scratch_bytes(nnz, n, esz) + 4096;
+            break;
+        case SUP_WS_BLOCKS:
+            if (n_blocks < 1) return sup_fail(nullptr, SUP_ERR_INVALID_ARG, "sup_workspace_bytes: n_blocks < 1");
+            p = size_t(n_blocks) * al(size_t(n + 1) * 8) + al(size_t(nnz) * 4) + al(size_t(nnz) * esz) + al(size_t(m) * esz) + 1024;
+            s = sup_transpose_scratch_bytes(nnz, n, esz) + al(size_t(n_blocks) * 8) + 4096;
+            break;
+        case SUP_WS_DOSE:  // (m, n, nnz) describe D_body
+            p = al(size_t(n + 1) * 8) + al(size_t(nnz) * 4) + al(size_t(nnz) * esz) + al(size_t(m) * esz) + 1024;
+            s = sup_transpose_scratch_bytes(nnz, n, esz) + 4096;
+            break;
+        default:
+            return sup_fail(nullptr, SUP_ERR_INVALID_ARG, "sup_workspace_bytes: unknown kind");
+    }
+    *persistent_bytes = al(p);
+    *scratch_bytes = al(s);
+    return SUP_OK;
+}
+
+static bool aligned256(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 255u) == 0; }
+
+extern "C" sup_status sup_create(sup_handle* out, const sup_csr* A, const void* lb, const void* ub, const void* box_lo,
+                                 const void* box_hi, const void* weights, int dtype, void* workspace, size_t workspace_bytes,
+                                 void* scratch, size_t scratch_bytes, void* cuda_stream) {
+    if (!out) return sup_fail(nullptr, SUP_ERR_INVALID_ARG, "sup_create: out is NULL");
+    *out = nullptr;
+    if (!A || !A->rowptr || !A->col || !A->val || !lb || !ub || !box_lo || !box_hi)
+        return sup_fail(nullptr, SUP_ERR_INVALID_ARG, "sup_create: NULL array argument");
+    if (A->m <= 0 || A->n <= 0 || A->nnz < 0 || A->n > 0x7fffffffLL || A->m > 0x7fffffffLL || A->nnz > 0x7fffffffLL)
+        return sup_fail(nullptr, SUP_ERR_INVALID_ARG, "sup_create: m, n must be in [1, 2^31), nnz in [0, 2^31)");
+    if (dtype != SUP_F32 && dtype != SUP_F64) return sup_fail(nullptr, SUP_ERR_INVALID_ARG, "sup_create: bad dtype");
+    size_t need_p = 0, need_s = 0;
+    sup_workspace_bytes(SUP_WS_CREATE, A->m, A->n, A->nnz, dtype, 1, &need_p, &need_s);
+    if (!workspace || !scratch || workspace_bytes < need_p || scratch_bytes < need_s || !aligned256(workspace) || !aligned256(scratch))
+        return sup_fail(nullptr, SUP_ERR_WORKSPACE, "sup_create: workspace needs %zu + %zu scratch bytes, 256-byte aligned", need_p, need_s);
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return sup_fail(nullptr, SUP_ERR_CUDA, "sup_create: no usable CUDA device (libsup has no CPU fallback)");
+    }
+    sup_ctx* h = new (std::nothrow) sup_ctx;
+    if (!h) return sup_fail(nullptr, SUP_ERR_INVALID_ARG, "sup_create: out of host memory");
+    h->dt = dtype;
+    h->esz = dtype == SUP_F32 ? 4 : 8;
+    h->stream = static_cast<cudaStream_t>(cuda_stream);
+    h->num_sms = prop.multiProcessorCount;
+    h->m = A->m;
+    h->n = A->n;
+    h->nnz = A->nnz;
+    h->A.rows = A->m;
+    h->A.cols = A->n;
+    h->A.nnz = A->nnz;
+    h->A.rowptr = A->rowptr;
+    h->A.col = A->col;
+    h->A.val = A->val;
+    h->lb = lb;
+    h->ub = ub;
+    h->lo = box_lo;
+    h->hi = box_hi;
+    h->g_fwd = sup_pick_group(h->nnz, h->m);
+    h->g_bwd = sup_pick_group(h->nnz, h->n);
+
+    Bump B{static_cast<char*>(workspace), workspace_bytes, 0, true};
+    int64_t* at_rowptr = static_cast<int64_t*>(B.take(size_t(h->n + 1) * 8));
+    int32_t* at_col = static_cast<int32_t*>(B.take(size_t(h->nnz) * 4));
+    void* at_val = B.take(size_t(h->nnz) * h->esz);
+    h->d = B.take(size_t(h->m) * h->esz);
+    h->w = static_cast<double*>(B.take(size_t(h->m) * 8));
+    h->invnorm = static_cast<double*>(B.take(size_t(h->m) * 8));
+    h->y = B.take(size_t(h->m) * h->esz);
+    h->g = B.take(size_t(h->n) * h->esz);
+    h->xdev = B.take(size_t(h->n) * h->esz);
+    h->partials = static_cast<double*>(B.take(2 * SUP_MAX_PARTIALS * 8));
+    h->state = static_cast<DevState*>(B.take(sizeof(DevState)));
+    sup_status rc = SUP_OK;
+    if (!B.ok) rc = sup_fail(h, SUP_ERR_WORKSPACE, "sup_create: workspace too small");
+    if (rc == SUP_OK && cudaMemsetAsync(h->state, 0, sizeof(DevState), h->stream) != cudaSuccess)
+        rc = sup_fail(h, SUP_ERR_CUDA, "sup_create: cannot touch the workspace: %s", cudaGetErrorString(cudaGetLastError()));
+    if (rc == SUP_OK) rc = sup_setup_rows(h, weights, scratch, scratch_bytes);
+    if (rc == SUP_OK)
+        rc = sup_transpose_rows(h, h->A, 0, h->m, 0, h->nnz, at_rowptr, at_col, at_val, 0, scratch, scratch_bytes);
+    if (rc == SUP_OK && cudaStreamSynchronize(h->stream) != cudaSuccess)
+        rc = sup_fail(h, SUP_ERR_CUDA, "sup_create: %s", cudaGetErrorString(cudaGetLastError()));
+    if (rc != SUP_OK) {
+        memcpy(g_create_error, h->err, sizeof(g_create_error));
+        delete h;
+        return rc;
+    }
+    h->AT.rows = h->n;
+    h->AT.cols = h->m;
+    h->AT.nnz = h->nnz;
+    h->AT.rowptr = at_rowptr;
+    h->AT.col = at_col;
+    h->AT.val = at_val;
+    *out = h;
+    return SUP_OK;
+}
+
+static void drop_graph(sup_ctx* h) {
+    if (h->gexec) cudaGraphExecDestroy(h->gexec);
+    if (h->graph) cudaGraphDestroy(h->graph);
+    h->gexec = nullptr;
+    h->graph = nullptr;
+    h->graph_nodes = 0;
+}
+
+extern "C" sup_status sup_destroy(sup_handle h) {
+    if (!h) return SUP_OK;
+    cudaStreamSynchronize(h->stream);
+    drop_graph(h);
+    delete h;
+    return SUP_OK;
+}
+
+extern "C" sup_status sup_set_blocks(sup_handle h, int n_blocks, const int64_t* block_rowptr, void* workspace,
+                                     size_t workspace_bytes, void* scratch, size_t scratch_bytes) {
+    if (!h) return SUP_ERR_INVALID_ARG;
+    if (n_blocks < 1 || !block_rowptr) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_set_blocks: n_blocks < 1 or NULL block_rowptr");
+    if (block_rowptr[0] != 0 || block_rowptr[n_blocks] != h->m)
+        return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_set_blocks: block_rowptr must run from 0 to m");
+    for (int t = 0; t < n_blocks; ++t)
+        if (block_rowptr[t] > block_rowptr[t + 1]) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_set_blocks: block_rowptr not monotone");
+    size_t need_p = 0, need_s = 0;
+    sup_workspace_bytes(SUP_WS_BLOCKS, h->m, h->n, h->nnz, h->dt, n_blocks, &need_p, &need_s);
+    if (!workspace || !scratch || workspace_bytes < need_p || scratch_bytes < need_s || !aligned256(workspace) || !aligned256(scratch))
+        return sup_fail(h, SUP_ERR_WORKSPACE, "sup_set_blocks: workspace needs %zu + %zu scratch bytes, 256-byte aligned", need_p, need_s);
+    drop_graph(h);
+    h->n_blocks = 0;
+    std::vector<int64_t> ebound(n_blocks + 1);  // A's rowptr at the block boundaries
+    for (int t = 0; t <= n_blocks; ++t)
+        SUP_CUDA(h, cudaMemcpyAsync(&ebound[t], h->A.rowptr + block_rowptr[t], 8, cudaMemcpyDeviceToHost, h->stream));
+    SUP_CUDA(h, cudaStreamSynchronize(h->stream));
+    Bump B{static_cast<char*>(workspace), workspace_bytes, 0, true};
+    int32_t* col = static_cast<int32_t*>(B.take(size_t(h->nnz) * 4));
+    void* val = B.take(size_t(h->nnz) * h->esz);
+    h->d_blk = B.take(size_t(h->m) * h->esz);
+    h->ATb.assign(n_blocks, CsrD());
+    h->g_bwd_blk.assign(n_blocks, 32);
+    h->block_rowptr.assign(block_rowptr, block_rowptr + n_blocks + 1);
+    for (int t = 0; t < n_blocks; ++t) {
+        int64_t* rowptr_t = static_cast<int64_t*>(B.take(size_t(h->n + 1) * 8));
+        if (!B.ok) return sup_fail(h, SUP_ERR_WORKSPACE, "sup_set_blocks: workspace too small");
+        sup_status rc = sup_transpose_rows(h, h->A, block_rowptr[t], block_rowptr[t + 1], ebound[t], ebound[t + 1], rowptr_t,
+                                           col, val, ebound[t], scratch, scratch_bytes);
+        if (rc != SUP_OK) return rc;
+        CsrD& T = h->ATb[t];
+        T.rows = h->n;
+        T.cols = h->m;
+        T.nnz = ebound[t + 1] - ebound[t];
+        T.rowptr = rowptr_t;
+        T.col = col;
+        T.val = val;
+        h->g_bwd_blk[t] = sup_pick_group(T.nnz, h->n);
+    }
+    h->n_blocks = n_blocks;
+    sup_status rc = sup_setup_block_scaling(h, scratch, scratch_bytes);
+    if (rc != SUP_OK) { h->n_blocks = 0; return rc; }
+    SUP_CUDA(h, cudaStreamSynchronize(h->stream));
+    return SUP_OK;
+}
+
+extern "C" sup_status sup_set_dose_matrix(sup_handle h, const sup_csr* D, void* workspace, size_t workspace_bytes,
+                                          void* scratch, size_t scratch_bytes) {
+    if (!h) return SUP_ERR_INVALID_ARG;
+    if (!D || !D->rowptr || !D->col || !D->val || D->m <= 0 || D->n != h->n || D->nnz < 0 || D->nnz > 0x7fffffffLL)
+        return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_set_dose_matrix: bad matrix (needs n columns)");
+    size_t need_p = 0, need_s = 0;
+    sup_workspace_bytes(SUP_WS_DOSE, D->m, D->n, D->nnz, h->dt, 1, &need_p, &need_s);
+    if (!workspace || !scratch || workspace_bytes < need_p || scratch_bytes < need_s || !aligned256(workspace) || !aligned256(scratch))
+        return sup_fail(h, SUP_ERR_WORKSPACE, "sup_set_dose_matrix: workspace needs %zu + %zu scratch bytes, 256-byte aligned", need_p, need_s);
+    drop_graph(h);
+    h->has_dose = false;
+    CsrD Dm;
+    Dm.rows = D->m;
+    Dm.cols = D->n;
+    Dm.nnz = D->nnz;
+    Dm.rowptr = D->rowptr;
+    Dm.col = D->col;
+    Dm.val = D->val;
+    sup_status rc = sup_validate(h, Dm, false, scratch);
+    if (rc != SUP_OK) return rc;
+    Bump B{static_cast<char*>(workspace), workspace_bytes, 0, true};
+    int64_t* rp = static_cast<int64_t*>(B.take(size_t(D->n + 1) * 8));
+    int32_t* col = static_cast<int32_t*>(B.take(size_t(D->nnz) * 4));
+    void* val = B.take(size_t(D->nnz) * h->esz);
+    h->r_dose = B.take(size_t(D->m) * h->esz);
+    if (!B.ok) return sup_fail(h, SUP_ERR_WORKSPACE, "sup_set_dose_matrix: workspace too small");
+    rc = sup_transpose_rows(h, Dm, 0, D->m, 0, D->nnz, rp, col, val, 0, scratch, scratch_bytes);
+    if (rc != SUP_OK) return rc;
+    SUP_CUDA(h, cudaStreamSynchronize(h->stream));
+    h->D = Dm;
+    h->DT.rows = D->n;
+    h->DT.cols = D->m;
+    h->DT.nnz = D->nnz;
+    h->DT.rowptr = rp;
+    h->DT.col = col;
+    h->DT.val = val;
+    h->g_d = sup_pick_group(D->nnz, D->m);
+    h->g_dt = sup_pick_group(D->nnz, D->n);
+    h->has_dose = true;
+    return SUP_OK;
+}
+
+// ---- sweeps ----------------------------------------------------------------------------------------------------
+static void enqueue_simultaneous(sup_ctx* h, void* x, double lambda) {
+    sup_launch_fwd(h, x, 0, h->m, h->d);
+    sup_launch_bwd(h, h->AT, h->g_bwd, x, lambda);
+}
+static void enqueue_block_sweep(sup_ctx* h, void* x, double lambda) {
+    for (int t = 0; t < h->n_blocks; ++t) {
+        if (h->block_rowptr[t + 1] == h->block_rowptr[t]) continue;
+        sup_launch_fwd(h, x, h->block_rowptr[t], h->block_rowptr[t + 1], h->d_blk);
+        sup_launch_bwd(h, h->ATb[t], h->g_bwd_blk[t], x, lambda);
+    }
+}
+
+static sup_status check_lambda(sup_ctx* h, double lambda) {
+    if (!(lambda >= 0.0 && lambda <= 2.0)) return sup_fail(h, SUP_ERR_INVALID_ARG, "lambda must be in [0,2] (PAPER.md:L44)");
+    return SUP_OK;
+}
+
+extern "C" sup_status sup_project_simultaneous(sup_handle h, void* x, double lambda, int n_sweeps) {
+    if (!h) return SUP_ERR_INVALID_ARG;
+    if (!x || n_sweeps < 0) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_project_simultaneous: NULL x or n_sweeps < 0");
+    if (check_lambda(h, lambda) != SUP_OK) return SUP_ERR_INVALID_ARG;
+    for (int s = 0; s < n_sweeps; ++s) enqueue_simultaneous(h, x, lambda);
+    SUP_CUDA(h, cudaGetLastError());
+    return SUP_OK;
+}
+
+extern "C" sup_status sup_forward_violation(sup_handle h, const void* x) {
+    if (!h) return SUP_ERR_INVALID_ARG;
+    if (!x) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_forward_violation: NULL x");
+    sup_launch_fwd(h, x, 0, h->m, h->d);
+    SUP_CUDA(h, cudaGetLastError());
+    return SUP_OK;
+}
+
+extern "C" sup_status sup_backproject_update(sup_handle h, void* x, double lambda) {
+    if (!h) return SUP_ERR_INVALID_ARG;
+    if (!x) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_backproject_update: NULL x");
+    if (check_lambda(h, lambda) != SUP_OK) return SUP_ERR_INVALID_ARG;
+    sup_launch_bwd(h, h->AT, h->g_bwd, x, lambda);
+    SUP_CUDA(h, cudaGetLastError());
+    return SUP_OK;
+}
+
+extern "C" sup_status sup_block_iterative(sup_handle h, void* x, double lambda, int n_sweeps) {
+    if (!h) return SUP_ERR_INVALID_ARG;
+    if (!x || n_sweeps < 0) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_block_iterative: NULL x or n_sweeps < 0");
+    if (h->n_blocks < 1) return sup_fail(h, SUP_ERR_STATE, "sup_block_iterative: call sup_set_blocks first");
+    if (check_lambda(h, lambda) != SUP_OK) return SUP_ERR_INVALID_ARG;
+    for (int s = 0; s < n_sweeps; ++s) enqueue_block_sweep(h, x, lambda);
+    SUP_CUDA(h, cudaGetLastError());
+    return SUP_OK;
+}
+
+// ---- perturbation phase alone ----------------------------------------------------------------------------------
+static sup_status check_step(sup_ctx* h, int N, double beta0, double a) {
+    if (N < 0) return sup_fail(h, SUP_ERR_INVALID_ARG, "N must be >= 0");
+    if (!(beta0 >= 0.0) || isinf(beta0)) return sup_fail(h, SUP_ERR_INVALID_ARG, "beta0 must be finite and >= 0");
+    if (!(a > 0.0 && a < 1.0)) return sup_fail(h, SUP_ERR_INVALID_ARG, "a must be in (0,1) (PAPER.md:L99)");
+    return SUP_OK;
+}
+
+static sup_status check_objective(sup_ctx* h, int kind, const int64_t* shape, int64_t* ny, int64_t* nx) {
+    *ny = *nx = 0;
+    switch (kind) {
+        case SUP_OBJ_NONE:
+        case SUP_OBJ_TV1D: return SUP_OK;
+        case SUP_OBJ_TV2D:
+            if (!shape || shape[0] < 1 || shape[1] < 1 || shape[0] * shape[1] != h->n)
+                return sup_fail(h, SUP_ERR_INVALID_ARG, "TV2D needs shape = {ny, nx} with ny*nx == n");
+            *ny = shape[0];
+            *nx = shape[1];
+            return SUP_OK;
+        case SUP_OBJ_DOSE:
+            if (!h->has_dose) return sup_fail(h, SUP_ERR_STATE, "dose objective: call sup_set_dose_matrix first");
+            return SUP_OK;
+    }
+    return sup_fail(h, SUP_ERR_INVALID_ARG, "unknown objective kind %d", kind);
+}
+
+static sup_status read_state(sup_ctx* h, sup_state* out) {
+    DevState s;
+    SUP_CUDA(h, cudaMemcpyAsync(&s, h->state, sizeof(DevState), cudaMemcpyDeviceToHost, h->stream));
+    SUP_CUDA(h, cudaStreamSynchronize(h->stream));
+    out->ell = s.ell;
+    out->k = s.k;
+    out->n_trials = s.n_trials;
+    out->n_decisions = s.n_dec;
+    out->warn = s.warn;
+    out->fault = s.fault;
+    out->f = s.f;
+    return SUP_OK;
+}
+
+extern "C" sup_status sup_get_state(sup_handle h, sup_state* out) {
+    if (!h) return SUP_ERR_INVALID_ARG;
+    if (!out) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_get_state: NULL out");
+    sup_status rc = read_state(h, out);
+    if (rc != SUP_OK) return rc;
+    if (out->fault & 1) return sup_fail(h, SUP_ERR_CUDA, "device-side grid barrier timed out");
+    if (out->fault & 2) return sup_fail(h, SUP_ERR_NONFINITE, "non-finite objective value");
+    return SUP_OK;
+}
+
+static sup_status perturb_alone(sup_ctx* h, void* x, int kind, const int64_t* shape, int N, double beta0, double a, int64_t* ell) {
+    if (!x || !ell) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_perturb: NULL x or ell");
+    if (check_step(h, N, beta0, a) != SUP_OK) return SUP_ERR_INVALID_ARG;
+    int64_t ny, nx;
+    sup_status rc = check_objective(h, kind, shape, &ny, &nx);
+    if (rc != SUP_OK) return rc;
+    sup_launch_begin_run(h, *ell, 0);
+    if (N > 0) {
+        PerturbParams pp = {kind, ny, nx, N, beta0, a, SUP_STEP_PER_TRIAL, nullptr, nullptr, 0};
+        rc = sup_launch_perturb(h, x, pp);
+        if (rc != SUP_OK) return rc;
+    }
+    sup_state s;
+    rc = sup_get_state(h, &s);
+    if (rc != SUP_OK) return rc;
+    *ell = s.ell;
+    return SUP_OK;
+}
+
+extern "C" sup_status sup_perturb_tv(sup_handle h, void* x, int dims, const int64_t* shape, int N, double beta0, double a,
+                                     int64_t* ell) {
+    if (!h) return SUP_ERR_INVALID_ARG;
+    if (dims != 1 && dims != 2) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_perturb_tv: dims must be 1 or 2");
+    if (dims == 1 && shape && shape[0] != h->n) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_perturb_tv: shape[0] != n");
+    return perturb_alone(h, x, dims == 2 ? SUP_OBJ_TV2D : SUP_OBJ_TV1D, shape, N, beta0, a, ell);
+}
+
+extern "C" sup_status sup_perturb_dose(sup_handle h, void* x, int N, double beta0, double a, int64_t* ell) {
+    if (!h) return SUP_ERR_INVALID_ARG;
+    return perturb_alone(h, x, SUP_OBJ_DOSE, nullptr, N, beta0, a, ell);
+}
+
+// ---- Algorithm 1 -----------------------------------------------------------------------------------------------
+struct RunPlan {
+    void* x;
+    int N;
+    double beta0, a;
+    sup_options o;
+    int64_t ny, nx;
+};
+
+static sup_status enqueue_superiorized_sweep(sup_ctx* h, const RunPlan& P) {
+    if (P.N > 0 && P.o.objective != SUP_OBJ_NONE) {
+        PerturbParams pp = {P.o.objective, P.ny, P.nx, P.N, P.beta0, P.a, P.o.step_policy, P.o.decisions, P.o.decision_f,
+                            P.o.decisions_cap};
+        sup_status rc = sup_launch_perturb(h, P.x, pp);
+        if (rc != SUP_OK) return rc;
+    }
+    if (P.o.block_iterative) enqueue_block_sweep(h, P.x, P.o.lambda);
+    else enqueue_simultaneous(h, P.x, P.o.lambda);
+    if (P.o.trace_mode && P.o.trace) {
+        double* slot = reinterpret_cast<double*>(reinterpret_cast<char*>(h->state) + offsetof(DevState, scalar_out));
+        sup_launch_proximity(h, P.x, 0, 2.0, slot);
+        sup_launch_trace_slot(h, P.o.trace, 0);
+        sup_launch_objective(h, P.x, P.o.objective, P.ny, P.nx, slot);
+        sup_launch_trace_slot(h, P.o.trace, 1);
+    }
+    sup_launch_end_sweep(h, P.o.trace);
+    return SUP_OK;
+}
+
+static sup_status run_superiorize(sup_ctx* h, void* x, int n_iter, int N, double beta0, double a, const sup_options* opt) {
+    if (!x || !opt || n_iter < 0) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_superiorize: NULL x/opt or n_iter < 0");
+    if (check_step(h, N, beta0, a) != SUP_OK || check_lambda(h, opt->lambda) != SUP_OK) return SUP_ERR_INVALID_ARG;
+    if (opt->step_policy != SUP_STEP_PER_TRIAL && opt->step_policy != SUP_STEP_PER_SWEEP)
+        return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_superiorize: unknown step policy");
+    if (opt->block_iterative && h->n_blocks < 1) return sup_fail(h, SUP_ERR_STATE, "sup_superiorize: call sup_set_blocks first");
+    if ((opt->decisions || opt->decision_f) && opt->decisions_cap < 0) return sup_fail(h, SUP_ERR_INVALID_ARG, "decisions_cap < 0");
+    RunPlan P;
+    P.x = x;
+    P.N = N;
+    P.beta0 = beta0;
+    P.a = a;
+    P.o = *opt;
+    sup_status rc = check_objective(h, opt->objective, opt->shape, &P.ny, &P.nx);
+    if (rc != SUP_OK) return rc;
+    sup_launch_begin_run(h, opt->ell0, opt->k0);
+
+    bool graph = opt->use_graph && h->stream != nullptr && !h->graph_failed && n_iter > 1;
+    if (graph) {
+        sup_ctx::GraphKey key;
+        key.x = x;
+        key.N = N;
+        key.objective = opt->objective;
+        key.block = opt->block_iterative;
+        key.policy = opt->step_policy;
+        key.trace_mode = opt->trace_mode;
+        key.beta0 = beta0;
+        key.a = a;
+        key.lambda = opt->lambda;
+        key.s0 = P.ny;
+        key.s1 = P.nx;
+        key.trace = opt->trace;
+        key.dec = opt->decisions;
+        key.decf = opt->decision_f;
+        key.cap = opt->decisions_cap;
+        if (!h->gexec || !(key == h->gkey)) {
+            drop_graph(h);
+            const int64_t launches_before = h->launches;
+            cudaError_t e = cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal);
+            if (e == cudaSuccess) {
+                rc = enqueue_superiorized_sweep(h, P);
+                cudaGraph_t gr = nullptr;
+                e = cudaStreamEndCapture(h->stream, &gr);
+                if (rc == SUP_OK && e == cudaSuccess && gr) {
+                    h->graph = gr;
+                    e = cudaGraphInstantiate(&h->gexec, gr, 0);
+                    size_t nn = 0;
+                    if (e == cudaSuccess) cudaGraphGetNodes(gr, nullptr, &nn);
+                    h->graph_nodes = int(nn);
+                } else if (gr) {
+                    cudaGraphDestroy(gr);
+                }
+            }
+            h->launches = launches_before;
+            if (e != cudaSuccess || rc != SUP_OK || !h->gexec) {
+                cudaGetLastError();
+                drop_graph(h);
+                h->graph_failed = true;  // e.g. cooperative launch not capturable: fall back to direct launches
+                graph = false;
+            } else {
+                h->gkey = key;
+            }
+        }
+    }
+    for (int it = 0; it < n_iter; ++it) {
+        if (graph) {
+            SUP_CUDA(h, cudaGraphLaunch(h->gexec, h->stream));
+            h->launches += h->graph_nodes;
+        } else {
+            rc = enqueue_superiorized_sweep(h, P);
+            if (rc != SUP_OK) return rc;
+        }
+    }
+    SUP_CUDA(h, cudaGetLastError());
+    return SUP_OK;
+}
+
+extern "C" sup_status sup_superiorize(sup_handle h, void* x, int n_iter, int N, double beta0, double a, const sup_options* opt) {
+    if (!h) return SUP_ERR_INVALID_ARG;
+    return run_superiorize(h, x, n_iter, N, beta0, a, opt);
+}
+
+extern "C" sup_status sup_superiorize_host(sup_handle h, void* x_host, int n_iter, int N, double beta0, double a,
+                                           const sup_options* opt) {
+    if (!h) return SUP_ERR_INVALID_ARG;
+    if (!x_host) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_superiorize_host: NULL x");
+    const size_t bytes = size_t(h->n) * h->esz;
+    SUP_CUDA(h, cudaMemcpyAsync(h->xdev, x_host, bytes, cudaMemcpyHostToDevice, h->stream));
+    sup_status rc = run_superiorize(h, h->xdev, n_iter, N, beta0, a, opt);
+    if (rc != SUP_OK) return rc;
+    SUP_CUDA(h, cudaMemcpyAsync(x_host, h->xdev, bytes, cudaMemcpyDeviceToHost, h->stream));
+    SUP_CUDA(h, cudaStreamSynchronize(h->stream));
+    return SUP_OK;
+}
+
+// ---- scalars -----------------------------------------------------------------------------------------------------
+static sup_status fetch_scalar(sup_ctx* h, double* out) {
+    const double* slot = reinterpret_cast<const double*>(reinterpret_cast<const char*>(h->state) + offsetof(DevState, scalar_out));
+    SUP_CUDA(h, cudaMemcpyAsync(out, slot, 8, cudaMemcpyDeviceToHost, h->stream));
+    SUP_CUDA(h, cudaStreamSynchronize(h->stream));
+    if (isnan(*out)) return sup_fail(h, SUP_ERR_NONFINITE, "result is NaN");
+    return SUP_OK;
+}
+
+extern "C" sup_status sup_proximity(sup_handle h, const void* x, int mode, double p, double* out) {
+    if (!h) return SUP_ERR_INVALID_ARG;
+    if (!x || !out || mode < 0 || mode > 2) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_proximity: NULL x/out or mode not in {0,1,2}");
+    if (mode == 1 && !(p > 0.0)) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_proximity: p must be > 0");
+    double* slot = reinterpret_cast<double*>(reinterpret_cast<char*>(h->state) + offsetof(DevState, scalar_out));
+    sup_launch_proximity(h, x, mode, p, slot);
+    return fetch_scalar(h, out);
+}
+
+extern "C" sup_status sup_objective(sup_handle h, const void* x, int kind, const int64_t* shape, double* out) {
+    if (!h) return SUP_ERR_INVALID_ARG;
+    if (!x || !out) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_objective: NULL x or out");
+    int64_t ny, nx;
+    sup_status rc = check_objective(h, kind, shape, &ny, &nx);
+    if (rc != SUP_OK) return rc;
+    double* slot = reinterpret_cast<double*>(reinterpret_cast<char*>(h->state) + offsetof(DevState, scalar_out));
+    sup_launch_objective(h, x, kind, ny, nx, slot);
+    return fetch_scalar(h, out);
+}
+
+extern "C" sup_status sup_get_derived(sup_handle h, int which, void* dst, size_t dst_bytes) {
+    if (!h) return SUP_ERR_INVALID_ARG;
+    const void* src = nullptr;
+    size_t bytes = 0;
+    switch (which) {
+        case 0: src = h->d; bytes = size_t(h->m) * h->esz; break;
+        case 1: src = h->AT.rowptr; bytes = size_t(h->n + 1) * 8; break;
+        case 2: src = h->AT.col; bytes = size_t(h->nnz) * 4; break;
+        case 3: src = h->AT.val; bytes = size_t(h->nnz) * h->esz; break;
+        default: return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_get_derived: unknown array");
+    }
+    if (!dst || dst_bytes < bytes) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_get_derived: dst too small (%zu needed)", bytes);
+    SUP_CUDA(h, cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, h->stream));
+    SUP_CUDA(h, cudaStreamSynchronize(h->stream));
+    return SUP_OK;
+}

@@ -1,0 +1,158 @@
+// sup_internal.cuh -- shared declarations of libsup's translation units (not part of the public ABI).
+// Method and readings: include/sup.h, DESIGN.md.  Nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include <vector>
+
+#include "sup.h"
+
+#define SUP_THREADS 256          // threads per CTA of every kernel
+#define SUP_MAX_PARTIALS 2048    // upper bound on the grid of any kernel that feeds a two-stage reduction
+#define SUP_J_MAX 10000          // trials per reduction step (A-12)
+
+struct CsrD {  // device CSR (borrowed or living in workspace)
+    int64_t rows = 0, cols = 0, nnz = 0;
+    const int64_t* rowptr = nullptr;
+    const int32_t* col = nullptr;
+    const void* val = nullptr;
+};
+
+// device-resident run state; one per handle
+struct DevState {
+    long long ell;        // step-size exponent l
+    long long k;          // absolute sweep index
+    long long it;         // sweep index inside the current sup_superiorize run (row of `trace`)
+    long long n_trials;   // trials since the run started
+    long long sweep_trials;
+    long long n_dec;      // decisions logged (may exceed cap)
+    int warn;
+    int fault;
+    double f;             // objective carried by the last perturbation phase
+    double scalar_out;    // result slot of finalize kernels (proximity / objective)
+    unsigned bar_count;   // grid barrier of the perturbation kernel
+    unsigned bar_gen;
+};
+
+struct Bump {  // bump allocator over caller-provided workspace
+    char* base = nullptr;
+    size_t cap = 0, off = 0;
+    bool ok = true;
+    void* take(size_t bytes) {
+        size_t a = (bytes + 255) & ~size_t(255);
+        if (off + a > cap) { ok = false; return nullptr; }
+        void* p = base + off;
+        off += a;
+        return p;
+    }
+};
+
+struct sup_ctx {
+    int dt = 0;
+    size_t esz = 4;
+    cudaStream_t stream = nullptr;
+    int num_sms = 148;
+    int64_t m = 0, n = 0, nnz = 0;
+    CsrD A, AT;
+    const void *lb = nullptr, *ub = nullptr, *lo = nullptr, *hi = nullptr;
+    void* d = nullptr;          // [m] dtype: w_i / ||a_i||^2
+    double* w = nullptr;        // [m] normalised weights
+    double* invnorm = nullptr;  // [m] 1/||a_i|| (0 for empty rows)
+    void* y = nullptr;          // [m] dtype: scaled violation d_i c_i
+    void* g = nullptr;          // [n] dtype: gradient of the objective
+    void* xdev = nullptr;       // [n] dtype: staging copy of x for sup_superiorize_host
+    double* partials = nullptr; // [2][SUP_MAX_PARTIALS]
+    DevState* state = nullptr;
+    int g_fwd = 32, g_bwd = 32; // lanes per row of the two products
+    // block-iterative
+    int n_blocks = 0;
+    std::vector<int64_t> block_rowptr;
+    std::vector<CsrD> ATb;
+    std::vector<int> g_bwd_blk;
+    void* d_blk = nullptr;      // [m] dtype: (w_i/W_t)/||a_i||^2
+    // dose objective
+    bool has_dose = false;
+    CsrD D, DT;
+    void* r_dose = nullptr;     // [md] dtype
+    int g_d = 8, g_dt = 32;
+    // cached graph of one superiorized sweep
+    cudaGraphExec_t gexec = nullptr;
+    cudaGraph_t graph = nullptr;
+    int graph_nodes = 0;
+    bool graph_failed = false;
+    struct GraphKey {
+        const void* x = nullptr;
+        int N = 0, objective = 0, block = 0, policy = 0, trace_mode = 0;
+        double beta0 = 0, a = 0, lambda = 0;
+        int64_t s0 = 0, s1 = 0;
+        const void *trace = nullptr, *dec = nullptr, *decf = nullptr;
+        int64_t cap = 0;
+        bool operator==(const GraphKey& o) const {
+            return x == o.x && N == o.N && objective == o.objective && block == o.block && policy == o.policy &&
+                   trace_mode == o.trace_mode && beta0 == o.beta0 && a == o.a && lambda == o.lambda && s0 == o.s0 &&
+                   s1 == o.s1 && trace == o.trace && dec == o.dec && decf == o.decf && cap == o.cap;
+        }
+    } gkey;
+    int64_t launches = 0;
+    char err[512] = {0};
+};
+
+sup_status sup_fail(sup_ctx* h, sup_status s, const char* fmt, ...);
+extern char g_create_error[512];
+
+#define SUP_CUDA(h, call)                                                                            \
+    do {                                                                                             \
+        cudaError_t e__ = (call);                                                                    \
+        if (e__ != cudaSuccess)                                                                      \
+            return sup_fail((h), SUP_ERR_CUDA, "%s:%d %s: %s", __FILE__, __LINE__, #call, cudaGetErrorString(e__)); \
+    } while (0)
+
+static inline int sup_pick_group(int64_t nnz, int64_t rows) {
+    // lanes cooperating on one row: about a quarter of the mean row length, a power of two in [4, 32]
+    double avg = rows > 0 ? double(nnz) / double(rows) : 0.0;
+    int g = 4;
+    while (g < 32 && avg > 4.0 * g) g <<= 1;
+    return g;
+}
+static inline int sup_grid_for(int64_t work_items, int per_block, int cap) {
+    int64_t b = (work_items + per_block - 1) / per_block;
+    if (b < 1) b = 1;
+    if (b > cap) b = cap;
+    return int(b);
+}
+
+// ---- setup (sup_setup.cu) ---------------------------------------------------------------------------------
+size_t sup_transpose_scratch_bytes(int64_t nnz, int64_t cols, size_t esz);
+// transposes rows [r0, r1) of A into `out` (cols x (r1-r0) CSR whose "col" entries are ORIGINAL row indices);
+// out arrays must be preallocated: rowptr [A.cols+1], col/val [nnz of the row range].  Stable in row order.
+sup_status sup_transpose_rows(sup_ctx* h, const CsrD& A, int64_t r0, int64_t r1, int64_t e0, int64_t e1,
+                              int64_t* out_rowptr, int32_t* out_col, void* out_val, int64_t out_base, void* scratch,
+                              size_t scratch_bytes);
+sup_status sup_setup_rows(sup_ctx* h, const void* weights, void* scratch, size_t scratch_bytes);
+sup_status sup_setup_block_scaling(sup_ctx* h, void* scratch, size_t scratch_bytes);
+sup_status sup_validate(sup_ctx* h, const CsrD& A, bool check_bounds, void* scratch);
+
+// ---- products (sup_spmv.cu) -------------------------------------------------------------------------------
+void sup_launch_fwd(sup_ctx* h, const void* x, int64_t r0, int64_t r1, const void* dscale);
+void sup_launch_bwd(sup_ctx* h, const CsrD& AT, int G, void* x, double lambda);
+void sup_launch_proximity(sup_ctx* h, const void* x, int mode, double p, double* out_dev);
+
+// ---- perturbation (sup_perturb.cu) ------------------------------------------------------------------------
+struct PerturbParams {
+    int objective;
+    int64_t ny, nx;
+    int N;
+    double beta0, a;
+    int policy;
+    int8_t* decisions;
+    double* decision_f;
+    int64_t cap;
+};
+sup_status sup_launch_perturb(sup_ctx* h, void* x, const PerturbParams& pp);
+void sup_launch_objective(sup_ctx* h, const void* x, int kind, int64_t ny, int64_t nx, double* out_dev);
+void sup_launch_end_sweep(sup_ctx* h, double* trace);
+void sup_launch_trace_slot(sup_ctx* h, double* trace, int slot);  // trace[it][slot] = state->scalar_out
+void sup_launch_begin_run(sup_ctx* h, int64_t ell0, int64_t k0);
+int sup_perturb_grid(sup_ctx* h, int objective);

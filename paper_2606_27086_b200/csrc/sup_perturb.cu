@@ -1,0 +1,521 @@
+// sup_perturb.cu -- S5-S7 of the hot path: the perturbation phase of Algorithm 1
+// as ONE persistent cooperative kernel per phase.
+//
+//   fx <- f(x)
+//   for n = 0..N-1:  g <- grad f(x^{k,n}) (A-7), s <- ||g||_2, v = -g/s (A-6)
+//        trial loop:  beta <- beta0 * a^l (A-10, A-20: pow in fp64), z <- x + beta v, l <- l+1,
+//                     accept iff f(z) <= f(x^{k,n}) (L149, A-11); at most J_max trials (A-12)
+//
+// The number of trials is data dependent, so the loop lives on the device: all CTAs of the grid are co-resident
+// (cooperative launch), meet at a grid barrier after every reduction and take the accept decision redundantly
+// from the same partial sums summed in the same order -- no host round trip, and the launch is capturable in a
+// CUDA graph.  z is never stored: z_p = round_T(x_p - (beta/s) g_p) is recomputed wherever it is needed.
+// Objectives: TV2D (Eq. 15; gradient A-8, shared-memory tile with halo, fused with sum g^2),
+// TV1D (A-16), DOSE ||D x||^2 with g = 2 D^T (D x) (A-15).  Objective terms, norms and beta are fp64 in both modes.
+#include <math.h>
+
+#include "sup_internal.cuh"
+
+#define TILE_H 16
+#define TILE_W 64
+#define BARRIER_SPIN_LIMIT (1u << 24)
+
+template <typename T>
+struct PArgs {
+    T* x;
+    T* g;
+    int64_t n, ny, nx;
+    int N;
+    double beta0, a;
+    int policy;
+    DevState* st;
+    double* partials;  // [2][SUP_MAX_PARTIALS]
+    int8_t* decisions;
+    double* decision_f;
+    int64_t cap;
+    // dose
+    int64_t md;
+    const int64_t* d_rowptr;
+    const int32_t* d_col;
+    const T* d_val;
+    const int64_t* dt_rowptr;
+    const int32_t* dt_col;
+    const T* dt_val;
+    T* r;
+    int g_d, g_dt;
+};
+
+// ---- grid barrier (all CTAs co-resident by cooperative launch) ----------------------------------------------
+__device__ __forceinline__ void grid_barrier(DevState* st) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        volatile unsigned* gen_p = &st->bar_gen;
+        const unsigned gen = *gen_p;
+        const unsigned arrived = atomicAdd(&st->bar_count, 1u);
+        if (arrived == gridDim.x - 1) {
+            st->bar_count = 0;
+            __threadfence();
+            atomicExch(&st->bar_gen, gen + 1u);
+        } else {
+            unsigned spins = 0;
+            while (*gen_p == gen) {
+                __nanosleep(64);
+                if (++spins > BARRIER_SPIN_LIMIT) {  // never hang the device: flag and fall through
+                    atomicOr(&st->fault, 1);
+                    break;
+                }
+            }
+        }
+        __threadfence();
+    }
+    __syncthreads();
+}
+
+// sum over the CTA, result valid in every thread; fixed order
+__device__ __forceinline__ double cta_sum(double v) {
+    __shared__ double ws[SUP_THREADS / 32];
+    __shared__ double tot;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    __syncthreads();
+    if (lane == 0) ws[wid] = v;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int q = 0; q < SUP_THREADS / 32; ++q) t += ws[q];
+        tot = t;
+    }
+    __syncthreads();
+    return tot;
+}
+
+// every CTA sums the same gridDim.x partials in the same order -> identical value everywhere
+__device__ __forceinline__ double reduce_partials(const double* partials) {
+    double s = 0.0;
+    for (int q = threadIdx.x; q < int(gridDim.x); q += SUP_THREADS) s += __ldcg(partials + q);
+    return cta_sum(s);
+}
+
+template <typename T>
+__device__ __forceinline__ double zval(const T* __restrict__ x, const T* __restrict__ g, double coef, int64_t p) {
+    const double xv = double(__ldcg(x + p));
+    if (coef == 0.0) return xv;
+    return double(T(fma(-coef, double(__ldcg(g + p)), xv)));  // z rounded to the storage type, as it would be stored
+}
+
+// ---- objective value of z = x - coef g : this thread's share (not yet reduced) ------------------------------
+template <typename T>
+__device__ double tv2d_share(const PArgs<T>& A, double coef) {
+    // Eq. 15: terms for i < ny-1, j < nx-1 only
+    const int64_t h = A.ny - 1, w = A.nx - 1;
+    const int64_t total = h > 0 && w > 0 ? h * w : 0;
+    double acc = 0.0;
+    for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q < total; q += int64_t(gridDim.x) * blockDim.x) {
+        const int64_t i = q / w, j = q - i * w;
+        const int64_t p = i * A.nx + j;
+        const double z00 = zval(A.x, A.g, coef, p), z10 = zval(A.x, A.g, coef, p + A.nx), z01 = zval(A.x, A.g, coef, p + 1);
+        const double dx = z10 - z00, dy = z01 - z00;
+        acc += sqrt(dx * dx + dy * dy);
+    }
+    return acc;
+}
+
+template <typename T>
+__device__ double tv1d_share(const PArgs<T>& A, double coef) {
+    double acc = 0.0;
+    for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q + 1 < A.n; q += int64_t(gridDim.x) * blockDim.x)
+        acc += fabs(zval(A.x, A.g, coef, q + 1) - zval(A.x, A.g, coef, q));
+    return acc;
+}
+
+// group-of-G row dot against z (dose) or against a plain vector
+template <typename T, bool ZV>
+__device__ __forceinline__ T coop_row_dot(const T* __restrict__ val, const int32_t* __restrict__ col, int64_t s, int64_t e,
+                                          const T* __restrict__ x, const T* __restrict__ g, double coef, int gl, int G) {
+    T a0 = T(0), a1 = T(0);
+    int64_t k = s + gl;
+    for (; k + G < e; k += 2 * int64_t(G)) {
+        const int c0 = __ldcs(col + k), c1 = __ldcs(col + k + G);
+        const T v0 = __ldcs(val + k), v1 = __ldcs(val + k + G);
+        a0 += v0 * (ZV ? T(zval(x, g, coef, c0)) : __ldcg(x + c0));
+        a1 += v1 * (ZV ? T(zval(x, g, coef, c1)) : __ldcg(x + c1));
+    }
+    if (k < e) a0 += __ldcs(val + k) * (ZV ? T(zval(x, g, coef, __ldcs(col + k))) : __ldcg(x + __ldcs(col + k)));
+    T acc = a0 + a1;
+    for (int o = G >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o, G);
+    return acc;
+}
+
+template <typename T>
+__device__ double dose_share(const PArgs<T>& A, double coef, bool store_r) {
+    // f(z) = sum_i (D z)_i^2; optionally stores r = D z (used by the gradient with coef = 0)
+    const int G = A.g_d;
+    const int gl = threadIdx.x % G, lane = threadIdx.x & 31;
+    const int64_t gid = (int64_t(blockIdx.x) * blockDim.x + threadIdx.x) / G;
+    const int64_t ngroups = (int64_t(gridDim.x) * blockDim.x) / G;
+    double acc = 0.0;
+    for (int64_t i0 = gid - lane / G; i0 < A.md; i0 += ngroups) {  // warp-uniform bound
+        const int64_t i = i0 + lane / G;
+        const bool valid = i < A.md;
+        const int64_t s = valid ? A.d_rowptr[i] : 0, e = valid ? A.d_rowptr[i + 1] : 0;
+        const T r = coop_row_dot<T, true>(A.d_val, A.d_col, s, e, A.x, A.g, coef, gl, G);
+        if (valid && gl == 0) {
+            acc += double(r) * double(r);
+            if (store_r) A.r[i] = r;
+        }
+    }
+    return acc;
+}
+
+template <typename T, int OBJ>
+__device__ __forceinline__ double objective_share(const PArgs<T>& A, double coef) {
+    if (OBJ == SUP_OBJ_TV2D) return tv2d_share(A, coef);
+    if (OBJ == SUP_OBJ_TV1D) return tv1d_share(A, coef);
+    if (OBJ == SUP_OBJ_DOSE) return dose_share(A, coef, false);
+    return 0.0;
+}
+
+// ---- gradient: writes g, returns this thread's share of sum g^2 ----------------------------------------------
+// TV2D (A-8): g_ij = -(dx_ij+dy_ij)/t_ij [i<ny-1, j<nx-1] + dx_{i-1,j}/t_{i-1,j} [i>=1, j<nx-1] + dy_{i,j-1}/t_{i,j-1} [j>=1, i<ny-1];
+// a term with t = 0 contributes 0 (A-9).  One CTA stages a TILE_H x TILE_W tile plus a one-pixel halo in shared memory.
+template <typename T>
+__device__ double tv2d_grad_share(const PArgs<T>& A) {
+    __shared__ double tile[TILE_H + 2][TILE_W + 2 + 1];
+    const int64_t ny = A.ny, nx = A.nx;
+    const int64_t tiles_y = (ny + TILE_H - 1) / TILE_H, tiles_x = (nx + TILE_W - 1) / TILE_W;
+    double acc = 0.0;
+    for (int64_t t = blockIdx.x; t < tiles_y * tiles_x; t += gridDim.x) {
+        const int64_t ty = t / tiles_x, tx = t - ty * tiles_x;
+        const int64_t i0 = ty * TILE_H - 1, j0 = tx * TILE_W - 1;  // top-left of the halo
+        __syncthreads();
+        for (int q = threadIdx.x; q < (TILE_H + 2) * (TILE_W + 2); q += SUP_THREADS) {
+            const int li = q / (TILE_W + 2), lj = q - li * (TILE_W + 2);
+            const int64_t i = i0 + li, j = j0 + lj;
+            tile[li][lj] = (i >= 0 && i < ny && j >= 0 && j < nx) ? double(__ldcg(A.x + i * nx + j)) : 0.0;
+        }
+        __syncthreads();
+        for (int q = threadIdx.x; q < TILE_H * TILE_W; q += SUP_THREADS) {
+            const int li = q / TILE_W + 1, lj = q % TILE_W + 1;
+            const int64_t i = i0 + li, j = j0 + lj;
+            if (i >= ny || j >= nx) continue;
+            double gv = 0.0;
+            const double c = tile[li][lj];
+            if (i + 1 < ny && j + 1 < nx) {  // own term (i, j)
+                const double dx = tile[li + 1][lj] - c, dy = tile[li][lj + 1] - c;
+                const double tt = sqrt(dx * dx + dy * dy);
+                if (tt > 0.0) gv -= (dx + dy) / tt;
+            }
+            if (i >= 1 && j + 1 < nx) {  // term (i-1, j): dx_{i-1,j} = X_ij - X_{i-1,j}
+                const double b = tile[li - 1][lj];
+                const double dx = c - b, dy = tile[li - 1][lj + 1] - b;
+                const double tt = sqrt(dx * dx + dy * dy);
+                if (tt > 0.0) gv += dx / tt;
+            }
+            if (j >= 1 && i + 1 < ny) {  // term (i, j-1): dy_{i,j-1} = X_ij - X_{i,j-1}
+                const double b = tile[li][lj - 1];
+                const double dx = tile[li + 1][lj - 1] - b, dy = c - b;
+                const double tt = sqrt(dx * dx + dy * dy);
+                if (tt > 0.0) gv += dy / tt;
+            }
+            const T gs = T(gv);
+            A.g[i * nx + j] = gs;
+            acc += double(gs) * double(gs);
+        }
+    }
+    return acc;
+}
+
+template <typename T>
+__device__ double tv1d_grad_share(const PArgs<T>& A) {
+    double acc = 0.0;
+    for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q < A.n; q += int64_t(gridDim.x) * blockDim.x) {
+        const double c = double(__ldcg(A.x + q));
+        double gv = 0.0;
+        if (q >= 1) {
+            const double dl = c - double(__ldcg(A.x + q - 1));
+            gv += double((dl > 0.0) - (dl < 0.0));
+        }
+        if (q + 1 < A.n) {
+            const double dr = double(__ldcg(A.x + q + 1)) - c;
+            gv -= double((dr > 0.0) - (dr < 0.0));
+        }
+        A.g[q] = T(gv);
+        acc += gv * gv;
+    }
+    return acc;
+}
+
+template <typename T>
+__device__ double dose_grad_share(const PArgs<T>& A) {
+    // r = D x has been stored by dose_share(store_r) and a grid barrier passed; g_j = 2 sum_i D_ij r_i over row j of D^T
+    const int G = A.g_dt;
+    const int gl = threadIdx.x % G, lane = threadIdx.x & 31;
+    const int64_t gid = (int64_t(blockIdx.x) * blockDim.x + threadIdx.x) / G;
+    const int64_t ngroups = (int64_t(gridDim.x) * blockDim.x) / G;
+    double acc = 0.0;
+    for (int64_t j0 = gid - lane / G; j0 < A.n; j0 += ngroups) {
+        const int64_t j = j0 + lane / G;
+        const bool valid = j < A.n;
+        const int64_t s = valid ? A.dt_rowptr[j] : 0, e = valid ? A.dt_rowptr[j + 1] : 0;
+        const T u = coop_row_dot<T, false>(A.dt_val, A.dt_col, s, e, A.r, nullptr, 0.0, gl, G);
+        if (valid && gl == 0) {
+            const T gs = T(2) * u;
+            A.g[j] = gs;
+            acc += double(gs) * double(gs);
+        }
+    }
+    return acc;
+}
+
+// ---- the perturbation phase ----------------------------------------------------------------------------------
+template <typename T, int OBJ>
+__global__ void __launch_bounds__(SUP_THREADS) k_perturb(PArgs<T> A) {
+    DevState* st = A.st;
+    long long ell = *(volatile long long*)&st->ell;
+    const long long k = *(volatile long long*)&st->k;
+    long long ndec = *(volatile long long*)&st->n_dec;
+    long long trials = 0;
+    int warn = 0, fault = 0;
+    int slot = 0;
+    double* P0 = A.partials;
+    double* P1 = A.partials + SUP_MAX_PARTIALS;
+
+    // fx = f(x)
+    double sh = cta_sum(objective_share<T, OBJ>(A, 0.0));
+    if (threadIdx.x == 0) P0[blockIdx.x] = sh;
+    grid_barrier(st);
+    double fx = reduce_partials(P0);
+    slot = 1;
+    if (!isfinite(fx)) fault |= 2;
+
+    for (int nred = 0; nred < A.N; ++nred) {
+        double* P = slot ? P1 : P0;
+        slot ^= 1;
+        if (OBJ == SUP_OBJ_DOSE) {  // r = D x first
+            dose_share(A, 0.0, true);
+            grid_barrier(st);
+            sh = cta_sum(dose_grad_share(A));
+        } else if (OBJ == SUP_OBJ_TV2D) {
+            sh = cta_sum(tv2d_grad_share(A));
+        } else {
+            sh = cta_sum(tv1d_grad_share(A));
+        }
+        if (threadIdx.x == 0) P[blockIdx.x] = sh;
+        grid_barrier(st);
+        const double s = sqrt(reduce_partials(P));
+        bool accepted = false;
+        long long jloc = 0;
+        for (int trial = 0; trial < SUP_J_MAX && !accepted; ++trial) {
+            const double expo = A.policy == SUP_STEP_PER_TRIAL ? double(ell) : double(k + jloc);
+            const double beta = A.beta0 * pow(A.a, expo);
+            const double coef = s > 0.0 ? beta / s : 0.0;
+            P = slot ? P1 : P0;
+            slot ^= 1;
+            sh = cta_sum(objective_share<T, OBJ>(A, coef));
+            if (threadIdx.x == 0) P[blockIdx.x] = sh;
+            grid_barrier(st);
+            const double fz = reduce_partials(P);
+            ++ell;
+            ++jloc;
+            ++trials;
+            const bool acc = fz <= fx;  // NaN compares false -> rejected (A-11)
+            if (blockIdx.x == 0 && threadIdx.x == 0) {
+                if (A.decisions && ndec < A.cap) A.decisions[ndec] = acc ? 1 : 0;
+                if (A.decision_f && ndec < A.cap) {
+                    A.decision_f[2 * ndec] = fz;
+                    A.decision_f[2 * ndec + 1] = fx;
+                }
+            }
+            ++ndec;
+            if (acc) {
+                if (coef != 0.0)
+                    for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q < A.n; q += int64_t(gridDim.x) * blockDim.x)
+                        A.x[q] = T(zval(A.x, A.g, coef, q));
+                grid_barrier(st);  // x^{k,n+1} visible to everyone before the next gradient
+                fx = fz;
+                accepted = true;
+            }
+            if (*(volatile int*)&st->fault & 1) break;  // a barrier timed out: stop looping
+        }
+        if (!accepted) warn |= 1;  // A-12: step skipped
+        if (*(volatile int*)&st->fault & 1) break;
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        st->ell = ell;
+        st->n_dec = ndec;
+        st->n_trials += trials;
+        st->sweep_trials += trials;
+        st->f = fx;
+        if (warn) atomicOr(&st->warn, warn);
+        if (fault) atomicOr(&st->fault, fault);
+    }
+}
+
+// ---- stand-alone objective value (sup_objective, trace mode) -------------------------------------------------
+template <typename T, int OBJ>
+__global__ void __launch_bounds__(SUP_THREADS) k_objective(PArgs<T> A) {
+    const double sh = cta_sum(objective_share<T, OBJ>(A, 0.0));
+    if (threadIdx.x == 0) A.partials[blockIdx.x] = sh;
+}
+__global__ void k_sum_final(const double* __restrict__ partials, int np, double* __restrict__ out) {
+    __shared__ double shm[SUP_THREADS];
+    double s = 0.0;
+    for (int q = threadIdx.x; q < np; q += SUP_THREADS) s += partials[q];
+    shm[threadIdx.x] = s;
+    __syncthreads();
+    for (int o = SUP_THREADS / 2; o > 0; o >>= 1) {
+        if (threadIdx.x < o) shm[threadIdx.x] += shm[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *out = shm[0];
+}
+
+__global__ void k_end_sweep(DevState* st, double* trace) {
+    if (trace) {
+        trace[4 * st->it + 2] = double(st->sweep_trials);
+        trace[4 * st->it + 3] = double(st->ell);
+    }
+    st->sweep_trials = 0;
+    st->k += 1;
+    st->it += 1;
+}
+__global__ void k_trace_slot(DevState* st, double* trace, int slot) { trace[4 * st->it + slot] = st->scalar_out; }
+
+// ---- host side --------------------------------------------------------------------------------------------------
+template <typename T>
+static PArgs<T> make_args(sup_ctx* h, void* x, const PerturbParams& pp) {
+    PArgs<T> A;
+    A.x = static_cast<T*>(x);
+    A.g = static_cast<T*>(h->g);
+    A.n = h->n;
+    A.ny = pp.ny;
+    A.nx = pp.nx;
+    A.N = pp.N;
+    A.beta0 = pp.beta0;
+    A.a = pp.a;
+    A.policy = pp.policy;
+    A.st = h->state;
+    A.partials = h->partials;
+    A.decisions = pp.decisions;
+    A.decision_f = pp.decision_f;
+    A.cap = pp.cap;
+    A.md = h->D.rows;
+    A.d_rowptr = h->D.rowptr;
+    A.d_col = h->D.col;
+    A.d_val = static_cast<const T*>(h->D.val);
+    A.dt_rowptr = h->DT.rowptr;
+    A.dt_col = h->DT.col;
+    A.dt_val = static_cast<const T*>(h->DT.val);
+    A.r = static_cast<T*>(h->r_dose);
+    A.g_d = h->g_d;
+    A.g_dt = h->g_dt;
+    return A;
+}
+
+template <typename T>
+static const void* perturb_kernel(int objective) {
+    switch (objective) {
+        case SUP_OBJ_TV2D: return reinterpret_cast<const void*>(&k_perturb<T, SUP_OBJ_TV2D>);
+        case SUP_OBJ_TV1D: return reinterpret_cast<const void*>(&k_perturb<T, SUP_OBJ_TV1D>);
+        case SUP_OBJ_DOSE: return reinterpret_cast<const void*>(&k_perturb<T, SUP_OBJ_DOSE>);
+    }
+    return nullptr;
+}
+
+// grid of the cooperative kernel: enough CTAs for the work, never more than can be co-resident or than the
+// partial-sum slots; small problems get small grids (a barrier costs more with more CTAs)
+int sup_perturb_grid(sup_ctx* h, int objective) {
+    const void* fn = h->dt == SUP_F32 ? perturb_kernel<float>(objective) : perturb_kernel<double>(objective);
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, SUP_THREADS, 0) != cudaSuccess || per_sm < 1) return 0;
+    int64_t cap = int64_t(per_sm) * h->num_sms;
+    if (cap > SUP_MAX_PARTIALS) cap = SUP_MAX_PARTIALS;
+    int64_t want;
+    if (objective == SUP_OBJ_DOSE) {
+        want = (h->D.rows * h->g_d + SUP_THREADS - 1) / SUP_THREADS;
+        if (want > 4 * int64_t(h->num_sms)) want = 4 * int64_t(h->num_sms);
+    } else {
+        want = (h->n + 4 * SUP_THREADS - 1) / (4 * SUP_THREADS);  // about four elements per thread
+        if (want > 2 * int64_t(h->num_sms)) want = 2 * int64_t(h->num_sms);
+    }
+    if (want < 1) want = 1;
+    return int(want < cap ? want : cap);
+}
+
+sup_status sup_launch_perturb(sup_ctx* h, void* x, const PerturbParams& pp) {
+    const int grid = sup_perturb_grid(h, pp.objective);
+    if (grid < 1) return sup_fail(h, SUP_ERR_CUDA, "perturbation kernel cannot be made resident");
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(unsigned(grid));
+    cfg.blockDim = dim3(SUP_THREADS);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = h->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeCooperative;
+    attr[0].val.cooperative = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    if (h->dt == SUP_F32) {
+        PArgs<float> A = make_args<float>(h, x, pp);
+        void* args[] = {&A};
+        SUP_CUDA(h, cudaLaunchKernelExC(&cfg, perturb_kernel<float>(pp.objective), args));
+    } else {
+        PArgs<double> A = make_args<double>(h, x, pp);
+        void* args[] = {&A};
+        SUP_CUDA(h, cudaLaunchKernelExC(&cfg, perturb_kernel<double>(pp.objective), args));
+    }
+    h->launches++;
+    return SUP_OK;
+}
+
+template <typename T>
+static void launch_objective_t(sup_ctx* h, const void* x, int kind, int64_t ny, int64_t nx, double* out_dev) {
+    PerturbParams pp = {};
+    pp.objective = kind;
+    pp.ny = ny;
+    pp.nx = nx;
+    PArgs<T> A = make_args<T>(h, const_cast<void*>(x), pp);
+    int grid = h->num_sms * 4;
+    if (grid > SUP_MAX_PARTIALS) grid = SUP_MAX_PARTIALS;
+    const int64_t work = kind == SUP_OBJ_DOSE ? h->D.rows * h->g_d : h->n;
+    grid = sup_grid_for(work, SUP_THREADS, grid);
+    if (kind == SUP_OBJ_TV2D) k_objective<T, SUP_OBJ_TV2D><<<grid, SUP_THREADS, 0, h->stream>>>(A);
+    else if (kind == SUP_OBJ_TV1D) k_objective<T, SUP_OBJ_TV1D><<<grid, SUP_THREADS, 0, h->stream>>>(A);
+    else if (kind == SUP_OBJ_DOSE) k_objective<T, SUP_OBJ_DOSE><<<grid, SUP_THREADS, 0, h->stream>>>(A);
+    else k_objective<T, SUP_OBJ_NONE><<<1, SUP_THREADS, 0, h->stream>>>(A);
+    k_sum_final<<<1, SUP_THREADS, 0, h->stream>>>(h->partials, kind == SUP_OBJ_NONE ? 1 : grid, out_dev);
+    h->launches += 2;
+}
+
+void sup_launch_objective(sup_ctx* h, const void* x, int kind, int64_t ny, int64_t nx, double* out_dev) {
+    if (h->dt == SUP_F32) launch_objective_t<float>(h, x, kind, ny, nx, out_dev);
+    else launch_objective_t<double>(h, x, kind, ny, nx, out_dev);
+}
+
+void sup_launch_end_sweep(sup_ctx* h, double* trace) {
+    k_end_sweep<<<1, 1, 0, h->stream>>>(h->state, trace);
+    h->launches++;
+}
+
+void sup_launch_trace_slot(sup_ctx* h, double* trace, int slot) {
+    k_trace_slot<<<1, 1, 0, h->stream>>>(h->state, trace, slot);
+    h->launches++;
+}
+
+__global__ void k_begin_run(DevState* st, long long ell0, long long k0) {
+    st->ell = ell0;
+    st->k = k0;
+    st->it = 0;
+    st->n_trials = 0;
+    st->sweep_trials = 0;
+    st->n_dec = 0;
+    st->warn = 0;
+    st->fault = 0;
+    st->bar_count = 0;
+}
+void sup_launch_begin_run(sup_ctx* h, int64_t ell0, int64_t k0) {
+    k_begin_run<<<1, 1, 0, h->stream>>>(h->state, ell0, k0);
+    h->launches++;
+}

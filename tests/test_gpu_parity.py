@@ -1,0 +1,438 @@
+"""GPU parity: libsup (through the C ABI, via the ctypes binding) against the fp64 oracle on the same seeded inputs.
+
+Bars (BASELINE.json north_star):
+  fp64 mode: relative L2 error of x <= 1e-10 after 10 sweeps;
+  fp32 mode: <= 1e-4 at sweep 10 and <= 1e-3 at the final sweep; proximity and objective within 1e-4 relative;
+  integer / index work (transposed CSR, decision traces, step-size exponent) bit-exact (A-13 governs knife edges).
+"""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+pytestmark = pytest.mark.gpu
+
+import gen  # noqa: E402
+from oracle.oracle import Oracle, PER_SWEEP, PER_TRIAL  # noqa: E402
+
+INF = np.inf
+
+
+def _sup():
+    import paper_2606_27086_b200 as sup
+
+    return sup
+
+
+def rel_l2(a, b):
+    a = np.asarray(a, np.float64)
+    b = np.asarray(b, np.float64)
+    nb = np.linalg.norm(b)
+    return np.linalg.norm(a - b) / nb if nb > 0 else np.linalg.norm(a - b)
+
+
+def close_scalar(g, o, rtol):
+    if abs(o) < 1e-30:
+        return abs(g) < 1e-12
+    return abs(g - o) <= rtol * abs(o)
+
+
+TD = {0: torch.float32, 1: torch.float64}
+SWEEP_TOL = {0: 1e-4, 1: 1e-10}
+FINAL_TOL = {0: 1e-3, 1: 1e-9}
+
+
+def make_handle(P, dtype, blocks=True):
+    from paper_2606_27086_b200.binding import create_from_problem
+
+    return create_from_problem(P, dtype=dtype, blocks=blocks)
+
+
+def xdev(P, dtype, x=None):
+    return torch.tensor(np.asarray(P.x0 if x is None else x), dtype=TD[dtype], device="cuda:0")
+
+
+PROBLEMS = {
+    "cfg1": lambda: gen.config1_tiny_ct(),
+    "cfg2": lambda: gen.config2_crosswell(),
+    "cfg5_k16": lambda: gen.config5_sweep_point(16, 16),
+    "cfg5_k64": lambda: gen.config5_sweep_point(16, 64),
+    "cfg5_k256_notv": lambda: gen.config5_sweep_point(16, 256, with_tv=False),
+    "cfg4_small": lambda: gen.config4_imrt(scale=0.2),
+    "cfg4_small_infeasible": lambda: gen.config4_imrt(scale=0.2, infeasible=True),
+    "ct_ragged": lambda: gen.config1_tiny_ct(n_pix=37, n_angles=23, n_bins=61, n_sweeps=12, N=3),
+}
+_cache = {}
+
+
+def problem(name):
+    if name not in _cache:
+        _cache[name] = PROBLEMS[name]()
+    return _cache[name]
+
+
+# ------------------------------------------------------------------------------------------------------------
+# S0: transposed CSR and row scaling (index work: bit-exact)
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg5_k16", "cfg4_small", "ct_ragged"])
+@pytest.mark.parametrize("dtype", [0, 1])
+def test_transpose_and_scaling(name, dtype):
+    from paper_2606_27086_b200.binding import sup_get_derived
+
+    P = problem(name)
+    H = make_handle(P, dtype, blocks=False)
+    import scipy.sparse as sp
+
+    A = sp.csr_matrix((P.val.astype(np.float64), P.col, P.rowptr), shape=(P.m, P.n))
+    AT = A.T.tocsr()
+    AT.sort_indices()
+    rp = sup_get_derived(H, 1).cpu().numpy()
+    col = sup_get_derived(H, 2).cpu().numpy()
+    val = sup_get_derived(H, 3).cpu().numpy()
+    assert np.array_equal(rp, AT.indptr.astype(np.int64))
+    assert np.array_equal(col, AT.indices.astype(np.int32))  # every A^T row sorted by original row index (stable)
+    assert np.array_equal(val.astype(np.float64), AT.data)   # values moved, not recomputed: exact
+    O = Oracle.from_problem(P)
+    d = sup_get_derived(H, 0).cpu().numpy().astype(np.float64)
+    np.testing.assert_allclose(d, O.d, rtol=2e-7 if dtype == 0 else 1e-14, atol=0)
+
+
+# ------------------------------------------------------------------------------------------------------------
+# S1-S3: unperturbed sweeps; S4: proximity
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg5_k16", "cfg5_k64", "cfg5_k256_notv", "cfg4_small", "cfg4_small_infeasible", "ct_ragged"])
+@pytest.mark.parametrize("dtype", [0, 1])
+def test_simultaneous_sweeps(name, dtype):
+    sup = _sup()
+    P = problem(name)
+    H = make_handle(P, dtype, blocks=False)
+    O = Oracle.from_problem(P)
+    x = xdev(P, dtype)
+    xo = P.x0.astype(np.float64)
+    for s in (1, 9):
+        sup.sup_project_simultaneous(H, x, P.lam, s)
+        xo = O.sweep(xo, P.lam, s)
+        assert rel_l2(x.cpu().numpy(), xo) <= SWEEP_TOL[dtype], (name, s)
+    # proximity of the GPU iterate, all three modes, against the oracle evaluated on the SAME iterate
+    xg = x.cpu().numpy().astype(np.float64)
+    for mode, p in [(0, 2.0), (1, 2.0), (1, 1.0), (1, 1.5), (2, 0.0)]:
+        pg = sup.sup_proximity(H, x, mode, p if mode == 1 else 2.0)
+        po = O.proximity(xg, mode, p if mode == 1 else 2.0)
+        assert close_scalar(pg, po, 1e-4 if dtype == 0 else 1e-11), (name, mode, p, pg, po)
+
+
+@pytest.mark.parametrize("lam", [0.0, 0.5, 1.7, 2.0])
+def test_relaxation_values(lam):
+    sup = _sup()
+    P = problem("ct_ragged")
+    H = make_handle(P, 1, blocks=False)
+    O = Oracle.from_problem(P)
+    rng = np.random.default_rng(5)
+    x0 = rng.uniform(0, 1, P.n)
+    x = xdev(P, 1, x0)
+    sup.sup_project_simultaneous(H, x, lam, 3)
+    xo = O.sweep(x0, lam, 3)
+    assert rel_l2(x.cpu().numpy(), xo) <= 1e-12
+    if lam == 0.0:
+        assert np.array_equal(x.cpu().numpy(), np.clip(x0, P.lo, P.hi))
+
+
+def test_fixed_point_and_weights():
+    """x* inside C and the box is returned bit-identically (all c_i = 0); caller weights are normalised (A-3)."""
+    sup = _sup()
+    P = problem("cfg5_k16")
+    for dtype in (0, 1):
+        H = make_handle(P, dtype, blocks=False)
+        x = xdev(P, dtype, P.x_true)
+        before = x.clone()
+        sup.sup_project_simultaneous(H, x, 1.0, 3)
+        assert torch.equal(x, before)
+        assert sup.sup_proximity(H, x, 0) == 0.0
+    rng = np.random.default_rng(1)
+    w = rng.uniform(0.5, 2.0, P.m).astype(np.float32)
+    H = sup.sup_create(P.rowptr, P.col, P.val, P.lb, P.ub, P.lo, P.hi, w, dtype=1, n=P.n)
+    O = Oracle(P.m, P.n, P.rowptr, P.col, P.val, P.lb, P.ub, P.lo, P.hi, w)
+    x = xdev(P, 1)
+    sup.sup_project_simultaneous(H, x, 1.0, 5)
+    assert rel_l2(x.cpu().numpy(), O.sweep(P.x0, 1.0, 5)) <= 1e-12
+
+
+def test_empty_rows_and_infinite_bounds():
+    """Rows with ||a_i|| = 0 are inert even when 0 is outside [lb, ub] (A-4); +-inf bounds never produce NaN."""
+    sup = _sup()
+    rng = np.random.default_rng(3)
+    m, n = 300, 40
+    dense = rng.normal(size=(m, n)) * (rng.uniform(size=(m, n)) < 0.2)
+    dense[::7] = 0.0
+    import scipy.sparse as sp
+
+    S = sp.csr_matrix(dense)
+    S.sort_indices()
+    rp, c, v = S.indptr.astype(np.int64), S.indices.astype(np.int32), S.data
+    v = v.astype(np.float32)
+    lb = rng.uniform(-1, 0, m).astype(np.float32)
+    ub = (lb + rng.uniform(0.1, 1, m)).astype(np.float32)
+    lb[::3] = -INF
+    ub[1::3] = INF
+    lb[::7], ub[::7] = 1.0, 2.0  # empty rows whose slab excludes 0
+    lo = np.full(n, -INF, np.float32)
+    hi = np.full(n, INF, np.float32)
+    lo[:10] = -0.5
+    x0 = rng.normal(size=n).astype(np.float32) * 3
+    O = Oracle(m, n, rp, c, v, lb, ub, lo, hi)
+    for dtype in (0, 1):
+        H = sup.sup_create(rp, c, v, lb, ub, lo, hi, None, dtype=dtype, n=n)
+        x = torch.tensor(x0, dtype=TD[dtype], device="cuda:0")
+        sup.sup_project_simultaneous(H, x, 1.0, 10)
+        xg = x.cpu().numpy()
+        assert np.all(np.isfinite(xg))
+        assert rel_l2(xg, O.sweep(x0, 1.0, 10)) <= SWEEP_TOL[dtype]
+        for mode in (0, 1, 2):
+            assert close_scalar(sup.sup_proximity(H, x, mode, 2.0), O.proximity(xg.astype(np.float64), mode, 2.0), 1e-4 if dtype == 0 else 1e-11)
+
+
+# ------------------------------------------------------------------------------------------------------------
+# S9: block-iterative
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", [0, 1])
+@pytest.mark.parametrize("n_blocks", [1, 5, 16])
+def test_block_iterative(dtype, n_blocks):
+    sup = _sup()
+    base = gen.config1_tiny_ct(n_pix=48, n_angles=64, n_bins=69, n_sweeps=10, N=2)
+    P = gen.interleaved_angle_blocks(base, n_blocks)
+    H = make_handle(P, dtype)
+    O = Oracle.from_problem(P)
+    x = xdev(P, dtype)
+    sup.sup_block_iterative(H, x, 1.0, 10)
+    xo = O.block_sweep(P.x0, 1.0, 10)
+    assert rel_l2(x.cpu().numpy(), xo) <= SWEEP_TOL[dtype]
+    if n_blocks == 1:  # B = 1 is the simultaneous sweep
+        x2 = xdev(P, dtype)
+        sup.sup_project_simultaneous(H, x2, 1.0, 10)
+        assert rel_l2(x2.cpu().numpy(), x.cpu().numpy()) <= (1e-6 if dtype == 0 else 1e-13)
+
+
+# ------------------------------------------------------------------------------------------------------------
+# S5/S6/S7: objectives and one perturbation phase
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", [0, 1])
+def test_objective_values(dtype):
+    sup = _sup()
+    rng = np.random.default_rng(11)
+    for name, kind in [("cfg1", "tv2d"), ("ct_ragged", "tv2d"), ("cfg5_k16", "tv1d"), ("cfg4_small", "dose")]:
+        P = problem(name)
+        H = make_handle(P, dtype, blocks=False)
+        O = Oracle.from_problem(P)
+        xs = rng.uniform(0, 1, P.n).astype(np.float32)
+        x = xdev(P, dtype, xs)
+        fg = sup.sup_objective(H, x, kind, P.shape if kind == "tv2d" else None)
+        fo = O.objective_value(xs.astype(np.float64), kind, P.shape)
+        assert close_scalar(fg, fo, 1e-6 if dtype == 0 else 1e-12), (name, fg, fo)
+    # rectangular image: the last row / column start no term (Eq. 15)
+    P = problem("cfg1")
+    H = make_handle(P, dtype, blocks=False)
+    xs = rng.uniform(0, 1, P.n).astype(np.float32)
+    O = Oracle.from_problem(P)
+    for shape in [(32, 128), (128, 32), (1, 4096), (4096, 1), (2, 2048)]:
+        fg = sup.sup_objective(H, xdev(P, dtype, xs), "tv2d", shape)
+        assert close_scalar(fg, O.objective_value(xs.astype(np.float64), "tv2d", shape), 1e-12)
+
+
+@pytest.mark.parametrize("dtype", [0, 1])
+@pytest.mark.parametrize("name,kind", [("cfg1", "tv2d"), ("ct_ragged", "tv2d"), ("cfg5_k16", "tv1d"), ("cfg4_small", "dose")])
+def test_perturbation_phase(name, kind, dtype):
+    sup = _sup()
+    P = problem(name)
+    H = make_handle(P, dtype, blocks=False)
+    O = Oracle.from_problem(P)
+    rng = np.random.default_rng(2)
+    xs = (P.x_true if P.x_true is not None else rng.uniform(0, 1, P.n)).astype(np.float32)
+    if kind == "dose":
+        xs = rng.uniform(0.5, 1.5, P.n).astype(np.float32)
+    else:
+        xs = (xs + 0.05 * rng.normal(size=P.n)).astype(np.float32)
+    x = xdev(P, dtype, xs)
+    ell = 3
+    for phase in range(3):
+        shape = P.shape if kind == "tv2d" else (P.n,)
+        if kind == "dose":
+            ell_g = sup.sup_perturb_dose(H, x, 4, P.beta0, 0.9, ell)
+        else:
+            ell_g = sup.sup_perturb_tv(H, x, shape, 4, P.beta0, 0.9, ell)
+        st = sup.sup_get_state(H)
+        R = O.perturb(xs.astype(np.float64) if phase == 0 else xo, ell, 4, P.beta0, 0.9, kind=kind, shape=P.shape)
+        xo = R["x"]
+        assert ell_g == R["ell"], (phase, ell_g, R["ell"], R["margins"].min())
+        assert st["n_trials"] == R["trials"]
+        assert rel_l2(x.cpu().numpy(), xo) <= (1e-6 if dtype == 0 else 1e-13)
+        assert close_scalar(st["f"], R["fx"], 1e-5 if dtype == 0 else 1e-12)
+        ell = ell_g
+
+
+def test_flat_image_zero_gradient():
+    """g = 0 => v = 0 => z = x, accepted with equality, l advances, x untouched (A-6)."""
+    sup = _sup()
+    P = problem("cfg1")
+    H = make_handle(P, 0, blocks=False)
+    x = torch.full((P.n,), 0.25, dtype=torch.float32, device="cuda:0")
+    ell = sup.sup_perturb_tv(H, x, P.shape, 5, 1.0, 0.99, 0)
+    assert ell == 5
+    assert torch.all(x == 0.25)
+
+
+# ------------------------------------------------------------------------------------------------------------
+# S8: Algorithm 1 end to end
+# ------------------------------------------------------------------------------------------------------------
+def run_superiorized(P, dtype, n_iter, snaps, policy=PER_TRIAL, block=False, use_graph=True):
+    """Runs GPU and oracle; returns per-snapshot errors.  Applies the A-13 knife-edge protocol."""
+    sup = _sup()
+    H = make_handle(P, dtype)
+    O = Oracle.from_problem(P)
+    cap = 1 << 16
+    dec = torch.zeros(cap, dtype=torch.int8, device="cuda:0")
+    decf = torch.zeros((cap, 2), dtype=torch.float64, device="cuda:0")
+    trace = torch.zeros((n_iter, 4), dtype=torch.float64, device="cuda:0")
+    x = xdev(P, dtype)
+    stops = sorted(set(s for s in snaps if 0 < s < n_iter)) + [n_iter]
+    # the GPU run is split at the snapshot sweeps; state (x, l, k) carries over, logs are offset by hand
+    got = {}
+    k = 0
+    ell = 0
+    all_dec = []
+    tr = []
+    for stop in stops:
+        cnt = stop - k
+        dec.zero_()
+        trace_seg = torch.zeros((cnt, 4), dtype=torch.float64, device="cuda:0")
+        sup.sup_superiorize(H, x, cnt, P.N, P.beta0, P.a, objective=P.objective, shape=P.shape, lam=P.lam, block=block,
+                            policy=policy, ell0=ell, k0=k, trace=trace_seg, decisions=dec, decision_f=decf, use_graph=use_graph)
+        st = sup.sup_get_state(H)
+        assert st["fault"] == 0 and st["warn"] == 0
+        assert st["n_decisions"] <= cap
+        all_dec.append(dec[: st["n_decisions"]].cpu().numpy().copy())
+        ell = st["ell"]
+        k = stop
+        got[stop] = x.cpu().numpy().astype(np.float64)
+        tr.append(trace_seg.cpu().numpy())
+    gdec = np.concatenate(all_dec) if all_dec else np.zeros(0, np.int8)
+    gtrace = np.concatenate(tr)
+    R = O.superiorize(P.x0, n_iter, P.N, P.beta0, P.a, lam=P.lam, policy=policy, block=block, snapshots=snaps)
+    replayed = False
+    if not (gdec.size == R["decisions"].size and np.array_equal(gdec, R["decisions"])):
+        nmin = min(gdec.size, R["decisions"].size)
+        first = int(np.flatnonzero(gdec[:nmin] != R["decisions"][:nmin])[0]) if np.any(gdec[:nmin] != R["decisions"][:nmin]) else nmin
+        margin = R["margins"][first] if first < R["margins"].size else 0.0
+        assert margin < (1e-6 if dtype == 0 else 1e-12), f"decision traces differ at trial {first} with oracle margin {margin:g}: a bug, not a knife edge"
+        R = O.superiorize(P.x0, n_iter, P.N, P.beta0, P.a, lam=P.lam, policy=policy, block=block, snapshots=snaps, forced=gdec)
+        replayed = True
+    return dict(got=got, R=R, gtrace=gtrace, ell=ell, replayed=replayed, H=H, gdec=gdec)
+
+
+def check_superiorized(P, dtype, n_iter, policy=PER_TRIAL, block=False, use_graph=True):
+    snaps = (1, 10)
+    out = run_superiorized(P, dtype, n_iter, snaps, policy, block, use_graph)
+    R = out["R"]
+    assert out["ell"] == R["ell"]
+    for s, xg in out["got"].items():
+        tol = FINAL_TOL[dtype] if s == n_iter and s > 10 else SWEEP_TOL[dtype]
+        err = rel_l2(xg, R["snaps"][s])
+        assert err <= tol, (P.name, dtype, s, err)
+    # trace: proximity (Eq. 5) and objective after each compared sweep within 1e-4 relative; trials and l exact
+    for s in [t for t in (1, 10, n_iter) if t <= n_iter]:
+        g, o = out["gtrace"][s - 1], R["trace"][s - 1]
+        assert close_scalar(g[0], o[0], 1e-4), (P.name, "prox", s, g[0], o[0])
+        assert close_scalar(g[1], o[1], 1e-4), (P.name, "obj", s, g[1], o[1])
+        assert g[2] == o[2] and g[3] == o[3]
+    return out
+
+
+@pytest.mark.parametrize("dtype", [0, 1])
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg5_k16", "cfg5_k64", "cfg4_small", "cfg4_small_infeasible", "ct_ragged"])
+def test_superiorize_configs(name, dtype):
+    P = problem(name)
+    check_superiorized(P, dtype, P.n_sweeps if name not in ("cfg4_small", "cfg4_small_infeasible") else 40)
+
+
+@pytest.mark.parametrize("dtype", [0, 1])
+def test_superiorize_block_iterative(dtype):
+    base = gen.config1_tiny_ct(n_pix=48, n_angles=64, n_bins=69, n_sweeps=30, N=3)
+    P = gen.interleaved_angle_blocks(base, 16)
+    check_superiorized(P, dtype, 30, block=True)
+
+
+def test_superiorize_per_sweep_policy_and_no_graph():
+    P = problem("ct_ragged")
+    check_superiorized(P, 1, 12, policy=PER_SWEEP)
+    check_superiorized(P, 1, 12, use_graph=False)
+
+
+def test_beta_zero_and_N_zero_reproduce_basic_algorithm():
+    """Eq. 10 with beta v = 0: bit-identical to the unperturbed sweeps."""
+    sup = _sup()
+    P = problem("cfg1")
+    for dtype in (0, 1):
+        H = make_handle(P, dtype)
+        xa, xb, xc = xdev(P, dtype), xdev(P, dtype), xdev(P, dtype)
+        sup.sup_project_simultaneous(H, xa, 1.0, 7)
+        sup.sup_superiorize(H, xb, 7, 5, 0.0, 0.99, objective="tv2d", shape=P.shape)
+        sup.sup_superiorize(H, xc, 7, 0, 1.0, 0.99, objective="tv2d", shape=P.shape)
+        assert torch.equal(xa, xb) and torch.equal(xa, xc)
+
+
+def test_host_entry_matches_device_entry():
+    sup = _sup()
+    P = problem("cfg1")
+    H = make_handle(P, 0)
+    x = xdev(P, 0)
+    sup.sup_superiorize(H, x, 12, P.N, P.beta0, P.a, objective="tv2d", shape=P.shape)
+    xh = torch.tensor(P.x0, dtype=torch.float32).pin_memory()
+    sup.sup_superiorize_host(H, xh, 12, P.N, P.beta0, P.a, objective="tv2d", shape=P.shape)
+    assert torch.equal(x.cpu(), xh)
+
+
+def test_runs_are_deterministic():
+    sup = _sup()
+    P = problem("cfg2")
+    outs = []
+    for _ in range(2):
+        H = make_handle(P, 0)
+        x = xdev(P, 0)
+        sup.sup_superiorize(H, x, 20, P.N, P.beta0, P.a, objective="tv2d", shape=P.shape)
+        outs.append(x.cpu())
+    assert torch.equal(outs[0], outs[1])
+
+
+# ------------------------------------------------------------------------------------------------------------
+# errors
+# ------------------------------------------------------------------------------------------------------------
+def test_argument_errors():
+    sup = _sup()
+    P = problem("ct_ragged")
+    H = make_handle(P, 0, blocks=False)
+    x = xdev(P, 0)
+    with pytest.raises(sup.SupError) as e:
+        sup.sup_project_simultaneous(H, x, 2.5, 1)
+    assert e.value.status == 1
+    with pytest.raises(sup.SupError):
+        sup.sup_superiorize(H, x, 3, 2, 1.0, 1.0, objective="tv2d", shape=P.shape)  # a not in (0,1)
+    with pytest.raises(sup.SupError):
+        sup.sup_superiorize(H, x, 3, 2, 1.0, 0.9, objective="tv2d", shape=(5, 5))  # shape does not match n
+    with pytest.raises(sup.SupError) as e:
+        sup.sup_block_iterative(H, x, 1.0, 1)  # no blocks set
+    assert e.value.status == 5
+    with pytest.raises(sup.SupError) as e:
+        sup.sup_perturb_dose(H, x, 1, 1.0, 0.9, 0)  # no dose matrix
+    assert e.value.status == 5
+    bad_col = P.col.copy()
+    bad_col[3] = P.n + 7
+    with pytest.raises(sup.SupError) as e:
+        sup.sup_create(P.rowptr, bad_col, P.val, P.lb, P.ub, P.lo, P.hi, None, dtype=0, n=P.n)
+    assert e.value.status == 2
+    with pytest.raises(sup.SupError) as e:
+        sup.sup_create(P.rowptr, P.col, P.val, P.ub + 1, P.ub, P.lo, P.hi, None, dtype=0, n=P.n)  # lb > ub
+    assert e.value.status == 2
+    w = np.ones(P.m, np.float32)
+    w[5] = 0.0
+    with pytest.raises(sup.SupError) as e:
+        sup.sup_create(P.rowptr, P.col, P.val, P.lb, P.ub, P.lo, P.hi, w, dtype=0, n=P.n)  # weight <= 0
+    assert e.value.status == 2
