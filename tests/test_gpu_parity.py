@@ -264,7 +264,7 @@ def test_perturbation_phase(name, kind, dtype):
         xo = R["x"]
         assert ell_g == R["ell"], (phase, ell_g, R["ell"], R["margins"].min())
         assert st["n_trials"] == R["trials"]
-        assert rel_l2(x.cpu().numpy(), xo) <= (1e-6 if dtype == 0 else 1e-13)
+        assert rel_l2(x.cpu().numpy(), xo) <= (1e-5 if dtype == 0 else 1e-13)  # fp32 storage of x and g per step
         assert close_scalar(st["f"], R["fx"], 1e-5 if dtype == 0 else 1e-12)
         ell = ell_g
 
