@@ -22,9 +22,10 @@ PER_TRIAL, PER_SWEEP = 0, 1
 
 
 def build(force: bool = False) -> str:
-    """gcc -O2 (no -ffast-math, no OpenMP: the oracle is single-threaded scalar code)."""
+    """gcc -O2 -ffp-contract=off (no -ffast-math, no FMA contraction, no OpenMP: single-threaded scalar code;
+    reductions use binary128 accumulators from libgcc's soft-float, see sup_oracle.c)."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        subprocess.check_call(["gcc", "-O2", "-shared", "-fPIC", "-o", _LIB, _SRC, "-lm"])
+        subprocess.check_call(["gcc", "-O2", "-ffp-contract=off", "-shared", "-fPIC", "-o", _LIB, _SRC, "-lm"])
     return _LIB
 
 
@@ -88,20 +89,18 @@ class Oracle:
     # ---- feasibility-seeking --------------------------------------------------------------
     def sweep(self, x, lam=1.0, n_sweeps=1):
         x = np.array(x, np.float64)
-        u = np.empty(self.n)
         for _ in range(n_sweeps):
             _L().orc_sweep(_i64(self.m), _i64(self.n), _p(self.rowptr), _p(self.col), _p(self.val), _p(self.lb),
-                           _p(self.ub), _p(self.d), _p(self.lo), _p(self.hi), _dbl(lam), _p(x), _p(u))
+                           _p(self.ub), _p(self.d), _p(self.lo), _p(self.hi), _dbl(lam), _p(x))
         return x
 
     def block_sweep(self, x, lam=1.0, n_sweeps=1, block_rowptr=None):
         br = self.block_rowptr if block_rowptr is None else np.ascontiguousarray(block_rowptr, np.int64)
         x = np.array(x, np.float64)
-        u = np.empty(self.n)
         for _ in range(n_sweeps):
             _L().orc_block_sweep(_i64(self.m), _i64(self.n), _p(self.rowptr), _p(self.col), _p(self.val), _p(self.lb),
                                  _p(self.ub), _p(self.w), _p(self.d), _p(self.lo), _p(self.hi), _dbl(lam),
-                                 _int(br.size - 1), _p(br), _p(x), _p(u))
+                                 _int(br.size - 1), _p(br), _p(x))
         return x
 
     def proximity(self, x, mode=0, p=2.0):

@@ -5,9 +5,15 @@
  * cpu_baseline / --impl reference legs may call it.  It shares no code with the CUDA path
  * (paper_2606_27086_b200/csrc) and is written from the paper alone:
  *   /root/reference/PAPER.md = arXiv 2606.27086 (SupPy), cited as PAPER.md:L<line>.
- * Scalar loops, CSR traversed in storage order, back-projection as a scatter (no transposed matrix),
- * plain left-to-right fp64 sums.  Readings of the paper where it is silent/garbled are listed in
- * DESIGN.md ("Readings", A-1 .. A-22) and named at the line that uses them.
+ * Scalar loops, CSR traversed in storage order, back-projection as a scatter (no transposed matrix).
+ * Every value is an fp64 number and every elementwise operation is one IEEE-754 fp64 operation (built with
+ * -ffp-contract=off: no fused multiply-add).  Every REDUCTION (row dot product, back-projected sum, ||a_i||^2,
+ * weight sums, objective sums, ||g||^2) is accumulated in binary128 (acc_t) and rounded once to fp64: a product
+ * of two fp64 numbers is exact in binary128, so the result is the correctly rounded fp64 value of the sum and
+ * does not depend on summation order (reading A-22: the perturbed iteration amplifies last-bit
+ * differences by orders of magnitude per sweep, so "the sum" has to be one well-defined number).
+ * Readings of the paper where it is silent/garbled are listed in DESIGN.md ("Readings", A-1 .. A-22) and
+ * named at the line that uses them.
  *
  * Parity pins (tests/test_oracle_*.py): every function below is pinned by closed forms, invariants,
  * library special cases or brute force; nothing here is "parity unpinned".
@@ -16,6 +22,8 @@
 #include <stdint.h>
 #include <stdlib.h>
 #include <string.h>
+
+typedef __float128 acc_t; /* accumulator of every reduction (A-22) */
 
 typedef struct {
     int64_t m, n;
@@ -30,16 +38,18 @@ typedef struct {
 int orc_setup(int64_t m, const int64_t* rowptr, const int32_t* col, const double* val, const double* w_in,
               double* w, double* rho, double* d) {
     (void)col;
-    double sw = 0.0;
+    acc_t sw_acc = 0;
     for (int64_t i = 0; i < m; ++i) {
         double wi = w_in ? w_in[i] : 1.0;
         if (!(wi > 0.0)) return 1;
-        sw += wi;
+        sw_acc += wi;
     }
+    const double sw = (double)sw_acc;
     for (int64_t i = 0; i < m; ++i) {
         w[i] = (w_in ? w_in[i] : 1.0) / sw;
-        double r = 0.0;
-        for (int64_t k = rowptr[i]; k < rowptr[i + 1]; ++k) r += val[k] * val[k]; /* ||a^i||^2 */
+        acc_t r_acc = 0;
+        for (int64_t k = rowptr[i]; k < rowptr[i + 1]; ++k) r_acc += (acc_t)val[k] * val[k]; /* ||a^i||^2 */
+        const double r = (double)r_acc;
         rho[i] = r;
         d[i] = r > 0.0 ? w[i] / r : 0.0;
     }
@@ -54,24 +64,30 @@ static double violation(double r, double lb, double ub) {
     return 0.0;
 }
 
+/* <a^i, x>: the products are exact in binary128, the sum is rounded once to fp64 (A-22) */
+static double row_dot(const int64_t* rowptr, const int32_t* col, const double* val, int64_t i, const double* x) {
+    acc_t r = 0;
+    for (int64_t k = rowptr[i]; k < rowptr[i + 1]; ++k) r += (acc_t)val[k] * x[col[k]];
+    return (double)r;
+}
+
 /* ---- O-SWEEP on rows [r0, r1): x <- P_box(x - lambda * A^T D c(x)).
  * A-1: T(x) = x + lambda * sum_i w_i (P_{C_i}(x) - x)  (Eq. 2, 3 and the weights of Eq. 5 / Table A.5's D).
  * A-2: the box is applied after the relaxed step, un-relaxed.
  * dscale multiplies d_i (1 for the simultaneous sweep; 1/W_t for block t, A-14).  u is scratch [n]. */
 static void sweep_rows(const csr_t* A, int64_t r0, int64_t r1, const double* lb, const double* ub, const double* d,
-                       double dscale, const double* lo, const double* hi, double lambda, double* x, double* u) {
-    for (int64_t j = 0; j < A->n; ++j) u[j] = 0.0;
+                       double dscale, const double* lo, const double* hi, double lambda, double* x, acc_t* u) {
+    for (int64_t j = 0; j < A->n; ++j) u[j] = 0;
     for (int64_t i = r0; i < r1; ++i) {
-        double r = 0.0;
-        for (int64_t k = A->rowptr[i]; k < A->rowptr[i + 1]; ++k) r += A->val[k] * x[A->col[k]]; /* <a^i, x>, L41 */
+        const double r = row_dot(A->rowptr, A->col, A->val, i, x); /* <a^i, x>, L41 */
         double c = violation(r, lb[i], ub[i]);
         if (c != 0.0) {
             double y = (d[i] * dscale) * c;
-            for (int64_t k = A->rowptr[i]; k < A->rowptr[i + 1]; ++k) u[A->col[k]] += A->val[k] * y;
+            for (int64_t k = A->rowptr[i]; k < A->rowptr[i + 1]; ++k) u[A->col[k]] += (acc_t)A->val[k] * y;
         }
     }
     for (int64_t j = 0; j < A->n; ++j) {
-        double t = x[j] - lambda * u[j]; /* Eq. 3 (L46) */
+        double t = x[j] - lambda * (double)u[j]; /* Eq. 3 (L46) */
         if (t < lo[j]) t = lo[j];        /* BoxProjection, L427 */
         if (t > hi[j]) t = hi[j];
         x[j] = t;
@@ -79,10 +95,11 @@ static void sweep_rows(const csr_t* A, int64_t r0, int64_t r1, const double* lb,
 }
 
 void orc_sweep(int64_t m, int64_t n, const int64_t* rowptr, const int32_t* col, const double* val, const double* lb,
-               const double* ub, const double* d, const double* lo, const double* hi, double lambda, double* x,
-               double* u) {
+               const double* ub, const double* d, const double* lo, const double* hi, double lambda, double* x) {
     csr_t A = {m, n, rowptr, col, val};
+    acc_t* u = (acc_t*)malloc(sizeof(acc_t) * (size_t)n);
     sweep_rows(&A, 0, m, lb, ub, d, 1.0, lo, hi, lambda, x, u);
+    free(u);
 }
 
 /* ---- O-BLOCK-SWEEP (block-iterative family; A-14): blocks of contiguous rows visited in
@@ -90,15 +107,17 @@ void orc_sweep(int64_t m, int64_t n, const int64_t* rowptr, const int32_t* col, 
  * box after every block. */
 void orc_block_sweep(int64_t m, int64_t n, const int64_t* rowptr, const int32_t* col, const double* val,
                      const double* lb, const double* ub, const double* w, const double* d, const double* lo,
-                     const double* hi, double lambda, int n_blocks, const int64_t* block_rowptr, double* x,
-                     double* u) {
+                     const double* hi, double lambda, int n_blocks, const int64_t* block_rowptr, double* x) {
     csr_t A = {m, n, rowptr, col, val};
+    acc_t* u = (acc_t*)malloc(sizeof(acc_t) * (size_t)n);
     for (int t = 0; t < n_blocks; ++t) {
-        double W = 0.0;
-        for (int64_t i = block_rowptr[t]; i < block_rowptr[t + 1]; ++i) W += w[i];
+        acc_t W_acc = 0;
+        for (int64_t i = block_rowptr[t]; i < block_rowptr[t + 1]; ++i) W_acc += w[i];
+        const double W = (double)W_acc;
         if (!(W > 0.0)) continue;
         sweep_rows(&A, block_rowptr[t], block_rowptr[t + 1], lb, ub, d, 1.0 / W, lo, hi, lambda, x, u);
     }
+    free(u);
 }
 
 /* ---- O-PROX.  delta_i = |c_i| / ||a^i|| = Euclidean distance to C_i (0 for empty rows, A-4/A-5).
@@ -106,33 +125,36 @@ void orc_block_sweep(int64_t m, int64_t n, const int64_t* rowptr, const int32_t*
  * mode 2: max_i delta_i (Eq. 13). */
 double orc_proximity(int64_t m, const int64_t* rowptr, const int32_t* col, const double* val, const double* lb,
                      const double* ub, const double* w, const double* rho, const double* x, int mode, double p) {
-    double acc = 0.0;
+    acc_t acc = 0;
+    double mx = 0.0;
     for (int64_t i = 0; i < m; ++i) {
-        double r = 0.0;
-        for (int64_t k = rowptr[i]; k < rowptr[i + 1]; ++k) r += val[k] * x[col[k]];
+        const double r = row_dot(rowptr, col, val, i, x);
         double c = violation(r, lb[i], ub[i]);
         double delta = rho[i] > 0.0 ? fabs(c) / sqrt(rho[i]) : 0.0;
-        if (mode == 0) acc += w[i] * delta * delta;
+        if (mode == 0) acc += (w[i] * delta) * delta;
         else if (mode == 1) acc += w[i] * pow(delta, p);
-        else if (delta > acc) acc = delta;
+        else if (delta > mx) mx = delta;
     }
-    return mode == 0 ? 0.5 * acc : acc;
+    if (mode == 2) return mx;
+    return mode == 0 ? 0.5 * (double)acc : (double)acc;
 }
 
 /* ---- objectives ---------------------------------------------------------------------------------- */
 /* TV2D, Eq. 15 on an ny x nx row-major image X[i*nx+j]: terms only for i < ny-1, j < nx-1. */
 double orc_tv2d(const double* X, int64_t ny, int64_t nx) {
-    double s = 0.0;
+    acc_t s = 0;
     for (int64_t i = 0; i + 1 < ny; ++i)
         for (int64_t j = 0; j + 1 < nx; ++j) {
             double dx = X[(i + 1) * nx + j] - X[i * nx + j];
             double dy = X[i * nx + j + 1] - X[i * nx + j];
             s += sqrt(dx * dx + dy * dy);
         }
-    return s;
+    return (double)s;
 }
 
-/* Gradient of Eq. 15 as printed, term by term (A-8); a term with t = 0 contributes 0 (A-9). */
+/* Gradient of Eq. 15 as printed, term by term (A-8); a term with t = 0 contributes 0 (A-9).  A pixel receives at most
+ * three contributions, in the order of this loop: +dx/t of term (i-1,j), +dy/t of term (i,j-1), -(dx+dy)/t of its own
+ * term (i,j): g_ij = ((0 + a) + b) - c in fp64. */
 void orc_tv2d_grad(const double* X, int64_t ny, int64_t nx, double* g) {
     for (int64_t q = 0; q < ny * nx; ++q) g[q] = 0.0;
     for (int64_t i = 0; i + 1 < ny; ++i)
@@ -150,9 +172,9 @@ void orc_tv2d_grad(const double* X, int64_t ny, int64_t nx, double* g) {
 
 /* TV1D (A-16): f = sum_{i<n-1} |x_{i+1} - x_i|, subgradient with sgn(0) = 0. */
 double orc_tv1d(const double* x, int64_t n) {
-    double s = 0.0;
+    acc_t s = 0;
     for (int64_t i = 0; i + 1 < n; ++i) s += fabs(x[i + 1] - x[i]);
-    return s;
+    return (double)s;
 }
 void orc_tv1d_grad(const double* x, int64_t n, double* g) {
     for (int64_t i = 0; i < n; ++i) g[i] = 0.0;
@@ -166,22 +188,23 @@ void orc_tv1d_grad(const double* x, int64_t n, double* g) {
 
 /* DOSE (A-15): f = ||D x||^2, g = 2 D^T (D x); D is md x n CSR. */
 double orc_dose(int64_t md, const int64_t* rowptr, const int32_t* col, const double* val, const double* x) {
-    double s = 0.0;
+    acc_t s = 0;
     for (int64_t i = 0; i < md; ++i) {
-        double r = 0.0;
-        for (int64_t k = rowptr[i]; k < rowptr[i + 1]; ++k) r += val[k] * x[col[k]];
-        s += r * r;
+        const double r = row_dot(rowptr, col, val, i, x);
+        s += (acc_t)r * r;
     }
-    return s;
+    return (double)s;
 }
 void orc_dose_grad(int64_t md, int64_t n, const int64_t* rowptr, const int32_t* col, const double* val,
                    const double* x, double* g) {
-    for (int64_t j = 0; j < n; ++j) g[j] = 0.0;
+    acc_t* u = (acc_t*)malloc(sizeof(acc_t) * (size_t)n); /* u = D^T (D x) */
+    for (int64_t j = 0; j < n; ++j) u[j] = 0;
     for (int64_t i = 0; i < md; ++i) {
-        double r = 0.0;
-        for (int64_t k = rowptr[i]; k < rowptr[i + 1]; ++k) r += val[k] * x[col[k]];
-        for (int64_t k = rowptr[i]; k < rowptr[i + 1]; ++k) g[col[k]] += 2.0 * val[k] * r;
+        const double r = row_dot(rowptr, col, val, i, x);
+        for (int64_t k = rowptr[i]; k < rowptr[i + 1]; ++k) u[col[k]] += (acc_t)val[k] * r;
     }
+    for (int64_t j = 0; j < n; ++j) g[j] = 2.0 * (double)u[j];
+    free(u);
 }
 
 /* objective descriptor: kind 0 = none (f = 0, g = 0), 1 = TV2D (ny, nx), 2 = TV1D, 3 = DOSE */
@@ -214,7 +237,8 @@ static void obj_grad(const obj_t* O, int64_t n, const double* x, double* g) {
 /* ---- O-PERTURB: the perturbation phase, Algorithm 1 lines 4-17.
  *  fx <- f(x); for n = 0..N-1: g <- grad f(x^{k,n}) (A-7: recomputed at every reduction step);
  *  v <- -g/||g|| (A-6: minus sign per L84/L93; v = 0 if ||g|| = 0);
- *  trial loop: beta <- beta0 * a^l (A-10, A-20: pow in fp64), z <- x + beta v, l <- l+1,
+ *  trial loop: beta <- beta0 * a^l (A-10; A-20: a^l is the running fp64 product a_pow(l), not libm pow),
+ *  z <- x + beta v, l <- l+1,
  *  accept iff f(z) <= f(x^{k,n}) (L149, A-11).  J_max trials per step (A-12).
  *  policy 0 = PER_TRIAL: one persistent counter *ell, incremented on every trial, never reset.
  *  policy 1 = PER_SWEEP: beta_{k,j} = beta0 * a^{k+j}, j reset to 0 at every reduction step (literal Alg. 1).
@@ -222,6 +246,13 @@ static void obj_grad(const obj_t* O, int64_t n, const double* x, double* g) {
  *  forced: optional replay of a decision sequence (A-13 trace-replay); NULL = decide by the test.
  *  margins: optional per-trial |fz-fx|/max(1,|fx|).  Returns number of trials; *warn |= 1 if J_max hit. */
 #define J_MAX 10000
+/* a^e by e successive fp64 multiplications starting from 1 (A-20): every implementation of IEEE-754 gets the same
+ * bits, which libm pow() does not promise. */
+static double a_pow(double a, int64_t e) {
+    double p = 1.0;
+    for (int64_t q = 0; q < e; ++q) p *= a;
+    return p;
+}
 int64_t orc_perturb(int64_t n, const obj_t* O, double* x, int64_t* ell, int64_t k, int N, double beta0, double a,
                     int policy, double* g, double* z, int8_t* decisions, double* margins, int64_t cap_dec,
                     int64_t* n_dec, const int8_t* forced, int* warn, double* fx_out) {
@@ -229,14 +260,15 @@ int64_t orc_perturb(int64_t n, const obj_t* O, double* x, int64_t* ell, int64_t 
     int64_t trials = 0;
     for (int nred = 0; nred < N; ++nred) {
         obj_grad(O, n, x, g);
-        double s = 0.0;
-        for (int64_t j = 0; j < n; ++j) s += g[j] * g[j];
-        s = sqrt(s);
+        acc_t s_acc = 0;
+        for (int64_t j = 0; j < n; ++j) s_acc += (acc_t)g[j] * g[j];
+        const double s = sqrt((double)s_acc);
         int64_t jloc = 0;
         int accepted = 0;
+        double apow = a_pow(a, policy == 0 ? *ell : k); /* a^l resp. a^(k+0) */
         for (int trial = 0; trial < J_MAX && !accepted; ++trial) {
-            double expo = policy == 0 ? (double)(*ell) : (double)(k + jloc);
-            double beta = beta0 * pow(a, expo);
+            double beta = beta0 * apow;
+            apow *= a;
             for (int64_t j = 0; j < n; ++j) z[j] = s > 0.0 ? x[j] + beta * (-g[j] / s) : x[j];
             (*ell)++;
             jloc++;
@@ -274,7 +306,6 @@ int orc_superiorize(int64_t m, int64_t n, const int64_t* rowptr, const int32_t* 
     obj_t O = {obj_kind, ny, nx, md, d_rowptr, d_col, d_val};
     double* g = (double*)malloc(sizeof(double) * (size_t)n);
     double* z = (double*)malloc(sizeof(double) * (size_t)n);
-    double* u = (double*)malloc(sizeof(double) * (size_t)n);
     int warn = 0;
     for (int it = 0; it < n_iter; ++it) {
         int64_t k = k0 + it;
@@ -283,9 +314,9 @@ int orc_superiorize(int64_t m, int64_t n, const int64_t* rowptr, const int32_t* 
             trials = orc_perturb(n, &O, x, ell, k, N, beta0, a, policy, g, z, decisions, margins, cap_dec, n_dec,
                                  forced, &warn, NULL);
         if (n_blocks > 0)
-            orc_block_sweep(m, n, rowptr, col, val, lb, ub, w, d, lo, hi, lambda, n_blocks, block_rowptr, x, u);
+            orc_block_sweep(m, n, rowptr, col, val, lb, ub, w, d, lo, hi, lambda, n_blocks, block_rowptr, x);
         else
-            orc_sweep(m, n, rowptr, col, val, lb, ub, d, lo, hi, lambda, x, u);
+            orc_sweep(m, n, rowptr, col, val, lb, ub, d, lo, hi, lambda, x);
         if (trace) {
             trace[4 * it + 0] = orc_proximity(m, rowptr, col, val, lb, ub, w, rho, x, 0, 2.0);
             trace[4 * it + 1] = obj_value(&O, n, x);
@@ -295,7 +326,6 @@ int orc_superiorize(int64_t m, int64_t n, const int64_t* rowptr, const int32_t* 
     }
     free(g);
     free(z);
-    free(u);
     return warn;
 }
 
