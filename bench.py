@@ -43,6 +43,9 @@ def make_problem(name):
 
     if name == "cfg3":
         return gen.config3_lowdose_ct()
+    if name.startswith("ct:"):  # ct:<n_pix>:<n_angles>:<n_bins> -- same recipe as cfg3 at another size (experiments)
+        _, npx, na, nbn = name.split(":")
+        return gen.config3_lowdose_ct(n_pix=int(npx), n_angles=int(na), n_bins=int(nbn))
     if name == "cfg1":
         return gen.config1_tiny_ct()
     if name == "cfg2":
@@ -275,7 +278,7 @@ def run_ours(args, rank, world, local_rank):
         except Exception:
             pass
 
-    cpu_v, cpu_done, cpu_el = time_oracle(P, args.cpu_budget)
+    cpu_v, cpu_done, cpu_el = time_oracle(P, args.cpu_budget) if args.cpu_budget > 0 else (None, 0, 0.0)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",

@@ -2,6 +2,7 @@
 // (O-SWEEP, O-BLOCK-SWEEP, O-SUPERIORIZE of DESIGN.md) and CUDA-graph capture of one superiorized sweep (S8).
 #include <math.h>
 #include <stddef.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <new>
@@ -28,12 +29,15 @@ extern "C" sup_status sup_workspace_bytes(int kind, int64_t m, int64_t n, int64_
                 + al(size_t(m) * esz)                                                // d
                 + 2 * al(size_t(m) * 8)                                              // w, 1/||a||
                 + al(size_t(m) * esz) + 2 * al(size_t(n) * esz)                      // y, g, xdev
-                + al(2 * SUP_MAX_PARTIALS * 8) + al(sizeof(DevState)) + 1024;
+                + al(2 * SUP_MAX_PARTIALS * 8) + al(sizeof(DevState)) + 2 * sup_stream_table_bytes()
+                + al(size_t(nnz) * 4) + al(size_t((n + 511) & ~int64_t(511)) * esz)             // colg, xg
+                + 1024;
             s = sup_transpose_scratch_bytes(nnz, n, esz) + 4096;
             break;
         case SUP_WS_BLOCKS:
             if (n_blocks < 1) return sup_fail(nullptr, SUP_ERR_INVALID_ARG, "sup_workspace_bytes: n_blocks < 1");
-            p = size_t(n_blocks) * al(size_t(n + 1) * 8) + al(size_t(nnz) * 4) + al(size_t(nnz) * esz) + al(size_t(m) * esz) + 1024;
+            p = size_t(n_blocks) * al(size_t(n + 1) * 8) + al(size_t(nnz) * 4) + al(size_t(nnz) * esz) + al(size_t(m) * esz) +
+                2 * size_t(n_blocks) * sup_stream_table_bytes() + 1024;
             s = sup_transpose_scratch_bytes(nnz, n, esz) + al(size_t(n_blocks) * 8) + 4096;
             break;
         case SUP_WS_DOSE:  // (m, n, nnz) describe D_body
@@ -104,6 +108,15 @@ extern "C" sup_status sup_create(sup_handle* out, const sup_csr* A, const void* 
     h->xdev = B.take(size_t(h->n) * h->esz);
     h->partials = static_cast<double*>(B.take(2 * SUP_MAX_PARTIALS * 8));
     h->state = static_cast<DevState*>(B.take(sizeof(DevState)));
+    void* tab_a = B.take(sup_stream_table_bytes());
+    void* tab_at = B.take(sup_stream_table_bytes());
+    h->colg = static_cast<int32_t*>(B.take(size_t(h->nnz) * 4));
+    h->xg = B.take(size_t((h->n + 511) & ~int64_t(511)) * h->esz);
+    {
+        const char* env = getenv("SUP_NO_STREAM");
+        h->use_stream = !(env && env[0] == '1');
+    }
+    h->A.alloc_nnz = h->nnz;
     sup_status rc = SUP_OK;
     if (!B.ok) rc = sup_fail(h, SUP_ERR_WORKSPACE, "sup_create: workspace too small");
     if (rc == SUP_OK && cudaMemsetAsync(h->state, 0, sizeof(DevState), h->stream) != cudaSuccess)
@@ -124,6 +137,17 @@ extern "C" sup_status sup_create(sup_handle* out, const sup_csr* A, const void* 
     h->AT.rowptr = at_rowptr;
     h->AT.col = at_col;
     h->AT.val = at_val;
+    h->AT.alloc_nnz = h->nnz;
+    rc = sup_stream_plan(h, h->A, 0, h->m, sup_stream_chunks(true), tab_a, scratch, &h->A.plan);
+    if (rc == SUP_OK && h->use_stream) rc = sup_stream_setup_gather(h);
+    if (rc == SUP_OK && cudaMemsetAsync(h->xg, 0, size_t((h->n + 511) & ~int64_t(511)) * h->esz, h->stream) != cudaSuccess)
+        rc = sup_fail(h, SUP_ERR_CUDA, "sup_create: %s", cudaGetErrorString(cudaGetLastError()));
+    if (rc == SUP_OK) rc = sup_stream_plan(h, h->AT, 0, h->n, sup_stream_chunks(false), tab_at, scratch, &h->AT.plan);
+    if (rc != SUP_OK) {
+        memcpy(g_create_error, h->err, sizeof(g_create_error));
+        delete h;
+        return rc;
+    }
     *out = h;
     return SUP_OK;
 }
@@ -168,6 +192,7 @@ extern "C" sup_status sup_set_blocks(sup_handle h, int n_blocks, const int64_t* 
     h->d_blk = B.take(size_t(h->m) * h->esz);
     h->ATb.assign(n_blocks, CsrD());
     h->g_bwd_blk.assign(n_blocks, 32);
+    h->stream_fwd_blk.assign(n_blocks, StreamPlan());
     h->block_rowptr.assign(block_rowptr, block_rowptr + n_blocks + 1);
     for (int t = 0; t < n_blocks; ++t) {
         int64_t* rowptr_t = static_cast<int64_t*>(B.take(size_t(h->n + 1) * 8));
@@ -182,7 +207,14 @@ extern "C" sup_status sup_set_blocks(sup_handle h, int n_blocks, const int64_t* 
         T.rowptr = rowptr_t;
         T.col = col;
         T.val = val;
+        T.alloc_nnz = h->nnz;
         h->g_bwd_blk[t] = sup_pick_group(T.nnz, h->n);
+        void* tab_f = B.take(sup_stream_table_bytes());
+        void* tab_b = B.take(sup_stream_table_bytes());
+        if (!B.ok) return sup_fail(h, SUP_ERR_WORKSPACE, "sup_set_blocks: workspace too small");
+        rc = sup_stream_plan(h, h->A, block_rowptr[t], block_rowptr[t + 1], sup_stream_chunks(true), tab_f, scratch, &h->stream_fwd_blk[t]);
+        if (rc == SUP_OK) rc = sup_stream_plan(h, T, 0, h->n, sup_stream_chunks(false), tab_b, scratch, &T.plan);
+        if (rc != SUP_OK) return rc;
     }
     h->n_blocks = n_blocks;
     sup_status rc = sup_setup_block_scaling(h, scratch, scratch_bytes);
@@ -235,13 +267,13 @@ extern "C" sup_status sup_set_dose_matrix(sup_handle h, const sup_csr* D, void* 
 
 // ---- sweeps ----------------------------------------------------------------------------------------------------
 static void enqueue_simultaneous(sup_ctx* h, void* x, double lambda) {
-    sup_launch_fwd(h, x, 0, h->m, h->d);
+    sup_launch_fwd(h, x, 0, h->m, h->d, &h->A.plan);
     sup_launch_bwd(h, h->AT, h->g_bwd, x, lambda);
 }
 static void enqueue_block_sweep(sup_ctx* h, void* x, double lambda) {
     for (int t = 0; t < h->n_blocks; ++t) {
         if (h->block_rowptr[t + 1] == h->block_rowptr[t]) continue;
-        sup_launch_fwd(h, x, h->block_rowptr[t], h->block_rowptr[t + 1], h->d_blk);
+        sup_launch_fwd(h, x, h->block_rowptr[t], h->block_rowptr[t + 1], h->d_blk, &h->stream_fwd_blk[t]);
         sup_launch_bwd(h, h->ATb[t], h->g_bwd_blk[t], x, lambda);
     }
 }
@@ -255,6 +287,7 @@ extern "C" sup_status sup_project_simultaneous(sup_handle h, void* x, double lam
     if (!h) return SUP_ERR_INVALID_ARG;
     if (!x || n_sweeps < 0) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_project_simultaneous: NULL x or n_sweeps < 0");
     if (check_lambda(h, lambda) != SUP_OK) return SUP_ERR_INVALID_ARG;
+    h->xg_synced = false;  // x comes from the caller
     for (int s = 0; s < n_sweeps; ++s) enqueue_simultaneous(h, x, lambda);
     SUP_CUDA(h, cudaGetLastError());
     return SUP_OK;
@@ -263,7 +296,8 @@ extern "C" sup_status sup_project_simultaneous(sup_handle h, void* x, double lam
 extern "C" sup_status sup_forward_violation(sup_handle h, const void* x) {
     if (!h) return SUP_ERR_INVALID_ARG;
     if (!x) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_forward_violation: NULL x");
-    sup_launch_fwd(h, x, 0, h->m, h->d);
+    h->xg_synced = false;
+    sup_launch_fwd(h, x, 0, h->m, h->d, &h->A.plan);
     SUP_CUDA(h, cudaGetLastError());
     return SUP_OK;
 }
@@ -282,6 +316,7 @@ extern "C" sup_status sup_block_iterative(sup_handle h, void* x, double lambda, 
     if (!x || n_sweeps < 0) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_block_iterative: NULL x or n_sweeps < 0");
     if (h->n_blocks < 1) return sup_fail(h, SUP_ERR_STATE, "sup_block_iterative: call sup_set_blocks first");
     if (check_lambda(h, lambda) != SUP_OK) return SUP_ERR_INVALID_ARG;
+    h->xg_synced = false;
     for (int s = 0; s < n_sweeps; ++s) enqueue_block_sweep(h, x, lambda);
     SUP_CUDA(h, cudaGetLastError());
     return SUP_OK;
@@ -384,6 +419,7 @@ static sup_status enqueue_superiorized_sweep(sup_ctx* h, const RunPlan& P) {
                             P.o.decisions_cap};
         sup_status rc = sup_launch_perturb(h, P.x, pp);
         if (rc != SUP_OK) return rc;
+        h->xg_synced = false;  // the perturbation moved x
     }
     if (P.o.block_iterative) enqueue_block_sweep(h, P.x, P.o.lambda);
     else enqueue_simultaneous(h, P.x, P.o.lambda);
@@ -414,6 +450,7 @@ static sup_status run_superiorize(sup_ctx* h, void* x, int n_iter, int N, double
     sup_status rc = check_objective(h, opt->objective, opt->shape, &P.ny, &P.nx);
     if (rc != SUP_OK) return rc;
     sup_launch_begin_run(h, opt->ell0, opt->k0);
+    h->xg_synced = false;
 
     bool graph = opt->use_graph && h->stream != nullptr && !h->graph_failed && n_iter > 1;
     if (graph) {
@@ -531,6 +568,7 @@ extern "C" sup_status sup_get_derived(sup_handle h, int which, void* dst, size_t
         case 1: src = h->AT.rowptr; bytes = size_t(h->n + 1) * 8; break;
         case 2: src = h->AT.col; bytes = size_t(h->nnz) * 4; break;
         case 3: src = h->AT.val; bytes = size_t(h->nnz) * h->esz; break;
+        case 4: src = h->partials; bytes = 2 * SUP_MAX_PARTIALS * 8; break;  // debug: per-chunk clocks (SUP_DEBUG_CHUNKS=1)
         default: return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_get_derived: unknown array");
     }
     if (!dst || dst_bytes < bytes) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_get_derived: dst too small (%zu needed)", bytes);

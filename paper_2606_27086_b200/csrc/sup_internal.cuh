@@ -13,11 +13,25 @@
 #define SUP_MAX_PARTIALS 2048    // upper bound on the grid of any kernel that feeds a two-stage reduction
 #define SUP_J_MAX 10000          // trials per reduction step (A-12)
 
+// Plan of the bulk-copy-staged SpMV (sup_stream.cu) for one row range of one matrix: persistent CTA b owns rows
+// [part[b], part[b+1]) -- contiguous, balanced by nonzeros.  ok = false: the range does not qualify (a row too
+// long for the ring, misaligned arrays) and the group-per-row kernels of sup_spmv.cu are used instead.
+#define SUP_STREAM_NBMAX 4096  // upper bound on the persistent grid
+struct StreamPlan {
+    const int64_t* part = nullptr;  // device, [nb + 1]
+    int nb = 0;
+    int G = 32;        // lanes per row
+    bool ok = false;
+    int64_t max_row = 0;
+};
+
 struct CsrD {  // device CSR (borrowed or living in workspace)
     int64_t rows = 0, cols = 0, nnz = 0;
     const int64_t* rowptr = nullptr;
     const int32_t* col = nullptr;
     const void* val = nullptr;
+    int64_t alloc_nnz = 0;  // length of the col/val arrays (>= nnz; per-block transposes share one pair of arrays)
+    StreamPlan plan;  // plan for all rows
 };
 
 // device-resident run state; one per handle
@@ -66,11 +80,18 @@ struct sup_ctx {
     double* partials = nullptr; // [2][SUP_MAX_PARTIALS]
     DevState* state = nullptr;
     int g_fwd = 32, g_bwd = 32; // lanes per row of the two products
+    // De-aliased mirror of x for the forward gathers (sup_stream.cu): xg[sup_swz(j)] = x[j], colg = sup_swz(A.col).
+    int32_t* colg = nullptr;    // [nnz]
+    void* xg = nullptr;         // [n rounded up to 512] dtype
+    bool xg_synced = false;     // enqueue-time flag: xg mirrors x (set by the back-projection, cleared when x changes elsewhere)
+    int stream_nb = 0;          // persistent grid of the row-stream kernels (-1: unavailable)
+    bool use_stream = true;       // SUP_NO_STREAM=1 in the environment turns the row-stream kernels off (A/B measurements)
     // block-iterative
     int n_blocks = 0;
     std::vector<int64_t> block_rowptr;
     std::vector<CsrD> ATb;
     std::vector<int> g_bwd_blk;
+    std::vector<StreamPlan> stream_fwd_blk;  // forward product restricted to block t's rows of A
     void* d_blk = nullptr;      // [m] dtype: (w_i/W_t)/||a_i||^2
     // dose objective
     bool has_dose = false;
@@ -109,6 +130,13 @@ extern char g_create_error[512];
             return sup_fail((h), SUP_ERR_CUDA, "%s:%d %s: %s", __FILE__, __LINE__, #call, cudaGetErrorString(e__)); \
     } while (0)
 
+// Index swizzle of the forward gathers.  With a power-of-two image pitch (512 floats = 2 KB) the x entries a
+// near-vertical ray gathers all have the same address modulo 128 B, i.e. sit in the same L1 data bank: measured, the
+// chunks of the forward product at those angles run 1.6x slower than the median at pitch 512, 1.2x at 528, 1.08x at 520
+// (profiles/r01c_staged.md).  XOR-ing the five bank bits of the index with a fold of the upper bits is a bijection
+// inside every 128-byte line (sector membership is preserved too), and puts vertically adjacent pixels in different banks.
+__host__ __device__ static inline int sup_swz(int j) { return j ^ (((j >> 9) ^ (j >> 14)) & 31); }
+
 static inline int sup_pick_group(int64_t nnz, int64_t rows) {
     // lanes cooperating on one row: about a quarter of the mean row length, a power of two in [4, 32]
     double avg = rows > 0 ? double(nnz) / double(rows) : 0.0;
@@ -135,9 +163,21 @@ sup_status sup_setup_block_scaling(sup_ctx* h, void* scratch, size_t scratch_byt
 sup_status sup_validate(sup_ctx* h, const CsrD& A, bool check_bounds, void* scratch);
 
 // ---- products (sup_spmv.cu) -------------------------------------------------------------------------------
-void sup_launch_fwd(sup_ctx* h, const void* x, int64_t r0, int64_t r1, const void* dscale);
+void sup_launch_fwd(sup_ctx* h, const void* x, int64_t r0, int64_t r1, const void* dscale, const StreamPlan* rp);
 void sup_launch_bwd(sup_ctx* h, const CsrD& AT, int G, void* x, double lambda);
 void sup_launch_proximity(sup_ctx* h, const void* x, int mode, double p, double* out_dev);
+
+// ---- bulk-copy-staged products (sup_stream.cu) ---------------------------------------------------------------
+size_t sup_stream_table_bytes();  // bytes of one partition table (256-aligned)
+// Plans rows [r0, r1) of M: grid size, partition table (written into `table`, sup_stream_table_bytes() bytes of
+// persistent workspace), lanes per row; chunks_per_cta x resident CTAs chunks; synchronises the stream.  `scratch` needs 256 bytes.
+sup_status sup_stream_plan(sup_ctx* h, const CsrD& M, int64_t r0, int64_t r1, int chunks_per_cta, void* table, void* scratch,
+                           StreamPlan* out);
+int sup_stream_chunks(bool forward);  // chunks per resident CTA for the forward / transposed product
+void sup_launch_stream_fwd(sup_ctx* h, const StreamPlan& rp, const void* x, const void* dscale);
+void sup_launch_stream_bwd(sup_ctx* h, const CsrD& AT, const StreamPlan& rp, void* x, double lambda);
+sup_status sup_stream_setup_gather(sup_ctx* h);  // fills colg from A.col
+bool sup_stream_forward_uses_xg(const sup_ctx* h);
 
 // ---- perturbation (sup_perturb.cu) ------------------------------------------------------------------------
 struct PerturbParams {

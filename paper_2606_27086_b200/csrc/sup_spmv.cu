@@ -58,7 +58,8 @@ __global__ void __launch_bounds__(SUP_THREADS)
 template <typename T>
 __global__ void __launch_bounds__(SUP_THREADS)
     k_bwd(int64_t n, const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col, const T* __restrict__ val,
-          const T* __restrict__ y, const T* __restrict__ lo, const T* __restrict__ hi, T lambda, T* __restrict__ x, int G) {
+          const T* __restrict__ y, const T* __restrict__ lo, const T* __restrict__ hi, T lambda, T* __restrict__ x,
+          T* __restrict__ xg, int G) {
     const int gl = threadIdx.x % G;
     const int64_t j = (int64_t(blockIdx.x) * blockDim.x + threadIdx.x) / G;
     const bool valid = j < n;
@@ -69,13 +70,18 @@ __global__ void __launch_bounds__(SUP_THREADS)
         t = t < lo[j] ? lo[j] : t;  // box, un-relaxed (A-2)
         t = t > hi[j] ? hi[j] : t;
         x[j] = t;
+        if (xg) xg[sup_swz(int(j))] = t;  // de-aliased mirror read by the staged forward product (sup_stream.cu)
     }
 }
 
-void sup_launch_fwd(sup_ctx* h, const void* x, int64_t r0, int64_t r1, const void* dscale) {
+void sup_launch_fwd(sup_ctx* h, const void* x, int64_t r0, int64_t r1, const void* dscale, const StreamPlan* rp) {
     const int G = h->g_fwd;
     const int64_t rows = r1 - r0;
     if (rows <= 0) return;
+    if (rp && rp->ok) {
+        sup_launch_stream_fwd(h, *rp, x, dscale);
+        return;
+    }
     const unsigned grid = unsigned((rows * G + SUP_THREADS - 1) / SUP_THREADS);
     if (h->dt == SUP_F32)
         k_fwd<float><<<grid, SUP_THREADS, 0, h->stream>>>(
@@ -91,15 +97,23 @@ void sup_launch_fwd(sup_ctx* h, const void* x, int64_t r0, int64_t r1, const voi
 }
 
 void sup_launch_bwd(sup_ctx* h, const CsrD& AT, int G, void* x, double lambda) {
+    if (AT.plan.ok) {
+        sup_launch_stream_bwd(h, AT, AT.plan, x, lambda);
+        return;
+    }
     const unsigned grid = unsigned((AT.rows * G + SUP_THREADS - 1) / SUP_THREADS);
+    void* mirror = sup_stream_forward_uses_xg(h) ? h->xg : nullptr;
+    h->xg_synced = mirror != nullptr;
     if (h->dt == SUP_F32)
         k_bwd<float><<<grid, SUP_THREADS, 0, h->stream>>>(
             AT.rows, AT.rowptr, AT.col, static_cast<const float*>(AT.val), static_cast<const float*>(h->y),
-            static_cast<const float*>(h->lo), static_cast<const float*>(h->hi), float(lambda), static_cast<float*>(x), G);
+            static_cast<const float*>(h->lo), static_cast<const float*>(h->hi), float(lambda), static_cast<float*>(x),
+            static_cast<float*>(mirror), G);
     else
         k_bwd<double><<<grid, SUP_THREADS, 0, h->stream>>>(
             AT.rows, AT.rowptr, AT.col, static_cast<const double*>(AT.val), static_cast<const double*>(h->y),
-            static_cast<const double*>(h->lo), static_cast<const double*>(h->hi), lambda, static_cast<double*>(x), G);
+            static_cast<const double*>(h->lo), static_cast<const double*>(h->hi), lambda, static_cast<double*>(x),
+            static_cast<double*>(mirror), G);
     h->launches++;
 }
 

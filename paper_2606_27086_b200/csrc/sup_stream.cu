@@ -1,0 +1,495 @@
+// sup_stream.cu -- S1+S2 and S3 of the hot path as persistent kernels whose val/col stream is
+// staged through shared memory by the bulk-copy engine.
+//
+//   S1+S2  r_i = <a_i, x>, c_i = hyperslab violation (Eq. 2 on each face, L38-42; Eq. 20),
+//          y_i = d_i c_i, d_i = w_i/||a_i||^2 (L608)
+//   S3     u_j = sum_i a_ij y_i over row j of the explicit A^T,  x_j <- clip(x_j - lambda u_j) (Eq. 3; box L427)
+//
+// Why: ncu on the group-per-row kernels (profiles/r01a_spmv_baseline.md) shows DRAM traffic equal to the algorithmic
+// bytes but only 57-60 % of the measured copy bandwidth with nothing saturated; the L1 fills (stream + gather
+// misses, 3.35 GB per launch) all go through the LSU miss path.  Two earlier attempts are recorded in
+// profiles/r01b_ring_negative.md.  This version takes the stream off the LSU path:
+//   * one persistent CTA per SM owns a CONTIGUOUS row range balanced by nonzeros (partition table built at
+//     setup), hence a contiguous range of val[] and col[];
+//   * a producer thread pulls that range through a ring of RG_STAGES tiles (RG_TILE elements each) in shared
+//     memory with cp.async.bulk (L2 evict-first policy) completing on per-stage mbarriers; the ring (128 KB in
+//     fp32) is about twice the span the consumers work on, so ~64 KB per SM are in flight at all times and the
+//     stream never occupies L1, which is left to the x / y gathers;
+//   * a watcher thread waits on the stage barriers in order and publishes the count of completed tiles; the 16
+//     consumer warps take the rows in order (G lanes per row), poll that one counter for the tiles their rows
+//     need, read val/col from the ring (consecutive lanes -> consecutive words), gather x / y through L1
+//     (ld.global.nc), reduce with shuffles and run the fused epilogue.  Each consumer warp publishes how many
+//     tiles lie wholly before its next row; the producer refills a stage when every warp has passed it.
+// The summation order of a row depends only on G, not on the grid: results are deterministic.
+#include <math.h>
+#include <stdlib.h>
+
+#include "sup_internal.cuh"
+
+#define RG_TILE 1024                        // elements per stage
+#define RG_STAGES 16
+#define RG_ELEMS (RG_TILE * RG_STAGES)      // ring capacity in elements (a power of two)
+#define RG_CWARPS 16                        // consumer warps
+#define RG_THREADS (32 * (RG_CWARPS + 2))   // + producer warp + watcher warp
+#ifndef RG_UNROLL
+#define RG_UNROLL 16                        // independent gathers in flight per lane (a multiple of 4)
+#endif
+#define RG_TIMEOUT 8000000000LL             // ~4 s of SM clocks: a protocol bug must fault, not hang the GPU
+
+// ---- PTX wrappers (mbarrier + bulk copy) --------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return static_cast<uint32_t>(__cvta_generic_to_shared(p)); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("{\n .reg .b64 st;\n mbarrier.arrive.shared::cta.b64 st, [%0];\n}" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("{\n .reg .b64 st;\n mbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n}" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    uint32_t ok = 0;
+    long long t0 = 0;
+    for (;;) {
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+        if (ok) return;
+        if (t0 == 0) t0 = clock64();
+        else if (clock64() - t0 > RG_TIMEOUT) __trap();
+    }
+}
+__device__ __forceinline__ uint64_t l2_evict_first_policy() {
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar, uint64_t pol) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar), "l"(pol) : "memory");
+}
+
+template <typename T>
+__device__ __forceinline__ T hyperslab_violation(T r, T lb, T ub) {  // Eq. 2 on each face of lb <= r <= ub
+    return r > ub ? r - ub : (r < lb ? r - lb : T(0));
+}
+
+template <typename T>
+struct RgSmem {
+    T val[RG_ELEMS];
+    int32_t col[RG_ELEMS];
+    unsigned long long full[RG_STAGES];
+    int progress[RG_CWARPS];  // per consumer warp: tiles [0, progress) are no longer needed by it
+    int completed;            // tiles [0, completed) have landed in the ring
+};
+
+// Dot product of the ring elements k, k+G, k+2G, ... < e (offsets relative to the stream base) with gathered vec
+// entries, RG_UNROLL independent gathers in flight per lane.  Element u of a lane always goes to accumulator u mod 4, so the
+// result does not depend on where the row sits in the ring.  WRAP: the row crosses the end of the ring.
+template <typename T, int G, bool WRAP>
+__device__ __forceinline__ void ring_row_dot(const T* sval, const int32_t* scol, const T* __restrict__ vec, int k, int e,
+                                             T& a0, T& a1, T& a2, T& a3) {
+    int n = e - k;  // this lane's elements are k, k+G, ... while offset < n
+    int p = k & (RG_ELEMS - 1);
+    for (; n > 0; n -= RG_UNROLL * G, p += RG_UNROLL * G) {
+        int c[RG_UNROLL];
+        T v[RG_UNROLL], g[RG_UNROLL];
+        if (n > (RG_UNROLL - 1) * G) {
+#pragma unroll
+            for (int u = 0; u < RG_UNROLL; ++u) {
+                const int i = WRAP ? ((p + u * G) & (RG_ELEMS - 1)) : p + u * G;
+                c[u] = scol[i];
+                v[u] = sval[i];
+            }
+#pragma unroll
+            for (int u = 0; u < RG_UNROLL; ++u) g[u] = __ldg(vec + c[u]);
+        } else {  // last, partial group: predicated
+#pragma unroll
+            for (int u = 0; u < RG_UNROLL; ++u) {
+                const bool in = u * G < n;
+                const int i = WRAP ? ((p + u * G) & (RG_ELEMS - 1)) : p + u * G;
+                c[u] = in ? scol[i] : 0;
+                v[u] = in ? sval[i] : T(0);
+            }
+#pragma unroll
+            for (int u = 0; u < RG_UNROLL; ++u) g[u] = (u * G < n) ? __ldg(vec + c[u]) : T(0);
+        }
+#pragma unroll
+        for (int u = 0; u < RG_UNROLL; u += 4) {
+            a0 += v[u] * g[u];
+            a1 += v[u + 1] * g[u + 1];
+            a2 += v[u + 2] * g[u + 2];
+            a3 += v[u + 3] * g[u + 3];
+        }
+    }
+}
+
+// MODE 0: forward (vec = xg, col = colg, p1 = lb, p2 = ub, p3 = d, out = y);
+// MODE 1: backward (vec = y, p1 = lo, p2 = hi, out = x in place, out2 = xg mirror or NULL)
+template <typename T, int MODE, int G>
+__global__ void __launch_bounds__(RG_THREADS, 1)
+    k_staged(const int64_t* __restrict__ part, const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
+             const T* __restrict__ val, const T* __restrict__ vec, const T* __restrict__ p1, const T* __restrict__ p2,
+             const T* __restrict__ p3, T* out, T* out2, T lambda, int64_t nnz_total, double* dbg) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    RgSmem<T>& S = *reinterpret_cast<RgSmem<T>*>(smem_raw);
+    const int64_t rs = part[blockIdx.x], re = part[blockIdx.x + 1];
+    if (rs >= re) return;
+    const int64_t es = rowptr[rs], ee = rowptr[re];
+    const int64_t base = es & ~int64_t(3);  // 16-byte aligned start of the stream (4 elements)
+    const int ntiles = int((ee - base + RG_TILE - 1) / RG_TILE);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const long long t_begin = clock64();
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < RG_STAGES; ++s) mbar_init(smem_u32(&S.full[s]), 1);
+        for (int w = 0; w < RG_CWARPS; ++w) S.progress[w] = 0;
+        S.completed = 0;
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    volatile int* progress = S.progress;
+    volatile int* completed = &S.completed;
+
+    if (warp == RG_CWARPS) {
+        // ---- producer: one thread feeds the ring ------------------------------------------------------------------
+        if (lane == 0) {
+            const uint64_t pol = l2_evict_first_policy();
+            const int64_t bulk_limit = nnz_total & ~int64_t(3);  // bulk copies never read past the arrays' last whole 16 B
+            int freed = 0;                                        // min over the consumer warps' progress
+            for (int t = 0; t < ntiles; ++t) {
+                const int s = t % RG_STAGES;
+                if (t >= RG_STAGES && freed <= t - RG_STAGES) {
+                    const long long t0 = clock64();
+                    for (;;) {
+                        int mn = progress[0];
+#pragma unroll
+                        for (int w = 1; w < RG_CWARPS; ++w) {
+                            const int p = progress[w];
+                            mn = p < mn ? p : mn;
+                        }
+                        freed = mn;
+                        if (freed > t - RG_STAGES) break;
+                        if (clock64() - t0 > RG_TIMEOUT) __trap();
+                    }
+                    // the consumers' reads of the stage (generic proxy) precede the bulk write (async proxy)
+                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                }
+                const int64_t g0 = base + int64_t(t) * RG_TILE;
+                const int64_t g1 = (g0 + RG_TILE < ee) ? g0 + RG_TILE : ee;  // elements needed: [g0, g1)
+                int64_t gb = (g1 + 3) & ~int64_t(3);                          // bulk part: [g0, gb)
+                if (gb > nnz_total) gb = bulk_limit > g0 ? bulk_limit : g0;
+                for (int64_t g = gb; g < g1; ++g) {  // at most 3 ragged elements at the very end of the arrays
+                    S.val[s * RG_TILE + int(g - g0)] = val[g];
+                    S.col[s * RG_TILE + int(g - g0)] = col[g];
+                }
+                const uint32_t ne = uint32_t(gb - g0);
+                const uint32_t bar = smem_u32(&S.full[s]);
+                if (ne == 0) {
+                    mbar_arrive(bar);
+                } else {
+                    mbar_arrive_expect_tx(bar, ne * uint32_t(sizeof(T) + 4));
+                    bulk_g2s(smem_u32(&S.val[s * RG_TILE]), val + g0, ne * uint32_t(sizeof(T)), bar, pol);
+                    bulk_g2s(smem_u32(&S.col[s * RG_TILE]), col + g0, ne * 4u, bar, pol);
+                }
+            }
+        }
+        return;
+    }
+    if (warp == RG_CWARPS + 1) {
+        // ---- watcher: observes the stage barriers in order, publishes the number of landed tiles --------------------
+        if (lane == 0) {
+            for (int t = 0; t < ntiles; ++t) {
+                mbar_wait(smem_u32(&S.full[t % RG_STAGES]), (t / RG_STAGES) & 1);
+                __threadfence_block();
+                *completed = t + 1;
+            }
+        }
+        return;
+    }
+
+    // ---- consumers --------------------------------------------------------------------------------------------------
+    // All positions below are element offsets relative to `base` and fit an int (a CTA's range is < 2^31 elements).
+    constexpr int GPW = 32 / G;  // rows per warp per iteration
+    const int sub = lane / G, gl = lane % G;
+    const int64_t stride = int64_t(RG_CWARPS) * GPW;
+    int seen = 0;      // tiles [0, seen) known to have landed
+    int released = 0;  // value last stored to progress[warp]
+    int64_t rf = rs + int64_t(warp) * GPW;  // first row of this warp in the current iteration (warp-uniform)
+    int s = 0, e = 0;
+    if (rf < re) {
+        const int64_t r = rf + sub;
+        s = int(rowptr[r < re ? r : re] - base);
+        e = int(rowptr[r + 1 < re ? r + 1 : re] - base);
+    }
+    for (; rf < re; rf += stride) {
+        const int64_t r = rf + sub;
+        const bool valid = r < re;
+        // prefetch the next iteration's row extent and this row's epilogue operands before touching the ring
+        int s_next = 0, e_next = 0;
+        const int64_t rn = r + stride;
+        if (rf + stride < re) {
+            s_next = int(rowptr[rn < re ? rn : re] - base);
+            e_next = int(rowptr[rn + 1 < re ? rn + 1 : re] - base);
+        }
+        T q1 = T(0), q2 = T(0), q3 = T(0);
+        if (valid && gl == 0) {
+            q1 = p1[r];
+            q2 = p2[r];
+            q3 = MODE == 0 ? p3[r] : out[r];
+        }
+        const int w_start = __shfl_sync(0xffffffffu, s, 0), w_end = __shfl_sync(0xffffffffu, e, 31);
+        // Release every tile wholly before this warp's position.  Every lane consumed its previous rows' ring data
+        // (the values fed the shuffle reduction) before this point, and the warp is converged by the shuffle above.
+        int t_start = w_start / RG_TILE;
+        t_start = t_start < ntiles ? t_start : ntiles;
+        if (released < t_start) {
+            released = t_start;
+            if (lane == 0) progress[warp] = t_start;
+        }
+        // wait for the tiles this warp's rows span (span <= RG_STAGES - 1 tiles by the plan)
+        if (w_end > w_start) {
+            const int t_hi = (w_end - 1) / RG_TILE;
+            if (seen <= t_hi) {
+                const long long t0 = clock64();
+                while ((seen = *completed) <= t_hi)
+                    if (clock64() - t0 > RG_TIMEOUT) __trap();
+            }
+        }
+        asm volatile("" ::: "memory");
+        // row dot product from the ring
+        T a0 = T(0), a1 = T(0), a2 = T(0), a3 = T(0);
+        const bool wraps = (w_start & (RG_ELEMS - 1)) + (w_end - w_start) > RG_ELEMS;  // warp-uniform
+        if (!wraps) ring_row_dot<T, G, false>(S.val, S.col, vec, s + gl, e, a0, a1, a2, a3);
+        else ring_row_dot<T, G, true>(S.val, S.col, vec, s + gl, e, a0, a1, a2, a3);
+        T acc = (a0 + a1) + (a2 + a3);
+#pragma unroll
+        for (int o = G >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o, G);
+        if (valid && gl == 0) {
+            if (MODE == 0) {
+                out[r] = q3 * hyperslab_violation(acc, q1, q2);  // y_i = d_i c_i
+            } else {
+                T t = q3 - lambda * acc;  // Eq. 3
+                t = t < q1 ? q1 : t;      // box, un-relaxed (A-2)
+                t = t > q2 ? q2 : t;
+                out[r] = t;
+                if (out2) out2[sup_swz(int(r))] = t;  // keep the de-aliased mirror of x in step
+            }
+        }
+        s = s_next;
+        e = e_next;
+    }
+    // this warp needs nothing more
+    __syncwarp();
+    if (lane == 0) progress[warp] = ntiles;
+    if (dbg && lane == 0 && blockIdx.x < SUP_MAX_PARTIALS) {  // SUP_DEBUG_CHUNKS=1: per-chunk clocks (max over warps), SM id, size
+        unsigned smid;
+        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+        atomicMax(reinterpret_cast<unsigned long long*>(dbg) + blockIdx.x, (unsigned long long)(clock64() - t_begin));
+        if (warp == 0) dbg[SUP_MAX_PARTIALS + blockIdx.x] = double(smid) + double(ee - es) * 1024.0;
+    }
+}
+
+// ---- planning: partition table + eligibility -------------------------------------------------------------------------
+// part[b] = first row r in [r0, r1] with rowptr[r] >= e0 + (e1 - e0) * b / nb  (part[0] = r0, part[nb] = r1)
+__global__ void k_stream_partition(const int64_t* __restrict__ rowptr, int64_t r0, int64_t r1, int nb, int64_t* __restrict__ part) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b > nb) return;
+    if (b == 0) { part[0] = r0; return; }
+    if (b == nb) { part[nb] = r1; return; }
+    const int64_t e0 = rowptr[r0], e1 = rowptr[r1];
+    const int64_t target = e0 + ((e1 - e0) / nb) * b + (((e1 - e0) % nb) * b) / nb;
+    int64_t lo = r0, hi = r1;  // lower bound
+    while (lo < hi) {
+        const int64_t mid = lo + ((hi - lo) >> 1);
+        if (rowptr[mid] < target) lo = mid + 1;
+        else hi = mid;
+    }
+    part[b] = lo;
+}
+
+__global__ void __launch_bounds__(SUP_THREADS) k_stream_max_row(const int64_t* __restrict__ rowptr, int64_t r0, int64_t r1,
+                                                                 unsigned long long* __restrict__ out) {
+    unsigned long long mx = 0;
+    for (int64_t r = r0 + int64_t(blockIdx.x) * blockDim.x + threadIdx.x; r < r1; r += int64_t(gridDim.x) * blockDim.x) {
+        const unsigned long long len = (unsigned long long)(rowptr[r + 1] - rowptr[r]);
+        mx = len > mx ? len : mx;
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        const unsigned long long t = __shfl_xor_sync(0xffffffffu, mx, o);
+        mx = t > mx ? t : mx;
+    }
+    if ((threadIdx.x & 31) == 0 && mx > 0) atomicMax(out, mx);
+}
+
+size_t sup_stream_table_bytes() { return ((size_t(SUP_STREAM_NBMAX) + 1) * 8 + 255) & ~size_t(255); }
+
+template <typename T, int MODE>
+static int staged_occupancy() {
+    if (cudaFuncSetAttribute(k_staged<T, MODE, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(sizeof(RgSmem<T>))) != cudaSuccess) {
+        cudaGetLastError();
+        return 0;
+    }
+    int occ = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_staged<T, MODE, 32>, RG_THREADS, sizeof(RgSmem<T>)) != cudaSuccess) {
+        cudaGetLastError();
+        return 0;
+    }
+    return occ;
+}
+
+static int stream_grid(sup_ctx* h) {  // persistent grid = resident CTAs per SM x SMs (0: unavailable)
+    if (h->stream_nb) return h->stream_nb > 0 ? h->stream_nb : 0;
+    int a, b;
+    if (h->dt == SUP_F32) { a = staged_occupancy<float, 0>(); b = staged_occupancy<float, 1>(); }
+    else { a = staged_occupancy<double, 0>(); b = staged_occupancy<double, 1>(); }
+    const int occ = a < b ? a : b;
+    if (occ < 1) {
+        h->stream_nb = -1;
+        return 0;
+    }
+    h->stream_nb = occ * h->num_sms;
+    return h->stream_nb;
+}
+
+int sup_stream_chunks(bool forward) {
+    const char* env = getenv(forward ? "SUP_CHUNKS_FWD" : "SUP_CHUNKS_BWD");
+    const int v = env ? atoi(env) : 0;
+    return v > 0 ? v : 1;
+}
+
+sup_status sup_stream_plan(sup_ctx* h, const CsrD& M, int64_t r0, int64_t r1, int chunks_per_cta, void* table, void* scratch,
+                           StreamPlan* out) {
+    *out = StreamPlan();
+    if (!h->use_stream || r1 <= r0) return SUP_OK;
+    int nb = stream_grid(h);
+    if (nb < 1) return SUP_OK;
+    {   // optionally more, smaller chunks than resident CTAs (SUP_CHUNKS_FWD / SUP_CHUNKS_BWD; default 1)
+        int64_t want = int64_t(nb) * (chunks_per_cta > 0 ? chunks_per_cta : 1);
+        const int64_t most = (r1 - r0 + 63) / 64;  // keep >= 64 rows per chunk
+        if (want > most) want = most;
+        if (want > SUP_STREAM_NBMAX) want = SUP_STREAM_NBMAX;
+        nb = want < 1 ? 1 : int(want);
+    }
+    // bulk copies need 16-byte aligned sources (element offsets are multiples of 4)
+    if ((reinterpret_cast<uintptr_t>(M.val) & 15) || (reinterpret_cast<uintptr_t>(M.col) & 15)) return SUP_OK;
+    unsigned long long* mx = static_cast<unsigned long long*>(scratch);
+    SUP_CUDA(h, cudaMemsetAsync(mx, 0, 8, h->stream));
+    const int grid = sup_grid_for(r1 - r0, SUP_THREADS, h->num_sms * 8);
+    k_stream_max_row<<<grid, SUP_THREADS, 0, h->stream>>>(M.rowptr, r0, r1, mx);
+    k_stream_partition<<<(nb + 1 + 127) / 128, 128, 0, h->stream>>>(M.rowptr, r0, r1, nb, static_cast<int64_t*>(table));
+    unsigned long long mx_h = 0;
+    int64_t ends[2] = {0, 0};
+    SUP_CUDA(h, cudaMemcpyAsync(&mx_h, mx, 8, cudaMemcpyDeviceToHost, h->stream));
+    SUP_CUDA(h, cudaMemcpyAsync(&ends[0], M.rowptr + r0, 8, cudaMemcpyDeviceToHost, h->stream));
+    SUP_CUDA(h, cudaMemcpyAsync(&ends[1], M.rowptr + r1, 8, cudaMemcpyDeviceToHost, h->stream));
+    SUP_CUDA(h, cudaStreamSynchronize(h->stream));
+    SUP_CUDA(h, cudaGetLastError());
+    // Lanes per row: the rows a warp holds at once (32/G of them) should total ~a tile -- enough elements per lane to
+    // amortise the per-row work, few enough that the 16 warps' rows together leave ring stages free for prefetch --
+    // and must never span more than RG_STAGES - 1 tiles.
+    const double avg = double(ends[1] - ends[0]) / double(r1 - r0);
+    int G = 4;
+    while (G < 32 && avg * (32 / G) > 960.0) G <<= 1;
+    if (const char* env = getenv("SUP_STREAM_G")) {
+        const int g = atoi(env);
+        if (g == 4 || g == 8 || g == 16 || g == 32) G = g;
+    }
+    const int64_t cap = int64_t(RG_STAGES - 2) * RG_TILE;
+    while (G < 32 && int64_t(mx_h) * (32 / G) > cap) G <<= 1;
+    out->max_row = int64_t(mx_h);
+    if (int64_t(mx_h) * (32 / G) > cap) return SUP_OK;  // a row too long for the ring: group-per-row kernels
+    out->part = static_cast<const int64_t*>(table);
+    out->nb = nb;
+    out->G = G;
+    out->ok = true;
+    return SUP_OK;
+}
+
+// ---- launchers --------------------------------------------------------------------------------------------------------
+static bool stream_debug() {
+    static int v = -1;
+    if (v < 0) {
+        const char* env = getenv("SUP_DEBUG_CHUNKS");
+        v = env && env[0] == '1';
+    }
+    return v == 1;
+}
+
+template <typename T, int MODE, int G>
+static void launch_staged_g(sup_ctx* h, const StreamPlan& sp, const CsrD& M, const void* vec, const void* p1, const void* p2,
+                            const void* p3, void* out, void* out2, double lambda) {
+    static bool attr_set = false;  // per instantiation: opt in to > 48 KB of dynamic shared memory once
+    if (!attr_set) {
+        cudaFuncSetAttribute(k_staged<T, MODE, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(sizeof(RgSmem<T>)));
+        attr_set = true;
+    }
+    k_staged<T, MODE, G><<<sp.nb, RG_THREADS, sizeof(RgSmem<T>), h->stream>>>(
+        sp.part, M.rowptr, M.col, static_cast<const T*>(M.val), static_cast<const T*>(vec), static_cast<const T*>(p1),
+        static_cast<const T*>(p2), static_cast<const T*>(p3), static_cast<T*>(out), static_cast<T*>(out2), T(lambda),
+        M.alloc_nnz, stream_debug() ? h->partials : nullptr);
+    h->launches++;
+}
+
+template <typename T, int MODE>
+static void launch_staged(sup_ctx* h, const StreamPlan& sp, const CsrD& M, const void* vec, const void* p1, const void* p2,
+                          const void* p3, void* out, void* out2, double lambda) {
+    switch (sp.G) {
+        case 4: launch_staged_g<T, MODE, 4>(h, sp, M, vec, p1, p2, p3, out, out2, lambda); break;
+        case 8: launch_staged_g<T, MODE, 8>(h, sp, M, vec, p1, p2, p3, out, out2, lambda); break;
+        case 16: launch_staged_g<T, MODE, 16>(h, sp, M, vec, p1, p2, p3, out, out2, lambda); break;
+        default: launch_staged_g<T, MODE, 32>(h, sp, M, vec, p1, p2, p3, out, out2, lambda); break;
+    }
+}
+
+// ---- de-aliased mirror of x ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(SUP_THREADS) k_swizzle_cols(const int32_t* __restrict__ col, int64_t nnz, int32_t* __restrict__ colg) {
+    for (int64_t k = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; k < nnz; k += int64_t(gridDim.x) * blockDim.x)
+        colg[k] = sup_swz(col[k]);
+}
+
+template <typename T>
+__global__ void __launch_bounds__(SUP_THREADS) k_swizzle_copy(const T* __restrict__ x, int n, T* __restrict__ xg) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j < n) xg[sup_swz(j)] = x[j];
+}
+
+sup_status sup_stream_setup_gather(sup_ctx* h) {
+    if (!h->colg || h->nnz == 0) return SUP_OK;
+    k_swizzle_cols<<<sup_grid_for(h->nnz, SUP_THREADS, h->num_sms * 16), SUP_THREADS, 0, h->stream>>>(h->A.col, h->nnz, h->colg);
+    h->launches++;
+    SUP_CUDA(h, cudaGetLastError());
+    return SUP_OK;
+}
+
+bool sup_stream_forward_uses_xg(const sup_ctx* h) {
+    if (!h->colg || !h->xg) return false;
+    if (h->A.plan.ok) return true;
+    for (const StreamPlan& p : h->stream_fwd_blk)
+        if (p.ok) return true;
+    return false;
+}
+
+void sup_launch_stream_fwd(sup_ctx* h, const StreamPlan& sp, const void* x, const void* dscale) {
+    CsrD M = h->A;
+    const void* vec = x;
+    if (h->colg && h->xg) {
+        if (!h->xg_synced) {
+            const unsigned grid = unsigned((h->n + SUP_THREADS - 1) / SUP_THREADS);
+            if (h->dt == SUP_F32) k_swizzle_copy<float><<<grid, SUP_THREADS, 0, h->stream>>>(static_cast<const float*>(x), int(h->n), static_cast<float*>(h->xg));
+            else k_swizzle_copy<double><<<grid, SUP_THREADS, 0, h->stream>>>(static_cast<const double*>(x), int(h->n), static_cast<double*>(h->xg));
+            h->launches++;
+            h->xg_synced = true;
+        }
+        M.col = h->colg;
+        vec = h->xg;
+    }
+    if (h->dt == SUP_F32) launch_staged<float, 0>(h, sp, M, vec, h->lb, h->ub, dscale, h->y, nullptr, 0.0);
+    else launch_staged<double, 0>(h, sp, M, vec, h->lb, h->ub, dscale, h->y, nullptr, 0.0);
+}
+
+void sup_launch_stream_bwd(sup_ctx* h, const CsrD& AT, const StreamPlan& sp, void* x, double lambda) {
+    void* mirror = sup_stream_forward_uses_xg(h) ? h->xg : nullptr;
+    if (h->dt == SUP_F32) launch_staged<float, 1>(h, sp, AT, h->y, h->lo, h->hi, nullptr, x, mirror, lambda);
+    else launch_staged<double, 1>(h, sp, AT, h->y, h->lo, h->hi, nullptr, x, mirror, lambda);
+    h->xg_synced = mirror != nullptr;
+}
