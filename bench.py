@@ -103,6 +103,32 @@ class ClockSampler(threading.Thread):
         return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx or None, "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def dist_setup(world, backend, device=None):
+    """One process per GPU (RANK/WORLD_SIZE/MASTER_* from the environment).  The path has no exchange step
+    ("replicas only"): the process group is used for the barrier and the max over ranks only."""
+    if world <= 1:
+        return None
+    import torch
+    import torch.distributed as dist
+
+    if backend == "nccl":
+        dist.init_process_group("nccl", device_id=torch.device(device))
+    else:
+        dist.init_process_group(backend)
+    return dist
+
+
+def max_over_ranks(value, dist, device="cpu"):
+    """The timed region of a multi-rank run is the slowest rank's."""
+    if dist is None:
+        return float(value)
+    import torch
+
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 def time_oracle(P, budget_s=20.0):
     """cpu_baseline: the oracle as it stands, single thread, on a bounded sample (a few superiorized sweeps)."""
     from oracle.oracle import Oracle
@@ -162,11 +188,7 @@ def run_ours(args, rank, world, local_rank):
         raise SystemExit("bench.py needs a CUDA device (libsup has no CPU fallback)")
     torch.cuda.set_device(local_rank)
     dev = f"cuda:{local_rank}"
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-
-        dist.init_process_group("nccl", device_id=torch.device(dev))
+    dist = dist_setup(world, "nccl", dev)
 
     P = make_problem(args.workload)
     t0 = time.perf_counter()
@@ -205,10 +227,7 @@ def run_ours(args, rank, world, local_rank):
     launches = H.launches - launches0
     st = sup.sup_get_state(H)
     sampler.stop_flag = True
-    if dist is not None:
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, dist, dev)
     value = world * args.steps * S / (ms * 1e-3)
 
     # ---- e2e: the C-ABI call with HOST buffers (pinned), H2D + D2H inside the timed region -------------------
@@ -223,10 +242,7 @@ def run_ours(args, rank, world, local_rank):
         xh.copy_(xh0)
         sup.sup_superiorize_host(H, xh, S, P.N, P.beta0, P.a, **kw)  # synchronises
     e2e_s = time.perf_counter() - t0
-    if dist is not None:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = max_over_ranks(e2e_s, dist, dev)
     e2e = world * args.steps * S / e2e_s
     checksum = float(xh.double().sum())
 

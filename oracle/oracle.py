@@ -162,8 +162,9 @@ class Oracle:
                     warn=warn.value)
 
     def superiorize(self, x0, n_iter, N, beta0, a, lam=1.0, policy=PER_TRIAL, block=False, snapshots=(), ell0=0,
-                    forced=None, kind=None, shape=None, cap=1 << 22):
-        """Algorithm 1 for n_iter sweeps.  snapshots: sweep counts (1-based: 'after s sweeps') at which x is copied.
+                    forced=None, kind=None, shape=None, cap=1 << 22, k0=0):
+        """Algorithm 1 for n_iter sweeps (absolute sweep indices k0 .. k0+n_iter-1; k0 only matters to PER_SWEEP).
+        snapshots: sweep counts (1-based: 'after s sweeps') at which x is copied.
         Returns dict(x, ell, trace[n_iter,4] = (prox0, f, trials, ell), snaps{count: x}, decisions, margins, warn)."""
         x = np.array(x0, np.float64)
         ell = _i64(int(ell0))
@@ -185,7 +186,7 @@ class Oracle:
             warn |= _L().orc_superiorize(
                 _i64(self.m), _i64(self.n), _p(self.rowptr), _p(self.col), _p(self.val), _p(self.lb), _p(self.ub),
                 _p(self.w), _p(self.rho), _p(self.d), _p(self.lo), _p(self.hi), _dbl(lam), _int(nb),
-                _p(self.block_rowptr) if nb else None, *self._obj_args(kind, shape), _p(x), ctypes.byref(ell), _i64(k),
+                _p(self.block_rowptr) if nb else None, *self._obj_args(kind, shape), _p(x), ctypes.byref(ell), _i64(k0 + k),
                 _int(cnt), _int(N), _dbl(beta0), _dbl(a), _int(policy), _p(tr), _p(dec), _p(mar), _i64(cap),
                 ctypes.byref(ndec), _p(forced_a))
             trace[k:stop] = tr

@@ -10,6 +10,8 @@ import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIBPATH = os.path.join(_HERE, "libsup.so")
+if os.environ.get("SUP_LIBSUP_VARIANT"):  # A/B measurements of build-time kernel parameters (see build.py build_variant)
+    _LIBPATH = os.path.join(_HERE, "libsup_" + os.environ["SUP_LIBSUP_VARIANT"] + ".so")
 _lib = None
 
 F32, F64 = 0, 1

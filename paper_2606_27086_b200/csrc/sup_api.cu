@@ -138,11 +138,11 @@ extern "C" sup_status sup_create(sup_handle* out, const sup_csr* A, const void* 
     h->AT.col = at_col;
     h->AT.val = at_val;
     h->AT.alloc_nnz = h->nnz;
-    rc = sup_stream_plan(h, h->A, 0, h->m, sup_stream_chunks(true), tab_a, scratch, &h->A.plan);
+    rc = sup_stream_plan(h, h->A, 0, h->m, true, tab_a, scratch, &h->A.plan);
     if (rc == SUP_OK && h->use_stream) rc = sup_stream_setup_gather(h);
     if (rc == SUP_OK && cudaMemsetAsync(h->xg, 0, size_t((h->n + 511) & ~int64_t(511)) * h->esz, h->stream) != cudaSuccess)
         rc = sup_fail(h, SUP_ERR_CUDA, "sup_create: %s", cudaGetErrorString(cudaGetLastError()));
-    if (rc == SUP_OK) rc = sup_stream_plan(h, h->AT, 0, h->n, sup_stream_chunks(false), tab_at, scratch, &h->AT.plan);
+    if (rc == SUP_OK) rc = sup_stream_plan(h, h->AT, 0, h->n, false, tab_at, scratch, &h->AT.plan);
     if (rc != SUP_OK) {
         memcpy(g_create_error, h->err, sizeof(g_create_error));
         delete h;
@@ -212,8 +212,8 @@ extern "C" sup_status sup_set_blocks(sup_handle h, int n_blocks, const int64_t* 
         void* tab_f = B.take(sup_stream_table_bytes());
         void* tab_b = B.take(sup_stream_table_bytes());
         if (!B.ok) return sup_fail(h, SUP_ERR_WORKSPACE, "sup_set_blocks: workspace too small");
-        rc = sup_stream_plan(h, h->A, block_rowptr[t], block_rowptr[t + 1], sup_stream_chunks(true), tab_f, scratch, &h->stream_fwd_blk[t]);
-        if (rc == SUP_OK) rc = sup_stream_plan(h, T, 0, h->n, sup_stream_chunks(false), tab_b, scratch, &T.plan);
+        rc = sup_stream_plan(h, h->A, block_rowptr[t], block_rowptr[t + 1], true, tab_f, scratch, &h->stream_fwd_blk[t]);
+        if (rc == SUP_OK) rc = sup_stream_plan(h, T, 0, h->n, false, tab_b, scratch, &T.plan);
         if (rc != SUP_OK) return rc;
     }
     h->n_blocks = n_blocks;

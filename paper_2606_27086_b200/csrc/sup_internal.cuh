@@ -170,10 +170,9 @@ void sup_launch_proximity(sup_ctx* h, const void* x, int mode, double p, double*
 // ---- bulk-copy-staged products (sup_stream.cu) ---------------------------------------------------------------
 size_t sup_stream_table_bytes();  // bytes of one partition table (256-aligned)
 // Plans rows [r0, r1) of M: grid size, partition table (written into `table`, sup_stream_table_bytes() bytes of
-// persistent workspace), lanes per row; chunks_per_cta x resident CTAs chunks; synchronises the stream.  `scratch` needs 256 bytes.
-sup_status sup_stream_plan(sup_ctx* h, const CsrD& M, int64_t r0, int64_t r1, int chunks_per_cta, void* table, void* scratch,
+// persistent workspace), lanes per row; `forward` only selects which tuning overrides apply; synchronises the stream.  `scratch` needs 256 bytes.
+sup_status sup_stream_plan(sup_ctx* h, const CsrD& M, int64_t r0, int64_t r1, bool forward, void* table, void* scratch,
                            StreamPlan* out);
-int sup_stream_chunks(bool forward);  // chunks per resident CTA for the forward / transposed product
 void sup_launch_stream_fwd(sup_ctx* h, const StreamPlan& rp, const void* x, const void* dscale);
 void sup_launch_stream_bwd(sup_ctx* h, const CsrD& AT, const StreamPlan& rp, void* x, double lambda);
 sup_status sup_stream_setup_gather(sup_ctx* h);  // fills colg from A.col

@@ -19,6 +19,7 @@
 #define TILE_H 16
 #define TILE_W 64
 #define BARRIER_SPIN_LIMIT (1u << 24)
+#define SUP_TRIAL_BATCH 4  // candidate steps evaluated per pass (TV objectives)
 
 template <typename T>
 struct PArgs {
@@ -91,6 +92,31 @@ __device__ __forceinline__ double cta_sum(double v) {
     return tot;
 }
 
+// B sums at once (same order per value as cta_sum)
+template <int B>
+__device__ __forceinline__ void cta_sum_batch(double* v) {
+    __shared__ double wsb[B][SUP_THREADS / 32];
+    __shared__ double totb[B];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int b = 0; b < B; ++b)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v[b] += __shfl_xor_sync(0xffffffffu, v[b], o);
+    __syncthreads();
+    if (lane == 0)
+#pragma unroll
+        for (int b = 0; b < B; ++b) wsb[b][wid] = v[b];
+    __syncthreads();
+    if (threadIdx.x < B) {
+        double t = 0.0;
+        for (int q = 0; q < SUP_THREADS / 32; ++q) t += wsb[threadIdx.x][q];
+        totb[threadIdx.x] = t;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int b = 0; b < B; ++b) v[b] = totb[b];
+}
+
 // every CTA sums the same gridDim.x partials in the same order -> identical value everywhere
 __device__ __forceinline__ double reduce_partials(const double* partials) {
     double s = 0.0;
@@ -120,6 +146,48 @@ __device__ double tv2d_share(const PArgs<T>& A, double coef) {
         acc += sqrt(dx * dx + dy * dy);
     }
     return acc;
+}
+
+// the same for up to SUP_TRIAL_BATCH candidate steps at once: x and g are read once, every candidate's terms are
+// accumulated in the order tv2d_share uses, so each result equals the one-at-a-time value bit for bit
+template <typename T, int B>
+__device__ void tv2d_share_batch(const PArgs<T>& A, const double* coef, double* acc) {
+    const int64_t h = A.ny - 1, w = A.nx - 1;
+    const int64_t total = h > 0 && w > 0 ? h * w : 0;
+#pragma unroll
+    for (int b = 0; b < B; ++b) acc[b] = 0.0;
+    for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q < total; q += int64_t(gridDim.x) * blockDim.x) {
+        const int64_t i = q / w, j = q - i * w;
+        const int64_t p = i * A.nx + j;
+        const double x00 = double(__ldcg(A.x + p)), x10 = double(__ldcg(A.x + p + A.nx)), x01 = double(__ldcg(A.x + p + 1));
+        const double g00 = double(__ldcg(A.g + p)), g10 = double(__ldcg(A.g + p + A.nx)), g01 = double(__ldcg(A.g + p + 1));
+#pragma unroll
+        for (int b = 0; b < B; ++b) {
+            const double c = coef[b];
+            const double z00 = c == 0.0 ? x00 : double(T(fma(-c, g00, x00)));
+            const double z10 = c == 0.0 ? x10 : double(T(fma(-c, g10, x10)));
+            const double z01 = c == 0.0 ? x01 : double(T(fma(-c, g01, x01)));
+            const double dx = z10 - z00, dy = z01 - z00;
+            acc[b] += sqrt(dx * dx + dy * dy);
+        }
+    }
+}
+
+template <typename T, int B>
+__device__ void tv1d_share_batch(const PArgs<T>& A, const double* coef, double* acc) {
+#pragma unroll
+    for (int b = 0; b < B; ++b) acc[b] = 0.0;
+    for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q + 1 < A.n; q += int64_t(gridDim.x) * blockDim.x) {
+        const double x0 = double(__ldcg(A.x + q)), x1 = double(__ldcg(A.x + q + 1));
+        const double g0 = double(__ldcg(A.g + q)), g1 = double(__ldcg(A.g + q + 1));
+#pragma unroll
+        for (int b = 0; b < B; ++b) {
+            const double c = coef[b];
+            const double z0 = c == 0.0 ? x0 : double(T(fma(-c, g0, x0)));
+            const double z1 = c == 0.0 ? x1 : double(T(fma(-c, g1, x1)));
+            acc[b] += fabs(z1 - z0);
+        }
+    }
 }
 
 template <typename T>
@@ -307,35 +375,56 @@ __global__ void __launch_bounds__(SUP_THREADS) k_perturb(PArgs<T> A) {
         const double s = sqrt(reduce_partials(P));
         bool accepted = false;
         long long jloc = 0;
-        for (int trial = 0; trial < SUP_J_MAX && !accepted; ++trial) {
-            const double expo = A.policy == SUP_STEP_PER_TRIAL ? double(ell) : double(k + jloc);
-            const double beta = A.beta0 * pow(A.a, expo);
-            const double coef = s > 0.0 ? beta / s : 0.0;
+        // Trials are evaluated SUP_TRIAL_BATCH candidates per pass for the TV objectives (their step sizes are known in
+        // advance: beta0 a^l, beta0 a^(l+1), ...), then decided strictly in order: the first candidate with
+        // f(z) <= f(x^{k,n}) is accepted and the later ones are discarded uncounted -- the sequence of trials, decisions
+        // and l is exactly Algorithm 1's; only the number of grid barriers per reduction step drops.
+        constexpr int B = OBJ == SUP_OBJ_DOSE ? 1 : SUP_TRIAL_BATCH;
+        for (int trial = 0; trial < SUP_J_MAX && !accepted; trial += B) {
+            double coef[B], fzb[B];
+#pragma unroll
+            for (int b = 0; b < B; ++b) {
+                const double expo = A.policy == SUP_STEP_PER_TRIAL ? double(ell + b) : double(k + jloc + b);
+                const double beta = A.beta0 * pow(A.a, expo);
+                coef[b] = s > 0.0 ? beta / s : 0.0;
+            }
             P = slot ? P1 : P0;
             slot ^= 1;
-            sh = cta_sum(objective_share<T, OBJ>(A, coef));
-            if (threadIdx.x == 0) P[blockIdx.x] = sh;
-            grid_barrier(st);
-            const double fz = reduce_partials(P);
-            ++ell;
-            ++jloc;
-            ++trials;
-            const bool acc = fz <= fx;  // NaN compares false -> rejected (A-11)
-            if (blockIdx.x == 0 && threadIdx.x == 0) {
-                if (A.decisions && ndec < A.cap) A.decisions[ndec] = acc ? 1 : 0;
-                if (A.decision_f && ndec < A.cap) {
-                    A.decision_f[2 * ndec] = fz;
-                    A.decision_f[2 * ndec + 1] = fx;
-                }
+            if (B == 1) {
+                fzb[0] = cta_sum(objective_share<T, OBJ>(A, coef[0]));
+                if (threadIdx.x == 0) P[blockIdx.x] = fzb[0];
+            } else {
+                if (OBJ == SUP_OBJ_TV2D) tv2d_share_batch<T, B>(A, coef, fzb);
+                else tv1d_share_batch<T, B>(A, coef, fzb);
+                cta_sum_batch<B>(fzb);
+                if (threadIdx.x < B) P[threadIdx.x * (SUP_MAX_PARTIALS / B) + blockIdx.x] = fzb[threadIdx.x];
             }
-            ++ndec;
-            if (acc) {
-                if (coef != 0.0)
-                    for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q < A.n; q += int64_t(gridDim.x) * blockDim.x)
-                        A.x[q] = T(zval(A.x, A.g, coef, q));
-                grid_barrier(st);  // x^{k,n+1} visible to everyone before the next gradient
-                fx = fz;
-                accepted = true;
+            grid_barrier(st);
+#pragma unroll
+            for (int b = 0; b < B; ++b) fzb[b] = reduce_partials(P + b * (SUP_MAX_PARTIALS / B));
+            for (int b = 0; b < B && !accepted && trial + b < SUP_J_MAX; ++b) {
+                const double fz = fzb[b];
+                ++ell;
+                ++jloc;
+                ++trials;
+                const bool acc = fz <= fx;  // NaN compares false -> rejected (A-11)
+                if (blockIdx.x == 0 && threadIdx.x == 0) {
+                    if (A.decisions && ndec < A.cap) A.decisions[ndec] = acc ? 1 : 0;
+                    if (A.decision_f && ndec < A.cap) {
+                        A.decision_f[2 * ndec] = fz;
+                        A.decision_f[2 * ndec + 1] = fx;
+                    }
+                }
+                ++ndec;
+                if (acc) {
+                    const double cf = coef[b];
+                    if (cf != 0.0)
+                        for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q < A.n; q += int64_t(gridDim.x) * blockDim.x)
+                            A.x[q] = T(zval(A.x, A.g, cf, q));
+                    grid_barrier(st);  // x^{k,n+1} visible to everyone before the next gradient
+                    fx = fz;
+                    accepted = true;
+                }
             }
             if (*(volatile int*)&st->fault & 1) break;  // a barrier timed out: stop looping
         }
@@ -439,6 +528,7 @@ int sup_perturb_grid(sup_ctx* h, int objective) {
     } else {
         want = (h->n + 4 * SUP_THREADS - 1) / (4 * SUP_THREADS);  // about four elements per thread
         if (want > 2 * int64_t(h->num_sms)) want = 2 * int64_t(h->num_sms);
+        if (want > SUP_MAX_PARTIALS / SUP_TRIAL_BATCH) want = SUP_MAX_PARTIALS / SUP_TRIAL_BATCH;  // one partial row per candidate
     }
     if (want < 1) want = 1;
     return int(want < cap ? want : cap);

