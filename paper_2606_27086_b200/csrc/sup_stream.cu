@@ -32,7 +32,7 @@
 #ifndef RG_STAGES
 #define RG_STAGES 16
 #endif
-#define RG_ELEMS (RG_TILE * RG_STAGES)      // ring capacity in elements (a power of two)
+#define RG_ELEMS (RG_TILE * RG_STAGES)      // ring capacity in elements (need not be a power of two)
 #define RG_CWARPS 16                        // consumer warps
 #define RG_THREADS (32 * (RG_CWARPS + 1))   // + producer warp
 #ifndef RG_PLANES
@@ -98,14 +98,16 @@ template <typename T, int G, bool WRAP>
 __device__ __forceinline__ void ring_row_dot(const T* sval, const int32_t* scol, const T* __restrict__ vec, int k, int e,
                                              T& a0, T& a1, T& a2, T& a3) {
     int n = e - k;  // this lane's elements are k, k+G, ... while offset < n
-    int p = k & (RG_ELEMS - 1);
+    int p = k % RG_ELEMS;
     for (; n > 0; n -= RG_UNROLL * G, p += RG_UNROLL * G) {
+        if (WRAP && p >= RG_ELEMS) p -= RG_ELEMS;
         int c[RG_UNROLL];
         T v[RG_UNROLL], g[RG_UNROLL];
         if (n > (RG_UNROLL - 1) * G) {
 #pragma unroll
             for (int u = 0; u < RG_UNROLL; ++u) {
-                const int i = WRAP ? ((p + u * G) & (RG_ELEMS - 1)) : p + u * G;
+                int i = p + u * G;
+                if (WRAP && i >= RG_ELEMS) i -= RG_ELEMS;
                 c[u] = scol[i];
                 v[u] = sval[i];
             }
@@ -115,7 +117,8 @@ __device__ __forceinline__ void ring_row_dot(const T* sval, const int32_t* scol,
 #pragma unroll
             for (int u = 0; u < RG_UNROLL; ++u) {
                 const bool in = u * G < n;
-                const int i = WRAP ? ((p + u * G) & (RG_ELEMS - 1)) : p + u * G;
+                int i = p + u * G;
+                if (WRAP && i >= RG_ELEMS) i -= RG_ELEMS;
                 c[u] = in ? scol[i] : 0;
                 v[u] = in ? sval[i] : T(0);
             }
@@ -270,7 +273,7 @@ __global__ void __launch_bounds__(32 * (NCW + 1), 1)
         asm volatile("" ::: "memory");
         // row dot product from the ring
         T a0 = T(0), a1 = T(0), a2 = T(0), a3 = T(0);
-        const bool wraps = (w_start & (RG_ELEMS - 1)) + (w_end - w_start) > RG_ELEMS;  // warp-uniform
+        const bool wraps = (w_start % RG_ELEMS) + (w_end - w_start) > RG_ELEMS;  // warp-uniform
         if (!wraps) ring_row_dot<T, G, false>(S.val, S.col, vec, s + gl, e, a0, a1, a2, a3);
         else ring_row_dot<T, G, true>(S.val, S.col, vec, s + gl, e, a0, a1, a2, a3);
         T acc = (a0 + a1) + (a2 + a3);
