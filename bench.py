@@ -278,6 +278,7 @@ def run_ours(args, rank, world, local_rank):
         t_ms = a.elapsed_time(b) / reps
         kern[name] = {"ms": t_ms, "algorithmic_bytes": nbytes, "gbs": nbytes / (t_ms * 1e-3) / 1e9}
     # unperturbed sweep (both kernels) for the share check
+    H._check(sup.lib().sup_project_simultaneous(H.h, xs.data_ptr(), 1.0, 3))
     a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     H.stream.synchronize()
     a.record(H.stream)
@@ -291,12 +292,14 @@ def run_ours(args, rank, world, local_rank):
             "kernels": kern, "basic_sweep_ms": sweep_ms,
             "basic_sweep_gbs": (bytes_fwd + bytes_bwd) / (sweep_ms * 1e-3) / 1e9,
             "superiorized_sweep_ms": ms / (args.steps * S)}
-    tr = os.path.join(ROOT, "profiles", "traffic.json")
+    tr = os.path.join(ROOT, "profiles", "traffic.csv")  # per-launch DRAM bytes from the committed ncu --set full capture
     if os.path.exists(tr):
-        try:
-            roof["traffic"] = json.load(open(tr)).get(args.workload, {}).get(dom)
-        except Exception:
-            pass
+        import csv
+
+        for row in csv.DictReader(open(tr)):
+            if row["workload"] == args.workload and row["kernel"] == dom and not args.block:
+                roof["traffic"] = int(row["dram_bytes_per_launch"])
+                roof["traffic_source"] = "profiles/" + row["source"]
 
     cpu_v, cpu_done, cpu_el = time_oracle(P, args.cpu_budget) if args.cpu_budget > 0 else (None, 0, 0.0)
     line = {

@@ -174,7 +174,8 @@ sup_status sup_proximity(sup_handle h, const void* x, int mode, double p, double
 sup_status sup_objective(sup_handle h, const void* x, int kind, const int64_t* shape, double* out);
 
 /* Copies derived arrays for inspection/tests: which = 0: d [m] (dtype); 1: A^T rowptr [n+1] int64;
- * 2: A^T col [nnz] int32 (original row indices); 3: A^T val [nnz] (dtype).  dst is a DEVICE pointer. */
+ * 2: A^T col [nnz] int32 (original row indices); 3: A^T val [nnz] (dtype); 5: y [m] (dtype), the scaled violation
+ * d_i c_i(x) left by the last forward product (sup_forward_violation or a sweep).  dst is a DEVICE pointer. */
 sup_status sup_get_derived(sup_handle h, int which, void* dst, size_t dst_bytes);
 
 /* Number of kernel launches this handle has enqueued so far (graph replays count their kernel nodes). */

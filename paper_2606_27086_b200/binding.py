@@ -322,7 +322,7 @@ def sup_objective(H: SupHandle, x: torch.Tensor, kind, shape=None) -> float:
 
 
 def sup_get_derived(H: SupHandle, which: int) -> torch.Tensor:
-    shapes = {0: (H.m, H.tdtype), 1: (H.n + 1, torch.int64), 2: (H.nnz, torch.int32), 3: (H.nnz, H.tdtype)}
+    shapes = {0: (H.m, H.tdtype), 1: (H.n + 1, torch.int64), 2: (H.nnz, torch.int32), 3: (H.nnz, H.tdtype), 5: (H.m, H.tdtype)}
     cnt, dt = shapes[which]
     out = torch.empty(cnt, dtype=dt, device=H.device)
     H._enter()

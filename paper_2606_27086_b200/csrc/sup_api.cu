@@ -568,6 +568,7 @@ extern "C" sup_status sup_get_derived(sup_handle h, int which, void* dst, size_t
         case 1: src = h->AT.rowptr; bytes = size_t(h->n + 1) * 8; break;
         case 2: src = h->AT.col; bytes = size_t(h->nnz) * 4; break;
         case 3: src = h->AT.val; bytes = size_t(h->nnz) * h->esz; break;
+        case 5: src = h->y; bytes = size_t(h->m) * h->esz; break;  // y = D c(x) of the last forward product
         case 4: src = h->partials; bytes = 2 * SUP_MAX_PARTIALS * 8; break;  // debug: per-chunk clocks (SUP_DEBUG_CHUNKS=1)
         default: return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_get_derived: unknown array");
     }

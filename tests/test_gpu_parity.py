@@ -559,3 +559,63 @@ def test_argument_errors():
     with pytest.raises(sup.SupError) as e:
         sup.sup_create(P.rowptr, P.col, P.val, P.lb, P.ub, P.lo, P.hi, w, dtype=0, n=P.n)  # weight <= 0
     assert e.value.status == 2
+
+
+# ------------------------------------------------------------------------------------------------------------
+# full size: BASELINE.json configs[2] in the launch configuration bench.py times
+# ------------------------------------------------------------------------------------------------------------
+def test_full_size_config3_sampled_rows_columns_and_invariants():
+    """512x512 low-dose CT (m = 524 880, nnz = 2.4e8), fp32, the staged kernels and the CUDA graph bench.py uses.
+    The oracle needs ~26 s per sweep here, so: sampled outputs recomputed one by one in fp64 from the definitions
+    (y_i = d_i c_i(<a_i,x>), Eq. 2 / L608; x_j <- clip(x_j - lambda sum_i a_ij y_i), Eq. 3 / L427), and properties that
+    hold at any size (proximity non-increasing along unperturbed sweeps, iterate inside the box, bit-identical reruns)."""
+    from paper_2606_27086_b200.binding import sup_get_derived
+
+    sup = _sup()
+    P = gen.config3_lowdose_ct()
+    H = make_handle(P, 0, blocks=False)
+    x = xdev(P, 0)
+    prox = []
+    for _ in range(4):
+        sup.sup_project_simultaneous(H, x, 1.0, 1)
+        prox.append(sup.sup_proximity(H, x, 0))
+        assert float(x.min()) >= 0.0  # box [0, inf)
+    assert all(b <= a * (1 + 1e-6) for a, b in zip(prox, prox[1:])), prox
+    # forward product on sampled rows
+    rng = np.random.default_rng(7)
+    xh = x.cpu().numpy().astype(np.float64)
+    sup.sup_forward_violation(H, x)
+    y = sup_get_derived(H, 5).cpu().numpy().astype(np.float64)
+    rows = np.unique(np.concatenate([rng.integers(0, P.m, 3000), np.arange(0, 60), np.arange(P.m - 60, P.m)]))
+    worst = 0.0
+    for i in rows:
+        s, e = P.rowptr[i], P.rowptr[i + 1]
+        a = P.val[s:e].astype(np.float64)
+        rho = float(np.dot(a, a))
+        r = float(np.dot(a, xh[P.col[s:e]]))
+        lb, ub = float(P.lb[i]), float(P.ub[i])
+        c = r - ub if r > ub else (r - lb if r < lb else 0.0)
+        yi = (1.0 / P.m) / rho * c if rho > 0 else 0.0
+        # fp32 row dot: |r| error ~ 1e-6 |r| can move c by that much in absolute terms
+        tol = 1e-4 * abs(yi) + (1.0 / P.m) / max(rho, 1e-30) * 1e-5 * max(abs(r), 1.0) if rho > 0 else 0.0
+        assert abs(y[i] - yi) <= tol, (i, y[i], yi, r, lb, ub)
+        worst = max(worst, abs(y[i] - yi) / max(abs(yi), 1e-30) if yi != 0 else 0.0)
+    # back-projection on sampled columns (entries of column j found by scanning col[])
+    xb = x.clone()
+    sup.sup_backproject_update(H, xb, 1.0)
+    xn = xb.cpu().numpy().astype(np.float64)
+    rowid = np.repeat(np.arange(P.m, dtype=np.int64), np.diff(P.rowptr))
+    for j in rng.integers(0, P.n, 24):
+        k = np.flatnonzero(P.col == j)
+        u = float(np.dot(P.val[k].astype(np.float64), y[rowid[k]]))
+        want = max(0.0, xh[j] - u)
+        assert abs(xn[j] - want) <= 1e-5 * max(abs(want), abs(xh[j]), 1e-3), (j, xn[j], want)
+    # superiorized run, CUDA graph: deterministic, state sane, objective did not blow up
+    outs = []
+    for _ in range(2):
+        xs = xdev(P, 0)
+        sup.sup_superiorize(H, xs, 6, P.N, P.beta0, P.a, objective=P.objective, shape=P.shape, lam=P.lam)
+        st = sup.sup_get_state(H)
+        assert st["fault"] == 0 and st["warn"] == 0 and st["ell"] >= 6 * P.N and np.isfinite(st["f"])
+        outs.append(xs.cpu())
+    assert torch.equal(outs[0], outs[1])
