@@ -13,6 +13,7 @@
 // Objectives: TV2D (Eq. 15; gradient A-8, shared-memory tile with halo, fused with sum g^2),
 // TV1D (A-16), DOSE ||D x||^2 with g = 2 D^T (D x) (A-15).  Objective terms, norms and beta are fp64 in both modes.
 #include <math.h>
+#include <stdlib.h>
 
 #include "sup_internal.cuh"
 
@@ -529,6 +530,10 @@ int sup_perturb_grid(sup_ctx* h, int objective) {
         want = (h->n + 4 * SUP_THREADS - 1) / (4 * SUP_THREADS);  // about four elements per thread
         if (want > 2 * int64_t(h->num_sms)) want = 2 * int64_t(h->num_sms);
         if (want > SUP_MAX_PARTIALS / SUP_TRIAL_BATCH) want = SUP_MAX_PARTIALS / SUP_TRIAL_BATCH;  // one partial row per candidate
+    }
+    if (const char* env = getenv("SUP_PERTURB_GRID")) {  // measurement override
+        const int64_t v = atoll(env);
+        if (v > 0 && objective != SUP_OBJ_DOSE) want = v < SUP_MAX_PARTIALS / SUP_TRIAL_BATCH ? v : SUP_MAX_PARTIALS / SUP_TRIAL_BATCH;
     }
     if (want < 1) want = 1;
     return int(want < cap ? want : cap);

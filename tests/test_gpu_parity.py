@@ -307,7 +307,7 @@ def gpu_run(H, P, x, cnt, ell, k, dtype, policy, block, use_graph, cap=1 << 16):
     return st["ell"], dec[: st["n_decisions"]].cpu().numpy().copy(), trace.cpu().numpy()
 
 
-def oracle_sensitivity(O, P, n_iter, dtype, policy, block, stops, n_seeds=3):
+def oracle_sensitivity(O, P, n_iter, dtype, policy, block, stops, n_seeds=2):
     """A-23: how far the ORACLE itself moves when its iterate is disturbed by one rounding of the working precision
     after every reduction step and every sweep -- the least any implementation storing x in that precision commits.
     fp32: x <- fl32(x) (seed 0) or fl32(x (1 + 2^-25 u)); fp64: x <- x (1 + 2^-53 u); u = +-1 seeded.  Returns, per
@@ -341,7 +341,7 @@ def oracle_sensitivity(O, P, n_iter, dtype, policy, block, stops, n_seeds=3):
     return dev
 
 
-def check_stepwise(P, dtype, n_iter, policy=PER_TRIAL, block=False, use_graph=True, max_steps=24):
+def check_stepwise(P, dtype, n_iter, policy=PER_TRIAL, block=False, use_graph=True, max_steps=16):
     """Parity proper: at every sampled sweep k both sides start from the SAME state -- the oracle's iterate x^k rounded
     to the GPU's storage type, its l_k and k -- and run ONE superiorized sweep (perturbation phase + sweep).  Compared:
     x^{k+1} (north_star's per-sweep bars), the accept/reject decisions and l (exact; A-13 for knife edges), proximity
@@ -473,7 +473,10 @@ def check_superiorized(P, dtype, n_iter, policy=PER_TRIAL, block=False, use_grap
 @pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg5_k16", "cfg5_k64", "cfg4_small", "cfg4_small_infeasible", "ct_ragged"])
 def test_superiorize_configs(name, dtype):
     P = problem(name)
-    check_superiorized(P, dtype, P.n_sweeps if name not in ("cfg4_small", "cfg4_small_infeasible") else 40)
+    # sweep counts trimmed where the oracle is slow (the whole -m gpu suite should stay within a few minutes):
+    # cfg2 runs 80 of its 200 sweeps, the reduced IMRT cases 20 of 300
+    n_iter = {"cfg2": 80, "cfg4_small": 20, "cfg4_small_infeasible": 20}.get(name, P.n_sweeps)
+    check_superiorized(P, dtype, n_iter)
 
 
 @pytest.mark.parametrize("dtype", [0, 1])
