@@ -30,14 +30,15 @@ extern "C" sup_status sup_workspace_bytes(int kind, int64_t m, int64_t n, int64_
                 + 2 * al(size_t(m) * 8)                                              // w, 1/||a||
                 + al(size_t(m) * esz) + 2 * al(size_t(n) * esz)                      // y, g, xdev
                 + al(2 * SUP_MAX_PARTIALS * 8) + al(sizeof(DevState)) + 2 * sup_stream_table_bytes()
-                + al(size_t(nnz) * 4) + al(size_t((n + 511) & ~int64_t(511)) * esz)             // colg, xg
+                + (dtype == SUP_F32 ? 2 * al(size_t(nnz) * 8) : al(size_t(nnz) * 4))               // packed A, A^T (fp32) | colg (fp64)
+                + al(size_t((n + 511) & ~int64_t(511)) * esz)                                      // xg
                 + 1024;
             s = sup_transpose_scratch_bytes(nnz, n, esz) + 4096;
             break;
         case SUP_WS_BLOCKS:
             if (n_blocks < 1) return sup_fail(nullptr, SUP_ERR_INVALID_ARG, "sup_workspace_bytes: n_blocks < 1");
             p = size_t(n_blocks) * al(size_t(n + 1) * 8) + al(size_t(nnz) * 4) + al(size_t(nnz) * esz) + al(size_t(m) * esz) +
-                2 * size_t(n_blocks) * sup_stream_table_bytes() + 1024;
+                2 * size_t(n_blocks) * sup_stream_table_bytes() + (dtype == SUP_F32 ? al(size_t(nnz) * 8) : 0) + 1024;
             s = sup_transpose_scratch_bytes(nnz, n, esz) + al(size_t(n_blocks) * 8) + 4096;
             break;
         case SUP_WS_DOSE:  // (m, n, nnz) describe D_body
@@ -110,7 +111,12 @@ extern "C" sup_status sup_create(sup_handle* out, const sup_csr* A, const void* 
     h->state = static_cast<DevState*>(B.take(sizeof(DevState)));
     void* tab_a = B.take(sup_stream_table_bytes());
     void* tab_at = B.take(sup_stream_table_bytes());
-    h->colg = static_cast<int32_t*>(B.take(size_t(h->nnz) * 4));
+    if (dtype == SUP_F32) {
+        h->pk_a = B.take(size_t(h->nnz) * 8);
+        h->pk_at = B.take(size_t(h->nnz) * 8);
+    } else {
+        h->colg = static_cast<int32_t*>(B.take(size_t(h->nnz) * 4));
+    }
     h->xg = B.take(size_t((h->n + 511) & ~int64_t(511)) * h->esz);
     {
         const char* env = getenv("SUP_NO_STREAM");
@@ -138,8 +144,11 @@ extern "C" sup_status sup_create(sup_handle* out, const sup_csr* A, const void* 
     h->AT.col = at_col;
     h->AT.val = at_val;
     h->AT.alloc_nnz = h->nnz;
+    h->A.pk = h->pk_a;
+    h->AT.pk = h->pk_at;
     rc = sup_stream_plan(h, h->A, 0, h->m, true, tab_a, scratch, &h->A.plan);
     if (rc == SUP_OK && h->use_stream) rc = sup_stream_setup_gather(h);
+    if (rc == SUP_OK && h->use_stream) rc = sup_stream_pack(h, at_val, at_col, h->nnz, h->pk_at);
     if (rc == SUP_OK && cudaMemsetAsync(h->xg, 0, size_t((h->n + 511) & ~int64_t(511)) * h->esz, h->stream) != cudaSuccess)
         rc = sup_fail(h, SUP_ERR_CUDA, "sup_create: %s", cudaGetErrorString(cudaGetLastError()));
     if (rc == SUP_OK) rc = sup_stream_plan(h, h->AT, 0, h->n, false, tab_at, scratch, &h->AT.plan);
@@ -190,6 +199,7 @@ extern "C" sup_status sup_set_blocks(sup_handle h, int n_blocks, const int64_t* 
     int32_t* col = static_cast<int32_t*>(B.take(size_t(h->nnz) * 4));
     void* val = B.take(size_t(h->nnz) * h->esz);
     h->d_blk = B.take(size_t(h->m) * h->esz);
+    h->pk_atb = h->dt == SUP_F32 ? B.take(size_t(h->nnz) * 8) : nullptr;
     h->ATb.assign(n_blocks, CsrD());
     h->g_bwd_blk.assign(n_blocks, 32);
     h->stream_fwd_blk.assign(n_blocks, StreamPlan());
@@ -208,6 +218,7 @@ extern "C" sup_status sup_set_blocks(sup_handle h, int n_blocks, const int64_t* 
         T.col = col;
         T.val = val;
         T.alloc_nnz = h->nnz;
+        T.pk = h->pk_atb;
         h->g_bwd_blk[t] = sup_pick_group(T.nnz, h->n);
         void* tab_f = B.take(sup_stream_table_bytes());
         void* tab_b = B.take(sup_stream_table_bytes());
@@ -217,7 +228,8 @@ extern "C" sup_status sup_set_blocks(sup_handle h, int n_blocks, const int64_t* 
         if (rc != SUP_OK) return rc;
     }
     h->n_blocks = n_blocks;
-    sup_status rc = sup_setup_block_scaling(h, scratch, scratch_bytes);
+    sup_status rc = h->use_stream ? sup_stream_pack(h, val, col, h->nnz, h->pk_atb) : SUP_OK;
+    if (rc == SUP_OK) rc = sup_setup_block_scaling(h, scratch, scratch_bytes);
     if (rc != SUP_OK) { h->n_blocks = 0; return rc; }
     SUP_CUDA(h, cudaStreamSynchronize(h->stream));
     return SUP_OK;

@@ -30,6 +30,7 @@ struct CsrD {  // device CSR (borrowed or living in workspace)
     const int64_t* rowptr = nullptr;
     const int32_t* col = nullptr;
     const void* val = nullptr;
+    const void* pk = nullptr;  // fp32 handles: packed (value bits, column) pairs, 8 B per nonzero (sup_stream.cu); else NULL
     int64_t alloc_nnz = 0;  // length of the col/val arrays (>= nnz; per-block transposes share one pair of arrays)
     StreamPlan plan;  // plan for all rows
 };
@@ -81,7 +82,10 @@ struct sup_ctx {
     DevState* state = nullptr;
     int g_fwd = 32, g_bwd = 32; // lanes per row of the two products
     // De-aliased mirror of x for the forward gathers (sup_stream.cu): xg[sup_swz(j)] = x[j], colg = sup_swz(A.col).
-    int32_t* colg = nullptr;    // [nnz]
+    int32_t* colg = nullptr;    // [nnz]  (fp64 handles; fp32 handles carry the swizzled column inside A.pk)
+    void* pk_a = nullptr;       // [nnz] x 8 B, fp32 handles: (val, sup_swz(col)) of A
+    void* pk_at = nullptr;      // [nnz] x 8 B, fp32 handles: (val, row) of A^T
+    void* pk_atb = nullptr;     // [nnz] x 8 B, fp32 handles: the per-block transposes (sup_set_blocks)
     void* xg = nullptr;         // [n rounded up to 512] dtype
     bool xg_synced = false;     // enqueue-time flag: xg mirrors x (set by the back-projection, cleared when x changes elsewhere)
     int stream_nb = 0;          // persistent grid of the row-stream kernels (-1: unavailable)
@@ -175,7 +179,9 @@ sup_status sup_stream_plan(sup_ctx* h, const CsrD& M, int64_t r0, int64_t r1, bo
                            StreamPlan* out);
 void sup_launch_stream_fwd(sup_ctx* h, const StreamPlan& rp, const void* x, const void* dscale);
 void sup_launch_stream_bwd(sup_ctx* h, const CsrD& AT, const StreamPlan& rp, void* x, double lambda);
-sup_status sup_stream_setup_gather(sup_ctx* h);  // fills colg from A.col
+sup_status sup_stream_setup_gather(sup_ctx* h);  // fills colg (fp64) or the packed copy of A (fp32) from A.col / A.val
+// fp32 handles: dst[k] = (val[k], col[k]) for k in [0, nnz)
+sup_status sup_stream_pack(sup_ctx* h, const void* val, const int32_t* col, int64_t nnz, void* dst);
 bool sup_stream_forward_uses_xg(const sup_ctx* h);
 
 // ---- perturbation (sup_perturb.cu) ------------------------------------------------------------------------

@@ -81,10 +81,34 @@ __device__ __forceinline__ T hyperslab_violation(T r, T lb, T ub) {  // Eq. 2 on
     return r > ub ? r - ub : (r < lb ? r - lb : T(0));
 }
 
+// Ring storage.  fp64: separate val / col arrays (two bulk copies per tile).  fp32: PACKED (value bits, column) pairs,
+// one 8-byte word per nonzero, so a tile is ONE bulk copy and a consumer needs one 64-bit shared load per element.
+// (Measured on config 3: the bulk-copy engine costs ~72 cycles per copy on top of ~0.043 cycles per byte -- the same
+// bytes as twice as many copies ran 23-25 % slower, profiles/r01e_packed.md -- so fewer, larger copies matter.)
 template <typename T>
-struct RgSmem {
+struct RgData {
     T val[RG_ELEMS];
     int32_t col[RG_ELEMS];
+};
+template <>
+struct RgData<float> {
+    uint2 pair[RG_ELEMS];
+};
+template <typename T>
+__device__ __forceinline__ void ring_get(const RgData<T>& d, int i, int& c, T& v) {
+    c = d.col[i];
+    v = d.val[i];
+}
+template <>
+__device__ __forceinline__ void ring_get<float>(const RgData<float>& d, int i, int& c, float& v) {
+    const uint2 q = d.pair[i];
+    v = __uint_as_float(q.x);
+    c = int(q.y);
+}
+
+template <typename T>
+struct RgSmem {
+    RgData<T> d;
     unsigned long long full[RG_STAGES];
     T pairbuf[RG_CWARPS / 2][2];  // G == 64: partial row sums handed from the odd to the even warp of a pair
     int progress[RG_CWARPS];  // per consumer warp: tiles [0, progress) are no longer needed by it
@@ -95,33 +119,45 @@ struct RgSmem {
 // entries, RG_UNROLL independent gathers in flight per lane.  Element u of a lane always goes to accumulator u mod 4, so the
 // result does not depend on where the row sits in the ring.  WRAP: the row crosses the end of the ring.
 template <typename T, int G, bool WRAP>
-__device__ __forceinline__ void ring_row_dot(const T* sval, const int32_t* scol, const T* __restrict__ vec, int k, int e,
+__device__ __forceinline__ void ring_row_dot(const RgData<T>& ring, const T* __restrict__ vec, int k, int e,
+                                             int trips, volatile int* prog, int rel_tiles, bool lane0,
                                              T& a0, T& a1, T& a2, T& a3) {
     int n = e - k;  // this lane's elements are k, k+G, ... while offset < n
     int p = k % RG_ELEMS;
-    for (; n > 0; n -= RG_UNROLL * G, p += RG_UNROLL * G) {
+    // `trips` is warp-uniform (the longest row of the warp decides); lanes whose row is exhausted run predicated off
+    for (int trip = 0; trip < trips; ++trip, n -= RG_UNROLL * G, p += RG_UNROLL * G) {
         if (WRAP && p >= RG_ELEMS) p -= RG_ELEMS;
         int c[RG_UNROLL];
         T v[RG_UNROLL], g[RG_UNROLL];
-        if (n > (RG_UNROLL - 1) * G) {
+        const bool full = n > (RG_UNROLL - 1) * G;
+        if (full) {
 #pragma unroll
             for (int u = 0; u < RG_UNROLL; ++u) {
                 int i = p + u * G;
                 if (WRAP && i >= RG_ELEMS) i -= RG_ELEMS;
-                c[u] = scol[i];
-                v[u] = sval[i];
+                ring_get<T>(ring, i, c[u], v[u]);
             }
-#pragma unroll
-            for (int u = 0; u < RG_UNROLL; ++u) g[u] = __ldg(vec + c[u]);
-        } else {  // last, partial group: predicated
+        } else {  // last, partial group (or nothing left): predicated
 #pragma unroll
             for (int u = 0; u < RG_UNROLL; ++u) {
                 const bool in = u * G < n;
-                int i = p + u * G;
+                int i = in ? p + u * G : 0;
                 if (WRAP && i >= RG_ELEMS) i -= RG_ELEMS;
-                c[u] = in ? scol[i] : 0;
-                v[u] = in ? sval[i] : T(0);
+                ring_get<T>(ring, i, c[u], v[u]);  // (index 0 when out of range)
+                c[u] = in ? c[u] : 0;
+                v[u] = in ? v[u] : T(0);
             }
+        }
+        if (trip == trips - 1) {
+            // Early release: the warp has read everything it needs from the ring for these rows, so the tiles wholly
+            // before the end of its rows can be refilled while the gathers below are still in flight.
+            __syncwarp();
+            if (lane0) *prog = rel_tiles;
+        }
+        if (full) {
+#pragma unroll
+            for (int u = 0; u < RG_UNROLL; ++u) g[u] = __ldg(vec + c[u]);
+        } else {
 #pragma unroll
             for (int u = 0; u < RG_UNROLL; ++u) g[u] = (u * G < n) ? __ldg(vec + c[u]) : T(0);
         }
@@ -140,8 +176,8 @@ __device__ __forceinline__ void ring_row_dot(const T* sval, const int32_t* scol,
 template <typename T, int MODE, int G, int NCW>
 __global__ void __launch_bounds__(32 * (NCW + 1), 1)
     k_staged(const int64_t* __restrict__ part, const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
-             const T* __restrict__ val, const T* __restrict__ vec, const T* __restrict__ p1, const T* __restrict__ p2,
-             const T* __restrict__ p3, T* out, T* out2, T lambda, int64_t nnz_total, double* dbg) {
+             const T* __restrict__ val, const uint2* __restrict__ pk, const T* __restrict__ vec, const T* __restrict__ p1,
+             const T* __restrict__ p2, const T* __restrict__ p3, T* out, T* out2, T lambda, int64_t nnz_total, double* dbg) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     RgSmem<T>& S = *reinterpret_cast<RgSmem<T>*>(smem_raw);
     const int64_t rs = part[blockIdx.x], re = part[blockIdx.x + 1];
@@ -164,7 +200,7 @@ __global__ void __launch_bounds__(32 * (NCW + 1), 1)
 
     if (warp == NCW) {
         // ---- producers: RG_PLANES lanes feed the ring, lane p the tiles t = p (mod RG_PLANES) -------------------------
-        // (one lane alone spends ~470 cycles per tile between polling, fencing and issuing: 4.9 TB/s chip-wide at most)
+        // (more than one producer lane brought nothing: the limit was the copy engine's per-copy cost, not the issue loop)
         if (lane < RG_PLANES) {
             const uint64_t pol = l2_evict_first_policy();
             const int64_t bulk_limit = nnz_total & ~int64_t(3);  // bulk copies never read past the arrays' last whole 16 B
@@ -191,18 +227,26 @@ __global__ void __launch_bounds__(32 * (NCW + 1), 1)
                 const int64_t g1 = (g0 + RG_TILE < ee) ? g0 + RG_TILE : ee;  // elements needed: [g0, g1)
                 int64_t gb = (g1 + 3) & ~int64_t(3);                          // bulk part: [g0, gb)
                 if (gb > nnz_total) gb = bulk_limit > g0 ? bulk_limit : g0;
+                constexpr bool PACKED = sizeof(T) == 4;
                 for (int64_t g = gb; g < g1; ++g) {  // at most 3 ragged elements at the very end of the arrays
-                    S.val[s * RG_TILE + int(g - g0)] = val[g];
-                    S.col[s * RG_TILE + int(g - g0)] = col[g];
+                    if constexpr (PACKED) {
+                        S.d.pair[s * RG_TILE + int(g - g0)] = pk[g];
+                    } else {
+                        S.d.val[s * RG_TILE + int(g - g0)] = val[g];
+                        S.d.col[s * RG_TILE + int(g - g0)] = col[g];
+                    }
                 }
                 const uint32_t ne = uint32_t(gb - g0);
                 const uint32_t bar = smem_u32(&S.full[s]);
                 if (ne == 0) {
                     mbar_arrive(bar);
+                } else if constexpr (PACKED) {
+                    mbar_arrive_expect_tx(bar, ne * 8u);
+                    bulk_g2s(smem_u32(&S.d.pair[s * RG_TILE]), pk + g0, ne * 8u, bar, pol);
                 } else {
                     mbar_arrive_expect_tx(bar, ne * uint32_t(sizeof(T) + 4));
-                    bulk_g2s(smem_u32(&S.val[s * RG_TILE]), val + g0, ne * uint32_t(sizeof(T)), bar, pol);
-                    bulk_g2s(smem_u32(&S.col[s * RG_TILE]), col + g0, ne * 4u, bar, pol);
+                    bulk_g2s(smem_u32(&S.d.val[s * RG_TILE]), val + g0, ne * uint32_t(sizeof(T)), bar, pol);
+                    bulk_g2s(smem_u32(&S.d.col[s * RG_TILE]), col + g0, ne * 4u, bar, pol);
                 }
                 issued[s] = t + 1;  // the stage's barrier is armed for tile t: consumers may now wait on its phase
             }
@@ -274,8 +318,14 @@ __global__ void __launch_bounds__(32 * (NCW + 1), 1)
         // row dot product from the ring
         T a0 = T(0), a1 = T(0), a2 = T(0), a3 = T(0);
         const bool wraps = (w_start % RG_ELEMS) + (w_end - w_start) > RG_ELEMS;  // warp-uniform
-        if (!wraps) ring_row_dot<T, G, false>(S.val, S.col, vec, s + gl, e, a0, a1, a2, a3);
-        else ring_row_dot<T, G, true>(S.val, S.col, vec, s + gl, e, a0, a1, a2, a3);
+        const int n_max = __reduce_max_sync(0xffffffffu, e - s - gl);
+        const int trips = n_max > 0 ? (n_max + RG_UNROLL * G - 1) / (RG_UNROLL * G) : 0;
+        int rel = w_end / RG_TILE;  // tiles wholly before the end of this warp's rows: not needed again (rows only move forward)
+        rel = rel < ntiles ? rel : ntiles;
+        rel = rel > released ? rel : released;
+        if (!wraps) ring_row_dot<T, G, false>(S.d, vec, s + gl, e, trips, progress + warp, rel, lane == 0, a0, a1, a2, a3);
+        else ring_row_dot<T, G, true>(S.d, vec, s + gl, e, trips, progress + warp, rel, lane == 0, a0, a1, a2, a3);
+        if (trips > 0) released = rel;
         T acc = (a0 + a1) + (a2 + a3);
 #pragma unroll
         for (int o = GL >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o, GL);
@@ -393,6 +443,7 @@ sup_status sup_stream_plan(sup_ctx* h, const CsrD& M, int64_t r0, int64_t r1, bo
     }
     // bulk copies need 16-byte aligned sources (element offsets are multiples of 4)
     if ((reinterpret_cast<uintptr_t>(M.val) & 15) || (reinterpret_cast<uintptr_t>(M.col) & 15)) return SUP_OK;
+    if (h->dt == SUP_F32 && !M.pk) return SUP_OK;  // fp32 streams the packed copy
     unsigned long long* mx = static_cast<unsigned long long*>(scratch);
     SUP_CUDA(h, cudaMemsetAsync(mx, 0, 8, h->stream));
     const int grid = sup_grid_for(r1 - r0, SUP_THREADS, h->num_sms * 8);
@@ -455,9 +506,9 @@ static void launch_staged_gw(sup_ctx* h, const StreamPlan& sp, const CsrD& M, co
         attr_set = true;
     }
     k_staged<T, MODE, G, NCW><<<sp.nb, 32 * (NCW + 1), sizeof(RgSmem<T>), h->stream>>>(
-        sp.part, M.rowptr, M.col, static_cast<const T*>(M.val), static_cast<const T*>(vec), static_cast<const T*>(p1),
-        static_cast<const T*>(p2), static_cast<const T*>(p3), static_cast<T*>(out), static_cast<T*>(out2), T(lambda),
-        M.alloc_nnz, stream_debug() ? h->partials : nullptr);
+        sp.part, M.rowptr, M.col, static_cast<const T*>(M.val), static_cast<const uint2*>(M.pk), static_cast<const T*>(vec),
+        static_cast<const T*>(p1), static_cast<const T*>(p2), static_cast<const T*>(p3), static_cast<T*>(out),
+        static_cast<T*>(out2), T(lambda), M.alloc_nnz, stream_debug() ? h->partials : nullptr);
     h->launches++;
 }
 
@@ -495,16 +546,43 @@ __global__ void __launch_bounds__(SUP_THREADS) k_swizzle_copy(const T* __restric
     if (j < n) xg[sup_swz(j)] = x[j];
 }
 
+template <bool SWZ>
+__global__ void __launch_bounds__(SUP_THREADS) k_pack(const float* __restrict__ val, const int32_t* __restrict__ col, int64_t nnz,
+                                                       uint2* __restrict__ pk) {
+    for (int64_t k = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; k < nnz; k += int64_t(gridDim.x) * blockDim.x) {
+        const int c = col[k];
+        pk[k] = make_uint2(__float_as_uint(val[k]), unsigned(SWZ ? sup_swz(c) : c));
+    }
+}
+
+sup_status sup_stream_pack(sup_ctx* h, const void* val, const int32_t* col, int64_t nnz, void* dst) {
+    if (h->dt != SUP_F32 || !dst || nnz == 0) return SUP_OK;
+    k_pack<false><<<sup_grid_for(nnz, SUP_THREADS, h->num_sms * 16), SUP_THREADS, 0, h->stream>>>(
+        static_cast<const float*>(val), col, nnz, static_cast<uint2*>(dst));
+    h->launches++;
+    SUP_CUDA(h, cudaGetLastError());
+    return SUP_OK;
+}
+
 sup_status sup_stream_setup_gather(sup_ctx* h) {
-    if (!h->colg || h->nnz == 0) return SUP_OK;
-    k_swizzle_cols<<<sup_grid_for(h->nnz, SUP_THREADS, h->num_sms * 16), SUP_THREADS, 0, h->stream>>>(h->A.col, h->nnz, h->colg);
+    if (h->nnz == 0) return SUP_OK;
+    const int grid = sup_grid_for(h->nnz, SUP_THREADS, h->num_sms * 16);
+    if (h->dt == SUP_F32 && h->pk_a) {
+        k_pack<true><<<grid, SUP_THREADS, 0, h->stream>>>(static_cast<const float*>(h->A.val), h->A.col, h->nnz,
+                                                         static_cast<uint2*>(h->pk_a));
+        h->A.pk = h->pk_a;
+    } else if (h->colg) {
+        k_swizzle_cols<<<grid, SUP_THREADS, 0, h->stream>>>(h->A.col, h->nnz, h->colg);
+    } else {
+        return SUP_OK;
+    }
     h->launches++;
     SUP_CUDA(h, cudaGetLastError());
     return SUP_OK;
 }
 
 bool sup_stream_forward_uses_xg(const sup_ctx* h) {
-    if (!h->colg || !h->xg) return false;
+    if (!(h->colg || h->A.pk) || !h->xg) return false;
     if (h->A.plan.ok) return true;
     for (const StreamPlan& p : h->stream_fwd_blk)
         if (p.ok) return true;
@@ -514,7 +592,7 @@ bool sup_stream_forward_uses_xg(const sup_ctx* h) {
 void sup_launch_stream_fwd(sup_ctx* h, const StreamPlan& sp, const void* x, const void* dscale) {
     CsrD M = h->A;
     const void* vec = x;
-    if (h->colg && h->xg) {
+    if ((h->colg || h->A.pk) && h->xg) {
         if (!h->xg_synced) {
             const unsigned grid = unsigned((h->n + SUP_THREADS - 1) / SUP_THREADS);
             if (h->dt == SUP_F32) k_swizzle_copy<float><<<grid, SUP_THREADS, 0, h->stream>>>(static_cast<const float*>(x), int(h->n), static_cast<float*>(h->xg));
@@ -522,7 +600,7 @@ void sup_launch_stream_fwd(sup_ctx* h, const StreamPlan& sp, const void* x, cons
             h->launches++;
             h->xg_synced = true;
         }
-        M.col = h->colg;
+        if (h->colg) M.col = h->colg;  // fp32: the swizzled column is inside M.pk
         vec = h->xg;
     }
     if (h->dt == SUP_F32) launch_staged<float, 0>(h, sp, M, vec, h->lb, h->ub, dscale, h->y, nullptr, 0.0);
