@@ -390,7 +390,7 @@ static sup_status perturb_alone(sup_ctx* h, void* x, int kind, const int64_t* sh
     int64_t ny, nx;
     sup_status rc = check_objective(h, kind, shape, &ny, &nx);
     if (rc != SUP_OK) return rc;
-    sup_launch_begin_run(h, *ell, 0);
+    sup_launch_begin_run(h, *ell, 0, a);
     if (N > 0) {
         PerturbParams pp = {kind, ny, nx, N, beta0, a, SUP_STEP_PER_TRIAL, nullptr, nullptr, 0};
         rc = sup_launch_perturb(h, x, pp);
@@ -461,7 +461,7 @@ static sup_status run_superiorize(sup_ctx* h, void* x, int n_iter, int N, double
     P.o = *opt;
     sup_status rc = check_objective(h, opt->objective, opt->shape, &P.ny, &P.nx);
     if (rc != SUP_OK) return rc;
-    sup_launch_begin_run(h, opt->ell0, opt->k0);
+    sup_launch_begin_run(h, opt->ell0, opt->k0, a);
     h->xg_synced = false;
 
     bool graph = opt->use_graph && h->stream != nullptr && !h->graph_failed && n_iter > 1;

@@ -46,6 +46,7 @@ struct DevState {
     int warn;
     int fault;
     double f;             // objective carried by the last perturbation phase
+    double apow;          // a^l as the running fp64 product (PER_TRIAL; A-20)
     double scalar_out;    // result slot of finalize kernels (proximity / objective)
     unsigned bar_count;   // grid barrier of the perturbation kernel
     unsigned bar_gen;
@@ -199,5 +200,5 @@ sup_status sup_launch_perturb(sup_ctx* h, void* x, const PerturbParams& pp);
 void sup_launch_objective(sup_ctx* h, const void* x, int kind, int64_t ny, int64_t nx, double* out_dev);
 void sup_launch_end_sweep(sup_ctx* h, double* trace);
 void sup_launch_trace_slot(sup_ctx* h, double* trace, int slot);  // trace[it][slot] = state->scalar_out
-void sup_launch_begin_run(sup_ctx* h, int64_t ell0, int64_t k0);
+void sup_launch_begin_run(sup_ctx* h, int64_t ell0, int64_t k0, double a);
 int sup_perturb_grid(sup_ctx* h, int objective);

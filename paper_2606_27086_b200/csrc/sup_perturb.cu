@@ -11,7 +11,8 @@
 // from the same partial sums summed in the same order -- no host round trip, and the launch is capturable in a
 // CUDA graph.  z is never stored: z_p = round_T(x_p - (beta/s) g_p) is recomputed wherever it is needed.
 // Objectives: TV2D (Eq. 15; gradient A-8, shared-memory tile with halo, fused with sum g^2),
-// TV1D (A-16), DOSE ||D x||^2 with g = 2 D^T (D x) (A-15).  Objective terms, norms and beta are fp64 in both modes.
+// TV1D (A-16), DOSE ||D x||^2 with g = 2 D^T (D x) (A-15).  Objective terms, norms and beta are fp64 in both modes; a^l is the
+// running fp64 product, bit-identical to the oracle's (A-20).
 #include <math.h>
 #include <stdlib.h>
 
@@ -62,7 +63,9 @@ __device__ __forceinline__ void grid_barrier(DevState* st) {
         } else {
             unsigned spins = 0;
             while (*gen_p == gen) {
+#ifndef SUP_BARRIER_NOSLEEP
                 __nanosleep(64);
+#endif
                 if (++spins > BARRIER_SPIN_LIMIT) {  // never hang the device: flag and fall through
                     atomicOr(&st->fault, 1);
                     break;
@@ -343,6 +346,7 @@ template <typename T, int OBJ>
 __global__ void __launch_bounds__(SUP_THREADS) k_perturb(PArgs<T> A) {
     DevState* st = A.st;
     long long ell = *(volatile long long*)&st->ell;
+    double apow = *(volatile double*)&st->apow;  // a^ell, running product
     const long long k = *(volatile long long*)&st->k;
     long long ndec = *(volatile long long*)&st->n_dec;
     long long trials = 0;
@@ -383,11 +387,19 @@ __global__ void __launch_bounds__(SUP_THREADS) k_perturb(PArgs<T> A) {
         constexpr int B = OBJ == SUP_OBJ_DOSE ? 1 : SUP_TRIAL_BATCH;
         for (int trial = 0; trial < SUP_J_MAX && !accepted; trial += B) {
             double coef[B], fzb[B];
+            {
+                // a^(exponent of candidate 0) by successive multiplication from 1, like the oracle (A-20): PER_TRIAL carries
+                // the running product a^l across trials and sweeps; PER_SWEEP rebuilds a^(k+j) (k is small)
+                double ap = apow;
+                if (A.policy != SUP_STEP_PER_TRIAL) {
+                    ap = 1.0;
+                    for (long long q = 0; q < k + jloc; ++q) ap *= A.a;
+                }
 #pragma unroll
-            for (int b = 0; b < B; ++b) {
-                const double expo = A.policy == SUP_STEP_PER_TRIAL ? double(ell + b) : double(k + jloc + b);
-                const double beta = A.beta0 * pow(A.a, expo);
-                coef[b] = s > 0.0 ? beta / s : 0.0;
+                for (int b = 0; b < B; ++b) {
+                    coef[b] = s > 0.0 ? (A.beta0 * ap) / s : 0.0;
+                    ap *= A.a;
+                }
             }
             P = slot ? P1 : P0;
             slot ^= 1;
@@ -406,6 +418,7 @@ __global__ void __launch_bounds__(SUP_THREADS) k_perturb(PArgs<T> A) {
             for (int b = 0; b < B && !accepted && trial + b < SUP_J_MAX; ++b) {
                 const double fz = fzb[b];
                 ++ell;
+                apow *= A.a;
                 ++jloc;
                 ++trials;
                 const bool acc = fz <= fx;  // NaN compares false -> rejected (A-11)
@@ -434,6 +447,7 @@ __global__ void __launch_bounds__(SUP_THREADS) k_perturb(PArgs<T> A) {
     }
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         st->ell = ell;
+        st->apow = apow;
         st->n_dec = ndec;
         st->n_trials += trials;
         st->sweep_trials += trials;
@@ -599,8 +613,9 @@ void sup_launch_trace_slot(sup_ctx* h, double* trace, int slot) {
     h->launches++;
 }
 
-__global__ void k_begin_run(DevState* st, long long ell0, long long k0) {
+__global__ void k_begin_run(DevState* st, long long ell0, long long k0, double apow0) {
     st->ell = ell0;
+    st->apow = apow0;
     st->k = k0;
     st->it = 0;
     st->n_trials = 0;
@@ -610,7 +625,11 @@ __global__ void k_begin_run(DevState* st, long long ell0, long long k0) {
     st->fault = 0;
     st->bar_count = 0;
 }
-void sup_launch_begin_run(sup_ctx* h, int64_t ell0, int64_t k0) {
-    k_begin_run<<<1, 1, 0, h->stream>>>(h->state, ell0, k0);
+void sup_launch_begin_run(sup_ctx* h, int64_t ell0, int64_t k0, double a) {
+    // a^l0: exactly 1 for a fresh run, so the running product below reproduces the oracle's step sizes bit for bit (A-20)
+    double apow0 = 1.0;
+    for (int64_t i = 0; i < ell0 && i < 100000; ++i) apow0 *= a;
+    if (ell0 >= 100000) apow0 = pow(a, double(ell0));
+    k_begin_run<<<1, 1, 0, h->stream>>>(h->state, ell0, k0, apow0);
     h->launches++;
 }
