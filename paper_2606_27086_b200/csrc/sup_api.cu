@@ -28,7 +28,7 @@ extern "C" sup_status sup_workspace_bytes(int kind, int64_t m, int64_t n, int64_
             p = al(size_t(n + 1) * 8) + al(size_t(nnz) * 4) + al(size_t(nnz) * esz)  // A^T
                 + al(size_t(m) * esz)                                                // d
                 + 2 * al(size_t(m) * 8)                                              // w, 1/||a||
-                + al(size_t(m) * esz) + 2 * al(size_t(n) * esz)                      // y, g, xdev
+                + al(size_t(m) * esz) + 4 * al(size_t(n) * esz)                      // y, g, xdev, x2, g2
                 + al(2 * SUP_MAX_PARTIALS * 8) + al(sizeof(DevState)) + 2 * sup_stream_table_bytes()
                 + (dtype == SUP_F32 ? 2 * al(size_t(nnz) * 8) : al(size_t(nnz) * 4))               // packed A, A^T (fp32) | colg (fp64)
                 + al(size_t((n + 511) & ~int64_t(511)) * esz)                                      // xg
@@ -107,6 +107,8 @@ extern "C" sup_status sup_create(sup_handle* out, const sup_csr* A, const void* 
     h->y = B.take(size_t(h->m) * h->esz);
     h->g = B.take(size_t(h->n) * h->esz);
     h->xdev = B.take(size_t(h->n) * h->esz);
+    h->x2 = B.take(size_t(h->n) * h->esz);
+    h->g2 = B.take(size_t(h->n) * h->esz);
     h->partials = static_cast<double*>(B.take(2 * SUP_MAX_PARTIALS * 8));
     h->state = static_cast<DevState*>(B.take(sizeof(DevState)));
     void* tab_a = B.take(sup_stream_table_bytes());

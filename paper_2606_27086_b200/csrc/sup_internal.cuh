@@ -78,6 +78,8 @@ struct sup_ctx {
     double* invnorm = nullptr;  // [m] 1/||a_i|| (0 for empty rows)
     void* y = nullptr;          // [m] dtype: scaled violation d_i c_i
     void* g = nullptr;          // [n] dtype: gradient of the objective
+    void* x2 = nullptr;         // [n] dtype: second iterate buffer of the perturbation kernel (deferred accepted steps)
+    void* g2 = nullptr;         // [n] dtype: second gradient buffer
     void* xdev = nullptr;       // [n] dtype: staging copy of x for sup_superiorize_host
     double* partials = nullptr; // [2][SUP_MAX_PARTIALS]
     DevState* state = nullptr;

@@ -27,6 +27,8 @@ template <typename T>
 struct PArgs {
     T* x;
     T* g;
+    T* x2;  // second iterate / gradient buffers (TV objectives: an accepted step is applied inside the next gradient pass)
+    T* g2;
     int64_t n, ny, nx;
     int N;
     double beta0, a;
@@ -135,6 +137,11 @@ __device__ __forceinline__ double zval(const T* __restrict__ x, const T* __restr
     return double(T(fma(-coef, double(__ldcg(g + p)), xv)));  // z rounded to the storage type, as it would be stored
 }
 
+// sqrt(d) and 1/sqrt(d) for the TV terms via rsqrt (1 ulp, a short MUFU + Newton chain) instead of IEEE sqrt and
+// divide, whose dependent fp64 sequences were the latency of every phase of this kernel: t = d * rsqrt(d) is within
+// 2 ulp of sqrt(d), far inside the fp64 parity bar (1e-10) and the knife-edge threshold of the accept test (1e-12).
+__device__ __forceinline__ double tv_norm(double d) { return d > 0.0 ? d * rsqrt(d) : 0.0; }
+
 // ---- objective value of z = x - coef g : this thread's share (not yet reduced) ------------------------------
 template <typename T>
 __device__ double tv2d_share(const PArgs<T>& A, double coef) {
@@ -147,7 +154,7 @@ __device__ double tv2d_share(const PArgs<T>& A, double coef) {
         const int64_t p = i * A.nx + j;
         const double z00 = zval(A.x, A.g, coef, p), z10 = zval(A.x, A.g, coef, p + A.nx), z01 = zval(A.x, A.g, coef, p + 1);
         const double dx = z10 - z00, dy = z01 - z00;
-        acc += sqrt(dx * dx + dy * dy);
+        acc += tv_norm(dx * dx + dy * dy);
     }
     return acc;
 }
@@ -172,7 +179,7 @@ __device__ void tv2d_share_batch(const PArgs<T>& A, const double* coef, double* 
             const double z10 = c == 0.0 ? x10 : double(T(fma(-c, g10, x10)));
             const double z01 = c == 0.0 ? x01 : double(T(fma(-c, g01, x01)));
             const double dx = z10 - z00, dy = z01 - z00;
-            acc[b] += sqrt(dx * dx + dy * dy);
+            acc[b] += tv_norm(dx * dx + dy * dy);
         }
     }
 }
@@ -252,8 +259,9 @@ __device__ __forceinline__ double objective_share(const PArgs<T>& A, double coef
 // ---- gradient: writes g, returns this thread's share of sum g^2 ----------------------------------------------
 // TV2D (A-8): g_ij = -(dx_ij+dy_ij)/t_ij [i<ny-1, j<nx-1] + dx_{i-1,j}/t_{i-1,j} [i>=1, j<nx-1] + dy_{i,j-1}/t_{i,j-1} [j>=1, i<ny-1];
 // a term with t = 0 contributes 0 (A-9).  One CTA stages a TILE_H x TILE_W tile plus a one-pixel halo in shared memory.
+// Reads the iterate as z = x - pend * g (pend = 0: x itself), writes z to xo when a step is pending, the gradient of z to go.
 template <typename T>
-__device__ double tv2d_grad_share(const PArgs<T>& A) {
+__device__ double tv2d_grad_share(const PArgs<T>& A, double pend, T* __restrict__ xo, T* __restrict__ go) {
     __shared__ double tile[TILE_H + 2][TILE_W + 2 + 1];
     const int64_t ny = A.ny, nx = A.nx;
     const int64_t tiles_y = (ny + TILE_H - 1) / TILE_H, tiles_x = (nx + TILE_W - 1) / TILE_W;
@@ -265,7 +273,7 @@ __device__ double tv2d_grad_share(const PArgs<T>& A) {
         for (int q = threadIdx.x; q < (TILE_H + 2) * (TILE_W + 2); q += SUP_THREADS) {
             const int li = q / (TILE_W + 2), lj = q - li * (TILE_W + 2);
             const int64_t i = i0 + li, j = j0 + lj;
-            tile[li][lj] = (i >= 0 && i < ny && j >= 0 && j < nx) ? double(__ldcg(A.x + i * nx + j)) : 0.0;
+            tile[li][lj] = (i >= 0 && i < ny && j >= 0 && j < nx) ? zval(A.x, A.g, pend, i * nx + j) : 0.0;
         }
         __syncthreads();
         for (int q = threadIdx.x; q < TILE_H * TILE_W; q += SUP_THREADS) {
@@ -276,23 +284,24 @@ __device__ double tv2d_grad_share(const PArgs<T>& A) {
             const double c = tile[li][lj];
             if (i + 1 < ny && j + 1 < nx) {  // own term (i, j)
                 const double dx = tile[li + 1][lj] - c, dy = tile[li][lj + 1] - c;
-                const double tt = sqrt(dx * dx + dy * dy);
-                if (tt > 0.0) gv -= (dx + dy) / tt;
+                const double d2 = dx * dx + dy * dy;
+                if (d2 > 0.0) gv -= (dx + dy) * rsqrt(d2);
             }
             if (i >= 1 && j + 1 < nx) {  // term (i-1, j): dx_{i-1,j} = X_ij - X_{i-1,j}
                 const double b = tile[li - 1][lj];
                 const double dx = c - b, dy = tile[li - 1][lj + 1] - b;
-                const double tt = sqrt(dx * dx + dy * dy);
-                if (tt > 0.0) gv += dx / tt;
+                const double d2 = dx * dx + dy * dy;
+                if (d2 > 0.0) gv += dx * rsqrt(d2);
             }
             if (j >= 1 && i + 1 < ny) {  // term (i, j-1): dy_{i,j-1} = X_ij - X_{i,j-1}
                 const double b = tile[li][lj - 1];
                 const double dx = tile[li + 1][lj - 1] - b, dy = c - b;
-                const double tt = sqrt(dx * dx + dy * dy);
-                if (tt > 0.0) gv += dy / tt;
+                const double d2 = dx * dx + dy * dy;
+                if (d2 > 0.0) gv += dy * rsqrt(d2);
             }
             const T gs = T(gv);
-            A.g[i * nx + j] = gs;
+            go[i * nx + j] = gs;
+            if (pend != 0.0) xo[i * nx + j] = T(c);  // c is z rounded to T already
             acc += double(gs) * double(gs);
         }
     }
@@ -300,20 +309,21 @@ __device__ double tv2d_grad_share(const PArgs<T>& A) {
 }
 
 template <typename T>
-__device__ double tv1d_grad_share(const PArgs<T>& A) {
+__device__ double tv1d_grad_share(const PArgs<T>& A, double pend, T* __restrict__ xo, T* __restrict__ go) {
     double acc = 0.0;
     for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q < A.n; q += int64_t(gridDim.x) * blockDim.x) {
-        const double c = double(__ldcg(A.x + q));
+        const double c = zval(A.x, A.g, pend, q);
         double gv = 0.0;
         if (q >= 1) {
-            const double dl = c - double(__ldcg(A.x + q - 1));
+            const double dl = c - zval(A.x, A.g, pend, q - 1);
             gv += double((dl > 0.0) - (dl < 0.0));
         }
         if (q + 1 < A.n) {
-            const double dr = double(__ldcg(A.x + q + 1)) - c;
+            const double dr = zval(A.x, A.g, pend, q + 1) - c;
             gv -= double((dr > 0.0) - (dr < 0.0));
         }
-        A.g[q] = T(gv);
+        go[q] = T(gv);
+        if (pend != 0.0) xo[q] = T(c);
         acc += gv * gv;
     }
     return acc;
@@ -343,7 +353,24 @@ __device__ double dose_grad_share(const PArgs<T>& A) {
 
 // ---- the perturbation phase ----------------------------------------------------------------------------------
 template <typename T, int OBJ>
-__global__ void __launch_bounds__(SUP_THREADS) k_perturb(PArgs<T> A) {
+__global__ void __launch_bounds__(SUP_THREADS) k_perturb(PArgs<T> Ain) {
+    // TV objectives: an accepted step is not written out at once.  It stays pending (x^{k,n+1} = x - pend g) and is applied
+    // inside the next gradient pass, which reads z on the fly and writes z and its gradient to the SECOND pair of
+    // buffers (the halo of a tile needs the neighbours' old x and g, so it cannot be done in place).  That removes one
+    // pass and one grid barrier per reduction step; the arithmetic, z = round_T(x - coef g), is unchanged.
+    const PArgs<T>& A = Ain;
+    T* xc = Ain.x;   // current iterate / gradient buffers and the other pair
+    T* gc = Ain.g;
+    T* xo = Ain.x2;
+    T* go = Ain.g2;
+    auto view = [&]() {  // the argument block with the current buffers
+        PArgs<T> V = Ain;
+        V.x = xc;
+        V.g = gc;
+        return V;
+    };
+    double pend = 0.0;
+    constexpr bool DEFER = OBJ == SUP_OBJ_TV2D || OBJ == SUP_OBJ_TV1D;
     DevState* st = A.st;
     long long ell = *(volatile long long*)&st->ell;
     double apow = *(volatile double*)&st->apow;  // a^ell, running product
@@ -356,7 +383,7 @@ __global__ void __launch_bounds__(SUP_THREADS) k_perturb(PArgs<T> A) {
     double* P1 = A.partials + SUP_MAX_PARTIALS;
 
     // fx = f(x)
-    double sh = cta_sum(objective_share<T, OBJ>(A, 0.0));
+    double sh = cta_sum(objective_share<T, OBJ>(view(), 0.0));
     if (threadIdx.x == 0) P0[blockIdx.x] = sh;
     grid_barrier(st);
     double fx = reduce_partials(P0);
@@ -367,16 +394,27 @@ __global__ void __launch_bounds__(SUP_THREADS) k_perturb(PArgs<T> A) {
         double* P = slot ? P1 : P0;
         slot ^= 1;
         if (OBJ == SUP_OBJ_DOSE) {  // r = D x first
-            dose_share(A, 0.0, true);
+            dose_share(view(), 0.0, true);
             grid_barrier(st);
-            sh = cta_sum(dose_grad_share(A));
+            sh = cta_sum(dose_grad_share(view()));
         } else if (OBJ == SUP_OBJ_TV2D) {
-            sh = cta_sum(tv2d_grad_share(A));
+            sh = cta_sum(tv2d_grad_share(view(), pend, xo, go));
         } else {
-            sh = cta_sum(tv1d_grad_share(A));
+            sh = cta_sum(tv1d_grad_share(view(), pend, xo, go));
         }
         if (threadIdx.x == 0) P[blockIdx.x] = sh;
         grid_barrier(st);
+        if (DEFER) {  // the new gradient (and, if a step was pending, the new iterate) live in the other buffers now
+            T* t = gc;
+            gc = go;
+            go = t;
+            if (pend != 0.0) {
+                t = xc;
+                xc = xo;
+                xo = t;
+                pend = 0.0;
+            }
+        }
         const double s = sqrt(reduce_partials(P));
         bool accepted = false;
         long long jloc = 0;
@@ -404,11 +442,11 @@ __global__ void __launch_bounds__(SUP_THREADS) k_perturb(PArgs<T> A) {
             P = slot ? P1 : P0;
             slot ^= 1;
             if (B == 1) {
-                fzb[0] = cta_sum(objective_share<T, OBJ>(A, coef[0]));
+                fzb[0] = cta_sum(objective_share<T, OBJ>(view(), coef[0]));
                 if (threadIdx.x == 0) P[blockIdx.x] = fzb[0];
             } else {
-                if (OBJ == SUP_OBJ_TV2D) tv2d_share_batch<T, B>(A, coef, fzb);
-                else tv1d_share_batch<T, B>(A, coef, fzb);
+                if (OBJ == SUP_OBJ_TV2D) tv2d_share_batch<T, B>(view(), coef, fzb);
+                else tv1d_share_batch<T, B>(view(), coef, fzb);
                 cta_sum_batch<B>(fzb);
                 if (threadIdx.x < B) P[threadIdx.x * (SUP_MAX_PARTIALS / B) + blockIdx.x] = fzb[threadIdx.x];
             }
@@ -432,10 +470,17 @@ __global__ void __launch_bounds__(SUP_THREADS) k_perturb(PArgs<T> A) {
                 ++ndec;
                 if (acc) {
                     const double cf = coef[b];
-                    if (cf != 0.0)
-                        for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q < A.n; q += int64_t(gridDim.x) * blockDim.x)
-                            A.x[q] = T(zval(A.x, A.g, cf, q));
-                    grid_barrier(st);  // x^{k,n+1} visible to everyone before the next gradient
+                    if (DEFER) {
+                        pend = cf;
+#ifdef SUP_DEFER_DEBUG
+                        grid_barrier(st);
+#endif
+                    } else {
+                        if (cf != 0.0)
+                            for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q < A.n; q += int64_t(gridDim.x) * blockDim.x)
+                                xc[q] = T(zval(xc, gc, cf, q));
+                        grid_barrier(st);  // x^{k,n+1} visible to everyone before the next gradient
+                    }
                     fx = fz;
                     accepted = true;
                 }
@@ -444,6 +489,10 @@ __global__ void __launch_bounds__(SUP_THREADS) k_perturb(PArgs<T> A) {
         }
         if (!accepted) warn |= 1;  // A-12: step skipped
         if (*(volatile int*)&st->fault & 1) break;
+    }
+    if (DEFER && (pend != 0.0 || xc != Ain.x)) {  // leave the final iterate in the caller's x (element-wise: no barrier needed)
+        for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q < A.n; q += int64_t(gridDim.x) * blockDim.x)
+            Ain.x[q] = T(zval(xc, gc, pend, q));
     }
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         st->ell = ell;
@@ -493,6 +542,8 @@ static PArgs<T> make_args(sup_ctx* h, void* x, const PerturbParams& pp) {
     PArgs<T> A;
     A.x = static_cast<T*>(x);
     A.g = static_cast<T*>(h->g);
+    A.x2 = static_cast<T*>(h->x2);
+    A.g2 = static_cast<T*>(h->g2);
     A.n = h->n;
     A.ny = pp.ny;
     A.nx = pp.nx;
