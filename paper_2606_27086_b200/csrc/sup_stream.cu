@@ -32,7 +32,12 @@
 #ifndef RG_STAGES
 #define RG_STAGES 16
 #endif
-#define RG_ELEMS (RG_TILE * RG_STAGES)      // ring capacity in elements (need not be a power of two)
+#ifndef RG_STAGES_FWD
+#define RG_STAGES_FWD 20                    // fp32 forward product: a deeper ring (5.00 -> 5.15 TB/s); the back-projection needs that
+#endif                                      // shared memory as L1 for its y gathers (20 stages there: 5.10 -> 3.78 TB/s)
+// stages of the ring of k_staged<T, MODE>; the ring capacity STG * RG_TILE need not be a power of two
+template <typename T, int MODE>
+__host__ __device__ constexpr int rg_stages() { return (MODE == 0 && sizeof(T) == 4) ? RG_STAGES_FWD : RG_STAGES; }
 #define RG_CWARPS 16                        // consumer warps
 #define RG_THREADS (32 * (RG_CWARPS + 1))   // + producer warp
 #ifndef RG_PLANES
@@ -85,44 +90,45 @@ __device__ __forceinline__ T hyperslab_violation(T r, T lb, T ub) {  // Eq. 2 on
 // one 8-byte word per nonzero, so a tile is ONE bulk copy and a consumer needs one 64-bit shared load per element.
 // (Measured on config 3: the bulk-copy engine costs ~72 cycles per copy on top of ~0.043 cycles per byte -- the same
 // bytes as twice as many copies ran 23-25 % slower, profiles/r01e_packed.md -- so fewer, larger copies matter.)
-template <typename T>
+template <typename T, int STG>
 struct RgData {
-    T val[RG_ELEMS];
-    int32_t col[RG_ELEMS];
+    T val[STG * RG_TILE];
+    int32_t col[STG * RG_TILE];
 };
-template <>
-struct RgData<float> {
-    uint2 pair[RG_ELEMS];
+template <int STG>
+struct RgData<float, STG> {
+    uint2 pair[STG * RG_TILE];
 };
-template <typename T>
-__device__ __forceinline__ void ring_get(const RgData<T>& d, int i, int& c, T& v) {
+template <int STG>
+__device__ __forceinline__ void ring_get(const RgData<double, STG>& d, int i, int& c, double& v) {
     c = d.col[i];
     v = d.val[i];
 }
-template <>
-__device__ __forceinline__ void ring_get<float>(const RgData<float>& d, int i, int& c, float& v) {
+template <int STG>
+__device__ __forceinline__ void ring_get(const RgData<float, STG>& d, int i, int& c, float& v) {
     const uint2 q = d.pair[i];
     v = __uint_as_float(q.x);
     c = int(q.y);
 }
 
-template <typename T>
+template <typename T, int STG>
 struct RgSmem {
-    RgData<T> d;
-    unsigned long long full[RG_STAGES];
+    RgData<T, STG> d;
+    unsigned long long full[STG];
     T pairbuf[RG_CWARPS / 2][2];  // G == 64: partial row sums handed from the odd to the even warp of a pair
     int progress[RG_CWARPS];  // per consumer warp: tiles [0, progress) are no longer needed by it
-    int issued[RG_STAGES];    // per stage: 1 + the tile its barrier is currently armed for (0: none yet)
+    int issued[STG];          // per stage: 1 + the tile its barrier is currently armed for (0: none yet)
 };
 
 // Dot product of the ring elements k, k+G, k+2G, ... < e (offsets relative to the stream base) with gathered vec
 // entries, RG_UNROLL independent gathers in flight per lane.  Element u of a lane always goes to accumulator u mod 4, so the
 // result does not depend on where the row sits in the ring.  WRAP: the row crosses the end of the ring.
-template <typename T, int G, bool WRAP>
-__device__ __forceinline__ void ring_row_dot(const RgData<T>& ring, const T* __restrict__ vec, int k, int e,
+template <typename T, int G, bool WRAP, int STG>
+__device__ __forceinline__ void ring_row_dot(const RgData<T, STG>& ring, const T* __restrict__ vec, int k, int e,
                                              int trips, volatile int* prog, int rel_tiles, bool lane0,
                                              T& a0, T& a1, T& a2, T& a3) {
     int n = e - k;  // this lane's elements are k, k+G, ... while offset < n
+    constexpr int RG_ELEMS = STG * RG_TILE;
     int p = k % RG_ELEMS;
     // `trips` is warp-uniform (the longest row of the warp decides); lanes whose row is exhausted run predicated off
     for (int trip = 0; trip < trips; ++trip, n -= RG_UNROLL * G, p += RG_UNROLL * G) {
@@ -135,7 +141,7 @@ __device__ __forceinline__ void ring_row_dot(const RgData<T>& ring, const T* __r
             for (int u = 0; u < RG_UNROLL; ++u) {
                 int i = p + u * G;
                 if (WRAP && i >= RG_ELEMS) i -= RG_ELEMS;
-                ring_get<T>(ring, i, c[u], v[u]);
+                ring_get(ring, i, c[u], v[u]);
             }
         } else {  // last, partial group (or nothing left): predicated
 #pragma unroll
@@ -143,7 +149,7 @@ __device__ __forceinline__ void ring_row_dot(const RgData<T>& ring, const T* __r
                 const bool in = u * G < n;
                 int i = in ? p + u * G : 0;
                 if (WRAP && i >= RG_ELEMS) i -= RG_ELEMS;
-                ring_get<T>(ring, i, c[u], v[u]);  // (index 0 when out of range)
+                ring_get(ring, i, c[u], v[u]);  // (index 0 when out of range)
                 c[u] = in ? c[u] : 0;
                 v[u] = in ? v[u] : T(0);
             }
@@ -179,7 +185,9 @@ __global__ void __launch_bounds__(32 * (NCW + 1), 1)
              const T* __restrict__ val, const uint2* __restrict__ pk, const T* __restrict__ vec, const T* __restrict__ p1,
              const T* __restrict__ p2, const T* __restrict__ p3, T* out, T* out2, T lambda, int64_t nnz_total, double* dbg) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    RgSmem<T>& S = *reinterpret_cast<RgSmem<T>*>(smem_raw);
+    constexpr int STG = rg_stages<T, MODE>();
+    constexpr int RG_ELEMS = STG * RG_TILE;
+    RgSmem<T, STG>& S = *reinterpret_cast<RgSmem<T, STG>*>(smem_raw);
     const int64_t rs = part[blockIdx.x], re = part[blockIdx.x + 1];
     if (rs >= re) return;
     const int64_t es = rowptr[rs], ee = rowptr[re];
@@ -189,9 +197,9 @@ __global__ void __launch_bounds__(32 * (NCW + 1), 1)
     const long long t_begin = clock64();
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < RG_STAGES; ++s) mbar_init(smem_u32(&S.full[s]), 1);
+        for (int s = 0; s < STG; ++s) mbar_init(smem_u32(&S.full[s]), 1);
         for (int w = 0; w < NCW; ++w) S.progress[w] = 0;
-        for (int st = 0; st < RG_STAGES; ++st) S.issued[st] = 0;
+        for (int st = 0; st < STG; ++st) S.issued[st] = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -206,8 +214,8 @@ __global__ void __launch_bounds__(32 * (NCW + 1), 1)
             const int64_t bulk_limit = nnz_total & ~int64_t(3);  // bulk copies never read past the arrays' last whole 16 B
             int freed = 0;                                        // min over the consumer warps' progress
             for (int t = lane; t < ntiles; t += RG_PLANES) {
-                const int s = t % RG_STAGES;
-                if (t >= RG_STAGES && freed <= t - RG_STAGES) {
+                const int s = t % STG;
+                if (t >= STG && freed <= t - STG) {
                     const long long t0 = clock64();
                     for (;;) {
                         int mn = progress[0];
@@ -217,7 +225,7 @@ __global__ void __launch_bounds__(32 * (NCW + 1), 1)
                             mn = p < mn ? p : mn;
                         }
                         freed = mn;
-                        if (freed > t - RG_STAGES) break;
+                        if (freed > t - STG) break;
                         if (clock64() - t0 > RG_TIMEOUT) __trap();
                     }
                     // the consumers' reads of the stage (generic proxy) precede the bulk write (async proxy)
@@ -299,18 +307,18 @@ __global__ void __launch_bounds__(32 * (NCW + 1), 1)
             released = t_start;
             if (lane == 0) progress[warp] = t_start;
         }
-        // Wait for the tiles this warp's rows span (span <= RG_STAGES - 1 tiles by the plan): first until the stage is
+        // Wait for the tiles this warp's rows span (span <= STG - 1 tiles by the plan): first until the stage is
         // armed for THAT tile (so the phase parity is unambiguous), then on the stage's mbarrier (a hardware wait).
         if (w_end > w_start) {
             const int t_hi = (w_end - 1) / RG_TILE;
             for (int t = seen > t_start ? seen : t_start; t <= t_hi; ++t) {
-                const int st = t % RG_STAGES;
+                const int st = t % STG;
                 if (issued[st] != t + 1) {
                     const long long t0 = clock64();
                     while (issued[st] != t + 1)
                         if (clock64() - t0 > RG_TIMEOUT) __trap();
                 }
-                mbar_wait(smem_u32(&S.full[st]), (t / RG_STAGES) & 1);
+                mbar_wait(smem_u32(&S.full[st]), (t / STG) & 1);
             }
             seen = seen > t_hi + 1 ? seen : t_hi + 1;
         }
@@ -323,8 +331,8 @@ __global__ void __launch_bounds__(32 * (NCW + 1), 1)
         int rel = w_end / RG_TILE;  // tiles wholly before the end of this warp's rows: not needed again (rows only move forward)
         rel = rel < ntiles ? rel : ntiles;
         rel = rel > released ? rel : released;
-        if (!wraps) ring_row_dot<T, G, false>(S.d, vec, s + gl, e, trips, progress + warp, rel, lane == 0, a0, a1, a2, a3);
-        else ring_row_dot<T, G, true>(S.d, vec, s + gl, e, trips, progress + warp, rel, lane == 0, a0, a1, a2, a3);
+        if (!wraps) ring_row_dot<T, G, false, STG>(S.d, vec, s + gl, e, trips, progress + warp, rel, lane == 0, a0, a1, a2, a3);
+        else ring_row_dot<T, G, true, STG>(S.d, vec, s + gl, e, trips, progress + warp, rel, lane == 0, a0, a1, a2, a3);
         if (trips > 0) released = rel;
         T acc = (a0 + a1) + (a2 + a3);
 #pragma unroll
@@ -395,12 +403,12 @@ size_t sup_stream_table_bytes() { return ((size_t(SUP_STREAM_NBMAX) + 1) * 8 + 2
 
 template <typename T, int MODE>
 static int staged_occupancy() {
-    if (cudaFuncSetAttribute(k_staged<T, MODE, 32, RG_CWARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(sizeof(RgSmem<T>))) != cudaSuccess) {
+    if (cudaFuncSetAttribute(k_staged<T, MODE, 32, RG_CWARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(sizeof(RgSmem<T, rg_stages<T, MODE>()>))) != cudaSuccess) {
         cudaGetLastError();
         return 0;
     }
     int occ = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_staged<T, MODE, 32, RG_CWARPS>, RG_THREADS, sizeof(RgSmem<T>)) != cudaSuccess) {
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_staged<T, MODE, 32, RG_CWARPS>, RG_THREADS, sizeof(RgSmem<T, rg_stages<T, MODE>()>)) != cudaSuccess) {
         cudaGetLastError();
         return 0;
     }
@@ -502,10 +510,10 @@ static void launch_staged_gw(sup_ctx* h, const StreamPlan& sp, const CsrD& M, co
                              const void* p3, void* out, void* out2, double lambda) {
     static bool attr_set = false;  // per instantiation: opt in to > 48 KB of dynamic shared memory once
     if (!attr_set) {
-        cudaFuncSetAttribute(k_staged<T, MODE, G, NCW>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(sizeof(RgSmem<T>)));
+        cudaFuncSetAttribute(k_staged<T, MODE, G, NCW>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(sizeof(RgSmem<T, rg_stages<T, MODE>()>)));
         attr_set = true;
     }
-    k_staged<T, MODE, G, NCW><<<sp.nb, 32 * (NCW + 1), sizeof(RgSmem<T>), h->stream>>>(
+    k_staged<T, MODE, G, NCW><<<sp.nb, 32 * (NCW + 1), sizeof(RgSmem<T, rg_stages<T, MODE>()>), h->stream>>>(
         sp.part, M.rowptr, M.col, static_cast<const T*>(M.val), static_cast<const uint2*>(M.pk), static_cast<const T*>(vec),
         static_cast<const T*>(p1), static_cast<const T*>(p2), static_cast<const T*>(p3), static_cast<T*>(out),
         static_cast<T*>(out2), T(lambda), M.alloc_nnz, stream_debug() ? h->partials : nullptr);

@@ -341,7 +341,7 @@ def oracle_sensitivity(O, P, n_iter, dtype, policy, block, stops, n_seeds=2):
     return dev
 
 
-def check_stepwise(P, dtype, n_iter, policy=PER_TRIAL, block=False, use_graph=True, max_steps=16):
+def check_stepwise(P, dtype, n_iter, policy=PER_TRIAL, block=False, use_graph=True, max_steps=12):
     """Parity proper: at every sampled sweep k both sides start from the SAME state -- the oracle's iterate x^k rounded
     to the GPU's storage type, its l_k and k -- and run ONE superiorized sweep (perturbation phase + sweep).  Compared:
     x^{k+1} (north_star's per-sweep bars), the accept/reject decisions and l (exact; A-13 for knife edges), proximity
@@ -474,8 +474,8 @@ def check_superiorized(P, dtype, n_iter, policy=PER_TRIAL, block=False, use_grap
 def test_superiorize_configs(name, dtype):
     P = problem(name)
     # sweep counts trimmed where the oracle is slow (the whole -m gpu suite should stay within a few minutes):
-    # cfg2 runs 80 of its 200 sweeps, the reduced IMRT cases 20 of 300
-    n_iter = {"cfg2": 80, "cfg4_small": 20, "cfg4_small_infeasible": 20}.get(name, P.n_sweeps)
+    # cfg2 runs 60 of its 200 sweeps, the reduced IMRT cases 20 of 300
+    n_iter = {"cfg2": 60, "cfg4_small": 20, "cfg4_small_infeasible": 20}.get(name, P.n_sweeps)
     check_superiorized(P, dtype, n_iter)
 
 
