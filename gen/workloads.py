@@ -294,7 +294,9 @@ def config4_imrt(scale=1.0, infeasible=False, n_sweeps=300, N=3, seed=SEED0 + 4)
     Zg, Yg, Xg = np.meshgrid(Z, Y, X, indexing="ij")
     body = (Xg / 240.0) ** 2 + (Yg / 240.0) ** 2 + (Zg / 150.0) ** 2 <= 1.0
     r_ptv, r1, r2 = 30.0, 20.0, 15.0
-    d1 = (r_ptv + r1 - 5.0) if infeasible else 65.0
+    # the infeasible variant overlaps OAR1 and the PTV by 5 mm (BASELINE.json); on the coarse test grids (scale < 1, voxels
+    # up to 20 mm) by at least 1.6 voxels, so that some voxel centres do fall in both structures
+    d1 = (r_ptv + r1 - max(5.0, 1.6 * h)) if infeasible else 65.0
     d2 = 60.0
     while True:
         a1, a2 = rng.uniform(0, 2 * np.pi, 2)
