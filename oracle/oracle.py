@@ -162,9 +162,10 @@ class Oracle:
                     warn=warn.value)
 
     def superiorize(self, x0, n_iter, N, beta0, a, lam=1.0, policy=PER_TRIAL, block=False, snapshots=(), ell0=0,
-                    forced=None, kind=None, shape=None, cap=1 << 22, k0=0):
+                    forced=None, kind=None, shape=None, cap=1 << 22, k0=0, n_restart=0):
         """Algorithm 1 for n_iter sweeps (absolute sweep indices k0 .. k0+n_iter-1; k0 only matters to PER_SWEEP).
         snapshots: sweep counts (1-based: 'after s sweeps') at which x is copied.
+        n_restart > 0: restarted perturbations, l <- r at the start of sweep r * n_restart (A-24).
         Returns dict(x, ell, trace[n_iter,4] = (prox0, f, trials, ell), snaps{count: x}, decisions, margins, warn)."""
         x = np.array(x0, np.float64)
         ell = _i64(int(ell0))
@@ -188,7 +189,7 @@ class Oracle:
                 _p(self.w), _p(self.rho), _p(self.d), _p(self.lo), _p(self.hi), _dbl(lam), _int(nb),
                 _p(self.block_rowptr) if nb else None, *self._obj_args(kind, shape), _p(x), ctypes.byref(ell), _i64(k0 + k),
                 _int(cnt), _int(N), _dbl(beta0), _dbl(a), _int(policy), _p(tr), _p(dec), _p(mar), _i64(cap),
-                ctypes.byref(ndec), _p(forced_a))
+                ctypes.byref(ndec), _p(forced_a), _i64(int(n_restart)))
             trace[k:stop] = tr
             k = stop
             snaps[stop] = x.copy()

@@ -302,7 +302,7 @@ int orc_superiorize(int64_t m, int64_t n, const int64_t* rowptr, const int32_t* 
                     int obj_kind, int64_t ny, int64_t nx, int64_t md, const int64_t* d_rowptr, const int32_t* d_col,
                     const double* d_val, double* x, int64_t* ell, int64_t k0, int n_iter, int N, double beta0,
                     double a, int policy, double* trace, int8_t* decisions, double* margins, int64_t cap_dec,
-                    int64_t* n_dec, const int8_t* forced) {
+                    int64_t* n_dec, const int8_t* forced, int64_t n_restart) {
     obj_t O = {obj_kind, ny, nx, md, d_rowptr, d_col, d_val};
     double* g = (double*)malloc(sizeof(double) * (size_t)n);
     double* z = (double*)malloc(sizeof(double) * (size_t)n);
@@ -310,6 +310,10 @@ int orc_superiorize(int64_t m, int64_t n, const int64_t* rowptr, const int32_t* 
     for (int it = 0; it < n_iter; ++it) {
         int64_t k = k0 + it;
         int64_t trials = 0;
+        /* restarted perturbations ("l was restarted after every 50 iterations"; A-24): at the start of
+         * sweep k = r * n_restart, r = 1, 2, ..., the exponent is reset to r ("l = 1 after the first restart, l = 2 after
+         * the second"), which keeps sum beta finite: cycle r contributes at most beta0 a^r / (1 - a). */
+        if (n_restart > 0 && k > 0 && k % n_restart == 0) *ell = k / n_restart;
         if (N > 0 && obj_kind != 0)
             trials = orc_perturb(n, &O, x, ell, k, N, beta0, a, policy, g, z, decisions, margins, cap_dec, n_dec,
                                  forced, &warn, NULL);

@@ -538,3 +538,40 @@ def test_conditioning_of_superiorized_iteration():
     assert dev[-1] > 1e-4                    # ten sweeps: above the free-running fp32 bar
     assert dev[-1] > 1e3 * dev[0]            # growth by orders of magnitude
     assert max(devb) < 5e-7                  # basic algorithm: no amplification
+
+
+def test_restarted_perturbations():
+    """A-24: with n_restart = R the exponent is reset to r at the start of sweep r*R (r = 1, 2, ...).
+    Pins: R = 0 (and R > n_iter) is the plain run bit for bit; before the first restart nothing changes; the l recorded
+    after every sweep equals (restart value or previous l) + that sweep's trials; the exponents used in cycle r are
+    >= r, so the cycle's steps sum to at most beta0 a^r / (1 - a) (bounded perturbations, L97)."""
+    import gen
+
+    P = gen.config1_tiny_ct(n_pix=24, n_angles=20, n_bins=35, n_sweeps=14, N=3)
+    O = Oracle.from_problem(P)
+    a, R = 0.8, 4
+    plain = O.superiorize(P.x0, 14, P.N, P.beta0, a, lam=P.lam, snapshots=range(1, 15))
+    for off in (0, 100):
+        same = O.superiorize(P.x0, 14, P.N, P.beta0, a, lam=P.lam, n_restart=off)
+        assert np.array_equal(same["x"], plain["x"]) and same["ell"] == plain["ell"]
+    rs = O.superiorize(P.x0, 14, P.N, P.beta0, a, lam=P.lam, snapshots=range(1, 15), n_restart=R)
+    for s in range(1, R + 1):  # sweeps 0..R-1 are untouched
+        assert np.array_equal(rs["snaps"][s], plain["snaps"][s])
+    assert not np.array_equal(rs["snaps"][R + 1], plain["snaps"][R + 1])  # the restart enlarged the steps of sweep R
+    ell = 0
+    for k in range(14):
+        if k > 0 and k % R == 0:
+            ell = k // R
+        ell += int(rs["trace"][k, 2])
+        assert int(rs["trace"][k, 3]) == ell
+    assert rs["ell"] == ell
+    # resuming a run across a restart boundary is the same run (state = x, l, k)
+    first = O.superiorize(P.x0, 6, P.N, P.beta0, a, lam=P.lam, n_restart=R)
+    second = O.superiorize(first["x"], 8, P.N, P.beta0, a, lam=P.lam, n_restart=R, ell0=first["ell"], k0=6)
+    assert np.array_equal(second["x"], rs["x"]) and second["ell"] == rs["ell"]
+    # bounded perturbations (L97): in cycle r every exponent is >= r, so the phase of sweep k moves x by at most
+    # beta0 sum_{e >= l_start} a^e; checked on the first sweep after the restart, whose phase starts from l = 1
+    xR = rs["snaps"][R]
+    pert = O.perturb(xR, 1, P.N, P.beta0, a)
+    assert np.linalg.norm(pert["x"] - xR) <= P.beta0 * a / (1 - a) + 1e-12
+    assert np.all(np.isfinite(rs["trace"]))
