@@ -95,6 +95,8 @@ typedef struct {
     double* decision_f;    /* device, [decisions_cap][2] = {f(z), f(x^{k,n})} per trial; NULL = off */
     int64_t decisions_cap;
     int use_graph;         /* 1: capture one sweep into a CUDA graph and replay it (default path of bench.py) */
+    int64_t n_restart;     /* > 0: restarted perturbations: at the start of sweep k = r * n_restart,
+                              r = 1, 2, ..., the exponent l is reset to r (PER_TRIAL policy; A-24).  0: off */
 } sup_options;
 
 /* final state of a run, read back by sup_get_state (host struct) */

@@ -34,7 +34,8 @@ class _Csr(Structure):
 class _Options(Structure):
     _fields_ = [("objective", c_int), ("shape", c_int64 * 3), ("lambda_", c_double), ("block_iterative", c_int),
                 ("step_policy", c_int), ("ell0", c_int64), ("k0", c_int64), ("trace_mode", c_int), ("trace", c_void_p),
-                ("decisions", c_void_p), ("decision_f", c_void_p), ("decisions_cap", c_int64), ("use_graph", c_int)]
+                ("decisions", c_void_p), ("decision_f", c_void_p), ("decisions_cap", c_int64), ("use_graph", c_int),
+                ("n_restart", c_int64)]
 
 
 class _State(Structure):
@@ -257,7 +258,7 @@ def sup_perturb_dose(H: SupHandle, x: torch.Tensor, N, beta0, a, ell=0):
     return e.value
 
 
-def _options(H, objective, shape, lam, block, policy, ell0, k0, trace, decisions, decision_f, use_graph):
+def _options(H, objective, shape, lam, block, policy, ell0, k0, trace, decisions, decision_f, use_graph, n_restart=0):
     o = _Options()
     o.objective = _OBJ[objective] if not isinstance(objective, int) else objective
     if shape is not None and o.objective == OBJ_TV2D:
@@ -272,14 +273,15 @@ def _options(H, objective, shape, lam, block, policy, ell0, k0, trace, decisions
     o.decision_f = decision_f.data_ptr() if decision_f is not None else None
     o.decisions_cap = int(decisions.numel()) if decisions is not None else (int(decision_f.shape[0]) if decision_f is not None else 0)
     o.use_graph = int(bool(use_graph))
+    o.n_restart = int(n_restart)
     return o
 
 
 def sup_superiorize(H: SupHandle, x: torch.Tensor, n_iter, N, beta0, a, objective=None, shape=None, lam=1.0, block=False,
-                    policy=PER_TRIAL, ell0=0, k0=0, trace=None, decisions=None, decision_f=None, use_graph=True):
+                    policy=PER_TRIAL, ell0=0, k0=0, trace=None, decisions=None, decision_f=None, use_graph=True, n_restart=0):
     """Algorithm 1 on device tensor x (in place, asynchronous).  trace: float64 [n_iter,4] device tensor or None;
     decisions: int8 [cap] device tensor or None; decision_f: float64 [cap,2] device tensor or None."""
-    o = _options(H, objective, shape, lam, block, policy, ell0, k0, trace, decisions, decision_f, use_graph)
+    o = _options(H, objective, shape, lam, block, policy, ell0, k0, trace, decisions, decision_f, use_graph, n_restart)
     H._enter()
     H._check(lib().sup_superiorize(H.h, _ptr(x), n_iter, N, beta0, a, byref(o)))
     H._exit()
@@ -287,10 +289,10 @@ def sup_superiorize(H: SupHandle, x: torch.Tensor, n_iter, N, beta0, a, objectiv
 
 
 def sup_superiorize_host(H: SupHandle, x_host: torch.Tensor, n_iter, N, beta0, a, objective=None, shape=None, lam=1.0,
-                         block=False, policy=PER_TRIAL, ell0=0, k0=0, use_graph=True):
+                         block=False, policy=PER_TRIAL, ell0=0, k0=0, use_graph=True, n_restart=0):
     """Same with x a (pinned) HOST tensor: H2D copy, run, D2H copy, synchronise -- the end-to-end entry."""
     assert not x_host.is_cuda and x_host.dtype == H.tdtype and x_host.is_contiguous()
-    o = _options(H, objective, shape, lam, block, policy, ell0, k0, None, None, None, use_graph)
+    o = _options(H, objective, shape, lam, block, policy, ell0, k0, None, None, None, use_graph, n_restart)
     H._enter()
     H._check(lib().sup_superiorize_host(H.h, c_void_p(x_host.data_ptr()), n_iter, N, beta0, a, byref(o)))
     H._exit()

@@ -394,7 +394,7 @@ static sup_status perturb_alone(sup_ctx* h, void* x, int kind, const int64_t* sh
     if (rc != SUP_OK) return rc;
     sup_launch_begin_run(h, *ell, 0, a);
     if (N > 0) {
-        PerturbParams pp = {kind, ny, nx, N, beta0, a, SUP_STEP_PER_TRIAL, nullptr, nullptr, 0};
+        PerturbParams pp = {kind, ny, nx, N, beta0, a, SUP_STEP_PER_TRIAL, nullptr, nullptr, 0, 0};
         rc = sup_launch_perturb(h, x, pp);
         if (rc != SUP_OK) return rc;
     }
@@ -430,7 +430,7 @@ struct RunPlan {
 static sup_status enqueue_superiorized_sweep(sup_ctx* h, const RunPlan& P) {
     if (P.N > 0 && P.o.objective != SUP_OBJ_NONE) {
         PerturbParams pp = {P.o.objective, P.ny, P.nx, P.N, P.beta0, P.a, P.o.step_policy, P.o.decisions, P.o.decision_f,
-                            P.o.decisions_cap};
+                            P.o.decisions_cap, P.o.n_restart};
         sup_status rc = sup_launch_perturb(h, P.x, pp);
         if (rc != SUP_OK) return rc;
         h->xg_synced = false;  // the perturbation moved x
@@ -455,6 +455,7 @@ static sup_status run_superiorize(sup_ctx* h, void* x, int n_iter, int N, double
         return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_superiorize: unknown step policy");
     if (opt->block_iterative && h->n_blocks < 1) return sup_fail(h, SUP_ERR_STATE, "sup_superiorize: call sup_set_blocks first");
     if ((opt->decisions || opt->decision_f) && opt->decisions_cap < 0) return sup_fail(h, SUP_ERR_INVALID_ARG, "decisions_cap < 0");
+    if (opt->n_restart < 0) return sup_fail(h, SUP_ERR_INVALID_ARG, "n_restart < 0");
     RunPlan P;
     P.x = x;
     P.N = N;
@@ -484,6 +485,7 @@ static sup_status run_superiorize(sup_ctx* h, void* x, int n_iter, int N, double
         key.dec = opt->decisions;
         key.decf = opt->decision_f;
         key.cap = opt->decisions_cap;
+        key.n_restart = opt->n_restart;
         if (!h->gexec || !(key == h->gkey)) {
             drop_graph(h);
             const int64_t launches_before = h->launches;

@@ -113,6 +113,7 @@ struct sup_ctx {
     struct GraphKey {
         const void* x = nullptr;
         int N = 0, objective = 0, block = 0, policy = 0, trace_mode = 0;
+        int64_t n_restart = 0;
         double beta0 = 0, a = 0, lambda = 0;
         int64_t s0 = 0, s1 = 0;
         const void *trace = nullptr, *dec = nullptr, *decf = nullptr;
@@ -120,7 +121,7 @@ struct sup_ctx {
         bool operator==(const GraphKey& o) const {
             return x == o.x && N == o.N && objective == o.objective && block == o.block && policy == o.policy &&
                    trace_mode == o.trace_mode && beta0 == o.beta0 && a == o.a && lambda == o.lambda && s0 == o.s0 &&
-                   s1 == o.s1 && trace == o.trace && dec == o.dec && decf == o.decf && cap == o.cap;
+                   s1 == o.s1 && trace == o.trace && dec == o.dec && decf == o.decf && cap == o.cap && n_restart == o.n_restart;
         }
     } gkey;
     int64_t launches = 0;
@@ -197,6 +198,7 @@ struct PerturbParams {
     int8_t* decisions;
     double* decision_f;
     int64_t cap;
+    int64_t n_restart;
 };
 sup_status sup_launch_perturb(sup_ctx* h, void* x, const PerturbParams& pp);
 void sup_launch_objective(sup_ctx* h, const void* x, int kind, int64_t ny, int64_t nx, double* out_dev);

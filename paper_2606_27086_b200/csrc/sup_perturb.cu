@@ -33,6 +33,7 @@ struct PArgs {
     int N;
     double beta0, a;
     int policy;
+    long long n_restart;
     DevState* st;
     double* partials;  // [2][SUP_MAX_PARTIALS]
     int8_t* decisions;
@@ -377,6 +378,12 @@ __global__ void __launch_bounds__(SUP_THREADS) k_perturb(PArgs<T> Ain) {
     const long long k = *(volatile long long*)&st->k;
     long long ndec = *(volatile long long*)&st->n_dec;
     long long trials = 0;
+    // restarted perturbations (A-24): at the start of sweep k = r * n_restart the exponent is reset to r
+    if (A.n_restart > 0 && k > 0 && k % A.n_restart == 0) {
+        ell = k / A.n_restart;
+        apow = 1.0;
+        for (long long q = 0; q < ell; ++q) apow *= A.a;
+    }
     int warn = 0, fault = 0;
     int slot = 0;
     double* P0 = A.partials;
@@ -551,6 +558,7 @@ static PArgs<T> make_args(sup_ctx* h, void* x, const PerturbParams& pp) {
     A.beta0 = pp.beta0;
     A.a = pp.a;
     A.policy = pp.policy;
+    A.n_restart = pp.n_restart;
     A.st = h->state;
     A.partials = h->partials;
     A.decisions = pp.decisions;

@@ -624,3 +624,42 @@ def test_full_size_config3_sampled_rows_columns_and_invariants():
         assert st["fault"] == 0 and st["warn"] == 0 and st["ell"] >= 6 * P.N and np.isfinite(st["f"])
         outs.append(xs.cpu())
     assert torch.equal(outs[0], outs[1])
+
+
+# ------------------------------------------------------------------------------------------------------------
+# restarted perturbations (A-24)
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", [0, 1])
+def test_restarted_perturbations(dtype):
+    """l <- r at the start of sweep r * n_restart.  Step-wise over every sweep (common state x^k, l_k, k -- the restart is a
+    function of k, so resuming at any k must reproduce it), then the whole run with the graph replay: l and the trial
+    counts per sweep exactly, x within the free-running bars (this small case is not conditioning-limited)."""
+    sup = _sup()
+    P = problem("ct_ragged")
+    R_, n_iter, a = 4, 12, 0.9
+    H = make_handle(P, dtype)
+    O = Oracle.from_problem(P)
+    ref = O.superiorize(P.x0, n_iter, P.N, P.beta0, a, lam=P.lam, snapshots=range(1, n_iter + 1), n_restart=R_)
+    assert int(ref["trace"][R_, 3]) == 1 + int(ref["trace"][R_, 2])  # the oracle did restart at sweep R
+    for k in range(n_iter):
+        xs = round_to(P.x0 if k == 0 else ref["snaps"][k], dtype)
+        ell = 0 if k == 0 else int(ref["trace"][k - 1, 3])
+        one = O.superiorize(xs, 1, P.N, P.beta0, a, lam=P.lam, ell0=ell, k0=k, n_restart=R_)
+        x = xdev(P, dtype, xs)
+        sup.sup_superiorize(H, x, 1, P.N, P.beta0, a, objective=P.objective, shape=P.shape, lam=P.lam, ell0=ell, k0=k, n_restart=R_)
+        st = sup.sup_get_state(H)
+        assert st["ell"] == one["ell"], (k, st["ell"], one["ell"])
+        assert rel_l2(x.cpu().numpy(), one["x"]) <= STEP_TOL[dtype], k
+    x = xdev(P, dtype)
+    trace = torch.zeros((n_iter, 4), dtype=torch.float64, device="cuda:0")
+    sup.sup_superiorize(H, x, n_iter, P.N, P.beta0, a, objective=P.objective, shape=P.shape, lam=P.lam, trace=trace, n_restart=R_)
+    st = sup.sup_get_state(H)
+    tr = trace.cpu().numpy()
+    assert st["ell"] == ref["ell"]
+    assert np.array_equal(tr[:, 2], ref["trace"][:, 2]) and np.array_equal(tr[:, 3], ref["trace"][:, 3])
+    assert rel_l2(x.cpu().numpy(), ref["x"]) <= FINAL_TOL[dtype]
+    # n_restart = 0 and n_restart > n_iter are the plain run
+    xa, xb = xdev(P, dtype), xdev(P, dtype)
+    sup.sup_superiorize(H, xa, n_iter, P.N, P.beta0, a, objective=P.objective, shape=P.shape, lam=P.lam)
+    sup.sup_superiorize(H, xb, n_iter, P.N, P.beta0, a, objective=P.objective, shape=P.shape, lam=P.lam, n_restart=100)
+    assert torch.equal(xa, xb) and not torch.equal(xa, x)
