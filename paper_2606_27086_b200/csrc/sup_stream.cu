@@ -368,18 +368,24 @@ __global__ void __launch_bounds__(32 * (NCW + 1), 1)
 }
 
 // ---- planning: partition table + eligibility -------------------------------------------------------------------------
-// part[b] = first row r in [r0, r1] with rowptr[r] >= e0 + (e1 - e0) * b / nb  (part[0] = r0, part[nb] = r1)
+// Rows are split by COST, not by nonzeros alone: cost(r0..r) = nonzeros + RG_ROW_COST per row (a row costs its shuffles,
+// barrier waits and epilogue even when it is empty: config 4 has body voxels no beamlet reaches, config 3 rays that miss
+// the image).  part[b] = first row r in [r0, r1] with cost(r0..r) >= total * b / nb  (part[0] = r0, part[nb] = r1).
+#ifndef RG_ROW_COST
+#define RG_ROW_COST 16
+#endif
 __global__ void k_stream_partition(const int64_t* __restrict__ rowptr, int64_t r0, int64_t r1, int nb, int64_t* __restrict__ part) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b > nb) return;
     if (b == 0) { part[0] = r0; return; }
     if (b == nb) { part[nb] = r1; return; }
-    const int64_t e0 = rowptr[r0], e1 = rowptr[r1];
-    const int64_t target = e0 + ((e1 - e0) / nb) * b + (((e1 - e0) % nb) * b) / nb;
-    int64_t lo = r0, hi = r1;  // lower bound
+    const int64_t e0 = rowptr[r0];
+    const int64_t total = (rowptr[r1] - e0) + int64_t(RG_ROW_COST) * (r1 - r0);
+    const int64_t target = (total / nb) * b + ((total % nb) * b) / nb;
+    int64_t lo = r0, hi = r1;  // lower bound on the monotone key
     while (lo < hi) {
         const int64_t mid = lo + ((hi - lo) >> 1);
-        if (rowptr[mid] < target) lo = mid + 1;
+        if ((rowptr[mid] - e0) + int64_t(RG_ROW_COST) * (mid - r0) < target) lo = mid + 1;
         else hi = mid;
     }
     part[b] = lo;
