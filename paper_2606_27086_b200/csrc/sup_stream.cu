@@ -115,6 +115,7 @@ template <typename T, int STG>
 struct RgSmem {
     RgData<T, STG> d;
     unsigned long long full[STG];
+    T ctabuf[2][RG_CWARPS];       // G == 0: the consumer warps' partial sums of one long row (double-buffered by row parity)
     T pairbuf[RG_CWARPS / 2][2];  // G == 64: partial row sums handed from the odd to the even warp of a pair
     int progress[RG_CWARPS];  // per consumer warp: tiles [0, progress) are no longer needed by it
     int issued[STG];          // per stage: 1 + the tile its barrier is currently armed for (0: none yet)
@@ -261,7 +262,85 @@ __global__ void __launch_bounds__(32 * (NCW + 1), 1)
         }
         return;
     }
-    // ---- consumers --------------------------------------------------------------------------------------------------
+    // ---- consumers, G == 0: LONG rows -- the whole CTA works on one row at a time ----------------------------------------
+    // (rows of thousands of nonzeros, e.g. config 4's A^T: one row per warp would put NCW x row bytes in flight, far more
+    // than the ring holds).  The row is cut into pieces of 32 NCW x RG_UNROLL elements; every lane takes RG_UNROLL elements
+    // of a piece, tiles are released piece by piece, so the row length is unbounded; the warps' partial sums meet in shared
+    // memory and warp 0 adds them in a fixed order.
+    if constexpr (G == 0) {
+        constexpr int GT = 32 * NCW;
+        constexpr int CH = GT * RG_UNROLL;
+        const int gl = warp * 32 + lane;
+        int seen = 0, released = 0, iter = 0;
+        int s = int(rowptr[rs] - base), e = int(rowptr[rs + 1] - base);
+        for (int64_t r = rs; r < re; ++r, ++iter) {
+            int s_next = 0, e_next = 0;
+            if (r + 1 < re) {
+                s_next = e;
+                e_next = int(rowptr[r + 2] - base);
+            }
+            T q1 = T(0), q2 = T(0), q3 = T(0);
+            if (gl == 0) {
+                q1 = p1[r];
+                q2 = p2[r];
+                q3 = MODE == 0 ? p3[r] : out[r];
+            }
+            T a0 = T(0), a1 = T(0), a2 = T(0), a3 = T(0);
+            for (int ps = s; ps < e; ps += CH) {
+                const int pe = e < ps + CH ? e : ps + CH;
+                int t_start = ps / RG_TILE;
+                t_start = t_start < ntiles ? t_start : ntiles;
+                if (released < t_start) {
+                    released = t_start;
+                    if (lane == 0) progress[warp] = t_start;
+                }
+                const int t_hi = (pe - 1) / RG_TILE;
+                for (int t = seen > t_start ? seen : t_start; t <= t_hi; ++t) {
+                    const int st = t % STG;
+                    if (issued[st] != t + 1) {
+                        const long long t0 = clock64();
+                        while (issued[st] != t + 1)
+                            if (clock64() - t0 > RG_TIMEOUT) __trap();
+                    }
+                    mbar_wait(smem_u32(&S.full[st]), (t / STG) & 1);
+                }
+                seen = seen > t_hi + 1 ? seen : t_hi + 1;
+                asm volatile("" ::: "memory");
+                int rel = pe / RG_TILE;
+                rel = rel < ntiles ? rel : ntiles;
+                rel = rel > released ? rel : released;
+                const bool wraps = (ps % RG_ELEMS) + (pe - ps) > RG_ELEMS;
+                if (!wraps) ring_row_dot<T, GT, false, STG>(S.d, vec, ps + gl, pe, 1, progress + warp, rel, lane == 0, a0, a1, a2, a3);
+                else ring_row_dot<T, GT, true, STG>(S.d, vec, ps + gl, pe, 1, progress + warp, rel, lane == 0, a0, a1, a2, a3);
+                released = rel;
+            }
+            T acc = (a0 + a1) + (a2 + a3);
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+            if (lane == 0) S.ctabuf[iter & 1][warp] = acc;
+            asm volatile("bar.sync 1, %0;" ::"n"(GT) : "memory");
+            if (gl == 0) {
+                T tot = T(0);
+#pragma unroll
+                for (int w = 0; w < NCW; ++w) tot += S.ctabuf[iter & 1][w];
+                if (MODE == 0) {
+                    out[r] = q3 * hyperslab_violation(tot, q1, q2);
+                } else {
+                    T t = q3 - lambda * tot;
+                    t = t < q1 ? q1 : t;
+                    t = t > q2 ? q2 : t;
+                    out[r] = t;
+                    if (out2) out2[sup_swz(int(r))] = t;
+                }
+            }
+            s = s_next;
+            e = e_next;
+        }
+        __syncwarp();
+        if (lane == 0) progress[warp] = ntiles;
+        return;
+    } else {
+    // ---- consumers, G >= 4 --------------------------------------------------------------------------------------------------
     // All positions below are element offsets relative to `base` and fit an int (a CTA's range is < 2^31 elements).
     // G <= 32: G lanes per row, 32/G rows per warp.  G == 64: a PAIR of warps per row (halves the rows in flight, hence
     // the ring span, for long rows); the odd warp hands its partial sum to the even one through shared memory.
@@ -364,6 +443,7 @@ __global__ void __launch_bounds__(32 * (NCW + 1), 1)
         asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
         atomicMax(reinterpret_cast<unsigned long long*>(dbg) + blockIdx.x, (unsigned long long)(clock64() - t_begin));
         if (warp == 0) dbg[SUP_MAX_PARTIALS + blockIdx.x] = double(smid) + double(ee - es) * 1024.0;
+    }
     }
 }
 
@@ -478,12 +558,12 @@ sup_status sup_stream_plan(sup_ctx* h, const CsrD& M, int64_t r0, int64_t r1, bo
     while (G < 32 && avg * (32.0 / G) > 960.0) G <<= 1;  // a warp's rows total ~a tile (G = 64, a warp pair per row, only by override)
     if (const char* env = getenv(forward ? "SUP_STREAM_G_FWD" : "SUP_STREAM_G_BWD")) {
         const int g = atoi(env);
-        if (g == 4 || g == 8 || g == 16 || g == 32 || g == 64) G = g;
+        if (g == 0 || g == 4 || g == 8 || g == 16 || g == 32 || g == 64) G = g;
     }
     const int64_t cap = int64_t(RG_STAGES - 2) * RG_TILE;
-    while (G < 32 && int64_t(mx_h) * (32 / G) > cap) G <<= 1;
+    while (G < 32 && G > 0 && int64_t(mx_h) * (32 / G) > cap) G <<= 1;
+    if (G != 0 && (avg > 2048.0 || int64_t(mx_h) * (G >= 32 ? 1 : 32 / G) > cap)) G = 0;  // long rows: the whole CTA per row, no length limit
     out->max_row = int64_t(mx_h);
-    if (int64_t(mx_h) * (G >= 32 ? 1 : 32 / G) > cap) return SUP_OK;  // a row too long for the ring: group-per-row kernels
     out->part = static_cast<const int64_t*>(table);
     out->nb = nb;
     out->G = G;
@@ -544,6 +624,7 @@ static void launch_staged(sup_ctx* h, const StreamPlan& sp, const CsrD& M, const
         case 8: launch_staged_g<T, MODE, 8>(h, sp, M, vec, p1, p2, p3, out, out2, lambda); break;
         case 16: launch_staged_g<T, MODE, 16>(h, sp, M, vec, p1, p2, p3, out, out2, lambda); break;
         case 64: launch_staged_g<T, MODE, 64>(h, sp, M, vec, p1, p2, p3, out, out2, lambda); break;
+        case 0: launch_staged_g<T, MODE, 0>(h, sp, M, vec, p1, p2, p3, out, out2, lambda); break;
         default: launch_staged_g<T, MODE, 32>(h, sp, M, vec, p1, p2, p3, out, out2, lambda); break;
     }
 }

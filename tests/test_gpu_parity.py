@@ -663,3 +663,24 @@ def test_restarted_perturbations(dtype):
     sup.sup_superiorize(H, xa, n_iter, P.N, P.beta0, a, objective=P.objective, shape=P.shape, lam=P.lam)
     sup.sup_superiorize(H, xb, n_iter, P.N, P.beta0, a, objective=P.objective, shape=P.shape, lam=P.lam, n_restart=100)
     assert torch.equal(xa, xb) and not torch.equal(xa, x)
+
+
+@pytest.mark.parametrize("dtype", [0, 1])
+@pytest.mark.parametrize("name", ["cfg4_small", "ct_ragged", "cfg5_k16"])
+def test_long_row_mode_of_the_staged_kernels(name, dtype, monkeypatch):
+    """The whole-CTA-per-row mode (chosen for rows of thousands of nonzeros: config 4's A^T at full size) forced on both
+    products of small problems, including rows shorter than a piece, empty rows and rows spanning several ring tiles."""
+    sup = _sup()
+    monkeypatch.setenv("SUP_STREAM_G_FWD", "0")
+    monkeypatch.setenv("SUP_STREAM_G_BWD", "0")
+    P = problem(name)
+    H = make_handle(P, dtype, blocks=False)
+    O = Oracle.from_problem(P)
+    x = xdev(P, dtype)
+    xo = P.x0.astype(np.float64)
+    for s in (1, 6):
+        sup.sup_project_simultaneous(H, x, P.lam, s)
+        xo = O.sweep(xo, P.lam, s)
+        assert rel_l2(x.cpu().numpy(), xo) <= SWEEP_TOL[dtype], (name, s)
+    xg = x.cpu().numpy().astype(np.float64)
+    assert close_scalar(sup.sup_proximity(H, x, 0), O.proximity(xg, 0), 1e-4 if dtype == 0 else 1e-10)
