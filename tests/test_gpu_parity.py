@@ -684,3 +684,49 @@ def test_long_row_mode_of_the_staged_kernels(name, dtype, monkeypatch):
         assert rel_l2(x.cpu().numpy(), xo) <= SWEEP_TOL[dtype], (name, s)
     xg = x.cpu().numpy().astype(np.float64)
     assert close_scalar(sup.sup_proximity(H, x, 0), O.proximity(xg, 0), 1e-4 if dtype == 0 else 1e-10)
+
+
+# ------------------------------------------------------------------------------------------------------------
+# degenerate inputs
+# ------------------------------------------------------------------------------------------------------------
+def _mini(rowptr, col, val, lb, ub, lo, hi, n):
+    f4 = lambda a: np.asarray(a, np.float32)
+    return dict(rowptr=np.asarray(rowptr, np.int64), col=np.asarray(col, np.int32), val=f4(val), lb=f4(lb), ub=f4(ub),
+                lo=f4(lo), hi=f4(hi), n=n)
+
+
+DEGENERATE = {
+    "one_by_one": _mini([0, 1], [0], [2.0], [1.0], [1.5], [-5.0], [5.0], 1),
+    "one_long_row": _mini([0, 5000], np.arange(5000), np.linspace(0.1, 1.0, 5000), [3.0], [4.0], np.full(5000, -1.0), np.full(5000, 1.0), 5000),
+    "one_long_column": _mini(np.arange(4001), np.zeros(4000, np.int32), np.linspace(0.5, 1.5, 4000), np.full(4000, 0.2), np.full(4000, 0.3), [-9.0], [9.0], 1),
+    "all_rows_empty_but_one": _mini([0, 0, 0, 2, 2], [1, 3], [1.0, -1.0], [-INF, 5.0, 0.5, -INF], [INF, 6.0, INF, 1.0], np.zeros(4), np.ones(4), 4),
+    "image_one_pixel_wide": _mini([0, 2, 3], [0, 5, 2], [1.0, 1.0, 2.0], [0.5, 0.1], [0.6, 0.2], np.zeros(6), np.ones(6), 6),
+}
+
+
+@pytest.mark.parametrize("dtype", [0, 1])
+@pytest.mark.parametrize("name", sorted(DEGENERATE))
+def test_degenerate_inputs(name, dtype):
+    """1x1 systems, a single row / a single column of thousands of entries (long-row mode), almost all rows empty with
+    one-sided and empty hyperslabs, zero sweeps, and TV on images one pixel wide (no term exists: f = 0, g = 0)."""
+    sup = _sup()
+    D = DEGENERATE[name]
+    m = D["rowptr"].size - 1
+    H = sup.sup_create(D["rowptr"], D["col"], D["val"], D["lb"], D["ub"], D["lo"], D["hi"], None, dtype=dtype, n=D["n"])
+    O = Oracle(m, D["n"], D["rowptr"], D["col"], D["val"], D["lb"], D["ub"], D["lo"], D["hi"])
+    x0 = np.clip(np.zeros(D["n"]), D["lo"], D["hi"]).astype(np.float64)
+    x = torch.tensor(x0, dtype=TD[dtype], device="cuda:0")
+    sup.sup_project_simultaneous(H, x, 1.0, 0)  # zero sweeps: untouched
+    assert np.array_equal(x.cpu().numpy().astype(np.float64), x0)
+    sup.sup_project_simultaneous(H, x, 1.3, 5)
+    xo = O.sweep(x0, 1.3, 5)
+    assert rel_l2(x.cpu().numpy(), xo) <= SWEEP_TOL[dtype], name
+    for mode in (0, 2):
+        assert close_scalar(sup.sup_proximity(H, x, mode), O.proximity(x.cpu().numpy().astype(np.float64), mode), 1e-4 if dtype == 0 else 1e-10)
+    if name == "image_one_pixel_wide":
+        for shape in ((6, 1), (1, 6)):
+            xs = torch.tensor(np.linspace(0.0, 1.0, 6), dtype=TD[dtype], device="cuda:0")
+            before = xs.clone()
+            assert sup.sup_objective(H, xs, "tv2d", shape) == 0.0
+            ell = sup.sup_perturb_tv(H, xs, shape, 3, 1.0, 0.9, 0)
+            assert ell == 3 and torch.equal(xs, before)  # g = 0: every step accepted with equality, x untouched (A-6)
