@@ -42,7 +42,7 @@ extern "C" sup_status sup_workspace_bytes(int kind, int64_t m, int64_t n, int64_
             s = sup_transpose_scratch_bytes(nnz, n, esz) + al(size_t(n_blocks) * 8) + 4096;
             break;
         case SUP_WS_DOSE:  // (m, n, nnz) describe D_body
-            p = al(size_t(n + 1) * 8) + al(size_t(nnz) * 4) + al(size_t(nnz) * esz) + al(size_t(m) * esz) + 1024;
+            p = al(size_t(n + 1) * 8) + al(size_t(nnz) * 4) + al(size_t(nnz) * esz) + 2 * al(size_t(m) * esz) + 1024;
             s = sup_transpose_scratch_bytes(nnz, n, esz) + 4096;
             break;
         default:
@@ -262,6 +262,7 @@ extern "C" sup_status sup_set_dose_matrix(sup_handle h, const sup_csr* D, void* 
     int32_t* col = static_cast<int32_t*>(B.take(size_t(D->nnz) * 4));
     void* val = B.take(size_t(D->nnz) * h->esz);
     h->r_dose = B.take(size_t(D->m) * h->esz);
+    h->q_dose = B.take(size_t(D->m) * h->esz);
     if (!B.ok) return sup_fail(h, SUP_ERR_WORKSPACE, "sup_set_dose_matrix: workspace too small");
     rc = sup_transpose_rows(h, Dm, 0, D->m, 0, D->nnz, rp, col, val, 0, scratch, scratch_bytes);
     if (rc != SUP_OK) return rc;

@@ -104,6 +104,7 @@ struct sup_ctx {
     bool has_dose = false;
     CsrD D, DT;
     void* r_dose = nullptr;     // [md] dtype
+    void* q_dose = nullptr;     // [md] dtype: D g
     int g_d = 8, g_dt = 32;
     // cached graph of one superiorized sweep
     cudaGraphExec_t gexec = nullptr;

@@ -48,6 +48,7 @@ struct PArgs {
     const int32_t* dt_col;
     const T* dt_val;
     T* r;
+    T* q;  // [md]: D g of the current reduction step (dose objective)
     int g_d, g_dt;
 };
 
@@ -249,6 +250,28 @@ __device__ double dose_share(const PArgs<T>& A, double coef, bool store_r) {
     return acc;
 }
 
+// q = D g (stored), returns this thread's share of sum q^2: with it a trial step needs no matrix pass,
+//   f(x - c g) = ||r - c q||^2 = f(x) - c ||g||^2 + c^2 ||q||^2     (r = D x, g = 2 D^T r  =>  <r, q> = ||g||^2 / 2)
+template <typename T>
+__device__ double dose_q_share(const PArgs<T>& A) {
+    const int G = A.g_d;
+    const int gl = threadIdx.x % G, lane = threadIdx.x & 31;
+    const int64_t gid = (int64_t(blockIdx.x) * blockDim.x + threadIdx.x) / G;
+    const int64_t ngroups = (int64_t(gridDim.x) * blockDim.x) / G;
+    double acc = 0.0;
+    for (int64_t i0 = gid - lane / G; i0 < A.md; i0 += ngroups) {
+        const int64_t i = i0 + lane / G;
+        const bool valid = i < A.md;
+        const int64_t s = valid ? A.d_rowptr[i] : 0, e = valid ? A.d_rowptr[i + 1] : 0;
+        const T qv = coop_row_dot<T, false>(A.d_val, A.d_col, s, e, A.g, nullptr, 0.0, gl, G);
+        if (valid && gl == 0) {
+            acc += double(qv) * double(qv);
+            A.q[i] = qv;
+        }
+    }
+    return acc;
+}
+
 template <typename T, int OBJ>
 __device__ __forceinline__ double objective_share(const PArgs<T>& A, double coef) {
     if (OBJ == SUP_OBJ_TV2D) return tv2d_share(A, coef);
@@ -389,14 +412,84 @@ __global__ void __launch_bounds__(SUP_THREADS) k_perturb(PArgs<T> Ain) {
     double* P0 = A.partials;
     double* P1 = A.partials + SUP_MAX_PARTIALS;
 
-    // fx = f(x)
-    double sh = cta_sum(objective_share<T, OBJ>(view(), 0.0));
+    // fx = f(x)  (dose: r = D x is stored on the way and then carried, r <- r - c q, through the phase)
+    double sh = OBJ == SUP_OBJ_DOSE ? cta_sum(dose_share(view(), 0.0, true)) : cta_sum(objective_share<T, OBJ>(view(), 0.0));
     if (threadIdx.x == 0) P0[blockIdx.x] = sh;
     grid_barrier(st);
     double fx = reduce_partials(P0);
     slot = 1;
     if (!isfinite(fx)) fault |= 2;
 
+    if constexpr (OBJ == SUP_OBJ_DOSE) {
+        // Quadratic objective: with q = D g the objective along the step is the closed form above, so the trial loop is
+        // scalar work and a reduction step costs two matrix passes (g = 2 D^T r, q = D g) instead of three or more.
+        for (int nred = 0; nred < A.N; ++nred) {
+            double* P = slot ? P1 : P0;
+            slot ^= 1;
+            sh = cta_sum(dose_grad_share(view()));
+            if (threadIdx.x == 0) P[blockIdx.x] = sh;
+            grid_barrier(st);
+            const double s2 = reduce_partials(P);
+            const double s = sqrt(s2);
+            P = slot ? P1 : P0;
+            slot ^= 1;
+            sh = cta_sum(dose_q_share(view()));
+            if (threadIdx.x == 0) P[blockIdx.x] = sh;
+            grid_barrier(st);
+            const double q2 = reduce_partials(P);
+            bool accepted = false;
+            long long jloc = 0;
+            double cf = 0.0, fz_acc = fx;
+            for (int trial = 0; trial < SUP_J_MAX && !accepted; ++trial) {
+                double ap = apow;
+                if (A.policy != SUP_STEP_PER_TRIAL) {
+                    ap = 1.0;
+                    for (long long q = 0; q < k + jloc; ++q) ap *= A.a;
+                }
+                const double c = s > 0.0 ? (A.beta0 * ap) / s : 0.0;
+                const double fz = c == 0.0 ? fx : fx - c * s2 + c * c * q2;
+                ++ell;
+                apow *= A.a;
+                ++jloc;
+                ++trials;
+                const bool acc = fz <= fx;
+                if (blockIdx.x == 0 && threadIdx.x == 0) {
+                    if (A.decisions && ndec < A.cap) A.decisions[ndec] = acc ? 1 : 0;
+                    if (A.decision_f && ndec < A.cap) {
+                        A.decision_f[2 * ndec] = fz;
+                        A.decision_f[2 * ndec + 1] = fx;
+                    }
+                }
+                ++ndec;
+                if (acc) {
+                    accepted = true;
+                    cf = c;
+                    fz_acc = fz;
+                }
+            }
+            if (accepted && cf != 0.0) {
+                const int64_t tid = int64_t(blockIdx.x) * blockDim.x + threadIdx.x, nth = int64_t(gridDim.x) * blockDim.x;
+                for (int64_t j = tid; j < A.n; j += nth) xc[j] = T(zval(xc, gc, cf, j));
+                double rr = 0.0;
+                for (int64_t i = tid; i < A.md; i += nth) {
+                    const T rn = T(zval(A.r, A.q, cf, i));  // r <- round_T(r - c q)
+                    A.r[i] = rn;
+                    rr += double(rn) * double(rn);
+                }
+                P = slot ? P1 : P0;
+                slot ^= 1;
+                sh = cta_sum(rr);
+                if (threadIdx.x == 0) P[blockIdx.x] = sh;
+                grid_barrier(st);  // x^{k,n+1} and r visible to everyone before the next gradient
+                fx = reduce_partials(P);
+            } else if (accepted) {
+                fx = fz_acc;
+            } else {
+                warn |= 1;  // A-12: step skipped
+            }
+            if (*(volatile int*)&st->fault & 1) break;
+        }
+    } else
     for (int nred = 0; nred < A.N; ++nred) {
         double* P = slot ? P1 : P0;
         slot ^= 1;
@@ -572,6 +665,7 @@ static PArgs<T> make_args(sup_ctx* h, void* x, const PerturbParams& pp) {
     A.dt_col = h->DT.col;
     A.dt_val = static_cast<const T*>(h->DT.val);
     A.r = static_cast<T*>(h->r_dose);
+    A.q = static_cast<T*>(h->q_dose);
     A.g_d = h->g_d;
     A.g_dt = h->g_dt;
     return A;
