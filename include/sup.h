@@ -15,8 +15,9 @@
  * CONVENTIONS
  *  - Every array argument is a DEVICE pointer owned by the caller unless its comment says "host".
  *    The library BORROWS A, lb, ub, box_lo, box_hi (and D_body) for the handle's lifetime and never frees them.
- *  - The library never allocates device memory.  Everything it derives (transposed CSR, row scaling, scratch
- *    vectors, reduction partials, device-side state) lives in caller-provided WORKSPACE memory whose size comes
+ *  - The library never allocates device memory.  Everything it derives (transposed CSR, the packed (value, column)
+ *    copies of A and A^T that the fp32 kernels stream, row scaling, scratch vectors, reduction partials, device-side
+ *    state) lives in caller-provided WORKSPACE memory whose size comes
  *    from sup_workspace_bytes().  "persistent" workspace must stay alive until sup_destroy(); "scratch"
  *    workspace is only used during the call that takes it and may be freed once that call's stream work is done
  *    (the calls that take scratch synchronise the stream before returning).
