@@ -9,18 +9,21 @@
 // bytes but only 57-60 % of the measured copy bandwidth with nothing saturated; the L1 fills (stream + gather
 // misses, 3.35 GB per launch) all go through the LSU miss path.  Two earlier attempts are recorded in
 // profiles/r01b_ring_negative.md.  This version takes the stream off the LSU path:
-//   * one persistent CTA per SM owns a CONTIGUOUS row range balanced by nonzeros (partition table built at
-//     setup), hence a contiguous range of val[] and col[];
-//   * a producer thread pulls that range through a ring of RG_STAGES tiles (RG_TILE elements each) in shared
-//     memory with cp.async.bulk (L2 evict-first policy) completing on per-stage mbarriers; the ring (128 KB in
-//     fp32) is about twice the span the consumers work on, so ~64 KB per SM are in flight at all times and the
-//     stream never occupies L1, which is left to the x / y gathers;
-//   * a watcher thread waits on the stage barriers in order and publishes the count of completed tiles; the 16
-//     consumer warps take the rows in order (G lanes per row), poll that one counter for the tiles their rows
-//     need, read val/col from the ring (consecutive lanes -> consecutive words), gather x / y through L1
-//     (ld.global.nc), reduce with shuffles and run the fused epilogue.  Each consumer warp publishes how many
-//     tiles lie wholly before its next row; the producer refills a stage when every warp has passed it.
-// The summation order of a row depends only on G, not on the grid: results are deterministic.
+//   * one persistent CTA per SM owns a CONTIGUOUS row range balanced by cost (nonzeros + a constant per row;
+//     partition table built at setup), hence a contiguous range of the matrix stream;
+//   * fp32 handles stream PACKED (value bits, column) pairs -- one cp.async.bulk per 8 KB tile, one 64-bit shared
+//     load per element (the copy engine costs ~72 cycles per copy, profiles/r01e_packed.md); fp64 handles stream
+//     val[] and col[] as two copies per tile;
+//   * a producer thread pulls the range through a ring of tiles in shared memory (20 stages for the fp32 forward
+//     product, 16 otherwise), L2 evict-first, completing on per-stage mbarriers; the stream never occupies L1,
+//     which is left to the x / y gathers, and it announces each armed stage in issued[];
+//   * the consumer warps (12 by default) take the rows in order (G lanes per row; G = 64: a warp pair per row;
+//     G = 0: the whole CTA per row, for rows of thousands of entries), wait on the barriers of the tiles their rows
+//     span, read the ring (consecutive lanes -> consecutive words), gather x / y through L1 (ld.global.nc, 16 in
+//     flight per lane), reduce with shuffles and run the fused epilogue.  Each consumer warp publishes how many
+//     tiles lie wholly before its rows; the producer refills a stage when every warp has passed it.
+// The forward product gathers from xg, the bank-swizzled mirror of x (sup_swz), which the back-projection keeps
+// in step.  The summation order of a row depends only on G, not on the grid: results are deterministic.
 #include <math.h>
 #include <stdlib.h>
 
@@ -178,7 +181,7 @@ __device__ __forceinline__ void ring_row_dot(const RgData<T, STG>& ring, const T
     }
 }
 
-// MODE 0: forward (vec = xg, col = colg, p1 = lb, p2 = ub, p3 = d, out = y);
+// MODE 0: forward (vec = xg, columns swizzled (pk / colg), p1 = lb, p2 = ub, p3 = d, out = y);
 // MODE 1: backward (vec = y, p1 = lo, p2 = hi, out = x in place, out2 = xg mirror or NULL)
 template <typename T, int MODE, int G, int NCW>
 __global__ void __launch_bounds__(32 * (NCW + 1), 1)
