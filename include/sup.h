@@ -135,6 +135,15 @@ sup_status sup_set_blocks(sup_handle h, int n_blocks, const int64_t* block_rowpt
 sup_status sup_set_dose_matrix(sup_handle h, const sup_csr* D_body, void* workspace, size_t workspace_bytes,
                                void* scratch, size_t scratch_bytes);
 
+/* Expert control of the two product kernels (S1+S2, S3), for tests and measurements: how many
+ * lanes cooperate on one row of A (forward) and of A^T (backward).  -1: the planner's choice from the mean and the
+ * longest row (default); 4, 8, 16, 32: that many lanes of a warp per row; 64: a pair of warps per row; 0: the whole CTA
+ * per row (what the planner picks for rows of thousands of nonzeros); -2 (either argument): do not use the bulk-copy
+ * staged kernels at all but the plain group-per-row kernels.  A request that the longest row cannot satisfy is
+ * widened by the planner.  Re-plans in place, drops the cached graph, synchronises the stream.  Results differ
+ * between settings only by the summation order inside a row. */
+sup_status sup_set_row_mode(sup_handle h, int lanes_forward, int lanes_backward);
+
 /* n_sweeps simultaneous sweeps x <- P_box(x - lambda A^T D c(x)), in place (O-SWEEP; Eq. 2, 3; L427). */
 sup_status sup_project_simultaneous(sup_handle h, void* x, double lambda, int n_sweeps);
 

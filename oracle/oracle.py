@@ -17,7 +17,8 @@ _SRC = os.path.join(_HERE, "sup_oracle.c")
 _LIB = os.path.join(_HERE, "_sup_oracle.so")
 _lib = None
 
-OBJ_KIND = {None: 0, "none": 0, "tv2d": 1, "tv1d": 2, "dose": 3}
+OBJ_KIND = {None: 0, "none": 0, "tv2d": 1, "tv1d": 2, "dose": 3, "mean": 4, "tv3d": 5}
+ALGORITHM = {"sim": 0, "block": 1, "drop": 2, "emr": 3}
 PER_TRIAL, PER_SWEEP = 0, 1
 
 
@@ -25,7 +26,9 @@ def build(force: bool = False) -> str:
     """gcc -O2 -ffp-contract=off (no -ffast-math, no FMA contraction, no OpenMP: single-threaded scalar code;
     reductions use binary128 accumulators from libgcc's soft-float, see sup_oracle.c)."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        subprocess.check_call(["gcc", "-O2", "-ffp-contract=off", "-shared", "-fPIC", "-o", _LIB, _SRC, "-lm"])
+        tmp = f"{_LIB}.{os.getpid()}.tmp"  # build aside and rename: a process that has the old library mapped keeps it
+        subprocess.check_call(["gcc", "-O2", "-ffp-contract=off", "-shared", "-fPIC", "-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, _LIB)
     return _LIB
 
 
@@ -38,6 +41,10 @@ def _L():
         _lib.orc_tv2d.restype = ctypes.c_double
         _lib.orc_tv1d.restype = ctypes.c_double
         _lib.orc_dose.restype = ctypes.c_double
+        _lib.orc_mean.restype = ctypes.c_double
+        _lib.orc_tv3d.restype = ctypes.c_double
+        _lib.orc_perturb_phase3.restype = ctypes.c_int64
+        _lib.orc_superiorize_ex.restype = ctypes.c_int
         _lib.orc_perturb_phase.restype = ctypes.c_int64
         _lib.orc_setup.restype = ctypes.c_int
         _lib.orc_superiorize.restype = ctypes.c_int
@@ -49,6 +56,11 @@ def _p(a):
 
 
 _i64, _dbl, _int = ctypes.c_int64, ctypes.c_double, ctypes.c_int
+
+
+class _RunOpt(ctypes.Structure):  # run_opt_t of sup_oracle.c
+    _fields_ = [("algorithm", _int), ("stop_enabled", _int), ("prox_tol", _dbl), ("dprox_tol", _dbl), ("n_consec", _int),
+                ("dobj_tol", _dbl), ("n_restart", _i64), ("nz", _i64)]
 
 
 class Oracle:
@@ -103,6 +115,23 @@ class Oracle:
                                  _int(br.size - 1), _p(br), _p(x))
         return x
 
+    def drop_sweep(self, x, lam=1.0, n_sweeps=1):
+        """DROP, Table A.5: x - lam Z A^T M c(x), then the box."""
+        x = np.array(x, np.float64)
+        for _ in range(n_sweeps):
+            _L().orc_drop_sweep(_i64(self.m), _i64(self.n), _p(self.rowptr), _p(self.col), _p(self.val), _p(self.lb),
+                                _p(self.ub), _p(self.w), _p(self.lo), _p(self.hi), _dbl(lam), _p(x))
+        return x
+
+    def emr_sweep(self, x, n_sweeps=1, return_step=False):
+        """EMR, Table A.5: x - (||p||^2 / ||M^(1/2) A p||^2) p, p = A^T M c(x), then the box."""
+        x = np.array(x, np.float64)
+        step = _dbl(0.0)
+        for _ in range(n_sweeps):
+            _L().orc_emr_sweep(_i64(self.m), _i64(self.n), _p(self.rowptr), _p(self.col), _p(self.val), _p(self.lb),
+                               _p(self.ub), _p(self.w), _p(self.lo), _p(self.hi), _p(x), ctypes.byref(step))
+        return (x, step.value) if return_step else x
+
     def proximity(self, x, mode=0, p=2.0):
         x = np.ascontiguousarray(x, np.float64)
         return _L().orc_proximity(_i64(self.m), _p(self.rowptr), _p(self.col), _p(self.val), _p(self.lb), _p(self.ub),
@@ -113,7 +142,7 @@ class Oracle:
         kind = self.objective if kind is None else kind
         shape = self.shape if shape is None else shape
         k = OBJ_KIND[kind]
-        ny, nx = (shape if k == 1 else (0, 0))
+        ny, nx = (shape if k == 1 else (tuple(shape)[1:] if k == 5 else (0, 0)))
         return (_int(k), _i64(ny), _i64(nx), _i64(self.md), _p(self.d_rowptr), _p(self.d_col), _p(self.d_val))
 
     def objective_value(self, x, kind=None, shape=None):
@@ -127,6 +156,10 @@ class Oracle:
             return L.orc_tv1d(_p(x), _i64(x.size))
         if kind == "dose":
             return L.orc_dose(_i64(self.md), _p(self.d_rowptr), _p(self.d_col), _p(self.d_val), _p(x))
+        if kind == "mean":
+            return L.orc_mean(_i64(self.md), _p(self.d_rowptr), _p(self.d_col), _p(self.d_val), _p(x))
+        if kind == "tv3d":
+            return L.orc_tv3d(_p(x), _i64(shape[0]), _i64(shape[1]), _i64(shape[2]))
         return 0.0
 
     def objective_grad(self, x, kind=None, shape=None):
@@ -141,6 +174,10 @@ class Oracle:
             L.orc_tv1d_grad(_p(x), _i64(x.size), _p(g))
         elif kind == "dose":
             L.orc_dose_grad(_i64(self.md), _i64(self.n), _p(self.d_rowptr), _p(self.d_col), _p(self.d_val), _p(x), _p(g))
+        elif kind == "mean":
+            L.orc_mean_grad(_i64(self.md), _i64(self.n), _p(self.d_rowptr), _p(self.d_col), _p(self.d_val), _p(g))
+        elif kind == "tv3d":
+            L.orc_tv3d_grad(_p(x), _i64(shape[0]), _i64(shape[1]), _i64(shape[2]), _p(g))
         return g
 
     # ---- perturbation phase / superiorization ---------------------------------------------
@@ -154,9 +191,15 @@ class Oracle:
         warn = _int(0)
         fx = _dbl(0.0)
         forced_a = None if forced is None else np.ascontiguousarray(forced, np.int8)
-        t = _L().orc_perturb_phase(_i64(self.n), *self._obj_args(kind, shape), _p(x), ctypes.byref(ell_c), _i64(k),
-                                   _int(N), _dbl(beta0), _dbl(a), _int(policy), _p(dec), _p(mar), _i64(cap),
-                                   ctypes.byref(ndec), _p(forced_a), ctypes.byref(warn), ctypes.byref(fx))
+        if (self.objective if kind is None else kind) == "tv3d":
+            sh = self.shape if shape is None else shape
+            t = _L().orc_perturb_phase3(_i64(self.n), _int(5), _i64(sh[0]), _i64(sh[1]), _i64(sh[2]), _p(x), ctypes.byref(ell_c),
+                                        _i64(k), _int(N), _dbl(beta0), _dbl(a), _int(policy), _p(dec), _p(mar), _i64(cap),
+                                        ctypes.byref(ndec), _p(forced_a), ctypes.byref(warn), ctypes.byref(fx))
+        else:
+            t = _L().orc_perturb_phase(_i64(self.n), *self._obj_args(kind, shape), _p(x), ctypes.byref(ell_c), _i64(k),
+                                       _int(N), _dbl(beta0), _dbl(a), _int(policy), _p(dec), _p(mar), _i64(cap),
+                                       ctypes.byref(ndec), _p(forced_a), ctypes.byref(warn), ctypes.byref(fx))
         nd = min(ndec.value, cap)
         return dict(x=x, ell=ell_c.value, trials=int(t), decisions=dec[:nd].copy(), margins=mar[:nd].copy(), fx=fx.value,
                     warn=warn.value)
@@ -196,3 +239,35 @@ class Oracle:
         nd = min(ndec.value, cap)
         return dict(x=x, ell=ell.value, trace=trace, snaps=snaps, decisions=dec[:nd].copy(), margins=mar[:nd].copy(),
                     warn=warn)
+
+    def run(self, x0, n_iter, N=0, beta0=1.0, a=0.99, lam=1.0, algorithm="sim", policy=PER_TRIAL, ell0=0, k0=0, kind=None,
+            shape=None, n_restart=0, stop=None, forced=None, cap=1 << 22):
+        """Algorithm 1 through orc_superiorize_ex: `algorithm` in {'sim', 'block', 'drop', 'emr'} (Table A.5), any objective
+        (incl. 'mean', 'tv3d'), and the paper's stopping rule when stop = dict(prox_tol, dprox_tol, n_consec, dobj_tol)
+        (reading A-25).  One call, no snapshots (the rule's counters live inside the call).
+        Returns dict(x, ell, n_done, stop_reason, trace[n_done,4], decisions, margins, warn)."""
+        kind = self.objective if kind is None else kind
+        shape = self.shape if shape is None else shape
+        x = np.array(x0, np.float64)
+        ell = _i64(int(ell0))
+        trace = np.zeros((max(n_iter, 1), 4))
+        dec = np.zeros(cap, np.int8)
+        mar = np.zeros(cap)
+        ndec = _i64(0)
+        forced_a = None if forced is None else np.ascontiguousarray(forced, np.int8)
+        nb = self.block_rowptr.size - 1 if algorithm == "block" else 0
+        opt = _RunOpt(ALGORITHM[algorithm], int(stop is not None), 0.0, 0.0, 0, 0.0, int(n_restart),
+                      int(shape[0]) if OBJ_KIND[kind] == 5 else 0)
+        if stop is not None:
+            opt.prox_tol, opt.dprox_tol = float(stop.get("prox_tol", 1e-6)), float(stop.get("dprox_tol", 1e-8))
+            opt.n_consec, opt.dobj_tol = int(stop.get("n_consec", 5)), float(stop.get("dobj_tol", 1e-6))
+        n_done, reason = _int(0), _int(0)
+        warn = _L().orc_superiorize_ex(
+            _i64(self.m), _i64(self.n), _p(self.rowptr), _p(self.col), _p(self.val), _p(self.lb), _p(self.ub), _p(self.w),
+            _p(self.rho), _p(self.d), _p(self.lo), _p(self.hi), _dbl(lam), _int(nb), _p(self.block_rowptr) if nb else None,
+            *self._obj_args(kind, shape), _p(x), ctypes.byref(ell), _i64(k0), _int(n_iter), _int(N), _dbl(beta0), _dbl(a),
+            _int(policy), _p(trace), _p(dec), _p(mar), _i64(cap), ctypes.byref(ndec), _p(forced_a), ctypes.byref(opt),
+            ctypes.byref(n_done), ctypes.byref(reason))
+        nd = min(ndec.value, cap)
+        return dict(x=x, ell=ell.value, n_done=n_done.value, stop_reason=reason.value, trace=trace[: n_done.value].copy(),
+                    decisions=dec[:nd].copy(), margins=mar[:nd].copy(), warn=warn)

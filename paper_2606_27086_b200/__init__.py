@@ -21,6 +21,7 @@ from .binding import (  # noqa: F401
     sup_proximity,
     sup_set_blocks,
     sup_set_dose_matrix,
+    sup_set_row_mode,
     sup_superiorize,
     sup_superiorize_host,
     sup_workspace_bytes,

@@ -10,8 +10,6 @@ import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIBPATH = os.path.join(_HERE, "libsup.so")
-if os.environ.get("SUP_LIBSUP_VARIANT"):  # A/B measurements of build-time kernel parameters (see build.py build_variant)
-    _LIBPATH = os.path.join(_HERE, "libsup_" + os.environ["SUP_LIBSUP_VARIANT"] + ".so")
 _lib = None
 
 F32, F64 = 0, 1
@@ -75,9 +73,10 @@ def lib():
         L.sup_proximity.argtypes = [c_void_p, c_void_p, c_int, c_double, POINTER(c_double)]
         L.sup_objective.argtypes = [c_void_p, c_void_p, c_int, POINTER(c_int64), POINTER(c_double)]
         L.sup_get_derived.argtypes = [c_void_p, c_int, c_void_p, c_size_t]
+        L.sup_set_row_mode.argtypes = [c_void_p, c_int, c_int]
         for f in ("sup_workspace_bytes", "sup_create", "sup_destroy", "sup_set_blocks", "sup_set_dose_matrix",
                   "sup_project_simultaneous", "sup_block_iterative", "sup_forward_violation", "sup_backproject_update", "sup_perturb_tv", "sup_perturb_dose", "sup_superiorize",
-                  "sup_superiorize_host", "sup_get_state", "sup_proximity", "sup_objective", "sup_get_derived"):
+                  "sup_superiorize_host", "sup_get_state", "sup_proximity", "sup_objective", "sup_get_derived", "sup_set_row_mode"):
             getattr(L, f).restype = c_int
         _lib = L
     return _lib
@@ -207,6 +206,12 @@ def sup_set_dose_matrix(H: SupHandle, rowptr, col, val):
     H.keep += [keepD, ws]
     H._enter()
     H._check(lib().sup_set_dose_matrix(H.h, byref(D), _ptr(ws), ws.numel(), _ptr(scratch), scratch.numel()))
+    H._exit()
+
+
+def sup_set_row_mode(H: SupHandle, lanes_forward=-1, lanes_backward=-1):
+    H._enter()
+    H._check(lib().sup_set_row_mode(H.h, int(lanes_forward), int(lanes_backward)))
     H._exit()
 
 

@@ -55,6 +55,19 @@ extern "C" sup_status sup_workspace_bytes(int kind, int64_t m, int64_t n, int64_
 
 static bool aligned256(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 255u) == 0; }
 
+// Every entry point runs with the handle's device current (the device the workspace lives on) and restores the caller's.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(int dev) {
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = cudaSetDevice(dev) == cudaSuccess;
+    }
+    ~DeviceGuard() {
+        if (switched) cudaSetDevice(prev);
+    }
+};
+#define SUP_ENTER(h) DeviceGuard guard__((h)->device)
+
 extern "C" sup_status sup_create(sup_handle* out, const sup_csr* A, const void* lb, const void* ub, const void* box_lo,
                                  const void* box_hi, const void* weights, int dtype, void* workspace, size_t workspace_bytes,
                                  void* scratch, size_t scratch_bytes, void* cuda_stream) {
@@ -71,12 +84,22 @@ extern "C" sup_status sup_create(sup_handle* out, const sup_csr* A, const void* 
         return sup_fail(nullptr, SUP_ERR_WORKSPACE, "sup_create: workspace needs %zu + %zu scratch bytes, 256-byte aligned", need_p, need_s);
     int dev = 0;
     cudaDeviceProp prop;
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+    cudaPointerAttributes pattr;
+    if (cudaGetDevice(&dev) != cudaSuccess) {
         cudaGetLastError();
         return sup_fail(nullptr, SUP_ERR_CUDA, "sup_create: no usable CUDA device (libsup has no CPU fallback)");
     }
+    // the handle lives on the device that owns the workspace, whatever device is current in the calling thread
+    if (cudaPointerGetAttributes(&pattr, workspace) == cudaSuccess && pattr.type == cudaMemoryTypeDevice) dev = pattr.device;
+    else cudaGetLastError();
+    DeviceGuard guard(dev);
+    if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return sup_fail(nullptr, SUP_ERR_CUDA, "sup_create: cannot query device %d", dev);
+    }
     sup_ctx* h = new (std::nothrow) sup_ctx;
     if (!h) return sup_fail(nullptr, SUP_ERR_INVALID_ARG, "sup_create: out of host memory");
+    h->device = dev;
     h->dt = dtype;
     h->esz = dtype == SUP_F32 ? 4 : 8;
     h->stream = static_cast<cudaStream_t>(cuda_stream);
@@ -120,10 +143,6 @@ extern "C" sup_status sup_create(sup_handle* out, const sup_csr* A, const void* 
         h->colg = static_cast<int32_t*>(B.take(size_t(h->nnz) * 4));
     }
     h->xg = B.take(size_t((h->n + 511) & ~int64_t(511)) * h->esz);
-    {
-        const char* env = getenv("SUP_NO_STREAM");
-        h->use_stream = !(env && env[0] == '1');
-    }
     h->A.alloc_nnz = h->nnz;
     sup_status rc = SUP_OK;
     if (!B.ok) rc = sup_fail(h, SUP_ERR_WORKSPACE, "sup_create: workspace too small");
@@ -173,6 +192,7 @@ static void drop_graph(sup_ctx* h) {
 
 extern "C" sup_status sup_destroy(sup_handle h) {
     if (!h) return SUP_OK;
+    SUP_ENTER(h);
     cudaStreamSynchronize(h->stream);
     drop_graph(h);
     delete h;
@@ -182,6 +202,7 @@ extern "C" sup_status sup_destroy(sup_handle h) {
 extern "C" sup_status sup_set_blocks(sup_handle h, int n_blocks, const int64_t* block_rowptr, void* workspace,
                                      size_t workspace_bytes, void* scratch, size_t scratch_bytes) {
     if (!h) return SUP_ERR_INVALID_ARG;
+    SUP_ENTER(h);
     if (n_blocks < 1 || !block_rowptr) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_set_blocks: n_blocks < 1 or NULL block_rowptr");
     if (block_rowptr[0] != 0 || block_rowptr[n_blocks] != h->m)
         return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_set_blocks: block_rowptr must run from 0 to m");
@@ -240,6 +261,7 @@ extern "C" sup_status sup_set_blocks(sup_handle h, int n_blocks, const int64_t* 
 extern "C" sup_status sup_set_dose_matrix(sup_handle h, const sup_csr* D, void* workspace, size_t workspace_bytes,
                                           void* scratch, size_t scratch_bytes) {
     if (!h) return SUP_ERR_INVALID_ARG;
+    SUP_ENTER(h);
     if (!D || !D->rowptr || !D->col || !D->val || D->m <= 0 || D->n != h->n || D->nnz < 0 || D->nnz > 0x7fffffffLL)
         return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_set_dose_matrix: bad matrix (needs n columns)");
     size_t need_p = 0, need_s = 0;
@@ -280,6 +302,29 @@ extern "C" sup_status sup_set_dose_matrix(sup_handle h, const sup_csr* D, void* 
     return SUP_OK;
 }
 
+extern "C" sup_status sup_set_row_mode(sup_handle h, int lanes_forward, int lanes_backward) {
+    if (!h) return SUP_ERR_INVALID_ARG;
+    SUP_ENTER(h);
+    for (int v : {lanes_forward, lanes_backward})
+        if (!(v == -2 || v == -1 || v == 0 || v == 4 || v == 8 || v == 16 || v == 32 || v == 64))
+            return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_set_row_mode: lanes must be -2, -1, 0, 4, 8, 16, 32 or 64");
+    SUP_CUDA(h, cudaStreamSynchronize(h->stream));
+    drop_graph(h);
+    h->use_stream = lanes_forward != -2 && lanes_backward != -2;
+    h->lanes_fwd = lanes_forward < 0 ? -1 : lanes_forward;
+    h->lanes_bwd = lanes_backward < 0 ? -1 : lanes_backward;
+    h->xg_synced = false;
+    void* scratch = h->partials;  // 256 bytes are needed
+    sup_status rc = sup_stream_plan(h, h->A, 0, h->m, true, h->A.plan.table, scratch, &h->A.plan);
+    if (rc == SUP_OK) rc = sup_stream_plan(h, h->AT, 0, h->n, false, h->AT.plan.table, scratch, &h->AT.plan);
+    for (int t = 0; rc == SUP_OK && t < h->n_blocks; ++t) {
+        rc = sup_stream_plan(h, h->A, h->block_rowptr[t], h->block_rowptr[t + 1], true, h->stream_fwd_blk[t].table, scratch,
+                             &h->stream_fwd_blk[t]);
+        if (rc == SUP_OK) rc = sup_stream_plan(h, h->ATb[t], 0, h->n, false, h->ATb[t].plan.table, scratch, &h->ATb[t].plan);
+    }
+    return rc;
+}
+
 // ---- sweeps ----------------------------------------------------------------------------------------------------
 static void enqueue_simultaneous(sup_ctx* h, void* x, double lambda) {
     sup_launch_fwd(h, x, 0, h->m, h->d, &h->A.plan);
@@ -300,6 +345,7 @@ static sup_status check_lambda(sup_ctx* h, double lambda) {
 
 extern "C" sup_status sup_project_simultaneous(sup_handle h, void* x, double lambda, int n_sweeps) {
     if (!h) return SUP_ERR_INVALID_ARG;
+    SUP_ENTER(h);
     if (!x || n_sweeps < 0) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_project_simultaneous: NULL x or n_sweeps < 0");
     if (check_lambda(h, lambda) != SUP_OK) return SUP_ERR_INVALID_ARG;
     h->xg_synced = false;  // x comes from the caller
@@ -310,6 +356,7 @@ extern "C" sup_status sup_project_simultaneous(sup_handle h, void* x, double lam
 
 extern "C" sup_status sup_forward_violation(sup_handle h, const void* x) {
     if (!h) return SUP_ERR_INVALID_ARG;
+    SUP_ENTER(h);
     if (!x) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_forward_violation: NULL x");
     h->xg_synced = false;
     sup_launch_fwd(h, x, 0, h->m, h->d, &h->A.plan);
@@ -319,6 +366,7 @@ extern "C" sup_status sup_forward_violation(sup_handle h, const void* x) {
 
 extern "C" sup_status sup_backproject_update(sup_handle h, void* x, double lambda) {
     if (!h) return SUP_ERR_INVALID_ARG;
+    SUP_ENTER(h);
     if (!x) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_backproject_update: NULL x");
     if (check_lambda(h, lambda) != SUP_OK) return SUP_ERR_INVALID_ARG;
     sup_launch_bwd(h, h->AT, h->g_bwd, x, lambda);
@@ -328,6 +376,7 @@ extern "C" sup_status sup_backproject_update(sup_handle h, void* x, double lambd
 
 extern "C" sup_status sup_block_iterative(sup_handle h, void* x, double lambda, int n_sweeps) {
     if (!h) return SUP_ERR_INVALID_ARG;
+    SUP_ENTER(h);
     if (!x || n_sweeps < 0) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_block_iterative: NULL x or n_sweeps < 0");
     if (h->n_blocks < 1) return sup_fail(h, SUP_ERR_STATE, "sup_block_iterative: call sup_set_blocks first");
     if (check_lambda(h, lambda) != SUP_OK) return SUP_ERR_INVALID_ARG;
@@ -379,6 +428,7 @@ static sup_status read_state(sup_ctx* h, sup_state* out) {
 
 extern "C" sup_status sup_get_state(sup_handle h, sup_state* out) {
     if (!h) return SUP_ERR_INVALID_ARG;
+    SUP_ENTER(h);
     if (!out) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_get_state: NULL out");
     sup_status rc = read_state(h, out);
     if (rc != SUP_OK) return rc;
@@ -409,6 +459,7 @@ static sup_status perturb_alone(sup_ctx* h, void* x, int kind, const int64_t* sh
 extern "C" sup_status sup_perturb_tv(sup_handle h, void* x, int dims, const int64_t* shape, int N, double beta0, double a,
                                      int64_t* ell) {
     if (!h) return SUP_ERR_INVALID_ARG;
+    SUP_ENTER(h);
     if (dims != 1 && dims != 2) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_perturb_tv: dims must be 1 or 2");
     if (dims == 1 && shape && shape[0] != h->n) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_perturb_tv: shape[0] != n");
     return perturb_alone(h, x, dims == 2 ? SUP_OBJ_TV2D : SUP_OBJ_TV1D, shape, N, beta0, a, ell);
@@ -416,6 +467,7 @@ extern "C" sup_status sup_perturb_tv(sup_handle h, void* x, int dims, const int6
 
 extern "C" sup_status sup_perturb_dose(sup_handle h, void* x, int N, double beta0, double a, int64_t* ell) {
     if (!h) return SUP_ERR_INVALID_ARG;
+    SUP_ENTER(h);
     return perturb_alone(h, x, SUP_OBJ_DOSE, nullptr, N, beta0, a, ell);
 }
 
@@ -531,12 +583,14 @@ static sup_status run_superiorize(sup_ctx* h, void* x, int n_iter, int N, double
 
 extern "C" sup_status sup_superiorize(sup_handle h, void* x, int n_iter, int N, double beta0, double a, const sup_options* opt) {
     if (!h) return SUP_ERR_INVALID_ARG;
+    SUP_ENTER(h);
     return run_superiorize(h, x, n_iter, N, beta0, a, opt);
 }
 
 extern "C" sup_status sup_superiorize_host(sup_handle h, void* x_host, int n_iter, int N, double beta0, double a,
                                            const sup_options* opt) {
     if (!h) return SUP_ERR_INVALID_ARG;
+    SUP_ENTER(h);
     if (!x_host) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_superiorize_host: NULL x");
     const size_t bytes = size_t(h->n) * h->esz;
     SUP_CUDA(h, cudaMemcpyAsync(h->xdev, x_host, bytes, cudaMemcpyHostToDevice, h->stream));
@@ -558,6 +612,7 @@ static sup_status fetch_scalar(sup_ctx* h, double* out) {
 
 extern "C" sup_status sup_proximity(sup_handle h, const void* x, int mode, double p, double* out) {
     if (!h) return SUP_ERR_INVALID_ARG;
+    SUP_ENTER(h);
     if (!x || !out || mode < 0 || mode > 2) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_proximity: NULL x/out or mode not in {0,1,2}");
     if (mode == 1 && !(p > 0.0)) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_proximity: p must be > 0");
     double* slot = reinterpret_cast<double*>(reinterpret_cast<char*>(h->state) + offsetof(DevState, scalar_out));
@@ -567,6 +622,7 @@ extern "C" sup_status sup_proximity(sup_handle h, const void* x, int mode, doubl
 
 extern "C" sup_status sup_objective(sup_handle h, const void* x, int kind, const int64_t* shape, double* out) {
     if (!h) return SUP_ERR_INVALID_ARG;
+    SUP_ENTER(h);
     if (!x || !out) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_objective: NULL x or out");
     int64_t ny, nx;
     sup_status rc = check_objective(h, kind, shape, &ny, &nx);
@@ -578,6 +634,7 @@ extern "C" sup_status sup_objective(sup_handle h, const void* x, int kind, const
 
 extern "C" sup_status sup_get_derived(sup_handle h, int which, void* dst, size_t dst_bytes) {
     if (!h) return SUP_ERR_INVALID_ARG;
+    SUP_ENTER(h);
     const void* src = nullptr;
     size_t bytes = 0;
     switch (which) {
@@ -586,7 +643,6 @@ extern "C" sup_status sup_get_derived(sup_handle h, int which, void* dst, size_t
         case 2: src = h->AT.col; bytes = size_t(h->nnz) * 4; break;
         case 3: src = h->AT.val; bytes = size_t(h->nnz) * h->esz; break;
         case 5: src = h->y; bytes = size_t(h->m) * h->esz; break;  // y = D c(x) of the last forward product
-        case 4: src = h->partials; bytes = 2 * SUP_MAX_PARTIALS * 8; break;  // debug: per-chunk clocks (SUP_DEBUG_CHUNKS=1)
         default: return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_get_derived: unknown array");
     }
     if (!dst || dst_bytes < bytes) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_get_derived: dst too small (%zu needed)", bytes);

@@ -5,6 +5,7 @@
 #include <stdint.h>
 #include <stdio.h>
 
+#include <set>
 #include <vector>
 
 #include "sup.h"
@@ -23,6 +24,7 @@ struct StreamPlan {
     int G = 32;        // lanes per row
     bool ok = false;
     int64_t max_row = 0;
+    void* table = nullptr;  // the persistent memory `part` lives in (kept so that sup_set_row_mode can re-plan in place)
 };
 
 struct CsrD {  // device CSR (borrowed or living in workspace)
@@ -92,7 +94,10 @@ struct sup_ctx {
     void* xg = nullptr;         // [n rounded up to 512] dtype
     bool xg_synced = false;     // enqueue-time flag: xg mirrors x (set by the back-projection, cleared when x changes elsewhere)
     int stream_nb = 0;          // persistent grid of the row-stream kernels (-1: unavailable)
-    bool use_stream = true;       // SUP_NO_STREAM=1 in the environment turns the row-stream kernels off (A/B measurements)
+    bool use_stream = true;     // false: the group-per-row kernels of sup_spmv.cu (sup_set_row_mode(h, -2, -2))
+    int lanes_fwd = -1, lanes_bwd = -1;      // sup_set_row_mode overrides of the lanes per row (-1: planner's choice)
+    std::set<const void*> smem_opted_in;     // kernels already opted in to > 48 KB dynamic shared memory on this handle's device
+    int device = 0;             // CUDA device of the workspace; every entry point runs with it current
     // block-iterative
     int n_blocks = 0;
     std::vector<int64_t> block_rowptr;

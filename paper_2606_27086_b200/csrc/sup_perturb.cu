@@ -698,10 +698,6 @@ int sup_perturb_grid(sup_ctx* h, int objective) {
         if (want > 2 * int64_t(h->num_sms)) want = 2 * int64_t(h->num_sms);
         if (want > SUP_MAX_PARTIALS / SUP_TRIAL_BATCH) want = SUP_MAX_PARTIALS / SUP_TRIAL_BATCH;  // one partial row per candidate
     }
-    if (const char* env = getenv("SUP_PERTURB_GRID")) {  // measurement override
-        const int64_t v = atoll(env);
-        if (v > 0 && objective != SUP_OBJ_DOSE) want = v < SUP_MAX_PARTIALS / SUP_TRIAL_BATCH ? v : SUP_MAX_PARTIALS / SUP_TRIAL_BATCH;
-    }
     if (want < 1) want = 1;
     return int(want < cap ? want : cap);
 }

@@ -41,12 +41,10 @@
 // stages of the ring of k_staged<T, MODE>; the ring capacity STG * RG_TILE need not be a power of two
 template <typename T, int MODE>
 __host__ __device__ constexpr int rg_stages() { return (MODE == 0 && sizeof(T) == 4) ? RG_STAGES_FWD : RG_STAGES; }
-#define RG_CWARPS 16                        // consumer warps
-#define RG_THREADS (32 * (RG_CWARPS + 1))   // + producer warp
-#ifndef RG_PLANES
-#define RG_PLANES 1                         // producer lanes (1, 4, 8 measured: no gain from more than one)
+#define RG_CWARPS 16                        // upper bound on the consumer warps (sizes of the shared arrays)
+#ifndef RG_NCW
+#define RG_NCW 12                           // consumer warps: measured best on config 3 (8: 4.50/4.23, 12: 4.63/4.94, 16: 4.50/4.78 TB/s fwd/bwd)
 #endif
-#define RG_CWARPS_DEFAULT 12                // measured best on config 3 (8: 4.50/4.23, 12: 4.63/4.94, 16: 4.50/4.78 TB/s fwd/bwd)
 #ifndef RG_UNROLL
 #define RG_UNROLL 16                        // independent gathers in flight per lane (a multiple of 4)
 #endif
@@ -187,7 +185,7 @@ template <typename T, int MODE, int G, int NCW>
 __global__ void __launch_bounds__(32 * (NCW + 1), 1)
     k_staged(const int64_t* __restrict__ part, const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
              const T* __restrict__ val, const uint2* __restrict__ pk, const T* __restrict__ vec, const T* __restrict__ p1,
-             const T* __restrict__ p2, const T* __restrict__ p3, T* out, T* out2, T lambda, int64_t nnz_total, double* dbg) {
+             const T* __restrict__ p2, const T* __restrict__ p3, T* out, T* out2, T lambda, int64_t nnz_total) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int STG = rg_stages<T, MODE>();
     constexpr int RG_ELEMS = STG * RG_TILE;
@@ -196,9 +194,9 @@ __global__ void __launch_bounds__(32 * (NCW + 1), 1)
     if (rs >= re) return;
     const int64_t es = rowptr[rs], ee = rowptr[re];
     const int64_t base = es & ~int64_t(3);  // 16-byte aligned start of the stream (4 elements)
-    const int ntiles = int((ee - base + RG_TILE - 1) / RG_TILE);
+    // an all-empty range streams nothing (no copy may be left in flight when the CTA exits)
+    const int ntiles = ee > es ? int((ee - base + RG_TILE - 1) / RG_TILE) : 0;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const long long t_begin = clock64();
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < STG; ++s) mbar_init(smem_u32(&S.full[s]), 1);
@@ -211,13 +209,13 @@ __global__ void __launch_bounds__(32 * (NCW + 1), 1)
     volatile int* issued = S.issued;
 
     if (warp == NCW) {
-        // ---- producers: RG_PLANES lanes feed the ring, lane p the tiles t = p (mod RG_PLANES) -------------------------
-        // (more than one producer lane brought nothing: the limit was the copy engine's per-copy cost, not the issue loop)
-        if (lane < RG_PLANES) {
+        // ---- producer: one lane feeds the ring (more lanes brought nothing: the limit is the copy engine's per-copy
+        // cost, not the issue loop; profiles/r01c_staged.md) -----------------------------------------------------------
+        if (lane == 0) {
             const uint64_t pol = l2_evict_first_policy();
             const int64_t bulk_limit = nnz_total & ~int64_t(3);  // bulk copies never read past the arrays' last whole 16 B
             int freed = 0;                                        // min over the consumer warps' progress
-            for (int t = lane; t < ntiles; t += RG_PLANES) {
+            for (int t = 0; t < ntiles; ++t) {
                 const int s = t % STG;
                 if (t >= STG && freed <= t - STG) {
                     const long long t0 = clock64();
@@ -262,6 +260,9 @@ __global__ void __launch_bounds__(32 * (NCW + 1), 1)
                 }
                 issued[s] = t + 1;  // the stage's barrier is armed for tile t: consumers may now wait on its phase
             }
+            // Do not leave while a copy may still be in flight into this CTA's shared memory (the consumers wait on every
+            // tile their rows touch, but a tile holding only alignment padding or the tail of an empty row has no reader).
+            for (int t = ntiles > STG ? ntiles - STG : 0; t < ntiles; ++t) mbar_wait(smem_u32(&S.full[t % STG]), (t / STG) & 1);
         }
         return;
     }
@@ -441,12 +442,6 @@ __global__ void __launch_bounds__(32 * (NCW + 1), 1)
     // this warp needs nothing more
     __syncwarp();
     if (lane == 0) progress[warp] = ntiles;
-    if (dbg && lane == 0 && blockIdx.x < SUP_MAX_PARTIALS) {  // SUP_DEBUG_CHUNKS=1: per-chunk clocks (max over warps), SM id, size
-        unsigned smid;
-        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
-        atomicMax(reinterpret_cast<unsigned long long*>(dbg) + blockIdx.x, (unsigned long long)(clock64() - t_begin));
-        if (warp == 0) dbg[SUP_MAX_PARTIALS + blockIdx.x] = double(smid) + double(ee - es) * 1024.0;
-    }
     }
 }
 
@@ -492,12 +487,11 @@ size_t sup_stream_table_bytes() { return ((size_t(SUP_STREAM_NBMAX) + 1) * 8 + 2
 
 template <typename T, int MODE>
 static int staged_occupancy() {
-    if (cudaFuncSetAttribute(k_staged<T, MODE, 32, RG_CWARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(sizeof(RgSmem<T, rg_stages<T, MODE>()>))) != cudaSuccess) {
-        cudaGetLastError();
-        return 0;
-    }
+    const void* fn = reinterpret_cast<const void*>(&k_staged<T, MODE, 32, RG_NCW>);
+    const int smem = int(sizeof(RgSmem<T, rg_stages<T, MODE>()>));
     int occ = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_staged<T, MODE, 32, RG_CWARPS>, RG_THREADS, sizeof(RgSmem<T, rg_stages<T, MODE>()>)) != cudaSuccess) {
+    if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess ||
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, 32 * (RG_NCW + 1), smem) != cudaSuccess) {
         cudaGetLastError();
         return 0;
     }
@@ -518,22 +512,16 @@ static int stream_grid(sup_ctx* h) {  // persistent grid = resident CTAs per SM 
     return h->stream_nb;
 }
 
-static int sup_stream_chunks(bool forward) {
-    const char* env = getenv(forward ? "SUP_CHUNKS_FWD" : "SUP_CHUNKS_BWD");
-    const int v = env ? atoi(env) : 0;
-    return v > 0 ? v : 1;
-}
-
 sup_status sup_stream_plan(sup_ctx* h, const CsrD& M, int64_t r0, int64_t r1, bool forward, void* table, void* scratch,
                            StreamPlan* out) {
-    const int chunks_per_cta = sup_stream_chunks(forward);
     *out = StreamPlan();
+    out->table = table;
     if (!h->use_stream || r1 <= r0) return SUP_OK;
     int nb = stream_grid(h);
     if (nb < 1) return SUP_OK;
-    {   // optionally more, smaller chunks than resident CTAs (SUP_CHUNKS_FWD / SUP_CHUNKS_BWD; default 1)
-        int64_t want = int64_t(nb) * (chunks_per_cta > 0 ? chunks_per_cta : 1);
-        const int64_t most = (r1 - r0 + 63) / 64;  // keep >= 64 rows per chunk
+    {   // one chunk per resident CTA, but keep >= 64 rows per chunk
+        int64_t want = nb;
+        const int64_t most = (r1 - r0 + 63) / 64;
         if (want > most) want = most;
         if (want > SUP_STREAM_NBMAX) want = SUP_STREAM_NBMAX;
         nb = want < 1 ? 1 : int(want);
@@ -554,15 +542,13 @@ sup_status sup_stream_plan(sup_ctx* h, const CsrD& M, int64_t r0, int64_t r1, bo
     SUP_CUDA(h, cudaStreamSynchronize(h->stream));
     SUP_CUDA(h, cudaGetLastError());
     // Lanes per row: the rows a warp holds at once (32/G of them) should total ~a tile -- enough elements per lane to
-    // amortise the per-row work, few enough that the 16 warps' rows together leave ring stages free for prefetch --
-    // and must never span more than RG_STAGES - 1 tiles.
+    // amortise the per-row work, few enough that the consumer warps' rows together leave ring stages free for prefetch --
+    // and must never span more than RG_STAGES - 1 tiles.  sup_set_row_mode() overrides the choice.
     const double avg = double(ends[1] - ends[0]) / double(r1 - r0);
     int G = 4;
-    while (G < 32 && avg * (32.0 / G) > 960.0) G <<= 1;  // a warp's rows total ~a tile (G = 64, a warp pair per row, only by override)
-    if (const char* env = getenv(forward ? "SUP_STREAM_G_FWD" : "SUP_STREAM_G_BWD")) {
-        const int g = atoi(env);
-        if (g == 0 || g == 4 || g == 8 || g == 16 || g == 32 || g == 64) G = g;
-    }
+    while (G < 32 && avg * (32.0 / G) > 960.0) G <<= 1;
+    const int forced = forward ? h->lanes_fwd : h->lanes_bwd;
+    if (forced >= 0) G = forced;
     const int64_t cap = int64_t(RG_STAGES - 2) * RG_TILE;
     while (G < 32 && G > 0 && int64_t(mx_h) * (32 / G) > cap) G <<= 1;
     if (G != 0 && (avg > 2048.0 || int64_t(mx_h) * (G >= 32 ? 1 : 32 / G) > cap)) G = 0;  // long rows: the whole CTA per row, no length limit
@@ -575,48 +561,20 @@ sup_status sup_stream_plan(sup_ctx* h, const CsrD& M, int64_t r0, int64_t r1, bo
 }
 
 // ---- launchers --------------------------------------------------------------------------------------------------------
-static bool stream_debug() {
-    static int v = -1;
-    if (v < 0) {
-        const char* env = getenv("SUP_DEBUG_CHUNKS");
-        v = env && env[0] == '1';
-    }
-    return v == 1;
-}
-
-static int stream_cwarps() {  // consumer warps per CTA: 8, 12 or 16 (SUP_STREAM_CWARPS)
-    static int v = -1;
-    if (v < 0) {
-        const char* env = getenv("SUP_STREAM_CWARPS");
-        v = env ? atoi(env) : RG_CWARPS_DEFAULT;
-        if (v != 8 && v != 12 && v != 16) v = RG_CWARPS_DEFAULT;
-    }
-    return v;
-}
-
-template <typename T, int MODE, int G, int NCW>
-static void launch_staged_gw(sup_ctx* h, const StreamPlan& sp, const CsrD& M, const void* vec, const void* p1, const void* p2,
-                             const void* p3, void* out, void* out2, double lambda) {
-    static bool attr_set = false;  // per instantiation: opt in to > 48 KB of dynamic shared memory once
-    if (!attr_set) {
-        cudaFuncSetAttribute(k_staged<T, MODE, G, NCW>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(sizeof(RgSmem<T, rg_stages<T, MODE>()>)));
-        attr_set = true;
-    }
-    k_staged<T, MODE, G, NCW><<<sp.nb, 32 * (NCW + 1), sizeof(RgSmem<T, rg_stages<T, MODE>()>), h->stream>>>(
-        sp.part, M.rowptr, M.col, static_cast<const T*>(M.val), static_cast<const uint2*>(M.pk), static_cast<const T*>(vec),
-        static_cast<const T*>(p1), static_cast<const T*>(p2), static_cast<const T*>(p3), static_cast<T*>(out),
-        static_cast<T*>(out2), T(lambda), M.alloc_nnz, stream_debug() ? h->partials : nullptr);
-    h->launches++;
-}
-
 template <typename T, int MODE, int G>
 static void launch_staged_g(sup_ctx* h, const StreamPlan& sp, const CsrD& M, const void* vec, const void* p1, const void* p2,
                             const void* p3, void* out, void* out2, double lambda) {
-    switch (stream_cwarps()) {
-        case 8: launch_staged_gw<T, MODE, G, 8>(h, sp, M, vec, p1, p2, p3, out, out2, lambda); break;
-        case 12: launch_staged_gw<T, MODE, G, 12>(h, sp, M, vec, p1, p2, p3, out, out2, lambda); break;
-        default: launch_staged_gw<T, MODE, G, 16>(h, sp, M, vec, p1, p2, p3, out, out2, lambda); break;
+    const void* fn = reinterpret_cast<const void*>(&k_staged<T, MODE, G, RG_NCW>);
+    constexpr int smem = int(sizeof(RgSmem<T, rg_stages<T, MODE>()>));
+    if (!h->smem_opted_in.count(fn)) {  // per handle, hence per device: opt in to > 48 KB of dynamic shared memory
+        cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        h->smem_opted_in.insert(fn);
     }
+    k_staged<T, MODE, G, RG_NCW><<<sp.nb, 32 * (RG_NCW + 1), smem, h->stream>>>(
+        sp.part, M.rowptr, M.col, static_cast<const T*>(M.val), static_cast<const uint2*>(M.pk), static_cast<const T*>(vec),
+        static_cast<const T*>(p1), static_cast<const T*>(p2), static_cast<const T*>(p3), static_cast<T*>(out),
+        static_cast<T*>(out2), T(lambda), M.alloc_nnz);
+    h->launches++;
 }
 
 template <typename T, int MODE>

@@ -667,14 +667,13 @@ def test_restarted_perturbations(dtype):
 
 @pytest.mark.parametrize("dtype", [0, 1])
 @pytest.mark.parametrize("name", ["cfg4_small", "ct_ragged", "cfg5_k16"])
-def test_long_row_mode_of_the_staged_kernels(name, dtype, monkeypatch):
+def test_long_row_mode_of_the_staged_kernels(name, dtype):
     """The whole-CTA-per-row mode (chosen for rows of thousands of nonzeros: config 4's A^T at full size) forced on both
     products of small problems, including rows shorter than a piece, empty rows and rows spanning several ring tiles."""
     sup = _sup()
-    monkeypatch.setenv("SUP_STREAM_G_FWD", "0")
-    monkeypatch.setenv("SUP_STREAM_G_BWD", "0")
     P = problem(name)
     H = make_handle(P, dtype, blocks=False)
+    sup.sup_set_row_mode(H, 0, 0)
     O = Oracle.from_problem(P)
     x = xdev(P, dtype)
     xo = P.x0.astype(np.float64)

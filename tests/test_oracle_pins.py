@@ -575,3 +575,218 @@ def test_restarted_perturbations():
     pert = O.perturb(xR, 1, P.N, P.beta0, a)
     assert np.linalg.norm(pert["x"] - xR) <= P.beta0 * a / (1 - a) + 1e-12
     assert np.all(np.isfinite(rs["trace"]))
+
+
+# ------------------------------------------------------------------------------------------------
+# DROP and EMR (Table A.5)
+# ------------------------------------------------------------------------------------------------
+def equality_system(rng, m, n, density=0.6, noise=0.0):
+    A = rng.normal(size=(m, n)) * (rng.random((m, n)) < density)
+    A[np.abs(A).sum(1) == 0, 0] = 1.0
+    A[0, np.abs(A).sum(0) == 0] = 0.5  # every column holds at least one entry
+    b = A @ rng.uniform(0.2, 0.8, n) + noise * rng.normal(size=m)
+    return A, b
+
+
+@pytest.mark.parametrize("seed", range(3))
+def test_drop_is_the_printed_update(seed):
+    """x - Z A^T M (A x - b), Z = diag(1/nnz(A_:,j)), M = diag(w_i), sum w = 1 -- the dense NumPy expression of the table."""
+    rng = np.random.default_rng(100 + seed)
+    m, n = 14, 6
+    A, b = equality_system(rng, m, n, noise=0.1)
+    w = rng.uniform(0.5, 2.0, m)
+    O = make(A, b, b, w=w)
+    x = rng.normal(size=n)
+    Z = 1.0 / np.count_nonzero(A, axis=0)
+    M = w / w.sum()
+    for lam in (1.0, 0.3):
+        np.testing.assert_allclose(O.drop_sweep(x, lam), x - lam * Z * (A.T @ (M * (A @ x - b))), rtol=1e-13, atol=1e-15)
+    # a column with one stored entry per row-support: with Z = I (every column has exactly one entry) DROP is x - A^T M c
+    D = np.diag(rng.uniform(0.5, 2.0, n))
+    Od = make(D, np.ones(n), np.ones(n))
+    np.testing.assert_allclose(Od.drop_sweep(x), x - D.T @ ((1.0 / n) * (D @ x - 1.0)), rtol=1e-13)
+    # a feasible point is fixed, and the box follows the step (L427)
+    xs = np.linalg.lstsq(A[:n], b[:n], rcond=None)[0]
+    Of = make(A[:n], b[:n], b[:n])
+    np.testing.assert_allclose(Of.drop_sweep(xs), xs, atol=1e-12)
+    Ob = make(A, b, b, lo=np.full(n, 0.4), hi=np.full(n, 0.6), w=w)
+    np.testing.assert_array_equal(Ob.drop_sweep(x), np.clip(O.drop_sweep(x), 0.4, 0.6))
+
+
+@pytest.mark.parametrize("seed", range(3))
+def test_emr_step_is_the_exact_line_minimiser(seed):
+    """EMR's factor ||p||^2 / ||M^(1/2) A p||^2 minimises phi(t) = ||M^(1/2)(A(x - t p) - b)||^2: phi'(t*) = 0, checked on
+    the oracle's new point, by finite differences of phi, and against the dense expression."""
+    rng = np.random.default_rng(200 + seed)
+    m, n = 12, 7
+    A, b = equality_system(rng, m, n, noise=0.2)
+    w = rng.uniform(0.5, 2.0, m)
+    M = w / w.sum()
+    O = make(A, b, b, w=w)
+    x = rng.normal(size=n)
+    xn, t = O.emr_sweep(x, return_step=True)
+    p = A.T @ (M * (A @ x - b))
+    assert t == pytest.approx((p @ p) / np.sum(M * (A @ p) ** 2), rel=1e-13)
+    np.testing.assert_allclose(xn, x - t * p, rtol=1e-13, atol=1e-15)
+    phi = lambda s: float(np.sum(M * (A @ (x - s * p) - b) ** 2))
+    # derivative at the new point along p: -2 <M^(1/2) A p, M^(1/2)(A xn - b)> = 0
+    assert abs(np.sum(M * (A @ p) * (A @ xn - b))) <= 1e-12 * np.sum(M * (A @ p) ** 2) * max(1.0, abs(t))
+    h = 1e-5 * t
+    assert phi(t) <= phi(t + h) and phi(t) <= phi(t - h)
+    assert abs(phi(t + h) - phi(t - h)) <= 1e-7 * phi(t) + 1e-18
+    # the weighted residual never increases, and on a consistent system EMR converges to a solution
+    Ac, bc = equality_system(rng, m, n)
+    Oc = make(Ac, bc, bc)
+    xc = np.zeros(n)
+    res = [np.sum((Ac @ xc - bc) ** 2)]
+    for _ in range(400):
+        xc = Oc.emr_sweep(xc)
+        res.append(np.sum((Ac @ xc - bc) ** 2))
+    assert all(b_ <= a_ * (1 + 1e-12) for a_, b_ in zip(res, res[1:]))
+    assert res[-1] <= 1e-12 * res[0]
+    # p = 0 (feasible point): step 0, x untouched
+    xf = np.linalg.lstsq(Ac, bc, rcond=None)[0]
+    np.testing.assert_allclose(Oc.emr_sweep(xf), xf, atol=1e-12)
+
+
+def test_drop_and_emr_inside_algorithm_1():
+    """Oracle.run with algorithm='drop'/'emr' is perturbation phase + that sweep, replayed by hand from the primitives."""
+    rng = np.random.default_rng(7)
+    ny, nx = 5, 6
+    n = ny * nx
+    A, b = equality_system(rng, 40, n, density=0.3, noise=0.05)
+    O = make(A, b, b, lo=np.zeros(n), hi=np.ones(n), objective="tv2d", shape=(ny, nx))
+    x0 = rng.uniform(0, 1, n)
+    for alg, sweep in (("drop", lambda x: O.drop_sweep(x, 0.8)), ("emr", lambda x: O.emr_sweep(x))):
+        R = O.run(x0, 4, N=2, beta0=0.5, a=0.8, lam=0.8, algorithm=alg)
+        x, ell = x0.copy(), 0
+        for k in range(4):
+            Pp = O.perturb(x, ell, 2, 0.5, 0.8, k=k)
+            x, ell = sweep(Pp["x"]), Pp["ell"]
+        np.testing.assert_array_equal(R["x"], x)
+        assert R["ell"] == ell and R["n_done"] == 4 and R["stop_reason"] == 0
+
+
+# ------------------------------------------------------------------------------------------------
+# SURVEY.md 8(f) rank 3: f_Mean (Eq. 21, PAPER.md:L389-393) and 3-D TV (Eq. 15 with a third difference, A-27)
+# ------------------------------------------------------------------------------------------------
+def test_mean_objective_is_linear_and_every_step_is_accepted():
+    rng = np.random.default_rng(9)
+    md, n = 11, 5
+    D = rng.uniform(0, 1, (md, n)) * (rng.random((md, n)) < 0.7)
+    rp, c, v = dense_to_csr(D)
+    O = make(np.eye(n), np.zeros(n), np.ones(n), dose=(rp, c, v, md), objective="mean")
+    x = rng.uniform(0, 2, n)
+    g = O.objective_grad(x)
+    assert O.objective_value(x) == pytest.approx((D @ x).mean(), rel=1e-14)
+    np.testing.assert_allclose(g, D.T @ np.ones(md) / md, rtol=1e-14)
+    np.testing.assert_array_equal(g, O.objective_grad(rng.normal(size=n)))  # constant gradient
+    assert O.objective_value(x) == pytest.approx(g @ x, rel=1e-13)
+    # f(x + beta v) - f(x) = -beta ||g|| exactly (v = -g/||g||): every trial is accepted, l advances by N
+    res = O.perturb(x, 2, N=3, beta0=0.7, a=0.9)
+    betas = 0.7 * 0.9 ** np.arange(2, 5)
+    assert list(res["decisions"]) == [1, 1, 1] and res["ell"] == 5
+    np.testing.assert_allclose(res["x"], x - betas.sum() * g / np.linalg.norm(g), rtol=1e-13)
+    assert res["fx"] == pytest.approx(O.objective_value(x) - betas.sum() * np.linalg.norm(g), rel=1e-12)
+
+
+def tv3(O, X):
+    return O.objective_value(np.asarray(X, float).ravel(), "tv3d", X.shape)
+
+
+def tv3g(O, X):
+    return O.objective_grad(np.asarray(X, float).ravel(), "tv3d", X.shape).reshape(X.shape)
+
+
+def test_tv3d_value_closed_forms(O0):
+    nz, ny, nx = 4, 5, 6
+    assert tv3(O0, np.full((nz, ny, nx), 1.3)) == 0.0
+    i, j, k = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    al, be, ga = 0.3, -1.1, 0.7
+    assert tv3(O0, al * i + be * j + ga * k) == pytest.approx((nz - 1) * (ny - 1) * (nx - 1) * np.sqrt(al**2 + be**2 + ga**2), rel=1e-13)
+    X = np.zeros((nz, ny, nx))
+    X[2, 2, 2] = 0.8  # one interior voxel: three terms see it as a neighbour (delta each), its own term sqrt(3) delta
+    assert tv3(O0, X) == pytest.approx((3 + np.sqrt(3)) * 0.8, rel=1e-14)
+    Y = np.random.default_rng(0).uniform(size=(nz, ny, nx))
+    base = tv3(O0, Y)
+    Y2 = Y.copy()
+    Y2[-1, -1, -1] += 5.0  # the last corner starts no term and is nobody's +1 neighbour along all three axes of a term
+    assert tv3(O0, Y2) == base
+    # a volume constant along z reduces to (nz-1) copies of the 2-D value on the slices
+    S = np.random.default_rng(1).uniform(size=(ny, nx))
+    assert tv3(O0, np.broadcast_to(S, (nz, ny, nx)).copy()) == pytest.approx((nz - 1) * tv(O0, S), rel=1e-13)
+
+
+def test_tv3d_gradient(O0):
+    rng = np.random.default_rng(3)
+    nz, ny, nx = 4, 5, 3
+    X = rng.uniform(size=(nz, ny, nx))
+    g = tv3g(O0, X)
+    h = 1e-6
+    for _ in range(25):
+        q = tuple(rng.integers(0, s) for s in X.shape)
+        Xp, Xm = X.copy(), X.copy()
+        Xp[q] += h
+        Xm[q] -= h
+        assert g[q] == pytest.approx((tv3(O0, Xp) - tv3(O0, Xm)) / (2 * h), abs=2e-7)
+    assert abs(g.sum()) <= 1e-12  # TV ignores constants
+    assert np.sum(g * X) == pytest.approx(tv3(O0, X), rel=1e-12)  # 1-homogeneous
+    assert np.all(tv3g(O0, np.full((nz, ny, nx), 2.0)) == 0.0)  # t = 0 terms contribute 0 (A-9)
+    # perturbation phase with the 3-D objective: accepted steps really decrease f
+    O = make(np.eye(X.size), np.zeros(X.size), np.ones(X.size), objective="tv3d", shape=X.shape)
+    res = O.perturb(X.ravel(), 0, N=3, beta0=0.5, a=0.7)
+    assert res["fx"] <= tv3(O0, X) and res["fx"] == pytest.approx(tv3(O0, res["x"].reshape(X.shape)), rel=1e-14)
+
+
+# ------------------------------------------------------------------------------------------------
+# SURVEY.md 8(f) rank 1b: the paper's stopping rule (PAPER.md:L217-223, L239-243; reading A-25)
+# ------------------------------------------------------------------------------------------------
+def test_stopping_rule_never_firing_is_the_fixed_run_bitwise():
+    rng = np.random.default_rng(12)
+    A, lb, ub, _ = random_system(rng, 20, 6, consistent=False)
+    O = make(A, lb, ub, lo=np.zeros(6), hi=np.ones(6), objective="tv1d")
+    x0 = rng.uniform(0, 1, 6)
+    ref = O.run(x0, 15, N=2, beta0=0.5, a=0.9)
+    R = O.run(x0, 15, N=2, beta0=0.5, a=0.9, stop=dict(prox_tol=-1.0, dprox_tol=0.0, n_consec=5, dobj_tol=0.0))
+    assert R["n_done"] == 15 and R["stop_reason"] == 0
+    np.testing.assert_array_equal(R["x"], ref["x"])
+    np.testing.assert_array_equal(R["x"], O.superiorize(x0, 15, 2, 0.5, 0.9, kind="tv1d")["x"])
+
+
+def test_stopping_rule_fires_where_the_definition_says():
+    """Replay: P^k (Eq. 12, p = 2) and f^k recomputed from the per-sweep iterates of a fixed-length run; the rule must stop
+    at the first k with (P^k <= P* or N consecutive dP < dP*) [and df < df*]."""
+    rng = np.random.default_rng(13)
+    A, lb, ub, _ = random_system(rng, 12, 5, consistent=True, slack=0.4)
+    n = 5
+    for perturbed in (False, True):
+        O = make(A, lb, ub, lo=np.zeros(n), hi=np.ones(n), objective="tv1d" if perturbed else None)
+        x0 = rng.uniform(0, 1, n)
+        N = 2 if perturbed else 0
+        K = 400
+        xs = [x0]
+        x, ell = x0.copy(), 0
+        for k in range(K):
+            if perturbed:
+                Pp = O.perturb(x, ell, N, 0.3, 0.8, k=k)
+                x, ell = Pp["x"], Pp["ell"]
+            x = O.sweep(x)
+            xs.append(x)
+        Pk = [O.proximity(v, 1, 2.0) for v in xs]
+        fk = [O.objective_value(v) if perturbed else 0.0 for v in xs]
+        for stop in (dict(prox_tol=1e-9, dprox_tol=0.0, n_consec=5, dobj_tol=1e-3),
+                     dict(prox_tol=-1.0, dprox_tol=1e-6, n_consec=3, dobj_tol=1e-2)):
+            want, consec = K, 0
+            for k in range(1, K):
+                c1 = Pk[k] <= stop["prox_tol"]
+                consec = consec + 1 if abs(Pk[k] - Pk[k - 1]) / max(1.0, Pk[k - 1]) < stop["dprox_tol"] else 0
+                c2 = consec >= stop["n_consec"]
+                cf = abs(fk[k] - fk[k - 1]) / max(1.0, fk[k - 1]) < stop["dobj_tol"]
+                if (c1 or c2) and (cf or not perturbed):
+                    want = k
+                    reason = c1 + 2 * c2 + 4 * (perturbed and cf)
+                    break
+            R = O.run(x0, K, N=N, beta0=0.3, a=0.8, stop=stop)
+            assert want < K, "the test system must trigger the rule"
+            assert R["n_done"] == want and R["stop_reason"] == reason
+            np.testing.assert_array_equal(R["x"], xs[want])
