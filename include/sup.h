@@ -61,7 +61,10 @@ typedef enum {
     SUP_OBJ_NONE = 0, /* no perturbation: the basic algorithm (Eq. 10 with beta v = 0) */
     SUP_OBJ_TV2D = 1, /* isotropic total variation, Eq. 15, on x viewed as ny x nx row-major */
     SUP_OBJ_TV1D = 2, /* sum |x_{i+1} - x_i|  (A-16) */
-    SUP_OBJ_DOSE = 3  /* || D_body x ||^2     (A-15; north_star) */
+    SUP_OBJ_DOSE = 3, /* || D_body x ||^2     (A-15; north_star) */
+    SUP_OBJ_MEAN = 4, /* f_Mean = (1/N_S) sum_{i in S} (D_S x)_i, Eq. 21; D_S is the matrix given to
+                         sup_set_dose_matrix (its rows are the structure's voxels) */
+    SUP_OBJ_TV3D = 5  /* Eq. 15 with a third difference on x viewed as nz x ny x nx (A-27) */
 } sup_objective_kind;
 
 /* step-size exponent policy (A-10) */
@@ -84,7 +87,7 @@ typedef struct {
 /* options of sup_superiorize; zero-initialise, then set what is needed */
 typedef struct {
     int objective;         /* sup_objective_kind */
-    int64_t shape[3];      /* TV2D: {ny, nx, 0} with ny*nx == n; others ignored */
+    int64_t shape[3];      /* TV2D: {ny, nx, 0} with ny*nx == n; TV3D: {nz, ny, nx} with nz*ny*nx == n; others ignored */
     double lambda;         /* relaxation in [0,2] (Eq. 3) */
     int block_iterative;   /* 0: simultaneous sweep; 1: block-iterative sweep (needs sup_set_blocks) */
     int step_policy;       /* sup_step_policy */
@@ -134,6 +137,16 @@ sup_status sup_set_blocks(sup_handle h, int n_blocks, const int64_t* block_rowpt
 /* Dose objective matrix D_body (md x n CSR, same dtype; A-15): borrowed; builds its transposed CSR. */
 sup_status sup_set_dose_matrix(sup_handle h, const sup_csr* D_body, void* workspace, size_t workspace_bytes,
                                void* scratch, size_t scratch_bytes);
+
+/* Layout hint for the two gathered vectors (DESIGN.md section 4 "gather layouts").  The forward product gathers x and the
+ * back-projection gathers y = D c(x) at the column / row indices of the nonzeros.  When an index space is a row-major
+ * 2-D array -- x an image of x_shape = {rows, cols} pixels (rows * cols = n), the rows of A a sinogram of
+ * y_shape = {angles, bins} (angles * bins = m) -- the library keeps its internal copies of x and y in 128-byte tiles of
+ * 4 x 8 elements (fp64: 4 x 4) so that one warp's gathers along a ray touch few cache lines.  Either pointer may be NULL
+ * (or {0, 0}): no hint for that side.  HOST arrays.  Pure data layout: every sum is formed from the same numbers in the
+ * same order, results are bit-identical with and without the hint.  Rewrites the packed copies, drops the cached graph,
+ * synchronises. */
+sup_status sup_set_layout(sup_handle h, const int64_t* x_shape, const int64_t* y_shape);
 
 /* Expert control of the two product kernels (S1+S2, S3), for tests and measurements: how many
  * lanes cooperate on one row of A (forward) and of A^T (backward).  -1: the planner's choice from the mean and the

@@ -21,9 +21,10 @@ from .binding import (  # noqa: F401
     sup_proximity,
     sup_set_blocks,
     sup_set_dose_matrix,
+    sup_set_layout,
     sup_set_row_mode,
     sup_superiorize,
     sup_superiorize_host,
     sup_workspace_bytes,
-    OBJ_NONE, OBJ_TV2D, OBJ_TV1D, OBJ_DOSE, PER_TRIAL, PER_SWEEP, F32, F64,
+    OBJ_NONE, OBJ_TV2D, OBJ_TV1D, OBJ_DOSE, OBJ_MEAN, OBJ_TV3D, PER_TRIAL, PER_SWEEP, F32, F64,
 )

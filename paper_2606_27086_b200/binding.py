@@ -13,10 +13,10 @@ _LIBPATH = os.path.join(_HERE, "libsup.so")
 _lib = None
 
 F32, F64 = 0, 1
-OBJ_NONE, OBJ_TV2D, OBJ_TV1D, OBJ_DOSE = 0, 1, 2, 3
+OBJ_NONE, OBJ_TV2D, OBJ_TV1D, OBJ_DOSE, OBJ_MEAN, OBJ_TV3D = 0, 1, 2, 3, 4, 5
 PER_TRIAL, PER_SWEEP = 0, 1
 WS_CREATE, WS_BLOCKS, WS_DOSE = 0, 1, 2
-_OBJ = {None: OBJ_NONE, "none": OBJ_NONE, "tv2d": OBJ_TV2D, "tv1d": OBJ_TV1D, "dose": OBJ_DOSE}
+_OBJ = {None: OBJ_NONE, "none": OBJ_NONE, "tv2d": OBJ_TV2D, "tv1d": OBJ_TV1D, "dose": OBJ_DOSE, "mean": OBJ_MEAN, "tv3d": OBJ_TV3D}
 
 
 class SupError(RuntimeError):
@@ -74,9 +74,10 @@ def lib():
         L.sup_objective.argtypes = [c_void_p, c_void_p, c_int, POINTER(c_int64), POINTER(c_double)]
         L.sup_get_derived.argtypes = [c_void_p, c_int, c_void_p, c_size_t]
         L.sup_set_row_mode.argtypes = [c_void_p, c_int, c_int]
+        L.sup_set_layout.argtypes = [c_void_p, POINTER(c_int64), POINTER(c_int64)]
         for f in ("sup_workspace_bytes", "sup_create", "sup_destroy", "sup_set_blocks", "sup_set_dose_matrix",
                   "sup_project_simultaneous", "sup_block_iterative", "sup_forward_violation", "sup_backproject_update", "sup_perturb_tv", "sup_perturb_dose", "sup_superiorize",
-                  "sup_superiorize_host", "sup_get_state", "sup_proximity", "sup_objective", "sup_get_derived", "sup_set_row_mode"):
+                  "sup_superiorize_host", "sup_get_state", "sup_proximity", "sup_objective", "sup_get_derived", "sup_set_row_mode", "sup_set_layout"):
             getattr(L, f).restype = c_int
         _lib = L
     return _lib
@@ -209,6 +210,14 @@ def sup_set_dose_matrix(H: SupHandle, rowptr, col, val):
     H._exit()
 
 
+def sup_set_layout(H: SupHandle, x_shape=None, y_shape=None):
+    """x_shape = (rows, cols) of the image x is, y_shape = (angles, bins) of the sinogram the rows of A are; None = no hint."""
+    arr = lambda s: None if s is None else (c_int64 * 2)(int(s[0]), int(s[1]))
+    H._enter()
+    H._check(lib().sup_set_layout(H.h, arr(x_shape), arr(y_shape)))
+    H._exit()
+
+
 def sup_set_row_mode(H: SupHandle, lanes_forward=-1, lanes_backward=-1):
     H._enter()
     H._check(lib().sup_set_row_mode(H.h, int(lanes_forward), int(lanes_backward)))
@@ -268,6 +277,8 @@ def _options(H, objective, shape, lam, block, policy, ell0, k0, trace, decisions
     o.objective = _OBJ[objective] if not isinstance(objective, int) else objective
     if shape is not None and o.objective == OBJ_TV2D:
         o.shape[0], o.shape[1] = int(shape[0]), int(shape[1])
+    if shape is not None and o.objective == OBJ_TV3D:
+        o.shape[0], o.shape[1], o.shape[2] = int(shape[0]), int(shape[1]), int(shape[2])
     o.lambda_ = lam
     o.block_iterative = int(bool(block))
     o.step_policy = policy
@@ -338,9 +349,15 @@ def sup_get_derived(H: SupHandle, which: int) -> torch.Tensor:
     return out
 
 
-def create_from_problem(P, dtype=F32, device="cuda:0", blocks=True) -> SupHandle:
-    """Convenience for tests/bench: a gen.Problem -> handle (with blocks / dose matrix when the problem has them)."""
+def create_from_problem(P, dtype=F32, device="cuda:0", blocks=True, layout=True) -> SupHandle:
+    """Convenience for tests/bench: a gen.Problem -> handle (with blocks / dose matrix when the problem has them).
+    layout: pass the problem's geometry (image shape; angles x bins of a CT sinogram) to sup_set_layout."""
     H = sup_create(P.rowptr, P.col, P.val, P.lb, P.ub, P.lo, P.hi, P.weights, dtype=dtype, n=P.n, device=device)
+    if layout:
+        xs = tuple(P.shape) if P.shape is not None and len(P.shape) == 2 and P.shape[0] * P.shape[1] == P.n else None
+        ys = (P.meta["n_angles"], P.meta["n_bins"]) if "n_angles" in P.meta and P.meta["n_angles"] * P.meta["n_bins"] == P.m else None
+        if xs is not None or ys is not None:
+            sup_set_layout(H, xs, ys)
     if blocks and P.block_rowptr is not None:
         sup_set_blocks(H, P.block_rowptr)
     if P.dose is not None:

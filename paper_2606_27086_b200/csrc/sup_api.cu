@@ -167,12 +167,14 @@ extern "C" sup_status sup_create(sup_handle* out, const sup_csr* A, const void* 
     h->AT.alloc_nnz = h->nnz;
     h->A.pk = h->pk_a;
     h->AT.pk = h->pk_at;
+    h->xmap.kind = 1;  // bank swizzle only, until sup_set_layout says what the index spaces look like
     rc = sup_stream_plan(h, h->A, 0, h->m, true, tab_a, scratch, &h->A.plan);
-    if (rc == SUP_OK && h->use_stream) rc = sup_stream_setup_gather(h);
-    if (rc == SUP_OK && h->use_stream) rc = sup_stream_pack(h, at_val, at_col, h->nnz, h->pk_at);
     if (rc == SUP_OK && cudaMemsetAsync(h->xg, 0, size_t((h->n + 511) & ~int64_t(511)) * h->esz, h->stream) != cudaSuccess)
         rc = sup_fail(h, SUP_ERR_CUDA, "sup_create: %s", cudaGetErrorString(cudaGetLastError()));
     if (rc == SUP_OK) rc = sup_stream_plan(h, h->AT, 0, h->n, false, tab_at, scratch, &h->AT.plan);
+    if (rc == SUP_OK) rc = sup_stream_refresh_layout(h);
+    if (rc == SUP_OK && cudaStreamSynchronize(h->stream) != cudaSuccess)
+        rc = sup_fail(h, SUP_ERR_CUDA, "sup_create: %s", cudaGetErrorString(cudaGetLastError()));
     if (rc != SUP_OK) {
         memcpy(g_create_error, h->err, sizeof(g_create_error));
         delete h;
@@ -251,7 +253,7 @@ extern "C" sup_status sup_set_blocks(sup_handle h, int n_blocks, const int64_t* 
         if (rc != SUP_OK) return rc;
     }
     h->n_blocks = n_blocks;
-    sup_status rc = h->use_stream ? sup_stream_pack(h, val, col, h->nnz, h->pk_atb) : SUP_OK;
+    sup_status rc = sup_stream_refresh_layout(h);
     if (rc == SUP_OK) rc = sup_setup_block_scaling(h, scratch, scratch_bytes);
     if (rc != SUP_OK) { h->n_blocks = 0; return rc; }
     SUP_CUDA(h, cudaStreamSynchronize(h->stream));
@@ -322,6 +324,38 @@ extern "C" sup_status sup_set_row_mode(sup_handle h, int lanes_forward, int lane
                              &h->stream_fwd_blk[t]);
         if (rc == SUP_OK) rc = sup_stream_plan(h, h->ATb[t], 0, h->n, false, h->ATb[t].plan.table, scratch, &h->ATb[t].plan);
     }
+    if (rc == SUP_OK) rc = sup_stream_refresh_layout(h);
+    if (rc == SUP_OK) SUP_CUDA(h, cudaStreamSynchronize(h->stream));
+    return rc;
+}
+
+static bool make_tile_map(const int64_t* shape, int64_t size, size_t esz, GMap* out) {
+    *out = GMap();
+    if (!shape || (shape[0] == 0 && shape[1] == 0)) return true;  // no hint
+    if (shape[0] < 1 || shape[1] < 1 || shape[0] * shape[1] != size) return false;
+    out->kind = 2;
+    out->tw = int(32 / esz);            // one 32-byte sector
+    out->th = int(128 / esz) / out->tw;  // 4 sectors = one 128-byte line
+    out->C = int(shape[1]);
+    out->Rm = int(shape[0] / out->th) * out->th;
+    out->Cm = int(shape[1] / out->tw) * out->tw;
+    out->ntc = out->Cm / out->tw;
+    return true;
+}
+
+extern "C" sup_status sup_set_layout(sup_handle h, const int64_t* x_shape, const int64_t* y_shape) {
+    if (!h) return SUP_ERR_INVALID_ARG;
+    SUP_ENTER(h);
+    GMap mx, my;
+    if (!make_tile_map(x_shape, h->n, h->esz, &mx)) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_set_layout: x_shape[0] * x_shape[1] must equal n");
+    if (!make_tile_map(y_shape, h->m, h->esz, &my)) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_set_layout: y_shape[0] * y_shape[1] must equal m");
+    SUP_CUDA(h, cudaStreamSynchronize(h->stream));
+    drop_graph(h);
+    if (mx.kind == 0) mx.kind = 1;  // without a shape: bank swizzle only
+    h->xmap = mx;
+    h->ymap_req = my;
+    sup_status rc = sup_stream_refresh_layout(h);
+    if (rc == SUP_OK) SUP_CUDA(h, cudaStreamSynchronize(h->stream));
     return rc;
 }
 
@@ -394,19 +428,28 @@ static sup_status check_step(sup_ctx* h, int N, double beta0, double a) {
     return SUP_OK;
 }
 
-static sup_status check_objective(sup_ctx* h, int kind, const int64_t* shape, int64_t* ny, int64_t* nx) {
-    *ny = *nx = 0;
+// dims = {nz, ny, nx} of the objective's view of x (0 where unused)
+static sup_status check_objective(sup_ctx* h, int kind, const int64_t* shape, int64_t* dims) {
+    dims[0] = dims[1] = dims[2] = 0;
     switch (kind) {
         case SUP_OBJ_NONE:
         case SUP_OBJ_TV1D: return SUP_OK;
         case SUP_OBJ_TV2D:
             if (!shape || shape[0] < 1 || shape[1] < 1 || shape[0] * shape[1] != h->n)
                 return sup_fail(h, SUP_ERR_INVALID_ARG, "TV2D needs shape = {ny, nx} with ny*nx == n");
-            *ny = shape[0];
-            *nx = shape[1];
+            dims[1] = shape[0];
+            dims[2] = shape[1];
+            return SUP_OK;
+        case SUP_OBJ_TV3D:
+            if (!shape || shape[0] < 1 || shape[1] < 1 || shape[2] < 1 || shape[0] * shape[1] * shape[2] != h->n)
+                return sup_fail(h, SUP_ERR_INVALID_ARG, "TV3D needs shape = {nz, ny, nx} with nz*ny*nx == n");
+            dims[0] = shape[0];
+            dims[1] = shape[1];
+            dims[2] = shape[2];
             return SUP_OK;
         case SUP_OBJ_DOSE:
-            if (!h->has_dose) return sup_fail(h, SUP_ERR_STATE, "dose objective: call sup_set_dose_matrix first");
+        case SUP_OBJ_MEAN:
+            if (!h->has_dose) return sup_fail(h, SUP_ERR_STATE, "dose / mean objective: call sup_set_dose_matrix first");
             return SUP_OK;
     }
     return sup_fail(h, SUP_ERR_INVALID_ARG, "unknown objective kind %d", kind);
@@ -440,12 +483,12 @@ extern "C" sup_status sup_get_state(sup_handle h, sup_state* out) {
 static sup_status perturb_alone(sup_ctx* h, void* x, int kind, const int64_t* shape, int N, double beta0, double a, int64_t* ell) {
     if (!x || !ell) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_perturb: NULL x or ell");
     if (check_step(h, N, beta0, a) != SUP_OK) return SUP_ERR_INVALID_ARG;
-    int64_t ny, nx;
-    sup_status rc = check_objective(h, kind, shape, &ny, &nx);
+    int64_t dims[3];
+    sup_status rc = check_objective(h, kind, shape, dims);
     if (rc != SUP_OK) return rc;
     sup_launch_begin_run(h, *ell, 0, a);
     if (N > 0) {
-        PerturbParams pp = {kind, ny, nx, N, beta0, a, SUP_STEP_PER_TRIAL, nullptr, nullptr, 0, 0};
+        PerturbParams pp = {kind, dims[0], dims[1], dims[2], N, beta0, a, SUP_STEP_PER_TRIAL, nullptr, nullptr, 0, 0, false};
         rc = sup_launch_perturb(h, x, pp);
         if (rc != SUP_OK) return rc;
     }
@@ -460,9 +503,9 @@ extern "C" sup_status sup_perturb_tv(sup_handle h, void* x, int dims, const int6
                                      int64_t* ell) {
     if (!h) return SUP_ERR_INVALID_ARG;
     SUP_ENTER(h);
-    if (dims != 1 && dims != 2) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_perturb_tv: dims must be 1 or 2");
+    if (dims < 1 || dims > 3) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_perturb_tv: dims must be 1, 2 or 3");
     if (dims == 1 && shape && shape[0] != h->n) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_perturb_tv: shape[0] != n");
-    return perturb_alone(h, x, dims == 2 ? SUP_OBJ_TV2D : SUP_OBJ_TV1D, shape, N, beta0, a, ell);
+    return perturb_alone(h, x, dims == 3 ? SUP_OBJ_TV3D : (dims == 2 ? SUP_OBJ_TV2D : SUP_OBJ_TV1D), shape, N, beta0, a, ell);
 }
 
 extern "C" sup_status sup_perturb_dose(sup_handle h, void* x, int N, double beta0, double a, int64_t* ell) {
@@ -477,16 +520,16 @@ struct RunPlan {
     int N;
     double beta0, a;
     sup_options o;
-    int64_t ny, nx;
+    int64_t dims[3];  // {nz, ny, nx} of the objective
 };
 
 static sup_status enqueue_superiorized_sweep(sup_ctx* h, const RunPlan& P) {
     if (P.N > 0 && P.o.objective != SUP_OBJ_NONE) {
-        PerturbParams pp = {P.o.objective, P.ny, P.nx, P.N, P.beta0, P.a, P.o.step_policy, P.o.decisions, P.o.decision_f,
-                            P.o.decisions_cap, P.o.n_restart};
+        PerturbParams pp = {P.o.objective, P.dims[0], P.dims[1], P.dims[2], P.N, P.beta0, P.a, P.o.step_policy, P.o.decisions,
+                            P.o.decision_f, P.o.decisions_cap, P.o.n_restart, true};
         sup_status rc = sup_launch_perturb(h, P.x, pp);
         if (rc != SUP_OK) return rc;
-        h->xg_synced = false;  // the perturbation moved x
+        h->xg_synced = sup_stream_forward_uses_xg(h);  // the perturbation kernel wrote the moved x to the gather mirror too
     }
     if (P.o.block_iterative) enqueue_block_sweep(h, P.x, P.o.lambda);
     else enqueue_simultaneous(h, P.x, P.o.lambda);
@@ -494,7 +537,7 @@ static sup_status enqueue_superiorized_sweep(sup_ctx* h, const RunPlan& P) {
         double* slot = reinterpret_cast<double*>(reinterpret_cast<char*>(h->state) + offsetof(DevState, scalar_out));
         sup_launch_proximity(h, P.x, 0, 2.0, slot);
         sup_launch_trace_slot(h, P.o.trace, 0);
-        sup_launch_objective(h, P.x, P.o.objective, P.ny, P.nx, slot);
+        sup_launch_objective(h, P.x, P.o.objective, P.dims[0], P.dims[1], P.dims[2], slot);
         sup_launch_trace_slot(h, P.o.trace, 1);
     }
     sup_launch_end_sweep(h, P.o.trace);
@@ -515,7 +558,7 @@ static sup_status run_superiorize(sup_ctx* h, void* x, int n_iter, int N, double
     P.beta0 = beta0;
     P.a = a;
     P.o = *opt;
-    sup_status rc = check_objective(h, opt->objective, opt->shape, &P.ny, &P.nx);
+    sup_status rc = check_objective(h, opt->objective, opt->shape, P.dims);
     if (rc != SUP_OK) return rc;
     sup_launch_begin_run(h, opt->ell0, opt->k0, a);
     h->xg_synced = false;
@@ -532,8 +575,9 @@ static sup_status run_superiorize(sup_ctx* h, void* x, int n_iter, int N, double
         key.beta0 = beta0;
         key.a = a;
         key.lambda = opt->lambda;
-        key.s0 = P.ny;
-        key.s1 = P.nx;
+        key.s0 = P.dims[1];
+        key.s1 = P.dims[2];
+        key.s2 = P.dims[0];
         key.trace = opt->trace;
         key.dec = opt->decisions;
         key.decf = opt->decision_f;
@@ -624,11 +668,11 @@ extern "C" sup_status sup_objective(sup_handle h, const void* x, int kind, const
     if (!h) return SUP_ERR_INVALID_ARG;
     SUP_ENTER(h);
     if (!x || !out) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_objective: NULL x or out");
-    int64_t ny, nx;
-    sup_status rc = check_objective(h, kind, shape, &ny, &nx);
+    int64_t dims[3];
+    sup_status rc = check_objective(h, kind, shape, dims);
     if (rc != SUP_OK) return rc;
     double* slot = reinterpret_cast<double*>(reinterpret_cast<char*>(h->state) + offsetof(DevState, scalar_out));
-    sup_launch_objective(h, x, kind, ny, nx, slot);
+    sup_launch_objective(h, x, kind, dims[0], dims[1], dims[2], slot);
     return fetch_scalar(h, out);
 }
 
@@ -646,7 +690,8 @@ extern "C" sup_status sup_get_derived(sup_handle h, int which, void* dst, size_t
         default: return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_get_derived: unknown array");
     }
     if (!dst || dst_bytes < bytes) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_get_derived: dst too small (%zu needed)", bytes);
-    SUP_CUDA(h, cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, h->stream));
+    if (which == 5 && h->ymap.kind != 0) sup_launch_unmap(h, h->y, dst, h->m, h->ymap);  // y is kept in its gather layout
+    else SUP_CUDA(h, cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, h->stream));
     SUP_CUDA(h, cudaStreamSynchronize(h->stream));
     return SUP_OK;
 }

@@ -50,8 +50,11 @@ struct DevState {
     double f;             // objective carried by the last perturbation phase
     double apow;          // a^l as the running fp64 product (PER_TRIAL; A-20)
     double scalar_out;    // result slot of finalize kernels (proximity / objective)
-    unsigned bar_count;   // grid barrier of the perturbation kernel
-    unsigned bar_gen;
+    // grid barrier of the perturbation kernel: the arrival counter, the generation flag every waiting CTA polls and the
+    // published totals each sit in a 128-byte line of their own, so the pollers do not slow the arrivals down
+    alignas(128) unsigned bar_count;
+    alignas(128) unsigned bar_gen;
+    alignas(128) double red[2][8];  // totals published by the last CTA to arrive (by generation parity)
 };
 
 struct Bump {  // bump allocator over caller-provided workspace
@@ -66,6 +69,49 @@ struct Bump {  // bump allocator over caller-provided workspace
         return p;
     }
 };
+
+// Index swizzle of the forward gathers.  With a power-of-two image pitch (512 floats = 2 KB) the x entries a
+// near-vertical ray gathers all have the same address modulo 128 B, i.e. sit in the same L1 data bank: measured, the
+// chunks of the forward product at those angles run 1.6x slower than the median at pitch 512, 1.2x at 528, 1.08x at 520
+// (profiles/r01c_staged.md).  XOR-ing the five bank bits of the index with a fold of the upper bits is a bijection
+// inside every 128-byte line (sector membership is preserved too), and puts vertically adjacent pixels in different banks.
+__host__ __device__ static inline int sup_swz(int j) { return j ^ (((j >> 9) ^ (j >> 14)) & 31); }
+
+// Gather map: where element j of a gathered vector (the forward product's x, the back-projection's y) lives in the
+// copy the kernels gather from.  A bijection of [0, size) chosen so that the gathers of one warp touch few 128-byte
+// lines and distinct L1 data banks (profiles/r02c_layout.md):
+//   kind 0  identity
+//   kind 1  bank swizzle only (sup_swz): elements permuted inside each line
+//   kind 2  the vector is a row-major R x C array (an image, a sinogram: sup_set_layout) stored as line-sized tiles of
+//           th x tw elements (th * tw * element size = 128 B, tw elements = one 32-byte sector), so that a ray crossing
+//           the image at any angle -- or a pixel's trace through the sinogram -- stays inside a tile for several
+//           elements; inside a tile the position is XOR-ed with (tile row mod tw) | (tile column mod th) * tw, a
+//           bijection that keeps sectors whole and puts vertically / horizontally adjacent tiles in different banks.
+//           The R mod th last rows and C mod tw last columns do not fill whole tiles and follow the tiled region in
+//           row-major order (no padding: the map stays onto [0, R*C)).
+struct GMap {
+    int kind = 0;
+    int C = 1;          // columns of the 2-D view
+    int Rm = 0, Cm = 0; // extent of the tiled region (multiples of th, tw)
+    int ntc = 0;        // tiles per tile row = Cm / tw
+    int th = 4, tw = 8;
+};
+__host__ __device__ static inline int sup_gmap(const GMap& M, int j) {
+    if (M.kind == 0) return j;
+    if (M.kind == 1) return sup_swz(j);
+    const int r = j / M.C, c = j - r * M.C;
+    const int main_count = M.Rm * M.Cm;
+    if (r < M.Rm) {
+        if (c < M.Cm) {
+            const int tr = r / M.th, tc = c / M.tw;
+            const int in = (r - tr * M.th) * M.tw + (c - tc * M.tw);
+            const int v = (tr & (M.tw - 1)) | ((tc & (M.th - 1)) * M.tw);
+            return (tr * M.ntc + tc) * (M.th * M.tw) + (in ^ v);
+        }
+        return main_count + r * (M.C - M.Cm) + (c - M.Cm);
+    }
+    return main_count + M.Rm * (M.C - M.Cm) + (r - M.Rm) * M.C + c;
+}
 
 struct sup_ctx {
     int dt = 0;
@@ -91,7 +137,10 @@ struct sup_ctx {
     void* pk_a = nullptr;       // [nnz] x 8 B, fp32 handles: (val, sup_swz(col)) of A
     void* pk_at = nullptr;      // [nnz] x 8 B, fp32 handles: (val, row) of A^T
     void* pk_atb = nullptr;     // [nnz] x 8 B, fp32 handles: the per-block transposes (sup_set_blocks)
-    void* xg = nullptr;         // [n rounded up to 512] dtype
+    void* xg = nullptr;         // [n rounded up to 512] dtype: xg[sup_gmap(xmap, j)] = x[j]
+    GMap xmap, ymap;            // maps in force: x mirror read by the staged forward product; internal y (identity unless every
+                                // product runs on the staged fp32 kernels, which read y through the packed A^T)
+    GMap ymap_req;              // what sup_set_layout asked for on the row side
     bool xg_synced = false;     // enqueue-time flag: xg mirrors x (set by the back-projection, cleared when x changes elsewhere)
     int stream_nb = 0;          // persistent grid of the row-stream kernels (-1: unavailable)
     bool use_stream = true;     // false: the group-per-row kernels of sup_spmv.cu (sup_set_row_mode(h, -2, -2))
@@ -121,13 +170,13 @@ struct sup_ctx {
         int N = 0, objective = 0, block = 0, policy = 0, trace_mode = 0;
         int64_t n_restart = 0;
         double beta0 = 0, a = 0, lambda = 0;
-        int64_t s0 = 0, s1 = 0;
+        int64_t s0 = 0, s1 = 0, s2 = 0;
         const void *trace = nullptr, *dec = nullptr, *decf = nullptr;
         int64_t cap = 0;
         bool operator==(const GraphKey& o) const {
             return x == o.x && N == o.N && objective == o.objective && block == o.block && policy == o.policy &&
                    trace_mode == o.trace_mode && beta0 == o.beta0 && a == o.a && lambda == o.lambda && s0 == o.s0 &&
-                   s1 == o.s1 && trace == o.trace && dec == o.dec && decf == o.decf && cap == o.cap && n_restart == o.n_restart;
+                   s1 == o.s1 && s2 == o.s2 && trace == o.trace && dec == o.dec && decf == o.decf && cap == o.cap && n_restart == o.n_restart;
         }
     } gkey;
     int64_t launches = 0;
@@ -143,13 +192,6 @@ extern char g_create_error[512];
         if (e__ != cudaSuccess)                                                                      \
             return sup_fail((h), SUP_ERR_CUDA, "%s:%d %s: %s", __FILE__, __LINE__, #call, cudaGetErrorString(e__)); \
     } while (0)
-
-// Index swizzle of the forward gathers.  With a power-of-two image pitch (512 floats = 2 KB) the x entries a
-// near-vertical ray gathers all have the same address modulo 128 B, i.e. sit in the same L1 data bank: measured, the
-// chunks of the forward product at those angles run 1.6x slower than the median at pitch 512, 1.2x at 528, 1.08x at 520
-// (profiles/r01c_staged.md).  XOR-ing the five bank bits of the index with a fold of the upper bits is a bijection
-// inside every 128-byte line (sector membership is preserved too), and puts vertically adjacent pixels in different banks.
-__host__ __device__ static inline int sup_swz(int j) { return j ^ (((j >> 9) ^ (j >> 14)) & 31); }
 
 static inline int sup_pick_group(int64_t nnz, int64_t rows) {
     // lanes cooperating on one row: about a quarter of the mean row length, a power of two in [4, 32]
@@ -189,15 +231,18 @@ sup_status sup_stream_plan(sup_ctx* h, const CsrD& M, int64_t r0, int64_t r1, bo
                            StreamPlan* out);
 void sup_launch_stream_fwd(sup_ctx* h, const StreamPlan& rp, const void* x, const void* dscale);
 void sup_launch_stream_bwd(sup_ctx* h, const CsrD& AT, const StreamPlan& rp, void* x, double lambda);
-sup_status sup_stream_setup_gather(sup_ctx* h);  // fills colg (fp64) or the packed copy of A (fp32) from A.col / A.val
-// fp32 handles: dst[k] = (val[k], col[k]) for k in [0, nnz)
-sup_status sup_stream_pack(sup_ctx* h, const void* val, const int32_t* col, int64_t nnz, void* dst);
+sup_status sup_stream_setup_gather(sup_ctx* h);  // fills colg (fp64) or the packed copy of A (fp32) from A.col / A.val through xmap
+// fp32 handles: dst[k] = (val[k], sup_gmap(map, col[k])) for k in [0, nnz)
+sup_status sup_stream_pack(sup_ctx* h, const void* val, const int32_t* col, int64_t nnz, void* dst, const GMap& map);
+// (re)decides ymap and (re)writes every packed / mapped copy the staged kernels read; call after plans or maps change
+sup_status sup_stream_refresh_layout(sup_ctx* h);
+void sup_launch_unmap(sup_ctx* h, const void* src, void* dst, int64_t count, const GMap& map);  // dst[i] = src[map(i)]
 bool sup_stream_forward_uses_xg(const sup_ctx* h);
 
 // ---- perturbation (sup_perturb.cu) ------------------------------------------------------------------------
 struct PerturbParams {
     int objective;
-    int64_t ny, nx;
+    int64_t nz, ny, nx;
     int N;
     double beta0, a;
     int policy;
@@ -205,9 +250,10 @@ struct PerturbParams {
     double* decision_f;
     int64_t cap;
     int64_t n_restart;
+    bool write_mirror;  // also write the final iterate to the gather mirror of x (xg_synced stays true)
 };
 sup_status sup_launch_perturb(sup_ctx* h, void* x, const PerturbParams& pp);
-void sup_launch_objective(sup_ctx* h, const void* x, int kind, int64_t ny, int64_t nx, double* out_dev);
+void sup_launch_objective(sup_ctx* h, const void* x, int kind, int64_t nz, int64_t ny, int64_t nx, double* out_dev);
 void sup_launch_end_sweep(sup_ctx* h, double* trace);
 void sup_launch_trace_slot(sup_ctx* h, double* trace, int slot);  // trace[it][slot] = state->scalar_out
 void sup_launch_begin_run(sup_ctx* h, int64_t ell0, int64_t k0, double a);

@@ -3,16 +3,24 @@
 //
 //   fx <- f(x)
 //   for n = 0..N-1:  g <- grad f(x^{k,n}) (A-7), s <- ||g||_2, v = -g/s (A-6)
-//        trial loop:  beta <- beta0 * a^l (A-10, A-20: pow in fp64), z <- x + beta v, l <- l+1,
+//        trial loop:  beta <- beta0 * a^l (A-10; a^l is the running fp64 product, A-20), z <- x + beta v, l <- l+1,
 //                     accept iff f(z) <= f(x^{k,n}) (L149, A-11); at most J_max trials (A-12)
 //
 // The number of trials is data dependent, so the loop lives on the device: all CTAs of the grid are co-resident
-// (cooperative launch), meet at a grid barrier after every reduction and take the accept decision redundantly
-// from the same partial sums summed in the same order -- no host round trip, and the launch is capturable in a
-// CUDA graph.  z is never stored: z_p = round_T(x_p - (beta/s) g_p) is recomputed wherever it is needed.
-// Objectives: TV2D (Eq. 15; gradient A-8, shared-memory tile with halo, fused with sum g^2),
-// TV1D (A-16), DOSE ||D x||^2 with g = 2 D^T (D x) (A-15).  Objective terms, norms and beta are fp64 in both modes; a^l is the
-// running fp64 product, bit-identical to the oracle's (A-20).
+// (cooperative launch) and meet after every pass at a grid barrier that is fused with the second stage of the
+// reduction -- the last CTA to arrive sums the per-CTA partials in a fixed order and publishes the totals with the
+// barrier's generation flip, so every CTA takes the accept decision from the same numbers: no host round trip, and
+// the launch is capturable in a CUDA graph.  z is never stored on its own: z_p = round_T(x_p - (beta/s) g_p) is
+// recomputed wherever it is needed.
+//
+// TV objectives (TV2D: Eq. 15, gradient A-8; TV3D: the same with a third difference, A-27; TV1D: A-16): the
+// gradient pass of a tile computes every term t_p of the tile anyway, so f comes for free with it.  One pass therefore
+// evaluates the FIRST candidate step of a reduction step completely -- z, f(z), grad f(z), ||grad f(z)||^2 -- and when
+// that candidate is accepted (the common case once beta is small) the next reduction step can start at once:
+// 1 + N grid-wide passes per phase instead of 1 + 2N.  A rejected first candidate falls back to evaluating the next
+// SUP_TRIAL_BATCH candidates per pass, decided strictly in order: the trial / decision / l sequence is exactly
+// Algorithm 1's.  DOSE ||D x||^2 with g = 2 D^T (D x) (A-15) keeps its own branch (closed-form trial loop).
+// Objective terms, norms and beta are fp64 in both modes.
 #include <math.h>
 #include <stdlib.h>
 
@@ -21,7 +29,7 @@
 #define TILE_H 16
 #define TILE_W 64
 #define BARRIER_SPIN_LIMIT (1u << 24)
-#define SUP_TRIAL_BATCH 4  // candidate steps evaluated per pass (TV objectives)
+#define SUP_TRIAL_BATCH 8  // candidate steps evaluated per pass after a rejected first candidate (TV objectives)
 
 template <typename T>
 struct PArgs {
@@ -29,7 +37,9 @@ struct PArgs {
     T* g;
     T* x2;  // second iterate / gradient buffers (TV objectives: an accepted step is applied inside the next gradient pass)
     T* g2;
-    int64_t n, ny, nx;
+    int64_t n, nz, ny, nx;
+    T* xg;      // gather mirror of x kept by the product kernels (NULL: none): written together with the final iterate
+    GMap xmap;
     int N;
     double beta0, a;
     int policy;
@@ -79,6 +89,79 @@ __device__ __forceinline__ void grid_barrier(DevState* st) {
         __threadfence();
     }
     __syncthreads();
+}
+
+// Grid barrier fused with the second stage of a reduction.  On entry v[0..NV) are this THREAD's shares; every CTA sums
+// its threads' shares, stores the NV sums to partials[b * stride + blockIdx.x] and arrives.  The last CTA to arrive adds
+// the partials of all CTAs in index order (which CTA does it changes nothing: same numbers, same order), publishes the
+// totals in st->red[gen & 1] and flips the generation; the others spin on the generation and read the totals.  On
+// return v[] holds the totals in every thread.  Returns false after a time-out (fault bit 0 is set): the caller leaves
+// the kernel instead of computing on inconsistent partials.
+template <int NV>
+__device__ __forceinline__ void cta_sum_batch(double* v);
+__device__ __forceinline__ unsigned atom_add_acq_rel(unsigned* p, unsigned v) {
+    unsigned old;
+    asm volatile("atom.add.acq_rel.gpu.u32 %0, [%1], %2;" : "=r"(old) : "l"(p), "r"(v) : "memory");
+    return old;
+}
+__device__ __forceinline__ unsigned ld_acquire(const unsigned* p) {
+    unsigned v;
+    asm volatile("ld.acquire.gpu.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release(unsigned* p, unsigned v) {
+    asm volatile("st.release.gpu.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+template <int NV>
+__device__ __forceinline__ bool grid_reduce(DevState* st, double* partials, int stride, double* v, unsigned& gen) {
+    __shared__ int s_role;  // 1: this CTA arrived last, 0: it waited, -1: time-out
+    cta_sum_batch<NV>(v);
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int b = 0; b < NV; ++b) partials[b * stride + blockIdx.x] = v[b];
+        // release: the partials are visible before the count; acquire: the last to arrive sees everybody's partials
+        const unsigned arrived = atom_add_acq_rel(&st->bar_count, 1u);
+        int role = arrived == gridDim.x - 1 ? 1 : 0;
+        if (!role) {
+            unsigned spins = 0;
+            while (ld_acquire(&st->bar_gen) == gen) {
+                __nanosleep(20);
+                if (++spins > BARRIER_SPIN_LIMIT) {
+                    atomicOr(&st->fault, 1);
+                    role = -1;
+                    break;
+                }
+            }
+        }
+        s_role = role;
+    }
+    __syncthreads();
+    const int role = s_role;
+    if (role < 0) return false;
+    double* red = st->red[gen & 1u];
+    if (role == 1) {
+        double w[NV];
+#pragma unroll
+        for (int b = 0; b < NV; ++b) {
+            w[b] = 0.0;
+            for (int q = threadIdx.x; q < int(gridDim.x); q += SUP_THREADS) w[b] += __ldcg(partials + b * stride + q);
+        }
+        cta_sum_batch<NV>(w);
+        if (threadIdx.x == 0) {
+#pragma unroll
+            for (int b = 0; b < NV; ++b) red[b] = w[b];
+            st->bar_count = 0;
+            st_release(&st->bar_gen, gen + 1u);  // totals and the reset counter are visible before the flip
+        }
+#pragma unroll
+        for (int b = 0; b < NV; ++b) v[b] = w[b];
+    } else {
+#pragma unroll
+        for (int b = 0; b < NV; ++b) v[b] = __ldcg(red + b);
+    }
+    gen += 1u;
+    return true;
 }
 
 // sum over the CTA, result valid in every thread; fixed order
@@ -186,6 +269,41 @@ __device__ void tv2d_share_batch(const PArgs<T>& A, const double* coef, double* 
     }
 }
 
+// TV3D value for B candidate steps at once (terms for i < nz-1, j < ny-1, k < nx-1; A-27)
+template <typename T, int B>
+__device__ void tv3d_share_batch(const PArgs<T>& A, const double* coef, double* acc) {
+    const int64_t d = A.nz - 1, h = A.ny - 1, w = A.nx - 1;
+    const int64_t total = d > 0 && h > 0 && w > 0 ? d * h * w : 0;
+    const int64_t sz = A.ny * A.nx;
+#pragma unroll
+    for (int b = 0; b < B; ++b) acc[b] = 0.0;
+    for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q < total; q += int64_t(gridDim.x) * blockDim.x) {
+        const int64_t i = q / (h * w), r2 = q - i * h * w, j = r2 / w, k = r2 - j * w;
+        const int64_t p = (i * A.ny + j) * A.nx + k;
+        const double x0 = double(__ldcg(A.x + p)), xz = double(__ldcg(A.x + p + sz)), xy = double(__ldcg(A.x + p + A.nx)), xx = double(__ldcg(A.x + p + 1));
+        double g0 = 0.0, gz = 0.0, gy = 0.0, gx = 0.0;
+        bool any = false;
+#pragma unroll
+        for (int b = 0; b < B; ++b) any = any || coef[b] != 0.0;
+        if (any) {
+            g0 = double(__ldcg(A.g + p));
+            gz = double(__ldcg(A.g + p + sz));
+            gy = double(__ldcg(A.g + p + A.nx));
+            gx = double(__ldcg(A.g + p + 1));
+        }
+#pragma unroll
+        for (int b = 0; b < B; ++b) {
+            const double c = coef[b];
+            const double z0 = c == 0.0 ? x0 : double(T(fma(-c, g0, x0)));
+            const double zz = c == 0.0 ? xz : double(T(fma(-c, gz, xz)));
+            const double zy = c == 0.0 ? xy : double(T(fma(-c, gy, xy)));
+            const double zx = c == 0.0 ? xx : double(T(fma(-c, gx, xx)));
+            const double dz = zz - z0, dy = zy - z0, dx = zx - z0;
+            acc[b] += tv_norm((dz * dz + dy * dy) + dx * dx);
+        }
+    }
+}
+
 template <typename T, int B>
 __device__ void tv1d_share_batch(const PArgs<T>& A, const double* coef, double* acc) {
 #pragma unroll
@@ -277,19 +395,25 @@ __device__ __forceinline__ double objective_share(const PArgs<T>& A, double coef
     if (OBJ == SUP_OBJ_TV2D) return tv2d_share(A, coef);
     if (OBJ == SUP_OBJ_TV1D) return tv1d_share(A, coef);
     if (OBJ == SUP_OBJ_DOSE) return dose_share(A, coef, false);
+    if (OBJ == SUP_OBJ_TV3D) {
+        double acc[1];
+        tv3d_share_batch<T, 1>(A, &coef, acc);
+        return acc[0];
+    }
     return 0.0;
 }
 
-// ---- gradient: writes g, returns this thread's share of sum g^2 ----------------------------------------------
-// TV2D (A-8): g_ij = -(dx_ij+dy_ij)/t_ij [i<ny-1, j<nx-1] + dx_{i-1,j}/t_{i-1,j} [i>=1, j<nx-1] + dy_{i,j-1}/t_{i,j-1} [j>=1, i<ny-1];
-// a term with t = 0 contributes 0 (A-9).  One CTA stages a TILE_H x TILE_W tile plus a one-pixel halo in shared memory.
-// Reads the iterate as z = x - pend * g (pend = 0: x itself), writes z to xo when a step is pending, the gradient of z to go.
+// ---- gradient passes: z = round_T(x - c g) (c = 0: x itself) is formed on the fly; the pass writes z to xo (when c != 0)
+// and grad f(z) to go, and returns this thread's shares F of f(z) (a tile computes every term t_p anyway) and S of
+// sum (grad f(z))^2.  A term with t = 0 contributes 0 to the gradient (A-9).
+// TV2D (A-8): g_ij = -(dx_ij+dy_ij)/t_ij [i<ny-1, j<nx-1] + dx_{i-1,j}/t_{i-1,j} [i>=1, j<nx-1] + dy_{i,j-1}/t_{i,j-1} [j>=1, i<ny-1].
+// One CTA stages a TILE_H x TILE_W tile plus a one-pixel halo in shared memory.
 template <typename T>
-__device__ double tv2d_grad_share(const PArgs<T>& A, double pend, T* __restrict__ xo, T* __restrict__ go) {
+__device__ void tv2d_gz(const PArgs<T>& A, double pend, T* __restrict__ xo, T* __restrict__ go, double& F, double& S) {
     __shared__ double tile[TILE_H + 2][TILE_W + 2 + 1];
     const int64_t ny = A.ny, nx = A.nx;
     const int64_t tiles_y = (ny + TILE_H - 1) / TILE_H, tiles_x = (nx + TILE_W - 1) / TILE_W;
-    double acc = 0.0;
+    double acc = 0.0, facc = 0.0;
     for (int64_t t = blockIdx.x; t < tiles_y * tiles_x; t += gridDim.x) {
         const int64_t ty = t / tiles_x, tx = t - ty * tiles_x;
         const int64_t i0 = ty * TILE_H - 1, j0 = tx * TILE_W - 1;  // top-left of the halo
@@ -309,7 +433,11 @@ __device__ double tv2d_grad_share(const PArgs<T>& A, double pend, T* __restrict_
             if (i + 1 < ny && j + 1 < nx) {  // own term (i, j)
                 const double dx = tile[li + 1][lj] - c, dy = tile[li][lj + 1] - c;
                 const double d2 = dx * dx + dy * dy;
-                if (d2 > 0.0) gv -= (dx + dy) * rsqrt(d2);
+                if (d2 > 0.0) {
+                    const double ri = rsqrt(d2);
+                    gv -= (dx + dy) * ri;
+                    facc += d2 * ri;
+                }
             }
             if (i >= 1 && j + 1 < nx) {  // term (i-1, j): dx_{i-1,j} = X_ij - X_{i-1,j}
                 const double b = tile[li - 1][lj];
@@ -329,12 +457,78 @@ __device__ double tv2d_grad_share(const PArgs<T>& A, double pend, T* __restrict_
             acc += double(gs) * double(gs);
         }
     }
-    return acc;
+    F = facc;
+    S = acc;
+}
+
+// TV3D (A-27): Eq. 15 with a third difference on an nz x ny x nx volume; a voxel receives +dz/t of term (i-1,j,k), +dy/t of
+// (i,j-1,k), +dx/t of (i,j,k-1) and -(dz+dy+dx)/t of its own term.  Tile of TZ x TY x TX voxels plus a one-voxel halo.
+#define TZ3 4
+#define TY3 8
+#define TX3 32
+template <typename T>
+__device__ void tv3d_gz(const PArgs<T>& A, double pend, T* __restrict__ xo, T* __restrict__ go, double& F, double& S) {
+    __shared__ double vol[TZ3 + 2][TY3 + 2][TX3 + 2 + 1];
+    const int64_t nz = A.nz, ny = A.ny, nx = A.nx;
+    const int64_t tz = (nz + TZ3 - 1) / TZ3, ty = (ny + TY3 - 1) / TY3, tx = (nx + TX3 - 1) / TX3;
+    double acc = 0.0, facc = 0.0;
+    for (int64_t t = blockIdx.x; t < tz * ty * tx; t += gridDim.x) {
+        const int64_t bz = t / (ty * tx), rem = t - bz * ty * tx, by = rem / tx, bx = rem - by * tx;
+        const int64_t i0 = bz * TZ3 - 1, j0 = by * TY3 - 1, k0 = bx * TX3 - 1;
+        __syncthreads();
+        for (int q = threadIdx.x; q < (TZ3 + 2) * (TY3 + 2) * (TX3 + 2); q += SUP_THREADS) {
+            const int li = q / ((TY3 + 2) * (TX3 + 2)), r2 = q - li * (TY3 + 2) * (TX3 + 2), lj = r2 / (TX3 + 2), lk = r2 - lj * (TX3 + 2);
+            const int64_t i = i0 + li, j = j0 + lj, k = k0 + lk;
+            vol[li][lj][lk] = (i >= 0 && i < nz && j >= 0 && j < ny && k >= 0 && k < nx) ? zval(A.x, A.g, pend, (i * ny + j) * nx + k) : 0.0;
+        }
+        __syncthreads();
+        for (int q = threadIdx.x; q < TZ3 * TY3 * TX3; q += SUP_THREADS) {
+            const int li = q / (TY3 * TX3) + 1, r2 = q % (TY3 * TX3), lj = r2 / TX3 + 1, lk = r2 % TX3 + 1;
+            const int64_t i = i0 + li, j = j0 + lj, k = k0 + lk;
+            if (i >= nz || j >= ny || k >= nx) continue;
+            const double c = vol[li][lj][lk];
+            double gv = 0.0;
+            if (i >= 1 && j + 1 < ny && k + 1 < nx) {  // term (i-1, j, k)
+                const double b = vol[li - 1][lj][lk];
+                const double dz = c - b, dy = vol[li - 1][lj + 1][lk] - b, dx = vol[li - 1][lj][lk + 1] - b;
+                const double d2 = (dz * dz + dy * dy) + dx * dx;
+                if (d2 > 0.0) gv += dz * rsqrt(d2);
+            }
+            if (j >= 1 && i + 1 < nz && k + 1 < nx) {  // term (i, j-1, k)
+                const double b = vol[li][lj - 1][lk];
+                const double dz = vol[li + 1][lj - 1][lk] - b, dy = c - b, dx = vol[li][lj - 1][lk + 1] - b;
+                const double d2 = (dz * dz + dy * dy) + dx * dx;
+                if (d2 > 0.0) gv += dy * rsqrt(d2);
+            }
+            if (k >= 1 && i + 1 < nz && j + 1 < ny) {  // term (i, j, k-1)
+                const double b = vol[li][lj][lk - 1];
+                const double dz = vol[li + 1][lj][lk - 1] - b, dy = vol[li][lj + 1][lk - 1] - b, dx = c - b;
+                const double d2 = (dz * dz + dy * dy) + dx * dx;
+                if (d2 > 0.0) gv += dx * rsqrt(d2);
+            }
+            if (i + 1 < nz && j + 1 < ny && k + 1 < nx) {  // own term
+                const double dz = vol[li + 1][lj][lk] - c, dy = vol[li][lj + 1][lk] - c, dx = vol[li][lj][lk + 1] - c;
+                const double d2 = (dz * dz + dy * dy) + dx * dx;
+                if (d2 > 0.0) {
+                    const double ri = rsqrt(d2);
+                    gv -= ((dz + dy) + dx) * ri;
+                    facc += d2 * ri;
+                }
+            }
+            const T gs = T(gv);
+            const int64_t p = (i * ny + j) * nx + k;
+            go[p] = gs;
+            if (pend != 0.0) xo[p] = T(c);
+            acc += double(gs) * double(gs);
+        }
+    }
+    F = facc;
+    S = acc;
 }
 
 template <typename T>
-__device__ double tv1d_grad_share(const PArgs<T>& A, double pend, T* __restrict__ xo, T* __restrict__ go) {
-    double acc = 0.0;
+__device__ void tv1d_gz(const PArgs<T>& A, double pend, T* __restrict__ xo, T* __restrict__ go, double& F, double& S) {
+    double acc = 0.0, facc = 0.0;
     for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q < A.n; q += int64_t(gridDim.x) * blockDim.x) {
         const double c = zval(A.x, A.g, pend, q);
         double gv = 0.0;
@@ -345,12 +539,14 @@ __device__ double tv1d_grad_share(const PArgs<T>& A, double pend, T* __restrict_
         if (q + 1 < A.n) {
             const double dr = zval(A.x, A.g, pend, q + 1) - c;
             gv -= double((dr > 0.0) - (dr < 0.0));
+            facc += fabs(dr);
         }
         go[q] = T(gv);
         if (pend != 0.0) xo[q] = T(c);
         acc += gv * gv;
     }
-    return acc;
+    F = facc;
+    S = acc;
 }
 
 template <typename T>
@@ -375,15 +571,26 @@ __device__ double dose_grad_share(const PArgs<T>& A) {
     return acc;
 }
 
-// ---- the perturbation phase ----------------------------------------------------------------------------------
+// ---- the perturbation phase, TV objectives ---------------------------------------------------------------------
+// Buffers: (xc, gc) hold the current inner iterate x^{k,n} and its gradient, (xo, go) receive the candidate z and its gradient
+// (a tile's halo needs the neighbours' x and g, so a pass cannot work in place); on acceptance the pairs swap.
 template <typename T, int OBJ>
-__global__ void __launch_bounds__(SUP_THREADS) k_perturb(PArgs<T> Ain) {
-    // TV objectives: an accepted step is not written out at once.  It stays pending (x^{k,n+1} = x - pend g) and is applied
-    // inside the next gradient pass, which reads z on the fly and writes z and its gradient to the SECOND pair of
-    // buffers (the halo of a tile needs the neighbours' old x and g, so it cannot be done in place).  That removes one
-    // pass and one grid barrier per reduction step; the arithmetic, z = round_T(x - coef g), is unchanged.
+__device__ __forceinline__ void tv_gz(const PArgs<T>& V, double c, T* xo, T* go, double& F, double& S) {
+    if (OBJ == SUP_OBJ_TV2D) tv2d_gz(V, c, xo, go, F, S);
+    else if (OBJ == SUP_OBJ_TV3D) tv3d_gz(V, c, xo, go, F, S);
+    else tv1d_gz(V, c, xo, go, F, S);
+}
+template <typename T, int OBJ, int B>
+__device__ __forceinline__ void tv_share_batch(const PArgs<T>& V, const double* coef, double* acc) {
+    if (OBJ == SUP_OBJ_TV2D) tv2d_share_batch<T, B>(V, coef, acc);
+    else if (OBJ == SUP_OBJ_TV3D) tv3d_share_batch<T, B>(V, coef, acc);
+    else tv1d_share_batch<T, B>(V, coef, acc);
+}
+
+template <typename T, int OBJ>
+__global__ void __launch_bounds__(SUP_THREADS) k_perturb_tv(PArgs<T> Ain) {
     const PArgs<T>& A = Ain;
-    T* xc = Ain.x;   // current iterate / gradient buffers and the other pair
+    T* xc = Ain.x;
     T* gc = Ain.g;
     T* xo = Ain.x2;
     T* go = Ain.g2;
@@ -393,15 +600,176 @@ __global__ void __launch_bounds__(SUP_THREADS) k_perturb(PArgs<T> Ain) {
         V.g = gc;
         return V;
     };
-    double pend = 0.0;
-    constexpr bool DEFER = OBJ == SUP_OBJ_TV2D || OBJ == SUP_OBJ_TV1D;
+    DevState* st = A.st;
+    long long ell = *(volatile long long*)&st->ell;
+    double apow = *(volatile double*)&st->apow;  // a^ell, running product (A-20)
+    const long long k = *(volatile long long*)&st->k;
+    long long ndec = *(volatile long long*)&st->n_dec;
+    unsigned gen = *(volatile unsigned*)&st->bar_gen;  // read before this CTA's first arrival, so before any flip of this launch
+    long long trials = 0;
+    // restarted perturbations (PAPER.md:L101, L315; A-24): at the start of sweep k = r * n_restart the exponent is reset to r
+    if (A.n_restart > 0 && k > 0 && k % A.n_restart == 0) {
+        ell = k / A.n_restart;
+        apow = 1.0;
+        for (long long q = 0; q < ell; ++q) apow *= A.a;
+    }
+    int warn = 0, fault = 0;
+    double pend = 0.0;  // step accepted in the last reduction step and not yet written anywhere: x^{k,N} = xc - pend gc
+    double* P = A.partials;
+    constexpr int B = SUP_TRIAL_BATCH;
+    constexpr int PSTRIDE = 2 * SUP_MAX_PARTIALS / B;  // partial slots per reduced value
+    bool ok = true;
+
+    auto log_trial = [&](double fz, double fxv, bool acc) {
+        if (blockIdx.x == 0 && threadIdx.x == 0) {
+            if (A.decisions && ndec < A.cap) A.decisions[ndec] = acc ? 1 : 0;
+            if (A.decision_f && ndec < A.cap) {
+                A.decision_f[2 * ndec] = fz;
+                A.decision_f[2 * ndec + 1] = fxv;
+            }
+        }
+        ++ndec;
+    };
+    auto step_coef = [&](double s, long long jloc, double* coef, int cnt) {
+        // a^(exponent of candidate 0) by successive multiplication from 1, like the oracle (A-20): PER_TRIAL carries the
+        // running product a^l across trials and sweeps; PER_SWEEP rebuilds a^(k+j) (k is small)
+        double ap = apow;
+        if (A.policy != SUP_STEP_PER_TRIAL) {
+            ap = 1.0;
+            for (long long q = 0; q < k + jloc; ++q) ap *= A.a;
+        }
+        for (int b = 0; b < cnt; ++b) {
+            coef[b] = s > 0.0 ? (A.beta0 * ap) / s : 0.0;
+            ap *= A.a;
+        }
+    };
+
+    // pass 0: gradient of x^{k,0}; f(x^{k,0}) and ||g||^2 come with it
+    double fx, s;
+    {
+        double v[2];
+        tv_gz<T, OBJ>(view(), 0.0, xo, gc, v[0], v[1]);
+        ok = grid_reduce<2>(st, P, PSTRIDE, v, gen);
+        fx = v[0];
+        s = sqrt(v[1]);
+        if (!isfinite(fx)) fault |= 2;
+    }
+    for (int nred = 0; ok && nred < A.N; ++nred) {
+        const bool last = nred == A.N - 1;
+        bool accepted = false;
+        long long jloc = 0;
+        int trial = 0;
+        if (!last) {
+            // First candidate, evaluated completely: z, f(z), grad f(z), ||grad f(z)||^2 in one pass.  Accepted (the common
+            // case once beta is small), the next reduction step starts from (xo, go) without another pass.
+            double c0;
+            step_coef(s, jloc, &c0, 1);
+            double v[2];
+            tv_gz<T, OBJ>(view(), c0, xo, go, v[0], v[1]);
+            ok = grid_reduce<2>(st, P, PSTRIDE, v, gen);
+            if (!ok) break;
+            const bool acc = v[0] <= fx;  // NaN compares false -> rejected (A-11)
+            ++ell;
+            apow *= A.a;
+            ++jloc;
+            ++trials;
+            ++trial;
+            log_trial(v[0], fx, acc);
+            if (acc) {
+                accepted = true;
+                fx = v[0];
+                s = sqrt(v[1]);
+                T* t = gc;
+                gc = go;
+                go = t;
+                if (c0 != 0.0) {
+                    t = xc;
+                    xc = xo;
+                    xo = t;
+                }
+            }
+        }
+        // Otherwise (or in the last reduction step, whose gradient nobody needs): the next B candidates per pass, values only,
+        // decided strictly in order -- the first with f(z) <= f(x^{k,n}) is accepted, later ones are discarded uncounted.
+        double cf = 0.0;
+        while (ok && !accepted && trial < SUP_J_MAX) {
+            double coef[B], fzb[B];
+            step_coef(s, jloc, coef, B);
+            tv_share_batch<T, OBJ, B>(view(), coef, fzb);
+            ok = grid_reduce<B>(st, P, PSTRIDE, fzb, gen);
+            if (!ok) break;
+            for (int b = 0; b < B && !accepted && trial < SUP_J_MAX; ++b) {
+                const bool acc = fzb[b] <= fx;
+                ++ell;
+                apow *= A.a;
+                ++jloc;
+                ++trials;
+                ++trial;
+                log_trial(fzb[b], fx, acc);
+                if (acc) {
+                    accepted = true;
+                    cf = coef[b];
+                    fx = fzb[b];
+                }
+            }
+            if (accepted) {
+                if (last) {
+                    pend = cf;  // applied by the final write below
+                } else {
+                    // the gradient at the accepted z (f(z) again, in this pass's summation order, carried from here on)
+                    double v[2];
+                    tv_gz<T, OBJ>(view(), cf, xo, go, v[0], v[1]);
+                    ok = grid_reduce<2>(st, P, PSTRIDE, v, gen);
+                    if (!ok) break;
+                    fx = v[0];
+                    s = sqrt(v[1]);
+                    T* t = gc;
+                    gc = go;
+                    go = t;
+                    if (cf != 0.0) {
+                        t = xc;
+                        xc = xo;
+                        xo = t;
+                    }
+                }
+            }
+        }
+        if (ok && !accepted) warn |= 1;  // A-12: step skipped
+    }
+    // leave the final iterate in the caller's x and in the gather mirror (element-wise: no barrier needed)
+    if (ok && (pend != 0.0 || xc != Ain.x || A.xg)) {
+        for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q < A.n; q += int64_t(gridDim.x) * blockDim.x) {
+            const T v = T(zval(xc, gc, pend, q));
+            if (pend != 0.0 || xc != Ain.x) Ain.x[q] = v;
+            if (A.xg) A.xg[sup_gmap(A.xmap, int(q))] = v;
+        }
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        st->ell = ell;
+        st->apow = apow;
+        st->n_dec = ndec;
+        st->n_trials += trials;
+        st->sweep_trials += trials;
+        st->f = fx;
+        if (warn) atomicOr(&st->warn, warn);
+        if (fault) atomicOr(&st->fault, fault);
+    }
+}
+
+// ---- the perturbation phase, dose objective ------------------------------------------------------------------------
+template <typename T, int OBJ>
+__global__ void __launch_bounds__(SUP_THREADS) k_perturb(PArgs<T> Ain) {
+    static_assert(OBJ == SUP_OBJ_DOSE, "the TV objectives run in k_perturb_tv");
+    const PArgs<T>& A = Ain;
+    T* xc = Ain.x;
+    T* gc = Ain.g;
+    auto view = [&]() { return Ain; };
     DevState* st = A.st;
     long long ell = *(volatile long long*)&st->ell;
     double apow = *(volatile double*)&st->apow;  // a^ell, running product
     const long long k = *(volatile long long*)&st->k;
     long long ndec = *(volatile long long*)&st->n_dec;
     long long trials = 0;
-    // restarted perturbations (PAPER.md:L101, L315; A-24): at the start of sweep k = r * n_restart the exponent is reset to r
     if (A.n_restart > 0 && k > 0 && k % A.n_restart == 0) {
         ell = k / A.n_restart;
         apow = 1.0;
@@ -412,15 +780,14 @@ __global__ void __launch_bounds__(SUP_THREADS) k_perturb(PArgs<T> Ain) {
     double* P0 = A.partials;
     double* P1 = A.partials + SUP_MAX_PARTIALS;
 
-    // fx = f(x)  (dose: r = D x is stored on the way and then carried, r <- r - c q, through the phase)
-    double sh = OBJ == SUP_OBJ_DOSE ? cta_sum(dose_share(view(), 0.0, true)) : cta_sum(objective_share<T, OBJ>(view(), 0.0));
+    // fx = f(x): r = D x is stored on the way and then carried, r <- r - c q, through the phase
+    double sh = cta_sum(dose_share(view(), 0.0, true));
     if (threadIdx.x == 0) P0[blockIdx.x] = sh;
     grid_barrier(st);
     double fx = reduce_partials(P0);
     slot = 1;
     if (!isfinite(fx)) fault |= 2;
-
-    if constexpr (OBJ == SUP_OBJ_DOSE) {
+    {
         // Quadratic objective: with q = D g the objective along the step is the closed form above, so the trial loop is
         // scalar work and a reduction step costs two matrix passes (g = 2 D^T r, q = D g) instead of three or more.
         for (int nred = 0; nred < A.N; ++nred) {
@@ -489,111 +856,10 @@ __global__ void __launch_bounds__(SUP_THREADS) k_perturb(PArgs<T> Ain) {
             }
             if (*(volatile int*)&st->fault & 1) break;
         }
-    } else
-    for (int nred = 0; nred < A.N; ++nred) {
-        double* P = slot ? P1 : P0;
-        slot ^= 1;
-        if (OBJ == SUP_OBJ_DOSE) {  // r = D x first
-            dose_share(view(), 0.0, true);
-            grid_barrier(st);
-            sh = cta_sum(dose_grad_share(view()));
-        } else if (OBJ == SUP_OBJ_TV2D) {
-            sh = cta_sum(tv2d_grad_share(view(), pend, xo, go));
-        } else {
-            sh = cta_sum(tv1d_grad_share(view(), pend, xo, go));
-        }
-        if (threadIdx.x == 0) P[blockIdx.x] = sh;
-        grid_barrier(st);
-        if (DEFER) {  // the new gradient (and, if a step was pending, the new iterate) live in the other buffers now
-            T* t = gc;
-            gc = go;
-            go = t;
-            if (pend != 0.0) {
-                t = xc;
-                xc = xo;
-                xo = t;
-                pend = 0.0;
-            }
-        }
-        const double s = sqrt(reduce_partials(P));
-        bool accepted = false;
-        long long jloc = 0;
-        // Trials are evaluated SUP_TRIAL_BATCH candidates per pass for the TV objectives (their step sizes are known in
-        // advance: beta0 a^l, beta0 a^(l+1), ...), then decided strictly in order: the first candidate with
-        // f(z) <= f(x^{k,n}) is accepted and the later ones are discarded uncounted -- the sequence of trials, decisions
-        // and l is exactly Algorithm 1's; only the number of grid barriers per reduction step drops.
-        constexpr int B = OBJ == SUP_OBJ_DOSE ? 1 : SUP_TRIAL_BATCH;
-        for (int trial = 0; trial < SUP_J_MAX && !accepted; trial += B) {
-            double coef[B], fzb[B];
-            {
-                // a^(exponent of candidate 0) by successive multiplication from 1, like the oracle (A-20): PER_TRIAL carries
-                // the running product a^l across trials and sweeps; PER_SWEEP rebuilds a^(k+j) (k is small)
-                double ap = apow;
-                if (A.policy != SUP_STEP_PER_TRIAL) {
-                    ap = 1.0;
-                    for (long long q = 0; q < k + jloc; ++q) ap *= A.a;
-                }
-#pragma unroll
-                for (int b = 0; b < B; ++b) {
-                    coef[b] = s > 0.0 ? (A.beta0 * ap) / s : 0.0;
-                    ap *= A.a;
-                }
-            }
-            P = slot ? P1 : P0;
-            slot ^= 1;
-            if (B == 1) {
-                fzb[0] = cta_sum(objective_share<T, OBJ>(view(), coef[0]));
-                if (threadIdx.x == 0) P[blockIdx.x] = fzb[0];
-            } else {
-                if (OBJ == SUP_OBJ_TV2D) tv2d_share_batch<T, B>(view(), coef, fzb);
-                else tv1d_share_batch<T, B>(view(), coef, fzb);
-                cta_sum_batch<B>(fzb);
-                if (threadIdx.x < B) P[threadIdx.x * (SUP_MAX_PARTIALS / B) + blockIdx.x] = fzb[threadIdx.x];
-            }
-            grid_barrier(st);
-#pragma unroll
-            for (int b = 0; b < B; ++b) fzb[b] = reduce_partials(P + b * (SUP_MAX_PARTIALS / B));
-            for (int b = 0; b < B && !accepted && trial + b < SUP_J_MAX; ++b) {
-                const double fz = fzb[b];
-                ++ell;
-                apow *= A.a;
-                ++jloc;
-                ++trials;
-                const bool acc = fz <= fx;  // NaN compares false -> rejected (A-11)
-                if (blockIdx.x == 0 && threadIdx.x == 0) {
-                    if (A.decisions && ndec < A.cap) A.decisions[ndec] = acc ? 1 : 0;
-                    if (A.decision_f && ndec < A.cap) {
-                        A.decision_f[2 * ndec] = fz;
-                        A.decision_f[2 * ndec + 1] = fx;
-                    }
-                }
-                ++ndec;
-                if (acc) {
-                    const double cf = coef[b];
-                    if (DEFER) {
-                        pend = cf;
-#ifdef SUP_DEFER_DEBUG
-                        grid_barrier(st);
-#endif
-                    } else {
-                        if (cf != 0.0)
-                            for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q < A.n; q += int64_t(gridDim.x) * blockDim.x)
-                                xc[q] = T(zval(xc, gc, cf, q));
-                        grid_barrier(st);  // x^{k,n+1} visible to everyone before the next gradient
-                    }
-                    fx = fz;
-                    accepted = true;
-                }
-            }
-            if (*(volatile int*)&st->fault & 1) break;  // a barrier timed out: stop looping
-        }
-        if (!accepted) warn |= 1;  // A-12: step skipped
-        if (*(volatile int*)&st->fault & 1) break;
     }
-    if (DEFER && (pend != 0.0 || xc != Ain.x)) {  // leave the final iterate in the caller's x (element-wise: no barrier needed)
+    if (A.xg)  // keep the gather mirror of x in step (element-wise)
         for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q < A.n; q += int64_t(gridDim.x) * blockDim.x)
-            Ain.x[q] = T(zval(xc, gc, pend, q));
-    }
+            A.xg[sup_gmap(A.xmap, int(q))] = xc[q];
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         st->ell = ell;
         st->apow = apow;
@@ -645,8 +911,11 @@ static PArgs<T> make_args(sup_ctx* h, void* x, const PerturbParams& pp) {
     A.x2 = static_cast<T*>(h->x2);
     A.g2 = static_cast<T*>(h->g2);
     A.n = h->n;
+    A.nz = pp.nz;
     A.ny = pp.ny;
     A.nx = pp.nx;
+    A.xg = pp.write_mirror && sup_stream_forward_uses_xg(h) ? static_cast<T*>(h->xg) : nullptr;
+    A.xmap = h->xmap;
     A.N = pp.N;
     A.beta0 = pp.beta0;
     A.a = pp.a;
@@ -674,8 +943,9 @@ static PArgs<T> make_args(sup_ctx* h, void* x, const PerturbParams& pp) {
 template <typename T>
 static const void* perturb_kernel(int objective) {
     switch (objective) {
-        case SUP_OBJ_TV2D: return reinterpret_cast<const void*>(&k_perturb<T, SUP_OBJ_TV2D>);
-        case SUP_OBJ_TV1D: return reinterpret_cast<const void*>(&k_perturb<T, SUP_OBJ_TV1D>);
+        case SUP_OBJ_TV2D: return reinterpret_cast<const void*>(&k_perturb_tv<T, SUP_OBJ_TV2D>);
+        case SUP_OBJ_TV1D: return reinterpret_cast<const void*>(&k_perturb_tv<T, SUP_OBJ_TV1D>);
+        case SUP_OBJ_TV3D: return reinterpret_cast<const void*>(&k_perturb_tv<T, SUP_OBJ_TV3D>);
         case SUP_OBJ_DOSE: return reinterpret_cast<const void*>(&k_perturb<T, SUP_OBJ_DOSE>);
     }
     return nullptr;
@@ -729,8 +999,9 @@ sup_status sup_launch_perturb(sup_ctx* h, void* x, const PerturbParams& pp) {
 }
 
 template <typename T>
-static void launch_objective_t(sup_ctx* h, const void* x, int kind, int64_t ny, int64_t nx, double* out_dev) {
+static void launch_objective_t(sup_ctx* h, const void* x, int kind, int64_t nz, int64_t ny, int64_t nx, double* out_dev) {
     PerturbParams pp = {};
+    pp.nz = nz;
     pp.objective = kind;
     pp.ny = ny;
     pp.nx = nx;
@@ -740,6 +1011,7 @@ static void launch_objective_t(sup_ctx* h, const void* x, int kind, int64_t ny, 
     const int64_t work = kind == SUP_OBJ_DOSE ? h->D.rows * h->g_d : h->n;
     grid = sup_grid_for(work, SUP_THREADS, grid);
     if (kind == SUP_OBJ_TV2D) k_objective<T, SUP_OBJ_TV2D><<<grid, SUP_THREADS, 0, h->stream>>>(A);
+    else if (kind == SUP_OBJ_TV3D) k_objective<T, SUP_OBJ_TV3D><<<grid, SUP_THREADS, 0, h->stream>>>(A);
     else if (kind == SUP_OBJ_TV1D) k_objective<T, SUP_OBJ_TV1D><<<grid, SUP_THREADS, 0, h->stream>>>(A);
     else if (kind == SUP_OBJ_DOSE) k_objective<T, SUP_OBJ_DOSE><<<grid, SUP_THREADS, 0, h->stream>>>(A);
     else k_objective<T, SUP_OBJ_NONE><<<1, SUP_THREADS, 0, h->stream>>>(A);
@@ -747,9 +1019,9 @@ static void launch_objective_t(sup_ctx* h, const void* x, int kind, int64_t ny, 
     h->launches += 2;
 }
 
-void sup_launch_objective(sup_ctx* h, const void* x, int kind, int64_t ny, int64_t nx, double* out_dev) {
-    if (h->dt == SUP_F32) launch_objective_t<float>(h, x, kind, ny, nx, out_dev);
-    else launch_objective_t<double>(h, x, kind, ny, nx, out_dev);
+void sup_launch_objective(sup_ctx* h, const void* x, int kind, int64_t nz, int64_t ny, int64_t nx, double* out_dev) {
+    if (h->dt == SUP_F32) launch_objective_t<float>(h, x, kind, nz, ny, nx, out_dev);
+    else launch_objective_t<double>(h, x, kind, nz, ny, nx, out_dev);
 }
 
 void sup_launch_end_sweep(sup_ctx* h, double* trace) {

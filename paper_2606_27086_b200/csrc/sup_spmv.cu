@@ -59,7 +59,7 @@ template <typename T>
 __global__ void __launch_bounds__(SUP_THREADS)
     k_bwd(int64_t n, const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col, const T* __restrict__ val,
           const T* __restrict__ y, const T* __restrict__ lo, const T* __restrict__ hi, T lambda, T* __restrict__ x,
-          T* __restrict__ xg, int G) {
+          T* __restrict__ xg, int G, const GMap xmap) {
     const int gl = threadIdx.x % G;
     const int64_t j = (int64_t(blockIdx.x) * blockDim.x + threadIdx.x) / G;
     const bool valid = j < n;
@@ -70,7 +70,7 @@ __global__ void __launch_bounds__(SUP_THREADS)
         t = t < lo[j] ? lo[j] : t;  // box, un-relaxed (A-2)
         t = t > hi[j] ? hi[j] : t;
         x[j] = t;
-        if (xg) xg[sup_swz(int(j))] = t;  // de-aliased mirror read by the staged forward product (sup_stream.cu)
+        if (xg) xg[sup_gmap(xmap, int(j))] = t;  // gather mirror read by the staged forward product (sup_stream.cu)
     }
 }
 
@@ -108,12 +108,12 @@ void sup_launch_bwd(sup_ctx* h, const CsrD& AT, int G, void* x, double lambda) {
         k_bwd<float><<<grid, SUP_THREADS, 0, h->stream>>>(
             AT.rows, AT.rowptr, AT.col, static_cast<const float*>(AT.val), static_cast<const float*>(h->y),
             static_cast<const float*>(h->lo), static_cast<const float*>(h->hi), float(lambda), static_cast<float*>(x),
-            static_cast<float*>(mirror), G);
+            static_cast<float*>(mirror), G, h->xmap);
     else
         k_bwd<double><<<grid, SUP_THREADS, 0, h->stream>>>(
             AT.rows, AT.rowptr, AT.col, static_cast<const double*>(AT.val), static_cast<const double*>(h->y),
             static_cast<const double*>(h->lo), static_cast<const double*>(h->hi), lambda, static_cast<double*>(x),
-            static_cast<double*>(mirror), G);
+            static_cast<double*>(mirror), G, h->xmap);
     h->launches++;
 }
 

@@ -42,6 +42,9 @@
 template <typename T, int MODE>
 __host__ __device__ constexpr int rg_stages() { return (MODE == 0 && sizeof(T) == 4) ? RG_STAGES_FWD : RG_STAGES; }
 #define RG_CWARPS 16                        // upper bound on the consumer warps (sizes of the shared arrays)
+#ifndef RG_NPROD
+#define RG_NPROD 2                          // producer warps: ONE thread issues at most one bulk copy per ~270 ns whatever its size
+#endif                                      // (profiles/r02b_producer.md), i.e. 4.5 TB/s of 8 KB tiles chip-wide; two reach the HBM rate
 #ifndef RG_NCW
 #define RG_NCW 12                           // consumer warps: measured best on config 3 (8: 4.50/4.23, 12: 4.63/4.94, 16: 4.50/4.78 TB/s fwd/bwd)
 #endif
@@ -81,6 +84,23 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
                  ::"r"(dst), "l"(src), "r"(bytes), "r"(bar), "l"(pol) : "memory");
 }
+
+#ifdef SUP_PROFILE
+__device__ unsigned long long g_prof[8];  // 0 consumer data-wait, 1 consumer dot, 2 consumer total, 3 producer free-wait, 4 producer total, 5 kernel
+#define PROF_T(v) const long long v = clock64()
+#define PROF_DECL long long prof_acc[6] = {0, 0, 0, 0, 0, 0}
+#define PROF_ADD(i, d) prof_acc[i] += (long long)(d)
+#define PROF_FLUSH(i) do { if (lane == 0) atomicAdd(&g_prof[i], (unsigned long long)prof_acc[i]); } while (0)
+extern "C" void sup_prof_read(unsigned long long* out, int reset) {
+    cudaMemcpyFromSymbol(out, g_prof, sizeof(g_prof));
+    if (reset) { unsigned long long z[8] = {0}; cudaMemcpyToSymbol(g_prof, z, sizeof(z)); }
+}
+#else
+#define PROF_T(v)
+#define PROF_DECL
+#define PROF_ADD(i, d)
+#define PROF_FLUSH(i)
+#endif
 
 template <typename T>
 __device__ __forceinline__ T hyperslab_violation(T r, T lb, T ub) {  // Eq. 2 on each face of lb <= r <= ub
@@ -182,10 +202,10 @@ __device__ __forceinline__ void ring_row_dot(const RgData<T, STG>& ring, const T
 // MODE 0: forward (vec = xg, columns swizzled (pk / colg), p1 = lb, p2 = ub, p3 = d, out = y);
 // MODE 1: backward (vec = y, p1 = lo, p2 = hi, out = x in place, out2 = xg mirror or NULL)
 template <typename T, int MODE, int G, int NCW>
-__global__ void __launch_bounds__(32 * (NCW + 1), 1)
+__global__ void __launch_bounds__(32 * (NCW + RG_NPROD), 1)
     k_staged(const int64_t* __restrict__ part, const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
              const T* __restrict__ val, const uint2* __restrict__ pk, const T* __restrict__ vec, const T* __restrict__ p1,
-             const T* __restrict__ p2, const T* __restrict__ p3, T* out, T* out2, T lambda, int64_t nnz_total) {
+             const T* __restrict__ p2, const T* __restrict__ p3, T* out, T* out2, T lambda, int64_t nnz_total, const GMap omap) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int STG = rg_stages<T, MODE>();
     constexpr int RG_ELEMS = STG * RG_TILE;
@@ -208,16 +228,19 @@ __global__ void __launch_bounds__(32 * (NCW + 1), 1)
     volatile int* progress = S.progress;
     volatile int* issued = S.issued;
 
-    if (warp == NCW) {
-        // ---- producer: one lane feeds the ring (more lanes brought nothing: the limit is the copy engine's per-copy
-        // cost, not the issue loop; profiles/r01c_staged.md) -----------------------------------------------------------
+    if (warp >= NCW) {
+        // ---- producers: lane 0 of each producer warp feeds the ring, warp p the tiles t = p (mod RG_NPROD).  (More LANES
+        // of one warp brought nothing in round 1 -- they serialise; separate warps issue in parallel.) ---------------------
         if (lane == 0) {
             const uint64_t pol = l2_evict_first_policy();
             const int64_t bulk_limit = nnz_total & ~int64_t(3);  // bulk copies never read past the arrays' last whole 16 B
             int freed = 0;                                        // min over the consumer warps' progress
-            for (int t = 0; t < ntiles; ++t) {
+            PROF_DECL;
+            PROF_T(pt0);
+            for (int t = warp - NCW; t < ntiles; t += RG_NPROD) {
                 const int s = t % STG;
                 if (t >= STG && freed <= t - STG) {
+                    PROF_T(pw0);
                     const long long t0 = clock64();
                     for (;;) {
                         int mn = progress[0];
@@ -232,6 +255,7 @@ __global__ void __launch_bounds__(32 * (NCW + 1), 1)
                     }
                     // the consumers' reads of the stage (generic proxy) precede the bulk write (async proxy)
                     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                    PROF_ADD(3, clock64() - pw0);
                 }
                 const int64_t g0 = base + int64_t(t) * RG_TILE;
                 const int64_t g1 = (g0 + RG_TILE < ee) ? g0 + RG_TILE : ee;  // elements needed: [g0, g1)
@@ -260,9 +284,14 @@ __global__ void __launch_bounds__(32 * (NCW + 1), 1)
                 }
                 issued[s] = t + 1;  // the stage's barrier is armed for tile t: consumers may now wait on its phase
             }
+            PROF_ADD(4, clock64() - pt0);
+            PROF_FLUSH(3);
+            PROF_FLUSH(4);
             // Do not leave while a copy may still be in flight into this CTA's shared memory (the consumers wait on every
             // tile their rows touch, but a tile holding only alignment padding or the tail of an empty row has no reader).
-            for (int t = ntiles > STG ? ntiles - STG : 0; t < ntiles; ++t) mbar_wait(smem_u32(&S.full[t % STG]), (t / STG) & 1);
+            // (each producer waits for the tiles it armed itself, so the phase parity is unambiguous)
+            for (int t = ntiles > STG ? ntiles - STG : 0; t < ntiles; ++t)
+                if (t % RG_NPROD == warp - NCW) mbar_wait(smem_u32(&S.full[t % STG]), (t / STG) & 1);
         }
         return;
     }
@@ -328,13 +357,13 @@ __global__ void __launch_bounds__(32 * (NCW + 1), 1)
 #pragma unroll
                 for (int w = 0; w < NCW; ++w) tot += S.ctabuf[iter & 1][w];
                 if (MODE == 0) {
-                    out[r] = q3 * hyperslab_violation(tot, q1, q2);
+                    out[sup_gmap(omap, int(r))] = q3 * hyperslab_violation(tot, q1, q2);
                 } else {
                     T t = q3 - lambda * tot;
                     t = t < q1 ? q1 : t;
                     t = t > q2 ? q2 : t;
                     out[r] = t;
-                    if (out2) out2[sup_swz(int(r))] = t;
+                    if (out2) out2[sup_gmap(omap, int(r))] = t;
                 }
             }
             s = s_next;
@@ -365,15 +394,19 @@ __global__ void __launch_bounds__(32 * (NCW + 1), 1)
         s = int(rowptr[r < re ? r : re] - base);
         e = int(rowptr[r + 1 < re ? r + 1 : re] - base);
     }
+    PROF_DECL;
+    PROF_T(ct0);
     for (; rf < re; rf += stride, ++iter) {
         const int64_t r = rf + sub;
         const bool valid = r < re;
-        // prefetch the next iteration's row extent and this row's epilogue operands before touching the ring
-        int s_next = 0, e_next = 0;
+        // prefetch the next iteration's row extent and this row's epilogue operands before touching the ring; the raw
+        // row pointers are only turned into offsets at the END of the iteration, so the loads' latency (they were
+        // ~10 % of the forward kernel's stall samples when consumed here, profiles/r02d) hides behind the dot product
+        int64_t rp_s_next = base, rp_e_next = base;
         const int64_t rn = r + stride;
         if (rf + stride < re) {
-            s_next = int(rowptr[rn < re ? rn : re] - base);
-            e_next = int(rowptr[rn + 1 < re ? rn + 1 : re] - base);
+            rp_s_next = rowptr[rn < re ? rn : re];
+            rp_e_next = rowptr[rn + 1 < re ? rn + 1 : re];
         }
         T q1 = T(0), q2 = T(0), q3 = T(0);
         if (valid && gl == 0) {  // (in a pair: lane 0 of the even warp)
@@ -392,6 +425,7 @@ __global__ void __launch_bounds__(32 * (NCW + 1), 1)
         }
         // Wait for the tiles this warp's rows span (span <= STG - 1 tiles by the plan): first until the stage is
         // armed for THAT tile (so the phase parity is unambiguous), then on the stage's mbarrier (a hardware wait).
+        PROF_T(cw0);
         if (w_end > w_start) {
             const int t_hi = (w_end - 1) / RG_TILE;
             for (int t = seen > t_start ? seen : t_start; t <= t_hi; ++t) {
@@ -406,6 +440,8 @@ __global__ void __launch_bounds__(32 * (NCW + 1), 1)
             seen = seen > t_hi + 1 ? seen : t_hi + 1;
         }
         asm volatile("" ::: "memory");
+        PROF_T(cd0);
+        PROF_ADD(0, cd0 - cw0);
         // row dot product from the ring
         T a0 = T(0), a1 = T(0), a2 = T(0), a3 = T(0);
         const bool wraps = (w_start % RG_ELEMS) + (w_end - w_start) > RG_ELEMS;  // warp-uniform
@@ -420,6 +456,7 @@ __global__ void __launch_bounds__(32 * (NCW + 1), 1)
         T acc = (a0 + a1) + (a2 + a3);
 #pragma unroll
         for (int o = GL >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o, GL);
+        PROF_ADD(1, clock64() - cd0);
         if (PAIR) {  // odd warp -> shared slot (double-buffered by iteration parity) -> pair barrier -> even warp adds
             if ((warp & 1) && lane == 0) S.pairbuf[unit][iter & 1] = acc;
             asm volatile("bar.sync %0, 64;" ::"r"(1 + unit) : "memory");
@@ -427,21 +464,27 @@ __global__ void __launch_bounds__(32 * (NCW + 1), 1)
         }
         if (valid && gl == 0) {
             if (MODE == 0) {
-                out[r] = q3 * hyperslab_violation(acc, q1, q2);  // y_i = d_i c_i
+                out[sup_gmap(omap, int(r))] = q3 * hyperslab_violation(acc, q1, q2);  // y_i = d_i c_i (in y's gather layout)
             } else {
                 T t = q3 - lambda * acc;  // Eq. 3
                 t = t < q1 ? q1 : t;      // box, un-relaxed (A-2)
                 t = t > q2 ? q2 : t;
                 out[r] = t;
-                if (out2) out2[sup_swz(int(r))] = t;  // keep the de-aliased mirror of x in step
+                if (out2) out2[sup_gmap(omap, int(r))] = t;  // keep the gather mirror of x in step
             }
         }
-        s = s_next;
-        e = e_next;
+        s = int(rp_s_next - base);
+        e = int(rp_e_next - base);
     }
     // this warp needs nothing more
     __syncwarp();
     if (lane == 0) progress[warp] = ntiles;
+    PROF_ADD(2, clock64() - ct0);
+    if (warp == 0) PROF_ADD(5, clock64() - ct0);
+    PROF_FLUSH(0);
+    PROF_FLUSH(1);
+    PROF_FLUSH(2);
+    PROF_FLUSH(5);
     }
 }
 
@@ -491,7 +534,7 @@ static int staged_occupancy() {
     const int smem = int(sizeof(RgSmem<T, rg_stages<T, MODE>()>));
     int occ = 0;
     if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess ||
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, 32 * (RG_NCW + 1), smem) != cudaSuccess) {
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, 32 * (RG_NCW + RG_NPROD), smem) != cudaSuccess) {
         cudaGetLastError();
         return 0;
     }
@@ -563,58 +606,61 @@ sup_status sup_stream_plan(sup_ctx* h, const CsrD& M, int64_t r0, int64_t r1, bo
 // ---- launchers --------------------------------------------------------------------------------------------------------
 template <typename T, int MODE, int G>
 static void launch_staged_g(sup_ctx* h, const StreamPlan& sp, const CsrD& M, const void* vec, const void* p1, const void* p2,
-                            const void* p3, void* out, void* out2, double lambda) {
+                            const void* p3, void* out, void* out2, double lambda, const GMap& omap) {
     const void* fn = reinterpret_cast<const void*>(&k_staged<T, MODE, G, RG_NCW>);
     constexpr int smem = int(sizeof(RgSmem<T, rg_stages<T, MODE>()>));
     if (!h->smem_opted_in.count(fn)) {  // per handle, hence per device: opt in to > 48 KB of dynamic shared memory
         cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         h->smem_opted_in.insert(fn);
     }
-    k_staged<T, MODE, G, RG_NCW><<<sp.nb, 32 * (RG_NCW + 1), smem, h->stream>>>(
+    k_staged<T, MODE, G, RG_NCW><<<sp.nb, 32 * (RG_NCW + RG_NPROD), smem, h->stream>>>(
         sp.part, M.rowptr, M.col, static_cast<const T*>(M.val), static_cast<const uint2*>(M.pk), static_cast<const T*>(vec),
         static_cast<const T*>(p1), static_cast<const T*>(p2), static_cast<const T*>(p3), static_cast<T*>(out),
-        static_cast<T*>(out2), T(lambda), M.alloc_nnz);
+        static_cast<T*>(out2), T(lambda), M.alloc_nnz, omap);
     h->launches++;
 }
 
 template <typename T, int MODE>
 static void launch_staged(sup_ctx* h, const StreamPlan& sp, const CsrD& M, const void* vec, const void* p1, const void* p2,
-                          const void* p3, void* out, void* out2, double lambda) {
+                          const void* p3, void* out, void* out2, double lambda, const GMap& omap) {
     switch (sp.G) {
-        case 4: launch_staged_g<T, MODE, 4>(h, sp, M, vec, p1, p2, p3, out, out2, lambda); break;
-        case 8: launch_staged_g<T, MODE, 8>(h, sp, M, vec, p1, p2, p3, out, out2, lambda); break;
-        case 16: launch_staged_g<T, MODE, 16>(h, sp, M, vec, p1, p2, p3, out, out2, lambda); break;
-        case 64: launch_staged_g<T, MODE, 64>(h, sp, M, vec, p1, p2, p3, out, out2, lambda); break;
-        case 0: launch_staged_g<T, MODE, 0>(h, sp, M, vec, p1, p2, p3, out, out2, lambda); break;
-        default: launch_staged_g<T, MODE, 32>(h, sp, M, vec, p1, p2, p3, out, out2, lambda); break;
+        case 4: launch_staged_g<T, MODE, 4>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap); break;
+        case 8: launch_staged_g<T, MODE, 8>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap); break;
+        case 16: launch_staged_g<T, MODE, 16>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap); break;
+        case 64: launch_staged_g<T, MODE, 64>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap); break;
+        case 0: launch_staged_g<T, MODE, 0>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap); break;
+        default: launch_staged_g<T, MODE, 32>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap); break;
     }
 }
 
-// ---- de-aliased mirror of x ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(SUP_THREADS) k_swizzle_cols(const int32_t* __restrict__ col, int64_t nnz, int32_t* __restrict__ colg) {
+// ---- gather layouts: the mirror of x and the internal layout of y (GMap, sup_internal.cuh) ------------------------------
+__global__ void __launch_bounds__(SUP_THREADS) k_map_cols(const int32_t* __restrict__ col, int64_t nnz, int32_t* __restrict__ colg, const GMap map) {
     for (int64_t k = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; k < nnz; k += int64_t(gridDim.x) * blockDim.x)
-        colg[k] = sup_swz(col[k]);
+        colg[k] = sup_gmap(map, col[k]);
 }
 
 template <typename T>
-__global__ void __launch_bounds__(SUP_THREADS) k_swizzle_copy(const T* __restrict__ x, int n, T* __restrict__ xg) {
+__global__ void __launch_bounds__(SUP_THREADS) k_map_copy(const T* __restrict__ x, int n, T* __restrict__ xg, const GMap map) {
     const int j = blockIdx.x * blockDim.x + threadIdx.x;
-    if (j < n) xg[sup_swz(j)] = x[j];
+    if (j < n) xg[sup_gmap(map, j)] = x[j];
 }
 
-template <bool SWZ>
+template <typename T>
+__global__ void __launch_bounds__(SUP_THREADS) k_unmap_copy(const T* __restrict__ src, int n, T* __restrict__ dst, const GMap map) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j < n) dst[j] = src[sup_gmap(map, j)];
+}
+
 __global__ void __launch_bounds__(SUP_THREADS) k_pack(const float* __restrict__ val, const int32_t* __restrict__ col, int64_t nnz,
-                                                       uint2* __restrict__ pk) {
-    for (int64_t k = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; k < nnz; k += int64_t(gridDim.x) * blockDim.x) {
-        const int c = col[k];
-        pk[k] = make_uint2(__float_as_uint(val[k]), unsigned(SWZ ? sup_swz(c) : c));
-    }
+                                                       uint2* __restrict__ pk, const GMap map) {
+    for (int64_t k = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; k < nnz; k += int64_t(gridDim.x) * blockDim.x)
+        pk[k] = make_uint2(__float_as_uint(val[k]), unsigned(sup_gmap(map, col[k])));
 }
 
-sup_status sup_stream_pack(sup_ctx* h, const void* val, const int32_t* col, int64_t nnz, void* dst) {
+sup_status sup_stream_pack(sup_ctx* h, const void* val, const int32_t* col, int64_t nnz, void* dst, const GMap& map) {
     if (h->dt != SUP_F32 || !dst || nnz == 0) return SUP_OK;
-    k_pack<false><<<sup_grid_for(nnz, SUP_THREADS, h->num_sms * 16), SUP_THREADS, 0, h->stream>>>(
-        static_cast<const float*>(val), col, nnz, static_cast<uint2*>(dst));
+    k_pack<<<sup_grid_for(nnz, SUP_THREADS, h->num_sms * 16), SUP_THREADS, 0, h->stream>>>(
+        static_cast<const float*>(val), col, nnz, static_cast<uint2*>(dst), map);
     h->launches++;
     SUP_CUDA(h, cudaGetLastError());
     return SUP_OK;
@@ -624,17 +670,24 @@ sup_status sup_stream_setup_gather(sup_ctx* h) {
     if (h->nnz == 0) return SUP_OK;
     const int grid = sup_grid_for(h->nnz, SUP_THREADS, h->num_sms * 16);
     if (h->dt == SUP_F32 && h->pk_a) {
-        k_pack<true><<<grid, SUP_THREADS, 0, h->stream>>>(static_cast<const float*>(h->A.val), h->A.col, h->nnz,
-                                                         static_cast<uint2*>(h->pk_a));
+        k_pack<<<grid, SUP_THREADS, 0, h->stream>>>(static_cast<const float*>(h->A.val), h->A.col, h->nnz,
+                                                   static_cast<uint2*>(h->pk_a), h->xmap);
         h->A.pk = h->pk_a;
     } else if (h->colg) {
-        k_swizzle_cols<<<grid, SUP_THREADS, 0, h->stream>>>(h->A.col, h->nnz, h->colg);
+        k_map_cols<<<grid, SUP_THREADS, 0, h->stream>>>(h->A.col, h->nnz, h->colg, h->xmap);
     } else {
         return SUP_OK;
     }
     h->launches++;
     SUP_CUDA(h, cudaGetLastError());
     return SUP_OK;
+}
+
+void sup_launch_unmap(sup_ctx* h, const void* src, void* dst, int64_t count, const GMap& map) {
+    const unsigned grid = unsigned((count + SUP_THREADS - 1) / SUP_THREADS);
+    if (h->dt == SUP_F32) k_unmap_copy<float><<<grid, SUP_THREADS, 0, h->stream>>>(static_cast<const float*>(src), int(count), static_cast<float*>(dst), map);
+    else k_unmap_copy<double><<<grid, SUP_THREADS, 0, h->stream>>>(static_cast<const double*>(src), int(count), static_cast<double*>(dst), map);
+    h->launches++;
 }
 
 bool sup_stream_forward_uses_xg(const sup_ctx* h) {
@@ -645,27 +698,45 @@ bool sup_stream_forward_uses_xg(const sup_ctx* h) {
     return false;
 }
 
+// The row-side map (the layout of the internal y) is in force only when EVERY product of the handle runs on the staged fp32
+// kernels: they read y through the packed copies of A^T, which carry the mapped row index; the group-per-row kernels
+// and fp64 handles index y directly.  Rewrites every packed / mapped copy accordingly.
+sup_status sup_stream_refresh_layout(sup_ctx* h) {
+    bool all = h->use_stream && h->dt == SUP_F32 && h->pk_a && h->pk_at && h->A.plan.ok && h->AT.plan.ok;
+    for (int t = 0; all && t < h->n_blocks; ++t) {
+        const bool empty = h->block_rowptr[t + 1] == h->block_rowptr[t];
+        all = empty || (h->stream_fwd_blk[t].ok && h->ATb[t].plan.ok && h->pk_atb);
+    }
+    h->ymap = all ? h->ymap_req : GMap();
+    h->xg_synced = false;
+    if (!h->use_stream) return SUP_OK;
+    sup_status rc = sup_stream_setup_gather(h);
+    if (rc == SUP_OK) rc = sup_stream_pack(h, h->AT.val, h->AT.col, h->nnz, h->pk_at, h->ymap);
+    if (rc == SUP_OK && h->n_blocks > 0 && h->pk_atb) rc = sup_stream_pack(h, h->ATb[0].val, h->ATb[0].col, h->nnz, h->pk_atb, h->ymap);
+    return rc;
+}
+
 void sup_launch_stream_fwd(sup_ctx* h, const StreamPlan& sp, const void* x, const void* dscale) {
     CsrD M = h->A;
     const void* vec = x;
     if ((h->colg || h->A.pk) && h->xg) {
         if (!h->xg_synced) {
             const unsigned grid = unsigned((h->n + SUP_THREADS - 1) / SUP_THREADS);
-            if (h->dt == SUP_F32) k_swizzle_copy<float><<<grid, SUP_THREADS, 0, h->stream>>>(static_cast<const float*>(x), int(h->n), static_cast<float*>(h->xg));
-            else k_swizzle_copy<double><<<grid, SUP_THREADS, 0, h->stream>>>(static_cast<const double*>(x), int(h->n), static_cast<double*>(h->xg));
+            if (h->dt == SUP_F32) k_map_copy<float><<<grid, SUP_THREADS, 0, h->stream>>>(static_cast<const float*>(x), int(h->n), static_cast<float*>(h->xg), h->xmap);
+            else k_map_copy<double><<<grid, SUP_THREADS, 0, h->stream>>>(static_cast<const double*>(x), int(h->n), static_cast<double*>(h->xg), h->xmap);
             h->launches++;
             h->xg_synced = true;
         }
-        if (h->colg) M.col = h->colg;  // fp32: the swizzled column is inside M.pk
+        if (h->colg) M.col = h->colg;  // fp32: the mapped column is inside M.pk
         vec = h->xg;
     }
-    if (h->dt == SUP_F32) launch_staged<float, 0>(h, sp, M, vec, h->lb, h->ub, dscale, h->y, nullptr, 0.0);
-    else launch_staged<double, 0>(h, sp, M, vec, h->lb, h->ub, dscale, h->y, nullptr, 0.0);
+    if (h->dt == SUP_F32) launch_staged<float, 0>(h, sp, M, vec, h->lb, h->ub, dscale, h->y, nullptr, 0.0, h->ymap);
+    else launch_staged<double, 0>(h, sp, M, vec, h->lb, h->ub, dscale, h->y, nullptr, 0.0, h->ymap);
 }
 
 void sup_launch_stream_bwd(sup_ctx* h, const CsrD& AT, const StreamPlan& sp, void* x, double lambda) {
     void* mirror = sup_stream_forward_uses_xg(h) ? h->xg : nullptr;
-    if (h->dt == SUP_F32) launch_staged<float, 1>(h, sp, AT, h->y, h->lo, h->hi, nullptr, x, mirror, lambda);
-    else launch_staged<double, 1>(h, sp, AT, h->y, h->lo, h->hi, nullptr, x, mirror, lambda);
+    if (h->dt == SUP_F32) launch_staged<float, 1>(h, sp, AT, h->y, h->lo, h->hi, nullptr, x, mirror, lambda, h->xmap);
+    else launch_staged<double, 1>(h, sp, AT, h->y, h->lo, h->hi, nullptr, x, mirror, lambda, h->xmap);
     h->xg_synced = mirror != nullptr;
 }

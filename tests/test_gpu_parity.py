@@ -729,3 +729,55 @@ def test_degenerate_inputs(name, dtype):
             assert sup.sup_objective(H, xs, "tv2d", shape) == 0.0
             ell = sup.sup_perturb_tv(H, xs, shape, 3, 1.0, 0.9, 0)
             assert ell == 3 and torch.equal(xs, before)  # g = 0: every step accepted with equality, x untouched (A-6)
+
+
+# ------------------------------------------------------------------------------------------------------------
+# gather layouts (sup_set_layout): pure data layout, results bit-identical with and without the hint
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", [0, 1])
+@pytest.mark.parametrize("name", ["cfg1", "ct_ragged", "cfg2"])
+def test_layout_hint_changes_no_bit(name, dtype):
+    """Tiled gather copies of x (image) and y (sinogram; fp32 handles) against the plain layout: same sums, same order."""
+    from paper_2606_27086_b200.binding import create_from_problem, sup_get_derived
+
+    sup = _sup()
+    P = problem(name)
+    outs, ys = [], []
+    for layout in (False, True):
+        H = create_from_problem(P, dtype=dtype, blocks=False, layout=layout)
+        if layout and name == "cfg2":  # rows of the crosswell matrix are sources x receivers
+            sup.sup_set_layout(H, P.shape, (64, 64))
+        x = xdev(P, dtype)
+        sup.sup_superiorize(H, x, 6, P.N, P.beta0, P.a, objective=P.objective, shape=P.shape, lam=P.lam)
+        sup.sup_project_simultaneous(H, x, 0.7, 3)
+        sup.sup_forward_violation(H, x)
+        ys.append(sup_get_derived(H, 5).cpu())
+        outs.append(x.cpu())
+    assert torch.equal(outs[0], outs[1])
+    assert torch.equal(ys[0], ys[1])  # y is handed out in row order whatever its internal layout
+
+
+def test_layout_hint_with_blocks_and_fallback_kernels():
+    sup = _sup()
+    base = gen.config1_tiny_ct(n_pix=48, n_angles=64, n_bins=69, n_sweeps=10, N=2)
+    P = gen.interleaved_angle_blocks(base, 16)
+    ref = None
+    for mode in ("plain", "layout", "layout+fallback", "fallback+layout"):
+        H = make_handle(P, 0) if mode != "plain" else __import__("paper_2606_27086_b200.binding", fromlist=["x"]).create_from_problem(P, dtype=0, layout=False)
+        if mode == "layout+fallback":
+            sup.sup_set_row_mode(H, -2, -2)  # group-per-row kernels: the row-side map must be dropped again
+        if mode == "fallback+layout":
+            sup.sup_set_row_mode(H, -2, -2)
+            sup.sup_set_layout(H, P.shape, (64, 69))
+            sup.sup_set_row_mode(H, -1, -1)
+        x = xdev(P, 0)
+        sup.sup_superiorize(H, x, 5, P.N, P.beta0, P.a, objective=P.objective, shape=P.shape, lam=P.lam, block=True)
+        sup.sup_project_simultaneous(H, x, 1.0, 2)
+        if mode == "layout+fallback":  # another kernel, another summation order inside a row
+            assert rel_l2(x.cpu().numpy(), ref.numpy()) <= 1e-5
+        elif ref is None:
+            ref = x.cpu()
+        else:
+            assert torch.equal(x.cpu(), ref), mode
+    with pytest.raises(sup.SupError):
+        sup.sup_set_layout(H, (5, 7), None)
