@@ -32,22 +32,24 @@
 #ifndef RG_TILE
 #define RG_TILE 1024                        // elements per stage
 #endif
-#ifndef RG_STAGES
-#define RG_STAGES 16
-#endif
-#ifndef RG_STAGES_FWD
-#define RG_STAGES_FWD 20                    // fp32 forward product: a deeper ring (5.00 -> 5.15 TB/s); the back-projection needs that
-#endif                                      // shared memory as L1 for its y gathers (20 stages there: 5.10 -> 3.78 TB/s)
-// stages of the ring of k_staged<T, MODE>; the ring capacity STG * RG_TILE need not be a power of two
-template <typename T, int MODE>
-__host__ __device__ constexpr int rg_stages() { return (MODE == 0 && sizeof(T) == 4) ? RG_STAGES_FWD : RG_STAGES; }
-#define RG_CWARPS 16                        // upper bound on the consumer warps (sizes of the shared arrays)
+// Shape of the persistent CTA: consumer warps NCW and ring stages STG (fp32 tiles are 8 KB of packed pairs, fp64 tiles
+// 12 KB of separate val / col).  More warps in flight hide more gather latency, but the rows they hold at once take ring
+// stages away from the prefetch, and the ring takes shared memory away from the L1 the gathers live in.  Two shapes per
+// direction (profiles/r02e_sweep.md, config 3):
+//   DEEP  -- the gathered vector has a tiled layout (sup_set_layout: its working set in L1 is ~2.6x smaller): 24 stages
+//            (the most that keeps the 196 KB shared-memory carve-out; 25 fall off a cliff), 14 / 18 warps forward / backward
+//   BASE  -- no layout known: round 1's shape, 12 warps, 20 stages forward / 16 backward (a deeper ring starves the L1)
+// fp64 handles: BASE warps with 16 stages (192 KB).
+#define RG_STAGES_MIN 16                    // what the planner may count on in every instantiation
+template <typename T, int MODE, bool DEEP>
+struct RgShape {
+    static constexpr int NCW = !DEEP || sizeof(T) != 4 ? 12 : (MODE == 0 ? 14 : 18);
+    static constexpr int STG = sizeof(T) != 4 ? 16 : (DEEP ? 24 : (MODE == 0 ? 20 : 16));
+};
+#define RG_CWARPS 24                        // upper bound on the consumer warps (sizes of the shared arrays)
 #ifndef RG_NPROD
 #define RG_NPROD 2                          // producer warps: ONE thread issues at most one bulk copy per ~270 ns whatever its size
 #endif                                      // (profiles/r02b_producer.md), i.e. 4.5 TB/s of 8 KB tiles chip-wide; two reach the HBM rate
-#ifndef RG_NCW
-#define RG_NCW 12                           // consumer warps: measured best on config 3 (8: 4.50/4.23, 12: 4.63/4.94, 16: 4.50/4.78 TB/s fwd/bwd)
-#endif
 #ifndef RG_UNROLL
 #define RG_UNROLL 16                        // independent gathers in flight per lane (a multiple of 4)
 #endif
@@ -201,13 +203,12 @@ __device__ __forceinline__ void ring_row_dot(const RgData<T, STG>& ring, const T
 
 // MODE 0: forward (vec = xg, columns swizzled (pk / colg), p1 = lb, p2 = ub, p3 = d, out = y);
 // MODE 1: backward (vec = y, p1 = lo, p2 = hi, out = x in place, out2 = xg mirror or NULL)
-template <typename T, int MODE, int G, int NCW>
+template <typename T, int MODE, int G, int NCW, int STG>
 __global__ void __launch_bounds__(32 * (NCW + RG_NPROD), 1)
     k_staged(const int64_t* __restrict__ part, const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
              const T* __restrict__ val, const uint2* __restrict__ pk, const T* __restrict__ vec, const T* __restrict__ p1,
              const T* __restrict__ p2, const T* __restrict__ p3, T* out, T* out2, T lambda, int64_t nnz_total, const GMap omap) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    constexpr int STG = rg_stages<T, MODE>();
     constexpr int RG_ELEMS = STG * RG_TILE;
     RgSmem<T, STG>& S = *reinterpret_cast<RgSmem<T, STG>*>(smem_raw);
     const int64_t rs = part[blockIdx.x], re = part[blockIdx.x + 1];
@@ -528,13 +529,14 @@ __global__ void __launch_bounds__(SUP_THREADS) k_stream_max_row(const int64_t* _
 
 size_t sup_stream_table_bytes() { return ((size_t(SUP_STREAM_NBMAX) + 1) * 8 + 255) & ~size_t(255); }
 
-template <typename T, int MODE>
+template <typename T, int MODE, bool DEEP>
 static int staged_occupancy() {
-    const void* fn = reinterpret_cast<const void*>(&k_staged<T, MODE, 32, RG_NCW>);
-    const int smem = int(sizeof(RgSmem<T, rg_stages<T, MODE>()>));
+    using Sh = RgShape<T, MODE, DEEP>;
+    const void* fn = reinterpret_cast<const void*>(&k_staged<T, MODE, 32, Sh::NCW, Sh::STG>);
+    const int smem = int(sizeof(RgSmem<T, Sh::STG>));
     int occ = 0;
     if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess ||
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, 32 * (RG_NCW + RG_NPROD), smem) != cudaSuccess) {
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, 32 * (Sh::NCW + RG_NPROD), smem) != cudaSuccess) {
         cudaGetLastError();
         return 0;
     }
@@ -544,8 +546,16 @@ static int staged_occupancy() {
 static int stream_grid(sup_ctx* h) {  // persistent grid = resident CTAs per SM x SMs (0: unavailable)
     if (h->stream_nb) return h->stream_nb > 0 ? h->stream_nb : 0;
     int a, b;
-    if (h->dt == SUP_F32) { a = staged_occupancy<float, 0>(); b = staged_occupancy<float, 1>(); }
-    else { a = staged_occupancy<double, 0>(); b = staged_occupancy<double, 1>(); }
+    if (h->dt == SUP_F32) {
+        a = staged_occupancy<float, 0, false>();
+        b = staged_occupancy<float, 1, false>();
+        const int c = staged_occupancy<float, 0, true>(), d = staged_occupancy<float, 1, true>();
+        a = a < c ? a : c;
+        b = b < d ? b : d;
+    } else {
+        a = staged_occupancy<double, 0, false>();
+        b = staged_occupancy<double, 1, false>();
+    }
     const int occ = a < b ? a : b;
     if (occ < 1) {
         h->stream_nb = -1;
@@ -586,13 +596,13 @@ sup_status sup_stream_plan(sup_ctx* h, const CsrD& M, int64_t r0, int64_t r1, bo
     SUP_CUDA(h, cudaGetLastError());
     // Lanes per row: the rows a warp holds at once (32/G of them) should total ~a tile -- enough elements per lane to
     // amortise the per-row work, few enough that the consumer warps' rows together leave ring stages free for prefetch --
-    // and must never span more than RG_STAGES - 1 tiles.  sup_set_row_mode() overrides the choice.
+    // and must never span more than RG_STAGES_MIN - 1 tiles.  sup_set_row_mode() overrides the choice.
     const double avg = double(ends[1] - ends[0]) / double(r1 - r0);
     int G = 4;
     while (G < 32 && avg * (32.0 / G) > 960.0) G <<= 1;
     const int forced = forward ? h->lanes_fwd : h->lanes_bwd;
     if (forced >= 0) G = forced;
-    const int64_t cap = int64_t(RG_STAGES - 2) * RG_TILE;
+    const int64_t cap = int64_t(RG_STAGES_MIN - 2) * RG_TILE;
     while (G < 32 && G > 0 && int64_t(mx_h) * (32 / G) > cap) G <<= 1;
     if (G != 0 && (avg > 2048.0 || int64_t(mx_h) * (G >= 32 ? 1 : 32 / G) > cap)) G = 0;  // long rows: the whole CTA per row, no length limit
     out->max_row = int64_t(mx_h);
@@ -604,33 +614,42 @@ sup_status sup_stream_plan(sup_ctx* h, const CsrD& M, int64_t r0, int64_t r1, bo
 }
 
 // ---- launchers --------------------------------------------------------------------------------------------------------
-template <typename T, int MODE, int G>
+template <typename T, int MODE, int G, bool DEEP>
 static void launch_staged_g(sup_ctx* h, const StreamPlan& sp, const CsrD& M, const void* vec, const void* p1, const void* p2,
                             const void* p3, void* out, void* out2, double lambda, const GMap& omap) {
-    const void* fn = reinterpret_cast<const void*>(&k_staged<T, MODE, G, RG_NCW>);
-    constexpr int smem = int(sizeof(RgSmem<T, rg_stages<T, MODE>()>));
+    using Sh = RgShape<T, MODE, DEEP>;
+    const void* fn = reinterpret_cast<const void*>(&k_staged<T, MODE, G, Sh::NCW, Sh::STG>);
+    constexpr int smem = int(sizeof(RgSmem<T, Sh::STG>));
     if (!h->smem_opted_in.count(fn)) {  // per handle, hence per device: opt in to > 48 KB of dynamic shared memory
         cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         h->smem_opted_in.insert(fn);
     }
-    k_staged<T, MODE, G, RG_NCW><<<sp.nb, 32 * (RG_NCW + RG_NPROD), smem, h->stream>>>(
+    k_staged<T, MODE, G, Sh::NCW, Sh::STG><<<sp.nb, 32 * (Sh::NCW + RG_NPROD), smem, h->stream>>>(
         sp.part, M.rowptr, M.col, static_cast<const T*>(M.val), static_cast<const uint2*>(M.pk), static_cast<const T*>(vec),
         static_cast<const T*>(p1), static_cast<const T*>(p2), static_cast<const T*>(p3), static_cast<T*>(out),
         static_cast<T*>(out2), T(lambda), M.alloc_nnz, omap);
     h->launches++;
 }
 
+// deep: the gathered vector (x for MODE 0, y for MODE 1) is kept in a tiled layout
+template <typename T, int MODE, bool DEEP>
+static void launch_staged_d(sup_ctx* h, const StreamPlan& sp, const CsrD& M, const void* vec, const void* p1, const void* p2,
+                            const void* p3, void* out, void* out2, double lambda, const GMap& omap) {
+    switch (sp.G) {
+        case 4: launch_staged_g<T, MODE, 4, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap); break;
+        case 8: launch_staged_g<T, MODE, 8, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap); break;
+        case 16: launch_staged_g<T, MODE, 16, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap); break;
+        case 64: launch_staged_g<T, MODE, 64, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap); break;
+        case 0: launch_staged_g<T, MODE, 0, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap); break;
+        default: launch_staged_g<T, MODE, 32, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap); break;
+    }
+}
+
 template <typename T, int MODE>
 static void launch_staged(sup_ctx* h, const StreamPlan& sp, const CsrD& M, const void* vec, const void* p1, const void* p2,
-                          const void* p3, void* out, void* out2, double lambda, const GMap& omap) {
-    switch (sp.G) {
-        case 4: launch_staged_g<T, MODE, 4>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap); break;
-        case 8: launch_staged_g<T, MODE, 8>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap); break;
-        case 16: launch_staged_g<T, MODE, 16>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap); break;
-        case 64: launch_staged_g<T, MODE, 64>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap); break;
-        case 0: launch_staged_g<T, MODE, 0>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap); break;
-        default: launch_staged_g<T, MODE, 32>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap); break;
-    }
+                          const void* p3, void* out, void* out2, double lambda, const GMap& omap, bool deep) {
+    if (deep && sizeof(T) == 4) launch_staged_d<T, MODE, true>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap);
+    else launch_staged_d<T, MODE, false>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap);
 }
 
 // ---- gather layouts: the mirror of x and the internal layout of y (GMap, sup_internal.cuh) ------------------------------
@@ -730,13 +749,13 @@ void sup_launch_stream_fwd(sup_ctx* h, const StreamPlan& sp, const void* x, cons
         if (h->colg) M.col = h->colg;  // fp32: the mapped column is inside M.pk
         vec = h->xg;
     }
-    if (h->dt == SUP_F32) launch_staged<float, 0>(h, sp, M, vec, h->lb, h->ub, dscale, h->y, nullptr, 0.0, h->ymap);
-    else launch_staged<double, 0>(h, sp, M, vec, h->lb, h->ub, dscale, h->y, nullptr, 0.0, h->ymap);
+    if (h->dt == SUP_F32) launch_staged<float, 0>(h, sp, M, vec, h->lb, h->ub, dscale, h->y, nullptr, 0.0, h->ymap, vec == h->xg && h->xmap.kind == 2);
+    else launch_staged<double, 0>(h, sp, M, vec, h->lb, h->ub, dscale, h->y, nullptr, 0.0, h->ymap, false);
 }
 
 void sup_launch_stream_bwd(sup_ctx* h, const CsrD& AT, const StreamPlan& sp, void* x, double lambda) {
     void* mirror = sup_stream_forward_uses_xg(h) ? h->xg : nullptr;
-    if (h->dt == SUP_F32) launch_staged<float, 1>(h, sp, AT, h->y, h->lo, h->hi, nullptr, x, mirror, lambda, h->xmap);
-    else launch_staged<double, 1>(h, sp, AT, h->y, h->lo, h->hi, nullptr, x, mirror, lambda, h->xmap);
+    if (h->dt == SUP_F32) launch_staged<float, 1>(h, sp, AT, h->y, h->lo, h->hi, nullptr, x, mirror, lambda, h->xmap, h->ymap.kind == 2);
+    else launch_staged<double, 1>(h, sp, AT, h->y, h->lo, h->hi, nullptr, x, mirror, lambda, h->xmap, false);
     h->xg_synced = mirror != nullptr;
 }

@@ -781,3 +781,52 @@ def test_layout_hint_with_blocks_and_fallback_kernels():
             assert torch.equal(x.cpu(), ref), mode
     with pytest.raises(sup.SupError):
         sup.sup_set_layout(H, (5, 7), None)
+
+
+# ------------------------------------------------------------------------------------------------------------
+# the CUDA-graph replay is the direct launch sequence, bit for bit (so the strict step-wise bars cover it)
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,block", [("cfg1", False), ("cfg2", False), ("cfg5_k16", False), ("cfg4_small", False), ("blocks", True)])
+def test_graph_replay_equals_direct_launches(name, block):
+    sup = _sup()
+    if block:
+        P = gen.interleaved_angle_blocks(gen.config1_tiny_ct(n_pix=48, n_angles=64, n_bins=69, n_sweeps=30, N=3), 16)
+    else:
+        P = problem(name)
+    H = make_handle(P, 0)
+    outs = []
+    for use_graph in (True, False):
+        x = xdev(P, 0)
+        dec = torch.zeros(1 << 16, dtype=torch.int8, device="cuda:0")
+        sup.sup_superiorize(H, x, 12, P.N, P.beta0, P.a, objective=P.objective, shape=P.shape, lam=P.lam, block=block,
+                            decisions=dec, use_graph=use_graph)
+        st = sup.sup_get_state(H)
+        outs.append((x.cpu(), st["ell"], dec[: st["n_decisions"]].cpu()))
+    assert torch.equal(outs[0][0], outs[1][0]) and outs[0][1] == outs[1][1] and torch.equal(outs[0][2], outs[1][2])
+
+
+def test_unaligned_all_empty_row_ranges():
+    """Runs of empty rows that start at an element offset which is not a multiple of 4: a persistent CTA may own nothing but
+    empty rows and must then stream nothing (round-1 advice: a bulk copy was left in flight)."""
+    sup = _sup()
+    rng = np.random.default_rng(17)
+    m, n = 40000, 64
+    counts = np.zeros(m, np.int64)
+    counts[:5] = [3, 2, 1, 3, 2]            # 11 entries, then thousands of empty rows: every later range is all-empty, offset 11
+    counts[m - 3:] = [5, 1, 7]
+    rowptr = np.zeros(m + 1, np.int64)
+    np.cumsum(counts, out=rowptr[1:])
+    col = np.concatenate([np.sort(rng.choice(n, c, replace=False)) for c in counts if c]).astype(np.int32)
+    val = rng.uniform(0.5, 1.5, col.size).astype(np.float32)
+    lb = rng.uniform(-1, 0, m).astype(np.float32)
+    ub = (lb + 0.5).astype(np.float32)
+    lo, hi = np.full(n, -2.0, np.float32), np.full(n, 2.0, np.float32)
+    x0 = rng.normal(size=n).astype(np.float32)
+    O = Oracle(m, n, rowptr, col, val, lb, ub, lo, hi)
+    for dtype in (0, 1):
+        H = sup.sup_create(rowptr, col, val, lb, ub, lo, hi, None, dtype=dtype, n=n)
+        for lanes in ((-1, -1), (0, 0), (4, 4)):
+            sup.sup_set_row_mode(H, *lanes)
+            x = torch.tensor(x0, dtype=TD[dtype], device="cuda:0")
+            sup.sup_project_simultaneous(H, x, 1.0, 6)
+            assert rel_l2(x.cpu().numpy(), O.sweep(x0, 1.0, 6)) <= SWEEP_TOL[dtype], (dtype, lanes)
