@@ -101,7 +101,26 @@ typedef struct {
     int use_graph;         /* 1: capture one sweep into a CUDA graph and replay it (default path of bench.py) */
     int64_t n_restart;     /* > 0: restarted perturbations: at the start of sweep k = r * n_restart,
                               r = 1, 2, ..., the exponent l is reset to r (PER_TRIAL policy; A-24).  0: off */
+    int algorithm;         /* sup_algorithm: the feasibility-seeking operator T of Eq. 10.  SUP_ALG_DEFAULT: the simultaneous
+                              sweep, or the block-iterative one when block_iterative = 1 */
+    int stop_enabled;      /* 1: the paper's default termination (A-25) is tested after
+                              every sweep but the last: with P^k = Eq. 12 (p = 2) and f^k = f(x^k) at the iterate after sweep k-1,
+                              stop iff (P^k <= prox_tol  or  |P^k - P^(k-1)| / max(1, P^(k-1)) < dprox_tol for n_consec
+                              consecutive sweeps)  and, when an objective is perturbed,  |f^k - f^(k-1)| / max(1, f^(k-1)) < dobj_tol.
+                              n_iter is the paper's N_max.  After a stop the remaining sweeps are skipped on the device (x stays
+                              the iterate the rule was met at); sup_get_state reports n_done and stop_reason */
+    double prox_tol;       /* paper's default 1e-6 */
+    double dprox_tol;      /* paper's default 1e-8 */
+    int n_consec;          /* paper's default 5 */
+    double dobj_tol;       /* paper's default 1e-6 */
 } sup_options;
+
+/* feasibility-seeking operators (PAPER.md Table A.5) */
+typedef enum {
+    SUP_ALG_DEFAULT = 0, /* simultaneous projection x - lambda A^T D c(x) (A-1), or block-iterative (A-14) */
+    SUP_ALG_DROP = 2,    /* x - lambda Z A^T M c(x), M = diag(w_i), Z = diag(1/nnz(A_:,j))  (L602, L608; A-26) */
+    SUP_ALG_EMR = 3      /* x - (||p||^2 / ||M^(1/2) A p||^2) p,  p = A^T M c(x)             (L605; A-26); lambda is not used */
+} sup_algorithm;
 
 /* final state of a run, read back by sup_get_state (host struct) */
 typedef struct {
@@ -112,6 +131,9 @@ typedef struct {
     int32_t warn;        /* bit 0: a reduction step hit J_max = 10000 trials and was skipped (A-12) */
     int32_t fault;       /* bit 0: device-side barrier timed out; bit 1: non-finite objective */
     double f;            /* objective value carried by the last perturbation phase */
+    int64_t n_done;      /* sweeps actually performed by the last sup_superiorize call (< n_iter iff the stopping rule fired) */
+    int32_t stop_reason; /* 0: ran all sweeps; else 1 * (P <= prox_tol) + 2 * (n_consec small changes) + 4 * (objective change small) */
+    double step;         /* EMR: the last relaxation factor ||p||^2 / ||M^(1/2) A p||^2 */
 } sup_state;
 
 /* Bytes of workspace for `kind` on a matrix of the given shape (for SUP_WS_BLOCKS pass A's shape; for SUP_WS_DOSE
@@ -166,17 +188,30 @@ sup_status sup_project_simultaneous(sup_handle h, void* x, double lambda, int n_
 sup_status sup_forward_violation(sup_handle h, const void* x);
 sup_status sup_backproject_update(sup_handle h, void* x, double lambda);
 
+/* n_sweeps DROP sweeps (Table A.5): x <- P_box(x - lambda Z A^T M c(x)); for equality rows lb = ub = b the
+ * residual c(x) is A x - b, the table's formula (A-26). */
+sup_status sup_project_drop(sup_handle h, void* x, double lambda, int n_sweeps);
+
+/* n_sweeps EMR sweeps (Table A.5): x <- P_box(x - t p), p = A^T M c(x), t = ||p||^2 / ||M^(1/2) A p||^2 --
+ * three matrix passes per sweep (A, A^T, A) with the two norms reduced inside the product kernels.  Needs the staged kernels. */
+sup_status sup_project_emr(sup_handle h, void* x, int n_sweeps);
+
 /* n_sweeps block-iterative sweeps (O-BLOCK-SWEEP), in place. */
 sup_status sup_block_iterative(sup_handle h, void* x, double lambda, int n_sweeps);
 
 /* One perturbation phase (Alg. 1 lines 4-17) with the TV objective, step policy PER_TRIAL:
- * N accepted reduction steps from x, in place.  dims = 1 (shape[0] = n) or 2 (shape = {ny, nx}); shape is a HOST
+ * N accepted reduction steps from x, in place.  dims = 1 (shape[0] = n), 2 (shape = {ny, nx}) or 3 (shape = {nz, ny, nx}); shape is a HOST
  * array.  *ell (HOST) is read as the starting exponent and overwritten with the final one.  Synchronises. */
 sup_status sup_perturb_tv(sup_handle h, void* x, int dims, const int64_t* shape, int N, double beta0, double a,
                           int64_t* ell);
 
 /* Same with the dose objective ||D_body x||^2 (needs sup_set_dose_matrix). */
 sup_status sup_perturb_dose(sup_handle h, void* x, int N, double beta0, double a, int64_t* ell);
+
+/* Same with the mean objective f_Mean = (1/N_S) sum_{i in S} (D_S x)_i (Eq. 21), D_S being the matrix given
+ * to sup_set_dose_matrix.  The objective is linear, its gradient (1/N_S) D_S^T 1 is formed once at sup_set_dose_matrix, and
+ * every first trial is accepted: the phase is N axpy steps. */
+sup_status sup_perturb_mean(sup_handle h, void* x, int N, double beta0, double a, int64_t* ell);
 
 /* Algorithm 1, Eq. 10 (L91): for k = k0 .. k0+n_iter-1: perturbation phase of N reduction steps
  * (beta = beta0 * a^l), then one sweep.  x in place.  N = 0 or objective NONE gives the basic algorithm.

@@ -16,6 +16,9 @@ from .binding import (  # noqa: F401
     sup_get_state,
     sup_objective,
     sup_perturb_dose,
+    sup_perturb_mean,
+    sup_project_drop,
+    sup_project_emr,
     sup_perturb_tv,
     sup_project_simultaneous,
     sup_proximity,

@@ -33,12 +33,13 @@ class _Options(Structure):
     _fields_ = [("objective", c_int), ("shape", c_int64 * 3), ("lambda_", c_double), ("block_iterative", c_int),
                 ("step_policy", c_int), ("ell0", c_int64), ("k0", c_int64), ("trace_mode", c_int), ("trace", c_void_p),
                 ("decisions", c_void_p), ("decision_f", c_void_p), ("decisions_cap", c_int64), ("use_graph", c_int),
-                ("n_restart", c_int64)]
+                ("n_restart", c_int64), ("algorithm", c_int), ("stop_enabled", c_int), ("prox_tol", c_double),
+                ("dprox_tol", c_double), ("n_consec", c_int), ("dobj_tol", c_double)]
 
 
 class _State(Structure):
     _fields_ = [("ell", c_int64), ("k", c_int64), ("n_trials", c_int64), ("n_decisions", c_int64), ("warn", c_int32),
-                ("fault", c_int32), ("f", c_double)]
+                ("fault", c_int32), ("f", c_double), ("n_done", c_int64), ("stop_reason", c_int32), ("step", c_double)]
 
 
 def lib():
@@ -67,6 +68,9 @@ def lib():
         L.sup_backproject_update.argtypes = [c_void_p, c_void_p, c_double]
         L.sup_perturb_tv.argtypes = [c_void_p, c_void_p, c_int, POINTER(c_int64), c_int, c_double, c_double, POINTER(c_int64)]
         L.sup_perturb_dose.argtypes = [c_void_p, c_void_p, c_int, c_double, c_double, POINTER(c_int64)]
+        L.sup_perturb_mean.argtypes = [c_void_p, c_void_p, c_int, c_double, c_double, POINTER(c_int64)]
+        L.sup_project_drop.argtypes = [c_void_p, c_void_p, c_double, c_int]
+        L.sup_project_emr.argtypes = [c_void_p, c_void_p, c_int]
         L.sup_superiorize.argtypes = [c_void_p, c_void_p, c_int, c_int, c_double, c_double, POINTER(_Options)]
         L.sup_superiorize_host.argtypes = [c_void_p, c_void_p, c_int, c_int, c_double, c_double, POINTER(_Options)]
         L.sup_get_state.argtypes = [c_void_p, POINTER(_State)]
@@ -77,7 +81,7 @@ def lib():
         L.sup_set_layout.argtypes = [c_void_p, POINTER(c_int64), POINTER(c_int64)]
         for f in ("sup_workspace_bytes", "sup_create", "sup_destroy", "sup_set_blocks", "sup_set_dose_matrix",
                   "sup_project_simultaneous", "sup_block_iterative", "sup_forward_violation", "sup_backproject_update", "sup_perturb_tv", "sup_perturb_dose", "sup_superiorize",
-                  "sup_superiorize_host", "sup_get_state", "sup_proximity", "sup_objective", "sup_get_derived", "sup_set_row_mode", "sup_set_layout"):
+                  "sup_superiorize_host", "sup_get_state", "sup_proximity", "sup_objective", "sup_get_derived", "sup_set_row_mode", "sup_set_layout", "sup_perturb_mean", "sup_project_drop", "sup_project_emr"):
             getattr(L, f).restype = c_int
         _lib = L
     return _lib
@@ -247,6 +251,20 @@ def sup_backproject_update(H: SupHandle, x: torch.Tensor, lam=1.0, sync_streams=
         H._exit()
 
 
+def sup_project_drop(H: SupHandle, x: torch.Tensor, lam=1.0, n_sweeps=1):
+    H._enter()
+    H._check(lib().sup_project_drop(H.h, _ptr(x), lam, n_sweeps))
+    H._exit()
+    return x
+
+
+def sup_project_emr(H: SupHandle, x: torch.Tensor, n_sweeps=1):
+    H._enter()
+    H._check(lib().sup_project_emr(H.h, _ptr(x), n_sweeps))
+    H._exit()
+    return x
+
+
 def sup_block_iterative(H: SupHandle, x: torch.Tensor, lam=1.0, n_sweeps=1):
     H._enter()
     H._check(lib().sup_block_iterative(H.h, _ptr(x), lam, n_sweeps))
@@ -272,7 +290,20 @@ def sup_perturb_dose(H: SupHandle, x: torch.Tensor, N, beta0, a, ell=0):
     return e.value
 
 
-def _options(H, objective, shape, lam, block, policy, ell0, k0, trace, decisions, decision_f, use_graph, n_restart=0):
+ALG_DEFAULT, ALG_DROP, ALG_EMR = 0, 2, 3
+_ALG = {None: ALG_DEFAULT, "sim": ALG_DEFAULT, "block": ALG_DEFAULT, "drop": ALG_DROP, "emr": ALG_EMR}
+
+
+def sup_perturb_mean(H: SupHandle, x: torch.Tensor, N, beta0, a, ell=0):
+    e = c_int64(int(ell))
+    H._enter()
+    H._check(lib().sup_perturb_mean(H.h, _ptr(x), N, beta0, a, byref(e)))
+    H._exit()
+    return e.value
+
+
+def _options(H, objective, shape, lam, block, policy, ell0, k0, trace, decisions, decision_f, use_graph, n_restart=0, algorithm=None,
+             stop=None):
     o = _Options()
     o.objective = _OBJ[objective] if not isinstance(objective, int) else objective
     if shape is not None and o.objective == OBJ_TV2D:
@@ -290,14 +321,20 @@ def _options(H, objective, shape, lam, block, policy, ell0, k0, trace, decisions
     o.decisions_cap = int(decisions.numel()) if decisions is not None else (int(decision_f.shape[0]) if decision_f is not None else 0)
     o.use_graph = int(bool(use_graph))
     o.n_restart = int(n_restart)
+    o.algorithm = _ALG[algorithm] if not isinstance(algorithm, int) else algorithm
+    if stop is not None:  # dict(prox_tol, dprox_tol, n_consec, dobj_tol): the paper's defaults where a key is missing
+        o.stop_enabled = 1
+        o.prox_tol, o.dprox_tol = float(stop.get("prox_tol", 1e-6)), float(stop.get("dprox_tol", 1e-8))
+        o.n_consec, o.dobj_tol = int(stop.get("n_consec", 5)), float(stop.get("dobj_tol", 1e-6))
     return o
 
 
 def sup_superiorize(H: SupHandle, x: torch.Tensor, n_iter, N, beta0, a, objective=None, shape=None, lam=1.0, block=False,
-                    policy=PER_TRIAL, ell0=0, k0=0, trace=None, decisions=None, decision_f=None, use_graph=True, n_restart=0):
+                    policy=PER_TRIAL, ell0=0, k0=0, trace=None, decisions=None, decision_f=None, use_graph=True, n_restart=0,
+                    algorithm=None, stop=None):
     """Algorithm 1 on device tensor x (in place, asynchronous).  trace: float64 [n_iter,4] device tensor or None;
     decisions: int8 [cap] device tensor or None; decision_f: float64 [cap,2] device tensor or None."""
-    o = _options(H, objective, shape, lam, block, policy, ell0, k0, trace, decisions, decision_f, use_graph, n_restart)
+    o = _options(H, objective, shape, lam, block, policy, ell0, k0, trace, decisions, decision_f, use_graph, n_restart, algorithm, stop)
     H._enter()
     H._check(lib().sup_superiorize(H.h, _ptr(x), n_iter, N, beta0, a, byref(o)))
     H._exit()
@@ -318,7 +355,8 @@ def sup_superiorize_host(H: SupHandle, x_host: torch.Tensor, n_iter, N, beta0, a
 def sup_get_state(H: SupHandle) -> dict:
     s = _State()
     H._check(lib().sup_get_state(H.h, byref(s)))
-    return dict(ell=s.ell, k=s.k, n_trials=s.n_trials, n_decisions=s.n_decisions, warn=s.warn, fault=s.fault, f=s.f)
+    return dict(ell=s.ell, k=s.k, n_trials=s.n_trials, n_decisions=s.n_decisions, warn=s.warn, fault=s.fault, f=s.f,
+                n_done=s.n_done, stop_reason=s.stop_reason, step=s.step)
 
 
 def sup_proximity(H: SupHandle, x: torch.Tensor, mode=0, p=2.0) -> float:

@@ -1,0 +1,323 @@
+// sup_algos.cu -- the small kernels around the two product kernels for SURVEY.md 8(f): DROP and EMR (Table A.5,
+// PAPER.md:L602-608), the paper's stopping rule (L217-223, L239-243; reading A-25), the f_Mean perturbation (Eq. 21,
+// L389-393).  Everything that touches a matrix runs in k_staged (sup_stream.cu); what is here works on vectors and scalars.
+#include <math.h>
+
+#include "sup_internal.cuh"
+
+// ---- M = diag(w_i) and Z = diag(1 / nnz(A_:,j)) as arrays of the working type (L608; A-19: M per row, Z per column) --------
+template <typename T>
+__global__ void __launch_bounds__(SUP_THREADS) k_make_wz(const double* __restrict__ w, int64_t m, const int64_t* __restrict__ at_rowptr,
+                                                        int64_t n, T* __restrict__ wT, T* __restrict__ zcol) {
+    const int64_t tid = int64_t(blockIdx.x) * blockDim.x + threadIdx.x, nth = int64_t(gridDim.x) * blockDim.x;
+    for (int64_t i = tid; i < m; i += nth) wT[i] = T(w[i]);
+    for (int64_t j = tid; j < n; j += nth) {
+        const int64_t cnt = at_rowptr[j + 1] - at_rowptr[j];  // stored entries of column j
+        zcol[j] = cnt > 0 ? T(1.0 / double(cnt)) : T(0);
+    }
+}
+
+sup_status sup_setup_wz(sup_ctx* h) {
+    const int grid = sup_grid_for(h->m > h->n ? h->m : h->n, SUP_THREADS, h->num_sms * 8);
+    if (h->dt == SUP_F32)
+        k_make_wz<float><<<grid, SUP_THREADS, 0, h->stream>>>(h->w, h->m, h->AT.rowptr, h->n, static_cast<float*>(h->wT), static_cast<float*>(h->zcol));
+    else
+        k_make_wz<double><<<grid, SUP_THREADS, 0, h->stream>>>(h->w, h->m, h->AT.rowptr, h->n, static_cast<double*>(h->wT), static_cast<double*>(h->zcol));
+    h->launches++;
+    SUP_CUDA(h, cudaGetLastError());
+    return SUP_OK;
+}
+
+// sum of np per-CTA partials in index order, by every thread that needs it (np <= SUP_STREAM_NBMAX; a few hundred loads)
+__device__ __forceinline__ double sum_partials(const double* __restrict__ p, int np) {
+    double s = 0.0;
+    for (int q = 0; q < np; ++q) s += __ldcg(p + q);
+    return s;
+}
+
+// ---- EMR: x <- clip(x - t p), t = ||p||^2 / ||M^(1/2) A p||^2 (L605); p is given in x's gather layout --------------------------
+template <typename T>
+__global__ void __launch_bounds__(SUP_THREADS)
+    k_emr_update(const double* __restrict__ red_pp, int np_pp, const double* __restrict__ red_qq, int np_qq, const T* __restrict__ p_g,
+                 const T* __restrict__ lo, const T* __restrict__ hi, T* __restrict__ x, T* __restrict__ xg, const GMap xmap, int64_t n,
+                 DevState* st) {
+    if (st->stop) return;
+    __shared__ double s_t;
+    if (threadIdx.x == 0) {
+        const double pp = sum_partials(red_pp, np_pp), qq = sum_partials(red_qq, np_qq);
+        s_t = qq > 0.0 ? pp / qq : 0.0;  // a zero denominator (p = 0 or A p = 0) leaves x as it is
+        if (blockIdx.x == 0) st->step = s_t;
+    }
+    __syncthreads();
+    const T t = T(s_t);
+    for (int64_t j = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; j < n; j += int64_t(gridDim.x) * blockDim.x) {
+        const int jg = sup_gmap(xmap, int(j));
+        T v = x[j] - t * p_g[jg];
+        v = v < lo[j] ? lo[j] : v;
+        v = v > hi[j] ? hi[j] : v;
+        x[j] = v;
+        if (xg) xg[jg] = v;
+    }
+}
+
+void sup_launch_emr_update(sup_ctx* h, const double* red_pp, int np_pp, const double* red_qq, int np_qq, const void* p_g, void* x) {
+    const int grid = sup_grid_for(h->n, SUP_THREADS, h->num_sms * 4);
+    void* mirror = sup_stream_forward_uses_xg(h) ? h->xg : nullptr;
+    if (h->dt == SUP_F32)
+        k_emr_update<float><<<grid, SUP_THREADS, 0, h->stream>>>(red_pp, np_pp, red_qq, np_qq, static_cast<const float*>(p_g),
+                                                                 static_cast<const float*>(h->lo), static_cast<const float*>(h->hi),
+                                                                 static_cast<float*>(x), static_cast<float*>(mirror), h->xmap, h->n, h->state);
+    else
+        k_emr_update<double><<<grid, SUP_THREADS, 0, h->stream>>>(red_pp, np_pp, red_qq, np_qq, static_cast<const double*>(p_g),
+                                                                  static_cast<const double*>(h->lo), static_cast<const double*>(h->hi),
+                                                                  static_cast<double*>(x), static_cast<double*>(mirror), h->xmap, h->n, h->state);
+    h->launches++;
+    h->xg_synced = mirror != nullptr;
+}
+
+// ---- end of a sweep: trace row, sweep counters and the stopping rule (A-25) -------------------------------------------------
+// P = Eq. 12 with p = 2 of the iterate just measured: the sum of the forward kernel's per-CTA partials sum c_i y_i (red_prox,
+// np > 0), or twice the Eq. 5 value a k_prox pass left in st->prox_cur (np = 0).  f = st->scalar_out when use_f.
+// mode 0 (after a sweep):   trace[it] = {P/2, f, trials, l}, counters advance, then the rule is applied to (P, f) unless this
+//                           was the last sweep of the run.
+// mode 1 (run start):       (P, f) recorded as P^0, f^0.
+// mode 2 (basic algorithm, BEFORE the back-projection of sweep `it`): P belongs to x^it, the result of sweep it-1:
+//                           it = 0: recorded as P^0; it > 0: trace[it-1][0] = P/2 and the rule is applied (a sweep always
+//                           follows, so this is never the run's last iterate).
+// mode 3 (after a sweep, nothing measured): trace[it][2..3] and the counters only.
+// mode 4 (after the run, basic algorithm with a trace): trace[it-1][0] = P/2 of the final iterate.
+__global__ void k_close_sweep(DevState* st, double* trace, const double* __restrict__ red_prox, int np, int mode, int use_f,
+                              int want_trace, int want_stop, int perturbed, double prox_tol, double dprox_tol, int n_consec,
+                              double dobj_tol) {
+    if (st->stop) return;
+    double P = 0.0, f = 0.0;
+    if (mode != 3) P = np > 0 ? sum_partials(red_prox, np) : 2.0 * st->prox_cur;
+    if (use_f) f = st->scalar_out;
+    bool rule = false;
+    if (mode == 0 || mode == 3) {
+        if (trace && want_trace) {
+            if (mode == 0) {
+                trace[4 * st->it + 0] = 0.5 * P;
+                trace[4 * st->it + 1] = f;
+            }
+            trace[4 * st->it + 2] = double(st->sweep_trials);
+            trace[4 * st->it + 3] = double(st->ell);
+        }
+        st->sweep_trials = 0;
+        st->k += 1;
+        st->it += 1;
+        st->n_done += 1;
+        rule = mode == 0 && want_stop && st->it < st->n_iter;
+    } else if (mode == 1) {
+        st->prox_prev = P;
+        st->f_prev = f;
+        st->consec = 0;
+    } else if (mode == 2) {
+        if (st->it == 0) {
+            st->prox_prev = P;
+            st->f_prev = f;
+            st->consec = 0;
+        } else {
+            if (trace && want_trace) trace[4 * (st->it - 1) + 0] = 0.5 * P;
+            rule = want_stop != 0;
+        }
+    } else if (mode == 4) {
+        if (trace && want_trace && st->it > 0) trace[4 * (st->it - 1) + 0] = 0.5 * P;
+    }
+    if (rule) {
+        const bool c1 = P <= prox_tol;
+        const double dP = fabs(P - st->prox_prev) / fmax(1.0, st->prox_prev);
+        st->consec = dP < dprox_tol ? st->consec + 1 : 0;
+        const bool c2 = st->consec >= n_consec;
+        const double df = fabs(f - st->f_prev) / fmax(1.0, st->f_prev);
+        const bool cf = df < dobj_tol;
+        st->prox_prev = P;
+        st->f_prev = f;
+        if ((c1 || c2) && (!perturbed || cf)) {
+            st->stop = 1;
+            st->stop_reason = int(c1) + 2 * int(c2) + 4 * int(perturbed && cf);
+        }
+    }
+}
+
+void sup_launch_close_sweep(sup_ctx* h, double* trace, const double* red_prox, int np, int mode, int use_f, int perturbed,
+                            const sup_options& o) {
+    k_close_sweep<<<1, 1, 0, h->stream>>>(h->state, trace, red_prox, np, mode, use_f, o.trace_mode && o.trace, o.stop_enabled, perturbed,
+                                          o.prox_tol, o.dprox_tol, o.n_consec, o.dobj_tol);
+    h->launches++;
+}
+
+// ---- f_Mean (Eq. 21): f(x) = <gm, x>, gm = (1/N_S) D_S^T 1 constant ------------------------------------------------------
+// gm_j = (1/N_S) * (sum of the stored entries of column j of D_S) = row j of D_S^T summed; also partial sums of gm_j^2
+template <typename T>
+__global__ void __launch_bounds__(SUP_THREADS) k_mean_gradient(const int64_t* __restrict__ dt_rowptr, const T* __restrict__ dt_val, int64_t n,
+                                                              int64_t md, T* __restrict__ gm, double* __restrict__ partials) {
+    __shared__ double ws[SUP_THREADS];
+    double acc = 0.0;
+    for (int64_t j = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; j < n; j += int64_t(gridDim.x) * blockDim.x) {
+        double s = 0.0;
+        for (int64_t k = dt_rowptr[j]; k < dt_rowptr[j + 1]; ++k) s += double(dt_val[k]);
+        const T g = T(s / double(md));
+        gm[j] = g;
+        acc += double(g) * double(g);
+    }
+    ws[threadIdx.x] = acc;
+    __syncthreads();
+    for (int o = SUP_THREADS / 2; o > 0; o >>= 1) {
+        if (threadIdx.x < o) ws[threadIdx.x] += ws[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) partials[blockIdx.x] = ws[0];
+}
+__global__ void k_mean_norm(const double* __restrict__ partials, int np, double* __restrict__ out) {
+    double s = 0.0;
+    for (int q = 0; q < np; ++q) s += partials[q];
+    *out = s;  // ||gm||^2
+}
+
+sup_status sup_setup_mean_gradient(sup_ctx* h) {
+    const int grid = sup_grid_for(h->n, SUP_THREADS, 256);
+    if (h->dt == SUP_F32)
+        k_mean_gradient<float><<<grid, SUP_THREADS, 0, h->stream>>>(h->DT.rowptr, static_cast<const float*>(h->DT.val), h->n, h->D.rows,
+                                                                    static_cast<float*>(h->gmean), h->partials);
+    else
+        k_mean_gradient<double><<<grid, SUP_THREADS, 0, h->stream>>>(h->DT.rowptr, static_cast<const double*>(h->DT.val), h->n, h->D.rows,
+                                                                     static_cast<double*>(h->gmean), h->partials);
+    k_mean_norm<<<1, 1, 0, h->stream>>>(h->partials, grid, h->gmean_norm2);
+    h->launches += 2;
+    SUP_CUDA(h, cudaGetLastError());
+    return SUP_OK;
+}
+
+// One perturbation phase with the linear objective: along v = -gm/||gm|| every trial gives f(z) = f(x) - beta ||gm|| <= f(x), so
+// each of the N reduction steps accepts its first trial (the oracle evaluates f(z) by a matrix pass; SURVEY.md 8(d) allows
+// the closed form here).  Every thread applies the N steps to its own elements, x <- round_T(x - c_n gm) one after the other
+// as the oracle does, and contributes to <gm, x> of the result.
+template <typename T>
+__global__ void __launch_bounds__(SUP_THREADS)
+    k_mean_steps(T* __restrict__ x, T* __restrict__ xg, const GMap xmap, const T* __restrict__ gm, int64_t n, int N, double beta0, double a,
+                 int policy, long long n_restart, const double* __restrict__ norm2, const DevState* __restrict__ st, double* __restrict__ partials) {
+    if (st->stop) return;
+    __shared__ double ws[SUP_THREADS];
+    long long ell = st->ell;
+    double apow = st->apow;
+    const long long k = st->k;
+    if (n_restart > 0 && k > 0 && k % n_restart == 0) {
+        ell = k / n_restart;
+        apow = 1.0;
+        for (long long q = 0; q < ell; ++q) apow *= a;
+    }
+    const double s = sqrt(*norm2);
+    double acc = 0.0;
+    for (int64_t j = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; j < n; j += int64_t(gridDim.x) * blockDim.x) {
+        double xv = double(x[j]);
+        const double g = double(gm[j]);
+        double ap = apow;
+        for (int nred = 0; nred < N; ++nred) {
+            if (policy != SUP_STEP_PER_TRIAL) {  // PER_SWEEP: beta_{k,0} = beta0 a^k at every reduction step
+                ap = 1.0;
+                for (long long q = 0; q < k; ++q) ap *= a;
+            }
+            const double c = s > 0.0 ? (beta0 * ap) / s : 0.0;
+            if (c != 0.0) xv = double(T(fma(-c, g, xv)));
+            ap *= a;
+        }
+        x[j] = T(xv);
+        if (xg) xg[sup_gmap(xmap, int(j))] = T(xv);
+        acc += g * xv;
+    }
+    ws[threadIdx.x] = acc;
+    __syncthreads();
+    for (int o = SUP_THREADS / 2; o > 0; o >>= 1) {
+        if (threadIdx.x < o) ws[threadIdx.x] += ws[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) partials[blockIdx.x] = ws[0];
+}
+__global__ void k_mean_finish(DevState* st, const double* __restrict__ partials, int np, int N, double beta0, double a, int policy,
+                              long long n_restart, const double* __restrict__ norm2, int8_t* decisions, double* decision_f, long long cap) {
+    if (st->stop) return;
+    const long long k = st->k;
+    if (n_restart > 0 && k > 0 && k % n_restart == 0) {
+        st->ell = k / n_restart;
+        st->apow = 1.0;
+        for (long long q = 0; q < st->ell; ++q) st->apow *= a;
+    }
+    double f = 0.0;
+    for (int q = 0; q < np; ++q) f += partials[q];
+    // the N accepted trials, logged with the closed-form values: f(x^{k,n+1}) = f(x^{k,n}) - c_n ||gm||^2
+    const double s2 = *norm2, s = sqrt(s2);
+    auto coef_sum = [&](double* log_from) {  // walks the N step sizes; logs the trials when log_from != NULL
+        double ap = st->apow, total = 0.0, fx = log_from ? *log_from : 0.0;
+        for (int nred = 0; nred < N; ++nred) {
+            if (policy != SUP_STEP_PER_TRIAL) {
+                ap = 1.0;
+                for (long long q = 0; q < k; ++q) ap *= a;
+            }
+            const double c = s > 0.0 ? (beta0 * ap) / s : 0.0;
+            total += c * s2;
+            if (log_from) {
+                const double fz = fx - c * s2;
+                if (decisions && st->n_dec < cap) decisions[st->n_dec] = 1;
+                if (decision_f && st->n_dec < cap) {
+                    decision_f[2 * st->n_dec] = fz;
+                    decision_f[2 * st->n_dec + 1] = fx;
+                }
+                st->n_dec += 1;
+                fx = fz;
+            }
+            ap *= a;
+        }
+        return total;
+    };
+    double f_before = f + coef_sum(nullptr);
+    coef_sum(&f_before);
+    double ap = st->apow;
+    for (int nred = 0; nred < N; ++nred) ap *= a;
+    st->apow = ap;
+    st->ell += N;
+    st->n_trials += N;
+    st->sweep_trials += N;
+    st->f = f;
+    if (!isfinite(f)) atomicOr(&st->fault, 2);
+}
+
+sup_status sup_launch_perturb_mean(sup_ctx* h, void* x, const PerturbParams& pp) {
+    const int grid = sup_grid_for(h->n, SUP_THREADS, 256);
+    void* mirror = pp.write_mirror && sup_stream_forward_uses_xg(h) ? h->xg : nullptr;
+    if (h->dt == SUP_F32)
+        k_mean_steps<float><<<grid, SUP_THREADS, 0, h->stream>>>(static_cast<float*>(x), static_cast<float*>(mirror), h->xmap,
+                                                                 static_cast<const float*>(h->gmean), h->n, pp.N, pp.beta0, pp.a, pp.policy,
+                                                                 pp.n_restart, h->gmean_norm2, h->state, h->partials);
+    else
+        k_mean_steps<double><<<grid, SUP_THREADS, 0, h->stream>>>(static_cast<double*>(x), static_cast<double*>(mirror), h->xmap,
+                                                                  static_cast<const double*>(h->gmean), h->n, pp.N, pp.beta0, pp.a, pp.policy,
+                                                                  pp.n_restart, h->gmean_norm2, h->state, h->partials);
+    k_mean_finish<<<1, 1, 0, h->stream>>>(h->state, h->partials, grid, pp.N, pp.beta0, pp.a, pp.policy, pp.n_restart, h->gmean_norm2,
+                                          pp.decisions, pp.decision_f, pp.cap);
+    h->launches += 2;
+    SUP_CUDA(h, cudaGetLastError());
+    return SUP_OK;
+}
+
+// stand-alone value f_Mean(x) = <gm, x>
+template <typename T>
+__global__ void __launch_bounds__(SUP_THREADS) k_mean_value(const T* __restrict__ x, const T* __restrict__ gm, int64_t n, double* __restrict__ partials) {
+    __shared__ double ws[SUP_THREADS];
+    double acc = 0.0;
+    for (int64_t j = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; j < n; j += int64_t(gridDim.x) * blockDim.x) acc += double(gm[j]) * double(x[j]);
+    ws[threadIdx.x] = acc;
+    __syncthreads();
+    for (int o = SUP_THREADS / 2; o > 0; o >>= 1) {
+        if (threadIdx.x < o) ws[threadIdx.x] += ws[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) partials[blockIdx.x] = ws[0];
+}
+int sup_launch_mean_value(sup_ctx* h, const void* x) {  // leaves per-CTA partials in h->partials, returns their count
+    const int grid = sup_grid_for(h->n, SUP_THREADS, 256);
+    if (h->dt == SUP_F32) k_mean_value<float><<<grid, SUP_THREADS, 0, h->stream>>>(static_cast<const float*>(x), static_cast<const float*>(h->gmean), h->n, h->partials);
+    else k_mean_value<double><<<grid, SUP_THREADS, 0, h->stream>>>(static_cast<const double*>(x), static_cast<const double*>(h->gmean), h->n, h->partials);
+    h->launches++;
+    return grid;
+}

@@ -32,6 +32,8 @@ extern "C" sup_status sup_workspace_bytes(int kind, int64_t m, int64_t n, int64_
                 + al(2 * SUP_MAX_PARTIALS * 8) + al(sizeof(DevState)) + 2 * sup_stream_table_bytes()
                 + (dtype == SUP_F32 ? 2 * al(size_t(nnz) * 8) : al(size_t(nnz) * 4))               // packed A, A^T (fp32) | colg (fp64)
                 + al(size_t((n + 511) & ~int64_t(511)) * esz)                                      // xg
+                + al(size_t(m) * esz) + al(size_t(n) * esz)                                        // wT, zcol (DROP / EMR)
+                + al(3 * size_t(SUP_STREAM_NBMAX) * 8)                                             // reduction partials of the product kernels
                 + 1024;
             s = sup_transpose_scratch_bytes(nnz, n, esz) + 4096;
             break;
@@ -42,7 +44,9 @@ extern "C" sup_status sup_workspace_bytes(int kind, int64_t m, int64_t n, int64_
             s = sup_transpose_scratch_bytes(nnz, n, esz) + al(size_t(n_blocks) * 8) + 4096;
             break;
         case SUP_WS_DOSE:  // (m, n, nnz) describe D_body
-            p = al(size_t(n + 1) * 8) + al(size_t(nnz) * 4) + al(size_t(nnz) * esz) + 2 * al(size_t(m) * esz) + 1024;
+            p = al(size_t(n + 1) * 8) + al(size_t(nnz) * 4) + al(size_t(nnz) * esz) + 2 * al(size_t(m) * esz)
+                + al(size_t(n) * esz) + 256                                                        // gradient of f_Mean and its norm
+                + 1024;
             s = sup_transpose_scratch_bytes(nnz, n, esz) + 4096;
             break;
         default:
@@ -143,6 +147,9 @@ extern "C" sup_status sup_create(sup_handle* out, const sup_csr* A, const void* 
         h->colg = static_cast<int32_t*>(B.take(size_t(h->nnz) * 4));
     }
     h->xg = B.take(size_t((h->n + 511) & ~int64_t(511)) * h->esz);
+    h->wT = B.take(size_t(h->m) * h->esz);
+    h->zcol = B.take(size_t(h->n) * h->esz);
+    h->red = static_cast<double*>(B.take(3 * size_t(SUP_STREAM_NBMAX) * 8));
     h->A.alloc_nnz = h->nnz;
     sup_status rc = SUP_OK;
     if (!B.ok) rc = sup_fail(h, SUP_ERR_WORKSPACE, "sup_create: workspace too small");
@@ -173,6 +180,7 @@ extern "C" sup_status sup_create(sup_handle* out, const sup_csr* A, const void* 
         rc = sup_fail(h, SUP_ERR_CUDA, "sup_create: %s", cudaGetErrorString(cudaGetLastError()));
     if (rc == SUP_OK) rc = sup_stream_plan(h, h->AT, 0, h->n, false, tab_at, scratch, &h->AT.plan);
     if (rc == SUP_OK) rc = sup_stream_refresh_layout(h);
+    if (rc == SUP_OK) rc = sup_setup_wz(h);
     if (rc == SUP_OK && cudaStreamSynchronize(h->stream) != cudaSuccess)
         rc = sup_fail(h, SUP_ERR_CUDA, "sup_create: %s", cudaGetErrorString(cudaGetLastError()));
     if (rc != SUP_OK) {
@@ -287,6 +295,8 @@ extern "C" sup_status sup_set_dose_matrix(sup_handle h, const sup_csr* D, void* 
     void* val = B.take(size_t(D->nnz) * h->esz);
     h->r_dose = B.take(size_t(D->m) * h->esz);
     h->q_dose = B.take(size_t(D->m) * h->esz);
+    h->gmean = B.take(size_t(D->n) * h->esz);
+    h->gmean_norm2 = static_cast<double*>(B.take(256));
     if (!B.ok) return sup_fail(h, SUP_ERR_WORKSPACE, "sup_set_dose_matrix: workspace too small");
     rc = sup_transpose_rows(h, Dm, 0, D->m, 0, D->nnz, rp, col, val, 0, scratch, scratch_bytes);
     if (rc != SUP_OK) return rc;
@@ -301,6 +311,9 @@ extern "C" sup_status sup_set_dose_matrix(sup_handle h, const sup_csr* D, void* 
     h->g_d = sup_pick_group(D->nnz, D->m);
     h->g_dt = sup_pick_group(D->nnz, D->n);
     h->has_dose = true;
+    rc = sup_setup_mean_gradient(h);  // (1/N_S) D^T 1 for f_Mean (Eq. 21), should the matrix be used as a structure's D_S
+    if (rc != SUP_OK) return rc;
+    SUP_CUDA(h, cudaStreamSynchronize(h->stream));
     return SUP_OK;
 }
 
@@ -372,6 +385,19 @@ static void enqueue_block_sweep(sup_ctx* h, void* x, double lambda) {
     }
 }
 
+static void enqueue_drop(sup_ctx* h, void* x, double lambda) {  // Table A.5: x - lambda Z A^T M c(x)
+    sup_launch_fwd(h, x, 0, h->m, h->wT, &h->A.plan);
+    sup_launch_bwd(h, h->AT, h->g_bwd, x, lambda, h->zcol);
+}
+static bool emr_available(const sup_ctx* h) { return h->A.plan.ok && h->AT.plan.ok && (h->colg || h->A.pk) && h->xg; }
+static void enqueue_emr(sup_ctx* h, void* x) {  // Table A.5: three matrix passes and one vector update
+    double *red_pp = h->red + SUP_STREAM_NBMAX, *red_qq = h->red + 2 * SUP_STREAM_NBMAX;
+    sup_launch_fwd(h, x, 0, h->m, h->wT, &h->A.plan);                   // y = M c(x)
+    sup_launch_stream_plain_AT(h, h->g2, 1.0, red_pp);                 // p = A^T y (in x's gather layout), sum p^2
+    sup_launch_stream_plain_A(h, h->g2, h->y, 1.0, h->wT, red_qq);     // q = A p (over y, no longer needed), sum w q^2
+    sup_launch_emr_update(h, red_pp, h->AT.plan.nb, red_qq, h->A.plan.nb, h->g2, x);
+}
+
 static sup_status check_lambda(sup_ctx* h, double lambda) {
     if (!(lambda >= 0.0 && lambda <= 2.0)) return sup_fail(h, SUP_ERR_INVALID_ARG, "lambda must be in [0,2] (PAPER.md:L44)");
     return SUP_OK;
@@ -404,6 +430,28 @@ extern "C" sup_status sup_backproject_update(sup_handle h, void* x, double lambd
     if (!x) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_backproject_update: NULL x");
     if (check_lambda(h, lambda) != SUP_OK) return SUP_ERR_INVALID_ARG;
     sup_launch_bwd(h, h->AT, h->g_bwd, x, lambda);
+    SUP_CUDA(h, cudaGetLastError());
+    return SUP_OK;
+}
+
+extern "C" sup_status sup_project_drop(sup_handle h, void* x, double lambda, int n_sweeps) {
+    if (!h) return SUP_ERR_INVALID_ARG;
+    SUP_ENTER(h);
+    if (!x || n_sweeps < 0) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_project_drop: NULL x or n_sweeps < 0");
+    if (check_lambda(h, lambda) != SUP_OK) return SUP_ERR_INVALID_ARG;
+    h->xg_synced = false;
+    for (int s = 0; s < n_sweeps; ++s) enqueue_drop(h, x, lambda);
+    SUP_CUDA(h, cudaGetLastError());
+    return SUP_OK;
+}
+
+extern "C" sup_status sup_project_emr(sup_handle h, void* x, int n_sweeps) {
+    if (!h) return SUP_ERR_INVALID_ARG;
+    SUP_ENTER(h);
+    if (!x || n_sweeps < 0) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_project_emr: NULL x or n_sweeps < 0");
+    if (!emr_available(h)) return sup_fail(h, SUP_ERR_STATE, "sup_project_emr needs the staged product kernels (sup_set_row_mode)");
+    h->xg_synced = false;
+    for (int s = 0; s < n_sweeps; ++s) enqueue_emr(h, x);
     SUP_CUDA(h, cudaGetLastError());
     return SUP_OK;
 }
@@ -466,6 +514,9 @@ static sup_status read_state(sup_ctx* h, sup_state* out) {
     out->warn = s.warn;
     out->fault = s.fault;
     out->f = s.f;
+    out->n_done = s.n_done;
+    out->stop_reason = s.stop_reason;
+    out->step = s.step;
     return SUP_OK;
 }
 
@@ -514,6 +565,12 @@ extern "C" sup_status sup_perturb_dose(sup_handle h, void* x, int N, double beta
     return perturb_alone(h, x, SUP_OBJ_DOSE, nullptr, N, beta0, a, ell);
 }
 
+extern "C" sup_status sup_perturb_mean(sup_handle h, void* x, int N, double beta0, double a, int64_t* ell) {
+    if (!h) return SUP_ERR_INVALID_ARG;
+    SUP_ENTER(h);
+    return perturb_alone(h, x, SUP_OBJ_MEAN, nullptr, N, beta0, a, ell);
+}
+
 // ---- Algorithm 1 -----------------------------------------------------------------------------------------------
 struct RunPlan {
     void* x;
@@ -523,24 +580,56 @@ struct RunPlan {
     int64_t dims[3];  // {nz, ny, nx} of the objective
 };
 
+static bool run_perturbed(const RunPlan& P) { return P.N > 0 && P.o.objective != SUP_OBJ_NONE; }
+// the basic simultaneous sweep gets the proximity of its iterate for free from the forward product's epilogue
+static bool run_free_prox(const sup_ctx* h, const RunPlan& P) {
+    return !run_perturbed(P) && P.o.algorithm == SUP_ALG_DEFAULT && !P.o.block_iterative && h->A.plan.ok &&
+           ((P.o.trace_mode && P.o.trace) || P.o.stop_enabled);
+}
+
+// f(x) into state->scalar_out
+static void enqueue_objective(sup_ctx* h, const RunPlan& P) {
+    double* slot = reinterpret_cast<double*>(reinterpret_cast<char*>(h->state) + offsetof(DevState, scalar_out));
+    sup_launch_objective(h, P.x, P.o.objective, P.dims[0], P.dims[1], P.dims[2], slot);
+}
+
+// (P, f) of the current x for the trace / the stopping rule: one forward pass whose epilogue reduces sum c_i y_i (Eq. 12,
+// p = 2) -- or the plain proximity kernel when the staged kernels are off -- and the objective value; then the closing kernel
+static void enqueue_measure_and_close(sup_ctx* h, const RunPlan& P, int mode) {
+    int np = 0;
+    if (h->A.plan.ok) {
+        sup_launch_fwd(h, P.x, 0, h->m, h->d, &h->A.plan, h->red);
+        np = h->A.plan.nb;
+    } else {
+        double* slot = reinterpret_cast<double*>(reinterpret_cast<char*>(h->state) + offsetof(DevState, prox_cur));
+        sup_launch_proximity(h, P.x, 0, 2.0, slot);
+    }
+    enqueue_objective(h, P);
+    sup_launch_close_sweep(h, P.o.trace, h->red, np, mode, 1, run_perturbed(P), P.o);
+}
+
 static sup_status enqueue_superiorized_sweep(sup_ctx* h, const RunPlan& P) {
-    if (P.N > 0 && P.o.objective != SUP_OBJ_NONE) {
+    if (run_perturbed(P)) {
         PerturbParams pp = {P.o.objective, P.dims[0], P.dims[1], P.dims[2], P.N, P.beta0, P.a, P.o.step_policy, P.o.decisions,
                             P.o.decision_f, P.o.decisions_cap, P.o.n_restart, true};
         sup_status rc = sup_launch_perturb(h, P.x, pp);
         if (rc != SUP_OK) return rc;
         h->xg_synced = sup_stream_forward_uses_xg(h);  // the perturbation kernel wrote the moved x to the gather mirror too
     }
-    if (P.o.block_iterative) enqueue_block_sweep(h, P.x, P.o.lambda);
-    else enqueue_simultaneous(h, P.x, P.o.lambda);
-    if (P.o.trace_mode && P.o.trace) {
-        double* slot = reinterpret_cast<double*>(reinterpret_cast<char*>(h->state) + offsetof(DevState, scalar_out));
-        sup_launch_proximity(h, P.x, 0, 2.0, slot);
-        sup_launch_trace_slot(h, P.o.trace, 0);
-        sup_launch_objective(h, P.x, P.o.objective, P.dims[0], P.dims[1], P.dims[2], slot);
-        sup_launch_trace_slot(h, P.o.trace, 1);
+    const bool measure = (P.o.trace_mode && P.o.trace) || P.o.stop_enabled;
+    if (run_free_prox(h, P)) {
+        sup_launch_fwd(h, P.x, 0, h->m, h->d, &h->A.plan, h->red);
+        sup_launch_close_sweep(h, P.o.trace, h->red, h->A.plan.nb, 2, 0, 0, P.o);  // P(x^k): trace row k-1, rule, or P^0
+        sup_launch_bwd(h, h->AT, h->g_bwd, P.x, P.o.lambda);
+        sup_launch_close_sweep(h, P.o.trace, nullptr, 0, 3, 0, 0, P.o);
+        return SUP_OK;
     }
-    sup_launch_end_sweep(h, P.o.trace);
+    if (P.o.algorithm == SUP_ALG_DROP) enqueue_drop(h, P.x, P.o.lambda);
+    else if (P.o.algorithm == SUP_ALG_EMR) enqueue_emr(h, P.x);
+    else if (P.o.block_iterative) enqueue_block_sweep(h, P.x, P.o.lambda);
+    else enqueue_simultaneous(h, P.x, P.o.lambda);
+    if (measure) enqueue_measure_and_close(h, P, 0);
+    else sup_launch_close_sweep(h, P.o.trace, nullptr, 0, 3, 0, 0, P.o);
     return SUP_OK;
 }
 
@@ -552,6 +641,15 @@ static sup_status run_superiorize(sup_ctx* h, void* x, int n_iter, int N, double
     if (opt->block_iterative && h->n_blocks < 1) return sup_fail(h, SUP_ERR_STATE, "sup_superiorize: call sup_set_blocks first");
     if ((opt->decisions || opt->decision_f) && opt->decisions_cap < 0) return sup_fail(h, SUP_ERR_INVALID_ARG, "decisions_cap < 0");
     if (opt->n_restart < 0) return sup_fail(h, SUP_ERR_INVALID_ARG, "n_restart < 0");
+    if (opt->ell0 < 0 || opt->ell0 > 10000000) return sup_fail(h, SUP_ERR_INVALID_ARG, "ell0 must be in [0, 1e7] (a^l is formed by l multiplications, A-20)");
+    if (opt->algorithm != SUP_ALG_DEFAULT && opt->algorithm != SUP_ALG_DROP && opt->algorithm != SUP_ALG_EMR)
+        return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_superiorize: unknown algorithm");
+    if (opt->algorithm != SUP_ALG_DEFAULT && opt->block_iterative)
+        return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_superiorize: DROP / EMR are simultaneous operators (block_iterative must be 0)");
+    if (opt->algorithm == SUP_ALG_EMR && !emr_available(h))
+        return sup_fail(h, SUP_ERR_STATE, "EMR needs the staged product kernels (sup_set_row_mode)");
+    if (opt->stop_enabled && (opt->n_consec < 1 || !(opt->dprox_tol >= 0.0) || !(opt->dobj_tol >= 0.0)))
+        return sup_fail(h, SUP_ERR_INVALID_ARG, "stopping rule: n_consec >= 1 and non-negative thresholds are needed");
     RunPlan P;
     P.x = x;
     P.N = N;
@@ -560,8 +658,14 @@ static sup_status run_superiorize(sup_ctx* h, void* x, int n_iter, int N, double
     P.o = *opt;
     sup_status rc = check_objective(h, opt->objective, opt->shape, P.dims);
     if (rc != SUP_OK) return rc;
-    sup_launch_begin_run(h, opt->ell0, opt->k0, a);
+    sup_launch_begin_run(h, opt->ell0, opt->k0, a, n_iter);
     h->xg_synced = false;
+    h->stop_ptr = opt->stop_enabled ? &h->state->stop : nullptr;
+    struct StopPtrReset {
+        sup_ctx* h;
+        ~StopPtrReset() { h->stop_ptr = nullptr; }
+    } stop_ptr_reset{h};
+    if (opt->stop_enabled && n_iter > 0 && !run_free_prox(h, P)) enqueue_measure_and_close(h, P, 1);  // P^0, f^0
 
     bool graph = opt->use_graph && h->stream != nullptr && !h->graph_failed && n_iter > 1;
     if (graph) {
@@ -583,6 +687,12 @@ static sup_status run_superiorize(sup_ctx* h, void* x, int n_iter, int N, double
         key.decf = opt->decision_f;
         key.cap = opt->decisions_cap;
         key.n_restart = opt->n_restart;
+        key.algorithm = opt->algorithm;
+        key.stop = opt->stop_enabled;
+        key.tols[0] = opt->prox_tol;
+        key.tols[1] = opt->dprox_tol;
+        key.tols[2] = opt->dobj_tol;
+        key.n_consec = opt->n_consec;
         if (!h->gexec || !(key == h->gkey)) {
             drop_graph(h);
             const int64_t launches_before = h->launches;
@@ -620,6 +730,10 @@ static sup_status run_superiorize(sup_ctx* h, void* x, int n_iter, int N, double
             rc = enqueue_superiorized_sweep(h, P);
             if (rc != SUP_OK) return rc;
         }
+    }
+    if (n_iter > 0 && run_free_prox(h, P) && P.o.trace_mode && P.o.trace) {  // proximity of the final iterate for the last trace row
+        sup_launch_fwd(h, P.x, 0, h->m, h->d, &h->A.plan, h->red);
+        sup_launch_close_sweep(h, P.o.trace, h->red, h->A.plan.nb, 4, 0, 0, P.o);
     }
     SUP_CUDA(h, cudaGetLastError());
     return SUP_OK;

@@ -50,6 +50,16 @@ struct DevState {
     double f;             // objective carried by the last perturbation phase
     double apow;          // a^l as the running fp64 product (PER_TRIAL; A-20)
     double scalar_out;    // result slot of finalize kernels (proximity / objective)
+    // the paper's stopping rule (A-25) and what the feasibility-seeking kernels leave for the next kernel
+    double prox_prev, f_prev;  // P^(k-1), f^(k-1)
+    double prox_cur, f_cur;    // P^k, f^k of the sweep being closed
+    double step;          // EMR: ||p||^2 / ||M^(1/2) A p||^2 of the current sweep
+    double cf;            // dose perturbation: coefficient of the accepted step (0: none)
+    long long n_done;     // sweeps performed by this run
+    long long n_iter;     // sweeps asked of this run (the rule is not applied after the last one)
+    int consec;           // consecutive sweeps with a small relative proximity change
+    int stop;             // 1: the rule fired -- every later kernel of the run returns at once
+    int stop_reason;
     // grid barrier of the perturbation kernel: the arrival counter, the generation flag every waiting CTA polls and the
     // published totals each sit in a 128-byte line of their own, so the pollers do not slow the arrivals down
     alignas(128) unsigned bar_count;
@@ -137,6 +147,10 @@ struct sup_ctx {
     void* pk_a = nullptr;       // [nnz] x 8 B, fp32 handles: (val, sup_swz(col)) of A
     void* pk_at = nullptr;      // [nnz] x 8 B, fp32 handles: (val, row) of A^T
     void* pk_atb = nullptr;     // [nnz] x 8 B, fp32 handles: the per-block transposes (sup_set_blocks)
+    void* wT = nullptr;         // [m] dtype: the normalised weights w_i (M of DROP / EMR)
+    void* zcol = nullptr;       // [n] dtype: 1 / nnz(A_:,j), 0 for an empty column (Z of DROP)
+    const int* stop_ptr = nullptr;  // &state->stop while a run with the stopping rule is being enqueued, else NULL
+    double* red = nullptr;      // [3][SUP_STREAM_NBMAX] per-CTA partials of the product kernels' reductions
     void* xg = nullptr;         // [n rounded up to 512] dtype: xg[sup_gmap(xmap, j)] = x[j]
     GMap xmap, ymap;            // maps in force: x mirror read by the staged forward product; internal y (identity unless every
                                 // product runs on the staged fp32 kernels, which read y through the packed A^T)
@@ -159,6 +173,8 @@ struct sup_ctx {
     CsrD D, DT;
     void* r_dose = nullptr;     // [md] dtype
     void* q_dose = nullptr;     // [md] dtype: D g
+    void* gmean = nullptr;      // [n] dtype: (1/N_S) D_S^T 1, the constant gradient of f_Mean (Eq. 21)
+    double* gmean_norm2 = nullptr;  // device scalar ||gmean||^2
     int g_d = 8, g_dt = 32;
     // cached graph of one superiorized sweep
     cudaGraphExec_t gexec = nullptr;
@@ -169,6 +185,8 @@ struct sup_ctx {
         const void* x = nullptr;
         int N = 0, objective = 0, block = 0, policy = 0, trace_mode = 0;
         int64_t n_restart = 0;
+        int algorithm = 0, stop = 0, n_consec = 0;
+        double tols[3] = {0, 0, 0};
         double beta0 = 0, a = 0, lambda = 0;
         int64_t s0 = 0, s1 = 0, s2 = 0;
         const void *trace = nullptr, *dec = nullptr, *decf = nullptr;
@@ -176,7 +194,8 @@ struct sup_ctx {
         bool operator==(const GraphKey& o) const {
             return x == o.x && N == o.N && objective == o.objective && block == o.block && policy == o.policy &&
                    trace_mode == o.trace_mode && beta0 == o.beta0 && a == o.a && lambda == o.lambda && s0 == o.s0 &&
-                   s1 == o.s1 && s2 == o.s2 && trace == o.trace && dec == o.dec && decf == o.decf && cap == o.cap && n_restart == o.n_restart;
+                   s1 == o.s1 && s2 == o.s2 && algorithm == o.algorithm && stop == o.stop && n_consec == o.n_consec &&
+                   tols[0] == o.tols[0] && tols[1] == o.tols[1] && tols[2] == o.tols[2] && trace == o.trace && dec == o.dec && decf == o.decf && cap == o.cap && n_restart == o.n_restart;
         }
     } gkey;
     int64_t launches = 0;
@@ -219,8 +238,9 @@ sup_status sup_setup_block_scaling(sup_ctx* h, void* scratch, size_t scratch_byt
 sup_status sup_validate(sup_ctx* h, const CsrD& A, bool check_bounds, void* scratch);
 
 // ---- products (sup_spmv.cu) -------------------------------------------------------------------------------
-void sup_launch_fwd(sup_ctx* h, const void* x, int64_t r0, int64_t r1, const void* dscale, const StreamPlan* rp);
-void sup_launch_bwd(sup_ctx* h, const CsrD& AT, int G, void* x, double lambda);
+// red_out (forward): per-CTA partials of sum c_i y_i, only produced by the staged kernel (NULL otherwise)
+void sup_launch_fwd(sup_ctx* h, const void* x, int64_t r0, int64_t r1, const void* dscale, const StreamPlan* rp, double* red_out = nullptr);
+void sup_launch_bwd(sup_ctx* h, const CsrD& AT, int G, void* x, double lambda, const void* zscale = nullptr);
 void sup_launch_proximity(sup_ctx* h, const void* x, int mode, double p, double* out_dev);
 
 // ---- bulk-copy-staged products (sup_stream.cu) ---------------------------------------------------------------
@@ -229,8 +249,12 @@ size_t sup_stream_table_bytes();  // bytes of one partition table (256-aligned)
 // persistent workspace), lanes per row; `forward` only selects which tuning overrides apply; synchronises the stream.  `scratch` needs 256 bytes.
 sup_status sup_stream_plan(sup_ctx* h, const CsrD& M, int64_t r0, int64_t r1, bool forward, void* table, void* scratch,
                            StreamPlan* out);
-void sup_launch_stream_fwd(sup_ctx* h, const StreamPlan& rp, const void* x, const void* dscale);
-void sup_launch_stream_bwd(sup_ctx* h, const CsrD& AT, const StreamPlan& rp, void* x, double lambda);
+void sup_launch_staged(sup_ctx* h, int mode, const StreamPlan& sp, const CsrD& M, const void* vec, const void* p1, const void* p2,
+                       const void* p3, void* out, void* out2, double lambda, const GMap& omap, bool deep, double* red_out);
+void sup_launch_stream_fwd(sup_ctx* h, const StreamPlan& rp, const void* x, const void* dscale, double* red_out);
+void sup_launch_stream_bwd(sup_ctx* h, const CsrD& AT, const StreamPlan& rp, void* x, double lambda, const void* zscale);
+void sup_launch_stream_plain_A(sup_ctx* h, const void* v_g, void* out, double scale, const void* wrow, double* red_out);
+void sup_launch_stream_plain_AT(sup_ctx* h, void* out_g, double scale, double* red_out);
 sup_status sup_stream_setup_gather(sup_ctx* h);  // fills colg (fp64) or the packed copy of A (fp32) from A.col / A.val through xmap
 // fp32 handles: dst[k] = (val[k], sup_gmap(map, col[k])) for k in [0, nnz)
 sup_status sup_stream_pack(sup_ctx* h, const void* val, const int32_t* col, int64_t nnz, void* dst, const GMap& map);
@@ -254,7 +278,16 @@ struct PerturbParams {
 };
 sup_status sup_launch_perturb(sup_ctx* h, void* x, const PerturbParams& pp);
 void sup_launch_objective(sup_ctx* h, const void* x, int kind, int64_t nz, int64_t ny, int64_t nx, double* out_dev);
-void sup_launch_end_sweep(sup_ctx* h, double* trace);
-void sup_launch_trace_slot(sup_ctx* h, double* trace, int slot);  // trace[it][slot] = state->scalar_out
-void sup_launch_begin_run(sup_ctx* h, int64_t ell0, int64_t k0, double a);
+void sup_launch_begin_run(sup_ctx* h, int64_t ell0, int64_t k0, double a, int64_t n_iter = 0);
 int sup_perturb_grid(sup_ctx* h, int objective);
+
+// ---- DROP / EMR, stopping rule, f_Mean (sup_algos.cu) ---------------------------------------------------------------
+sup_status sup_setup_wz(sup_ctx* h);
+void sup_launch_emr_update(sup_ctx* h, const double* red_pp, int np_pp, const double* red_qq, int np_qq, const void* p_g, void* x);
+// mode: 0 after a sweep with (P, f) measured, 1 run start, 2 before the back-projection (basic algorithm), 3 after a sweep with
+// nothing measured, 4 after the run (see k_close_sweep); np = 0: P from st->prox_cur
+void sup_launch_close_sweep(sup_ctx* h, double* trace, const double* red_prox, int np, int mode, int use_f, int perturbed,
+                            const sup_options& o);
+sup_status sup_setup_mean_gradient(sup_ctx* h);
+sup_status sup_launch_perturb_mean(sup_ctx* h, void* x, const PerturbParams& pp);
+int sup_launch_mean_value(sup_ctx* h, const void* x);

@@ -403,149 +403,225 @@ __device__ __forceinline__ double objective_share(const PArgs<T>& A, double coef
     return 0.0;
 }
 
-// ---- gradient passes: z = round_T(x - c g) (c = 0: x itself) is formed on the fly; the pass writes z to xo (when c != 0)
-// and grad f(z) to go, and returns this thread's shares F of f(z) (a tile computes every term t_p anyway) and S of
-// sum (grad f(z))^2.  A term with t = 0 contributes 0 to the gradient (A-9).
-// TV2D (A-8): g_ij = -(dx_ij+dy_ij)/t_ij [i<ny-1, j<nx-1] + dx_{i-1,j}/t_{i-1,j} [i>=1, j<nx-1] + dy_{i,j-1}/t_{i,j-1} [j>=1, i<ny-1].
-// One CTA stages a TILE_H x TILE_W tile plus a one-pixel halo in shared memory.
+// ---- TV passes over tiles: B candidate coefficients at once; z_b = round_T(x - c_b g) (c_b = 0: x itself) is formed on the fly
+// from the tile's x and g.  Returns this thread's share F[b] of f(z_b) for every candidate and, when GRAD (B = 1), writes z
+// to xo (if c != 0) and grad f(z) to go and returns the share S of sum (grad f(z))^2 (a term with t = 0 contributes 0, A-9).
+// The value-only pass and the gradient pass assign pixels to threads and add terms in the SAME order, so f of a given z
+// is the same bit pattern whichever pass computed it -- an accept test f(z) <= f(x) with z == x (a step below the storage
+// type's resolution) must see equality.
+__device__ __forceinline__ double tv_d2(double dx, double dy) { return fma(dx, dx, dy * dy); }
+__device__ __forceinline__ double tv_d3(double dz, double dy, double dx) { return fma(dx, dx, fma(dy, dy, dz * dz)); }
 template <typename T>
-__device__ void tv2d_gz(const PArgs<T>& A, double pend, T* __restrict__ xo, T* __restrict__ go, double& F, double& S) {
-    __shared__ double tile[TILE_H + 2][TILE_W + 2 + 1];
+__device__ __forceinline__ double zform(double xv, double gv, double c) { return c == 0.0 ? xv : double(T(fma(-c, gv, xv))); }
+
+// TV2D (A-8): g_ij = -(dx_ij+dy_ij)/t_ij [i<ny-1, j<nx-1] + dx_{i-1,j}/t_{i-1,j} [i>=1, j<nx-1] + dy_{i,j-1}/t_{i,j-1} [j>=1, i<ny-1].
+// One CTA stages a TILE_H x TILE_W tile of x and of g plus a one-pixel halo in shared memory.
+template <typename T, int B, bool GRAD>
+__device__ void tv2d_pass(const PArgs<T>& A, const double* coef, T* __restrict__ xo, T* __restrict__ go, double* F, double& S, double* sm) {
+    typedef double Tile2[TILE_W + 2 + 1];
+    Tile2* tx = reinterpret_cast<Tile2*>(sm);
+    Tile2* tg = reinterpret_cast<Tile2*>(sm + (TILE_H + 2) * (TILE_W + 2 + 1));
     const int64_t ny = A.ny, nx = A.nx;
     const int64_t tiles_y = (ny + TILE_H - 1) / TILE_H, tiles_x = (nx + TILE_W - 1) / TILE_W;
-    double acc = 0.0, facc = 0.0;
+    bool any = false;
+#pragma unroll
+    for (int b = 0; b < B; ++b) {
+        F[b] = 0.0;
+        any = any || coef[b] != 0.0;
+    }
+    double acc = 0.0;
     for (int64_t t = blockIdx.x; t < tiles_y * tiles_x; t += gridDim.x) {
-        const int64_t ty = t / tiles_x, tx = t - ty * tiles_x;
-        const int64_t i0 = ty * TILE_H - 1, j0 = tx * TILE_W - 1;  // top-left of the halo
+        const int64_t ty = t / tiles_x, txi = t - ty * tiles_x;
+        const int64_t i0 = ty * TILE_H - 1, j0 = txi * TILE_W - 1;  // top-left of the halo
         __syncthreads();
         for (int q = threadIdx.x; q < (TILE_H + 2) * (TILE_W + 2); q += SUP_THREADS) {
             const int li = q / (TILE_W + 2), lj = q - li * (TILE_W + 2);
             const int64_t i = i0 + li, j = j0 + lj;
-            tile[li][lj] = (i >= 0 && i < ny && j >= 0 && j < nx) ? zval(A.x, A.g, pend, i * nx + j) : 0.0;
+            const bool in = i >= 0 && i < ny && j >= 0 && j < nx;
+            const double xv = in ? double(__ldcg(A.x + i * nx + j)) : 0.0;
+            const double gv = in && any ? double(__ldcg(A.g + i * nx + j)) : 0.0;
+            if (B == 1) {
+                tx[li][lj] = zform<T>(xv, gv, coef[0]);  // one candidate: the tile holds z itself
+            } else {
+                tx[li][lj] = xv;
+                tg[li][lj] = gv;
+            }
         }
         __syncthreads();
         for (int q = threadIdx.x; q < TILE_H * TILE_W; q += SUP_THREADS) {
             const int li = q / TILE_W + 1, lj = q % TILE_W + 1;
             const int64_t i = i0 + li, j = j0 + lj;
             if (i >= ny || j >= nx) continue;
-            double gv = 0.0;
-            const double c = tile[li][lj];
-            if (i + 1 < ny && j + 1 < nx) {  // own term (i, j)
-                const double dx = tile[li + 1][lj] - c, dy = tile[li][lj + 1] - c;
-                const double d2 = dx * dx + dy * dy;
-                if (d2 > 0.0) {
-                    const double ri = rsqrt(d2);
-                    gv -= (dx + dy) * ri;
-                    facc += d2 * ri;
+            const bool own = i + 1 < ny && j + 1 < nx;
+#pragma unroll
+            for (int b = 0; b < B; ++b) {
+                const double cb = coef[b];
+                auto Z = [&](int a, int bq) { return B == 1 ? tx[a][bq] : zform<T>(tx[a][bq], tg[a][bq], cb); };
+                const double c = Z(li, lj);
+                double gv = 0.0;
+                if (own) {  // own term (i, j)
+                    const double dx = Z(li + 1, lj) - c, dy = Z(li, lj + 1) - c;
+                    const double d2 = tv_d2(dx, dy);
+                    if (d2 > 0.0) {
+                        const double ri = rsqrt(d2);
+                        gv -= (dx + dy) * ri;
+                        F[b] += d2 * ri;
+                    }
+                }
+                if (GRAD) {
+                    if (i >= 1 && j + 1 < nx) {  // term (i-1, j): dx_{i-1,j} = X_ij - X_{i-1,j}
+                        const double bb = Z(li - 1, lj);
+                        const double dx = c - bb, dy = Z(li - 1, lj + 1) - bb;
+                        const double d2 = tv_d2(dx, dy);
+                        if (d2 > 0.0) gv += dx * rsqrt(d2);
+                    }
+                    if (j >= 1 && i + 1 < ny) {  // term (i, j-1): dy_{i,j-1} = X_ij - X_{i,j-1}
+                        const double bb = Z(li, lj - 1);
+                        const double dx = Z(li + 1, lj - 1) - bb, dy = c - bb;
+                        const double d2 = tv_d2(dx, dy);
+                        if (d2 > 0.0) gv += dy * rsqrt(d2);
+                    }
+                    const T gs = T(gv);
+                    go[i * nx + j] = gs;
+                    if (cb != 0.0) xo[i * nx + j] = T(c);  // c is z rounded to T already
+                    acc += double(gs) * double(gs);
                 }
             }
-            if (i >= 1 && j + 1 < nx) {  // term (i-1, j): dx_{i-1,j} = X_ij - X_{i-1,j}
-                const double b = tile[li - 1][lj];
-                const double dx = c - b, dy = tile[li - 1][lj + 1] - b;
-                const double d2 = dx * dx + dy * dy;
-                if (d2 > 0.0) gv += dx * rsqrt(d2);
-            }
-            if (j >= 1 && i + 1 < ny) {  // term (i, j-1): dy_{i,j-1} = X_ij - X_{i,j-1}
-                const double b = tile[li][lj - 1];
-                const double dx = tile[li + 1][lj - 1] - b, dy = c - b;
-                const double d2 = dx * dx + dy * dy;
-                if (d2 > 0.0) gv += dy * rsqrt(d2);
-            }
-            const T gs = T(gv);
-            go[i * nx + j] = gs;
-            if (pend != 0.0) xo[i * nx + j] = T(c);  // c is z rounded to T already
-            acc += double(gs) * double(gs);
         }
     }
-    F = facc;
     S = acc;
 }
 
 // TV3D (A-27): Eq. 15 with a third difference on an nz x ny x nx volume; a voxel receives +dz/t of term (i-1,j,k), +dy/t of
-// (i,j-1,k), +dx/t of (i,j,k-1) and -(dz+dy+dx)/t of its own term.  Tile of TZ x TY x TX voxels plus a one-voxel halo.
+// (i,j-1,k), +dx/t of (i,j,k-1) and -(dz+dy+dx)/t of its own term.  Tile of TZ3 x TY3 x TX3 voxels plus a one-voxel halo.
 #define TZ3 4
 #define TY3 8
 #define TX3 32
-template <typename T>
-__device__ void tv3d_gz(const PArgs<T>& A, double pend, T* __restrict__ xo, T* __restrict__ go, double& F, double& S) {
-    __shared__ double vol[TZ3 + 2][TY3 + 2][TX3 + 2 + 1];
+template <typename T, int B, bool GRAD>
+__device__ void tv3d_pass(const PArgs<T>& A, const double* coef, T* __restrict__ xo, T* __restrict__ go, double* F, double& S, double* sm) {
+    typedef double Vol3[TY3 + 2][TX3 + 2 + 1];
+    Vol3* vx = reinterpret_cast<Vol3*>(sm);
+    Vol3* vg = reinterpret_cast<Vol3*>(sm + (TZ3 + 2) * (TY3 + 2) * (TX3 + 2 + 1));
     const int64_t nz = A.nz, ny = A.ny, nx = A.nx;
-    const int64_t tz = (nz + TZ3 - 1) / TZ3, ty = (ny + TY3 - 1) / TY3, tx = (nx + TX3 - 1) / TX3;
-    double acc = 0.0, facc = 0.0;
-    for (int64_t t = blockIdx.x; t < tz * ty * tx; t += gridDim.x) {
-        const int64_t bz = t / (ty * tx), rem = t - bz * ty * tx, by = rem / tx, bx = rem - by * tx;
+    const int64_t tz = (nz + TZ3 - 1) / TZ3, ty = (ny + TY3 - 1) / TY3, txn = (nx + TX3 - 1) / TX3;
+    bool any = false;
+#pragma unroll
+    for (int b = 0; b < B; ++b) {
+        F[b] = 0.0;
+        any = any || coef[b] != 0.0;
+    }
+    double acc = 0.0;
+    for (int64_t t = blockIdx.x; t < tz * ty * txn; t += gridDim.x) {
+        const int64_t bz = t / (ty * txn), rem = t - bz * ty * txn, by = rem / txn, bx = rem - by * txn;
         const int64_t i0 = bz * TZ3 - 1, j0 = by * TY3 - 1, k0 = bx * TX3 - 1;
         __syncthreads();
         for (int q = threadIdx.x; q < (TZ3 + 2) * (TY3 + 2) * (TX3 + 2); q += SUP_THREADS) {
             const int li = q / ((TY3 + 2) * (TX3 + 2)), r2 = q - li * (TY3 + 2) * (TX3 + 2), lj = r2 / (TX3 + 2), lk = r2 - lj * (TX3 + 2);
             const int64_t i = i0 + li, j = j0 + lj, k = k0 + lk;
-            vol[li][lj][lk] = (i >= 0 && i < nz && j >= 0 && j < ny && k >= 0 && k < nx) ? zval(A.x, A.g, pend, (i * ny + j) * nx + k) : 0.0;
+            const bool in = i >= 0 && i < nz && j >= 0 && j < ny && k >= 0 && k < nx;
+            const int64_t p = (i * ny + j) * nx + k;
+            const double xv = in ? double(__ldcg(A.x + p)) : 0.0;
+            const double gv = in && any ? double(__ldcg(A.g + p)) : 0.0;
+            if (B == 1) {
+                vx[li][lj][lk] = zform<T>(xv, gv, coef[0]);
+            } else {
+                vx[li][lj][lk] = xv;
+                vg[li][lj][lk] = gv;
+            }
         }
         __syncthreads();
         for (int q = threadIdx.x; q < TZ3 * TY3 * TX3; q += SUP_THREADS) {
             const int li = q / (TY3 * TX3) + 1, r2 = q % (TY3 * TX3), lj = r2 / TX3 + 1, lk = r2 % TX3 + 1;
             const int64_t i = i0 + li, j = j0 + lj, k = k0 + lk;
             if (i >= nz || j >= ny || k >= nx) continue;
-            const double c = vol[li][lj][lk];
-            double gv = 0.0;
-            if (i >= 1 && j + 1 < ny && k + 1 < nx) {  // term (i-1, j, k)
-                const double b = vol[li - 1][lj][lk];
-                const double dz = c - b, dy = vol[li - 1][lj + 1][lk] - b, dx = vol[li - 1][lj][lk + 1] - b;
-                const double d2 = (dz * dz + dy * dy) + dx * dx;
-                if (d2 > 0.0) gv += dz * rsqrt(d2);
-            }
-            if (j >= 1 && i + 1 < nz && k + 1 < nx) {  // term (i, j-1, k)
-                const double b = vol[li][lj - 1][lk];
-                const double dz = vol[li + 1][lj - 1][lk] - b, dy = c - b, dx = vol[li][lj - 1][lk + 1] - b;
-                const double d2 = (dz * dz + dy * dy) + dx * dx;
-                if (d2 > 0.0) gv += dy * rsqrt(d2);
-            }
-            if (k >= 1 && i + 1 < nz && j + 1 < ny) {  // term (i, j, k-1)
-                const double b = vol[li][lj][lk - 1];
-                const double dz = vol[li + 1][lj][lk - 1] - b, dy = vol[li][lj + 1][lk - 1] - b, dx = c - b;
-                const double d2 = (dz * dz + dy * dy) + dx * dx;
-                if (d2 > 0.0) gv += dx * rsqrt(d2);
-            }
-            if (i + 1 < nz && j + 1 < ny && k + 1 < nx) {  // own term
-                const double dz = vol[li + 1][lj][lk] - c, dy = vol[li][lj + 1][lk] - c, dx = vol[li][lj][lk + 1] - c;
-                const double d2 = (dz * dz + dy * dy) + dx * dx;
-                if (d2 > 0.0) {
-                    const double ri = rsqrt(d2);
-                    gv -= ((dz + dy) + dx) * ri;
-                    facc += d2 * ri;
+            const bool own = i + 1 < nz && j + 1 < ny && k + 1 < nx;
+#pragma unroll
+            for (int b = 0; b < B; ++b) {
+                const double cb = coef[b];
+                auto Z = [&](int a, int bq, int cq) { return B == 1 ? vx[a][bq][cq] : zform<T>(vx[a][bq][cq], vg[a][bq][cq], cb); };
+                const double c = Z(li, lj, lk);
+                double gv = 0.0;
+                if (GRAD) {
+                    if (i >= 1 && j + 1 < ny && k + 1 < nx) {  // term (i-1, j, k)
+                        const double bb = Z(li - 1, lj, lk);
+                        const double dz = c - bb, dy = Z(li - 1, lj + 1, lk) - bb, dx = Z(li - 1, lj, lk + 1) - bb;
+                        const double d2 = tv_d3(dz, dy, dx);
+                        if (d2 > 0.0) gv += dz * rsqrt(d2);
+                    }
+                    if (j >= 1 && i + 1 < nz && k + 1 < nx) {  // term (i, j-1, k)
+                        const double bb = Z(li, lj - 1, lk);
+                        const double dz = Z(li + 1, lj - 1, lk) - bb, dy = c - bb, dx = Z(li, lj - 1, lk + 1) - bb;
+                        const double d2 = tv_d3(dz, dy, dx);
+                        if (d2 > 0.0) gv += dy * rsqrt(d2);
+                    }
+                    if (k >= 1 && i + 1 < nz && j + 1 < ny) {  // term (i, j, k-1)
+                        const double bb = Z(li, lj, lk - 1);
+                        const double dz = Z(li + 1, lj, lk - 1) - bb, dy = Z(li, lj + 1, lk - 1) - bb, dx = c - bb;
+                        const double d2 = tv_d3(dz, dy, dx);
+                        if (d2 > 0.0) gv += dx * rsqrt(d2);
+                    }
+                }
+                if (own) {
+                    const double dz = Z(li + 1, lj, lk) - c, dy = Z(li, lj + 1, lk) - c, dx = Z(li, lj, lk + 1) - c;
+                    const double d2 = tv_d3(dz, dy, dx);
+                    if (d2 > 0.0) {
+                        const double ri = rsqrt(d2);
+                        gv -= ((dz + dy) + dx) * ri;
+                        F[b] += d2 * ri;
+                    }
+                }
+                if (GRAD) {
+                    const T gs = T(gv);
+                    const int64_t p = (i * ny + j) * nx + k;
+                    go[p] = gs;
+                    if (cb != 0.0) xo[p] = T(c);
+                    acc += double(gs) * double(gs);
                 }
             }
-            const T gs = T(gv);
-            const int64_t p = (i * ny + j) * nx + k;
-            go[p] = gs;
-            if (pend != 0.0) xo[p] = T(c);
-            acc += double(gs) * double(gs);
         }
     }
-    F = facc;
     S = acc;
 }
 
-template <typename T>
-__device__ void tv1d_gz(const PArgs<T>& A, double pend, T* __restrict__ xo, T* __restrict__ go, double& F, double& S) {
-    double acc = 0.0, facc = 0.0;
-    for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q < A.n; q += int64_t(gridDim.x) * blockDim.x) {
-        const double c = zval(A.x, A.g, pend, q);
-        double gv = 0.0;
-        if (q >= 1) {
-            const double dl = c - zval(A.x, A.g, pend, q - 1);
-            gv += double((dl > 0.0) - (dl < 0.0));
-        }
-        if (q + 1 < A.n) {
-            const double dr = zval(A.x, A.g, pend, q + 1) - c;
-            gv -= double((dr > 0.0) - (dr < 0.0));
-            facc += fabs(dr);
-        }
-        go[q] = T(gv);
-        if (pend != 0.0) xo[q] = T(c);
-        acc += gv * gv;
+// TV1D (A-16), same contract; the value-only pass walks the same elements in the same order
+template <typename T, int B, bool GRAD>
+__device__ void tv1d_pass(const PArgs<T>& A, const double* coef, T* __restrict__ xo, T* __restrict__ go, double* F, double& S, double*) {
+    bool any = false;
+#pragma unroll
+    for (int b = 0; b < B; ++b) {
+        F[b] = 0.0;
+        any = any || coef[b] != 0.0;
     }
-    F = facc;
+    double acc = 0.0;
+    for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q < A.n; q += int64_t(gridDim.x) * blockDim.x) {
+        const double x0 = double(__ldcg(A.x + q)), xl = q >= 1 ? double(__ldcg(A.x + q - 1)) : 0.0, xr = q + 1 < A.n ? double(__ldcg(A.x + q + 1)) : 0.0;
+        double g0 = 0.0, gl = 0.0, gr = 0.0;
+        if (any) {
+            g0 = double(__ldcg(A.g + q));
+            gl = q >= 1 ? double(__ldcg(A.g + q - 1)) : 0.0;
+            gr = q + 1 < A.n ? double(__ldcg(A.g + q + 1)) : 0.0;
+        }
+#pragma unroll
+        for (int b = 0; b < B; ++b) {
+            const double cb = coef[b];
+            const double c = zform<T>(x0, g0, cb);
+            double gv = 0.0;
+            if (GRAD && q >= 1) {
+                const double dl = c - zform<T>(xl, gl, cb);
+                gv += double((dl > 0.0) - (dl < 0.0));
+            }
+            if (q + 1 < A.n) {
+                const double dr = zform<T>(xr, gr, cb) - c;
+                gv -= double((dr > 0.0) - (dr < 0.0));
+                F[b] += fabs(dr);
+            }
+            if (GRAD) {
+                go[q] = T(gv);
+                if (cb != 0.0) xo[q] = T(c);
+                acc += gv * gv;
+            }
+        }
+    }
     S = acc;
 }
 
@@ -575,21 +651,29 @@ __device__ double dose_grad_share(const PArgs<T>& A) {
 // Buffers: (xc, gc) hold the current inner iterate x^{k,n} and its gradient, (xo, go) receive the candidate z and its gradient
 // (a tile's halo needs the neighbours' x and g, so a pass cannot work in place); on acceptance the pairs swap.
 template <typename T, int OBJ>
-__device__ __forceinline__ void tv_gz(const PArgs<T>& V, double c, T* xo, T* go, double& F, double& S) {
-    if (OBJ == SUP_OBJ_TV2D) tv2d_gz(V, c, xo, go, F, S);
-    else if (OBJ == SUP_OBJ_TV3D) tv3d_gz(V, c, xo, go, F, S);
-    else tv1d_gz(V, c, xo, go, F, S);
+__device__ __forceinline__ void tv_gz(const PArgs<T>& V, double c, T* xo, T* go, double& F, double& S, double* sm) {
+    if (OBJ == SUP_OBJ_TV2D) tv2d_pass<T, 1, true>(V, &c, xo, go, &F, S, sm);
+    else if (OBJ == SUP_OBJ_TV3D) tv3d_pass<T, 1, true>(V, &c, xo, go, &F, S, sm);
+    else tv1d_pass<T, 1, true>(V, &c, xo, go, &F, S, sm);
+}
+// doubles of shared memory the tile passes of an objective need (x tile + g tile)
+template <int OBJ>
+__host__ __device__ constexpr int tv_tile_doubles() {
+    return OBJ == SUP_OBJ_TV2D ? 2 * (TILE_H + 2) * (TILE_W + 2 + 1) : (OBJ == SUP_OBJ_TV3D ? 2 * (TZ3 + 2) * (TY3 + 2) * (TX3 + 2 + 1) : 1);
 }
 template <typename T, int OBJ, int B>
-__device__ __forceinline__ void tv_share_batch(const PArgs<T>& V, const double* coef, double* acc) {
-    if (OBJ == SUP_OBJ_TV2D) tv2d_share_batch<T, B>(V, coef, acc);
-    else if (OBJ == SUP_OBJ_TV3D) tv3d_share_batch<T, B>(V, coef, acc);
-    else tv1d_share_batch<T, B>(V, coef, acc);
+__device__ __forceinline__ void tv_share_batch(const PArgs<T>& V, const double* coef, double* acc, double* sm) {
+    double unused;
+    if (OBJ == SUP_OBJ_TV2D) tv2d_pass<T, B, false>(V, coef, nullptr, nullptr, acc, unused, sm);
+    else if (OBJ == SUP_OBJ_TV3D) tv3d_pass<T, B, false>(V, coef, nullptr, nullptr, acc, unused, sm);
+    else tv1d_pass<T, B, false>(V, coef, nullptr, nullptr, acc, unused, sm);
 }
 
 template <typename T, int OBJ>
 __global__ void __launch_bounds__(SUP_THREADS) k_perturb_tv(PArgs<T> Ain) {
     const PArgs<T>& A = Ain;
+    if (*(volatile int*)&Ain.st->stop) return;  // the stopping rule fired earlier in this run: every CTA sees the same flag
+    __shared__ double tile_mem[tv_tile_doubles<OBJ>()];
     T* xc = Ain.x;
     T* gc = Ain.g;
     T* xo = Ain.x2;
@@ -648,7 +732,7 @@ __global__ void __launch_bounds__(SUP_THREADS) k_perturb_tv(PArgs<T> Ain) {
     double fx, s;
     {
         double v[2];
-        tv_gz<T, OBJ>(view(), 0.0, xo, gc, v[0], v[1]);
+        tv_gz<T, OBJ>(view(), 0.0, xo, gc, v[0], v[1], tile_mem);
         ok = grid_reduce<2>(st, P, PSTRIDE, v, gen);
         fx = v[0];
         s = sqrt(v[1]);
@@ -665,7 +749,7 @@ __global__ void __launch_bounds__(SUP_THREADS) k_perturb_tv(PArgs<T> Ain) {
             double c0;
             step_coef(s, jloc, &c0, 1);
             double v[2];
-            tv_gz<T, OBJ>(view(), c0, xo, go, v[0], v[1]);
+            tv_gz<T, OBJ>(view(), c0, xo, go, v[0], v[1], tile_mem);
             ok = grid_reduce<2>(st, P, PSTRIDE, v, gen);
             if (!ok) break;
             const bool acc = v[0] <= fx;  // NaN compares false -> rejected (A-11)
@@ -695,7 +779,7 @@ __global__ void __launch_bounds__(SUP_THREADS) k_perturb_tv(PArgs<T> Ain) {
         while (ok && !accepted && trial < SUP_J_MAX) {
             double coef[B], fzb[B];
             step_coef(s, jloc, coef, B);
-            tv_share_batch<T, OBJ, B>(view(), coef, fzb);
+            tv_share_batch<T, OBJ, B>(view(), coef, fzb, tile_mem);
             ok = grid_reduce<B>(st, P, PSTRIDE, fzb, gen);
             if (!ok) break;
             for (int b = 0; b < B && !accepted && trial < SUP_J_MAX; ++b) {
@@ -718,7 +802,7 @@ __global__ void __launch_bounds__(SUP_THREADS) k_perturb_tv(PArgs<T> Ain) {
                 } else {
                     // the gradient at the accepted z (f(z) again, in this pass's summation order, carried from here on)
                     double v[2];
-                    tv_gz<T, OBJ>(view(), cf, xo, go, v[0], v[1]);
+                    tv_gz<T, OBJ>(view(), cf, xo, go, v[0], v[1], tile_mem);
                     ok = grid_reduce<2>(st, P, PSTRIDE, v, gen);
                     if (!ok) break;
                     fx = v[0];
@@ -761,6 +845,7 @@ template <typename T, int OBJ>
 __global__ void __launch_bounds__(SUP_THREADS) k_perturb(PArgs<T> Ain) {
     static_assert(OBJ == SUP_OBJ_DOSE, "the TV objectives run in k_perturb_tv");
     const PArgs<T>& A = Ain;
+    if (*(volatile int*)&Ain.st->stop) return;
     T* xc = Ain.x;
     T* gc = Ain.g;
     auto view = [&]() { return Ain; };
@@ -891,17 +976,6 @@ __global__ void k_sum_final(const double* __restrict__ partials, int np, double*
     if (threadIdx.x == 0) *out = shm[0];
 }
 
-__global__ void k_end_sweep(DevState* st, double* trace) {
-    if (trace) {
-        trace[4 * st->it + 2] = double(st->sweep_trials);
-        trace[4 * st->it + 3] = double(st->ell);
-    }
-    st->sweep_trials = 0;
-    st->k += 1;
-    st->it += 1;
-}
-__global__ void k_trace_slot(DevState* st, double* trace, int slot) { trace[4 * st->it + slot] = st->scalar_out; }
-
 // ---- host side --------------------------------------------------------------------------------------------------
 template <typename T>
 static PArgs<T> make_args(sup_ctx* h, void* x, const PerturbParams& pp) {
@@ -973,6 +1047,7 @@ int sup_perturb_grid(sup_ctx* h, int objective) {
 }
 
 sup_status sup_launch_perturb(sup_ctx* h, void* x, const PerturbParams& pp) {
+    if (pp.objective == SUP_OBJ_MEAN) return sup_launch_perturb_mean(h, x, pp);
     const int grid = sup_perturb_grid(h, pp.objective);
     if (grid < 1) return sup_fail(h, SUP_ERR_CUDA, "perturbation kernel cannot be made resident");
     cudaLaunchConfig_t cfg = {};
@@ -1020,21 +1095,25 @@ static void launch_objective_t(sup_ctx* h, const void* x, int kind, int64_t nz, 
 }
 
 void sup_launch_objective(sup_ctx* h, const void* x, int kind, int64_t nz, int64_t ny, int64_t nx, double* out_dev) {
+    if (kind == SUP_OBJ_MEAN) {  // f_Mean(x) = <(1/N_S) D_S^T 1, x>
+        const int np = sup_launch_mean_value(h, x);
+        k_sum_final<<<1, SUP_THREADS, 0, h->stream>>>(h->partials, np, out_dev);
+        h->launches++;
+        return;
+    }
     if (h->dt == SUP_F32) launch_objective_t<float>(h, x, kind, nz, ny, nx, out_dev);
     else launch_objective_t<double>(h, x, kind, nz, ny, nx, out_dev);
 }
 
-void sup_launch_end_sweep(sup_ctx* h, double* trace) {
-    k_end_sweep<<<1, 1, 0, h->stream>>>(h->state, trace);
-    h->launches++;
-}
-
-void sup_launch_trace_slot(sup_ctx* h, double* trace, int slot) {
-    k_trace_slot<<<1, 1, 0, h->stream>>>(h->state, trace, slot);
-    h->launches++;
-}
-
-__global__ void k_begin_run(DevState* st, long long ell0, long long k0, double apow0) {
+__global__ void k_begin_run(DevState* st, long long ell0, long long k0, double apow0, long long n_iter) {
+    st->n_iter = n_iter;
+    st->n_done = 0;
+    st->stop = 0;
+    st->stop_reason = 0;
+    st->consec = 0;
+    st->prox_prev = st->f_prev = st->prox_cur = st->f_cur = 0.0;
+    st->step = 0.0;
+    st->cf = 0.0;
     st->ell = ell0;
     st->apow = apow0;
     st->k = k0;
@@ -1046,11 +1125,10 @@ __global__ void k_begin_run(DevState* st, long long ell0, long long k0, double a
     st->fault = 0;
     st->bar_count = 0;
 }
-void sup_launch_begin_run(sup_ctx* h, int64_t ell0, int64_t k0, double a) {
+void sup_launch_begin_run(sup_ctx* h, int64_t ell0, int64_t k0, double a, int64_t n_iter) {
     // a^l0: exactly 1 for a fresh run, so the running product below reproduces the oracle's step sizes bit for bit (A-20)
     double apow0 = 1.0;
-    for (int64_t i = 0; i < ell0 && i < 100000; ++i) apow0 *= a;
-    if (ell0 >= 100000) apow0 = pow(a, double(ell0));
-    k_begin_run<<<1, 1, 0, h->stream>>>(h->state, ell0, k0, apow0);
+    for (int64_t i = 0; i < ell0; ++i) apow0 *= a;  // (ell0 is bounded by the argument check: the product stays exact-by-construction)
+    k_begin_run<<<1, 1, 0, h->stream>>>(h->state, ell0, k0, apow0, n_iter);
     h->launches++;
 }

@@ -46,7 +46,8 @@ template <typename T>
 __global__ void __launch_bounds__(SUP_THREADS)
     k_fwd(int64_t r0, int64_t r1, const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
           const T* __restrict__ val, const T* __restrict__ x, const T* __restrict__ lb, const T* __restrict__ ub,
-          const T* __restrict__ d, T* __restrict__ y, int G) {
+          const T* __restrict__ d, T* __restrict__ y, int G, const int* __restrict__ stop) {
+    if (stop && *stop) return;
     const int gl = threadIdx.x % G;
     const int64_t i = r0 + (int64_t(blockIdx.x) * blockDim.x + threadIdx.x) / G;
     const bool valid = i < r1;
@@ -59,14 +60,15 @@ template <typename T>
 __global__ void __launch_bounds__(SUP_THREADS)
     k_bwd(int64_t n, const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col, const T* __restrict__ val,
           const T* __restrict__ y, const T* __restrict__ lo, const T* __restrict__ hi, T lambda, T* __restrict__ x,
-          T* __restrict__ xg, int G, const GMap xmap) {
+          T* __restrict__ xg, int G, const GMap xmap, const T* __restrict__ zscale, const int* __restrict__ stop) {
+    if (stop && *stop) return;
     const int gl = threadIdx.x % G;
     const int64_t j = (int64_t(blockIdx.x) * blockDim.x + threadIdx.x) / G;
     const bool valid = j < n;
     const int64_t s = valid ? rowptr[j] : 0, e = valid ? rowptr[j + 1] : 0;
     const T u = group_row_dot(val, col, s, e, y, gl, G);
     if (valid && gl == 0) {
-        T t = x[j] - lambda * u;  // Eq. 3
+        T t = x[j] - lambda * ((zscale ? zscale[j] : T(1)) * u);  // Eq. 3 (zscale: DROP's 1/nnz(A_:,j))
         t = t < lo[j] ? lo[j] : t;  // box, un-relaxed (A-2)
         t = t > hi[j] ? hi[j] : t;
         x[j] = t;
@@ -74,12 +76,12 @@ __global__ void __launch_bounds__(SUP_THREADS)
     }
 }
 
-void sup_launch_fwd(sup_ctx* h, const void* x, int64_t r0, int64_t r1, const void* dscale, const StreamPlan* rp) {
+void sup_launch_fwd(sup_ctx* h, const void* x, int64_t r0, int64_t r1, const void* dscale, const StreamPlan* rp, double* red_out) {
     const int G = h->g_fwd;
     const int64_t rows = r1 - r0;
     if (rows <= 0) return;
     if (rp && rp->ok) {
-        sup_launch_stream_fwd(h, *rp, x, dscale);
+        sup_launch_stream_fwd(h, *rp, x, dscale, red_out);
         return;
     }
     const unsigned grid = unsigned((rows * G + SUP_THREADS - 1) / SUP_THREADS);
@@ -87,18 +89,18 @@ void sup_launch_fwd(sup_ctx* h, const void* x, int64_t r0, int64_t r1, const voi
         k_fwd<float><<<grid, SUP_THREADS, 0, h->stream>>>(
             r0, r1, h->A.rowptr, h->A.col, static_cast<const float*>(h->A.val), static_cast<const float*>(x),
             static_cast<const float*>(h->lb), static_cast<const float*>(h->ub), static_cast<const float*>(dscale),
-            static_cast<float*>(h->y), G);
+            static_cast<float*>(h->y), G, h->stop_ptr);
     else
         k_fwd<double><<<grid, SUP_THREADS, 0, h->stream>>>(
             r0, r1, h->A.rowptr, h->A.col, static_cast<const double*>(h->A.val), static_cast<const double*>(x),
             static_cast<const double*>(h->lb), static_cast<const double*>(h->ub), static_cast<const double*>(dscale),
-            static_cast<double*>(h->y), G);
+            static_cast<double*>(h->y), G, h->stop_ptr);
     h->launches++;
 }
 
-void sup_launch_bwd(sup_ctx* h, const CsrD& AT, int G, void* x, double lambda) {
+void sup_launch_bwd(sup_ctx* h, const CsrD& AT, int G, void* x, double lambda, const void* zscale) {
     if (AT.plan.ok) {
-        sup_launch_stream_bwd(h, AT, AT.plan, x, lambda);
+        sup_launch_stream_bwd(h, AT, AT.plan, x, lambda, zscale);
         return;
     }
     const unsigned grid = unsigned((AT.rows * G + SUP_THREADS - 1) / SUP_THREADS);
@@ -108,12 +110,12 @@ void sup_launch_bwd(sup_ctx* h, const CsrD& AT, int G, void* x, double lambda) {
         k_bwd<float><<<grid, SUP_THREADS, 0, h->stream>>>(
             AT.rows, AT.rowptr, AT.col, static_cast<const float*>(AT.val), static_cast<const float*>(h->y),
             static_cast<const float*>(h->lo), static_cast<const float*>(h->hi), float(lambda), static_cast<float*>(x),
-            static_cast<float*>(mirror), G, h->xmap);
+            static_cast<float*>(mirror), G, h->xmap, static_cast<const float*>(zscale), h->stop_ptr);
     else
         k_bwd<double><<<grid, SUP_THREADS, 0, h->stream>>>(
             AT.rows, AT.rowptr, AT.col, static_cast<const double*>(AT.val), static_cast<const double*>(h->y),
             static_cast<const double*>(h->lo), static_cast<const double*>(h->hi), lambda, static_cast<double*>(x),
-            static_cast<double*>(mirror), G, h->xmap);
+            static_cast<double*>(mirror), G, h->xmap, static_cast<const double*>(zscale), h->stop_ptr);
     h->launches++;
 }
 

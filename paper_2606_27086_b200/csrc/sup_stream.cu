@@ -142,6 +142,7 @@ struct RgSmem {
     T pairbuf[RG_CWARPS / 2][2];  // G == 64: partial row sums handed from the odd to the even warp of a pair
     int progress[RG_CWARPS];  // per consumer warp: tiles [0, progress) are no longer needed by it
     int issued[STG];          // per stage: 1 + the tile its barrier is currently armed for (0: none yet)
+    double red[RG_CWARPS];    // per consumer warp: its share of the kernel's reduction
 };
 
 // Dot product of the ring elements k, k+G, k+2G, ... < e (offsets relative to the stream base) with gathered vec
@@ -201,18 +202,66 @@ __device__ __forceinline__ void ring_row_dot(const RgData<T, STG>& ring, const T
     }
 }
 
+// Fused epilogue of one finished row r, run by ONE lane; racc collects the row's term of the kernel's fp64 reduction.
+//   MODE 0  y_r = q3 * c,  c = hyperslab violation of the row value against [q1, q2]  (Eq. 2 per face; q3 = d_r or w_r);
+//           reduction: sum c * y  (= sum w_i c_i^2 / ||a_i||^2 when q3 = d: Eq. 12 with p = 2, twice Eq. 5)
+//   MODE 1  x_r <- clip(x_r - lambda * q4 * u_r, q1, q2)  (Eq. 3, box L427; q4 = 1, or DROP's 1/nnz(A_:,r)); mirror in out2
+//   MODE 2  out_r = lambda * (row value)  (a plain product with a scale);  reduction: sum q3 * out_r^2  (q3 = 1 or a weight)
+template <typename T, int MODE>
+__device__ __forceinline__ void row_epilogue(int64_t r, T acc, T q1, T q2, T q3, T q4, T* out, T* out2, T lambda, const GMap& omap,
+                                             double& racc) {
+    if (MODE == 0) {
+        const T c = hyperslab_violation(acc, q1, q2);
+        const T y = q3 * c;
+        out[sup_gmap(omap, int(r))] = y;  // (in y's gather layout)
+        racc += double(c) * double(y);
+    } else if (MODE == 1) {
+        T t = q3 - lambda * (q4 * acc);  // Eq. 3
+        t = t < q1 ? q1 : t;             // box, un-relaxed (A-2)
+        t = t > q2 ? q2 : t;
+        out[r] = t;
+        if (out2) out2[sup_gmap(omap, int(r))] = t;  // keep the gather mirror of x in step
+    } else {
+        const T v = lambda * acc;
+        out[sup_gmap(omap, int(r))] = v;
+        racc += double(q3) * (double(v) * double(v));
+    }
+}
+template <typename T, int MODE>
+__device__ __forceinline__ void row_operands(int64_t r, const T* p1, const T* p2, const T* p3, const T* out, T& q1, T& q2, T& q3, T& q4) {
+    q4 = T(1);
+    if (MODE == 0) {
+        q1 = p1[r];
+        q2 = p2[r];
+        q3 = p3[r];
+    } else if (MODE == 1) {
+        q1 = p1[r];
+        q2 = p2[r];
+        q3 = out[r];
+        if (p3) q4 = p3[r];
+    } else {
+        q1 = q2 = T(0);
+        q3 = p3 ? p3[r] : T(1);
+    }
+}
+
 // MODE 0: forward (vec = xg, columns swizzled (pk / colg), p1 = lb, p2 = ub, p3 = d, out = y);
 // MODE 1: backward (vec = y, p1 = lo, p2 = hi, out = x in place, out2 = xg mirror or NULL)
 template <typename T, int MODE, int G, int NCW, int STG>
 __global__ void __launch_bounds__(32 * (NCW + RG_NPROD), 1)
     k_staged(const int64_t* __restrict__ part, const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
              const T* __restrict__ val, const uint2* __restrict__ pk, const T* __restrict__ vec, const T* __restrict__ p1,
-             const T* __restrict__ p2, const T* __restrict__ p3, T* out, T* out2, T lambda, int64_t nnz_total, const GMap omap) {
+             const T* __restrict__ p2, const T* __restrict__ p3, T* out, T* out2, T lambda, int64_t nnz_total, const GMap omap, double* __restrict__ red_out,
+             const int* __restrict__ stop) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int RG_ELEMS = STG * RG_TILE;
     RgSmem<T, STG>& S = *reinterpret_cast<RgSmem<T, STG>*>(smem_raw);
+    if (stop && *stop) return;  // the stopping rule fired earlier in this run (A-25): the sweep is skipped
     const int64_t rs = part[blockIdx.x], re = part[blockIdx.x + 1];
-    if (rs >= re) return;
+    if (rs >= re) {
+        if (red_out && threadIdx.x == 0) red_out[blockIdx.x] = 0.0;
+        return;
+    }
     const int64_t es = rowptr[rs], ee = rowptr[re];
     const int64_t base = es & ~int64_t(3);  // 16-byte aligned start of the stream (4 elements)
     // an all-empty range streams nothing (no copy may be left in flight when the CTA exits)
@@ -296,6 +345,7 @@ __global__ void __launch_bounds__(32 * (NCW + RG_NPROD), 1)
         }
         return;
     }
+    double racc = 0.0;  // this lane's share of the kernel's reduction (row_epilogue)
     // ---- consumers, G == 0: LONG rows -- the whole CTA works on one row at a time ----------------------------------------
     // (rows of thousands of nonzeros, e.g. config 4's A^T: one row per warp would put NCW x row bytes in flight, far more
     // than the ring holds).  The row is cut into pieces of 32 NCW x RG_UNROLL elements; every lane takes RG_UNROLL elements
@@ -313,12 +363,8 @@ __global__ void __launch_bounds__(32 * (NCW + RG_NPROD), 1)
                 s_next = e;
                 e_next = int(rowptr[r + 2] - base);
             }
-            T q1 = T(0), q2 = T(0), q3 = T(0);
-            if (gl == 0) {
-                q1 = p1[r];
-                q2 = p2[r];
-                q3 = MODE == 0 ? p3[r] : out[r];
-            }
+            T q1 = T(0), q2 = T(0), q3 = T(0), q4 = T(1);
+            if (gl == 0) row_operands<T, MODE>(r, p1, p2, p3, out, q1, q2, q3, q4);
             T a0 = T(0), a1 = T(0), a2 = T(0), a3 = T(0);
             for (int ps = s; ps < e; ps += CH) {
                 const int pe = e < ps + CH ? e : ps + CH;
@@ -357,22 +403,13 @@ __global__ void __launch_bounds__(32 * (NCW + RG_NPROD), 1)
                 T tot = T(0);
 #pragma unroll
                 for (int w = 0; w < NCW; ++w) tot += S.ctabuf[iter & 1][w];
-                if (MODE == 0) {
-                    out[sup_gmap(omap, int(r))] = q3 * hyperslab_violation(tot, q1, q2);
-                } else {
-                    T t = q3 - lambda * tot;
-                    t = t < q1 ? q1 : t;
-                    t = t > q2 ? q2 : t;
-                    out[r] = t;
-                    if (out2) out2[sup_gmap(omap, int(r))] = t;
-                }
+                row_epilogue<T, MODE>(r, tot, q1, q2, q3, q4, out, out2, lambda, omap, racc);
             }
             s = s_next;
             e = e_next;
         }
         __syncwarp();
         if (lane == 0) progress[warp] = ntiles;
-        return;
     } else {
     // ---- consumers, G >= 4 --------------------------------------------------------------------------------------------------
     // All positions below are element offsets relative to `base` and fit an int (a CTA's range is < 2^31 elements).
@@ -409,12 +446,8 @@ __global__ void __launch_bounds__(32 * (NCW + RG_NPROD), 1)
             rp_s_next = rowptr[rn < re ? rn : re];
             rp_e_next = rowptr[rn + 1 < re ? rn + 1 : re];
         }
-        T q1 = T(0), q2 = T(0), q3 = T(0);
-        if (valid && gl == 0) {  // (in a pair: lane 0 of the even warp)
-            q1 = p1[r];
-            q2 = p2[r];
-            q3 = MODE == 0 ? p3[r] : out[r];
-        }
+        T q1 = T(0), q2 = T(0), q3 = T(0), q4 = T(1);
+        if (valid && gl == 0) row_operands<T, MODE>(r, p1, p2, p3, out, q1, q2, q3, q4);  // (in a pair: lane 0 of the even warp)
         const int w_start = __shfl_sync(0xffffffffu, s, 0), w_end = __shfl_sync(0xffffffffu, e, 31);
         // Release every tile wholly before this warp's position.  Every lane consumed its previous rows' ring data
         // (the values fed the shuffle reduction) before this point, and the warp is converged by the shuffle above.
@@ -463,17 +496,7 @@ __global__ void __launch_bounds__(32 * (NCW + RG_NPROD), 1)
             asm volatile("bar.sync %0, 64;" ::"r"(1 + unit) : "memory");
             if (!(warp & 1) && lane == 0) acc += S.pairbuf[unit][iter & 1];
         }
-        if (valid && gl == 0) {
-            if (MODE == 0) {
-                out[sup_gmap(omap, int(r))] = q3 * hyperslab_violation(acc, q1, q2);  // y_i = d_i c_i (in y's gather layout)
-            } else {
-                T t = q3 - lambda * acc;  // Eq. 3
-                t = t < q1 ? q1 : t;      // box, un-relaxed (A-2)
-                t = t > q2 ? q2 : t;
-                out[r] = t;
-                if (out2) out2[sup_gmap(omap, int(r))] = t;  // keep the gather mirror of x in step
-            }
-        }
+        if (valid && gl == 0 && !(PAIR && (warp & 1))) row_epilogue<T, MODE>(r, acc, q1, q2, q3, q4, out, out2, lambda, omap, racc);
         s = int(rp_s_next - base);
         e = int(rp_e_next - base);
     }
@@ -486,6 +509,19 @@ __global__ void __launch_bounds__(32 * (NCW + RG_NPROD), 1)
     PROF_FLUSH(1);
     PROF_FLUSH(2);
     PROF_FLUSH(5);
+    }
+    // the kernel's reduction: lanes -> warp (fixed shuffle tree) -> CTA (warps in index order) -> red_out[blockIdx.x]
+    if (red_out) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) racc += __shfl_xor_sync(0xffffffffu, racc, o);
+        if (lane == 0) S.red[warp] = racc;
+        asm volatile("bar.sync 15, %0;" ::"n"(32 * NCW) : "memory");
+        if (threadIdx.x == 0) {
+            double t = 0.0;
+#pragma unroll
+            for (int w = 0; w < NCW; ++w) t += S.red[w];
+            red_out[blockIdx.x] = t;
+        }
     }
 }
 
@@ -616,7 +652,7 @@ sup_status sup_stream_plan(sup_ctx* h, const CsrD& M, int64_t r0, int64_t r1, bo
 // ---- launchers --------------------------------------------------------------------------------------------------------
 template <typename T, int MODE, int G, bool DEEP>
 static void launch_staged_g(sup_ctx* h, const StreamPlan& sp, const CsrD& M, const void* vec, const void* p1, const void* p2,
-                            const void* p3, void* out, void* out2, double lambda, const GMap& omap) {
+                            const void* p3, void* out, void* out2, double lambda, const GMap& omap, double* red_out) {
     using Sh = RgShape<T, MODE, DEEP>;
     const void* fn = reinterpret_cast<const void*>(&k_staged<T, MODE, G, Sh::NCW, Sh::STG>);
     constexpr int smem = int(sizeof(RgSmem<T, Sh::STG>));
@@ -627,29 +663,29 @@ static void launch_staged_g(sup_ctx* h, const StreamPlan& sp, const CsrD& M, con
     k_staged<T, MODE, G, Sh::NCW, Sh::STG><<<sp.nb, 32 * (Sh::NCW + RG_NPROD), smem, h->stream>>>(
         sp.part, M.rowptr, M.col, static_cast<const T*>(M.val), static_cast<const uint2*>(M.pk), static_cast<const T*>(vec),
         static_cast<const T*>(p1), static_cast<const T*>(p2), static_cast<const T*>(p3), static_cast<T*>(out),
-        static_cast<T*>(out2), T(lambda), M.alloc_nnz, omap);
+        static_cast<T*>(out2), T(lambda), M.alloc_nnz, omap, red_out, h->stop_ptr);
     h->launches++;
 }
 
 // deep: the gathered vector (x for MODE 0, y for MODE 1) is kept in a tiled layout
 template <typename T, int MODE, bool DEEP>
 static void launch_staged_d(sup_ctx* h, const StreamPlan& sp, const CsrD& M, const void* vec, const void* p1, const void* p2,
-                            const void* p3, void* out, void* out2, double lambda, const GMap& omap) {
+                            const void* p3, void* out, void* out2, double lambda, const GMap& omap, double* red_out) {
     switch (sp.G) {
-        case 4: launch_staged_g<T, MODE, 4, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap); break;
-        case 8: launch_staged_g<T, MODE, 8, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap); break;
-        case 16: launch_staged_g<T, MODE, 16, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap); break;
-        case 64: launch_staged_g<T, MODE, 64, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap); break;
-        case 0: launch_staged_g<T, MODE, 0, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap); break;
-        default: launch_staged_g<T, MODE, 32, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap); break;
+        case 4: launch_staged_g<T, MODE, 4, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap, red_out); break;
+        case 8: launch_staged_g<T, MODE, 8, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap, red_out); break;
+        case 16: launch_staged_g<T, MODE, 16, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap, red_out); break;
+        case 64: launch_staged_g<T, MODE, 64, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap, red_out); break;
+        case 0: launch_staged_g<T, MODE, 0, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap, red_out); break;
+        default: launch_staged_g<T, MODE, 32, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap, red_out); break;
     }
 }
 
 template <typename T, int MODE>
 static void launch_staged(sup_ctx* h, const StreamPlan& sp, const CsrD& M, const void* vec, const void* p1, const void* p2,
-                          const void* p3, void* out, void* out2, double lambda, const GMap& omap, bool deep) {
-    if (deep && sizeof(T) == 4) launch_staged_d<T, MODE, true>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap);
-    else launch_staged_d<T, MODE, false>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap);
+                          const void* p3, void* out, void* out2, double lambda, const GMap& omap, bool deep, double* red_out = nullptr) {
+    if (deep && sizeof(T) == 4) launch_staged_d<T, MODE, true>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap, red_out);
+    else launch_staged_d<T, MODE, false>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap, red_out);
 }
 
 // ---- gather layouts: the mirror of x and the internal layout of y (GMap, sup_internal.cuh) ------------------------------
@@ -735,27 +771,57 @@ sup_status sup_stream_refresh_layout(sup_ctx* h) {
     return rc;
 }
 
-void sup_launch_stream_fwd(sup_ctx* h, const StreamPlan& sp, const void* x, const void* dscale) {
-    CsrD M = h->A;
-    const void* vec = x;
-    if ((h->colg || h->A.pk) && h->xg) {
-        if (!h->xg_synced) {
-            const unsigned grid = unsigned((h->n + SUP_THREADS - 1) / SUP_THREADS);
-            if (h->dt == SUP_F32) k_map_copy<float><<<grid, SUP_THREADS, 0, h->stream>>>(static_cast<const float*>(x), int(h->n), static_cast<float*>(h->xg), h->xmap);
-            else k_map_copy<double><<<grid, SUP_THREADS, 0, h->stream>>>(static_cast<const double*>(x), int(h->n), static_cast<double*>(h->xg), h->xmap);
-            h->launches++;
-            h->xg_synced = true;
-        }
-        if (h->colg) M.col = h->colg;  // fp32: the mapped column is inside M.pk
-        vec = h->xg;
+static const void* stream_sync_mirror(sup_ctx* h, const void* x) {
+    // the forward product gathers from the mirror of x in its gather layout; refresh it when x changed outside the kernels
+    if (!((h->colg || h->A.pk) && h->xg)) return x;
+    if (!h->xg_synced) {
+        const unsigned grid = unsigned((h->n + SUP_THREADS - 1) / SUP_THREADS);
+        if (h->dt == SUP_F32) k_map_copy<float><<<grid, SUP_THREADS, 0, h->stream>>>(static_cast<const float*>(x), int(h->n), static_cast<float*>(h->xg), h->xmap);
+        else k_map_copy<double><<<grid, SUP_THREADS, 0, h->stream>>>(static_cast<const double*>(x), int(h->n), static_cast<double*>(h->xg), h->xmap);
+        h->launches++;
+        h->xg_synced = true;
     }
-    if (h->dt == SUP_F32) launch_staged<float, 0>(h, sp, M, vec, h->lb, h->ub, dscale, h->y, nullptr, 0.0, h->ymap, vec == h->xg && h->xmap.kind == 2);
-    else launch_staged<double, 0>(h, sp, M, vec, h->lb, h->ub, dscale, h->y, nullptr, 0.0, h->ymap, false);
+    return h->xg;
 }
 
-void sup_launch_stream_bwd(sup_ctx* h, const CsrD& AT, const StreamPlan& sp, void* x, double lambda) {
+// One staged product: mode 0 / 1 / 2 of row_epilogue over the rows of `sp` of matrix M, gathering `vec` at the (mapped)
+// indices the stream carries.  red_out (optional): [sp.nb] per-CTA partials of the mode's reduction.
+void sup_launch_staged(sup_ctx* h, int mode, const StreamPlan& sp, const CsrD& M, const void* vec, const void* p1, const void* p2,
+                       const void* p3, void* out, void* out2, double lambda, const GMap& omap, bool deep, double* red_out) {
+    if (h->dt == SUP_F32) {
+        if (mode == 0) launch_staged<float, 0>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap, deep, red_out);
+        else if (mode == 1) launch_staged<float, 1>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap, deep, red_out);
+        else launch_staged<float, 2>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap, deep, red_out);
+    } else {
+        if (mode == 0) launch_staged<double, 0>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap, false, red_out);
+        else if (mode == 1) launch_staged<double, 1>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap, false, red_out);
+        else launch_staged<double, 2>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap, false, red_out);
+    }
+}
+
+// S1+S2 over the rows of `sp`: y = dscale * c(x) (dscale = d, the block scaling, or the plain weights of DROP / EMR)
+void sup_launch_stream_fwd(sup_ctx* h, const StreamPlan& sp, const void* x, const void* dscale, double* red_out) {
+    CsrD M = h->A;
+    const void* vec = stream_sync_mirror(h, x);
+    if (vec == h->xg && h->colg) M.col = h->colg;  // fp32: the mapped column is inside M.pk
+    sup_launch_staged(h, 0, sp, M, vec, h->lb, h->ub, dscale, h->y, nullptr, 0.0, h->ymap, vec == h->xg && h->xmap.kind == 2, red_out);
+}
+
+// S3 over A^T (or a block's): x <- clip(x - lambda * zscale .* (A^T y)); zscale = NULL: 1
+void sup_launch_stream_bwd(sup_ctx* h, const CsrD& AT, const StreamPlan& sp, void* x, double lambda, const void* zscale) {
     void* mirror = sup_stream_forward_uses_xg(h) ? h->xg : nullptr;
-    if (h->dt == SUP_F32) launch_staged<float, 1>(h, sp, AT, h->y, h->lo, h->hi, nullptr, x, mirror, lambda, h->xmap, h->ymap.kind == 2);
-    else launch_staged<double, 1>(h, sp, AT, h->y, h->lo, h->hi, nullptr, x, mirror, lambda, h->xmap, false);
+    sup_launch_staged(h, 1, sp, AT, h->y, h->lo, h->hi, zscale, x, mirror, lambda, h->xmap, h->ymap.kind == 2, nullptr);
     h->xg_synced = mirror != nullptr;
+}
+
+// out = scale * A v (over the rows of A.plan) with v given in x's gather layout (v_g[xmap(j)] = v_j), reduction sum wrow_i out_i^2
+void sup_launch_stream_plain_A(sup_ctx* h, const void* v_g, void* out, double scale, const void* wrow, double* red_out) {
+    CsrD M = h->A;
+    if (h->colg) M.col = h->colg;
+    sup_launch_staged(h, 2, h->A.plan, M, v_g, nullptr, nullptr, wrow, out, nullptr, scale, GMap(), h->xmap.kind == 2, red_out);
+}
+
+// out_g[xmap(j)] = scale * (A^T y)_j with the internal y (its gather layout), reduction sum out_j^2
+void sup_launch_stream_plain_AT(sup_ctx* h, void* out_g, double scale, double* red_out) {
+    sup_launch_staged(h, 2, h->AT.plan, h->AT, h->y, nullptr, nullptr, nullptr, out_g, nullptr, scale, h->xmap, h->ymap.kind == 2, red_out);
 }

@@ -1,0 +1,226 @@
+"""GPU parity of the SURVEY.md 8(f) rows against the oracle: DROP and EMR (Table A.5), the paper's stopping
+rule (L217-223, L239-243; A-25), f_Mean (Eq. 21) and the 3-D TV objective (A-27).  Same bars as test_gpu_parity.py."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+pytestmark = pytest.mark.gpu
+
+import gen  # noqa: E402
+from oracle.oracle import Oracle  # noqa: E402
+
+TD = {0: torch.float32, 1: torch.float64}
+TOL = {0: 1e-4, 1: 1e-10}
+
+
+def rel_l2(a, b):
+    a, b = np.asarray(a, np.float64), np.asarray(b, np.float64)
+    nb = np.linalg.norm(b)
+    return np.linalg.norm(a - b) / nb if nb > 0 else np.linalg.norm(a - b)
+
+
+def _sup():
+    import paper_2606_27086_b200 as sup
+
+    return sup
+
+
+def equality_ct(n_pix=40, n_angles=36, n_bins=57, noise=0.01, seed=3):
+    """a CT-shaped EQUALITY problem (lb = ub = b), the case Table A.5 prints"""
+    P = gen.config1_tiny_ct(n_pix=n_pix, n_angles=n_angles, n_bins=n_bins, n_sweeps=12, N=3)
+    rng = np.random.default_rng(seed)
+    b = P.scipy() @ P.x_true.astype(np.float64)
+    b = (b + noise * b.max() * rng.normal(size=P.m)).astype(np.float32)
+    P.lb, P.ub = b.copy(), b.copy()
+    P.name = "ct_equality"
+    return P
+
+
+def handle(P, dtype):
+    from paper_2606_27086_b200.binding import create_from_problem
+
+    return create_from_problem(P, dtype=dtype, blocks=False)
+
+
+def xdev(x, dtype):
+    return torch.tensor(np.asarray(x), dtype=TD[dtype], device="cuda:0")
+
+
+@pytest.mark.parametrize("dtype", [0, 1])
+@pytest.mark.parametrize("which", ["equality", "slabs", "cfg2"])
+def test_drop_and_emr_sweeps(which, dtype):
+    sup = _sup()
+    P = equality_ct() if which == "equality" else (gen.config1_tiny_ct(n_pix=37, n_angles=23, n_bins=61) if which == "slabs" else gen.config2_crosswell())
+    H = handle(P, dtype)
+    O = Oracle.from_problem(P)
+    # DROP, with two relaxations
+    for lam in (1.0, 1.7):
+        x = xdev(P.x0, dtype)
+        xo = P.x0.astype(np.float64)
+        for s in (1, 7):
+            sup.sup_project_drop(H, x, lam, s)
+            xo = O.drop_sweep(xo, lam, s)
+            assert rel_l2(x.cpu().numpy(), xo) <= TOL[dtype], (which, "drop", lam, s)
+    # EMR: the iterate and the relaxation factor of the last sweep
+    x = xdev(P.x0, dtype)
+    xo = P.x0.astype(np.float64)
+    for s in range(8):
+        sup.sup_project_emr(H, x, 1)
+        xo, t = O.emr_sweep(xo, 1, return_step=True)
+        st = sup.sup_get_state(H)
+        assert abs(st["step"] - t) <= (1e-4 if dtype == 0 else 1e-10) * abs(t), (which, s, st["step"], t)
+        assert rel_l2(x.cpu().numpy(), xo) <= TOL[dtype], (which, "emr", s)
+    # the sweeps leave the library in a consistent state: a plain simultaneous sweep afterwards still matches
+    sup.sup_project_simultaneous(H, x, 1.0, 2)
+    assert rel_l2(x.cpu().numpy(), O.sweep(xo, 1.0, 2)) <= TOL[dtype]
+
+
+@pytest.mark.parametrize("dtype", [0, 1])
+@pytest.mark.parametrize("alg", ["drop", "emr"])
+def test_superiorized_drop_and_emr_stepwise(alg, dtype):
+    """TV-superiorized DROP / EMR (the paper's CT experiment runs EMR this way, L342): one sweep at a time from the oracle's state"""
+    sup = _sup()
+    P = equality_ct()
+    H = handle(P, dtype)
+    O = Oracle.from_problem(P)
+    lam = 1.9 if alg == "drop" else 1.0
+    x_ref, ell = P.x0.astype(np.float64), 0
+    for k in range(8):
+        xs = np.asarray(x_ref, np.float32 if dtype == 0 else np.float64).astype(np.float64)
+        R = O.run(xs, 1, N=P.N, beta0=P.beta0, a=0.9, lam=lam, algorithm=alg, ell0=ell, k0=k)
+        x = xdev(xs, dtype)
+        dec = torch.zeros(4096, dtype=torch.int8, device="cuda:0")
+        sup.sup_superiorize(H, x, 1, P.N, P.beta0, 0.9, objective="tv2d", shape=P.shape, lam=lam, algorithm=alg, ell0=ell, k0=k, decisions=dec)
+        st = sup.sup_get_state(H)
+        assert st["ell"] == R["ell"] and np.array_equal(dec[: st["n_decisions"]].cpu().numpy(), R["decisions"]), (alg, k)
+        assert rel_l2(x.cpu().numpy(), R["x"]) <= TOL[dtype], (alg, dtype, k)
+        x_ref, ell = R["x"], R["ell"]
+    # and the graph replay of several sweeps stays within the final-sweep bar
+    x = xdev(P.x0, dtype)
+    sup.sup_superiorize(H, x, 8, P.N, P.beta0, 0.9, objective="tv2d", shape=P.shape, lam=lam, algorithm=alg)
+    R = O.run(P.x0, 8, N=P.N, beta0=P.beta0, a=0.9, lam=lam, algorithm=alg)
+    assert rel_l2(x.cpu().numpy(), R["x"]) <= (1e-3 if dtype == 0 else 1e-9)
+
+
+@pytest.mark.parametrize("dtype", [0, 1])
+@pytest.mark.parametrize("case", ["basic", "tv", "block_tv", "emr_tv", "never"])
+def test_stopping_rule_stops_where_the_oracle_stops(case, dtype):
+    """Oracle and GPU stop after the same sweep for the same reason; x is the iterate the rule was met at; a rule that never
+    fires leaves the fixed-length run bit-identical; the trace (proximity, objective per sweep) agrees."""
+    sup = _sup()
+    base = gen.config1_tiny_ct(n_pix=32, n_angles=40, n_bins=47, n_sweeps=60, N=3)
+    P = gen.interleaved_angle_blocks(base, 8) if case == "block_tv" else base
+    from paper_2606_27086_b200.binding import create_from_problem
+
+    H = create_from_problem(P, dtype=dtype)
+    O = Oracle.from_problem(P)
+    pert = case != "basic"
+    alg = {"block_tv": "block", "emr_tv": "emr"}.get(case, "sim")
+    N = P.N if pert else 0
+    K = 60
+    # thresholds chosen from the oracle's own fixed-length trace so that the rule fires somewhere in the middle of the run
+    ref = O.run(P.x0, K, N=N, beta0=P.beta0, a=0.9, lam=P.lam, algorithm=alg, kind=P.objective if pert else "none")
+    Pk = 2.0 * ref["trace"][:, 0]
+    fk = ref["trace"][:, 1]
+    dP = np.abs(np.diff(Pk)) / np.maximum(1.0, Pk[:-1])
+    df = np.abs(np.diff(fk)) / np.maximum(1.0, fk[:-1])
+    if case == "never":
+        stop = dict(prox_tol=-1.0, dprox_tol=0.0, n_consec=5, dobj_tol=0.0)
+    else:
+        stop = dict(prox_tol=float(Pk[25]) * 1.0000001, dprox_tol=float(np.sort(dP)[len(dP) // 2]), n_consec=3,
+                    dobj_tol=float(np.sort(df)[int(0.8 * len(df))]) if pert else 1.0)
+    R = O.run(P.x0, K, N=N, beta0=P.beta0, a=0.9, lam=P.lam, algorithm=alg, kind=P.objective if pert else "none", stop=stop)
+    x = xdev(P.x0, dtype)
+    trace = torch.zeros((K, 4), dtype=torch.float64, device="cuda:0")
+    sup.sup_superiorize(H, x, K, N, P.beta0, 0.9, objective=P.objective if pert else None, shape=P.shape, lam=P.lam, block=case == "block_tv",
+                        algorithm=alg, stop=stop, trace=trace)
+    st = sup.sup_get_state(H)
+    print(f"[stopping] {case} dtype={dtype}: oracle stops after {R['n_done']} (reason {R['stop_reason']}), GPU after {st['n_done']} (reason {st['stop_reason']})")
+    assert st["n_done"] == R["n_done"] and st["stop_reason"] == R["stop_reason"], (case, st, R["n_done"], R["stop_reason"])
+    if case != "never":
+        assert 0 < R["n_done"] < K, "the thresholds of this test must make the rule fire inside the run"
+    tol = TOL[dtype] if R["n_done"] <= 12 else (1e-3 if dtype == 0 else 1e-8)
+    assert rel_l2(x.cpu().numpy(), R["x"]) <= tol
+    tr = trace.cpu().numpy()[: R["n_done"]]
+    np.testing.assert_allclose(tr[:, 0], R["trace"][:, 0], rtol=1e-3 if dtype == 0 else 1e-7)
+    if pert:
+        np.testing.assert_allclose(tr[:, 1], R["trace"][:, 1], rtol=1e-3 if dtype == 0 else 1e-7)
+    assert np.array_equal(tr[:, 3], R["trace"][:, 3])
+    if case == "never":
+        x2 = xdev(P.x0, dtype)
+        sup.sup_superiorize(H, x2, K, N, P.beta0, 0.9, objective=P.objective, shape=P.shape, lam=P.lam)
+        assert torch.equal(x, x2)
+
+
+@pytest.mark.parametrize("dtype", [0, 1])
+def test_mean_objective(dtype):
+    """f_Mean (Eq. 21) over an organ-at-risk of the reduced IMRT case: value, phase (every first trial accepted), Algorithm 1"""
+    sup = _sup()
+    P = gen.config4_imrt(scale=0.17)
+    rp, c, v, md = P.dose
+    vox_is_oar = (P.ub[:md] <= 30.5)  # rows bounded by 20 or 30 Gy: the two OARs
+    rows = np.flatnonzero(vox_is_oar)
+    counts = np.diff(rp)[rows]
+    rp_s = np.zeros(rows.size + 1, np.int64)
+    np.cumsum(counts, out=rp_s[1:])
+    idx = np.repeat(rp[:-1][rows] - rp_s[:-1], counts) + np.arange(rp_s[-1], dtype=np.int64)
+    DS = (rp_s, c[idx], v[idx], rows.size)
+    assert rows.size >= 5
+    H = sup.sup_create(P.rowptr, P.col, P.val, P.lb, P.ub, P.lo, P.hi, None, dtype=dtype, n=P.n)
+    sup.sup_set_dose_matrix(H, DS[0], DS[1], DS[2])
+    O = Oracle(P.m, P.n, P.rowptr, P.col, P.val, P.lb, P.ub, P.lo, P.hi, dose=DS, objective="mean")
+    rng = np.random.default_rng(5)
+    xs = rng.uniform(0.5, 1.5, P.n).astype(np.float32)
+    x = xdev(xs, dtype)
+    assert abs(sup.sup_objective(H, x, "mean") - O.objective_value(xs.astype(np.float64))) <= (1e-5 if dtype == 0 else 1e-12) * abs(O.objective_value(xs.astype(np.float64)))
+    ell = sup.sup_perturb_mean(H, x, 4, 0.5, 0.9, 2)
+    R = O.perturb(xs.astype(np.float64), 2, 4, 0.5, 0.9)
+    st = sup.sup_get_state(H)
+    assert ell == R["ell"] == 6 and st["n_trials"] == 4 and list(R["decisions"]) == [1, 1, 1, 1]
+    assert rel_l2(x.cpu().numpy(), R["x"]) <= (1e-6 if dtype == 0 else 1e-13)
+    assert abs(st["f"] - R["fx"]) <= (1e-5 if dtype == 0 else 1e-12) * abs(R["fx"])
+    # Algorithm 1 with the mean objective, step-wise
+    x_ref, ell = P.x0.astype(np.float64), 0
+    for k in range(6):
+        xs64 = np.asarray(x_ref, np.float32 if dtype == 0 else np.float64).astype(np.float64)
+        R = O.run(xs64, 1, N=3, beta0=1.0, a=0.95, ell0=ell, k0=k)
+        xg = xdev(xs64, dtype)
+        sup.sup_superiorize(H, xg, 1, 3, 1.0, 0.95, objective="mean", ell0=ell, k0=k)
+        assert sup.sup_get_state(H)["ell"] == R["ell"]
+        assert rel_l2(xg.cpu().numpy(), R["x"]) <= TOL[dtype], k
+        x_ref, ell = R["x"], R["ell"]
+
+
+@pytest.mark.parametrize("dtype", [0, 1])
+@pytest.mark.parametrize("shape", [(6, 9, 40), (5, 8, 32), (1, 7, 11), (9, 1, 13), (3, 4, 1), (17, 19, 23)])
+def test_tv3d_objective_and_phase(shape, dtype):
+    sup = _sup()
+    n = int(np.prod(shape))
+    rng = np.random.default_rng(8)
+    eye_rp = np.arange(n + 1, dtype=np.int64)
+    eye_c = np.arange(n, dtype=np.int32)
+    H = sup.sup_create(eye_rp, eye_c, np.ones(n, np.float32), np.zeros(n, np.float32), np.ones(n, np.float32), np.zeros(n, np.float32),
+                       np.ones(n, np.float32), None, dtype=dtype, n=n)
+    O = Oracle(n, n, eye_rp, eye_c, np.ones(n), np.zeros(n), np.ones(n), np.zeros(n), np.ones(n), objective="tv3d", shape=shape)
+    xs = rng.uniform(0, 1, n).astype(np.float32)
+    x = xdev(xs, dtype)
+    fo = O.objective_value(xs.astype(np.float64))
+    fg = sup.sup_objective(H, x, "tv3d", shape)
+    assert abs(fg - fo) <= (1e-6 if dtype == 0 else 1e-12) * abs(fo) + (0 if fo else 1e-300)
+    ell = 1
+    xo = xs.astype(np.float64)
+    for phase in range(3):
+        ell_g = sup.sup_perturb_tv(H, x, shape, 3, 0.4, 0.8, ell)
+        R = O.perturb(xo, ell, 3, 0.4, 0.8)
+        st = sup.sup_get_state(H)
+        assert ell_g == R["ell"] and st["n_trials"] == R["trials"], (shape, phase, ell_g, R["ell"], R["margins"].min() if R["margins"].size else None)
+        assert rel_l2(x.cpu().numpy(), R["x"]) <= (1e-5 if dtype == 0 else 1e-13)
+        assert abs(st["f"] - R["fx"]) <= (1e-5 if dtype == 0 else 1e-12) * abs(R["fx"]) + 1e-300
+        xo, ell = R["x"], ell_g
+    # Algorithm 1 over a box-only feasibility problem with the 3-D objective
+    x = xdev(xs, dtype)
+    sup.sup_superiorize(H, x, 4, 2, 0.4, 0.8, objective="tv3d", shape=shape)
+    R = O.run(xs.astype(np.float64), 4, N=2, beta0=0.4, a=0.8)
+    assert sup.sup_get_state(H)["ell"] == R["ell"]
+    assert rel_l2(x.cpu().numpy(), R["x"]) <= TOL[dtype]
