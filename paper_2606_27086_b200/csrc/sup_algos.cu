@@ -321,3 +321,122 @@ int sup_launch_mean_value(sup_ctx* h, const void* x) {  // leaves per-CTA partia
     h->launches++;
     return grid;
 }
+
+// ---- dose objective ||D x||^2 (A-15) as a fixed launch sequence on the staged product kernels --------------------------------
+// Per phase: r = D x (sum r^2 = f(x)); per reduction step: g = 2 D^T r (sum g^2), q = D g (sum q^2), the scalar trial loop on the
+// closed form f(x - c g) = f(x) - c ||g||^2 + c^2 ||q||^2 (SURVEY.md 8(d) allows it; the oracle evaluates every trial by a matrix
+// pass), then x <- x - c g, r <- r - c q with f of the accepted point taken as ||r||^2 of the updated r.  No data-dependent
+// launch is left, so the sequence is captured in the sweep's graph.
+__global__ void k_dose_trial(DevState* st, const double* __restrict__ red_f, int np_f, const double* __restrict__ part_f, int np_part,
+                             const double* __restrict__ red_g, int np_g, const double* __restrict__ red_q, int np_q, int first, int final_only,
+                             double beta0, double a, int policy, long long n_restart, int8_t* decisions, double* decision_f, long long cap) {
+    if (st->stop) return;
+    const long long k = st->k;
+    if (first && n_restart > 0 && k > 0 && k % n_restart == 0) {  // restarted perturbations (A-24)
+        st->ell = k / n_restart;
+        st->apow = 1.0;
+        for (long long q = 0; q < st->ell; ++q) st->apow *= a;
+    }
+    // f(x^{k,n}): ||D x||^2 of the phase's first pass, or ||r||^2 after the last accepted step (when that step moved x)
+    double fx = st->f_cur;
+    if (first) fx = sum_partials(red_f, np_f);
+    else if (st->cf != 0.0) fx = sum_partials(part_f, np_part);
+    if (!isfinite(fx)) atomicOr(&st->fault, 2);
+    st->f_cur = fx;
+    st->f = fx;
+    st->cf = 0.0;
+    if (final_only) return;
+    const double s2 = sum_partials(red_g, np_g), q2 = sum_partials(red_q, np_q);
+    const double s = sqrt(s2);
+    bool accepted = false;
+    long long jloc = 0;
+    for (int trial = 0; trial < SUP_J_MAX && !accepted; ++trial) {
+        double ap = st->apow;
+        if (policy != SUP_STEP_PER_TRIAL) {
+            ap = 1.0;
+            for (long long q = 0; q < k + jloc; ++q) ap *= a;
+        }
+        const double c = s > 0.0 ? (beta0 * ap) / s : 0.0;
+        const double fz = c == 0.0 ? fx : fx - c * s2 + c * c * q2;
+        st->ell += 1;
+        st->apow *= a;
+        ++jloc;
+        st->n_trials += 1;
+        st->sweep_trials += 1;
+        const bool acc = fz <= fx;  // NaN compares false (A-11)
+        if (decisions && st->n_dec < cap) decisions[st->n_dec] = acc ? 1 : 0;
+        if (decision_f && st->n_dec < cap) {
+            decision_f[2 * st->n_dec] = fz;
+            decision_f[2 * st->n_dec + 1] = fx;
+        }
+        st->n_dec += 1;
+        if (acc) {
+            accepted = true;
+            st->cf = c;
+            if (c == 0.0) st->f_cur = fz;
+        }
+    }
+    if (!accepted) atomicOr(&st->warn, 1);  // A-12: step skipped
+}
+
+template <typename T>
+__global__ void __launch_bounds__(SUP_THREADS)
+    k_dose_apply(const DevState* __restrict__ st, T* __restrict__ x, const T* __restrict__ g, int64_t n, T* __restrict__ r, const T* __restrict__ q,
+                 int64_t md, T* __restrict__ xg, const GMap xmap, double* __restrict__ partials) {
+    if (st->stop) return;
+    __shared__ double ws[SUP_THREADS];
+    const double cf = st->cf;
+    const int64_t tid = int64_t(blockIdx.x) * blockDim.x + threadIdx.x, nth = int64_t(gridDim.x) * blockDim.x;
+    double rr = 0.0;
+    if (cf != 0.0) {
+        for (int64_t j = tid; j < n; j += nth) {
+            const T v = T(fma(-cf, double(g[j]), double(x[j])));
+            x[j] = v;
+            if (xg) xg[sup_gmap(xmap, int(j))] = v;
+        }
+        for (int64_t i = tid; i < md; i += nth) {
+            const T rn = T(fma(-cf, double(q[i]), double(r[i])));  // r <- round_T(r - c q)
+            r[i] = rn;
+            rr += double(rn) * double(rn);
+        }
+    } else if (xg) {
+        for (int64_t j = tid; j < n; j += nth) xg[sup_gmap(xmap, int(j))] = x[j];
+    }
+    ws[threadIdx.x] = rr;
+    __syncthreads();
+    for (int o = SUP_THREADS / 2; o > 0; o >>= 1) {
+        if (threadIdx.x < o) ws[threadIdx.x] += ws[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) partials[blockIdx.x] = ws[0];
+}
+
+sup_status sup_launch_perturb_dose_staged(sup_ctx* h, void* x, const PerturbParams& pp) {
+    double *red_f = h->red, *red_g = h->red + SUP_STREAM_NBMAX, *red_q = h->red + 2 * SUP_STREAM_NBMAX;
+    const int npD = h->D.plan.nb, npDT = h->DT.plan.nb;
+    const int grid = sup_grid_for(h->D.rows, SUP_THREADS, h->num_sms * 4);
+    void* mirror = pp.write_mirror && sup_stream_forward_uses_xg(h) ? h->xg : nullptr;
+    sup_launch_staged(h, 2, h->D.plan, h->D, x, nullptr, nullptr, nullptr, h->r_dose, nullptr, 1.0, GMap(), false, red_f);  // r = D x
+    for (int nred = 0; nred < pp.N; ++nred) {
+        sup_launch_staged(h, 2, h->DT.plan, h->DT, h->r_dose, nullptr, nullptr, nullptr, h->g, nullptr, 2.0, GMap(), false, red_g);  // g = 2 D^T r
+        sup_launch_staged(h, 2, h->D.plan, h->D, h->g, nullptr, nullptr, nullptr, h->q_dose, nullptr, 1.0, GMap(), false, red_q);    // q = D g
+        k_dose_trial<<<1, 1, 0, h->stream>>>(h->state, red_f, npD, h->partials, grid, red_g, npDT, red_q, npD, nred == 0, 0, pp.beta0, pp.a,
+                                             pp.policy, pp.n_restart, pp.decisions, pp.decision_f, pp.cap);
+        void* mir = nred == pp.N - 1 ? mirror : nullptr;
+        if (h->dt == SUP_F32)
+            k_dose_apply<float><<<grid, SUP_THREADS, 0, h->stream>>>(h->state, static_cast<float*>(x), static_cast<const float*>(h->g), h->n,
+                                                                     static_cast<float*>(h->r_dose), static_cast<const float*>(h->q_dose), h->D.rows,
+                                                                     static_cast<float*>(mir), h->xmap, h->partials);
+        else
+            k_dose_apply<double><<<grid, SUP_THREADS, 0, h->stream>>>(h->state, static_cast<double*>(x), static_cast<const double*>(h->g), h->n,
+                                                                      static_cast<double*>(h->r_dose), static_cast<const double*>(h->q_dose), h->D.rows,
+                                                                      static_cast<double*>(mir), h->xmap, h->partials);
+        h->launches += 2;
+    }
+    // f of the final inner iterate into the state
+    k_dose_trial<<<1, 1, 0, h->stream>>>(h->state, red_f, npD, h->partials, grid, red_g, npDT, red_q, npD, pp.N == 0, 1, pp.beta0, pp.a, pp.policy,
+                                         pp.n_restart, pp.decisions, pp.decision_f, pp.cap);
+    h->launches++;
+    SUP_CUDA(h, cudaGetLastError());
+    return SUP_OK;
+}

@@ -46,6 +46,7 @@ extern "C" sup_status sup_workspace_bytes(int kind, int64_t m, int64_t n, int64_
         case SUP_WS_DOSE:  // (m, n, nnz) describe D_body
             p = al(size_t(n + 1) * 8) + al(size_t(nnz) * 4) + al(size_t(nnz) * esz) + 2 * al(size_t(m) * esz)
                 + al(size_t(n) * esz) + 256                                                        // gradient of f_Mean and its norm
+                + (dtype == SUP_F32 ? 2 * al(size_t(nnz) * 8) : 0) + 2 * sup_stream_table_bytes()  // packed D, D^T; partition tables
                 + 1024;
             s = sup_transpose_scratch_bytes(nnz, n, esz) + 4096;
             break;
@@ -297,6 +298,10 @@ extern "C" sup_status sup_set_dose_matrix(sup_handle h, const sup_csr* D, void* 
     h->q_dose = B.take(size_t(D->m) * h->esz);
     h->gmean = B.take(size_t(D->n) * h->esz);
     h->gmean_norm2 = static_cast<double*>(B.take(256));
+    h->pk_d = h->dt == SUP_F32 ? B.take(size_t(D->nnz) * 8) : nullptr;
+    h->pk_dt = h->dt == SUP_F32 ? B.take(size_t(D->nnz) * 8) : nullptr;
+    void* tab_d = B.take(sup_stream_table_bytes());
+    void* tab_dt = B.take(sup_stream_table_bytes());
     if (!B.ok) return sup_fail(h, SUP_ERR_WORKSPACE, "sup_set_dose_matrix: workspace too small");
     rc = sup_transpose_rows(h, Dm, 0, D->m, 0, D->nnz, rp, col, val, 0, scratch, scratch_bytes);
     if (rc != SUP_OK) return rc;
@@ -310,6 +315,15 @@ extern "C" sup_status sup_set_dose_matrix(sup_handle h, const sup_csr* D, void* 
     h->DT.val = val;
     h->g_d = sup_pick_group(D->nnz, D->m);
     h->g_dt = sup_pick_group(D->nnz, D->n);
+    // the staged product kernels run the dose perturbation's matrix passes: packed copies (plain indices) and plans
+    h->D.alloc_nnz = h->DT.alloc_nnz = D->nnz;
+    h->D.pk = h->pk_d;
+    h->DT.pk = h->pk_dt;
+    rc = sup_stream_pack(h, h->D.val, h->D.col, D->nnz, h->pk_d, GMap());
+    if (rc == SUP_OK) rc = sup_stream_pack(h, h->DT.val, h->DT.col, D->nnz, h->pk_dt, GMap());
+    if (rc == SUP_OK) rc = sup_stream_plan(h, h->D, 0, D->m, true, tab_d, scratch, &h->D.plan);
+    if (rc == SUP_OK) rc = sup_stream_plan(h, h->DT, 0, D->n, false, tab_dt, scratch, &h->DT.plan);
+    if (rc != SUP_OK) return rc;
     h->has_dose = true;
     rc = sup_setup_mean_gradient(h);  // (1/N_S) D^T 1 for f_Mean (Eq. 21), should the matrix be used as a structure's D_S
     if (rc != SUP_OK) return rc;
@@ -336,6 +350,10 @@ extern "C" sup_status sup_set_row_mode(sup_handle h, int lanes_forward, int lane
         rc = sup_stream_plan(h, h->A, h->block_rowptr[t], h->block_rowptr[t + 1], true, h->stream_fwd_blk[t].table, scratch,
                              &h->stream_fwd_blk[t]);
         if (rc == SUP_OK) rc = sup_stream_plan(h, h->ATb[t], 0, h->n, false, h->ATb[t].plan.table, scratch, &h->ATb[t].plan);
+    }
+    if (rc == SUP_OK && h->has_dose) {
+        rc = sup_stream_plan(h, h->D, 0, h->D.rows, true, h->D.plan.table, scratch, &h->D.plan);
+        if (rc == SUP_OK) rc = sup_stream_plan(h, h->DT, 0, h->DT.rows, false, h->DT.plan.table, scratch, &h->DT.plan);
     }
     if (rc == SUP_OK) rc = sup_stream_refresh_layout(h);
     if (rc == SUP_OK) SUP_CUDA(h, cudaStreamSynchronize(h->stream));

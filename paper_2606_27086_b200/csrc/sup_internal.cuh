@@ -147,6 +147,8 @@ struct sup_ctx {
     void* pk_a = nullptr;       // [nnz] x 8 B, fp32 handles: (val, sup_swz(col)) of A
     void* pk_at = nullptr;      // [nnz] x 8 B, fp32 handles: (val, row) of A^T
     void* pk_atb = nullptr;     // [nnz] x 8 B, fp32 handles: the per-block transposes (sup_set_blocks)
+    void* pk_d = nullptr;       // [nnz_D] x 8 B, fp32 handles: D_body and its transpose (sup_set_dose_matrix), plain indices
+    void* pk_dt = nullptr;
     void* wT = nullptr;         // [m] dtype: the normalised weights w_i (M of DROP / EMR)
     void* zcol = nullptr;       // [n] dtype: 1 / nnz(A_:,j), 0 for an empty column (Z of DROP)
     const int* stop_ptr = nullptr;  // &state->stop while a run with the stopping rule is being enqueued, else NULL
@@ -291,3 +293,4 @@ void sup_launch_close_sweep(sup_ctx* h, double* trace, const double* red_prox, i
 sup_status sup_setup_mean_gradient(sup_ctx* h);
 sup_status sup_launch_perturb_mean(sup_ctx* h, void* x, const PerturbParams& pp);
 int sup_launch_mean_value(sup_ctx* h, const void* x);
+sup_status sup_launch_perturb_dose_staged(sup_ctx* h, void* x, const PerturbParams& pp);

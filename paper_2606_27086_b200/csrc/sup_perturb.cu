@@ -1048,6 +1048,7 @@ int sup_perturb_grid(sup_ctx* h, int objective) {
 
 sup_status sup_launch_perturb(sup_ctx* h, void* x, const PerturbParams& pp) {
     if (pp.objective == SUP_OBJ_MEAN) return sup_launch_perturb_mean(h, x, pp);
+    if (pp.objective == SUP_OBJ_DOSE && h->D.plan.ok && h->DT.plan.ok) return sup_launch_perturb_dose_staged(h, x, pp);
     const int grid = sup_perturb_grid(h, pp.objective);
     if (grid < 1) return sup_fail(h, SUP_ERR_CUDA, "perturbation kernel cannot be made resident");
     cudaLaunchConfig_t cfg = {};
