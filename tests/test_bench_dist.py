@@ -59,3 +59,17 @@ def test_reference_arm_under_torchrun_prints_one_line_from_rank0():
     d = json.loads(lines[0])
     assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["cpu_baseline"]["kind"] == "oracle"
     assert d["value"] > 0 and d["e2e"]["h2d_bytes_per_step"] == 0
+
+
+def test_gpus_flag_means_n_ranks_or_fails_loudly():
+    """`bench.py --gpus N` without a launcher must itself become N ranks -- here, with no CUDA device, it must refuse instead of
+    silently timing one GPU; under a launcher the world size must equal --gpus."""
+    import torch
+
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2"], capture_output=True, text=True, timeout=300)
+    assert r.returncode != 0 and "only 0 CUDA device(s) visible" in (r.stdout + r.stderr)
+    env = dict(os.environ, WORLD_SIZE="4", RANK="0", LOCAL_RANK="0")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2"], capture_output=True, text=True, timeout=300, env=env)
+    assert r.returncode != 0 and "WORLD_SIZE=4" in (r.stdout + r.stderr)
