@@ -194,6 +194,8 @@ def run_ours(args, rank, world, local_rank):
     dist = dist_setup(world, "nccl", dev)
 
     P = make_problem(args.workload)
+    if args.sharded:
+        return run_sharded(args, P, rank, world, local_rank, dev, dist)
     if args.block:  # BASELINE.json configs[2], second run: block-iterative with 16 interleaved angle blocks (A-14)
         import gen
 
@@ -346,6 +348,53 @@ def run_ours(args, rank, world, local_rank):
         dist.destroy_process_group()
 
 
+def run_sharded(args, P, rank, world, local_rank, dev, dist):
+    """Row blocks of A per rank, replica of x, one all-reduce per sweep: total work is fixed -> strong scaling.
+    The sweeps are driven from Python (no CUDA graph across the collective), the perturbation phase is replicated."""
+    import torch
+
+    import paper_2606_27086_b200 as sup
+    from paper_2606_27086_b200.sharded import ShardedSup
+
+    group = dist.group.WORLD if dist is not None else None
+    Sh = ShardedSup(P, rank, world, dtype=sup.F32, device=dev, group=group)
+    S = P.n_sweeps
+    x0 = torch.tensor(P.x0, dtype=torch.float32, device=dev)
+    x = x0.clone()
+
+    def step():
+        x.copy_(x0)
+        Sh.superiorize(x, S, P.N, P.beta0, P.a, lam=P.lam)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches0 = Sh.H.launches
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    ms = max_over_ranks(e0.elapsed_time(e1), dist, dev)
+    if rank == 0:
+        line = {"metric": METRIC, "value": args.steps * S / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong",
+                "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": WORKLOAD_TEXT.get(args.workload, args.workload), "m": P.m, "n": P.n, "nnz": P.nnz, "sweeps_per_step": S,
+                           "parallelism": f"rows of A sharded over {world} rank(s), replica of x, one all-reduce of {P.n * 4} bytes per sweep",
+                           "rows_of_rank0": [int(Sh.cuts[0]), int(Sh.cuts[1])]},
+                "gpu_launches": int(Sh.H.launches - launches0), "checksum_x": float(x.double().sum())}
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -355,6 +404,8 @@ def main():
     ap.add_argument("--workload", default="cfg3")
     ap.add_argument("--cpu-budget", type=float, default=15.0)
     ap.add_argument("--block", action="store_true", help="block-iterative sweeps, 16 interleaved angle blocks (CT workloads)")
+    ap.add_argument("--sharded", action="store_true", help="row-sharded sweeps over the N ranks (one all-reduce of an n-vector per sweep; "
+                                                           "strong scaling) instead of N replicas")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

@@ -188,6 +188,14 @@ sup_status sup_project_simultaneous(sup_handle h, void* x, double lambda, int n_
 sup_status sup_forward_violation(sup_handle h, const void* x);
 sup_status sup_backproject_update(sup_handle h, void* x, double lambda);
 
+/* The halves of a ROW-SHARDED sweep: every GPU owns a block of rows of A (its own handle, created on that
+ * block) and a replica of x.  sup_forward_violation(h, x) forms the block's y; sup_backproject_partial writes the block's
+ * share u = scale * A_block^T y (length n, plain order, not applied) -- scale = the block's share of the global weights, because
+ * a handle normalises its weights over its own rows; the caller sums the u of all blocks (one all-reduce of an n-vector);
+ * sup_apply_update then does x <- P_box(x - lambda u) identically on every GPU (Eq. 3). */
+sup_status sup_backproject_partial(sup_handle h, void* u, double scale);
+sup_status sup_apply_update(sup_handle h, void* x, const void* u, double lambda);
+
 /* n_sweeps DROP sweeps (Table A.5): x <- P_box(x - lambda Z A^T M c(x)); for equality rows lb = ub = b the
  * residual c(x) is A x - b, the table's formula (A-26). */
 sup_status sup_project_drop(sup_handle h, void* x, double lambda, int n_sweeps);

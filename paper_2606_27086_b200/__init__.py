@@ -8,6 +8,8 @@ from .binding import (  # noqa: F401
     SupError,
     SupHandle,
     lib,
+    sup_apply_update,
+    sup_backproject_partial,
     sup_backproject_update,
     sup_block_iterative,
     sup_forward_violation,

@@ -70,6 +70,8 @@ def lib():
         L.sup_perturb_dose.argtypes = [c_void_p, c_void_p, c_int, c_double, c_double, POINTER(c_int64)]
         L.sup_perturb_mean.argtypes = [c_void_p, c_void_p, c_int, c_double, c_double, POINTER(c_int64)]
         L.sup_project_drop.argtypes = [c_void_p, c_void_p, c_double, c_int]
+        L.sup_backproject_partial.argtypes = [c_void_p, c_void_p, c_double]
+        L.sup_apply_update.argtypes = [c_void_p, c_void_p, c_void_p, c_double]
         L.sup_project_emr.argtypes = [c_void_p, c_void_p, c_int]
         L.sup_superiorize.argtypes = [c_void_p, c_void_p, c_int, c_int, c_double, c_double, POINTER(_Options)]
         L.sup_superiorize_host.argtypes = [c_void_p, c_void_p, c_int, c_int, c_double, c_double, POINTER(_Options)]
@@ -81,7 +83,7 @@ def lib():
         L.sup_set_layout.argtypes = [c_void_p, POINTER(c_int64), POINTER(c_int64)]
         for f in ("sup_workspace_bytes", "sup_create", "sup_destroy", "sup_set_blocks", "sup_set_dose_matrix",
                   "sup_project_simultaneous", "sup_block_iterative", "sup_forward_violation", "sup_backproject_update", "sup_perturb_tv", "sup_perturb_dose", "sup_superiorize",
-                  "sup_superiorize_host", "sup_get_state", "sup_proximity", "sup_objective", "sup_get_derived", "sup_set_row_mode", "sup_set_layout", "sup_perturb_mean", "sup_project_drop", "sup_project_emr"):
+                  "sup_superiorize_host", "sup_get_state", "sup_proximity", "sup_objective", "sup_get_derived", "sup_set_row_mode", "sup_set_layout", "sup_perturb_mean", "sup_project_drop", "sup_project_emr", "sup_backproject_partial", "sup_apply_update"):
             getattr(L, f).restype = c_int
         _lib = L
     return _lib
@@ -249,6 +251,20 @@ def sup_backproject_update(H: SupHandle, x: torch.Tensor, lam=1.0, sync_streams=
     H._check(lib().sup_backproject_update(H.h, _ptr(x), lam))
     if sync_streams:
         H._exit()
+
+
+def sup_backproject_partial(H: SupHandle, u: torch.Tensor, scale=1.0):
+    H._enter()
+    H._check(lib().sup_backproject_partial(H.h, _ptr(u), scale))
+    H._exit()
+    return u
+
+
+def sup_apply_update(H: SupHandle, x: torch.Tensor, u: torch.Tensor, lam=1.0):
+    H._enter()
+    H._check(lib().sup_apply_update(H.h, _ptr(x), _ptr(u), lam))
+    H._exit()
+    return x
 
 
 def sup_project_drop(H: SupHandle, x: torch.Tensor, lam=1.0, n_sweeps=1):

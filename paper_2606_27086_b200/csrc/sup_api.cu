@@ -452,6 +452,48 @@ extern "C" sup_status sup_backproject_update(sup_handle h, void* x, double lambd
     return SUP_OK;
 }
 
+// ---- the two halves of a ROW-SHARDED sweep: each GPU holds a block of rows of A and a replica of x ------------
+template <typename T>
+__global__ void __launch_bounds__(SUP_THREADS) k_apply_update(T* __restrict__ x, const T* __restrict__ u, const T* __restrict__ lo,
+                                                             const T* __restrict__ hi, T lambda, int64_t n, T* __restrict__ xg, const GMap xmap) {
+    for (int64_t j = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; j < n; j += int64_t(gridDim.x) * blockDim.x) {
+        T t = x[j] - lambda * u[j];  // Eq. 3
+        t = t < lo[j] ? lo[j] : t;   // box (L427)
+        t = t > hi[j] ? hi[j] : t;
+        x[j] = t;
+        if (xg) xg[sup_gmap(xmap, int(j))] = t;
+    }
+}
+
+extern "C" sup_status sup_backproject_partial(sup_handle h, void* u, double scale) {
+    if (!h) return SUP_ERR_INVALID_ARG;
+    SUP_ENTER(h);
+    if (!u) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_backproject_partial: NULL u");
+    if (!h->AT.plan.ok) return sup_fail(h, SUP_ERR_STATE, "sup_backproject_partial needs the staged product kernels (sup_set_row_mode)");
+    sup_launch_staged(h, 2, h->AT.plan, h->AT, h->y, nullptr, nullptr, nullptr, u, nullptr, scale, GMap(), h->ymap.kind == 2, nullptr);
+    SUP_CUDA(h, cudaGetLastError());
+    return SUP_OK;
+}
+
+extern "C" sup_status sup_apply_update(sup_handle h, void* x, const void* u, double lambda) {
+    if (!h) return SUP_ERR_INVALID_ARG;
+    SUP_ENTER(h);
+    if (!x || !u) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_apply_update: NULL x or u");
+    if (check_lambda(h, lambda) != SUP_OK) return SUP_ERR_INVALID_ARG;
+    const int grid = sup_grid_for(h->n, SUP_THREADS, h->num_sms * 4);
+    void* mirror = sup_stream_forward_uses_xg(h) ? h->xg : nullptr;
+    if (h->dt == SUP_F32)
+        k_apply_update<float><<<grid, SUP_THREADS, 0, h->stream>>>(static_cast<float*>(x), static_cast<const float*>(u), static_cast<const float*>(h->lo),
+                                                                   static_cast<const float*>(h->hi), float(lambda), h->n, static_cast<float*>(mirror), h->xmap);
+    else
+        k_apply_update<double><<<grid, SUP_THREADS, 0, h->stream>>>(static_cast<double*>(x), static_cast<const double*>(u), static_cast<const double*>(h->lo),
+                                                                    static_cast<const double*>(h->hi), lambda, h->n, static_cast<double*>(mirror), h->xmap);
+    h->launches++;
+    h->xg_synced = mirror != nullptr;
+    SUP_CUDA(h, cudaGetLastError());
+    return SUP_OK;
+}
+
 extern "C" sup_status sup_project_drop(sup_handle h, void* x, double lambda, int n_sweeps) {
     if (!h) return SUP_ERR_INVALID_ARG;
     SUP_ENTER(h);

@@ -224,3 +224,45 @@ def test_tv3d_objective_and_phase(shape, dtype):
     R = O.run(xs.astype(np.float64), 4, N=2, beta0=0.4, a=0.8)
     assert sup.sup_get_state(H)["ell"] == R["ell"]
     assert rel_l2(x.cpu().numpy(), R["x"]) <= TOL[dtype]
+
+
+@pytest.mark.parametrize("dtype", [0, 1])
+@pytest.mark.parametrize("world", [2, 3])
+def test_row_sharded_sweep_matches_single_handle(world, dtype):
+    """SURVEY.md 8(e) on the real kernels, emulated on one GPU (the blocks run one after the other, nothing waits on anything):
+    every block's share u_g = W_g A_g^T y_g summed = the unsharded back-projection; sharded superiorized sweeps against the
+    single-handle run (summation order differs: tolerance 1e-6 / 1e-12 per sweep) and against the oracle at the usual bars."""
+    sup = _sup()
+    from paper_2606_27086_b200.sharded import ShardedSup
+
+    P = gen.config1_tiny_ct(n_pix=40, n_angles=36, n_bins=57, n_sweeps=8, N=3)
+    shards = [ShardedSup(P, g, world, dtype=dtype) for g in range(world)]
+    assert sum(s.share for s in shards) == pytest.approx(1.0, rel=1e-12)
+    H = handle(P, dtype)
+    O = Oracle.from_problem(P)
+    x_ref = xdev(P.x0, dtype)
+    ell_ref = 0
+    for k in range(8):
+        xs = x_ref.clone()  # both start every sweep from the same state (DESIGN.md A-23: the TV iteration amplifies roundings)
+        # single handle: perturbation phase + sweep
+        ell = sup.sup_perturb_tv(shards[0].H, xs, P.shape, P.N, P.beta0, P.a, ell_ref)
+        ell_ref = sup.sup_perturb_tv(H, x_ref, P.shape, P.N, P.beta0, P.a, ell_ref)
+        assert ell == ell_ref and torch.equal(xs, x_ref)  # the replicated perturbation phase is bit-identical
+        sup.sup_project_simultaneous(H, x_ref, P.lam, 1)
+        # sharded: per-block shares, "all-reduce" by hand, identical update
+        u = torch.zeros_like(xs)
+        for s in shards:
+            u += s.partial(xs)
+        sup.sup_apply_update(shards[0].H, xs, u, P.lam)
+        assert rel_l2(xs.cpu().numpy(), x_ref.cpu().numpy()) <= (1e-6 if dtype == 0 else 1e-12), k
+    # the sharded driver on its own (world = 1 group-less shards would skip the reduction, so drive the blocks by hand) vs the oracle
+    xs, ell = xdev(P.x0, dtype), 0
+    for k in range(8):
+        ell = sup.sup_perturb_tv(shards[0].H, xs, P.shape, P.N, P.beta0, P.a, ell)
+        u = torch.zeros_like(xs)
+        for s in shards:
+            u += s.partial(xs)
+        sup.sup_apply_update(shards[0].H, xs, u, P.lam)
+    R = O.superiorize(P.x0, 8, P.N, P.beta0, P.a, lam=P.lam)
+    assert ell == R["ell"]
+    assert rel_l2(xs.cpu().numpy(), R["x"]) <= (1e-3 if dtype == 0 else 1e-9)
