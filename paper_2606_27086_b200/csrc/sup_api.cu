@@ -80,8 +80,10 @@ extern "C" sup_status sup_create(sup_handle* out, const sup_csr* A, const void* 
     *out = nullptr;
     if (!A || !A->rowptr || !A->col || !A->val || !lb || !ub || !box_lo || !box_hi)
         return sup_fail(nullptr, SUP_ERR_INVALID_ARG, "sup_create: NULL array argument");
-    if (A->m <= 0 || A->n <= 0 || A->nnz < 0 || A->n > 0x7fffffffLL || A->m > 0x7fffffffLL || A->nnz > 0x7fffffffLL)
-        return sup_fail(nullptr, SUP_ERR_INVALID_ARG, "sup_create: m, n must be in [1, 2^31), nnz in [0, 2^31)");
+    // rows and columns are 32-bit indices; the number of stored entries may exceed 2^31 (row pointers are 64-bit; the transpose
+    // ranks entries with 32-bit unsigned positions, hence the 2^32 - 1 limit)
+    if (A->m <= 0 || A->n <= 0 || A->nnz < 0 || A->n > 0x7fffffffLL || A->m > 0x7fffffffLL || A->nnz > 0xfffffffeLL)
+        return sup_fail(nullptr, SUP_ERR_INVALID_ARG, "sup_create: m, n must be in [1, 2^31), nnz in [0, 2^32 - 1)");
     if (dtype != SUP_F32 && dtype != SUP_F64) return sup_fail(nullptr, SUP_ERR_INVALID_ARG, "sup_create: bad dtype");
     size_t need_p = 0, need_s = 0;
     sup_workspace_bytes(SUP_WS_CREATE, A->m, A->n, A->nnz, dtype, 1, &need_p, &need_s);
@@ -273,7 +275,7 @@ extern "C" sup_status sup_set_dose_matrix(sup_handle h, const sup_csr* D, void* 
                                           void* scratch, size_t scratch_bytes) {
     if (!h) return SUP_ERR_INVALID_ARG;
     SUP_ENTER(h);
-    if (!D || !D->rowptr || !D->col || !D->val || D->m <= 0 || D->n != h->n || D->nnz < 0 || D->nnz > 0x7fffffffLL)
+    if (!D || !D->rowptr || !D->col || !D->val || D->m <= 0 || D->n != h->n || D->nnz < 0 || D->nnz > 0xfffffffeLL)
         return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_set_dose_matrix: bad matrix (needs n columns)");
     size_t need_p = 0, need_s = 0;
     sup_workspace_bytes(SUP_WS_DOSE, D->m, D->n, D->nnz, h->dt, 1, &need_p, &need_s);

@@ -201,7 +201,7 @@ sup_status sup_transpose_rows(sup_ctx* h, const CsrD& A, int64_t r0, int64_t r1,
                               int64_t* out_rowptr, int32_t* out_col, void* out_val, int64_t out_base, void* scratch,
                               size_t scratch_bytes) {
     const int64_t N = e1 - e0;
-    if (N > 0x7fffffffLL) return sup_fail(h, SUP_ERR_INVALID_ARG, "transpose: more than 2^31-1 entries in one block");
+    if (N > 0xfffffffeLL) return sup_fail(h, SUP_ERR_INVALID_ARG, "transpose: more than 2^32-2 entries in one block (32-bit unsigned ranks)");
     if (scratch_bytes < sup_transpose_scratch_bytes(N, A.cols, h->esz))
         return sup_fail(h, SUP_ERR_WORKSPACE, "transpose: scratch too small");
     cudaStream_t st = h->stream;

@@ -266,3 +266,57 @@ def test_row_sharded_sweep_matches_single_handle(world, dtype):
     R = O.superiorize(P.x0, 8, P.N, P.beta0, P.a, lam=P.lam)
     assert ell == R["ell"]
     assert rel_l2(xs.cpu().numpy(), R["x"]) <= (1e-3 if dtype == 0 else 1e-9)
+
+
+@pytest.mark.parametrize("lg,k", [(12, 16), (13, 64), (14, 256)])
+def test_device_generator_is_bit_identical(lg, k):
+    """gen/device.py (the config-5 generator for points too large for the host) against gen.config5_sweep_point"""
+    from gen.device import config5_on_device
+
+    P = gen.config5_sweep_point(lg, k)
+    G = config5_on_device(lg, k)
+    assert np.array_equal(G["rowptr"].cpu().numpy(), P.rowptr) and np.array_equal(G["col"].cpu().numpy(), P.col)
+    assert np.array_equal(G["val"].cpu().numpy(), P.val) and np.array_equal(G["x_true"].cpu().numpy(), P.x_true)
+    assert np.array_equal(G["lb"].cpu().numpy(), P.lb) and np.array_equal(G["ub"].cpu().numpy(), P.ub)
+
+
+def test_more_than_2_31_stored_entries():
+    """64-bit nnz: m = 2^23 rows x k = 256 = 2^31 stored entries (row pointers int64, 32-bit unsigned ranks in the transpose):
+    x* is a fixed point, the proximity decreases, seeded rows of y agree with an fp64 recomputation."""
+    sup = _sup()
+    from gen.device import config5_on_device
+    from paper_2606_27086_b200.binding import sup_get_derived
+
+    free_b, _ = torch.cuda.mem_get_info()
+    lg, k = 23, 256
+    if free_b < 72 * (1 << lg) * k + (2 << 30):
+        pytest.skip("not enough device memory for the 2^31-entry point")
+    G = config5_on_device(lg, k)
+    m, n = G["m"], G["n"]
+    H = sup.sup_create(G["rowptr"], G["col"], G["val"], G["lb"], G["ub"], G["lo"], G["hi"], None, dtype=0, n=n)
+    xs = G["x_true"].clone()
+    sup.sup_project_simultaneous(H, xs, 1.0, 1)
+    assert torch.equal(xs, G["x_true"])
+    x = G["x0"].clone()
+    p0 = sup.sup_proximity(H, x, 0)
+    sup.sup_project_simultaneous(H, x, 1.0, 2)
+    p2 = sup.sup_proximity(H, x, 0)
+    assert p2 < p0
+    sup.sup_forward_violation(H, x)
+    y = sup_get_derived(H, 5)
+    rng = np.random.default_rng(1)
+    rows = np.unique(np.concatenate([rng.integers(0, m, 2000), [0, m - 1, m // 2]]))
+    t = np.arange(k, dtype=np.uint64)[None, :]
+    h = gen.workloads.hash3(gen.SEED0 + 5, rows.astype(np.uint64)[:, None], t)
+    w = np.uint64(n // k)
+    cols = (t * w + h % w).astype(np.int64)
+    vals = (((h >> np.uint64(40)) + np.uint64(1)).astype(np.float64) / 2.0**24).astype(np.float32).astype(np.float64)
+    xh = x.cpu().numpy().astype(np.float64)
+    r = (vals * xh[cols]).sum(1)
+    lbh, ubh = G["lb"][rows].cpu().numpy().astype(np.float64), G["ub"][rows].cpu().numpy().astype(np.float64)
+    c = np.where(r > ubh, r - ubh, np.where(r < lbh, r - lbh, 0.0))
+    want = (1.0 / m) / (vals * vals).sum(1) * c
+    got = y[rows].cpu().numpy().astype(np.float64)
+    big = np.abs(c) > 1e-3
+    assert big.sum() > 100
+    np.testing.assert_allclose(got[big], want[big], rtol=2e-3)  # fp32 row dots of 256 terms against a violation of >= 1e-3
