@@ -46,6 +46,11 @@ struct RgShape {
     static constexpr int NCW = !DEEP || sizeof(T) != 4 ? 12 : (MODE == 0 ? 14 : 18);
     static constexpr int STG = sizeof(T) != 4 ? 16 : (DEEP ? 24 : (MODE == 0 ? 20 : 16));
 };
+#define RG_NCARRY 256
+#ifndef RG_SEG_MIN_AVG
+#define RG_SEG_MIN_AVG 1e300                // mean row length from which the planner would pick the segment mode (G = 1): never --
+                                            // it is correct but 1.7-3.7x slower than the row modes (profiles/r02j_segments.md); sup_set_row_mode(h, 1, 1) selects it
+#endif
 #define RG_CWARPS 24                        // upper bound on the consumer warps (sizes of the shared arrays)
 #ifndef RG_NPROD
 #define RG_NPROD 2                          // producer warps: ONE thread issues at most one bulk copy per ~270 ns whatever its size
@@ -88,7 +93,7 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
 }
 
 #ifdef SUP_PROFILE
-__device__ unsigned long long g_prof[8];  // 0 consumer data-wait, 1 consumer dot, 2 consumer total, 3 producer free-wait, 4 producer total, 5 kernel
+__device__ unsigned long long g_prof[8];  // G == 1 also: 6 carry wait, 7 accumulate phase  // 0 consumer data-wait, 1 consumer dot, 2 consumer total, 3 producer free-wait, 4 producer total, 5 kernel
 #define PROF_T(v) const long long v = clock64()
 #define PROF_DECL long long prof_acc[6] = {0, 0, 0, 0, 0, 0}
 #define PROF_ADD(i, d) prof_acc[i] += (long long)(d)
@@ -134,6 +139,32 @@ __device__ __forceinline__ void ring_get(const RgData<float, STG>& d, int i, int
     c = int(q.y);
 }
 
+template <typename T>
+struct CarrySlot;
+template <>
+struct CarrySlot<float> {
+    typedef unsigned long long type;  // value bits | flag << 32
+    static __device__ __forceinline__ void put(volatile type* p, float v, int flag) { *p = (type(unsigned(flag)) << 32) | type(__float_as_uint(v)); }
+    static __device__ __forceinline__ bool get(volatile type* p, int flag, float& v) {
+        const type w = *p;
+        v = __uint_as_float(unsigned(w));
+        return int(w >> 32) == flag;
+    }
+};
+template <>
+struct CarrySlot<double> {
+    typedef ulonglong2 type;  // .x value bits, .y flag: one 16-byte shared access
+    static __device__ __forceinline__ void put(volatile type* p, double v, int flag) {
+        asm volatile("st.volatile.shared.v2.b64 [%0], {%1, %2};" ::"r"(smem_u32(const_cast<type*>(p))), "l"(__double_as_longlong(v)), "l"((long long)flag) : "memory");
+    }
+    static __device__ __forceinline__ bool get(volatile type* p, int flag, double& v) {
+        long long a, b;
+        asm volatile("ld.volatile.shared.v2.b64 {%0, %1}, [%2];" : "=l"(a), "=l"(b) : "r"(smem_u32(const_cast<type*>(p))) : "memory");
+        v = __longlong_as_double(a);
+        return int(b) == flag;
+    }
+};
+
 template <typename T, int STG>
 struct RgSmem {
     RgData<T, STG> d;
@@ -143,6 +174,9 @@ struct RgSmem {
     int progress[RG_CWARPS];  // per consumer warp: tiles [0, progress) are no longer needed by it
     int issued[STG];          // per stage: 1 + the tile its barrier is currently armed for (0: none yet)
     double red[RG_CWARPS];    // per consumer warp: its share of the kernel's reduction
+    // G == 1: slot s mod RG_NCARRY = (partial sum of the row left open at the end of segment s, 1 + s), written and read as ONE
+    // vector access so that no fence is needed between value and flag
+    typename CarrySlot<T>::type carry[RG_NCARRY];
 };
 
 // Dot product of the ring elements k, k+G, k+2G, ... < e (offsets relative to the stream base) with gathered vec
@@ -227,6 +261,36 @@ __device__ __forceinline__ void row_epilogue(int64_t r, T acc, T q1, T q2, T q3,
         racc += double(q3) * (double(v) * double(v));
     }
 }
+// loads the compiler may not sink towards their use (the segment mode issues a row's operands long before the row's
+// sum is complete, and the use sits on the carry chain between segments, where an L2 round trip would serialise the warps)
+__device__ __forceinline__ float ld_pinned(const float* p) {
+    float v;
+    asm volatile("ld.global.f32 %0, [%1];" : "=f"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ double ld_pinned(const double* p) {
+    double v;
+    asm volatile("ld.global.f64 %0, [%1];" : "=d"(v) : "l"(p) : "memory");
+    return v;
+}
+template <typename T, int MODE>
+__device__ __forceinline__ void row_operands_pinned(int64_t r, const T* p1, const T* p2, const T* p3, const T* out, T& q1, T& q2, T& q3, T& q4) {
+    q4 = T(1);
+    if (MODE == 0) {
+        q1 = ld_pinned(p1 + r);
+        q2 = ld_pinned(p2 + r);
+        q3 = ld_pinned(p3 + r);
+    } else if (MODE == 1) {
+        q1 = ld_pinned(p1 + r);
+        q2 = ld_pinned(p2 + r);
+        q3 = ld_pinned(out + r);
+        if (p3) q4 = ld_pinned(p3 + r);
+    } else {
+        q1 = q2 = T(0);
+        q3 = p3 ? ld_pinned(p3 + r) : T(1);
+    }
+}
+
 template <typename T, int MODE>
 __device__ __forceinline__ void row_operands(int64_t r, const T* p1, const T* p2, const T* p3, const T* out, T& q1, T& q2, T& q3, T& q4) {
     q4 = T(1);
@@ -272,6 +336,7 @@ __global__ void __launch_bounds__(32 * (NCW + RG_NPROD), 1)
         for (int s = 0; s < STG; ++s) mbar_init(smem_u32(&S.full[s]), 1);
         for (int w = 0; w < NCW; ++w) S.progress[w] = 0;
         for (int st = 0; st < STG; ++st) S.issued[st] = 0;
+        for (int q = 0; q < RG_NCARRY; ++q) CarrySlot<T>::put(&S.carry[q], T(0), 0);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -410,6 +475,289 @@ __global__ void __launch_bounds__(32 * (NCW + RG_NPROD), 1)
         }
         __syncwarp();
         if (lane == 0) progress[warp] = ntiles;
+    } else if constexpr (G == 1) {
+    // ---- consumers, G == 1: SEGMENTS of the stream instead of rows (rows of hundreds of entries and more) ---------------------
+    // Warp w takes the segments w, w + NCW, ... of 32 x RG_UNROLL consecutive elements of the CTA's stream, whatever rows they belong
+    // to: every trip is full (no predicated partial groups), there is no per-row prologue, and the ring span of the warps in flight
+    // is NCW segments whatever the row lengths.  Lane l holds the elements S0 + 32 u + l; a group of 32 consecutive elements lies
+    // inside one row unless a row END falls into it (a warp-uniform test per group); where one does, the lanes before it finish
+    // that row: warp sum, plus the partial sum carried over from earlier segments, epilogue by the lane that prefetched the row's
+    // operands.  The sum of what follows the last row end of a segment is handed to the next segment through shared memory
+    // (carry[], in segment order: a fixed summation order).  Row ends are found in a window of 32 consecutive row pointers that
+    // each warp keeps sliding forward (loaded one segment ahead).
+        constexpr int SEG = 32 * RG_UNROLL;
+        static_assert(RG_TILE % SEG == 0, "a segment must not straddle two ring stages' end");
+        const unsigned FULLM = 0xffffffffu;
+        const int E = int(ee - base), F = int(es - base);  // valid elements of the stream: [F, E)
+        const int nseg = E > 0 ? (E + SEG - 1) / SEG : 1;  // (an all-empty range still has its rows to write)
+        volatile typename CarrySlot<T>::type* carry = S.carry;
+        auto load_window = [&](int64_t r) -> int {  // lane l: end of row r + l as a stream offset (rows beyond the range never end)
+            const int64_t rr = r + lane;
+            return rr < re ? int(rowptr[rr + 1] - base) : 0x7fffffff;
+        };
+        auto warp_sum = [&](T v) -> T {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(FULLM, v, o);
+            return v;
+        };
+        int64_t wrow = rs;               // first row of the window; rows before it are finished
+        int wend = load_window(wrow);
+        int seen = 0, released = 0;
+        // The first row that ends in a segment began in an earlier one: its sum needs the carry of the segment before.  Nothing else
+        // does -- in particular not the segment's own carry-out when a row ends in it -- so that row is parked (head_*) and only
+        // completed one segment of this warp later, when the carry has long been published: the warps never wait for each other
+        // except through segments no row ends in (rows longer than a segment).
+        bool head_pending = false;
+        T head_sum = T(0);
+        int head_lane = 0, head_seg = 0;
+        int64_t head_row = 0;
+        T hq1 = T(0), hq2 = T(0), hq3 = T(0), hq4 = T(1);
+        PROF_DECL;
+        PROF_T(ct0);
+        for (int sg = warp; sg < nseg; sg += NCW) {
+            PROF_T(it0);
+            const int S0 = sg * SEG;
+            const int S1 = S0 + SEG < E ? S0 + SEG : E;
+            // rows that ended at or before S0 were finished by earlier segments (segment 0: leading empty rows are its own)
+            int nskip = 0;
+            if (sg > 0) {
+                for (;;) {
+                    nskip = __popc(__ballot_sync(FULLM, wend <= S0));
+                    if (nskip < 32) break;
+                    wrow += 32;
+                    wend = load_window(wrow);
+                }
+            }
+            int jb = nskip;  // window lane of the next row to finish
+            int e_next = __shfl_sync(FULLM, wend, jb);
+            // Row-end window for this warp's NEXT segment (NCW segments ahead: usually < 32 rows further on), loaded now so that its
+            // latency hides behind this segment's work
+            const int64_t wrow_next = wrow + nskip;
+            const int wend_next = nskip ? load_window(wrow_next) : wend;
+            T q1 = T(0), q2 = T(0), q3 = T(0), q4 = T(1);
+            if (lane >= nskip && wend <= S1) row_operands_pinned<T, MODE>(wrow + lane, p1, p2, p3, out, q1, q2, q3, q4);  // rows finishing here
+            const int lo_valid = S0 > F ? S0 : F;
+            const bool has_data = S1 > lo_valid;
+            const int t_tile = S0 / RG_TILE;
+            if (has_data) {
+                if (released < t_tile) {
+                    released = t_tile;
+                    if (lane == 0) progress[warp] = t_tile;
+                }
+                for (int t = seen > t_tile ? seen : t_tile; t <= t_tile; ++t) {
+                    const int st = t % STG;
+                    if (issued[st] != t + 1) {
+                        const long long t0 = clock64();
+                        while (issued[st] != t + 1)
+                            if (clock64() - t0 > RG_TIMEOUT) __trap();
+                    }
+                    mbar_wait(smem_u32(&S.full[st]), (t / STG) & 1);
+                }
+                seen = seen > t_tile + 1 ? seen : t_tile + 1;
+                asm volatile("" ::: "memory");
+                PROF_ADD(0, clock64() - it0);
+            }
+            int rel = S1 / RG_TILE;  // tiles wholly before the end of the segment: not needed by this warp once it has read its elements
+            rel = rel < ntiles ? rel : ntiles;
+            const int p0 = S0 % RG_ELEMS + lane;  // (RG_ELEMS is a multiple of SEG: no wrap inside a segment)
+            bool any_end = false;
+            T acc = T(0);
+            PROF_T(ac0);
+            auto carry_of = [&](int seg) -> T {  // the carry-out of segment seg - 1 (0 for the first segment)
+                if (seg == 0) return T(0);
+                const int slot = (seg - 1) % RG_NCARRY;
+                T cv;
+                if (!CarrySlot<T>::get(&carry[slot], seg, cv)) {
+                    const long long t0 = clock64();
+                    while (!CarrySlot<T>::get(&carry[slot], seg, cv)) {
+                        __nanosleep(20);
+                        if (clock64() - t0 > RG_TIMEOUT) __trap();
+                    }
+                    PROF_ADD(3, clock64() - t0);
+                }
+                return cv;
+            };
+            // complete the row parked by this warp's PREVIOUS segment: its carry was published long ago, nobody waits
+            auto flush_head = [&]() {
+                if (!head_pending) return;
+                const T tot = carry_of(head_seg) + head_sum;
+                if (lane == head_lane) row_epilogue<T, MODE>(head_row, tot, hq1, hq2, hq3, hq4, out, out2, lambda, omap, racc);
+                head_pending = false;
+            };
+            auto park_head = [&](T sum, int jlane) {
+                flush_head();
+                head_pending = true;
+                head_sum = sum;
+                head_lane = jlane;
+                head_row = wrow + jlane;
+                head_seg = sg;
+                hq1 = q1;
+                hq2 = q2;
+                hq3 = q3;
+                hq4 = q4;
+            };
+            const int nfin = __popc(__ballot_sync(FULLM, wend <= S1)) - nskip;  // rows of the window that end in this segment
+            if (nfin <= 3 && nskip + nfin < 32) {
+                // ---- the usual case, straight-line code: at most three row ends, all inside the window ------------------------
+                T v[RG_UNROLL];
+                T g[RG_UNROLL];
+                if (has_data) {
+                    int c[RG_UNROLL];
+                    if (S1 - S0 == SEG && S0 >= F) {
+#pragma unroll
+                        for (int u = 0; u < RG_UNROLL; ++u) ring_get(S.d, p0 + 32 * u, c[u], v[u]);
+                    } else {  // first / last segment of the range: elements outside [F, E) are not the CTA's (or not loaded at all)
+#pragma unroll
+                        for (int u = 0; u < RG_UNROLL; ++u) {
+                            const int pos = S0 + 32 * u + lane;
+                            const bool ok = pos >= F && pos < S1;
+                            ring_get(S.d, p0 + 32 * u, c[u], v[u]);
+                            c[u] = ok ? c[u] : 0;
+                            v[u] = ok ? v[u] : T(0);
+                        }
+                    }
+                    __syncwarp();
+                    if (rel > released) {
+                        released = rel;
+                        if (lane == 0) progress[warp] = rel;
+                    }
+#pragma unroll
+                    for (int u = 0; u < RG_UNROLL; ++u) g[u] = __ldg(vec + c[u]);
+                } else {
+#pragma unroll
+                    for (int u = 0; u < RG_UNROLL; ++u) v[u] = g[u] = T(0);
+                }
+                int e1 = e_next;
+                int e2 = nfin > 1 ? __shfl_sync(FULLM, wend, jb + 1) : 0x7fffffff;
+                int e3 = nfin > 2 ? __shfl_sync(FULLM, wend, jb + 2) : 0x7fffffff;
+                if (nfin < 1) e1 = 0x7fffffff;
+                T s0 = T(0), s1 = T(0), s2 = T(0);  // this lane's shares of the rows that end here, in order
+                int nclosed = 0;
+#pragma unroll
+                for (int u = 0; u < RG_UNROLL; ++u) {
+                    const int gend = S0 + 32 * (u + 1);
+                    if (e1 > gend) {
+                        acc = fma(v[u], g[u], acc);  // the whole group lies inside the open row
+                    } else {
+                        const int pos = S0 + 32 * u + lane;
+                        const T prod = v[u] * g[u];
+                        bool used = false;
+#pragma unroll
+                        for (int k = 0; k < 3; ++k) {
+                            if (e1 <= gend) {  // a row ends inside (or right before / at the end of) this group
+                                if (!used && pos < e1) {
+                                    acc += prod;
+                                    used = true;
+                                }
+                                if (nclosed == 0) s0 = acc;
+                                else if (nclosed == 1) s1 = acc;
+                                else s2 = acc;
+                                ++nclosed;
+                                acc = T(0);
+                                e1 = e2;
+                                e2 = e3;
+                                e3 = 0x7fffffff;
+                            }
+                        }
+                        if (!used) acc += prod;
+                    }
+                }
+                if (nfin >= 1) {
+                    any_end = true;
+                    park_head(warp_sum(s0), jb);
+                }
+                if (nfin >= 2) {
+                    const T tot = warp_sum(s1);
+                    if (lane == jb + 1) row_epilogue<T, MODE>(wrow + jb + 1, tot, q1, q2, q3, q4, out, out2, lambda, omap, racc);
+                }
+                if (nfin >= 3) {
+                    const T tot = warp_sum(s2);
+                    if (lane == jb + 2) row_epilogue<T, MODE>(wrow + jb + 2, tot, q1, q2, q3, q4, out, out2, lambda, omap, racc);
+                }
+                jb += nfin;
+            } else {
+                // ---- many row ends in one segment (runs of empty rows, very short rows): compact loop, one group at a time ------
+#pragma unroll 1
+                for (int u = 0; u < RG_UNROLL; ++u) {
+                    const int gend = S0 + 32 * (u + 1);
+                    const int pos = S0 + 32 * u + lane;
+                    T prod = T(0);
+                    if (has_data) {
+                        const bool ok = pos >= F && pos < S1;
+                        int c;
+                        T vv;
+                        ring_get(S.d, p0 + 32 * u, c, vv);
+                        prod = ok ? vv * __ldg(vec + (ok ? c : 0)) : T(0);
+                    }
+                    bool used = false;
+                    while (e_next <= gend) {
+                        if (!used && pos < e_next) {
+                            acc += prod;
+                            used = true;
+                        }
+                        const T tot = warp_sum(acc);
+                        if (!any_end) {
+                            any_end = true;
+                            park_head(tot, jb);
+                        } else if (lane == jb) {
+                            row_epilogue<T, MODE>(wrow + jb, tot, q1, q2, q3, q4, out, out2, lambda, omap, racc);
+                        }
+                        acc = T(0);
+                        const int e_cur = e_next;
+                        ++jb;
+                        for (;;) {  // the rows that follow and end at the same place are empty: their lanes finish them together
+                            if (jb == 32) {  // window used up: slide it
+                                wrow += 32;
+                                wend = load_window(wrow);
+                                jb = 0;
+                                if (wend <= S1) row_operands_pinned<T, MODE>(wrow + lane, p1, p2, p3, out, q1, q2, q3, q4);
+                            }
+                            const unsigned same = __ballot_sync(FULLM, lane >= jb && wend == e_cur);
+                            const int run = __popc(same);  // (row ends do not decrease: the lanes form a run starting at jb)
+                            if (run == 0) break;
+                            if ((same >> lane) & 1u) row_epilogue<T, MODE>(wrow + lane, T(0), q1, q2, q3, q4, out, out2, lambda, omap, racc);
+                            jb += run;
+                            if (jb < 32) break;
+                        }
+                        e_next = __shfl_sync(FULLM, wend, jb);
+                    }
+                    if (!used) acc += prod;
+                }
+                __syncwarp();
+                if (has_data && rel > released) {
+                    released = rel;
+                    if (lane == 0) progress[warp] = rel;
+                }
+            }
+            // what follows the last row end belongs to a row that goes on: hand it to the next segment
+            T tail = warp_sum(acc);
+            if (!any_end) tail = carry_of(sg) + tail;  // no row ended here: the open row's sum so far passes through
+            if (lane == 0) CarrySlot<T>::put(&carry[sg % RG_NCARRY], tail, sg + 1);
+            flush_head();  // (deferring this to the warp's next segment deadlocked at config 3's size: profiles/r02j_segments.md)
+            PROF_ADD(1, clock64() - ac0);
+            // the window for this warp's next segment was loaded at the start of this one
+            wrow = wrow_next;
+            wend = wend_next;
+        }
+        if (head_pending) {  // the row parked by this warp's last segment
+            T cv = T(0);
+            if (head_seg > 0) {
+                const int slot = (head_seg - 1) % RG_NCARRY;
+                const long long t0 = clock64();
+                while (!CarrySlot<T>::get(&carry[slot], head_seg, cv)) {
+                    __nanosleep(20);
+                    if (clock64() - t0 > RG_TIMEOUT) __trap();
+                }
+            }
+            if (lane == head_lane) row_epilogue<T, MODE>(head_row, cv + head_sum, hq1, hq2, hq3, hq4, out, out2, lambda, omap, racc);
+        }
+        __syncwarp();
+        if (lane == 0) progress[warp] = ntiles;
+        PROF_ADD(2, clock64() - ct0);
+        PROF_FLUSH(0);
+        PROF_FLUSH(1);
+        PROF_FLUSH(2);
+        PROF_FLUSH(3);
     } else {
     // ---- consumers, G >= 4 --------------------------------------------------------------------------------------------------
     // All positions below are element offsets relative to `base` and fit an int (a CTA's range is < 2^31 elements).
@@ -636,11 +984,12 @@ sup_status sup_stream_plan(sup_ctx* h, const CsrD& M, int64_t r0, int64_t r1, bo
     const double avg = double(ends[1] - ends[0]) / double(r1 - r0);
     int G = 4;
     while (G < 32 && avg * (32.0 / G) > 960.0) G <<= 1;
+    if (avg >= RG_SEG_MIN_AVG && avg <= 2048.0) G = 1;  // rows of hundreds of entries: segments of the stream instead of rows
     const int forced = forward ? h->lanes_fwd : h->lanes_bwd;
     if (forced >= 0) G = forced;
     const int64_t cap = int64_t(RG_STAGES_MIN - 2) * RG_TILE;
-    while (G < 32 && G > 0 && int64_t(mx_h) * (32 / G) > cap) G <<= 1;
-    if (G != 0 && (avg > 2048.0 || int64_t(mx_h) * (G >= 32 ? 1 : 32 / G) > cap)) G = 0;  // long rows: the whole CTA per row, no length limit
+    while (G < 32 && G > 1 && int64_t(mx_h) * (32 / G) > cap) G <<= 1;
+    if (G > 1 && (avg > 2048.0 || int64_t(mx_h) * (G >= 32 ? 1 : 32 / G) > cap)) G = 0;  // long rows: the whole CTA per row, no length limit
     out->max_row = int64_t(mx_h);
     out->part = static_cast<const int64_t*>(table);
     out->nb = nb;
@@ -677,6 +1026,7 @@ static void launch_staged_d(sup_ctx* h, const StreamPlan& sp, const CsrD& M, con
         case 16: launch_staged_g<T, MODE, 16, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap, red_out); break;
         case 64: launch_staged_g<T, MODE, 64, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap, red_out); break;
         case 0: launch_staged_g<T, MODE, 0, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap, red_out); break;
+        case 1: launch_staged_g<T, MODE, 1, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap, red_out); break;
         default: launch_staged_g<T, MODE, 32, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap, red_out); break;
     }
 }

@@ -666,14 +666,16 @@ def test_restarted_perturbations(dtype):
 
 
 @pytest.mark.parametrize("dtype", [0, 1])
-@pytest.mark.parametrize("name", ["cfg4_small", "ct_ragged", "cfg5_k16"])
-def test_long_row_mode_of_the_staged_kernels(name, dtype):
-    """The whole-CTA-per-row mode (chosen for rows of thousands of nonzeros: config 4's A^T at full size) forced on both
-    products of small problems, including rows shorter than a piece, empty rows and rows spanning several ring tiles."""
+@pytest.mark.parametrize("lanes", [0, 1, 64])
+@pytest.mark.parametrize("name", ["cfg4_small", "ct_ragged", "cfg5_k16", "cfg2"])
+def test_long_row_mode_of_the_staged_kernels(name, lanes, dtype):
+    """The whole-CTA-per-row mode (lanes = 0; chosen for rows of thousands of nonzeros: config 4's A^T at full size), the segment
+    mode (lanes = 1) and the warp-pair mode (64) forced on both products of small problems, including rows shorter than a piece,
+    empty rows and rows spanning several ring tiles."""
     sup = _sup()
     P = problem(name)
     H = make_handle(P, dtype, blocks=False)
-    sup.sup_set_row_mode(H, 0, 0)
+    sup.sup_set_row_mode(H, lanes, lanes)
     O = Oracle.from_problem(P)
     x = xdev(P, dtype)
     xo = P.x0.astype(np.float64)
