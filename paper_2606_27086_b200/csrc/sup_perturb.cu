@@ -19,7 +19,7 @@
 // that candidate is accepted (the common case once beta is small) the next reduction step can start at once:
 // 1 + N grid-wide passes per phase instead of 1 + 2N.  A rejected first candidate falls back to evaluating the next
 // SUP_TRIAL_BATCH candidates per pass, decided strictly in order: the trial / decision / l sequence is exactly
-// Algorithm 1's.  DOSE ||D x||^2 with g = 2 D^T (D x) (A-15) keeps its own branch (closed-form trial loop).
+// Algorithm 1's.  The dose objective ||D x||^2 (A-15) and f_Mean run as launch sequences on the product kernels (sup_algos.cu).
 // Objective terms, norms and beta are fp64 in both modes.
 #include <math.h>
 #include <stdlib.h>
@@ -63,34 +63,6 @@ struct PArgs {
 };
 
 // ---- grid barrier (all CTAs co-resident by cooperative launch) ----------------------------------------------
-__device__ __forceinline__ void grid_barrier(DevState* st) {
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        __threadfence();
-        volatile unsigned* gen_p = &st->bar_gen;
-        const unsigned gen = *gen_p;
-        const unsigned arrived = atomicAdd(&st->bar_count, 1u);
-        if (arrived == gridDim.x - 1) {
-            st->bar_count = 0;
-            __threadfence();
-            atomicExch(&st->bar_gen, gen + 1u);
-        } else {
-            unsigned spins = 0;
-            while (*gen_p == gen) {
-#ifndef SUP_BARRIER_NOSLEEP
-                __nanosleep(64);
-#endif
-                if (++spins > BARRIER_SPIN_LIMIT) {  // never hang the device: flag and fall through
-                    atomicOr(&st->fault, 1);
-                    break;
-                }
-            }
-        }
-        __threadfence();
-    }
-    __syncthreads();
-}
-
 // Grid barrier fused with the second stage of a reduction.  On entry v[0..NV) are this THREAD's shares; every CTA sums
 // its threads' shares, stores the NV sums to partials[b * stride + blockIdx.x] and arrives.  The last CTA to arrive adds
 // the partials of all CTAs in index order (which CTA does it changes nothing: same numbers, same order), publishes the
@@ -206,13 +178,6 @@ __device__ __forceinline__ void cta_sum_batch(double* v) {
     __syncthreads();
 #pragma unroll
     for (int b = 0; b < B; ++b) v[b] = totb[b];
-}
-
-// every CTA sums the same gridDim.x partials in the same order -> identical value everywhere
-__device__ __forceinline__ double reduce_partials(const double* partials) {
-    double s = 0.0;
-    for (int q = threadIdx.x; q < int(gridDim.x); q += SUP_THREADS) s += __ldcg(partials + q);
-    return cta_sum(s);
 }
 
 template <typename T>
@@ -363,28 +328,6 @@ __device__ double dose_share(const PArgs<T>& A, double coef, bool store_r) {
         if (valid && gl == 0) {
             acc += double(r) * double(r);
             if (store_r) A.r[i] = r;
-        }
-    }
-    return acc;
-}
-
-// q = D g (stored), returns this thread's share of sum q^2: with it a trial step needs no matrix pass,
-//   f(x - c g) = ||r - c q||^2 = f(x) - c ||g||^2 + c^2 ||q||^2     (r = D x, g = 2 D^T r  =>  <r, q> = ||g||^2 / 2)
-template <typename T>
-__device__ double dose_q_share(const PArgs<T>& A) {
-    const int G = A.g_d;
-    const int gl = threadIdx.x % G, lane = threadIdx.x & 31;
-    const int64_t gid = (int64_t(blockIdx.x) * blockDim.x + threadIdx.x) / G;
-    const int64_t ngroups = (int64_t(gridDim.x) * blockDim.x) / G;
-    double acc = 0.0;
-    for (int64_t i0 = gid - lane / G; i0 < A.md; i0 += ngroups) {
-        const int64_t i = i0 + lane / G;
-        const bool valid = i < A.md;
-        const int64_t s = valid ? A.d_rowptr[i] : 0, e = valid ? A.d_rowptr[i + 1] : 0;
-        const T qv = coop_row_dot<T, false>(A.d_val, A.d_col, s, e, A.g, nullptr, 0.0, gl, G);
-        if (valid && gl == 0) {
-            acc += double(qv) * double(qv);
-            A.q[i] = qv;
         }
     }
     return acc;
@@ -625,28 +568,6 @@ __device__ void tv1d_pass(const PArgs<T>& A, const double* coef, T* __restrict__
     S = acc;
 }
 
-template <typename T>
-__device__ double dose_grad_share(const PArgs<T>& A) {
-    // r = D x has been stored by dose_share(store_r) and a grid barrier passed; g_j = 2 sum_i D_ij r_i over row j of D^T
-    const int G = A.g_dt;
-    const int gl = threadIdx.x % G, lane = threadIdx.x & 31;
-    const int64_t gid = (int64_t(blockIdx.x) * blockDim.x + threadIdx.x) / G;
-    const int64_t ngroups = (int64_t(gridDim.x) * blockDim.x) / G;
-    double acc = 0.0;
-    for (int64_t j0 = gid - lane / G; j0 < A.n; j0 += ngroups) {
-        const int64_t j = j0 + lane / G;
-        const bool valid = j < A.n;
-        const int64_t s = valid ? A.dt_rowptr[j] : 0, e = valid ? A.dt_rowptr[j + 1] : 0;
-        const T u = coop_row_dot<T, false>(A.dt_val, A.dt_col, s, e, A.r, nullptr, 0.0, gl, G);
-        if (valid && gl == 0) {
-            const T gs = T(2) * u;
-            A.g[j] = gs;
-            acc += double(gs) * double(gs);
-        }
-    }
-    return acc;
-}
-
 // ---- the perturbation phase, TV objectives ---------------------------------------------------------------------
 // Buffers: (xc, gc) hold the current inner iterate x^{k,n} and its gradient, (xo, go) receive the candidate z and its gradient
 // (a tile's halo needs the neighbours' x and g, so a pass cannot work in place); on acceptance the pairs swap.
@@ -840,123 +761,6 @@ __global__ void __launch_bounds__(SUP_THREADS) k_perturb_tv(PArgs<T> Ain) {
     }
 }
 
-// ---- the perturbation phase, dose objective ------------------------------------------------------------------------
-template <typename T, int OBJ>
-__global__ void __launch_bounds__(SUP_THREADS) k_perturb(PArgs<T> Ain) {
-    static_assert(OBJ == SUP_OBJ_DOSE, "the TV objectives run in k_perturb_tv");
-    const PArgs<T>& A = Ain;
-    if (*(volatile int*)&Ain.st->stop) return;
-    T* xc = Ain.x;
-    T* gc = Ain.g;
-    auto view = [&]() { return Ain; };
-    DevState* st = A.st;
-    long long ell = *(volatile long long*)&st->ell;
-    double apow = *(volatile double*)&st->apow;  // a^ell, running product
-    const long long k = *(volatile long long*)&st->k;
-    long long ndec = *(volatile long long*)&st->n_dec;
-    long long trials = 0;
-    if (A.n_restart > 0 && k > 0 && k % A.n_restart == 0) {
-        ell = k / A.n_restart;
-        apow = 1.0;
-        for (long long q = 0; q < ell; ++q) apow *= A.a;
-    }
-    int warn = 0, fault = 0;
-    int slot = 0;
-    double* P0 = A.partials;
-    double* P1 = A.partials + SUP_MAX_PARTIALS;
-
-    // fx = f(x): r = D x is stored on the way and then carried, r <- r - c q, through the phase
-    double sh = cta_sum(dose_share(view(), 0.0, true));
-    if (threadIdx.x == 0) P0[blockIdx.x] = sh;
-    grid_barrier(st);
-    double fx = reduce_partials(P0);
-    slot = 1;
-    if (!isfinite(fx)) fault |= 2;
-    {
-        // Quadratic objective: with q = D g the objective along the step is the closed form above, so the trial loop is
-        // scalar work and a reduction step costs two matrix passes (g = 2 D^T r, q = D g) instead of three or more.
-        for (int nred = 0; nred < A.N; ++nred) {
-            double* P = slot ? P1 : P0;
-            slot ^= 1;
-            sh = cta_sum(dose_grad_share(view()));
-            if (threadIdx.x == 0) P[blockIdx.x] = sh;
-            grid_barrier(st);
-            const double s2 = reduce_partials(P);
-            const double s = sqrt(s2);
-            P = slot ? P1 : P0;
-            slot ^= 1;
-            sh = cta_sum(dose_q_share(view()));
-            if (threadIdx.x == 0) P[blockIdx.x] = sh;
-            grid_barrier(st);
-            const double q2 = reduce_partials(P);
-            bool accepted = false;
-            long long jloc = 0;
-            double cf = 0.0, fz_acc = fx;
-            for (int trial = 0; trial < SUP_J_MAX && !accepted; ++trial) {
-                double ap = apow;
-                if (A.policy != SUP_STEP_PER_TRIAL) {
-                    ap = 1.0;
-                    for (long long q = 0; q < k + jloc; ++q) ap *= A.a;
-                }
-                const double c = s > 0.0 ? (A.beta0 * ap) / s : 0.0;
-                const double fz = c == 0.0 ? fx : fx - c * s2 + c * c * q2;
-                ++ell;
-                apow *= A.a;
-                ++jloc;
-                ++trials;
-                const bool acc = fz <= fx;
-                if (blockIdx.x == 0 && threadIdx.x == 0) {
-                    if (A.decisions && ndec < A.cap) A.decisions[ndec] = acc ? 1 : 0;
-                    if (A.decision_f && ndec < A.cap) {
-                        A.decision_f[2 * ndec] = fz;
-                        A.decision_f[2 * ndec + 1] = fx;
-                    }
-                }
-                ++ndec;
-                if (acc) {
-                    accepted = true;
-                    cf = c;
-                    fz_acc = fz;
-                }
-            }
-            if (accepted && cf != 0.0) {
-                const int64_t tid = int64_t(blockIdx.x) * blockDim.x + threadIdx.x, nth = int64_t(gridDim.x) * blockDim.x;
-                for (int64_t j = tid; j < A.n; j += nth) xc[j] = T(zval(xc, gc, cf, j));
-                double rr = 0.0;
-                for (int64_t i = tid; i < A.md; i += nth) {
-                    const T rn = T(zval(A.r, A.q, cf, i));  // r <- round_T(r - c q)
-                    A.r[i] = rn;
-                    rr += double(rn) * double(rn);
-                }
-                P = slot ? P1 : P0;
-                slot ^= 1;
-                sh = cta_sum(rr);
-                if (threadIdx.x == 0) P[blockIdx.x] = sh;
-                grid_barrier(st);  // x^{k,n+1} and r visible to everyone before the next gradient
-                fx = reduce_partials(P);
-            } else if (accepted) {
-                fx = fz_acc;
-            } else {
-                warn |= 1;  // A-12: step skipped
-            }
-            if (*(volatile int*)&st->fault & 1) break;
-        }
-    }
-    if (A.xg)  // keep the gather mirror of x in step (element-wise)
-        for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q < A.n; q += int64_t(gridDim.x) * blockDim.x)
-            A.xg[sup_gmap(A.xmap, int(q))] = xc[q];
-    if (blockIdx.x == 0 && threadIdx.x == 0) {
-        st->ell = ell;
-        st->apow = apow;
-        st->n_dec = ndec;
-        st->n_trials += trials;
-        st->sweep_trials += trials;
-        st->f = fx;
-        if (warn) atomicOr(&st->warn, warn);
-        if (fault) atomicOr(&st->fault, fault);
-    }
-}
-
 // ---- stand-alone objective value (sup_objective, trace mode) -------------------------------------------------
 template <typename T, int OBJ>
 __global__ void __launch_bounds__(SUP_THREADS) k_objective(PArgs<T> A) {
@@ -1020,7 +824,6 @@ static const void* perturb_kernel(int objective) {
         case SUP_OBJ_TV2D: return reinterpret_cast<const void*>(&k_perturb_tv<T, SUP_OBJ_TV2D>);
         case SUP_OBJ_TV1D: return reinterpret_cast<const void*>(&k_perturb_tv<T, SUP_OBJ_TV1D>);
         case SUP_OBJ_TV3D: return reinterpret_cast<const void*>(&k_perturb_tv<T, SUP_OBJ_TV3D>);
-        case SUP_OBJ_DOSE: return reinterpret_cast<const void*>(&k_perturb<T, SUP_OBJ_DOSE>);
     }
     return nullptr;
 }
@@ -1048,7 +851,10 @@ int sup_perturb_grid(sup_ctx* h, int objective) {
 
 sup_status sup_launch_perturb(sup_ctx* h, void* x, const PerturbParams& pp) {
     if (pp.objective == SUP_OBJ_MEAN) return sup_launch_perturb_mean(h, x, pp);
-    if (pp.objective == SUP_OBJ_DOSE && h->D.plan.ok && h->DT.plan.ok) return sup_launch_perturb_dose_staged(h, x, pp);
+    if (pp.objective == SUP_OBJ_DOSE) {
+        if (!(h->D.plan.ok && h->DT.plan.ok)) return sup_fail(h, SUP_ERR_STATE, "the dose perturbation runs on the staged product kernels (sup_set_row_mode)");
+        return sup_launch_perturb_dose_staged(h, x, pp);
+    }
     const int grid = sup_perturb_grid(h, pp.objective);
     if (grid < 1) return sup_fail(h, SUP_ERR_CUDA, "perturbation kernel cannot be made resident");
     cudaLaunchConfig_t cfg = {};
