@@ -44,6 +44,7 @@ def _L():
         _lib.orc_mean.restype = ctypes.c_double
         _lib.orc_tv3d.restype = ctypes.c_double
         _lib.orc_perturb_phase3.restype = ctypes.c_int64
+        _lib.orc_perturb_adaptive_phase.restype = ctypes.c_int64
         _lib.orc_superiorize_ex.restype = ctypes.c_int
         _lib.orc_perturb_phase.restype = ctypes.c_int64
         _lib.orc_setup.restype = ctypes.c_int
@@ -60,7 +61,7 @@ _i64, _dbl, _int = ctypes.c_int64, ctypes.c_double, ctypes.c_int
 
 class _RunOpt(ctypes.Structure):  # run_opt_t of sup_oracle.c
     _fields_ = [("algorithm", _int), ("stop_enabled", _int), ("prox_tol", _dbl), ("dprox_tol", _dbl), ("n_consec", _int),
-                ("dobj_tol", _dbl), ("n_restart", _i64), ("nz", _i64)]
+                ("dobj_tol", _dbl), ("n_restart", _i64), ("nz", _i64), ("step_rule", _int), ("f_ref", _dbl), ("f_ref_shrink", _dbl)]
 
 
 class Oracle:
@@ -204,6 +205,22 @@ class Oracle:
         return dict(x=x, ell=ell_c.value, trials=int(t), decisions=dec[:nd].copy(), margins=mar[:nd].copy(), fx=fx.value,
                     warn=warn.value)
 
+    def perturb_adaptive(self, x, N, f_ref, shrink=0.5, kind=None, shape=None, cap=1 << 16):
+        """One perturbation phase with Eq. 11's step size (reading A-30).
+        Returns dict(x, f_ref (updated), steps, decisions, fx)."""
+        kind = self.objective if kind is None else kind
+        shape = self.shape if shape is None else shape
+        x = np.array(x, np.float64)
+        dec = np.zeros(cap, np.int8)
+        ndec = _i64(0)
+        fr = _dbl(float(f_ref))
+        fx = _dbl(0.0)
+        oa = self._obj_args(kind, shape)
+        nz = int(shape[0]) if kind == "tv3d" else 0
+        t = _L().orc_perturb_adaptive_phase(_i64(self.n), _int(OBJ_KIND[kind]), _i64(nz), *oa[1:], _p(x), _int(N), ctypes.byref(fr),
+                                            _dbl(shrink), _p(dec), _i64(cap), ctypes.byref(ndec), ctypes.byref(fx))
+        return dict(x=x, f_ref=fr.value, steps=int(t), decisions=dec[: min(ndec.value, cap)].copy(), fx=fx.value)
+
     def superiorize(self, x0, n_iter, N, beta0, a, lam=1.0, policy=PER_TRIAL, block=False, snapshots=(), ell0=0,
                     forced=None, kind=None, shape=None, cap=1 << 22, k0=0, n_restart=0):
         """Algorithm 1 for n_iter sweeps (absolute sweep indices k0 .. k0+n_iter-1; k0 only matters to PER_SWEEP).
@@ -241,10 +258,12 @@ class Oracle:
                     warn=warn)
 
     def run(self, x0, n_iter, N=0, beta0=1.0, a=0.99, lam=1.0, algorithm="sim", policy=PER_TRIAL, ell0=0, k0=0, kind=None,
-            shape=None, n_restart=0, stop=None, forced=None, cap=1 << 22):
+            shape=None, n_restart=0, stop=None, forced=None, cap=1 << 22, adaptive=None):
         """Algorithm 1 through orc_superiorize_ex: `algorithm` in {'sim', 'block', 'drop', 'emr'} (Table A.5), any objective
         (incl. 'mean', 'tv3d'), and the paper's stopping rule when stop = dict(prox_tol, dprox_tol, n_consec, dobj_tol)
         (reading A-25).  One call, no snapshots (the rule's counters live inside the call).
+        adaptive = dict(f_ref, shrink): Eq. 11's step size instead of the power law (reading A-30); the updated reference
+        comes back as 'f_ref'.
         Returns dict(x, ell, n_done, stop_reason, trace[n_done,4], decisions, margins, warn)."""
         kind = self.objective if kind is None else kind
         shape = self.shape if shape is None else shape
@@ -261,6 +280,8 @@ class Oracle:
         if stop is not None:
             opt.prox_tol, opt.dprox_tol = float(stop.get("prox_tol", 1e-6)), float(stop.get("dprox_tol", 1e-8))
             opt.n_consec, opt.dobj_tol = int(stop.get("n_consec", 5)), float(stop.get("dobj_tol", 1e-6))
+        if adaptive is not None:
+            opt.step_rule, opt.f_ref, opt.f_ref_shrink = 1, float(adaptive["f_ref"]), float(adaptive.get("shrink", 0.5))
         n_done, reason = _int(0), _int(0)
         warn = _L().orc_superiorize_ex(
             _i64(self.m), _i64(self.n), _p(self.rowptr), _p(self.col), _p(self.val), _p(self.lb), _p(self.ub), _p(self.w),
@@ -270,4 +291,4 @@ class Oracle:
             ctypes.byref(n_done), ctypes.byref(reason))
         nd = min(ndec.value, cap)
         return dict(x=x, ell=ell.value, n_done=n_done.value, stop_reason=reason.value, trace=trace[: n_done.value].copy(),
-                    decisions=dec[:nd].copy(), margins=mar[:nd].copy(), warn=warn)
+                    decisions=dec[:nd].copy(), margins=mar[:nd].copy(), warn=warn, f_ref=opt.f_ref)

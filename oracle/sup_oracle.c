@@ -12,14 +12,16 @@
  * of two fp64 numbers is exact in binary128, so the result is the correctly rounded fp64 value of the sum and
  * does not depend on summation order (reading A-22: the perturbed iteration amplifies last-bit
  * differences by orders of magnitude per sweep, so "the sum" has to be one well-defined number).
- * Readings of the paper where it is silent/garbled are listed in DESIGN.md ("Readings", A-1 .. A-27) and
+ * Readings of the paper where it is silent/garbled are listed in DESIGN.md ("Readings", A-1 .. A-30) and
  * named at the line that uses them.
  *
  * Parity pins (tests/test_oracle_pins.py): every function below is pinned by closed forms, invariants,
  * library special cases or brute force -- the hyperslab sweeps, proximities, TV2D/TV1D/dose objectives and Algorithm 1
  * (round 1), and DROP / EMR (dense NumPy expression of Table A.5, exact line minimiser), f_Mean (linearity, exact
  * decrease -beta ||g||), TV3D (closed forms, finite differences, reduction to TV2D) and the stopping rule (replay from
- * the definition; never firing = bit-identical fixed run); nothing here is "parity unpinned".
+ * the definition; never firing = bit-identical fixed run), and Eq. 11's step (half-space projection: f lands on f_ref
+ * exactly for a linear f, Heron's square-root iteration for f = x^2).  PARITY UNPINNED: the f_ref update rule inside
+ * orc_perturb_adaptive (reading A-30) -- the paper only cites the rule, so no value of it can be checked against the paper.
  */
 #include <math.h>
 #include <stdint.h>
@@ -420,6 +422,44 @@ int64_t orc_perturb(int64_t n, const obj_t* O, double* x, int64_t* ell, int64_t 
     return trials;
 }
 
+/* ---- O-PERTURB-ADAPTIVE: the perturbation phase with the subgradient-projection step size of Eq. 11
+ * ("Nikazad et al. [7]"):
+ *      beta = 0                          if f(x) <= f_ref,
+ *      beta = (f(x) - f_ref) / ||g_f(x)||  if f(x) >  f_ref,
+ * used in Eq. 10 with v = -g/||g|| (A-6), i.e. x <- x - ((f(x) - f_ref)/||g||^2) g: the projection of x onto the half-space
+ * {y : f(x) + <g, y - x> <= f_ref}.  Eq. 11 DEFINES beta, so there is no trial loop, no accept test and no exponent l
+ * (reading A-30); N such steps per phase (N = 1 is the literal Eq. 10), each with f and g re-evaluated (A-7); a step with
+ * ||g|| = 0 is beta = 0.
+ * f_ref "is automatically updated throughout the iterations" (L108) by a rule the paper only cites.  Reading A-30 -- the
+ * part of this function that is PARITY UNPINNED against the paper (the rule is ours; the step itself is pinned):
+ *      if the phase started at a point with f(x^k) <= f_ref, then after the phase f_ref <- shrink * f(x^k), shrink in (0, 1]
+ *      (the iterate has reached the reference, so the reference is moved below it); otherwise f_ref is kept.
+ * decisions/n_dec: optional log, 1 = a step with beta > 0 was taken, 0 = beta = 0.  Returns the number of steps with beta > 0. */
+int64_t orc_perturb_adaptive(int64_t n, const obj_t* O, double* x, int N, double* f_ref, double shrink, double* g,
+                             int8_t* decisions, int64_t cap_dec, int64_t* n_dec, double* fx_out) {
+    const double f_start = obj_value(O, n, x);
+    double fx = f_start;
+    int64_t steps = 0;
+    for (int nred = 0; nred < N; ++nred) {
+        if (nred > 0) fx = obj_value(O, n, x);
+        obj_grad(O, n, x, g);
+        acc_t s_acc = 0;
+        for (int64_t j = 0; j < n; ++j) s_acc += (acc_t)g[j] * g[j];
+        const double s = sqrt((double)s_acc);
+        const int take = fx > *f_ref && s > 0.0;
+        if (take) {
+            const double beta = (fx - *f_ref) / s; /* Eq. 11 */
+            for (int64_t j = 0; j < n; ++j) x[j] = x[j] + beta * (-g[j] / s); /* Eq. 10's perturbation, v = -g/||g|| */
+            steps++;
+        }
+        if (decisions && *n_dec < cap_dec) decisions[*n_dec] = (int8_t)take;
+        (*n_dec)++;
+    }
+    if (f_start <= *f_ref) *f_ref = shrink * f_start;
+    if (fx_out) *fx_out = fx; /* f at the point the last step started from */
+    return steps;
+}
+
 /* ---- O-SUPERIORIZE: Algorithm 1, Eq. 10 (L91): for each sweep k the perturbation
  * phase comes first, then the feasibility-seeking operator T.  Runs sweeps k0 .. k0+n_iter-1 so that a caller can
  * take snapshots between calls (state = x, ell, k).
@@ -444,6 +484,9 @@ typedef struct {
     double dobj_tol;
     int64_t n_restart;
     int64_t nz; /* TV3D: shape = (nz, ny, nx) */
+    int step_rule;       /* 0: power law beta0 * a^l with the accept test (Alg. 1); 1: Eq. 11 (O-PERTURB-ADAPTIVE, A-30) */
+    double f_ref;        /* Eq. 11's reference value; UPDATED IN PLACE by the run (A-30) */
+    double f_ref_shrink; /* A-30's update factor */
 } run_opt_t;
 
 int orc_superiorize_ex(int64_t m, int64_t n, const int64_t* rowptr, const int32_t* col, const double* val,
@@ -452,7 +495,7 @@ int orc_superiorize_ex(int64_t m, int64_t n, const int64_t* rowptr, const int32_
                        int obj_kind, int64_t ny, int64_t nx, int64_t md, const int64_t* d_rowptr, const int32_t* d_col,
                        const double* d_val, double* x, int64_t* ell, int64_t k0, int n_iter, int N, double beta0,
                        double a, int policy, double* trace, int8_t* decisions, double* margins, int64_t cap_dec,
-                       int64_t* n_dec, const int8_t* forced, const run_opt_t* opt, int* n_done, int* stop_reason) {
+                       int64_t* n_dec, const int8_t* forced, run_opt_t* opt, int* n_done, int* stop_reason) {
     obj_t O = {obj_kind, ny, nx, md, d_rowptr, d_col, d_val, opt->nz};
     double* g = (double*)malloc(sizeof(double) * (size_t)n);
     double* z = (double*)malloc(sizeof(double) * (size_t)n);
@@ -473,7 +516,9 @@ int orc_superiorize_ex(int64_t m, int64_t n, const int64_t* rowptr, const int32_
          * sweep k = r * n_restart, r = 1, 2, ..., the exponent is reset to r ("l = 1 after the first restart, l = 2 after
          * the second"), which keeps sum beta finite: cycle r contributes at most beta0 a^r / (1 - a). */
         if (opt->n_restart > 0 && k > 0 && k % opt->n_restart == 0) *ell = k / opt->n_restart;
-        if (perturbed)
+        if (perturbed && opt->step_rule == 1)
+            trials = orc_perturb_adaptive(n, &O, x, N, &opt->f_ref, opt->f_ref_shrink, g, decisions, cap_dec, n_dec, NULL);
+        else if (perturbed)
             trials = orc_perturb(n, &O, x, ell, k, N, beta0, a, policy, g, z, decisions, margins, cap_dec, n_dec,
                                  forced, &warn, NULL);
         switch (opt->algorithm) {
@@ -518,7 +563,7 @@ int orc_superiorize(int64_t m, int64_t n, const int64_t* rowptr, const int32_t* 
                     const double* d_val, double* x, int64_t* ell, int64_t k0, int n_iter, int N, double beta0,
                     double a, int policy, double* trace, int8_t* decisions, double* margins, int64_t cap_dec,
                     int64_t* n_dec, const int8_t* forced, int64_t n_restart) {
-    run_opt_t opt = {n_blocks > 0 ? 1 : 0, 0, 0.0, 0.0, 0, 0.0, n_restart, 0};
+    run_opt_t opt = {n_blocks > 0 ? 1 : 0, 0, 0.0, 0.0, 0, 0.0, n_restart, 0, 0, 0.0, 0.0};
     return orc_superiorize_ex(m, n, rowptr, col, val, lb, ub, w, rho, d, lo, hi, lambda, n_blocks, block_rowptr, obj_kind,
                               ny, nx, md, d_rowptr, d_col, d_val, x, ell, k0, n_iter, N, beta0, a, policy, trace,
                               decisions, margins, cap_dec, n_dec, forced, &opt, NULL, NULL);
@@ -550,5 +595,17 @@ int64_t orc_perturb_phase3(int64_t n, int obj_kind, int64_t nz, int64_t ny, int6
                             warn, fx_out);
     free(g);
     free(z);
+    return t;
+}
+
+/* stand-alone adaptive phase (what sup_perturb_adaptive is checked against); nz = 0 unless TV3D */
+int64_t orc_perturb_adaptive_phase(int64_t n, int obj_kind, int64_t nz, int64_t ny, int64_t nx, int64_t md,
+                                   const int64_t* d_rowptr, const int32_t* d_col, const double* d_val, double* x, int N,
+                                   double* f_ref, double shrink, int8_t* decisions, int64_t cap_dec, int64_t* n_dec,
+                                   double* fx_out) {
+    obj_t O = {obj_kind, ny, nx, md, d_rowptr, d_col, d_val, nz};
+    double* g = (double*)malloc(sizeof(double) * (size_t)n);
+    int64_t t = orc_perturb_adaptive(n, &O, x, N, f_ref, shrink, g, decisions, cap_dec, n_dec, fx_out);
+    free(g);
     return t;
 }

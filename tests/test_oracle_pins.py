@@ -790,3 +790,99 @@ def test_stopping_rule_fires_where_the_definition_says():
             assert want < K, "the test system must trigger the rule"
             assert R["n_done"] == want and R["stop_reason"] == reason
             np.testing.assert_array_equal(R["x"], xs[want])
+
+
+# ------------------------------------------------------------------------------------------------
+# Eq. 11: the subgradient-projection step size; reading A-30
+def test_adaptive_step_lands_on_f_ref_for_a_linear_objective():
+    """x - ((f - f_ref)/||g||^2) g is the projection onto {y: f(x) + <g, y - x> <= f_ref}: for the linear f_Mean (Eq. 21) the
+    new point has f = f_ref exactly, it is the closest such point, and a second step (f = f_ref, not above) is beta = 0"""
+    rng = np.random.default_rng(21)
+    md, n = 9, 6
+    D = rng.uniform(0, 1, (md, n)) * (rng.random((md, n)) < 0.8)
+    rp, c, v = dense_to_csr(D)
+    O = make(np.eye(n), np.zeros(n), np.ones(n), dose=(rp, c, v, md), objective="mean")
+    x = rng.uniform(1, 2, n)
+    g = D.T @ np.ones(md) / md
+    f0 = g @ x
+    f_ref = 0.4 * f0
+    R = O.perturb_adaptive(x, 1, f_ref)
+    assert R["steps"] == 1 and list(R["decisions"]) == [1] and R["f_ref"] == f_ref  # started above the reference: kept
+    assert g @ R["x"] == pytest.approx(f_ref, rel=1e-13)
+    np.testing.assert_allclose(R["x"], x - (f0 - f_ref) / (g @ g) * g, rtol=1e-13)
+    # minimal distance: |x' - x| = (f0 - f_ref)/||g|| = beta of Eq. 11
+    assert np.linalg.norm(R["x"] - x) == pytest.approx((f0 - f_ref) / np.linalg.norm(g), rel=1e-13)
+    # N = 3: the later steps start at f ~ f_ref: whatever rounding leaves, they move x by < 1e-15 relative
+    R3 = O.perturb_adaptive(x, 3, f_ref)
+    np.testing.assert_allclose(R3["x"], R["x"], rtol=1e-14)
+
+
+def test_adaptive_step_on_x_squared_is_herons_iteration():
+    """f(x) = ||D x||^2 with D = (1): Eq. 11's step is x - (x^2 - f_ref)/(2x) = (x + f_ref/x)/2 -- the Babylonian square-root
+    iteration, whose iterates from x = 3, f_ref = 2 are the rationals 11/6, 193/132, 72097/50952"""
+    O = Oracle(1, 1, np.array([0, 1]), np.array([0], np.int32), np.array([1.0]), np.array([-INF]), np.array([INF]),
+               np.array([-INF]), np.array([INF]), dose=(np.array([0, 1]), np.array([0], np.int32), np.array([1.0]), 1), objective="dose")
+    want = [11 / 6, 193 / 132, 72097 / 50952]
+    for N in (1, 2, 3):
+        R = O.perturb_adaptive(np.array([3.0]), N, 2.0)
+        assert R["x"][0] == pytest.approx(want[N - 1], rel=1e-15) and R["steps"] == N and R["f_ref"] == 2.0
+    R = O.perturb_adaptive(np.array([3.0]), 8, 2.0)
+    assert R["x"][0] == pytest.approx(np.sqrt(2.0), rel=1e-15)
+    assert R["fx"] == pytest.approx(2.0, rel=1e-14)  # f at the point the last step started from
+    # with a general D: one step, dense NumPy restatement
+    rng = np.random.default_rng(5)
+    D = rng.normal(size=(7, 4))
+    rp, c, v = dense_to_csr(D)
+    O = make(np.eye(4), np.zeros(4), np.ones(4), dose=(rp, c, v, 7), objective="dose")
+    x = rng.normal(size=4)
+    f, g = np.sum((D @ x) ** 2), 2 * D.T @ (D @ x)
+    R = O.perturb_adaptive(x, 1, 0.3 * f)
+    np.testing.assert_allclose(R["x"], x - (0.7 * f) / (g @ g) * g, rtol=1e-13)
+
+
+def test_adaptive_step_is_zero_at_or_below_the_reference_and_moves_the_reference():
+    """Eq. 11, first case: f(x) <= f_ref gives beta = 0 (x untouched, bitwise); reading A-30: the reference then becomes
+    shrink * f(x^k); a zero gradient is beta = 0 too; TV objectives go through the same step"""
+    rng = np.random.default_rng(2)
+    O = make(np.eye(12), np.zeros(12), np.ones(12), objective="tv2d", shape=(3, 4))
+    X = rng.uniform(0, 1, (3, 4))
+    f0 = O.objective_value(X.ravel())
+    for fr in (f0, 2 * f0):  # equality counts as "not above"
+        R = O.perturb_adaptive(X.ravel(), 2, fr, shrink=0.25)
+        np.testing.assert_array_equal(R["x"], X.ravel())
+        assert R["steps"] == 0 and list(R["decisions"]) == [0, 0] and R["f_ref"] == 0.25 * f0
+    # above the reference: the step of Eq. 11 with the oracle's own gradient, and f goes down for a small enough step
+    g = O.objective_grad(X.ravel())
+    fr = 0.95 * f0
+    R = O.perturb_adaptive(X.ravel(), 1, fr)
+    np.testing.assert_allclose(R["x"], X.ravel() - (f0 - fr) / (g @ g) * g, rtol=1e-13)
+    assert O.objective_value(R["x"]) < f0 and R["f_ref"] == fr
+    # constant image: TV gradient is 0 -> no step although f = 0 > f_ref = -1
+    C = np.full(12, 0.5)
+    R = O.perturb_adaptive(C, 1, -1.0)
+    np.testing.assert_array_equal(R["x"], C)
+    assert R["steps"] == 0 and R["f_ref"] == -1.0
+    # 1-D TV, by hand: x = (0, 2, 1): f = 3, g = (-1, 2, -1), ||g||^2 = 6; f_ref = 0 -> x - (3/6) g = (0.5, 1, 1.5)
+    O1 = make(np.eye(3), np.zeros(3), np.ones(3), objective="tv1d")
+    R = O1.perturb_adaptive(np.array([0.0, 2.0, 1.0]), 1, 0.0)
+    np.testing.assert_allclose(R["x"], [0.5, 1.0, 1.5], rtol=1e-15)
+
+
+def test_adaptive_rule_inside_algorithm_1_is_phase_then_sweep():
+    """Eq. 10 with Eq. 11: each iteration is the adaptive phase followed by the sweep, the reference carried across iterations"""
+    rng = np.random.default_rng(13)
+    A, lb, ub, _ = random_system(rng, 14, 12)
+    O = make(A, lb, ub, objective="tv2d", shape=(3, 4))
+    x0 = rng.uniform(0, 1, 12)
+    fr0 = 0.9 * O.objective_value(x0)
+    R = O.run(x0, 6, N=2, lam=1.3, adaptive=dict(f_ref=fr0, shrink=0.5))
+    x, fr = x0.copy(), fr0
+    steps = []
+    for k in range(6):
+        P = O.perturb_adaptive(x, 2, fr, shrink=0.5)
+        x, fr = O.sweep(P["x"], 1.3), P["f_ref"]
+        steps.append(P["steps"])
+    np.testing.assert_array_equal(R["x"], x)
+    assert R["f_ref"] == fr and R["ell"] == 0
+    np.testing.assert_array_equal(R["trace"][:, 2], steps)
+    assert sum(steps) > 0 and fr < fr0  # the reference was reached at least once and moved down
