@@ -73,6 +73,15 @@ typedef enum {
     SUP_STEP_PER_SWEEP = 1  /* literal Alg. 1: beta_{k,j} = beta0 * a^(k+j), j reset at every reduction step */
 } sup_step_policy;
 
+/* step-size rule of the perturbation phase */
+typedef enum {
+    SUP_RULE_POWER = 0,   /* beta = beta0 * a^l, trial loop with the accept test f(z) <= f(x) (Algorithm 1) */
+    SUP_RULE_ADAPTIVE = 1 /* Eq. 11: beta = 0 if f(x) <= f_ref, else (f(x) - f_ref)/||g_f(x)||; the step
+                             x - ((f(x) - f_ref)/||g||^2) g is taken without a trial loop, N times per phase, l is not used
+                             (N, beta0, a of the call: only N is read).  TV and dose objectives.  The update of f_ref is the
+                             reading DESIGN.md A-30 (the paper only cites the rule: parity unpinned for that part) */
+} sup_step_rule;
+
 /* what a workspace query is for */
 typedef enum { SUP_WS_CREATE = 0, SUP_WS_BLOCKS = 1, SUP_WS_DOSE = 2 } sup_ws_kind;
 
@@ -113,6 +122,11 @@ typedef struct {
     double dprox_tol;      /* paper's default 1e-8 */
     int n_consec;          /* paper's default 5 */
     double dobj_tol;       /* paper's default 1e-6 */
+    int step_rule;         /* sup_step_rule: how beta_k is chosen.  SUP_RULE_POWER (0): beta0 * a^l with the accept test (Alg. 1) */
+    double f_ref;          /* SUP_RULE_ADAPTIVE: Eq. 11's reference value at the start of the run (resume state: pass the f_ref
+                              sup_get_state reported) */
+    double f_ref_shrink;   /* SUP_RULE_ADAPTIVE: in (0, 1]; when a perturbation phase starts at f(x^k) <= f_ref the reference
+                              becomes f_ref_shrink * f(x^k) after the phase (A-30) */
 } sup_options;
 
 /* feasibility-seeking operators (PAPER.md Table A.5) */
@@ -134,6 +148,7 @@ typedef struct {
     int64_t n_done;      /* sweeps actually performed by the last sup_superiorize call (< n_iter iff the stopping rule fired) */
     int32_t stop_reason; /* 0: ran all sweeps; else 1 * (P <= prox_tol) + 2 * (n_consec small changes) + 4 * (objective change small) */
     double step;         /* EMR: the last relaxation factor ||p||^2 / ||M^(1/2) A p||^2 */
+    double f_ref;        /* SUP_RULE_ADAPTIVE: Eq. 11's reference value after the run */
 } sup_state;
 
 /* Bytes of workspace for `kind` on a matrix of the given shape (for SUP_WS_BLOCKS pass A's shape; for SUP_WS_DOSE
@@ -221,6 +236,12 @@ sup_status sup_perturb_dose(sup_handle h, void* x, int N, double beta0, double a
  * to sup_set_dose_matrix.  The objective is linear, its gradient (1/N_S) D_S^T 1 is formed once at sup_set_dose_matrix, and
  * every first trial is accepted: the phase is N axpy steps. */
 sup_status sup_perturb_mean(sup_handle h, void* x, int N, double beta0, double a, int64_t* ell);
+
+/* One perturbation phase with Eq. 11's step size (SUP_RULE_ADAPTIVE above): N steps
+ * x <- x - ((f(x) - f_ref)/||g||^2) g, each only while f(x) > *f_ref and g != 0.  objective: SUP_OBJ_TV1D / TV2D / TV3D (shape as
+ * in sup_options) or SUP_OBJ_DOSE.  *f_ref (HOST) is read and, by the rule of DESIGN.md A-30, updated.  x in place.
+ * Synchronises.  SUP_ERR_INVALID_ARG for other objectives, shrink outside (0, 1] or a non-finite *f_ref. */
+sup_status sup_perturb_adaptive(sup_handle h, void* x, int objective, const int64_t* shape, int N, double* f_ref, double shrink);
 
 /* Algorithm 1, Eq. 10 (L91): for k = k0 .. k0+n_iter-1: perturbation phase of N reduction steps
  * (beta = beta0 * a^l), then one sweep.  x in place.  N = 0 or objective NONE gives the basic algorithm.

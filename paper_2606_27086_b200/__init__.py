@@ -18,6 +18,7 @@ from .binding import (  # noqa: F401
     sup_get_state,
     sup_objective,
     sup_perturb_dose,
+    sup_perturb_adaptive,
     sup_perturb_mean,
     sup_project_drop,
     sup_project_emr,

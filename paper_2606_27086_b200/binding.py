@@ -34,12 +34,13 @@ class _Options(Structure):
                 ("step_policy", c_int), ("ell0", c_int64), ("k0", c_int64), ("trace_mode", c_int), ("trace", c_void_p),
                 ("decisions", c_void_p), ("decision_f", c_void_p), ("decisions_cap", c_int64), ("use_graph", c_int),
                 ("n_restart", c_int64), ("algorithm", c_int), ("stop_enabled", c_int), ("prox_tol", c_double),
-                ("dprox_tol", c_double), ("n_consec", c_int), ("dobj_tol", c_double)]
+                ("dprox_tol", c_double), ("n_consec", c_int), ("dobj_tol", c_double), ("step_rule", c_int), ("f_ref", c_double),
+                ("f_ref_shrink", c_double)]
 
 
 class _State(Structure):
     _fields_ = [("ell", c_int64), ("k", c_int64), ("n_trials", c_int64), ("n_decisions", c_int64), ("warn", c_int32),
-                ("fault", c_int32), ("f", c_double), ("n_done", c_int64), ("stop_reason", c_int32), ("step", c_double)]
+                ("fault", c_int32), ("f", c_double), ("n_done", c_int64), ("stop_reason", c_int32), ("step", c_double), ("f_ref", c_double)]
 
 
 def lib():
@@ -69,6 +70,7 @@ def lib():
         L.sup_perturb_tv.argtypes = [c_void_p, c_void_p, c_int, POINTER(c_int64), c_int, c_double, c_double, POINTER(c_int64)]
         L.sup_perturb_dose.argtypes = [c_void_p, c_void_p, c_int, c_double, c_double, POINTER(c_int64)]
         L.sup_perturb_mean.argtypes = [c_void_p, c_void_p, c_int, c_double, c_double, POINTER(c_int64)]
+        L.sup_perturb_adaptive.argtypes = [c_void_p, c_void_p, c_int, POINTER(c_int64), c_int, POINTER(c_double), c_double]
         L.sup_project_drop.argtypes = [c_void_p, c_void_p, c_double, c_int]
         L.sup_backproject_partial.argtypes = [c_void_p, c_void_p, c_double]
         L.sup_apply_update.argtypes = [c_void_p, c_void_p, c_void_p, c_double]
@@ -318,8 +320,19 @@ def sup_perturb_mean(H: SupHandle, x: torch.Tensor, N, beta0, a, ell=0):
     return e.value
 
 
+def sup_perturb_adaptive(H: SupHandle, x: torch.Tensor, objective, N, f_ref, shrink=0.5, shape=None):
+    """One phase with Eq. 11's step size; returns the updated reference value."""
+    k = _OBJ[objective] if not isinstance(objective, int) else objective
+    sh = (c_int64 * 3)(*(list(shape) + [0] * (3 - len(shape)))) if shape is not None else None
+    fr = c_double(float(f_ref))
+    H._enter()
+    H._check(lib().sup_perturb_adaptive(H.h, _ptr(x), k, sh, int(N), byref(fr), c_double(float(shrink))))
+    H._exit()
+    return fr.value
+
+
 def _options(H, objective, shape, lam, block, policy, ell0, k0, trace, decisions, decision_f, use_graph, n_restart=0, algorithm=None,
-             stop=None):
+             stop=None, adaptive=None):
     o = _Options()
     o.objective = _OBJ[objective] if not isinstance(objective, int) else objective
     if shape is not None and o.objective == OBJ_TV2D:
@@ -342,15 +355,17 @@ def _options(H, objective, shape, lam, block, policy, ell0, k0, trace, decisions
         o.stop_enabled = 1
         o.prox_tol, o.dprox_tol = float(stop.get("prox_tol", 1e-6)), float(stop.get("dprox_tol", 1e-8))
         o.n_consec, o.dobj_tol = int(stop.get("n_consec", 5)), float(stop.get("dobj_tol", 1e-6))
+    if adaptive is not None:  # dict(f_ref, shrink): Eq. 11's step size (SUP_RULE_ADAPTIVE)
+        o.step_rule, o.f_ref, o.f_ref_shrink = 1, float(adaptive["f_ref"]), float(adaptive.get("shrink", 0.5))
     return o
 
 
 def sup_superiorize(H: SupHandle, x: torch.Tensor, n_iter, N, beta0, a, objective=None, shape=None, lam=1.0, block=False,
                     policy=PER_TRIAL, ell0=0, k0=0, trace=None, decisions=None, decision_f=None, use_graph=True, n_restart=0,
-                    algorithm=None, stop=None):
+                    algorithm=None, stop=None, adaptive=None):
     """Algorithm 1 on device tensor x (in place, asynchronous).  trace: float64 [n_iter,4] device tensor or None;
     decisions: int8 [cap] device tensor or None; decision_f: float64 [cap,2] device tensor or None."""
-    o = _options(H, objective, shape, lam, block, policy, ell0, k0, trace, decisions, decision_f, use_graph, n_restart, algorithm, stop)
+    o = _options(H, objective, shape, lam, block, policy, ell0, k0, trace, decisions, decision_f, use_graph, n_restart, algorithm, stop, adaptive)
     H._enter()
     H._check(lib().sup_superiorize(H.h, _ptr(x), n_iter, N, beta0, a, byref(o)))
     H._exit()
@@ -372,7 +387,7 @@ def sup_get_state(H: SupHandle) -> dict:
     s = _State()
     H._check(lib().sup_get_state(H.h, byref(s)))
     return dict(ell=s.ell, k=s.k, n_trials=s.n_trials, n_decisions=s.n_decisions, warn=s.warn, fault=s.fault, f=s.f,
-                n_done=s.n_done, stop_reason=s.stop_reason, step=s.step)
+                n_done=s.n_done, stop_reason=s.stop_reason, step=s.step, f_ref=s.f_ref)
 
 
 def sup_proximity(H: SupHandle, x: torch.Tensor, mode=0, p=2.0) -> float:

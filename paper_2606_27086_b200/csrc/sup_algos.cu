@@ -329,7 +329,8 @@ int sup_launch_mean_value(sup_ctx* h, const void* x) {  // leaves per-CTA partia
 // launch is left, so the sequence is captured in the sweep's graph.
 __global__ void k_dose_trial(DevState* st, const double* __restrict__ red_f, int np_f, const double* __restrict__ part_f, int np_part,
                              const double* __restrict__ red_g, int np_g, const double* __restrict__ red_q, int np_q, int first, int final_only,
-                             double beta0, double a, int policy, long long n_restart, int8_t* decisions, double* decision_f, long long cap) {
+                             double beta0, double a, int policy, long long n_restart, int8_t* decisions, double* decision_f, long long cap,
+                             int step_rule, double shrink) {
     if (st->stop) return;
     const long long k = st->k;
     if (first && n_restart > 0 && k > 0 && k % n_restart == 0) {  // restarted perturbations (A-24)
@@ -345,9 +346,29 @@ __global__ void k_dose_trial(DevState* st, const double* __restrict__ red_f, int
     st->f_cur = fx;
     st->f = fx;
     st->cf = 0.0;
-    if (final_only) return;
+    if (first) st->f_start = fx;
+    if (final_only) {
+        // adaptive rule (A-30): the phase started at or below the reference -> the reference moves below that value
+        if (step_rule == SUP_RULE_ADAPTIVE && st->f_start <= st->f_ref) st->f_ref = shrink * st->f_start;
+        return;
+    }
     const double s2 = sum_partials(red_g, np_g), q2 = sum_partials(red_q, np_q);
     const double s = sqrt(s2);
+    if (step_rule == SUP_RULE_ADAPTIVE) {  // Eq. 11: no trial loop, no exponent
+        const bool take = fx > st->f_ref && s > 0.0;
+        if (take) {
+            st->cf = ((fx - st->f_ref) / s) / s;
+            st->n_trials += 1;
+            st->sweep_trials += 1;
+        }
+        if (decisions && st->n_dec < cap) decisions[st->n_dec] = take ? 1 : 0;
+        if (decision_f && st->n_dec < cap) {
+            decision_f[2 * st->n_dec] = st->f_ref;
+            decision_f[2 * st->n_dec + 1] = fx;
+        }
+        st->n_dec += 1;
+        return;
+    }
     bool accepted = false;
     long long jloc = 0;
     for (int trial = 0; trial < SUP_J_MAX && !accepted; ++trial) {
@@ -421,7 +442,7 @@ sup_status sup_launch_perturb_dose_staged(sup_ctx* h, void* x, const PerturbPara
         sup_launch_staged(h, 2, h->DT.plan, h->DT, h->r_dose, nullptr, nullptr, nullptr, h->g, nullptr, 2.0, GMap(), false, red_g);  // g = 2 D^T r
         sup_launch_staged(h, 2, h->D.plan, h->D, h->g, nullptr, nullptr, nullptr, h->q_dose, nullptr, 1.0, GMap(), false, red_q);    // q = D g
         k_dose_trial<<<1, 1, 0, h->stream>>>(h->state, red_f, npD, h->partials, grid, red_g, npDT, red_q, npD, nred == 0, 0, pp.beta0, pp.a,
-                                             pp.policy, pp.n_restart, pp.decisions, pp.decision_f, pp.cap);
+                                             pp.policy, pp.n_restart, pp.decisions, pp.decision_f, pp.cap, pp.step_rule, pp.shrink);
         void* mir = nred == pp.N - 1 ? mirror : nullptr;
         if (h->dt == SUP_F32)
             k_dose_apply<float><<<grid, SUP_THREADS, 0, h->stream>>>(h->state, static_cast<float*>(x), static_cast<const float*>(h->g), h->n,
@@ -435,7 +456,7 @@ sup_status sup_launch_perturb_dose_staged(sup_ctx* h, void* x, const PerturbPara
     }
     // f of the final inner iterate into the state
     k_dose_trial<<<1, 1, 0, h->stream>>>(h->state, red_f, npD, h->partials, grid, red_g, npDT, red_q, npD, pp.N == 0, 1, pp.beta0, pp.a, pp.policy,
-                                         pp.n_restart, pp.decisions, pp.decision_f, pp.cap);
+                                         pp.n_restart, pp.decisions, pp.decision_f, pp.cap, pp.step_rule, pp.shrink);
     h->launches++;
     SUP_CUDA(h, cudaGetLastError());
     return SUP_OK;

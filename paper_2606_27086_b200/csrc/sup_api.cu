@@ -1,5 +1,6 @@
 // sup_api.cu -- the C ABI of libsup (include/sup.h): argument checks, workspace layout, the sweep loops
 // (O-SWEEP, O-BLOCK-SWEEP, O-SUPERIORIZE of DESIGN.md) and CUDA-graph capture of one superiorized sweep (S8).
+#include <cmath>
 #include <math.h>
 #include <stddef.h>
 #include <stdlib.h>
@@ -579,6 +580,7 @@ static sup_status read_state(sup_ctx* h, sup_state* out) {
     out->n_done = s.n_done;
     out->stop_reason = s.stop_reason;
     out->step = s.step;
+    out->f_ref = s.f_ref;
     return SUP_OK;
 }
 
@@ -590,6 +592,37 @@ extern "C" sup_status sup_get_state(sup_handle h, sup_state* out) {
     if (rc != SUP_OK) return rc;
     if (out->fault & 1) return sup_fail(h, SUP_ERR_CUDA, "device-side grid barrier timed out");
     if (out->fault & 2) return sup_fail(h, SUP_ERR_NONFINITE, "non-finite objective value");
+    return SUP_OK;
+}
+
+// Eq. 11's rule (A-30) is built for the objectives whose phase evaluates f and g in every step
+static sup_status check_adaptive(sup_ctx* h, int objective, double f_ref, double shrink) {
+    if (objective != SUP_OBJ_TV1D && objective != SUP_OBJ_TV2D && objective != SUP_OBJ_TV3D && objective != SUP_OBJ_DOSE)
+        return sup_fail(h, SUP_ERR_INVALID_ARG, "the adaptive step rule (Eq. 11) is available for TV and dose objectives");
+    if (!(shrink > 0.0 && shrink <= 1.0)) return sup_fail(h, SUP_ERR_INVALID_ARG, "f_ref_shrink must be in (0, 1]");
+    if (!std::isfinite(f_ref)) return sup_fail(h, SUP_ERR_INVALID_ARG, "f_ref must be finite");
+    return SUP_OK;
+}
+
+extern "C" sup_status sup_perturb_adaptive(sup_handle h, void* x, int objective, const int64_t* shape, int N, double* f_ref, double shrink) {
+    if (!h) return SUP_ERR_INVALID_ARG;
+    SUP_ENTER(h);
+    if (!x || !f_ref || N < 0) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_perturb_adaptive: NULL x / f_ref or N < 0");
+    sup_status rc = check_adaptive(h, objective, *f_ref, shrink);
+    if (rc != SUP_OK) return rc;
+    int64_t dims[3];
+    rc = check_objective(h, objective, shape, dims);
+    if (rc != SUP_OK) return rc;
+    sup_launch_begin_run(h, 0, 0, 1.0, 0, *f_ref);
+    if (N > 0) {
+        PerturbParams pp = {objective, dims[0], dims[1], dims[2], N, 0.0, 1.0, SUP_STEP_PER_TRIAL, nullptr, nullptr, 0, 0, false, SUP_RULE_ADAPTIVE, shrink};
+        rc = sup_launch_perturb(h, x, pp);
+        if (rc != SUP_OK) return rc;
+    }
+    sup_state s;
+    rc = sup_get_state(h, &s);
+    if (rc != SUP_OK) return rc;
+    *f_ref = s.f_ref;
     return SUP_OK;
 }
 
@@ -673,7 +706,7 @@ static void enqueue_measure_and_close(sup_ctx* h, const RunPlan& P, int mode) {
 static sup_status enqueue_superiorized_sweep(sup_ctx* h, const RunPlan& P) {
     if (run_perturbed(P)) {
         PerturbParams pp = {P.o.objective, P.dims[0], P.dims[1], P.dims[2], P.N, P.beta0, P.a, P.o.step_policy, P.o.decisions,
-                            P.o.decision_f, P.o.decisions_cap, P.o.n_restart, true};
+                            P.o.decision_f, P.o.decisions_cap, P.o.n_restart, true, P.o.step_rule, P.o.f_ref_shrink};
         sup_status rc = sup_launch_perturb(h, P.x, pp);
         if (rc != SUP_OK) return rc;
         h->xg_synced = sup_stream_forward_uses_xg(h);  // the perturbation kernel wrote the moved x to the gather mirror too
@@ -712,6 +745,12 @@ static sup_status run_superiorize(sup_ctx* h, void* x, int n_iter, int N, double
         return sup_fail(h, SUP_ERR_STATE, "EMR needs the staged product kernels (sup_set_row_mode)");
     if (opt->stop_enabled && (opt->n_consec < 1 || !(opt->dprox_tol >= 0.0) || !(opt->dobj_tol >= 0.0)))
         return sup_fail(h, SUP_ERR_INVALID_ARG, "stopping rule: n_consec >= 1 and non-negative thresholds are needed");
+    if (opt->step_rule != SUP_RULE_POWER && opt->step_rule != SUP_RULE_ADAPTIVE) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_superiorize: unknown step rule");
+    if (opt->step_rule == SUP_RULE_ADAPTIVE && N > 0 && opt->objective != SUP_OBJ_NONE) {
+        sup_status ra = check_adaptive(h, opt->objective, opt->f_ref, opt->f_ref_shrink);
+        if (ra != SUP_OK) return ra;
+        if (opt->n_restart > 0) return sup_fail(h, SUP_ERR_INVALID_ARG, "restarts belong to the power law (the adaptive rule has no exponent)");
+    }
     RunPlan P;
     P.x = x;
     P.N = N;
@@ -720,7 +759,7 @@ static sup_status run_superiorize(sup_ctx* h, void* x, int n_iter, int N, double
     P.o = *opt;
     sup_status rc = check_objective(h, opt->objective, opt->shape, P.dims);
     if (rc != SUP_OK) return rc;
-    sup_launch_begin_run(h, opt->ell0, opt->k0, a, n_iter);
+    sup_launch_begin_run(h, opt->ell0, opt->k0, a, n_iter, opt->f_ref);
     h->xg_synced = false;
     h->stop_ptr = opt->stop_enabled ? &h->state->stop : nullptr;
     struct StopPtrReset {
@@ -755,6 +794,8 @@ static sup_status run_superiorize(sup_ctx* h, void* x, int n_iter, int N, double
         key.tols[1] = opt->dprox_tol;
         key.tols[2] = opt->dobj_tol;
         key.n_consec = opt->n_consec;
+        key.step_rule = opt->step_rule;
+        key.shrink = opt->f_ref_shrink;
         if (!h->gexec || !(key == h->gkey)) {
             drop_graph(h);
             const int64_t launches_before = h->launches;

@@ -60,6 +60,8 @@ struct DevState {
     int consec;           // consecutive sweeps with a small relative proximity change
     int stop;             // 1: the rule fired -- every later kernel of the run returns at once
     int stop_reason;
+    double f_ref;         // Eq. 11's reference value (adaptive step rule, A-30)
+    double f_start;       // dose objective, adaptive rule: f at the start of the phase (decides the update of f_ref)
     // grid barrier of the perturbation kernel: the arrival counter, the generation flag every waiting CTA polls and the
     // published totals each sit in a 128-byte line of their own, so the pollers do not slow the arrivals down
     alignas(128) unsigned bar_count;
@@ -187,8 +189,8 @@ struct sup_ctx {
         const void* x = nullptr;
         int N = 0, objective = 0, block = 0, policy = 0, trace_mode = 0;
         int64_t n_restart = 0;
-        int algorithm = 0, stop = 0, n_consec = 0;
-        double tols[3] = {0, 0, 0};
+        int algorithm = 0, stop = 0, n_consec = 0, step_rule = 0;
+        double tols[3] = {0, 0, 0}, shrink = 0;
         double beta0 = 0, a = 0, lambda = 0;
         int64_t s0 = 0, s1 = 0, s2 = 0;
         const void *trace = nullptr, *dec = nullptr, *decf = nullptr;
@@ -197,7 +199,8 @@ struct sup_ctx {
             return x == o.x && N == o.N && objective == o.objective && block == o.block && policy == o.policy &&
                    trace_mode == o.trace_mode && beta0 == o.beta0 && a == o.a && lambda == o.lambda && s0 == o.s0 &&
                    s1 == o.s1 && s2 == o.s2 && algorithm == o.algorithm && stop == o.stop && n_consec == o.n_consec &&
-                   tols[0] == o.tols[0] && tols[1] == o.tols[1] && tols[2] == o.tols[2] && trace == o.trace && dec == o.dec && decf == o.decf && cap == o.cap && n_restart == o.n_restart;
+                   tols[0] == o.tols[0] && tols[1] == o.tols[1] && tols[2] == o.tols[2] && trace == o.trace && dec == o.dec && decf == o.decf && cap == o.cap && n_restart == o.n_restart &&
+                   step_rule == o.step_rule && shrink == o.shrink;
         }
     } gkey;
     int64_t launches = 0;
@@ -277,10 +280,12 @@ struct PerturbParams {
     int64_t cap;
     int64_t n_restart;
     bool write_mirror;  // also write the final iterate to the gather mirror of x (xg_synced stays true)
+    int step_rule = 0;  // sup_step_rule
+    double shrink = 1.0;
 };
 sup_status sup_launch_perturb(sup_ctx* h, void* x, const PerturbParams& pp);
 void sup_launch_objective(sup_ctx* h, const void* x, int kind, int64_t nz, int64_t ny, int64_t nx, double* out_dev);
-void sup_launch_begin_run(sup_ctx* h, int64_t ell0, int64_t k0, double a, int64_t n_iter = 0);
+void sup_launch_begin_run(sup_ctx* h, int64_t ell0, int64_t k0, double a, int64_t n_iter = 0, double f_ref = 0.0);
 int sup_perturb_grid(sup_ctx* h, int objective);
 
 // ---- DROP / EMR, stopping rule, f_Mean (sup_algos.cu) ---------------------------------------------------------------

@@ -44,6 +44,8 @@ struct PArgs {
     double beta0, a;
     int policy;
     long long n_restart;
+    int step_rule;  // sup_step_rule
+    double shrink;  // adaptive rule (A-30)
     DevState* st;
     double* partials;  // [2][SUP_MAX_PARTIALS]
     int8_t* decisions;
@@ -659,7 +661,38 @@ __global__ void __launch_bounds__(SUP_THREADS) k_perturb_tv(PArgs<T> Ain) {
         s = sqrt(v[1]);
         if (!isfinite(fx)) fault |= 2;
     }
-    for (int nred = 0; ok && nred < A.N; ++nred) {
+    // Eq. 11 (A-30): beta = (f - f_ref)/||g|| when f > f_ref, else 0; the step x - ((f - f_ref)/||g||^2) g is
+    // taken as it is -- no trial loop, no exponent.  Same passes as an always-accepted first candidate: 1 + N in all.
+    const bool adaptive = A.step_rule == SUP_RULE_ADAPTIVE;
+    const double f_ref = adaptive ? *(volatile double*)&st->f_ref : 0.0;
+    const double f_start = fx;
+    for (int nred = 0; ok && adaptive && nred < A.N; ++nred) {
+        const bool take = fx > f_ref && s > 0.0;
+        log_trial(f_ref, fx, take);
+        if (!take) continue;  // beta = 0: x^{k,n+1} = x^{k,n}, and so for every later step of this phase
+        ++trials;
+        const double c = ((fx - f_ref) / s) / s;
+        if (nred == A.N - 1) {
+            pend = c;  // applied by the final write below; f of the final point is not evaluated
+            break;
+        }
+        double v[2];
+        tv_gz<T, OBJ>(view(), c, xo, go, v[0], v[1], tile_mem);
+        ok = grid_reduce<2>(st, P, PSTRIDE, v, gen);
+        if (!ok) break;
+        fx = v[0];
+        s = sqrt(v[1]);
+        if (!isfinite(fx)) fault |= 2;
+        T* t = gc;
+        gc = go;
+        go = t;
+        if (c != 0.0) {
+            t = xc;
+            xc = xo;
+            xo = t;
+        }
+    }
+    for (int nred = 0; ok && !adaptive && nred < A.N; ++nred) {
         const bool last = nred == A.N - 1;
         bool accepted = false;
         long long jloc = 0;
@@ -756,6 +789,7 @@ __global__ void __launch_bounds__(SUP_THREADS) k_perturb_tv(PArgs<T> Ain) {
         st->n_trials += trials;
         st->sweep_trials += trials;
         st->f = fx;
+        if (adaptive && f_start <= f_ref) st->f_ref = A.shrink * f_start;  // the reference was reached: move it below (A-30)
         if (warn) atomicOr(&st->warn, warn);
         if (fault) atomicOr(&st->fault, fault);
     }
@@ -798,6 +832,8 @@ static PArgs<T> make_args(sup_ctx* h, void* x, const PerturbParams& pp) {
     A.beta0 = pp.beta0;
     A.a = pp.a;
     A.policy = pp.policy;
+    A.step_rule = pp.step_rule;
+    A.shrink = pp.shrink;
     A.n_restart = pp.n_restart;
     A.st = h->state;
     A.partials = h->partials;
@@ -912,7 +948,9 @@ void sup_launch_objective(sup_ctx* h, const void* x, int kind, int64_t nz, int64
     else launch_objective_t<double>(h, x, kind, nz, ny, nx, out_dev);
 }
 
-__global__ void k_begin_run(DevState* st, long long ell0, long long k0, double apow0, long long n_iter) {
+__global__ void k_begin_run(DevState* st, long long ell0, long long k0, double apow0, long long n_iter, double f_ref) {
+    st->f_ref = f_ref;
+    st->f_start = 0.0;
     st->n_iter = n_iter;
     st->n_done = 0;
     st->stop = 0;
@@ -932,10 +970,10 @@ __global__ void k_begin_run(DevState* st, long long ell0, long long k0, double a
     st->fault = 0;
     st->bar_count = 0;
 }
-void sup_launch_begin_run(sup_ctx* h, int64_t ell0, int64_t k0, double a, int64_t n_iter) {
+void sup_launch_begin_run(sup_ctx* h, int64_t ell0, int64_t k0, double a, int64_t n_iter, double f_ref) {
     // a^l0: exactly 1 for a fresh run, so the running product below reproduces the oracle's step sizes bit for bit (A-20)
     double apow0 = 1.0;
     for (int64_t i = 0; i < ell0; ++i) apow0 *= a;  // (ell0 is bounded by the argument check: the product stays exact-by-construction)
-    k_begin_run<<<1, 1, 0, h->stream>>>(h->state, ell0, k0, apow0, n_iter);
+    k_begin_run<<<1, 1, 0, h->stream>>>(h->state, ell0, k0, apow0, n_iter, f_ref);
     h->launches++;
 }

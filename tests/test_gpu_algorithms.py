@@ -320,3 +320,122 @@ def test_more_than_2_31_stored_entries():
     big = np.abs(c) > 1e-3
     assert big.sum() > 100
     np.testing.assert_allclose(got[big], want[big], rtol=2e-3)  # fp32 row dots of 256 terms against a violation of >= 1e-3
+
+
+# ---- Eq. 11: the subgradient-projection step size (SUP_RULE_ADAPTIVE, reading A-30) ----------------------
+def _identity_handle(sup, n, dtype):
+    rp, c = np.arange(n + 1, dtype=np.int64), np.arange(n, dtype=np.int32)
+    one, zero = np.ones(n, np.float32), np.zeros(n, np.float32)
+    H = sup.sup_create(rp, c, one, zero, one, zero, one, None, dtype=dtype, n=n)
+    return H, (n, n, rp, c, np.ones(n), np.zeros(n), np.ones(n), np.zeros(n), np.ones(n))
+
+
+@pytest.mark.parametrize("dtype", [0, 1])
+@pytest.mark.parametrize("kind,shape", [("tv2d", (37, 91)), ("tv2d", (130, 70)), ("tv1d", (5000,)), ("tv3d", (6, 9, 40))])
+def test_adaptive_phase_tv(kind, shape, dtype):
+    sup = _sup()
+    n = int(np.prod(shape))
+    H, oargs = _identity_handle(sup, n, dtype)
+    O = Oracle(*oargs, objective=kind, shape=shape if kind != "tv1d" else None)
+    xs = np.random.default_rng(17).uniform(0, 1, n).astype(np.float32)
+    f0 = O.objective_value(xs.astype(np.float64))
+    sh = None if kind == "tv1d" else shape
+    ptol, ftol = (2e-6, 1e-5) if dtype == 0 else (1e-13, 1e-12)
+    for N in (1, 3):
+        # above the reference: N steps of Eq. 11
+        x = xdev(xs, dtype)
+        fr = sup.sup_perturb_adaptive(H, x, kind, N, 0.9 * f0, 0.5, shape=sh)
+        R = O.perturb_adaptive(xs.astype(np.float64), N, 0.9 * f0, 0.5)
+        st = sup.sup_get_state(H)
+        assert st["n_trials"] == R["steps"] == N and st["n_decisions"] == N and fr == R["f_ref"] == 0.9 * f0
+        err = rel_l2(x.cpu().numpy(), R["x"])
+        assert err <= ptol, (kind, shape, N, err)
+        # at / below the reference: beta = 0, x untouched bit for bit, the reference moves to shrink * f(x)
+        x = xdev(xs, dtype)
+        fr = sup.sup_perturb_adaptive(H, x, kind, N, 2.0 * f0, 0.25, shape=sh)
+        assert torch.equal(x, xdev(xs, dtype)) and sup.sup_get_state(H)["n_trials"] == 0
+        assert abs(fr - 0.25 * f0) <= ftol * f0
+    # a constant image has a zero gradient: no step although f = 0 > f_ref
+    x = torch.full((n,), 0.5, dtype=TD[dtype], device="cuda:0")
+    fr = sup.sup_perturb_adaptive(H, x, kind, 2, -1.0, 0.5, shape=sh)
+    assert fr == -1.0 and bool((x == 0.5).all()) and sup.sup_get_state(H)["n_trials"] == 0
+
+
+@pytest.mark.parametrize("dtype", [0, 1])
+def test_adaptive_phase_dose_and_argument_errors(dtype):
+    sup = _sup()
+    P = gen.config4_imrt(scale=0.17)
+    H = handle(P, dtype)
+    O = Oracle.from_problem(P)
+    xs = np.random.default_rng(3).uniform(0.5, 1.5, P.n).astype(np.float32)
+    f0 = O.objective_value(xs.astype(np.float64), "dose")
+    for N in (1, 3):
+        x = xdev(xs, dtype)
+        fr = sup.sup_perturb_adaptive(H, x, "dose", N, 0.8 * f0, 0.5)
+        R = O.perturb_adaptive(xs.astype(np.float64), N, 0.8 * f0, 0.5, kind="dose")
+        st = sup.sup_get_state(H)
+        assert st["n_trials"] == R["steps"] == N and fr == 0.8 * f0
+        err = rel_l2(x.cpu().numpy(), R["x"])
+        assert err <= (2e-6 if dtype == 0 else 1e-12), (N, err)
+    x = xdev(xs, dtype)
+    fr = sup.sup_perturb_adaptive(H, x, "dose", 2, 1.5 * f0, 0.5)
+    assert torch.equal(x, xdev(xs, dtype)) and abs(fr - 0.5 * f0) <= (1e-5 if dtype == 0 else 1e-12) * f0
+    # arguments
+    with pytest.raises(Exception):
+        sup.sup_perturb_adaptive(H, x, "mean", 1, 0.0, 0.5)
+    with pytest.raises(Exception):
+        sup.sup_perturb_adaptive(H, x, "dose", 1, 0.0, 0.0)
+    with pytest.raises(Exception):
+        sup.sup_perturb_adaptive(H, x, "dose", 1, float("nan"), 0.5)
+    with pytest.raises(Exception):
+        sup.sup_superiorize(H, x, 2, 2, 1.0, 0.9, objective="dose", adaptive=dict(f_ref=0.0, shrink=0.5), n_restart=5)
+
+
+@pytest.mark.parametrize("dtype", [0, 1])
+@pytest.mark.parametrize("which", ["cfg1", "cfg4"])
+def test_adaptive_rule_inside_algorithm_1(which, dtype):
+    """Eq. 10 with Eq. 11's step size: step-wise from the oracle's own states (strict), then a free run through the graph replay
+    (step pattern identical, x within the free-run bound of A-23)"""
+    sup = _sup()
+    P = gen.config1_tiny_ct() if which == "cfg1" else gen.config4_imrt(scale=0.17)
+    H = handle(P, dtype)
+    O = Oracle.from_problem(P)
+    kw = dict(objective=P.objective, shape=P.shape, lam=P.lam)
+    f0 = O.objective_value(np.asarray(P.x0, np.float64))
+    x_ref = np.asarray(P.x0, np.float64)
+    if f0 == 0.0:  # x0 = 0: one basic sweep gives a start with f > 0
+        x_ref = O.sweep(x_ref, P.lam)
+        f0 = O.objective_value(x_ref)
+    fr, shrink, N, S = 0.7 * f0, 0.6, 2, 8
+    x_start = np.asarray(x_ref, np.float32 if dtype == 0 else np.float64).astype(np.float64)
+    took = 0
+    for k in range(S):
+        xs64 = np.asarray(x_ref, np.float32 if dtype == 0 else np.float64).astype(np.float64)
+        R = O.run(xs64, 1, N=N, lam=P.lam, adaptive=dict(f_ref=fr, shrink=shrink))
+        xg = xdev(xs64, dtype)
+        sup.sup_superiorize(H, xg, 1, N, 1.0, 0.9, adaptive=dict(f_ref=fr, shrink=shrink), **kw)
+        st = sup.sup_get_state(H)
+        assert st["n_trials"] == int(R["trace"][0, 2]) and st["ell"] == 0, (k, st, R["trace"])
+        if R["f_ref"] == fr:
+            assert st["f_ref"] == fr
+        else:
+            assert abs(st["f_ref"] - R["f_ref"]) <= (1e-5 if dtype == 0 else 1e-12) * abs(R["f_ref"])
+        err = rel_l2(xg.cpu().numpy(), R["x"])
+        assert err <= TOL[dtype], (which, k, err)
+        took += int(R["trace"][0, 2])
+        x_ref, fr = R["x"], R["f_ref"]
+    assert 0 < took  # some steps were taken, and (below) the reference moved at least once in the free run
+    # free run, CUDA graph
+    fr0 = 0.7 * f0
+    R = O.run(x_start, S, N=N, lam=P.lam, adaptive=dict(f_ref=fr0, shrink=shrink))
+    xg = xdev(x_start, dtype)
+    dec = torch.zeros(4 * S * N, dtype=torch.int8, device="cuda:0")
+    sup.sup_superiorize(H, xg, S, N, 1.0, 0.9, adaptive=dict(f_ref=fr0, shrink=shrink), decisions=dec, use_graph=True, **kw)
+    st = sup.sup_get_state(H)
+    gdec = dec[: st["n_decisions"]].cpu().numpy()
+    err = rel_l2(xg.cpu().numpy(), R["x"])
+    print(f"[adaptive free run] {which} dtype={dtype}: rel L2 {err:.3e}, steps {gdec.sum()} vs {R['decisions'].sum()}, f_ref {st['f_ref']:.6e} vs {R['f_ref']:.6e}")
+    assert st["n_decisions"] == S * N == R["decisions"].size
+    if np.array_equal(gdec, R["decisions"]):
+        assert err <= (5e-3 if dtype == 0 else 1e-8)
+        assert abs(st["f_ref"] - R["f_ref"]) <= (1e-3 if dtype == 0 else 1e-9) * abs(R["f_ref"])
