@@ -175,6 +175,12 @@ sup_status sup_set_blocks(sup_handle h, int n_blocks, const int64_t* block_rowpt
 sup_status sup_set_dose_matrix(sup_handle h, const sup_csr* D_body, void* workspace, size_t workspace_bytes,
                                void* scratch, size_t scratch_bytes);
 
+/* How the dose objective's perturbation phase is evaluated.  mode 0 (default): through the Gram matrix G = D_body^T D_body when
+ * sup_set_dose_matrix built it (it does when n <= 16384 and n^2 <= 2 nnz(D_body): f(x) = x^T G x, g = 2 G x, ||D g||^2 = g^T G g,
+ * 1 + N dense n x n products per phase instead of 1 + 2N passes over D_body, K4d), else by matrix passes.
+ * mode 1: always by matrix passes over D_body and its transpose.  Both are the same mathematics (A-15); they differ in rounding. */
+sup_status sup_set_dose_mode(sup_handle h, int mode);
+
 /* Layout hint for the two gathered vectors (DESIGN.md section 4 "gather layouts").  The forward product gathers x and the
  * back-projection gathers y = D c(x) at the column / row indices of the nonzeros.  When an index space is a row-major
  * 2-D array -- x an image of x_shape = {rows, cols} pixels (rows * cols = n), the rows of A a sinogram of

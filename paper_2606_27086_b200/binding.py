@@ -70,6 +70,7 @@ def lib():
         L.sup_perturb_tv.argtypes = [c_void_p, c_void_p, c_int, POINTER(c_int64), c_int, c_double, c_double, POINTER(c_int64)]
         L.sup_perturb_dose.argtypes = [c_void_p, c_void_p, c_int, c_double, c_double, POINTER(c_int64)]
         L.sup_perturb_mean.argtypes = [c_void_p, c_void_p, c_int, c_double, c_double, POINTER(c_int64)]
+        L.sup_set_dose_mode.argtypes = [c_void_p, c_int]
         L.sup_perturb_adaptive.argtypes = [c_void_p, c_void_p, c_int, POINTER(c_int64), c_int, POINTER(c_double), c_double]
         L.sup_project_drop.argtypes = [c_void_p, c_void_p, c_double, c_int]
         L.sup_backproject_partial.argtypes = [c_void_p, c_void_p, c_double]
@@ -318,6 +319,11 @@ def sup_perturb_mean(H: SupHandle, x: torch.Tensor, N, beta0, a, ell=0):
     H._check(lib().sup_perturb_mean(H.h, _ptr(x), N, beta0, a, byref(e)))
     H._exit()
     return e.value
+
+
+def sup_set_dose_mode(H: SupHandle, mode: int):
+    """0: the dose perturbation through the Gram matrix when it was built (default); 1: by matrix passes over D and D^T."""
+    H._check(lib().sup_set_dose_mode(H.h, int(mode)))
 
 
 def sup_perturb_adaptive(H: SupHandle, x: torch.Tensor, objective, N, f_ref, shrink=0.5, shape=None):

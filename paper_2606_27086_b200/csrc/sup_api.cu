@@ -48,6 +48,7 @@ extern "C" sup_status sup_workspace_bytes(int kind, int64_t m, int64_t n, int64_
             p = al(size_t(n + 1) * 8) + al(size_t(nnz) * 4) + al(size_t(nnz) * esz) + 2 * al(size_t(m) * esz)
                 + al(size_t(n) * esz) + 256                                                        // gradient of f_Mean and its norm
                 + (dtype == SUP_F32 ? 2 * al(size_t(nnz) * 8) : 0) + 2 * sup_stream_table_bytes()  // packed D, D^T; partition tables
+                + (sup_gram_applicable(n, nnz) ? al(size_t(n) * size_t(sup_gram_ld(n)) * esz) + al(size_t(n) * esz) : 0)  // G = D^T D, G g
                 + 1024;
             s = sup_transpose_scratch_bytes(nnz, n, esz) + 4096;
             break;
@@ -305,6 +306,12 @@ extern "C" sup_status sup_set_dose_matrix(sup_handle h, const sup_csr* D, void* 
     h->pk_dt = h->dt == SUP_F32 ? B.take(size_t(D->nnz) * 8) : nullptr;
     void* tab_d = B.take(sup_stream_table_bytes());
     void* tab_dt = B.take(sup_stream_table_bytes());
+    h->gram = h->gram_w = nullptr;
+    void *gram = nullptr, *gram_w = nullptr;
+    if (sup_gram_applicable(D->n, D->nnz)) {
+        gram = B.take(size_t(D->n) * size_t(sup_gram_ld(D->n)) * h->esz);
+        gram_w = B.take(size_t(D->n) * h->esz);
+    }
     if (!B.ok) return sup_fail(h, SUP_ERR_WORKSPACE, "sup_set_dose_matrix: workspace too small");
     rc = sup_transpose_rows(h, Dm, 0, D->m, 0, D->nnz, rp, col, val, 0, scratch, scratch_bytes);
     if (rc != SUP_OK) return rc;
@@ -327,10 +334,30 @@ extern "C" sup_status sup_set_dose_matrix(sup_handle h, const sup_csr* D, void* 
     if (rc == SUP_OK) rc = sup_stream_plan(h, h->D, 0, D->m, true, tab_d, scratch, &h->D.plan);
     if (rc == SUP_OK) rc = sup_stream_plan(h, h->DT, 0, D->n, false, tab_dt, scratch, &h->DT.plan);
     if (rc != SUP_OK) return rc;
+    if (gram) {  // the dose objective in n-space: G = D^T D (sup_gram.cu)
+        h->gram = gram;
+        h->gram_w = gram_w;
+        h->gram_ld = sup_gram_ld(D->n);
+        rc = sup_gram_build(h);
+        if (rc != SUP_OK) {
+            h->gram = nullptr;
+            return rc;
+        }
+    }
     h->has_dose = true;
     rc = sup_setup_mean_gradient(h);  // (1/N_S) D^T 1 for f_Mean (Eq. 21), should the matrix be used as a structure's D_S
     if (rc != SUP_OK) return rc;
     SUP_CUDA(h, cudaStreamSynchronize(h->stream));
+    return SUP_OK;
+}
+
+extern "C" sup_status sup_set_dose_mode(sup_handle h, int mode) {
+    if (!h) return SUP_ERR_INVALID_ARG;
+    SUP_ENTER(h);
+    if (mode != 0 && mode != 1) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_set_dose_mode: mode must be 0 (automatic) or 1 (matrix passes)");
+    SUP_CUDA(h, cudaStreamSynchronize(h->stream));
+    drop_graph(h);
+    h->dose_mode = mode;
     return SUP_OK;
 }
 

@@ -179,6 +179,10 @@ struct sup_ctx {
     void* q_dose = nullptr;     // [md] dtype: D g
     void* gmean = nullptr;      // [n] dtype: (1/N_S) D_S^T 1, the constant gradient of f_Mean (Eq. 21)
     double* gmean_norm2 = nullptr;  // device scalar ||gmean||^2
+    void* gram = nullptr;           // [n][gram_ld] G = D^T D of the dose matrix (sup_gram.cu), NULL when not applicable
+    int64_t gram_ld = 0;
+    void* gram_w = nullptr;         // [n] G g of the current reduction step
+    int dose_mode = 0;              // 0: Gram path when available, 1: matrix passes over D and D^T (sup_set_dose_mode)
     int g_d = 8, g_dt = 32;
     // cached graph of one superiorized sweep
     cudaGraphExec_t gexec = nullptr;
@@ -299,3 +303,9 @@ sup_status sup_setup_mean_gradient(sup_ctx* h);
 sup_status sup_launch_perturb_mean(sup_ctx* h, void* x, const PerturbParams& pp);
 int sup_launch_mean_value(sup_ctx* h, const void* x);
 sup_status sup_launch_perturb_dose_staged(sup_ctx* h, void* x, const PerturbParams& pp);
+
+// ---- dose objective through the Gram matrix (sup_gram.cu) -------------------------------------------------------------------------
+bool sup_gram_applicable(int64_t n, int64_t nnz);
+int64_t sup_gram_ld(int64_t n);
+sup_status sup_gram_build(sup_ctx* h);
+sup_status sup_launch_perturb_dose_gram(sup_ctx* h, void* x, const PerturbParams& pp);

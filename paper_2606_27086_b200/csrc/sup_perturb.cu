@@ -888,6 +888,7 @@ int sup_perturb_grid(sup_ctx* h, int objective) {
 sup_status sup_launch_perturb(sup_ctx* h, void* x, const PerturbParams& pp) {
     if (pp.objective == SUP_OBJ_MEAN) return sup_launch_perturb_mean(h, x, pp);
     if (pp.objective == SUP_OBJ_DOSE) {
+        if (h->gram && h->dose_mode == 0) return sup_launch_perturb_dose_gram(h, x, pp);
         if (!(h->D.plan.ok && h->DT.plan.ok)) return sup_fail(h, SUP_ERR_STATE, "the dose perturbation runs on the staged product kernels (sup_set_row_mode)");
         return sup_launch_perturb_dose_staged(h, x, pp);
     }

@@ -439,3 +439,82 @@ def test_adaptive_rule_inside_algorithm_1(which, dtype):
     if np.array_equal(gdec, R["decisions"]):
         assert err <= (5e-3 if dtype == 0 else 1e-8)
         assert abs(st["f_ref"] - R["f_ref"]) <= (1e-3 if dtype == 0 else 1e-9) * abs(R["f_ref"])
+
+
+# ---- dose objective: the Gram-matrix path (sup_gram.cu) and the matrix-pass path are the same mathematics --------------------------
+@pytest.mark.parametrize("dtype", [0, 1])
+@pytest.mark.parametrize("mode", [0, 1])
+def test_dose_phase_and_algorithm_1_in_both_dose_modes(mode, dtype):
+    """mode 0: f = x^T (D^T D) x with G = D^T D built at sup_set_dose_matrix; mode 1: passes over D and D^T.  Each against the oracle
+    (phase: trials, l, x, f; Algorithm 1 step-wise), and the Gram matrix itself against a dense fp64 product"""
+    sup = _sup()
+    P = gen.config4_imrt(scale=0.17)
+    H = handle(P, dtype)
+    sup.sup_set_dose_mode(H, mode)
+    O = Oracle.from_problem(P)
+    rng = np.random.default_rng(2)
+    xs = rng.uniform(0.5, 1.5, P.n).astype(np.float32)
+    x = xdev(xs, dtype)
+    ell, xo = 3, xs.astype(np.float64)
+    for phase in range(3):
+        ell_g = sup.sup_perturb_dose(H, x, 4, P.beta0, 0.9, ell)
+        st = sup.sup_get_state(H)
+        R = O.perturb(xo, ell, 4, P.beta0, 0.9, kind="dose")
+        xo = R["x"]
+        assert ell_g == R["ell"] and st["n_trials"] == R["trials"], (phase, ell_g, R["ell"])
+        assert rel_l2(x.cpu().numpy(), xo) <= (1e-5 if dtype == 0 else 1e-12), phase
+        assert abs(st["f"] - R["fx"]) <= (1e-5 if dtype == 0 else 1e-11) * abs(R["fx"]), phase
+        ell = ell_g
+    # Algorithm 1, step-wise from the oracle's own states
+    x_ref, ell = np.asarray(P.x0, np.float64), 0
+    for k in range(6):
+        xs64 = np.asarray(x_ref, np.float32 if dtype == 0 else np.float64).astype(np.float64)
+        R = O.run(xs64, 1, N=P.N, beta0=P.beta0, a=P.a, lam=P.lam, ell0=ell, k0=k)
+        xg = xdev(xs64, dtype)
+        sup.sup_superiorize(H, xg, 1, P.N, P.beta0, P.a, objective="dose", lam=P.lam, ell0=ell, k0=k)
+        assert sup.sup_get_state(H)["ell"] == R["ell"], k
+        assert rel_l2(xg.cpu().numpy(), R["x"]) <= TOL[dtype], k
+        x_ref, ell = R["x"], R["ell"]
+    # free run through the graph: bit-identical to direct launches
+    xa, xb = xdev(P.x0, dtype), xdev(P.x0, dtype)
+    sup.sup_superiorize(H, xa, 7, P.N, P.beta0, P.a, objective="dose", lam=P.lam, use_graph=True)
+    sup.sup_superiorize(H, xb, 7, P.N, P.beta0, P.a, objective="dose", lam=P.lam, use_graph=False)
+    assert torch.equal(xa, xb)
+
+
+def test_gram_matrix_is_dT_d():
+    """G x and x^T G x of the Gram path against a dense fp64 restatement, through the public calls: one phase with a step so small
+    that x does not move (beta0 tiny) reports f(x) = x^T G x; odd n (row padding) and rows longer than 64 entries included"""
+    sup = _sup()
+    rng = np.random.default_rng(11)
+    md, n = 700, 77  # n not a multiple of 4 or 32; n^2 <= 2 nnz holds
+    Dd = rng.uniform(0, 1, (md, n)) * (rng.random((md, n)) < 0.9)  # ~69 entries per row: the > 64 branch of the build kernel runs
+    Dd[5] = 0.0  # an empty row
+    rp = np.zeros(md + 1, np.int64)
+    cols, vals = [], []
+    for i in range(md):
+        nz = np.flatnonzero(Dd[i])
+        cols.append(nz)
+        vals.append(Dd[i, nz])
+        rp[i + 1] = rp[i] + nz.size
+    c, v = np.concatenate(cols).astype(np.int32), np.concatenate(vals)
+    assert n * n <= 2 * rp[-1] and np.diff(rp).max() > 64
+    eye_rp, eye_c = np.arange(n + 1, dtype=np.int64), np.arange(n, dtype=np.int32)
+    for dtype in (0, 1):
+        H = sup.sup_create(eye_rp, eye_c, np.ones(n, np.float32), np.zeros(n, np.float32), np.full(n, 9.0, np.float32), np.zeros(n, np.float32),
+                           np.full(n, 9.0, np.float32), None, dtype=dtype, n=n)
+        sup.sup_set_dose_matrix(H, rp, c, v.astype(np.float32))
+        D32 = Dd.astype(np.float32).astype(np.float64)
+        G = D32.T @ D32
+        xs = rng.uniform(0.5, 1.5, n).astype(np.float32)
+        x = xdev(xs, dtype)
+        sup.sup_perturb_dose(H, x, 1, 1e-30, 0.5, 0)
+        st = sup.sup_get_state(H)
+        f = xs.astype(np.float64) @ G @ xs.astype(np.float64)
+        assert abs(st["f"] - f) <= (2e-6 if dtype == 0 else 1e-12) * f
+        # one real step: x - c g with g = 2 G x, c = beta0 / ||g||
+        x = xdev(xs, dtype)
+        sup.sup_perturb_dose(H, x, 1, 0.01, 0.5, 0)
+        g = 2 * G @ xs.astype(np.float64)
+        want = xs.astype(np.float64) - 0.01 * g / np.linalg.norm(g)
+        assert rel_l2(x.cpu().numpy(), want) <= (2e-7 if dtype == 0 else 1e-13)
