@@ -114,9 +114,9 @@ struct GramVec<double> {
     static __device__ __forceinline__ double dot(const double2& a, const double2& b, double acc) { return fma(a.y, b.y, fma(a.x, b.x, acc)); }
 };
 
-template <typename T>
+template <typename T, bool VG>
 __global__ void __launch_bounds__(32 * GRAM_MV_WARPS, 1)
-    k_gram_matvec(const T* __restrict__ G, int n, int64_t ld, int rows_per_cta, const T* __restrict__ v, double scale, T* __restrict__ out,
+    k_gram_matvec(const T* __restrict__ G, int n, int64_t ld, const T* __restrict__ v, double scale, T* __restrict__ out,
                   double* __restrict__ red_vu, double* __restrict__ red_uu, const DevState* __restrict__ st) {
     if (*(volatile const int*)&st->stop) return;
     typedef typename GramVec<T>::V V;
@@ -125,11 +125,16 @@ __global__ void __launch_bounds__(32 * GRAM_MV_WARPS, 1)
     T* vs = reinterpret_cast<T*>(gram_smem);                                                // [ld]
     double* part = reinterpret_cast<double*>(gram_smem + ((size_t(ld) * sizeof(T) + 15) & ~size_t(15)));  // [rows_per_cta][GRAM_MV_WARPS]
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    for (int64_t q = threadIdx.x; q < ld; q += blockDim.x) vs[q] = q < n ? v[q] : T(0);
-    __syncthreads();
-    const int r0 = blockIdx.x * rows_per_cta, r1 = min(n, r0 + rows_per_cta);
+    if (!VG) {
+        for (int64_t q = threadIdx.x; q < ld; q += blockDim.x) vs[q] = q < n ? v[q] : T(0);
+        __syncthreads();
+    }
+    const int r0 = int(int64_t(blockIdx.x) * n / gridDim.x), r1 = int(int64_t(blockIdx.x + 1) * n / gridDim.x);  // rows split evenly (+-1)
     const int nvec = int(ld / VEC);
-    const V* vsv = reinterpret_cast<const V*>(vs);
+    // VG: v is 16-byte aligned and read through L1 (32 KB at n = 8 000: it stays there), which saves the staging pass and its barrier;
+    // the last, partial vector of v is assembled from scalars (G's padding is zero, v's does not exist)
+    const V* vsv = reinterpret_cast<const V*>(VG ? v : vs);
+    const int nfull = n / VEC;
     for (int r = r0; r < r1; r += GRAM_MV_ROWS) {
         const V* gp[GRAM_MV_ROWS];
         T acc[GRAM_MV_ROWS];
@@ -142,7 +147,17 @@ __global__ void __launch_bounds__(32 * GRAM_MV_WARPS, 1)
             V a[GRAM_MV_ROWS];
 #pragma unroll
             for (int u = 0; u < GRAM_MV_ROWS; ++u) a[u] = __ldcs(gp[u] + c);
-            const V b = vsv[c];
+            V b;
+            if (!VG) {
+                b = vsv[c];
+            } else if (c < nfull) {
+                b = __ldg(vsv + c);
+            } else {
+                T t[VEC];
+#pragma unroll
+                for (int e = 0; e < VEC; ++e) t[e] = c * VEC + e < n ? __ldg(v + c * VEC + e) : T(0);
+                b = *reinterpret_cast<const V*>(t);
+            }
 #pragma unroll
             for (int u = 0; u < GRAM_MV_ROWS; ++u) acc[u] = GramVec<T>::dot(a[u], b, acc[u]);
         }
@@ -162,7 +177,7 @@ __global__ void __launch_bounds__(32 * GRAM_MV_WARPS, 1)
         double u = 0.0;
         for (int w = 0; w < GRAM_MV_WARPS; ++w) u += part[rl * GRAM_MV_WARPS + w];
         out[r0 + rl] = T(scale * u);
-        pvu += double(vs[r0 + rl]) * u;
+        pvu += double(v[r0 + rl]) * u;
         puu += u * u;
     }
     // rows_per_cta <= blockDim.x: thread rl holds row rl's terms; sum them in row order
@@ -187,10 +202,13 @@ __global__ void __launch_bounds__(32 * GRAM_MV_WARPS, 1)
     }
 }
 
-// ---- the scalar part of a reduction step (one thread) -----------------------------------------------------------------------------
+// ---- the scalar part of a reduction step (one warp for the sums, one thread for the rest) -----------------------------------------------------------------------------
+// sum of np per-CTA partials by one warp: lane l adds entries l, l + 32, ..., then a butterfly -- a fixed order
 __device__ __forceinline__ double gram_sum(const double* __restrict__ p, int np) {
     double s = 0.0;
-    for (int q = 0; q < np; ++q) s += __ldcg(p + q);
+    for (int q = threadIdx.x; q < np; q += 32) s += __ldcg(p + q);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
     return s;
 }
 // first: f(x) = sum x u and ||g_0||^2 = 4 sum u^2 from pass 0; later steps: f carried as the closed form, ||g||^2 from k_gram_apply.
@@ -202,11 +220,12 @@ __global__ void k_gram_trial(DevState* st, const double* __restrict__ red_xu, co
     if (st->stop) return;
     const long long k = st->k;
     if (final_only) {
+        if (threadIdx.x != 0) return;
         st->f = st->f_cur;
         if (step_rule == SUP_RULE_ADAPTIVE && st->f_start <= st->f_ref) st->f_ref = shrink * st->f_start;  // A-30
         return;
     }
-    if (first && n_restart > 0 && k > 0 && k % n_restart == 0) {  // restarted perturbations (A-24)
+    if (threadIdx.x == 0 && first && n_restart > 0 && k > 0 && k % n_restart == 0) {  // restarted perturbations (A-24)
         st->ell = k / n_restart;
         st->apow = 1.0;
         for (long long q = 0; q < st->ell; ++q) st->apow *= a;
@@ -215,15 +234,16 @@ __global__ void k_gram_trial(DevState* st, const double* __restrict__ red_xu, co
     if (first) {
         fx = gram_sum(red_xu, np_mv);
         s2 = 4.0 * gram_sum(red_uu, np_mv);
-        st->f_start = fx;
     } else {
         s2 = gram_sum(part_gg, np_apply);
     }
+    const double q2 = gram_sum(red_gw, np_mv);
+    if (threadIdx.x != 0) return;  // the warp did the sums; one thread runs the trial loop
+    if (first) st->f_start = fx;
     if (!isfinite(fx)) atomicOr(&st->fault, 2);
     st->f_cur = fx;
     st->f = fx;
     st->cf = 0.0;
-    const double q2 = gram_sum(red_gw, np_mv);
     const double s = sqrt(s2);
     if (step_rule == SUP_RULE_ADAPTIVE) {  // Eq. 11 (A-30): no trial loop
         const bool take = fx > st->f_ref && s > 0.0;
@@ -304,7 +324,8 @@ __global__ void __launch_bounds__(SUP_THREADS)
 }
 
 // ---- host side ----------------------------------------------------------------------------------------------------------------------
-static int gram_rows_per_cta(const sup_ctx* h) { return int((h->n + h->num_sms - 1) / h->num_sms); }
+static int gram_mv_grid(const sup_ctx* h) { return int(std::min<int64_t>(h->n, h->num_sms)); }
+static int gram_rows_per_cta(const sup_ctx* h) { return int((h->n + gram_mv_grid(h) - 1) / gram_mv_grid(h)); }
 static size_t gram_mv_smem(const sup_ctx* h) {
     return ((size_t(h->gram_ld) * h->esz + 15) & ~size_t(15)) + size_t(gram_rows_per_cta(h)) * GRAM_MV_WARPS * sizeof(double);
 }
@@ -317,11 +338,12 @@ static sup_status gram_build_t(sup_ctx* h) {
     SUP_CUDA(h, cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, h->device));
     cudaFuncAttributes fb, fm;
     SUP_CUDA(h, cudaFuncGetAttributes(&fb, k_gram_build<T>));
-    SUP_CUDA(h, cudaFuncGetAttributes(&fm, k_gram_matvec<T>));
+    SUP_CUDA(h, cudaFuncGetAttributes(&fm, k_gram_matvec<T, false>));
     const int dyn_b = optin - int(fb.sharedSizeBytes), dyn_m = optin - int(fm.sharedSizeBytes);
     if (int64_t(smem) > dyn_b || int64_t(gram_mv_smem(h)) > dyn_m) return sup_fail(h, SUP_ERR_STATE, "Gram path: shared memory of this device is too small");
     SUP_CUDA(h, cudaFuncSetAttribute(k_gram_build<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn_b));
-    SUP_CUDA(h, cudaFuncSetAttribute(k_gram_matvec<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn_m));
+    SUP_CUDA(h, cudaFuncSetAttribute(k_gram_matvec<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn_m));
+    SUP_CUDA(h, cudaFuncSetAttribute(k_gram_matvec<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn_m));
     int per_sm = 1;
     SUP_CUDA(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_gram_build<T>, GRAM_BUILD_THREADS, smem));
     const int grid = int(std::min<int64_t>(n, int64_t(h->num_sms) * std::max(per_sm, 1)));
@@ -335,17 +357,16 @@ sup_status sup_gram_build(sup_ctx* h) { return h->dt == SUP_F32 ? gram_build_t<f
 
 template <typename T>
 static sup_status gram_matvec_t(sup_ctx* h, const void* v, double scale, void* out, double* red_vu, double* red_uu) {
-    const int rpc = gram_rows_per_cta(h);
-    const int grid = int((h->n + rpc - 1) / rpc);
+    const int grid = gram_mv_grid(h);
     const size_t smem = gram_mv_smem(h);
-    k_gram_matvec<T><<<grid, 32 * GRAM_MV_WARPS, smem, h->stream>>>(static_cast<const T*>(h->gram), int(h->n), h->gram_ld, rpc, static_cast<const T*>(v), scale,
-                                                                   static_cast<T*>(out), red_vu, red_uu, h->state);
+    if ((reinterpret_cast<uintptr_t>(v) & 15u) == 0)
+        k_gram_matvec<T, true><<<grid, 32 * GRAM_MV_WARPS, smem, h->stream>>>(static_cast<const T*>(h->gram), int(h->n), h->gram_ld, static_cast<const T*>(v),
+                                                                             scale, static_cast<T*>(out), red_vu, red_uu, h->state);
+    else
+        k_gram_matvec<T, false><<<grid, 32 * GRAM_MV_WARPS, smem, h->stream>>>(static_cast<const T*>(h->gram), int(h->n), h->gram_ld, static_cast<const T*>(v),
+                                                                              scale, static_cast<T*>(out), red_vu, red_uu, h->state);
     h->launches++;
     return SUP_OK;
-}
-static int gram_mv_grid(const sup_ctx* h) {
-    const int rpc = gram_rows_per_cta(h);
-    return int((h->n + rpc - 1) / rpc);
 }
 
 sup_status sup_launch_perturb_dose_gram(sup_ctx* h, void* x, const PerturbParams& pp) {
@@ -360,7 +381,7 @@ sup_status sup_launch_perturb_dose_gram(sup_ctx* h, void* x, const PerturbParams
     for (int nred = 0; nred < pp.N; ++nred) {
         rc = f32 ? gram_matvec_t<float>(h, h->g, 1.0, h->gram_w, red_gw, red_scratch) : gram_matvec_t<double>(h, h->g, 1.0, h->gram_w, red_gw, red_scratch);  // w = G g
         if (rc != SUP_OK) return rc;
-        k_gram_trial<<<1, 1, 0, h->stream>>>(h->state, red_xu, red_uu, np_mv, red_gw, h->partials, grid, nred == 0, 0, pp.beta0, pp.a, pp.policy, pp.n_restart,
+        k_gram_trial<<<1, 32, 0, h->stream>>>(h->state, red_xu, red_uu, np_mv, red_gw, h->partials, grid, nred == 0, 0, pp.beta0, pp.a, pp.policy, pp.n_restart,
                                              pp.decisions, pp.decision_f, pp.cap, pp.step_rule, pp.shrink);
         void* mir = nred == pp.N - 1 ? mirror : nullptr;
         if (f32)
@@ -371,7 +392,7 @@ sup_status sup_launch_perturb_dose_gram(sup_ctx* h, void* x, const PerturbParams
                                                                       static_cast<const double*>(h->gram_w), h->n, static_cast<double*>(mir), h->xmap, h->partials);
         h->launches += 2;
     }
-    k_gram_trial<<<1, 1, 0, h->stream>>>(h->state, red_xu, red_uu, np_mv, red_gw, h->partials, grid, 0, 1, pp.beta0, pp.a, pp.policy, pp.n_restart, pp.decisions,
+    k_gram_trial<<<1, 32, 0, h->stream>>>(h->state, red_xu, red_uu, np_mv, red_gw, h->partials, grid, 0, 1, pp.beta0, pp.a, pp.policy, pp.n_restart, pp.decisions,
                                          pp.decision_f, pp.cap, pp.step_rule, pp.shrink);
     h->launches++;
     SUP_CUDA(h, cudaGetLastError());

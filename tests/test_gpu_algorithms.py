@@ -518,3 +518,10 @@ def test_gram_matrix_is_dT_d():
         g = 2 * G @ xs.astype(np.float64)
         want = xs.astype(np.float64) - 0.01 * g / np.linalg.norm(g)
         assert rel_l2(x.cpu().numpy(), want) <= (2e-7 if dtype == 0 else 1e-13)
+        # an x that is not 16-byte aligned takes the kernel variant that stages the vector in shared memory: same bits
+        buf = torch.zeros(n + 1, dtype=TD[dtype], device="cuda:0")
+        xm = buf[1:]
+        xm.copy_(xdev(xs, dtype))
+        assert xm.data_ptr() % 16 != 0
+        sup.sup_perturb_dose(H, xm, 1, 0.01, 0.5, 0)
+        assert torch.equal(xm, x)
