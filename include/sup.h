@@ -193,10 +193,12 @@ sup_status sup_set_layout(sup_handle h, const int64_t* x_shape, const int64_t* y
 
 /* Expert control of the two product kernels (S1+S2, S3), for tests and measurements: how many
  * lanes cooperate on one row of A (forward) and of A^T (backward).  -1: the planner's choice from the mean and the
- * longest row (default); 1: SEGMENTS -- the warps take fixed-size pieces of the matrix stream whatever rows they belong to (the
- * planner's choice for rows of >= 128 entries on average); 4, 8, 16, 32: that many lanes of a warp per row; 64: a pair of warps per row; 0: the whole CTA
- * per row (what the planner picks for rows of thousands of nonzeros); -2 (either argument): do not use the bulk-copy
- * staged kernels at all but the plain group-per-row kernels.  A request that the longest row cannot satisfy is
+ * longest row (default); 2, 4, 8, 16, 32: that many lanes of a warp per row (the planner's choice for rows of up to ~1000 entries:
+ * 2 lanes up to ~60 entries per row, 32 from ~500); 64: a pair of warps per row; 128: CHUNKS -- a row is cut into pieces of 512 entries
+ * that go to the warps round-robin, the last warp to finish a row adds the pieces in order (the planner's choice for rows of more
+ * than 2048 entries on average, longest row <= 65536); 0: the whole CTA per row (rows longer than that); 1: SEGMENTS -- the warps
+ * take fixed-size pieces of the matrix stream whatever rows they belong to (never chosen: slower, profiles/r02j_segments.md);
+ * -2 (either argument): do not use the bulk-copy staged kernels at all but the plain group-per-row kernels.  A request that the longest row cannot satisfy is
  * widened by the planner.  Re-plans in place, drops the cached graph, synchronises the stream.  Results differ
  * between settings only by the summation order inside a row. */
 sup_status sup_set_row_mode(sup_handle h, int lanes_forward, int lanes_backward);

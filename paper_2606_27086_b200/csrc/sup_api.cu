@@ -365,8 +365,8 @@ extern "C" sup_status sup_set_row_mode(sup_handle h, int lanes_forward, int lane
     if (!h) return SUP_ERR_INVALID_ARG;
     SUP_ENTER(h);
     for (int v : {lanes_forward, lanes_backward})
-        if (!(v == -2 || v == -1 || v == 0 || v == 1 || v == 4 || v == 8 || v == 16 || v == 32 || v == 64))
-            return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_set_row_mode: lanes must be -2, -1, 0, 1, 4, 8, 16, 32 or 64");
+        if (!(v == -2 || v == -1 || v == 0 || v == 1 || v == 2 || v == 4 || v == 8 || v == 16 || v == 32 || v == 64 || v == 128))
+            return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_set_row_mode: lanes must be -2, -1, 0, 1, 2, 4, 8, 16, 32, 64 or 128");
     SUP_CUDA(h, cudaStreamSynchronize(h->stream));
     drop_graph(h);
     h->use_stream = lanes_forward != -2 && lanes_backward != -2;

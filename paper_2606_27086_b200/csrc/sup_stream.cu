@@ -51,6 +51,11 @@ struct RgShape {
 #define RG_SEG_MIN_AVG 1e300                // mean row length from which the planner would pick the segment mode (G = 1): never --
                                             // it is correct but 1.7-3.7x slower than the row modes (profiles/r02j_segments.md); sup_set_row_mode(h, 1, 1) selects it
 #endif
+// G == 128 (chunks of long rows): pool of chunk partial sums and row counters; see the consumer branch for the bounds
+#define RG_CHUNK_POOL 256
+#define RG_CHUNK_ROWS 64
+#define RG_CHUNK_KMAX 128
+static_assert(sizeof(float) * RG_CHUNK_POOL + 4 * RG_CHUNK_ROWS <= 8 * RG_NCARRY, "the chunk pool must fit the carry slots' space");
 #define RG_CWARPS 24                        // upper bound on the consumer warps (sizes of the shared arrays)
 #ifndef RG_NPROD
 #define RG_NPROD 2                          // producer warps: ONE thread issues at most one bulk copy per ~270 ns whatever its size
@@ -182,7 +187,15 @@ struct RgSmem {
     double red[RG_CWARPS];    // per consumer warp: its share of the kernel's reduction
     // G == 1: slot s mod RG_NCARRY = (partial sum of the row left open at the end of segment s, 1 + s), written and read as ONE
     // vector access so that no fence is needed between value and flag
-    typename CarrySlot<T>::type carry[RG_NCARRY];
+    // G == 128: partial sums of the chunks of multi-chunk rows (a pool indexed by the running chunk number) and one arrival
+    // counter per such row; shares its space with the carry slots (never both in one kernel)
+    union {
+        typename CarrySlot<T>::type carry[RG_NCARRY];
+        struct {
+            T part[RG_CHUNK_POOL];
+            int cnt[RG_CHUNK_ROWS];
+        } ck;
+    };
 };
 
 // Dot product of the ring elements k, k+G, k+2G, ... < e (offsets relative to the stream base) with gathered vec
@@ -342,7 +355,11 @@ __global__ void __launch_bounds__(32 * (NCW + RG_NPROD), 1)
         for (int s = 0; s < STG; ++s) mbar_init(smem_u32(&S.full[s]), 1);
         for (int w = 0; w < NCW; ++w) S.progress[w] = 0;
         for (int st = 0; st < STG; ++st) S.issued[st] = 0;
-        for (int q = 0; q < RG_NCARRY; ++q) CarrySlot<T>::put(&S.carry[q], T(0), 0);
+        if constexpr (G == 128) {
+            for (int q = 0; q < RG_CHUNK_ROWS; ++q) S.ck.cnt[q] = 0;
+        } else {
+            for (int q = 0; q < RG_NCARRY; ++q) CarrySlot<T>::put(&S.carry[q], T(0), 0);
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -481,6 +498,99 @@ __global__ void __launch_bounds__(32 * (NCW + RG_NPROD), 1)
             }
             s = s_next;
             e = e_next;
+        }
+        __syncwarp();
+        if (lane == 0) progress[warp] = ntiles;
+    } else if constexpr (G == 128) {
+    // ---- consumers, G == 128: CHUNKS of long rows (rows of thousands of entries: config 4's A^T) -----------------------------------
+    // A row of len elements is K = ceil(len / CHK) chunks of CHK = 32 x RG_UNROLL elements, aligned to the row's start; the chunks of
+    // the CTA's rows, numbered in stream order, go to the warps round-robin (chunk u to warp u mod NCW).  Every trip but a row's last
+    // is full, no warp waits for another, and the ring span of the warps in flight is NCW chunks whatever the row lengths.  A warp
+    // leaves its chunk's sum in the pool (slot = running chunk number of the multi-chunk rows, mod RG_CHUNK_POOL) and counts itself
+    // in on the row's counter; the warp that arrives last adds the K sums IN CHUNK ORDER and runs the epilogue, so the row value does
+    // not depend on the timing.  Bounds: a multi-chunk row has more than CHK (K - 1) elements and the warps are at most one ring
+    // (<= 24 576 elements) apart, so at most 48 multi-chunk rows and 96 + K pool slots are live at once: RG_CHUNK_ROWS = 64,
+    // K <= RG_CHUNK_KMAX = 128 (the planner checks the longest row) with RG_CHUNK_POOL = 256.
+        constexpr int CHK = 32 * RG_UNROLL;
+        int seen = 0, released = 0;
+        int u0 = 0;  // chunks before row r (all rows)
+        int mc = 0;  // chunks before row r, multi-chunk rows only
+        int mr = 0;  // multi-chunk rows before row r
+        int64_t rp = rowptr[rs];
+        for (int64_t r = rs; r < re; ++r) {
+            const int s = int(rp - base);
+            rp = rowptr[r + 1];
+            const int e = int(rp - base);
+            const int K = (e - s + CHK - 1) / CHK;
+            if (K == 0) {  // empty row: its epilogue by one lane of one warp
+                if (int((r - rs) % NCW) == warp && lane == 0) {
+                    T q1, q2, q3, q4;
+                    row_operands<T, MODE>(r, p1, p2, p3, out, q1, q2, q3, q4);
+                    row_epilogue<T, MODE>(r, T(0), q1, q2, q3, q4, out, out2, lambda, omap, racc);
+                }
+                continue;
+            }
+            int c = (warp - u0 % NCW + NCW) % NCW;  // this warp's first chunk of the row
+            for (; c < K; c += NCW) {
+                const int ps = s + c * CHK;
+                const int pe = e < ps + CHK ? e : ps + CHK;
+                int t_start = ps / RG_TILE;
+                t_start = t_start < ntiles ? t_start : ntiles;
+                if (released < t_start) {
+                    released = t_start;
+                    if (lane == 0) progress[warp] = t_start;
+                }
+                const int t_hi = (pe - 1) / RG_TILE;
+                for (int t = seen > t_start ? seen : t_start; t <= t_hi; ++t) {
+                    const int st = t % STG;
+                    if (issued[st] != t + 1) {
+                        const long long t0 = clock64();
+                        while (issued[st] != t + 1)
+                            if (clock64() - t0 > RG_TIMEOUT) __trap();
+                    }
+                    mbar_wait(smem_u32(&S.full[st]), (t / STG) & 1);
+                }
+                seen = seen > t_hi + 1 ? seen : t_hi + 1;
+                asm volatile("" ::: "memory");
+                int rel = pe / RG_TILE;
+                rel = rel < ntiles ? rel : ntiles;
+                rel = rel > released ? rel : released;
+                T a0 = T(0), a1 = T(0), a2 = T(0), a3 = T(0);
+                const bool wraps = (ps % RG_ELEMS) + (pe - ps) > RG_ELEMS;
+                if (!wraps) ring_row_dot<T, 32, false, STG>(S.d, vec, ps + lane, pe, 1, progress + warp, rel, lane == 0, a0, a1, a2, a3);
+                else ring_row_dot<T, 32, true, STG>(S.d, vec, ps + lane, pe, 1, progress + warp, rel, lane == 0, a0, a1, a2, a3);
+                released = rel;
+                T acc = (a0 + a1) + (a2 + a3);
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+                if (lane == 0) {
+                    bool finish = K == 1;
+                    T tot = acc;
+                    if (K > 1) {
+                        volatile T* pool = S.ck.part;
+                        pool[(mc + c) % RG_CHUNK_POOL] = acc;
+                        __threadfence_block();
+                        const int arrived = atomicAdd(&S.ck.cnt[mr % RG_CHUNK_ROWS], 1);
+                        if (arrived == K - 1) {  // the last chunk to arrive: add the K sums in chunk order
+                            __threadfence_block();
+                            tot = T(0);
+                            for (int q = 0; q < K; ++q) tot += pool[(mc + q) % RG_CHUNK_POOL];
+                            S.ck.cnt[mr % RG_CHUNK_ROWS] = 0;
+                            finish = true;
+                        }
+                    }
+                    if (finish) {
+                        T q1, q2, q3, q4;
+                        row_operands<T, MODE>(r, p1, p2, p3, out, q1, q2, q3, q4);
+                        row_epilogue<T, MODE>(r, tot, q1, q2, q3, q4, out, out2, lambda, omap, racc);
+                    }
+                }
+            }
+            u0 += K;
+            if (K > 1) {
+                mc += K;
+                ++mr;
+            }
         }
         __syncwarp();
         if (lane == 0) progress[warp] = ntiles;
@@ -993,15 +1103,19 @@ sup_status sup_stream_plan(sup_ctx* h, const CsrD& M, int64_t r0, int64_t r1, bo
     // amortise the per-row work, few enough that the consumer warps' rows together leave ring stages free for prefetch --
     // and must never span more than RG_STAGES_MIN - 1 tiles.  sup_set_row_mode() overrides the choice.
     const double avg = double(ends[1] - ends[0]) / double(r1 - r0);
-    int G = 4;
+    int G = 2;  // (2 lanes per row for rows of up to ~60 entries: config 4's forward product 3 190 -> 5 170 GB/s against 4 lanes)
     while (G < 32 && avg * (32.0 / G) > 960.0) G <<= 1;
-    if (avg >= RG_SEG_MIN_AVG || avg > 2048.0) G = 1;  // rows of thousands of entries (config 4's A^T): segments of the stream, 12 % faster
-                                                          // than the whole-CTA-per-row mode there (2 735 -> 3 069 GB/s); never for hundreds
+    if (avg >= RG_SEG_MIN_AVG) G = 1;
+    else if (avg > 2048.0) G = 128;  // rows of thousands of entries (config 4's A^T): chunks of rows round-robin over the warps
     const int forced = forward ? h->lanes_fwd : h->lanes_bwd;
     if (forced >= 0) G = forced;
     const int64_t cap = int64_t(RG_STAGES_MIN - 2) * RG_TILE;
-    while (G < 32 && G > 1 && int64_t(mx_h) * (32 / G) > cap) G <<= 1;
-    if (G > 1 && int64_t(mx_h) * (G >= 32 ? 1 : 32 / G) > cap) G = 0;  // a row too long for the ring in a lanes-per-row mode: the whole CTA per row
+    if (G == 128) {
+        if (int64_t(mx_h) > int64_t(RG_CHUNK_KMAX) * 32 * RG_UNROLL) G = 0;  // more chunks than the pool allows: the whole CTA per row
+    } else {
+        while (G < 32 && G > 1 && int64_t(mx_h) * (32 / G) > cap) G <<= 1;
+        if (G > 1 && int64_t(mx_h) * (G >= 32 ? 1 : 32 / G) > cap) G = 0;  // a row too long for the ring in a lanes-per-row mode: the whole CTA per row
+    }
     out->max_row = int64_t(mx_h);
     out->part = static_cast<const int64_t*>(table);
     out->nb = nb;
@@ -1033,11 +1147,13 @@ template <typename T, int MODE, bool DEEP>
 static void launch_staged_d(sup_ctx* h, const StreamPlan& sp, const CsrD& M, const void* vec, const void* p1, const void* p2,
                             const void* p3, void* out, void* out2, double lambda, const GMap& omap, double* red_out) {
     switch (sp.G) {
+        case 2: launch_staged_g<T, MODE, 2, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap, red_out); break;
         case 4: launch_staged_g<T, MODE, 4, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap, red_out); break;
         case 8: launch_staged_g<T, MODE, 8, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap, red_out); break;
         case 16: launch_staged_g<T, MODE, 16, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap, red_out); break;
         case 64: launch_staged_g<T, MODE, 64, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap, red_out); break;
         case 0: launch_staged_g<T, MODE, 0, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap, red_out); break;
+        case 128: launch_staged_g<T, MODE, 128, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap, red_out); break;
         case 1: launch_staged_g<T, MODE, 1, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap, red_out); break;
         default: launch_staged_g<T, MODE, 32, DEEP>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap, red_out); break;
     }

@@ -666,12 +666,12 @@ def test_restarted_perturbations(dtype):
 
 
 @pytest.mark.parametrize("dtype", [0, 1])
-@pytest.mark.parametrize("lanes", [0, 1, 64])
+@pytest.mark.parametrize("lanes", [0, 1, 2, 64, 128])
 @pytest.mark.parametrize("name", ["cfg4_small", "ct_ragged", "cfg5_k16", "cfg2"])
 def test_long_row_mode_of_the_staged_kernels(name, lanes, dtype):
-    """The whole-CTA-per-row mode (lanes = 0; chosen for rows of thousands of nonzeros: config 4's A^T at full size), the segment
-    mode (lanes = 1) and the warp-pair mode (64) forced on both products of small problems, including rows shorter than a piece,
-    empty rows and rows spanning several ring tiles."""
+    """The whole-CTA-per-row mode (lanes = 0), the segment mode (1), two lanes per row (2), the warp-pair mode (64) and the chunk mode
+    (128; chosen for rows of thousands of nonzeros: config 4's A^T at full size) forced on both products of small problems,
+    including rows shorter than a piece, empty rows and rows spanning several ring tiles."""
     sup = _sup()
     P = problem(name)
     H = make_handle(P, dtype, blocks=False)
