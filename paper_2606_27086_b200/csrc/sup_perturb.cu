@@ -613,6 +613,9 @@ __global__ void __launch_bounds__(SUP_THREADS) k_perturb_tv(PArgs<T> Ain) {
     const long long k = *(volatile long long*)&st->k;
     long long ndec = *(volatile long long*)&st->n_dec;
     unsigned gen = *(volatile unsigned*)&st->bar_gen;  // read before this CTA's first arrival, so before any flip of this launch
+    // Eq. 11's reference: like every other field of the state it is read HERE, before this CTA's first arrival at a grid barrier --
+    // CTA 0 rewrites it at the end of the kernel, which it can only reach after every CTA has arrived at the first barrier
+    const double f_ref = *(volatile double*)&st->f_ref;
     long long trials = 0;
     // restarted perturbations (A-24): at the start of sweep k = r * n_restart the exponent is reset to r
     if (A.n_restart > 0 && k > 0 && k % A.n_restart == 0) {
@@ -664,7 +667,6 @@ __global__ void __launch_bounds__(SUP_THREADS) k_perturb_tv(PArgs<T> Ain) {
     // Eq. 11 (A-30): beta = (f - f_ref)/||g|| when f > f_ref, else 0; the step x - ((f - f_ref)/||g||^2) g is
     // taken as it is -- no trial loop, no exponent.  Same passes as an always-accepted first candidate: 1 + N in all.
     const bool adaptive = A.step_rule == SUP_RULE_ADAPTIVE;
-    const double f_ref = adaptive ? *(volatile double*)&st->f_ref : 0.0;
     const double f_start = fx;
     for (int nred = 0; ok && adaptive && nred < A.N; ++nred) {
         const bool take = fx > f_ref && s > 0.0;

@@ -1162,6 +1162,10 @@ static void launch_staged_d(sup_ctx* h, const StreamPlan& sp, const CsrD& M, con
 template <typename T, int MODE>
 static void launch_staged(sup_ctx* h, const StreamPlan& sp, const CsrD& M, const void* vec, const void* p1, const void* p2,
                           const void* p3, void* out, void* out2, double lambda, const GMap& omap, bool deep, double* red_out = nullptr) {
+    // the deeper shape also pays when the gathered vector stays in L1 anyway (config 4's x: 32 KB) and in the chunk mode, whose ring
+    // span does not grow with the rows (config 4: forward 121 -> 114 us, back-projection 154 -> 148 us); with scattered gathers it
+    // costs L1 capacity (config 5: -3 %)
+    deep = deep || M.cols * int64_t(sizeof(T)) <= 49152 || sp.G == 128;
     if (deep && sizeof(T) == 4) launch_staged_d<T, MODE, true>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap, red_out);
     else launch_staged_d<T, MODE, false>(h, sp, M, vec, p1, p2, p3, out, out2, lambda, omap, red_out);
 }
