@@ -271,6 +271,21 @@ sup_status sup_proximity(sup_handle h, const void* x, int mode, double p, double
 /* Objective value f(x) for `kind` (sup_objective_kind); shape is a HOST array (TV2D: {ny, nx}).  *out is HOST. */
 sup_status sup_objective(sup_handle h, const void* x, int kind, const int64_t* shape, double* out);
 
+/* The ONE entry point that allocates nothing and needs no handle: the TV2D objective value f(X) of PAPER.md:L308-311 Eq. 15
+ * (= sup_objective(h, x, SUP_OBJ_TV2D, {ny, nx}, .)), for callers that cannot call cudaMalloc at that point (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid it).  Its scratch -- one partial sum per image row and an arrival counter --
+ * is a file-scope __device__ array of SUP_STATIC_MAX_ROWS doubles (128 KB) that every GPU which loads the library holds until the
+ * process exits; no cudaMalloc, cudaFree or allocating library routine is called.
+ *   x        DEVICE, [ny*nx] row-major, of type `dtype` (SUP_F32 / SUP_F64), on the CURRENT device (checked);
+ *   out_dev  DEVICE, one double, written by the kernel;   stream: cudaStream_t as void* (NULL = default stream).
+ * Asynchronous (the value is in *out_dev when the stream reaches that point).  ny > SUP_STATIC_MAX_ROWS or nx > 2^31 is refused with
+ * SUP_ERR_INVALID_ARG before any launch (text through sup_last_error(NULL)).  Terms and sums in fp64, fixed summation order (row
+ * sums, then the rows in order): the value differs from sup_objective's by the summation order only.
+ * The scratch is SHARED by all calls on a device and keeps the last call's contents; each call clears the counter and overwrites
+ * every row slot it reads.  Calls that OVERLAP on one GPU (different streams or host threads) RACE on it: serialise them. */
+#define SUP_STATIC_MAX_ROWS 16384
+sup_status sup_tv2d_value_static(const void* x, int dtype, int64_t ny, int64_t nx, double* out_dev, void* stream);
+
 /* Copies derived arrays for inspection/tests: which = 0: d [m] (dtype); 1: A^T rowptr [n+1] int64;
  * 2: A^T col [nnz] int32 (original row indices); 3: A^T val [nnz] (dtype); 5: y [m] (dtype), the scaled violation
  * d_i c_i(x) left by the last forward product (sup_forward_violation or a sweep).  dst is a DEVICE pointer. */

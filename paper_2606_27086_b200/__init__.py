@@ -32,6 +32,7 @@ from .binding import (  # noqa: F401
     sup_set_row_mode,
     sup_superiorize,
     sup_superiorize_host,
+    sup_tv2d_value_static,
     sup_workspace_bytes,
     OBJ_NONE, OBJ_TV2D, OBJ_TV1D, OBJ_DOSE, OBJ_MEAN, OBJ_TV3D, PER_TRIAL, PER_SWEEP, F32, F64,
 )

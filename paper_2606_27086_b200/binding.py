@@ -71,6 +71,7 @@ def lib():
         L.sup_perturb_dose.argtypes = [c_void_p, c_void_p, c_int, c_double, c_double, POINTER(c_int64)]
         L.sup_perturb_mean.argtypes = [c_void_p, c_void_p, c_int, c_double, c_double, POINTER(c_int64)]
         L.sup_set_dose_mode.argtypes = [c_void_p, c_int]
+        L.sup_tv2d_value_static.argtypes = [c_void_p, c_int, c_int64, c_int64, c_void_p, c_void_p]
         L.sup_perturb_adaptive.argtypes = [c_void_p, c_void_p, c_int, POINTER(c_int64), c_int, POINTER(c_double), c_double]
         L.sup_project_drop.argtypes = [c_void_p, c_void_p, c_double, c_int]
         L.sup_backproject_partial.argtypes = [c_void_p, c_void_p, c_double]
@@ -412,6 +413,26 @@ def sup_objective(H: SupHandle, x: torch.Tensor, kind, shape=None) -> float:
     H._check(lib().sup_objective(H.h, _ptr(x), k, sh, byref(out)))
     H._exit()
     return out.value
+
+
+STATIC_MAX_ROWS = 16384
+
+
+def sup_tv2d_value_static(x: torch.Tensor, shape, out: torch.Tensor = None, sync=True):
+    """TV2D value of the device tensor x (float32 / float64, ny*nx elements) through the entry point that allocates nothing
+    (sup_tv2d_value_static; scratch in a static device array, at most STATIC_MAX_ROWS rows).  out: a device float64 tensor of one
+    element (allocated here when None -- the C entry itself takes it from the caller).  Runs on torch's current stream.
+    Returns the value as a float when sync, else `out`."""
+    assert x.is_cuda and x.is_contiguous() and x.dtype in (torch.float32, torch.float64)
+    if out is None:
+        out = torch.empty(1, dtype=torch.float64, device=x.device)
+    with torch.cuda.device(x.device):
+        st = torch.cuda.current_stream(x.device)
+        rc = lib().sup_tv2d_value_static(_ptr(x), F32 if x.dtype == torch.float32 else F64, int(shape[0]), int(shape[1]), _ptr(out),
+                                         c_void_p(st.cuda_stream))
+    if rc:
+        raise SupError(rc, lib().sup_last_error(None).decode())
+    return float(out.item()) if sync else out
 
 
 def sup_get_derived(H: SupHandle, which: int) -> torch.Tensor:
