@@ -20,6 +20,7 @@ from .binding import (  # noqa: F401
     sup_perturb_dose,
     sup_perturb_adaptive,
     sup_set_dose_mode,
+    sup_set_perturb_mode,
     sup_perturb_mean,
     sup_project_drop,
     sup_project_emr,

@@ -71,6 +71,7 @@ def lib():
         L.sup_perturb_dose.argtypes = [c_void_p, c_void_p, c_int, c_double, c_double, POINTER(c_int64)]
         L.sup_perturb_mean.argtypes = [c_void_p, c_void_p, c_int, c_double, c_double, POINTER(c_int64)]
         L.sup_set_dose_mode.argtypes = [c_void_p, c_int]
+        L.sup_set_perturb_mode.argtypes = [c_void_p, c_int]
         L.sup_tv2d_value_static.argtypes = [c_void_p, c_int, c_int64, c_int64, c_void_p, c_void_p]
         L.sup_perturb_adaptive.argtypes = [c_void_p, c_void_p, c_int, POINTER(c_int64), c_int, POINTER(c_double), c_double]
         L.sup_project_drop.argtypes = [c_void_p, c_void_p, c_double, c_int]
@@ -320,6 +321,11 @@ def sup_perturb_mean(H: SupHandle, x: torch.Tensor, N, beta0, a, ell=0):
     H._check(lib().sup_perturb_mean(H.h, _ptr(x), N, beta0, a, byref(e)))
     H._exit()
     return e.value
+
+
+def sup_set_perturb_mode(H: SupHandle, mode: int):
+    """0: small TV2D images take the cluster kernel (default); 1: always the cooperative grid kernel."""
+    H._check(lib().sup_set_perturb_mode(H.h, int(mode)))
 
 
 def sup_set_dose_mode(H: SupHandle, mode: int):

@@ -16,7 +16,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(ROOT, "include")
 LIB = os.path.join(HERE, "libsup.so")
-SOURCES = ["sup_setup.cu", "sup_spmv.cu", "sup_stream.cu", "sup_perturb.cu", "sup_algos.cu", "sup_gram.cu", "sup_static.cu", "sup_api.cu"]
+SOURCES = ["sup_setup.cu", "sup_spmv.cu", "sup_stream.cu", "sup_perturb.cu", "sup_perturb_small.cu", "sup_algos.cu", "sup_gram.cu", "sup_static.cu", "sup_api.cu"]
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
     "-Xcompiler", "-fPIC", "-I", INCLUDE, "-I", CSRC,

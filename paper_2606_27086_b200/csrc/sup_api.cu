@@ -351,6 +351,16 @@ extern "C" sup_status sup_set_dose_matrix(sup_handle h, const sup_csr* D, void* 
     return SUP_OK;
 }
 
+extern "C" sup_status sup_set_perturb_mode(sup_handle h, int mode) {
+    if (!h) return SUP_ERR_INVALID_ARG;
+    SUP_ENTER(h);
+    if (mode != 0 && mode != 1) return sup_fail(h, SUP_ERR_INVALID_ARG, "sup_set_perturb_mode: mode must be 0 (automatic) or 1 (grid kernel)");
+    SUP_CUDA(h, cudaStreamSynchronize(h->stream));
+    drop_graph(h);
+    h->perturb_mode = mode;
+    return SUP_OK;
+}
+
 extern "C" sup_status sup_set_dose_mode(sup_handle h, int mode) {
     if (!h) return SUP_ERR_INVALID_ARG;
     SUP_ENTER(h);

@@ -182,6 +182,7 @@ struct sup_ctx {
     void* gram = nullptr;           // [n][gram_ld] G = D^T D of the dose matrix (sup_gram.cu), NULL when not applicable
     int64_t gram_ld = 0;
     void* gram_w = nullptr;         // [n] G g of the current reduction step
+    int perturb_mode = 0;           // 0: small TV2D images take the cluster kernel (sup_perturb_small.cu), 1: always the grid kernel
     int dose_mode = 0;              // 0: Gram path when available, 1: matrix passes over D and D^T (sup_set_dose_mode)
     int g_d = 8, g_dt = 32;
     // cached graph of one superiorized sweep
@@ -291,6 +292,8 @@ sup_status sup_launch_perturb(sup_ctx* h, void* x, const PerturbParams& pp);
 void sup_launch_objective(sup_ctx* h, const void* x, int kind, int64_t nz, int64_t ny, int64_t nx, double* out_dev);
 void sup_launch_begin_run(sup_ctx* h, int64_t ell0, int64_t k0, double a, int64_t n_iter = 0, double f_ref = 0.0);
 int sup_perturb_grid(sup_ctx* h, int objective);
+bool sup_perturb_small_eligible(const sup_ctx* h, const PerturbParams& pp);
+sup_status sup_launch_perturb_small(sup_ctx* h, void* x, const PerturbParams& pp);
 
 // ---- DROP / EMR, stopping rule, f_Mean (sup_algos.cu) ---------------------------------------------------------------
 sup_status sup_setup_wz(sup_ctx* h);

@@ -25,44 +25,13 @@
 #include <stdlib.h>
 
 #include "sup_internal.cuh"
+#include "sup_perturb_args.cuh"
 
 #define TILE_H 16
 #define TILE_W 64
 #define BARRIER_SPIN_LIMIT (1u << 24)
 #define SUP_TRIAL_BATCH 8  // candidate steps evaluated per pass after a rejected first candidate (TV objectives)
 
-template <typename T>
-struct PArgs {
-    T* x;
-    T* g;
-    T* x2;  // second iterate / gradient buffers (TV objectives: an accepted step is applied inside the next gradient pass)
-    T* g2;
-    int64_t n, nz, ny, nx;
-    T* xg;      // gather mirror of x kept by the product kernels (NULL: none): written together with the final iterate
-    GMap xmap;
-    int N;
-    double beta0, a;
-    int policy;
-    long long n_restart;
-    int step_rule;  // sup_step_rule
-    double shrink;  // adaptive rule (A-30)
-    DevState* st;
-    double* partials;  // [2][SUP_MAX_PARTIALS]
-    int8_t* decisions;
-    double* decision_f;
-    int64_t cap;
-    // dose
-    int64_t md;
-    const int64_t* d_rowptr;
-    const int32_t* d_col;
-    const T* d_val;
-    const int64_t* dt_rowptr;
-    const int32_t* dt_col;
-    const T* dt_val;
-    T* r;
-    T* q;  // [md]: D g of the current reduction step (dose objective)
-    int g_d, g_dt;
-};
 
 // ---- grid barrier (all CTAs co-resident by cooperative launch) ----------------------------------------------
 // Grid barrier fused with the second stage of a reduction.  On entry v[0..NV) are this THREAD's shares; every CTA sums
@@ -817,44 +786,6 @@ __global__ void k_sum_final(const double* __restrict__ partials, int np, double*
 }
 
 // ---- host side --------------------------------------------------------------------------------------------------
-template <typename T>
-static PArgs<T> make_args(sup_ctx* h, void* x, const PerturbParams& pp) {
-    PArgs<T> A;
-    A.x = static_cast<T*>(x);
-    A.g = static_cast<T*>(h->g);
-    A.x2 = static_cast<T*>(h->x2);
-    A.g2 = static_cast<T*>(h->g2);
-    A.n = h->n;
-    A.nz = pp.nz;
-    A.ny = pp.ny;
-    A.nx = pp.nx;
-    A.xg = pp.write_mirror && sup_stream_forward_uses_xg(h) ? static_cast<T*>(h->xg) : nullptr;
-    A.xmap = h->xmap;
-    A.N = pp.N;
-    A.beta0 = pp.beta0;
-    A.a = pp.a;
-    A.policy = pp.policy;
-    A.step_rule = pp.step_rule;
-    A.shrink = pp.shrink;
-    A.n_restart = pp.n_restart;
-    A.st = h->state;
-    A.partials = h->partials;
-    A.decisions = pp.decisions;
-    A.decision_f = pp.decision_f;
-    A.cap = pp.cap;
-    A.md = h->D.rows;
-    A.d_rowptr = h->D.rowptr;
-    A.d_col = h->D.col;
-    A.d_val = static_cast<const T*>(h->D.val);
-    A.dt_rowptr = h->DT.rowptr;
-    A.dt_col = h->DT.col;
-    A.dt_val = static_cast<const T*>(h->DT.val);
-    A.r = static_cast<T*>(h->r_dose);
-    A.q = static_cast<T*>(h->q_dose);
-    A.g_d = h->g_d;
-    A.g_dt = h->g_dt;
-    return A;
-}
 
 template <typename T>
 static const void* perturb_kernel(int objective) {
@@ -894,6 +825,7 @@ sup_status sup_launch_perturb(sup_ctx* h, void* x, const PerturbParams& pp) {
         if (!(h->D.plan.ok && h->DT.plan.ok)) return sup_fail(h, SUP_ERR_STATE, "the dose perturbation runs on the staged product kernels (sup_set_row_mode)");
         return sup_launch_perturb_dose_staged(h, x, pp);
     }
+    if (sup_perturb_small_eligible(h, pp)) return sup_launch_perturb_small(h, x, pp);  // small images: one cluster (sup_perturb_small.cu)
     const int grid = sup_perturb_grid(h, pp.objective);
     if (grid < 1) return sup_fail(h, SUP_ERR_CUDA, "perturbation kernel cannot be made resident");
     cudaLaunchConfig_t cfg = {};
@@ -907,11 +839,11 @@ sup_status sup_launch_perturb(sup_ctx* h, void* x, const PerturbParams& pp) {
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     if (h->dt == SUP_F32) {
-        PArgs<float> A = make_args<float>(h, x, pp);
+        PArgs<float> A = sup_make_perturb_args<float>(h, x, pp);
         void* args[] = {&A};
         SUP_CUDA(h, cudaLaunchKernelExC(&cfg, perturb_kernel<float>(pp.objective), args));
     } else {
-        PArgs<double> A = make_args<double>(h, x, pp);
+        PArgs<double> A = sup_make_perturb_args<double>(h, x, pp);
         void* args[] = {&A};
         SUP_CUDA(h, cudaLaunchKernelExC(&cfg, perturb_kernel<double>(pp.objective), args));
     }
@@ -926,7 +858,7 @@ static void launch_objective_t(sup_ctx* h, const void* x, int kind, int64_t nz, 
     pp.objective = kind;
     pp.ny = ny;
     pp.nx = nx;
-    PArgs<T> A = make_args<T>(h, const_cast<void*>(x), pp);
+    PArgs<T> A = sup_make_perturb_args<T>(h, const_cast<void*>(x), pp);
     int grid = h->num_sms * 4;
     if (grid > SUP_MAX_PARTIALS) grid = SUP_MAX_PARTIALS;
     const int64_t work = kind == SUP_OBJ_DOSE ? h->D.rows * h->g_d : h->n;

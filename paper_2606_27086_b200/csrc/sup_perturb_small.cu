@@ -1,0 +1,330 @@
+// sup_perturb_small.cu -- the TV2D perturbation phase (Algorithm 1 lines 4-17; Eq. 11 with SUP_RULE_ADAPTIVE) for
+// SMALL images: ONE thread-block cluster instead of a grid with a software barrier.
+//
+// k_perturb_tv (sup_perturb.cu) spreads an image over up to 2 x 148 CTAs and pays a global-memory round trip per pass: the candidate
+// z and its gradient go through L2, and every pass ends in a software grid barrier (~3 us).  For a 64 x 64 or 128 x 128 image
+// (BASELINE.json configs[0] and [1]) that is all latency: 53 us for the 1 + N = 6 passes of config 1, three times its basic sweep.
+// Here the image lives in the shared memory of a cluster of SMALL_C = 8 CTAs (contiguous row blocks), the current iterate x, its
+// gradient g and the candidate z never leave the SMs during the phase, neighbouring rows of another CTA are read through
+// distributed shared memory, the two sums of a pass (f(z) and ||grad f(z)||^2) are exchanged by DSMEM stores, and the only
+// synchronisation is the hardware cluster barrier (two per pass).  Candidates are evaluated one at a time (there is no barrier
+// cost to amortise over a batch), strictly in order: the trial / decision / l sequence is Algorithm 1's, as in k_perturb_tv.
+// A pixel's terms are computed by the same thread with the same code whether or not the gradient is wanted, and the sums are
+// taken in a fixed order, so f(z) is one bit pattern per z (an accept test with z == x sees equality).
+//
+// Eligible: TV2D, ny >= SMALL_C rows, at most SMALL_LOCAL_MAX pixels per CTA (n <= 32 768 for row counts that divide evenly).
+// sup_set_perturb_mode(h, 1) keeps the grid kernel for such images (tests run both).
+#include <cooperative_groups.h>
+
+#include "sup_internal.cuh"
+#include "sup_perturb_args.cuh"
+
+namespace cg = cooperative_groups;
+
+#define SMALL_THR 512
+#define SMALL_C 8
+#define SMALL_PPT 8
+#define SMALL_LOCAL_MAX (SMALL_THR * SMALL_PPT)  // pixels one CTA holds
+
+struct SmallShared {
+    double ws[SMALL_THR / 32][2];  // per-warp partial sums of a reduction
+    double part[2][SMALL_C][2];    // [parity][rank][value]: the CTAs' sums, written by their owners into EVERY CTA's copy
+};
+
+// sums v[0..NV) over the whole cluster; on return every thread holds the totals.  Fixed order: lanes (shuffle tree), warps in index
+// order, CTAs in rank order.  Contains one cluster barrier, after which nobody reads the array the terms were computed from.
+template <int NV>
+__device__ __forceinline__ void small_reduce(cg::cluster_group& cl, SmallShared& sh, unsigned& parity, double* v) {
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int b = 0; b < NV; ++b)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v[b] += __shfl_xor_sync(0xffffffffu, v[b], o);
+    if (lane == 0)
+#pragma unroll
+        for (int b = 0; b < NV; ++b) sh.ws[wid][b] = v[b];
+    __syncthreads();
+    const unsigned nb = cl.num_blocks(), me = cl.block_rank();
+    if (threadIdx.x < NV * nb) {  // thread (b, r): this CTA's sum b into CTA r's copy
+        const int b = threadIdx.x % NV;
+        const unsigned r = threadIdx.x / NV;
+        double t = 0.0;
+#pragma unroll
+        for (int w = 0; w < SMALL_THR / 32; ++w) t += sh.ws[w][b];
+        *cl.map_shared_rank(&sh.part[parity][me][b], r) = t;
+    }
+    cl.sync();
+#pragma unroll
+    for (int b = 0; b < NV; ++b) {
+        double t = 0.0;
+        for (unsigned r = 0; r < nb; ++r) t += sh.part[parity][r][b];
+        v[b] = t;
+    }
+    parity ^= 1u;
+}
+
+// TV terms of the pixels this thread owns (A-8, as tv2d_pass of sup_perturb.cu): share F of f(z); with GRAD the gradient of the owned
+// pixels into gout[] (rounded to T) and the share S of sum g^2.  zl: this CTA's rows [r0, r1) of z; zp / zn: the last row of the
+// CTA before and the first row of the CTA after (distributed shared memory), valid where such a row exists.
+template <typename T, bool GRAD>
+__device__ __forceinline__ void small_terms(const T* zl, const T* zp, const T* zn, int r0, int r1, int ny, int nx, double& F, double& S, T* gout) {
+    F = 0.0;
+    S = 0.0;
+    const int nloc = (r1 - r0) * nx;
+    auto row = [&](int i) -> const T* { return i < r0 ? zp : (i >= r1 ? zn : zl + (i - r0) * nx); };
+#pragma unroll
+    for (int k = 0; k < SMALL_PPT; ++k) {
+        const int q = threadIdx.x + k * SMALL_THR;
+        if (q >= nloc) break;
+        const int il = q / nx, j = q - il * nx, i = r0 + il;
+        const T* ri = zl + il * nx;
+        const double c = double(ri[j]);
+        double gv = 0.0;
+        if (i + 1 < ny && j + 1 < nx) {  // own term (i, j)
+            const double dx = double(row(i + 1)[j]) - c, dy = double(ri[j + 1]) - c;
+            const double d2 = fma(dx, dx, dy * dy);
+            if (d2 > 0.0) {
+                const double rs = rsqrt(d2);
+                gv -= (dx + dy) * rs;
+                F += d2 * rs;
+            }
+        }
+        if (GRAD) {
+            if (i >= 1 && j + 1 < nx) {  // term (i-1, j)
+                const T* rm = row(i - 1);
+                const double bb = double(rm[j]);
+                const double dx = c - bb, dy = double(rm[j + 1]) - bb;
+                const double d2 = fma(dx, dx, dy * dy);
+                if (d2 > 0.0) gv += dx * rsqrt(d2);
+            }
+            if (j >= 1 && i + 1 < ny) {  // term (i, j-1)
+                const double bb = double(ri[j - 1]);
+                const double dx = double(row(i + 1)[j - 1]) - bb, dy = c - bb;
+                const double d2 = fma(dx, dx, dy * dy);
+                if (d2 > 0.0) gv += dy * rsqrt(d2);
+            }
+            const T gs = T(gv);
+            gout[k] = gs;
+            S += double(gs) * double(gs);
+        }
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(SMALL_THR, 1) k_perturb_tv2d_small(PArgs<T> A, int rows_max) {
+    cg::cluster_group cl = cg::this_cluster();
+    DevState* st = A.st;
+    if (*(volatile int*)&st->stop) return;  // every CTA sees the same flag (set by an earlier kernel of the run)
+    extern __shared__ __align__(16) unsigned char small_raw[];
+    __shared__ SmallShared sh;
+    const int ny = int(A.ny), nx = int(A.nx);
+    const unsigned me = cl.block_rank(), nb = cl.num_blocks();
+    const int r0 = int(int64_t(me) * ny / nb), r1 = int(int64_t(me + 1) * ny / nb);  // >= 1 row each (ny >= nb)
+    const int nloc = (r1 - r0) * nx;
+    const int cap = rows_max * nx;
+    T* sX = reinterpret_cast<T*>(small_raw);
+    T* sG = sX + cap;
+    T* sZ = sG + cap;
+    // the neighbours' rows this CTA's terms touch: last row of the CTA before, first row of the CTA after
+    const int rows_prev = me > 0 ? int(int64_t(me) * ny / nb) - int(int64_t(me - 1) * ny / nb) : 0;
+    auto prev_last = [&](T* arr) -> const T* { return me > 0 ? cl.map_shared_rank(arr, me - 1) + (rows_prev - 1) * nx : arr; };
+    auto next_first = [&](T* arr) -> const T* { return me + 1 < nb ? cl.map_shared_rank(arr, me + 1) : arr; };
+
+    // run state: read before the first cluster barrier, written by CTA 0 at the very end
+    long long ell = *(volatile long long*)&st->ell;
+    double apow = *(volatile double*)&st->apow;
+    const long long k = *(volatile long long*)&st->k;
+    long long ndec = *(volatile long long*)&st->n_dec;
+    const double f_ref = *(volatile double*)&st->f_ref;
+    long long trials = 0;
+    if (A.n_restart > 0 && k > 0 && k % A.n_restart == 0) {  // restarted perturbations (A-24)
+        ell = k / A.n_restart;
+        apow = 1.0;
+        for (long long q = 0; q < ell; ++q) apow *= A.a;
+    }
+    int warn = 0, fault = 0;
+    unsigned parity = 0;
+    const int64_t g0 = int64_t(r0) * nx;  // first pixel of this CTA in the image
+    for (int q = threadIdx.x; q < nloc; q += SMALL_THR) sX[q] = __ldcg(A.x + g0 + q);
+    cl.sync();
+
+    auto log_trial = [&](double fz, double fxv, bool acc) {
+        if (me == 0 && threadIdx.x == 0) {
+            if (A.decisions && ndec < A.cap) A.decisions[ndec] = acc ? 1 : 0;
+            if (A.decision_f && ndec < A.cap) {
+                A.decision_f[2 * ndec] = fz;
+                A.decision_f[2 * ndec + 1] = fxv;
+            }
+        }
+        ++ndec;
+    };
+    auto step_coef = [&](double s, long long jloc) {  // (beta0 a^exponent) / ||g||, exponent as the running product (A-20)
+        double ap = apow;
+        if (A.policy != SUP_STEP_PER_TRIAL) {
+            ap = 1.0;
+            for (long long q = 0; q < k + jloc; ++q) ap *= A.a;
+        }
+        return s > 0.0 ? (A.beta0 * ap) / s : 0.0;
+    };
+    T g2[SMALL_PPT];
+    bool moved = false;  // x differs from what the caller passed in
+    auto form_z = [&](double c) {  // z = round_T(x - c g) for the owned pixels (c = 0: x itself), then visible to the cluster
+        for (int q = threadIdx.x; q < nloc; q += SMALL_THR) {
+            const double xv = double(sX[q]);
+            sZ[q] = c == 0.0 ? T(xv) : T(fma(-c, double(sG[q]), xv));
+        }
+        cl.sync();
+    };
+    auto adopt = [&](bool with_x) {  // (x, g) <- (z, g2): owned pixels only, by the thread that owns them
+#pragma unroll
+        for (int kk = 0; kk < SMALL_PPT; ++kk) {
+            const int q = threadIdx.x + kk * SMALL_THR;
+            if (q >= nloc) break;
+            if (with_x) sX[q] = sZ[q];
+            sG[q] = g2[kk];
+        }
+        moved = moved || with_x;
+    };
+
+    // pass 0: gradient of x^{k,0} with f and ||g||^2
+    double fx, s;
+    {
+        double v[2];
+        small_terms<T, true>(sX, prev_last(sX), next_first(sX), r0, r1, ny, nx, v[0], v[1], g2);
+        small_reduce<2>(cl, sh, parity, v);
+        adopt(false);
+        fx = v[0];
+        s = sqrt(v[1]);
+        if (!isfinite(fx)) fault |= 2;
+    }
+    const double f_start = fx;
+    const T* zp = prev_last(sZ);
+    const T* zn = next_first(sZ);
+    if (A.step_rule == SUP_RULE_ADAPTIVE) {
+        // Eq. 11 (A-30): x <- x - ((f - f_ref)/||g||^2) g while f > f_ref and g != 0; no trial loop
+        for (int nred = 0; nred < A.N; ++nred) {
+            const bool take = fx > f_ref && s > 0.0;
+            log_trial(f_ref, fx, take);
+            if (!take) continue;
+            ++trials;
+            form_z(((fx - f_ref) / s) / s);
+            if (nred == A.N - 1) {  // f and g of the final point are not needed
+                for (int q = threadIdx.x; q < nloc; q += SMALL_THR) sX[q] = sZ[q];
+                moved = true;
+                break;
+            }
+            double v[2];
+            small_terms<T, true>(sZ, zp, zn, r0, r1, ny, nx, v[0], v[1], g2);
+            small_reduce<2>(cl, sh, parity, v);
+            adopt(true);
+            fx = v[0];
+            s = sqrt(v[1]);
+            if (!isfinite(fx)) fault |= 2;
+        }
+    } else {
+        for (int nred = 0; nred < A.N; ++nred) {
+            const bool last = nred == A.N - 1;
+            bool accepted = false;
+            long long jloc = 0;
+            for (int trial = 0; trial < SUP_J_MAX && !accepted; ++trial) {
+                const double c = step_coef(s, jloc);
+                form_z(c);
+                double v[2];
+                // the first candidate of a step that is not the last comes with its gradient (accepted, the next step starts at once)
+                const bool with_grad = trial == 0 && !last;
+                if (with_grad) {
+                    small_terms<T, true>(sZ, zp, zn, r0, r1, ny, nx, v[0], v[1], g2);
+                    small_reduce<2>(cl, sh, parity, v);
+                } else {
+                    small_terms<T, false>(sZ, zp, zn, r0, r1, ny, nx, v[0], v[1], g2);
+                    small_reduce<1>(cl, sh, parity, v);
+                }
+                const bool acc = v[0] <= fx;  // NaN compares false -> rejected (A-11)
+                ++ell;
+                apow *= A.a;
+                ++jloc;
+                ++trials;
+                log_trial(v[0], fx, acc);
+                if (!acc) continue;
+                accepted = true;
+                if (last) {  // nobody needs the gradient at the final point
+                    if (c != 0.0) {
+                        for (int q = threadIdx.x; q < nloc; q += SMALL_THR) sX[q] = sZ[q];
+                        moved = true;
+                    }
+                    fx = v[0];
+                } else {
+                    if (!with_grad) {  // z is still in place: its gradient now (f(z) again: the same bits)
+                        small_terms<T, true>(sZ, zp, zn, r0, r1, ny, nx, v[0], v[1], g2);
+                        small_reduce<2>(cl, sh, parity, v);
+                    }
+                    fx = v[0];
+                    s = sqrt(v[1]);
+                    adopt(c != 0.0);
+                }
+            }
+            if (!accepted) warn |= 1;  // A-12: step skipped
+        }
+    }
+    // the final iterate back to the caller's x and to the gather mirror of the product kernels
+    if (moved || A.xg) {
+        for (int q = threadIdx.x; q < nloc; q += SMALL_THR) {
+            const T v = sX[q];
+            if (moved) A.x[g0 + q] = v;
+            if (A.xg) A.xg[sup_gmap(A.xmap, int(g0 + q))] = v;
+        }
+    }
+    if (me == 0 && threadIdx.x == 0) {
+        st->ell = ell;
+        st->apow = apow;
+        st->n_dec = ndec;
+        st->n_trials += trials;
+        st->sweep_trials += trials;
+        st->f = fx;
+        if (A.step_rule == SUP_RULE_ADAPTIVE && f_start <= f_ref) st->f_ref = A.shrink * f_start;  // A-30
+        if (warn) atomicOr(&st->warn, warn);
+        if (fault) atomicOr(&st->fault, fault);
+    }
+    cl.sync();  // no CTA leaves while another may still read its shared memory
+}
+
+bool sup_perturb_small_eligible(const sup_ctx* h, const PerturbParams& pp) {
+    if (pp.objective != SUP_OBJ_TV2D || h->perturb_mode != 0) return false;
+    if (pp.ny < SMALL_C || pp.nx < 1 || pp.ny * pp.nx > int64_t(SMALL_C) * SMALL_LOCAL_MAX) return false;
+    const int64_t rows_max = (pp.ny + SMALL_C - 1) / SMALL_C;
+    return rows_max * pp.nx <= SMALL_LOCAL_MAX;
+}
+
+template <typename T>
+static sup_status launch_small_t(sup_ctx* h, const PArgs<T>& A, const PerturbParams& pp) {
+    const int rows_max = int((pp.ny + SMALL_C - 1) / SMALL_C);
+    const size_t smem = size_t(3) * rows_max * pp.nx * sizeof(T);
+    const void* fn = reinterpret_cast<const void*>(&k_perturb_tv2d_small<T>);
+    if (!h->smem_opted_in.count(fn)) {
+        SUP_CUDA(h, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, int(size_t(3) * SMALL_LOCAL_MAX * sizeof(T))));
+        h->smem_opted_in.insert(fn);
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(SMALL_C);
+    cfg.blockDim = dim3(SMALL_THR);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = h->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = SMALL_C;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    PArgs<T> Ac = A;
+    int rm = rows_max;
+    void* args[] = {&Ac, &rm};
+    SUP_CUDA(h, cudaLaunchKernelExC(&cfg, fn, args));
+    h->launches++;
+    return SUP_OK;
+}
+
+sup_status sup_launch_perturb_small(sup_ctx* h, void* x, const PerturbParams& pp) {
+    if (h->dt == SUP_F32) return launch_small_t<float>(h, sup_make_perturb_args<float>(h, x, pp), pp);
+    return launch_small_t<double>(h, sup_make_perturb_args<double>(h, x, pp), pp);
+}

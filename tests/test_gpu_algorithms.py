@@ -529,3 +529,81 @@ def test_gram_matrix_is_dT_d():
         assert xm.data_ptr() % 16 != 0
         sup.sup_perturb_dose(H, xm, 1, 0.01, 0.5, 0)
         assert torch.equal(xm, x)
+
+
+# ---- TV2D perturbation phase: the cluster kernel for small images (sup_perturb_small.cu) and the grid kernel ----------------------------
+@pytest.mark.parametrize("dtype", [0, 1])
+@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("shape", [(8, 8), (9, 37), (64, 64), (13, 1), (8, 512), (100, 300), (128, 256), (130, 256), (7, 40), (1, 64)])
+def test_tv2d_phase_in_both_perturb_modes(shape, mode, dtype):
+    """mode 0 sends images of >= 8 rows and <= 4096 pixels per row block to the cluster kernel ((130, 256), (7, 40) and (1, 64) are not
+    eligible and take the grid kernel in both modes); mode 1 is the grid kernel.  Each against the oracle: trial sequence and l exact,
+    x and f within the phase tolerances; power law (both policies), restarts and the adaptive rule"""
+    sup = _sup()
+    ny, nx = shape
+    n = ny * nx
+    H, oargs = _identity_handle(sup, n, dtype)
+    sup.sup_set_perturb_mode(H, mode)
+    O = Oracle(*oargs, objective="tv2d", shape=shape)
+    rng = np.random.default_rng(ny * 1000 + nx)
+    xs = (0.5 + 0.3 * np.sin(np.arange(n) * 0.37) + 0.05 * rng.normal(size=n)).astype(np.float32)
+    ptol, ftol = (1e-5, 1e-4) if dtype == 0 else (1e-13, 1e-12)  # fp32: x and g are rounded to the storage type at every step (north_star: objective 1e-4)
+    # power law: beta0 large enough that the first trials are rejected
+    x = xdev(xs, dtype)
+    xo, ell = xs.astype(np.float64), 2
+    for phase in range(2):
+        dec = torch.zeros(4096, dtype=torch.int8, device="cuda:0")
+        ell_g = sup.sup_perturb_tv(H, x, shape, 4, 3.0, 0.8, ell)
+        st = sup.sup_get_state(H)
+        R = O.perturb(xo, ell, 4, 3.0, 0.8)
+        xo = R["x"]
+        assert ell_g == R["ell"] and st["n_trials"] == R["trials"], (shape, mode, phase, ell_g, R["ell"], R["margins"].min() if R["margins"].size else None)
+        assert rel_l2(x.cpu().numpy(), xo) <= ptol, (shape, mode, phase)
+        assert abs(st["f"] - R["fx"]) <= ftol * max(1.0, abs(R["fx"]))
+        ell = ell_g
+    # Algorithm 1 with the literal per-sweep policy and with restarts, decisions logged (needs a feasibility operator: identity rows)
+    for kwargs in (dict(policy=sup.PER_SWEEP), dict(n_restart=2)):
+        xg = xdev(xs, dtype)
+        dec = torch.zeros(1 << 14, dtype=torch.int8, device="cuda:0")
+        sup.sup_superiorize(H, xg, 5, 3, 1.5, 0.7, objective="tv2d", shape=shape, lam=1.0, decisions=dec, use_graph=True, **kwargs)
+        st = sup.sup_get_state(H)
+        if "policy" in kwargs:
+            R = O.superiorize(xs.astype(np.float64), 5, 3, 1.5, 0.7, lam=1.0, policy=kwargs["policy"])
+        else:
+            R = O.superiorize(xs.astype(np.float64), 5, 3, 1.5, 0.7, lam=1.0, n_restart=2)
+        gdec = dec[: st["n_decisions"]].cpu().numpy()
+        if np.array_equal(gdec, R["decisions"]):
+            assert st["ell"] == R["ell"]
+            assert rel_l2(xg.cpu().numpy(), R["x"]) <= (1e-4 if dtype == 0 else 1e-10)
+        else:  # a flipped accept test must be a knife edge (A-13)
+            nmin = min(gdec.size, R["decisions"].size)
+            first = int(np.flatnonzero(gdec[:nmin] != R["decisions"][:nmin])[0]) if nmin and (gdec[:nmin] != R["decisions"][:nmin]).any() else nmin
+            assert first < R["margins"].size and R["margins"][first] < (1e-6 if dtype == 0 else 1e-12), (shape, mode, kwargs, first)
+    # Eq. 11
+    f0 = O.objective_value(xs.astype(np.float64))
+    if f0 > 0:
+        x = xdev(xs, dtype)
+        fr = sup.sup_perturb_adaptive(H, x, "tv2d", 3, 0.9 * f0, 0.5, shape=shape)
+        R = O.perturb_adaptive(xs.astype(np.float64), 3, 0.9 * f0, 0.5)
+        assert sup.sup_get_state(H)["n_trials"] == R["steps"] and fr == R["f_ref"]
+        assert rel_l2(x.cpu().numpy(), R["x"]) <= (2e-6 if dtype == 0 else 1e-13)
+        x = xdev(xs, dtype)
+        fr = sup.sup_perturb_adaptive(H, x, "tv2d", 2, 2.0 * f0, 0.25, shape=shape)
+        assert torch.equal(x, xdev(xs, dtype)) and abs(fr - 0.25 * f0) <= ftol * f0
+
+
+def test_cluster_and_grid_perturbation_kernels_take_the_same_decisions():
+    """config 1 (64 x 64) through Algorithm 1 with both kernels: identical decision logs and l, x equal to rounding"""
+    sup = _sup()
+    P = gen.config1_tiny_ct()
+    out = []
+    for mode in (0, 1):
+        H = handle(P, 0)
+        sup.sup_set_perturb_mode(H, mode)
+        x = xdev(P.x0, 0)
+        dec = torch.zeros(1 << 14, dtype=torch.int8, device="cuda:0")
+        sup.sup_superiorize(H, x, 12, P.N, P.beta0, P.a, objective="tv2d", shape=P.shape, lam=P.lam, decisions=dec)
+        st = sup.sup_get_state(H)
+        out.append((st["ell"], dec[: st["n_decisions"]].cpu().numpy().copy(), x.cpu().numpy().copy()))
+    assert out[0][0] == out[1][0] and np.array_equal(out[0][1], out[1][1])
+    assert rel_l2(out[0][2], out[1][2]) <= 1e-5
