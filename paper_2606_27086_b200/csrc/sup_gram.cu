@@ -95,7 +95,9 @@ __global__ void __launch_bounds__(GRAM_BUILD_THREADS)
 // is 32 KB: one 16-byte load per thread and trip), four rows in flight per thread.  Products and the per-thread partial sums in the
 // handle's type (chains of ld / (16/sizeof(T) * threads) terms), everything after that in fp64, in a fixed order.
 #define GRAM_MV_WARPS 32
+#ifndef GRAM_MV_ROWS
 #define GRAM_MV_ROWS 4
+#endif
 template <typename T>
 struct GramVec;
 template <>
