@@ -182,6 +182,12 @@ struct sup_ctx {
     void* gram = nullptr;           // [n][gram_ld] G = D^T D of the dose matrix (sup_gram.cu), NULL when not applicable
     int64_t gram_ld = 0;
     void* gram_w = nullptr;         // [n] G g of the current reduction step
+#ifdef SUP_NO_PDL
+    bool pdl = false;
+#else
+    bool pdl = true;                // programmatic dependent launch between consecutive k_staged launches (sup_stream.cu)
+#endif
+    int64_t staged_seq = -1;        // value of `launches` right after the last k_staged launch
     int perturb_mode = 0;           // 0: small TV2D images take the cluster kernel (sup_perturb_small.cu), 1: always the grid kernel
     int dose_mode = 0;              // 0: Gram path when available, 1: matrix passes over D and D^T (sup_set_dose_mode)
     int g_d = 8, g_dt = 32;

@@ -330,6 +330,15 @@ __device__ __forceinline__ void row_operands(int64_t r, const T* p1, const T* p2
 
 // MODE 0: forward (vec = xg, columns swizzled (pk / colg), p1 = lb, p2 = ub, p3 = d, out = y);
 // MODE 1: backward (vec = y, p1 = lo, p2 = hi, out = x in place, out2 = xg mirror or NULL)
+// Programmatic dependent launch (sm_90+): a k_staged launch that directly follows another one on the handle's stream is given the
+// programmatic-serialization attribute.  Every CTA allows its dependents to launch as soon as it has started; a dependent CTA becomes
+// resident on an SM the moment the earlier kernel's CTA there exits (one CTA per SM: the ring owns the shared memory), its PRODUCERS
+// start streaming the matrix (static data) into the ring at once, its CONSUMERS first wait for the earlier grid to complete and flush
+// (they read x / y, which it writes).  The launch latency, the ring fill and the earlier kernel's tail (CTAs finish unevenly)
+// overlap; block-iterative sweeps have 32 such boundaries per sweep.  Without the attribute both instructions are no-ops.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 template <typename T, int MODE, int G, int NCW, int STG>
 __global__ void __launch_bounds__(32 * (NCW + RG_NPROD), 1)
     k_staged(const int64_t* __restrict__ part, const int64_t* __restrict__ rowptr, const int32_t* __restrict__ col,
@@ -339,9 +348,11 @@ __global__ void __launch_bounds__(32 * (NCW + RG_NPROD), 1)
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int RG_ELEMS = STG * RG_TILE;
     RgSmem<T, STG>& S = *reinterpret_cast<RgSmem<T, STG>*>(smem_raw);
-    if (stop && *stop) return;  // the stopping rule fired earlier in this run (A-25): the sweep is skipped
+    if (stop && *stop) return;  // the stopping rule fired earlier in this run (A-25): the sweep is skipped (no PDL with a stop flag)
+    pdl_launch_dependents();
     const int64_t rs = part[blockIdx.x], re = part[blockIdx.x + 1];
     if (rs >= re) {
+        pdl_wait();
         if (red_out && threadIdx.x == 0) red_out[blockIdx.x] = 0.0;
         return;
     }
@@ -435,6 +446,7 @@ __global__ void __launch_bounds__(32 * (NCW + RG_NPROD), 1)
         return;
     }
     double racc = 0.0;  // this lane's share of the kernel's reduction (row_epilogue)
+    pdl_wait();         // the vectors this kernel gathers and updates are complete and visible from here on
     // ---- consumers, G == 0: LONG rows -- the whole CTA works on one row at a time ----------------------------------------
     // (rows of thousands of nonzeros, e.g. config 4's A^T: one row per warp would put NCW x row bytes in flight, far more
     // than the ring holds).  The row is cut into pieces of 32 NCW x RG_UNROLL elements; every lane takes RG_UNROLL elements
@@ -1135,11 +1147,24 @@ static void launch_staged_g(sup_ctx* h, const StreamPlan& sp, const CsrD& M, con
         cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         h->smem_opted_in.insert(fn);
     }
-    k_staged<T, MODE, G, Sh::NCW, Sh::STG><<<sp.nb, 32 * (Sh::NCW + RG_NPROD), smem, h->stream>>>(
-        sp.part, M.rowptr, M.col, static_cast<const T*>(M.val), static_cast<const uint2*>(M.pk), static_cast<const T*>(vec),
-        static_cast<const T*>(p1), static_cast<const T*>(p2), static_cast<const T*>(p3), static_cast<T*>(out),
-        static_cast<T*>(out2), T(lambda), M.alloc_nnz, omap, red_out, h->stop_ptr);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(unsigned(sp.nb));
+    cfg.blockDim = dim3(32 * (Sh::NCW + RG_NPROD));
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = h->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    // only directly behind another k_staged launch of this handle (nothing else of the library was enqueued in between), and never
+    // with a stop flag (it is read before any wait)
+    cfg.numAttrs = (h->pdl && !h->stop_ptr && h->launches == h->staged_seq) ? 1 : 0;
+    cudaLaunchKernelEx(&cfg, k_staged<T, MODE, G, Sh::NCW, Sh::STG>, sp.part, M.rowptr, M.col, static_cast<const T*>(M.val),
+                       static_cast<const uint2*>(M.pk), static_cast<const T*>(vec), static_cast<const T*>(p1), static_cast<const T*>(p2),
+                       static_cast<const T*>(p3), static_cast<T*>(out), static_cast<T*>(out2), T(lambda), M.alloc_nnz, omap, red_out,
+                       static_cast<const int*>(h->stop_ptr));
     h->launches++;
+    h->staged_seq = h->launches;
 }
 
 // deep: the gathered vector (x for MODE 0, y for MODE 1) is kept in a tiled layout
