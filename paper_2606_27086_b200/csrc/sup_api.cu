@@ -852,7 +852,6 @@ static sup_status run_superiorize(sup_ctx* h, void* x, int n_iter, int N, double
                 }
             }
             h->launches = launches_before;
-            h->staged_seq = -1;  // (the counter was rewound: no stale match with a later launch)
             if (e != cudaSuccess || rc != SUP_OK || !h->gexec) {
                 cudaGetLastError();
                 drop_graph(h);

@@ -220,6 +220,7 @@ __global__ void k_gram_trial(DevState* st, const double* __restrict__ red_xu, co
                              double beta0, double a, int policy, long long n_restart, int8_t* decisions, double* decision_f, long long cap,
                              int step_rule, double shrink) {
     if (st->stop) return;
+    sup_pdl_trigger();
     const long long k = st->k;
     if (final_only) {
         if (threadIdx.x != 0) return;

@@ -69,6 +69,9 @@ struct DevState {
     alignas(128) double red[2][8];  // totals published by the last CTA to arrive (by generation parity)
 };
 
+// kernels that precede a product kernel in a sweep let it start early (sup_stream.cu: programmatic dependent launch)
+__device__ __forceinline__ void sup_pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 struct Bump {  // bump allocator over caller-provided workspace
     char* base = nullptr;
     size_t cap = 0, off = 0;
@@ -187,7 +190,6 @@ struct sup_ctx {
 #else
     bool pdl = true;                // programmatic dependent launch between consecutive k_staged launches (sup_stream.cu)
 #endif
-    int64_t staged_seq = -1;        // value of `launches` right after the last k_staged launch
     int perturb_mode = 0;           // 0: small TV2D images take the cluster kernel (sup_perturb_small.cu), 1: always the grid kernel
     int dose_mode = 0;              // 0: Gram path when available, 1: matrix passes over D and D^T (sup_set_dose_mode)
     int g_d = 8, g_dt = 32;

@@ -115,6 +115,7 @@ __global__ void __launch_bounds__(SMALL_THR, 1) k_perturb_tv2d_small(PArgs<T> A,
     cg::cluster_group cl = cg::this_cluster();
     DevState* st = A.st;
     if (*(volatile int*)&st->stop) return;  // every CTA sees the same flag (set by an earlier kernel of the run)
+    sup_pdl_trigger();  // the forward product that follows may become resident on the idle SMs and fill its ring meanwhile
     extern __shared__ __align__(16) unsigned char small_raw[];
     __shared__ SmallShared sh;
     const int ny = int(A.ny), nx = int(A.nx);

@@ -330,8 +330,7 @@ __device__ __forceinline__ void row_operands(int64_t r, const T* p1, const T* p2
 
 // MODE 0: forward (vec = xg, columns swizzled (pk / colg), p1 = lb, p2 = ub, p3 = d, out = y);
 // MODE 1: backward (vec = y, p1 = lo, p2 = hi, out = x in place, out2 = xg mirror or NULL)
-// Programmatic dependent launch (sm_90+): a k_staged launch that directly follows another one on the handle's stream is given the
-// programmatic-serialization attribute.  Every CTA allows its dependents to launch as soon as it has started; a dependent CTA becomes
+// Programmatic dependent launch (sm_90+): k_staged launches are given the programmatic-serialization attribute.  Every CTA allows its dependents to launch as soon as it has started; a dependent CTA becomes
 // resident on an SM the moment the earlier kernel's CTA there exits (one CTA per SM: the ring owns the shared memory), its PRODUCERS
 // start streaming the matrix (static data) into the ring at once, its CONSUMERS first wait for the earlier grid to complete and flush
 // (they read x / y, which it writes).  The launch latency, the ring fill and the earlier kernel's tail (CTAs finish unevenly)
@@ -1156,15 +1155,15 @@ static void launch_staged_g(sup_ctx* h, const StreamPlan& sp, const CsrD& M, con
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    // only directly behind another k_staged launch of this handle (nothing else of the library was enqueued in between), and never
-    // with a stop flag (it is read before any wait)
-    cfg.numAttrs = (h->pdl && !h->stop_ptr && h->launches == h->staged_seq) ? 1 : 0;
+    // Every launch carries it (the matrix, the partition table and the row pointers its producers read are written by set-up calls
+    // that end in a stream synchronisation; everything a sweep's kernels write is read behind griddepcontrol.wait), except with a
+    // stop flag, which is read before any wait.  Behind a kernel that never triggers, the attribute changes nothing.
+    cfg.numAttrs = (h->pdl && !h->stop_ptr) ? 1 : 0;
     cudaLaunchKernelEx(&cfg, k_staged<T, MODE, G, Sh::NCW, Sh::STG>, sp.part, M.rowptr, M.col, static_cast<const T*>(M.val),
                        static_cast<const uint2*>(M.pk), static_cast<const T*>(vec), static_cast<const T*>(p1), static_cast<const T*>(p2),
                        static_cast<const T*>(p3), static_cast<T*>(out), static_cast<T*>(out2), T(lambda), M.alloc_nnz, omap, red_out,
                        static_cast<const int*>(h->stop_ptr));
     h->launches++;
-    h->staged_seq = h->launches;
 }
 
 // deep: the gathered vector (x for MODE 0, y for MODE 1) is kept in a tiled layout
