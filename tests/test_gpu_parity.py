@@ -700,6 +700,12 @@ DEGENERATE = {
     "one_by_one": _mini([0, 1], [0], [2.0], [1.0], [1.5], [-5.0], [5.0], 1),
     "one_long_row": _mini([0, 5000], np.arange(5000), np.linspace(0.1, 1.0, 5000), [3.0], [4.0], np.full(5000, -1.0), np.full(5000, 1.0), 5000),
     "one_long_column": _mini(np.arange(4001), np.zeros(4000, np.int32), np.linspace(0.5, 1.5, 4000), np.full(4000, 0.2), np.full(4000, 0.3), [-9.0], [9.0], 1),
+    # 70 000 entries in one row / one column: more chunks than the chunk mode's pool allows (65 536 entries), so the planner must fall back to
+    # the whole-CTA-per-row mode; beside them rows of ~3 000 entries keep the mean above the chunk mode's threshold
+    "rows_beyond_the_chunk_pool": _mini(np.concatenate([[0], np.cumsum([70000, 3000, 2500, 3100])]),
+                                        np.concatenate([np.arange(70000), np.arange(3000), np.arange(100, 2600), np.arange(50, 3150)]),
+                                        np.concatenate([np.linspace(0.1, 1.0, 70000), np.linspace(1.0, 0.2, 3000), np.full(2500, 0.5), np.linspace(0.3, 0.4, 3100)]),
+                                        [30.0, 2.0, 1.0, 0.5], [31.0, 3.0, 1.5, 0.8], np.full(70000, -1.0), np.full(70000, 1.0), 70000),
     "all_rows_empty_but_one": _mini([0, 0, 0, 2, 2], [1, 3], [1.0, -1.0], [-INF, 5.0, 0.5, -INF], [INF, 6.0, INF, 1.0], np.zeros(4), np.ones(4), 4),
     "image_one_pixel_wide": _mini([0, 2, 3], [0, 5, 2], [1.0, 1.0, 2.0], [0.5, 0.1], [0.6, 0.2], np.zeros(6), np.ones(6), 6),
 }
