@@ -62,11 +62,9 @@ struct DevState {
     int stop_reason;
     double f_ref;         // Eq. 11's reference value (adaptive step rule, A-30)
     double f_start;       // dose objective, adaptive rule: f at the start of the phase (decides the update of f_ref)
-    // grid barrier of the perturbation kernel: the arrival counter, the generation flag every waiting CTA polls and the
-    // published totals each sit in a 128-byte line of their own, so the pollers do not slow the arrivals down
-    alignas(128) unsigned bar_count;
-    alignas(128) unsigned bar_gen;
-    alignas(128) double red[2][8];  // totals published by the last CTA to arrive (by generation parity)
+    // grid barrier of the perturbation kernel (grid_reduce, sup_perturb.cu), each field in a 128-byte line of its own
+    alignas(128) unsigned long long bar_count;  // arrivals, monotone within a run
+    alignas(128) unsigned long long bar_base;   // value of bar_count when the last launch's barriers were complete
 };
 
 // kernels that precede a product kernel in a sweep let it start early (sup_stream.cu: programmatic dependent launch)

@@ -34,76 +34,68 @@
 
 
 // ---- grid barrier (all CTAs co-resident by cooperative launch) ----------------------------------------------
-// Grid barrier fused with the second stage of a reduction.  On entry v[0..NV) are this THREAD's shares; every CTA sums
-// its threads' shares, stores the NV sums to partials[b * stride + blockIdx.x] and arrives.  The last CTA to arrive adds
-// the partials of all CTAs in index order (which CTA does it changes nothing: same numbers, same order), publishes the
-// totals in st->red[gen & 1] and flips the generation; the others spin on the generation and read the totals.  On
-// return v[] holds the totals in every thread.  Returns false after a time-out (fault bit 0 is set): the caller leaves
-// the kernel instead of computing on inconsistent partials.
+// Grid barrier fused with the second stage of a reduction.  On entry v[0..NV) are this THREAD's shares; every CTA sums its threads'
+// shares, stores the NV sums to its slots of the partials buffer and adds 1 to a MONOTONE arrival counter (a release: the partials
+// are visible before the count).  Then EVERY CTA waits until the counter has reached this barrier's target (an acquire) and adds the
+// partials of all CTAs itself, in the same fixed order -- the same numbers in the same order give the same bits in every CTA, which
+// is what keeps the kernel's control flow uniform.  Three L2 round trips per barrier (arrive, see the target, read the partials)
+// against four when the last CTA to arrive added the partials and published totals (arrive with the old value returned, read
+// partials, release a flag, read totals): 4.4 -> ~3.3 us at 256 CTAs (profiles/r02c).  The counter is never reset inside a launch;
+// a launch starts from st->bar_base, which CTA 0 of the launch before left there (a CTA reads it before its first arrival, and CTA 0
+// can only reach the end of a kernel after every CTA has arrived at its barriers).  The partials are double-buffered by barrier
+// parity: a CTA writes the buffer of barrier i + 2 only after barrier i + 1, which every CTA reaches after reading barrier i's.
+// On return v[] holds the totals in every thread.  Returns false after a time-out (fault bit 0 is set): the caller leaves the
+// kernel instead of computing on inconsistent partials.
 template <int NV>
 __device__ __forceinline__ void cta_sum_batch(double* v);
-__device__ __forceinline__ unsigned atom_add_acq_rel(unsigned* p, unsigned v) {
-    unsigned old;
-    asm volatile("atom.add.acq_rel.gpu.u32 %0, [%1], %2;" : "=r"(old) : "l"(p), "r"(v) : "memory");
-    return old;
+__device__ __forceinline__ void red_release_add(unsigned long long* p, unsigned long long v) {
+    asm volatile("red.release.gpu.global.add.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
-__device__ __forceinline__ unsigned ld_acquire(const unsigned* p) {
-    unsigned v;
-    asm volatile("ld.acquire.gpu.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+__device__ __forceinline__ unsigned long long ld_acquire(const unsigned long long* p) {
+    unsigned long long v;
+    asm volatile("ld.acquire.gpu.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
     return v;
 }
-__device__ __forceinline__ void st_release(unsigned* p, unsigned v) {
-    asm volatile("st.release.gpu.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
-}
+
+struct GridBar {
+    unsigned long long target;  // value of the arrival counter when the barrier last passed is complete
+    unsigned n;                 // barriers passed in this launch (parity selects the partials buffer)
+};
 
 template <int NV>
-__device__ __forceinline__ bool grid_reduce(DevState* st, double* partials, int stride, double* v, unsigned& gen) {
-    __shared__ int s_role;  // 1: this CTA arrived last, 0: it waited, -1: time-out
+__device__ __forceinline__ bool grid_reduce(DevState* st, double* partials, int stride, double* v, GridBar& gb) {
+    __shared__ int s_ok;
     cta_sum_batch<NV>(v);
+    gb.target += gridDim.x;
+    double* buf = partials + (gb.n & 1u) * SUP_MAX_PARTIALS;
+    gb.n += 1u;
     if (threadIdx.x == 0) {
 #pragma unroll
-        for (int b = 0; b < NV; ++b) partials[b * stride + blockIdx.x] = v[b];
-        // release: the partials are visible before the count; acquire: the last to arrive sees everybody's partials
-        const unsigned arrived = atom_add_acq_rel(&st->bar_count, 1u);
-        int role = arrived == gridDim.x - 1 ? 1 : 0;
-        if (!role) {
-            unsigned spins = 0;
-            while (ld_acquire(&st->bar_gen) == gen) {
-                __nanosleep(20);
-                if (++spins > BARRIER_SPIN_LIMIT) {
-                    atomicOr(&st->fault, 1);
-                    role = -1;
-                    break;
-                }
+        for (int b = 0; b < NV; ++b) buf[b * stride + blockIdx.x] = v[b];
+        red_release_add(&st->bar_count, 1ull);
+        int ok = 1;
+        unsigned spins = 0;
+        while (ld_acquire(&st->bar_count) < gb.target) {
+            __nanosleep(20);
+            if (++spins > BARRIER_SPIN_LIMIT) {
+                atomicOr(&st->fault, 1);
+                ok = 0;
+                break;
             }
         }
-        s_role = role;
+        s_ok = ok;
     }
     __syncthreads();
-    const int role = s_role;
-    if (role < 0) return false;
-    double* red = st->red[gen & 1u];
-    if (role == 1) {
-        double w[NV];
+    if (!s_ok) return false;
+    double w[NV];
 #pragma unroll
-        for (int b = 0; b < NV; ++b) {
-            w[b] = 0.0;
-            for (int q = threadIdx.x; q < int(gridDim.x); q += SUP_THREADS) w[b] += __ldcg(partials + b * stride + q);
-        }
-        cta_sum_batch<NV>(w);
-        if (threadIdx.x == 0) {
-#pragma unroll
-            for (int b = 0; b < NV; ++b) red[b] = w[b];
-            st->bar_count = 0;
-            st_release(&st->bar_gen, gen + 1u);  // totals and the reset counter are visible before the flip
-        }
-#pragma unroll
-        for (int b = 0; b < NV; ++b) v[b] = w[b];
-    } else {
-#pragma unroll
-        for (int b = 0; b < NV; ++b) v[b] = __ldcg(red + b);
+    for (int b = 0; b < NV; ++b) {
+        w[b] = 0.0;
+        for (int q = threadIdx.x; q < int(gridDim.x); q += SUP_THREADS) w[b] += __ldcg(buf + b * stride + q);
     }
-    gen += 1u;
+    cta_sum_batch<NV>(w);
+#pragma unroll
+    for (int b = 0; b < NV; ++b) v[b] = w[b];
     return true;
 }
 
@@ -581,7 +573,7 @@ __global__ void __launch_bounds__(SUP_THREADS) k_perturb_tv(PArgs<T> Ain) {
     double apow = *(volatile double*)&st->apow;  // a^ell, running product (A-20)
     const long long k = *(volatile long long*)&st->k;
     long long ndec = *(volatile long long*)&st->n_dec;
-    unsigned gen = *(volatile unsigned*)&st->bar_gen;  // read before this CTA's first arrival, so before any flip of this launch
+    GridBar gen = {*(volatile unsigned long long*)&st->bar_base, 0u};  // read before this CTA's first arrival (CTA 0 rewrites it at the end)
     // Eq. 11's reference: like every other field of the state it is read HERE, before this CTA's first arrival at a grid barrier --
     // CTA 0 rewrites it at the end of the kernel, which it can only reach after every CTA has arrived at the first barrier
     const double f_ref = *(volatile double*)&st->f_ref;
@@ -596,7 +588,7 @@ __global__ void __launch_bounds__(SUP_THREADS) k_perturb_tv(PArgs<T> Ain) {
     double pend = 0.0;  // step accepted in the last reduction step and not yet written anywhere: x^{k,N} = xc - pend gc
     double* P = A.partials;
     constexpr int B = SUP_TRIAL_BATCH;
-    constexpr int PSTRIDE = 2 * SUP_MAX_PARTIALS / B;  // partial slots per reduced value
+    constexpr int PSTRIDE = SUP_MAX_PARTIALS / B;  // partial slots per reduced value (two buffers of SUP_MAX_PARTIALS: barrier parity)
     bool ok = true;
 
     auto log_trial = [&](double fz, double fxv, bool acc) {
@@ -768,6 +760,7 @@ __global__ void __launch_bounds__(SUP_THREADS) k_perturb_tv(PArgs<T> Ain) {
         st->n_trials += trials;
         st->sweep_trials += trials;
         st->f = fx;
+        if (ok) st->bar_base = gen.target;  // where the next launch's barriers start
         if (adaptive && f_start <= f_ref) st->f_ref = A.shrink * f_start;  // the reference was reached: move it below (A-30)
         if (warn) atomicOr(&st->warn, warn);
         if (fault) atomicOr(&st->fault, fault);
@@ -912,6 +905,7 @@ __global__ void k_begin_run(DevState* st, long long ell0, long long k0, double a
     st->warn = 0;
     st->fault = 0;
     st->bar_count = 0;
+    st->bar_base = 0;
 }
 void sup_launch_begin_run(sup_ctx* h, int64_t ell0, int64_t k0, double a, int64_t n_iter, double f_ref) {
     // a^l0: exactly 1 for a fresh run, so the running product below reproduces the oracle's step sizes bit for bit (A-20)
