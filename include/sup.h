@@ -182,7 +182,7 @@ sup_status sup_set_dose_matrix(sup_handle h, const sup_csr* D_body, void* worksp
 sup_status sup_set_dose_mode(sup_handle h, int mode);
 
 /* Which kernel runs the TV2D perturbation phase.  mode 0 (default): images of at least 8 rows and at most 4096 pixels per row block
- * of ny/8 rows (n <= 32768) take the CLUSTER kernel -- the image stays in the shared memory of 8 CTAs for the whole phase, hardware
+ * of ny/8 rows (n <= 32768) take the CLUSTER kernel -- the image stays in the shared memory of 8 (or 16) CTAs for the whole phase, hardware
  * cluster barriers instead of a software grid barrier (K4s); larger images the cooperative grid kernel.
  * mode 1: always the grid kernel.  Same algorithm, same trial / decision / l sequence; sums in a different (fixed) order. */
 sup_status sup_set_perturb_mode(sup_handle h, int mode);

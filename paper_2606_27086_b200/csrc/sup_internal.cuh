@@ -188,6 +188,7 @@ struct sup_ctx {
 #else
     bool pdl = true;                // programmatic dependent launch between consecutive k_staged launches (sup_stream.cu)
 #endif
+    int cluster16 = 0;              // thread-block clusters of 16 for the small-image perturbation kernel: 0 not asked yet, 1 yes, -1 no
     int perturb_mode = 0;           // 0: small TV2D images take the cluster kernel (sup_perturb_small.cu), 1: always the grid kernel
     int dose_mode = 0;              // 0: Gram path when available, 1: matrix passes over D and D^T (sup_set_dose_mode)
     int g_d = 8, g_dt = 32;

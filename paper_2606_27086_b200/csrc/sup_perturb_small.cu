@@ -4,7 +4,7 @@
 // k_perturb_tv (sup_perturb.cu) spreads an image over up to 2 x 148 CTAs and pays a global-memory round trip per pass: the candidate
 // z and its gradient go through L2, and every pass ends in a software grid barrier (~3 us).  For a 64 x 64 or 128 x 128 image
 // (BASELINE.json configs[0] and [1]) that is all latency: 53 us for the 1 + N = 6 passes of config 1, three times its basic sweep.
-// Here the image lives in the shared memory of a cluster of SMALL_C = 8 CTAs (contiguous row blocks), the current iterate x, its
+// Here the image lives in the shared memory of a cluster of 8 CTAs (16 above 8 192 pixels: config 2's phase 69 -> 51 us) in contiguous row blocks, the current iterate x, its
 // gradient g and the candidate z never leave the SMs during the phase, neighbouring rows of another CTA are read through
 // distributed shared memory, the two sums of a pass (f(z) and ||grad f(z)||^2) are exchanged by DSMEM stores, and the only
 // synchronisation is the hardware cluster barrier (two per pass).  Candidates are evaluated one at a time (there is no barrier
@@ -22,13 +22,14 @@
 namespace cg = cooperative_groups;
 
 #define SMALL_THR 512
-#define SMALL_C 8
+#define SMALL_C 8       // portable cluster size: images of up to 8 192 pixels
+#define SMALL_CMAX 16   // non-portable size (opt-in, B200 has it): larger images, where a pass is bound by the fp64 work per CTA
 #define SMALL_PPT 8
 #define SMALL_LOCAL_MAX (SMALL_THR * SMALL_PPT)  // pixels one CTA holds
 
 struct SmallShared {
     double ws[SMALL_THR / 32][2];  // per-warp partial sums of a reduction
-    double part[2][SMALL_C][2];    // [parity][rank][value]: the CTAs' sums, written by their owners into EVERY CTA's copy
+    double part[2][SMALL_CMAX][2];    // [parity][rank][value]: the CTAs' sums, written by their owners into EVERY CTA's copy
 };
 
 // sums v[0..NV) over the whole cluster; on return every thread holds the totals.  Fixed order: lanes (shuffle tree), warps in index
@@ -289,30 +290,57 @@ __global__ void __launch_bounds__(SMALL_THR, 1) k_perturb_tv2d_small(PArgs<T> A,
     cl.sync();  // no CTA leaves while another may still read its shared memory
 }
 
+// cluster size for an ny x nx image: 8, or 16 for more than 8 192 pixels when the device takes the non-portable size; 0: not eligible
+static int small_cluster_size(const sup_ctx* h, int64_t ny, int64_t nx) {
+    if (ny < SMALL_C || nx < 1 || ny * nx > int64_t(SMALL_C) * SMALL_LOCAL_MAX) return 0;
+    int c = SMALL_C;
+    if (ny * nx > 8192 && ny >= SMALL_CMAX && h->cluster16 > 0) c = SMALL_CMAX;
+    const int64_t rows_max = (ny + c - 1) / c;
+    return rows_max * nx <= SMALL_LOCAL_MAX ? c : 0;
+}
+
 bool sup_perturb_small_eligible(const sup_ctx* h, const PerturbParams& pp) {
     if (pp.objective != SUP_OBJ_TV2D || h->perturb_mode != 0) return false;
-    if (pp.ny < SMALL_C || pp.nx < 1 || pp.ny * pp.nx > int64_t(SMALL_C) * SMALL_LOCAL_MAX) return false;
-    const int64_t rows_max = (pp.ny + SMALL_C - 1) / SMALL_C;
-    return rows_max * pp.nx <= SMALL_LOCAL_MAX;
+    return small_cluster_size(h, pp.ny, pp.nx) > 0;
 }
 
 template <typename T>
 static sup_status launch_small_t(sup_ctx* h, const PArgs<T>& A, const PerturbParams& pp) {
-    const int rows_max = int((pp.ny + SMALL_C - 1) / SMALL_C);
-    const size_t smem = size_t(3) * rows_max * pp.nx * sizeof(T);
     const void* fn = reinterpret_cast<const void*>(&k_perturb_tv2d_small<T>);
     if (!h->smem_opted_in.count(fn)) {
         SUP_CUDA(h, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, int(size_t(3) * SMALL_LOCAL_MAX * sizeof(T))));
+        // does this device take clusters of 16 for this kernel?  (asked once per handle; -1 = no)
+        h->cluster16 = -1;
+        if (cudaFuncSetAttribute(fn, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess) {
+            cudaLaunchConfig_t q = {};
+            q.gridDim = dim3(SMALL_CMAX);
+            q.blockDim = dim3(SMALL_THR);
+            q.dynamicSmemBytes = size_t(3) * SMALL_LOCAL_MAX * sizeof(T);
+            cudaLaunchAttribute qa[1];
+            qa[0].id = cudaLaunchAttributeClusterDimension;
+            qa[0].val.clusterDim.x = SMALL_CMAX;
+            qa[0].val.clusterDim.y = 1;
+            qa[0].val.clusterDim.z = 1;
+            q.attrs = qa;
+            q.numAttrs = 1;
+            int nclusters = 0;
+            if (cudaOccupancyMaxActiveClusters(&nclusters, fn, &q) == cudaSuccess && nclusters >= 1) h->cluster16 = 1;
+        }
+        cudaGetLastError();
         h->smem_opted_in.insert(fn);
     }
+    const int C = small_cluster_size(h, pp.ny, pp.nx);
+    if (C < 1) return sup_fail(h, SUP_ERR_STATE, "sup_launch_perturb_small: image not eligible");
+    const int rows_max = int((pp.ny + C - 1) / C);
+    const size_t smem = size_t(3) * rows_max * pp.nx * sizeof(T);
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(SMALL_C);
+    cfg.gridDim = dim3(C);
     cfg.blockDim = dim3(SMALL_THR);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = h->stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = SMALL_C;
+    attr[0].val.clusterDim.x = C;
     attr[0].val.clusterDim.y = 1;
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
