@@ -89,6 +89,9 @@ void sup_launch_emr_update(sup_ctx* h, const double* red_pp, int np_pp, const do
 __global__ void k_close_sweep(DevState* st, double* trace, const double* __restrict__ red_prox, int np, int mode, int use_f,
                               int want_trace, int want_stop, int perturbed, double prox_tol, double dprox_tol, int n_consec,
                               double dobj_tol) {
+    // launched with the programmatic-serialization attribute behind a product kernel: resident early, everything it reads is behind
+    // this wait (the earlier grid complete and flushed), so only the launch latency is hidden
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     if (st->stop) return;
     double P = 0.0, f = 0.0;
     if (mode != 3) P = np > 0 ? sum_partials(red_prox, np) : 2.0 * st->prox_cur;
@@ -142,8 +145,17 @@ __global__ void k_close_sweep(DevState* st, double* trace, const double* __restr
 
 void sup_launch_close_sweep(sup_ctx* h, double* trace, const double* red_prox, int np, int mode, int use_f, int perturbed,
                             const sup_options& o) {
-    k_close_sweep<<<1, 1, 0, h->stream>>>(h->state, trace, red_prox, np, mode, use_f, o.trace_mode && o.trace, o.stop_enabled, perturbed,
-                                          o.prox_tol, o.dprox_tol, o.n_consec, o.dobj_tol);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(1);
+    cfg.blockDim = dim3(1);
+    cfg.stream = h->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = h->pdl ? 1 : 0;
+    cudaLaunchKernelEx(&cfg, k_close_sweep, h->state, trace, red_prox, np, mode, use_f, int(o.trace_mode && o.trace), int(o.stop_enabled), perturbed,
+                       o.prox_tol, o.dprox_tol, o.n_consec, o.dobj_tol);
     h->launches++;
 }
 
