@@ -411,6 +411,9 @@ static bool make_tile_map(const int64_t* shape, int64_t size, size_t esz, GMap* 
     out->Rm = int(shape[0] / out->th) * out->th;
     out->Cm = int(shape[1] / out->tw) * out->tw;
     out->ntc = out->Cm / out->tw;
+    out->tw_shift = out->tw == 8 ? 3 : 2;  // 32 / esz: 8 (fp32) or 4 (fp64)
+    out->th_shift = 2;                     // th = 4
+    out->Cmagic = out->C > 1 ? ~0ull / (unsigned long long)out->C + 1ull : 0ull;  // ceil(2^64 / C) (2^64 / C itself for a power of two)
     return true;
 }
 

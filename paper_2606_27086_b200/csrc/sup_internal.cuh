@@ -107,17 +107,26 @@ struct GMap {
     int C = 1;          // columns of the 2-D view
     int Rm = 0, Cm = 0; // extent of the tiled region (multiples of th, tw)
     int ntc = 0;        // tiles per tile row = Cm / tw
-    int th = 4, tw = 8;
+    int th = 4, tw = 8; // powers of two (a 32-byte sector wide, four sectors high)
+    int th_shift = 2, tw_shift = 3;
+    unsigned long long Cmagic = 0;  // ceil(2^64 / C): j / C = mulhi64(j, Cmagic) exactly for every 32-bit j (device code; the
+                                    // epilogue of every row of the product kernels maps an index: three runtime divisions there
+                                    // were ~60 of the ~200 instructions a warp spends per row group outside the dot product)
 };
 __host__ __device__ static inline int sup_gmap(const GMap& M, int j) {
     if (M.kind == 0) return j;
     if (M.kind == 1) return sup_swz(j);
-    const int r = j / M.C, c = j - r * M.C;
+#ifdef __CUDA_ARCH__
+    const int r = M.Cmagic ? int(__umul64hi((unsigned long long)(unsigned)j, M.Cmagic)) : j;  // (Cmagic = 0: C = 1)
+#else
+    const int r = j / M.C;
+#endif
+    const int c = j - r * M.C;
     const int main_count = M.Rm * M.Cm;
     if (r < M.Rm) {
         if (c < M.Cm) {
-            const int tr = r / M.th, tc = c / M.tw;
-            const int in = (r - tr * M.th) * M.tw + (c - tc * M.tw);
+            const int tr = r >> M.th_shift, tc = c >> M.tw_shift;
+            const int in = ((r & (M.th - 1)) << M.tw_shift) + (c & (M.tw - 1));
             const int v = (tr & (M.tw - 1)) | ((tc & (M.th - 1)) * M.tw);
             return (tr * M.ntc + tc) * (M.th * M.tw) + (in ^ v);
         }
