@@ -337,7 +337,7 @@ __device__ void tv2d_pass(const PArgs<T>& A, const double* coef, T* __restrict__
     }
     double acc = 0.0;
     for (int64_t t = blockIdx.x; t < tiles_y * tiles_x; t += gridDim.x) {
-        const int64_t ty = t / tiles_x, txi = t - ty * tiles_x;
+        const int64_t ty = int64_t(unsigned(t) / unsigned(tiles_x)), txi = t - ty * tiles_x;  // (n < 2^31: a 32-bit division, a fifth of the 64-bit one)
         const int64_t i0 = ty * TILE_H - 1, j0 = txi * TILE_W - 1;  // top-left of the halo
         __syncthreads();
         for (int q = threadIdx.x; q < (TILE_H + 2) * (TILE_W + 2); q += SUP_THREADS) {
@@ -418,7 +418,7 @@ __device__ void tv3d_pass(const PArgs<T>& A, const double* coef, T* __restrict__
     }
     double acc = 0.0;
     for (int64_t t = blockIdx.x; t < tz * ty * txn; t += gridDim.x) {
-        const int64_t bz = t / (ty * txn), rem = t - bz * ty * txn, by = rem / txn, bx = rem - by * txn;
+        const int64_t bz = int64_t(unsigned(t) / unsigned(ty * txn)), rem = t - bz * ty * txn, by = int64_t(unsigned(rem) / unsigned(txn)), bx = rem - by * txn;
         const int64_t i0 = bz * TZ3 - 1, j0 = by * TY3 - 1, k0 = bx * TX3 - 1;
         __syncthreads();
         for (int q = threadIdx.x; q < (TZ3 + 2) * (TY3 + 2) * (TX3 + 2); q += SUP_THREADS) {

@@ -68,7 +68,8 @@ __device__ __forceinline__ void small_reduce(cg::cluster_group& cl, SmallShared&
 // pixels into gout[] (rounded to T) and the share S of sum g^2.  zl: this CTA's rows [r0, r1) of z; zp / zn: the last row of the
 // CTA before and the first row of the CTA after (distributed shared memory), valid where such a row exists.
 template <typename T, bool GRAD>
-__device__ __forceinline__ void small_terms(const T* zl, const T* zp, const T* zn, int r0, int r1, int ny, int nx, double& F, double& S, T* gout) {
+__device__ __forceinline__ void small_terms(const T* zl, const T* zp, const T* zn, int r0, int r1, int ny, int nx, double& F, double& S, T* gout,
+                                            const int* pij) {
     F = 0.0;
     S = 0.0;
     const int nloc = (r1 - r0) * nx;
@@ -77,7 +78,7 @@ __device__ __forceinline__ void small_terms(const T* zl, const T* zp, const T* z
     for (int k = 0; k < SMALL_PPT; ++k) {
         const int q = threadIdx.x + k * SMALL_THR;
         if (q >= nloc) break;
-        const int il = q / nx, j = q - il * nx, i = r0 + il;
+        const int il = pij[k] >> 16, j = pij[k] & 0xffff, i = r0 + il;  // (row, column) of the pixel: divided once, at the start of the kernel
         const T* ri = zl + il * nx;
         const double c = double(ri[j]);
         double gv = 0.0;
@@ -169,6 +170,13 @@ __global__ void __launch_bounds__(SMALL_THR, 1) k_perturb_tv2d_small(PArgs<T> A,
         return s > 0.0 ? (A.beta0 * ap) / s : 0.0;
     };
     T g2[SMALL_PPT];
+    int pij[SMALL_PPT];  // (local row << 16) | column of the pixels this thread owns (rows and columns are <= 4096 here)
+#pragma unroll
+    for (int kk = 0; kk < SMALL_PPT; ++kk) {
+        const int q = threadIdx.x + kk * SMALL_THR;
+        const int il = q < nloc ? q / nx : 0;
+        pij[kk] = (il << 16) | (q < nloc ? q - il * nx : 0);
+    }
     bool moved = false;  // x differs from what the caller passed in
     auto form_z = [&](double c) {  // z = round_T(x - c g) for the owned pixels (c = 0: x itself), then visible to the cluster
         for (int q = threadIdx.x; q < nloc; q += SMALL_THR) {
@@ -192,7 +200,7 @@ __global__ void __launch_bounds__(SMALL_THR, 1) k_perturb_tv2d_small(PArgs<T> A,
     double fx, s;
     {
         double v[2];
-        small_terms<T, true>(sX, prev_last(sX), next_first(sX), r0, r1, ny, nx, v[0], v[1], g2);
+        small_terms<T, true>(sX, prev_last(sX), next_first(sX), r0, r1, ny, nx, v[0], v[1], g2, pij);
         small_reduce<2>(cl, sh, parity, v);
         adopt(false);
         fx = v[0];
@@ -216,7 +224,7 @@ __global__ void __launch_bounds__(SMALL_THR, 1) k_perturb_tv2d_small(PArgs<T> A,
                 break;
             }
             double v[2];
-            small_terms<T, true>(sZ, zp, zn, r0, r1, ny, nx, v[0], v[1], g2);
+            small_terms<T, true>(sZ, zp, zn, r0, r1, ny, nx, v[0], v[1], g2, pij);
             small_reduce<2>(cl, sh, parity, v);
             adopt(true);
             fx = v[0];
@@ -235,10 +243,10 @@ __global__ void __launch_bounds__(SMALL_THR, 1) k_perturb_tv2d_small(PArgs<T> A,
                 // the first candidate of a step that is not the last comes with its gradient (accepted, the next step starts at once)
                 const bool with_grad = trial == 0 && !last;
                 if (with_grad) {
-                    small_terms<T, true>(sZ, zp, zn, r0, r1, ny, nx, v[0], v[1], g2);
+                    small_terms<T, true>(sZ, zp, zn, r0, r1, ny, nx, v[0], v[1], g2, pij);
                     small_reduce<2>(cl, sh, parity, v);
                 } else {
-                    small_terms<T, false>(sZ, zp, zn, r0, r1, ny, nx, v[0], v[1], g2);
+                    small_terms<T, false>(sZ, zp, zn, r0, r1, ny, nx, v[0], v[1], g2, pij);
                     small_reduce<1>(cl, sh, parity, v);
                 }
                 const bool acc = v[0] <= fx;  // NaN compares false -> rejected (A-11)
@@ -257,7 +265,7 @@ __global__ void __launch_bounds__(SMALL_THR, 1) k_perturb_tv2d_small(PArgs<T> A,
                     fx = v[0];
                 } else {
                     if (!with_grad) {  // z is still in place: its gradient now (f(z) again: the same bits)
-                        small_terms<T, true>(sZ, zp, zn, r0, r1, ny, nx, v[0], v[1], g2);
+                        small_terms<T, true>(sZ, zp, zn, r0, r1, ny, nx, v[0], v[1], g2, pij);
                         small_reduce<2>(cl, sh, parity, v);
                     }
                     fx = v[0];
