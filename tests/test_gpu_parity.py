@@ -813,6 +813,35 @@ def test_graph_replay_equals_direct_launches(name, block):
     assert torch.equal(outs[0][0], outs[1][0]) and outs[0][1] == outs[1][1] and torch.equal(outs[0][2], outs[1][2])
 
 
+@pytest.mark.parametrize("dtype", [0, 1])
+@pytest.mark.parametrize("name", ["cfg1", "ct_ragged", "cfg2", "cfg5_k16", "cfg4_small"])
+def test_dependent_launch_overlap_changes_no_bit(name, dtype):
+    """The product kernels are launched as programmatic dependents of each other (the next kernel's producers fill its ring while the
+    earlier kernel drains; its consumers wait for the earlier grid).  Back-to-back sweeps must give the bits of the same sweeps
+    with the device idle between any two kernels -- a consumer that read x or y too early would show up here."""
+    sup = _sup()
+    P = problem(name)
+    H = make_handle(P, dtype, blocks=False)
+    xa, xb = xdev(P, dtype), xdev(P, dtype)
+    sup.sup_project_simultaneous(H, xa, P.lam, 40)  # 80 kernels back to back
+    torch.cuda.synchronize()
+    for _ in range(40):
+        sup.sup_forward_violation(H, xb)
+        torch.cuda.synchronize()
+        sup.sup_backproject_update(H, xb, P.lam)
+        torch.cuda.synchronize()
+    assert torch.equal(xa, xb)
+    # three product kernels in a row per sweep (EMR), against the oracle-checked single sweeps, idle in between
+    if name in ("cfg1", "ct_ragged"):
+        xa, xb = xdev(P, dtype), xdev(P, dtype)
+        sup.sup_project_emr(H, xa, 15)
+        torch.cuda.synchronize()
+        for _ in range(15):
+            sup.sup_project_emr(H, xb, 1)
+            torch.cuda.synchronize()
+        assert torch.equal(xa, xb)
+
+
 def test_unaligned_all_empty_row_ranges():
     """Runs of empty rows that start at an element offset which is not a multiple of 4: a persistent CTA may own nothing but
     empty rows and must then stream nothing (round-1 advice: a bulk copy was left in flight)."""
