@@ -153,3 +153,23 @@ def test_config3_full_block_iterative_against_oracle_goldens():
 @pytest.mark.parametrize("variant", ["cfg4_full", "cfg4_full_infeasible"])
 def test_config4_full_against_oracle_goldens(variant, dtype):
     full_size_case(variant, dtype, 5, 4, block=False)
+
+
+def test_config3_full_back_to_back_kernels_equal_idle_device():
+    """At the size bench.py times: 10 sweeps enqueued back to back (each product kernel a programmatic dependent of the one before)
+    against the same 20 kernels with the device idle between any two -- bit-identical"""
+    import paper_2606_27086_b200 as sup
+
+    P, G, meta = load("cfg3_full_simul")
+    H = handle(P, 0)
+    xa = torch.tensor(P.x0, dtype=torch.float32, device="cuda:0")
+    xb = xa.clone()
+    sup.sup_project_simultaneous(H, xa, P.lam, 10)
+    torch.cuda.synchronize()
+    for _ in range(10):
+        sup.sup_forward_violation(H, xb)
+        torch.cuda.synchronize()
+        sup.sup_backproject_update(H, xb, P.lam)
+        torch.cuda.synchronize()
+    assert torch.equal(xa, xb)
+    assert rel_l2(xa.cpu().numpy(), G["basic_x10"]) <= 1e-4
