@@ -1010,7 +1010,8 @@ __global__ void __launch_bounds__(32 * (NCW + RG_NPROD), 1)
 // barrier waits and epilogue even when it is empty: config 4 has body voxels no beamlet reaches, config 3 rays that miss
 // the image).  part[b] = first row r in [r0, r1] with cost(r0..r) >= total * b / nb  (part[0] = r0, part[nb] = r1).
 #ifndef RG_ROW_COST
-#define RG_ROW_COST 16
+#define RG_ROW_COST 32  // (A/B at the end of round 2, 8 / 16 / 32 / 64: block-iterative config 3 933 / 931 / 917 / 907 us per sweep, config 4 forward
+                        //  136 / 113 / 112 / 114 us, config 3 forward 323 / 324 / 324 / 326 us)
 #endif
 __global__ void k_stream_partition(const int64_t* __restrict__ rowptr, int64_t r0, int64_t r1, int nb, int64_t* __restrict__ part) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
