@@ -26,10 +26,11 @@ namespace cg = cooperative_groups;
 #define SMALL_CMAX 16   // non-portable size (opt-in, B200 has it): larger images, where a pass is bound by the fp64 work per CTA
 #define SMALL_PPT 8
 #define SMALL_LOCAL_MAX (SMALL_THR * SMALL_PPT)  // pixels one CTA holds
+#define SMALL_NB 4        // candidates per value-only pass after a rejected first candidate
 
 struct SmallShared {
-    double ws[SMALL_THR / 32][2];  // per-warp partial sums of a reduction
-    double part[2][SMALL_CMAX][2];    // [parity][rank][value]: the CTAs' sums, written by their owners into EVERY CTA's copy
+    double ws[SMALL_THR / 32][SMALL_NB];  // per-warp partial sums of a reduction
+    double part[2][SMALL_CMAX][SMALL_NB];    // [parity][rank][value]: the CTAs' sums, written by their owners into EVERY CTA's copy
 };
 
 // sums v[0..NV) over the whole cluster; on return every thread holds the totals.  Fixed order: lanes (shuffle tree), warps in index
@@ -67,7 +68,7 @@ __device__ __forceinline__ void small_reduce(cg::cluster_group& cl, SmallShared&
 // TV terms of the pixels this thread owns (A-8, as tv2d_pass of sup_perturb.cu): share F of f(z); with GRAD the gradient of the owned
 // pixels into gout[] (rounded to T) and the share S of sum g^2.  zl: this CTA's rows [r0, r1) of z; zp / zn: the last row of the
 // CTA before and the first row of the CTA after (distributed shared memory), valid where such a row exists.
-template <typename T, bool GRAD>
+template <typename T, bool GRAD, int PPT>
 __device__ __forceinline__ void small_terms(const T* zl, const T* zp, const T* zn, int r0, int r1, int ny, int nx, double& F, double& S, T* gout,
                                             const int* pij) {
     F = 0.0;
@@ -75,7 +76,7 @@ __device__ __forceinline__ void small_terms(const T* zl, const T* zp, const T* z
     const int nloc = (r1 - r0) * nx;
     auto row = [&](int i) -> const T* { return i < r0 ? zp : (i >= r1 ? zn : zl + (i - r0) * nx); };
 #pragma unroll
-    for (int k = 0; k < SMALL_PPT; ++k) {
+    for (int k = 0; k < PPT; ++k) {
         const int q = threadIdx.x + k * SMALL_THR;
         if (q >= nloc) break;
         const int il = pij[k] >> 16, j = pij[k] & 0xffff, i = r0 + il;  // (row, column) of the pixel: divided once, at the start of the kernel
@@ -112,7 +113,39 @@ __device__ __forceinline__ void small_terms(const T* zl, const T* zp, const T* z
     }
 }
 
+// f(z_b), z_b = round_T(x - c_b g), for SMALL_NB candidates at once, z formed on the fly from x and g (this CTA's rows and the first row
+// of the CTA after it, read through distributed shared memory): the same operations on the same values as small_terms<T, false> on
+// a stored z_b, hence the same bits.  No z array, no cluster barrier before the terms: one barrier (the reduction's) per SMALL_NB trials.
 template <typename T>
+__device__ __forceinline__ void small_terms_batch(const T* xl, const T* gl, const T* xn, const T* gn, int r0, int r1, int ny, int nx, const double* coef,
+                                               double* F) {
+#pragma unroll
+    for (int b = 0; b < SMALL_NB; ++b) F[b] = 0.0;
+    const int nloc = (r1 - r0) * nx;
+#pragma unroll 1
+    for (int q = threadIdx.x; q < nloc; q += SMALL_THR) {
+        const int il = q / nx, j = q - il * nx, i = r0 + il;
+        if (i + 1 >= ny || j + 1 >= nx) continue;
+        const bool below_local = i + 1 < r1;
+        const double x0 = double(xl[q]), g0 = double(gl[q]);
+        const double x1 = double(below_local ? xl[q + nx] : xn[j]), g1 = double(below_local ? gl[q + nx] : gn[j]);
+        const double x2 = double(xl[q + 1]), g2v = double(gl[q + 1]);
+#pragma unroll
+        for (int b = 0; b < SMALL_NB; ++b) {
+            const double cb = coef[b];
+            const double c = cb == 0.0 ? x0 : double(T(fma(-cb, g0, x0)));
+            const double zd = cb == 0.0 ? x1 : double(T(fma(-cb, g1, x1)));
+            const double zr = cb == 0.0 ? x2 : double(T(fma(-cb, g2v, x2)));
+            const double dx = zd - c, dy = zr - c;
+            const double d2 = fma(dx, dx, dy * dy);
+            if (d2 > 0.0) F[b] += d2 * rsqrt(d2);
+        }
+    }
+}
+
+// PPT: pixels per thread the kernel is built for (2: images of up to 1 024 pixels per CTA -- configs 1 and 2 -- with a fraction of
+// the registers and of the unrolled code of the general PPT = SMALL_PPT build)
+template <typename T, int PPT>
 __global__ void __launch_bounds__(SMALL_THR, 1) k_perturb_tv2d_small(PArgs<T> A, int rows_max) {
     cg::cluster_group cl = cg::this_cluster();
     DevState* st = A.st;
@@ -169,10 +202,10 @@ __global__ void __launch_bounds__(SMALL_THR, 1) k_perturb_tv2d_small(PArgs<T> A,
         }
         return s > 0.0 ? (A.beta0 * ap) / s : 0.0;
     };
-    T g2[SMALL_PPT];
-    int pij[SMALL_PPT];  // (local row << 16) | column of the pixels this thread owns (rows and columns are <= 4096 here)
+    T g2[PPT];
+    int pij[PPT];  // (local row << 16) | column of the pixels this thread owns (rows and columns are <= 4096 here)
 #pragma unroll
-    for (int kk = 0; kk < SMALL_PPT; ++kk) {
+    for (int kk = 0; kk < PPT; ++kk) {
         const int q = threadIdx.x + kk * SMALL_THR;
         const int il = q < nloc ? q / nx : 0;
         pij[kk] = (il << 16) | (q < nloc ? q - il * nx : 0);
@@ -187,7 +220,7 @@ __global__ void __launch_bounds__(SMALL_THR, 1) k_perturb_tv2d_small(PArgs<T> A,
     };
     auto adopt = [&](bool with_x) {  // (x, g) <- (z, g2): owned pixels only, by the thread that owns them
 #pragma unroll
-        for (int kk = 0; kk < SMALL_PPT; ++kk) {
+        for (int kk = 0; kk < PPT; ++kk) {
             const int q = threadIdx.x + kk * SMALL_THR;
             if (q >= nloc) break;
             if (with_x) sX[q] = sZ[q];
@@ -200,7 +233,7 @@ __global__ void __launch_bounds__(SMALL_THR, 1) k_perturb_tv2d_small(PArgs<T> A,
     double fx, s;
     {
         double v[2];
-        small_terms<T, true>(sX, prev_last(sX), next_first(sX), r0, r1, ny, nx, v[0], v[1], g2, pij);
+        small_terms<T, true, PPT>(sX, prev_last(sX), next_first(sX), r0, r1, ny, nx, v[0], v[1], g2, pij);
         small_reduce<2>(cl, sh, parity, v);
         adopt(false);
         fx = v[0];
@@ -224,7 +257,7 @@ __global__ void __launch_bounds__(SMALL_THR, 1) k_perturb_tv2d_small(PArgs<T> A,
                 break;
             }
             double v[2];
-            small_terms<T, true>(sZ, zp, zn, r0, r1, ny, nx, v[0], v[1], g2, pij);
+            small_terms<T, true, PPT>(sZ, zp, zn, r0, r1, ny, nx, v[0], v[1], g2, pij);
             small_reduce<2>(cl, sh, parity, v);
             adopt(true);
             fx = v[0];
@@ -236,17 +269,17 @@ __global__ void __launch_bounds__(SMALL_THR, 1) k_perturb_tv2d_small(PArgs<T> A,
             const bool last = nred == A.N - 1;
             bool accepted = false;
             long long jloc = 0;
-            for (int trial = 0; trial < SUP_J_MAX && !accepted; ++trial) {
+            int trial = 0;
+            {   // the first candidate alone; when the step is not the last, with its gradient (accepted, the next step starts at once)
                 const double c = step_coef(s, jloc);
                 form_z(c);
                 double v[2];
-                // the first candidate of a step that is not the last comes with its gradient (accepted, the next step starts at once)
-                const bool with_grad = trial == 0 && !last;
+                const bool with_grad = !last;
                 if (with_grad) {
-                    small_terms<T, true>(sZ, zp, zn, r0, r1, ny, nx, v[0], v[1], g2, pij);
+                    small_terms<T, true, PPT>(sZ, zp, zn, r0, r1, ny, nx, v[0], v[1], g2, pij);
                     small_reduce<2>(cl, sh, parity, v);
                 } else {
-                    small_terms<T, false>(sZ, zp, zn, r0, r1, ny, nx, v[0], v[1], g2, pij);
+                    small_terms<T, false, PPT>(sZ, zp, zn, r0, r1, ny, nx, v[0], v[1], g2, pij);
                     small_reduce<1>(cl, sh, parity, v);
                 }
                 const bool acc = v[0] <= fx;  // NaN compares false -> rejected (A-11)
@@ -254,23 +287,70 @@ __global__ void __launch_bounds__(SMALL_THR, 1) k_perturb_tv2d_small(PArgs<T> A,
                 apow *= A.a;
                 ++jloc;
                 ++trials;
+                ++trial;
                 log_trial(v[0], fx, acc);
-                if (!acc) continue;
-                accepted = true;
-                if (last) {  // nobody needs the gradient at the final point
-                    if (c != 0.0) {
+                if (acc) {
+                    accepted = true;
+                    if (last) {  // nobody needs the gradient at the final point
+                        if (c != 0.0) {
+                            for (int q = threadIdx.x; q < nloc; q += SMALL_THR) sX[q] = sZ[q];
+                            moved = true;
+                        }
+                        fx = v[0];
+                    } else {
+                        fx = v[0];
+                        s = sqrt(v[1]);
+                        adopt(c != 0.0);
+                    }
+                }
+            }
+            // after a rejection: SMALL_NB candidates per pass, values only, decided strictly in order (later ones are discarded uncounted)
+            while (!accepted && trial < SUP_J_MAX) {
+                double coef[SMALL_NB], F[SMALL_NB];
+                {
+                    double ap = apow;
+                    if (A.policy != SUP_STEP_PER_TRIAL) {
+                        ap = 1.0;
+                        for (long long q = 0; q < k + jloc; ++q) ap *= A.a;
+                    }
+#pragma unroll
+                    for (int b = 0; b < SMALL_NB; ++b) {
+                        coef[b] = s > 0.0 ? (A.beta0 * ap) / s : 0.0;
+                        ap *= A.a;
+                    }
+                }
+                small_terms_batch<T>(sX, sG, next_first(sX), next_first(sG), r0, r1, ny, nx, coef, F);
+                small_reduce<SMALL_NB>(cl, sh, parity, F);
+                double cacc = 0.0, facc = 0.0;
+                for (int b = 0; b < SMALL_NB && !accepted && trial < SUP_J_MAX; ++b) {
+                    const bool acc = F[b] <= fx;
+                    ++ell;
+                    apow *= A.a;
+                    ++jloc;
+                    ++trials;
+                    ++trial;
+                    log_trial(F[b], fx, acc);
+                    if (acc) {
+                        accepted = true;
+                        cacc = coef[b];
+                        facc = F[b];
+                    }
+                }
+                if (!accepted) continue;
+                form_z(cacc);
+                if (last) {
+                    if (cacc != 0.0) {
                         for (int q = threadIdx.x; q < nloc; q += SMALL_THR) sX[q] = sZ[q];
                         moved = true;
                     }
-                    fx = v[0];
-                } else {
-                    if (!with_grad) {  // z is still in place: its gradient now (f(z) again: the same bits)
-                        small_terms<T, true>(sZ, zp, zn, r0, r1, ny, nx, v[0], v[1], g2, pij);
-                        small_reduce<2>(cl, sh, parity, v);
-                    }
+                    fx = facc;
+                } else {  // the gradient at the accepted z (f(z) again: the same bits)
+                    double v[2];
+                    small_terms<T, true, PPT>(sZ, zp, zn, r0, r1, ny, nx, v[0], v[1], g2, pij);
+                    small_reduce<2>(cl, sh, parity, v);
                     fx = v[0];
                     s = sqrt(v[1]);
-                    adopt(c != 0.0);
+                    adopt(cacc != 0.0);
                 }
             }
             if (!accepted) warn |= 1;  // A-12: step skipped
@@ -314,7 +394,10 @@ bool sup_perturb_small_eligible(const sup_ctx* h, const PerturbParams& pp) {
 
 template <typename T>
 static sup_status launch_small_t(sup_ctx* h, const PArgs<T>& A, const PerturbParams& pp) {
-    const void* fn = reinterpret_cast<const void*>(&k_perturb_tv2d_small<T>);
+    // (cluster16 must be known before the cluster size: ask with the general build's function once)
+    const void* fn8 = reinterpret_cast<const void*>(&k_perturb_tv2d_small<T, SMALL_PPT>);
+    const void* fn2 = reinterpret_cast<const void*>(&k_perturb_tv2d_small<T, 2>);
+    const void* fn = fn8;
     if (!h->smem_opted_in.count(fn)) {
         SUP_CUDA(h, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, int(size_t(3) * SMALL_LOCAL_MAX * sizeof(T))));
         // does this device take clusters of 16 for this kernel?  (asked once per handle; -1 = no)
@@ -334,6 +417,8 @@ static sup_status launch_small_t(sup_ctx* h, const PArgs<T>& A, const PerturbPar
             int nclusters = 0;
             if (cudaOccupancyMaxActiveClusters(&nclusters, fn, &q) == cudaSuccess && nclusters >= 1) h->cluster16 = 1;
         }
+        cudaFuncSetAttribute(fn2, cudaFuncAttributeMaxDynamicSharedMemorySize, int(size_t(3) * SMALL_LOCAL_MAX * sizeof(T)));
+        if (h->cluster16 > 0) cudaFuncSetAttribute(fn2, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
         cudaGetLastError();
         h->smem_opted_in.insert(fn);
     }
@@ -341,6 +426,7 @@ static sup_status launch_small_t(sup_ctx* h, const PArgs<T>& A, const PerturbPar
     if (C < 1) return sup_fail(h, SUP_ERR_STATE, "sup_launch_perturb_small: image not eligible");
     const int rows_max = int((pp.ny + C - 1) / C);
     const size_t smem = size_t(3) * rows_max * pp.nx * sizeof(T);
+    if (int64_t(rows_max) * pp.nx <= 2 * SMALL_THR) fn = fn2;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(C);
     cfg.blockDim = dim3(SMALL_THR);
